@@ -1,0 +1,106 @@
+"""The whole hot path, step by step -- oracle (test infrastructure; see oracle/__init__.py).
+
+`OraclePIMD` mirrors the problem statement of the C-ABI (create with types, masses, box, P, T,
+dt, gamma, seed; set_state; set_model; step(n); getters) but shares nothing with it.
+One step = PAPER.md:L165 BAOAB with the three normal-mode transforms of L192 and one force
+evaluation per step placed after the second A (DESIGN R-7); estimators (Appendix A) are taken
+after the closing B with x, f consistent.
+"""
+import numpy as np
+
+from .constants import KB, MVV2E
+from . import nm, integrator, se_e2_a
+
+
+class OraclePIMD:
+    def __init__(self, types, masses_per_type, box, n_beads, T, dt, gamma_centroid, seed):
+        self.types = np.asarray(types, dtype=np.int64)
+        self.N = self.types.size
+        self.masses = np.asarray(masses_per_type, dtype=np.float64)[self.types]   # per atom
+        self.box = np.asarray(box, dtype=np.float64)
+        self.P = int(n_beads)
+        self.T = float(T)
+        self.dt = float(dt)
+        self.gamma0 = float(gamma_centroid)
+        self.seed = int(seed)
+        self.M = nm.nm_matrix(self.P)
+        self.om = nm.omegas(self.P, self.T)
+        self.step_count = 0
+        self.model = None
+        self.k_spring = None
+        self.x = None
+        self.vt = None
+        self.f = None
+        self.ft = None
+        self.U = np.zeros(self.P)
+        self.Xi = np.zeros((self.P, 3, 3))
+        self.only_beads = None       # bench.py's bounded cpu_baseline sample: evaluate these beads only
+
+    # ---- inputs ----
+    def set_state(self, x, p):
+        """x[P,N,3] unwrapped Cartesian (A); p[P,N,3] Cartesian bead momenta ((g/mol) A/ps).
+        Internally v~ = M (p/m) (velocities live in normal-mode form)."""
+        self.x = np.array(x, dtype=np.float64).reshape(self.P, self.N, 3)
+        v = np.asarray(p, dtype=np.float64).reshape(self.P, self.N, 3) / self.masses[None, :, None]
+        self.vt = nm.to_nm(self.M, v)
+        self.step_count = 0
+        if self.model is not None or self.k_spring is not None:
+            self._forces()
+
+    def set_model(self, desc, weights):
+        self.model = se_e2_a.Model(desc, weights)
+        self.k_spring = None
+        if self.x is not None:
+            self._forces()
+
+    def set_model_harmonic(self, k_spring):
+        self.k_spring = float(k_spring)
+        self.model = None
+        if self.x is not None:
+            self._forces()
+
+    # ---- the path ----
+    def _forces(self):
+        f = np.zeros((self.P, self.N, 3))
+        beads = range(self.P) if self.only_beads is None else self.only_beads
+        for k in beads:
+            if self.k_spring is not None:
+                E, F, Xi = se_e2_a.harmonic_energy_forces(self.x[k], self.k_spring)
+            else:
+                E, F, Xi = se_e2_a.energy_forces(self.x[k], self.types, self.box, self.model)
+            f[k] = F
+            self.U[k] = E.sum()
+            self.Xi[k] = Xi
+        self.f = f
+        self.ft = nm.to_nm(self.M, f)
+
+    def step(self, n_steps=1):
+        for _ in range(int(n_steps)):
+            self.x, self.vt = integrator.baoab_positions_half(
+                self.x, self.vt, self.ft, self.masses, self.M, self.om, self.T, self.gamma0,
+                self.dt, self.seed, self.step_count)
+            self._forces()                                   # one force evaluation per step
+            self.vt, _ = integrator.baoab_finish(self.vt, self.f, self.masses, self.M, self.dt)
+            self.step_count += 1
+
+    # ---- outputs ----
+    def positions(self):
+        return self.x.copy()
+
+    def momenta(self):
+        """Cartesian bead momenta p = m M^T v~."""
+        return nm.from_nm(self.M, self.vt) * self.masses[None, :, None]
+
+    def forces(self):
+        return self.f.copy()
+
+    def virial(self):
+        return self.Xi.copy()
+
+    def energies(self):
+        return self.U.copy()
+
+    def estimators(self):
+        e = integrator.estimators(self.x, self.vt, self.f, self.U, self.masses, self.M, self.om, self.T)
+        e["step"] = self.step_count
+        return e

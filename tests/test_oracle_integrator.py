@@ -1,0 +1,217 @@
+"""Pins for oracle/integrator.py and oracle/pimd.py against closed forms and invariants (CPU only)."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import constants as C
+from oracle import integrator, nm, philox
+from oracle.pimd import OraclePIMD
+
+
+def _ho(P, T, dt, gamma0, n_part, bhw, seed=11, mass=1.008):
+    """n_part independent 3-D harmonic oscillators (one 'type'), beta*hbar*omega = bhw."""
+    omega = bhw * C.KB * T / C.HBAR
+    k_spring = mass * C.MVV2E * omega ** 2
+    o = OraclePIMD(np.zeros(n_part, dtype=int), [mass], [100.0, 100.0, 100.0], P, T, dt, gamma0, seed)
+    return o, omega, k_spring
+
+
+# ---------------------------------------------------------------- A step
+def test_a_step_composes_and_conserves_mode_energy():
+    P, T = 8, 300.0
+    om = nm.omegas(P, T)
+    rng = np.random.default_rng(0)
+    xt, vt = rng.standard_normal((P, 5, 3)), 50 * rng.standard_normal((P, 5, 3))
+    h = 0.3e-3
+    x1, v1 = integrator.a_step(*integrator.a_step(xt, vt, om, h), om, h)
+    x2, v2 = integrator.a_step(xt, vt, om, 2 * h)
+    assert np.abs(x1 - x2).max() < 1e-13 and np.abs(v1 - v2).max() < 1e-10
+    e0 = 0.5 * vt ** 2 + 0.5 * (om[:, None, None] * xt) ** 2
+    e1 = 0.5 * v2 ** 2 + 0.5 * (om[:, None, None] * x2) ** 2
+    assert np.abs(e1 - e0).max() < 1e-12 * np.abs(e0).max()
+    # centroid: free flight
+    assert np.allclose(x2[0], xt[0] + 2 * h * vt[0], rtol=0, atol=1e-15)
+    assert np.array_equal(v2[0], vt[0])
+    # backward in time undoes it (sign of the rotation)
+    xb, vb = integrator.a_step(x2, v2, om, -2 * h)
+    assert np.abs(xb - xt).max() < 1e-13
+
+
+def test_a_step_equals_fine_verlet_on_cartesian_ring_springs():
+    """Independent check of transform + frequencies + rotation: integrate Eq. 1's Cartesian spring
+    Hamiltonian (omega_n^2, DESIGN R-1) with tiny velocity-Verlet steps and compare with
+    M^T A(h) M."""
+    P, T, h = 6, 300.0, 0.4e-3
+    M, om, wP = nm.nm_matrix(P), nm.omegas(P, T), nm.omega_P(P, T)
+    rng = np.random.default_rng(3)
+    x, v = 0.05 * rng.standard_normal((P, 2, 3)), 30 * rng.standard_normal((P, 2, 3))
+    xt, vt = integrator.a_step(nm.to_nm(M, x), nm.to_nm(M, v), om, h)
+    xa, va = nm.from_nm(M, xt), nm.from_nm(M, vt)
+
+    def acc(y):                      # -d/dr_k sum_k 1/2 w_P^2 |r_k - r_{k+1}|^2  (unit mass)
+        return -wP ** 2 * (2 * y - np.roll(y, 1, axis=0) - np.roll(y, -1, axis=0))
+    n = 20000
+    d = h / n
+    y, w = x.copy(), v.copy()
+    a = acc(y)
+    for _ in range(n):
+        w += 0.5 * d * a
+        y += d * w
+        a = acc(y)
+        w += 0.5 * d * a
+    assert np.abs(y - xa).max() < 2e-9 * max(1.0, np.abs(xa).max())
+    assert np.abs(w - va).max() < 2e-8 * np.abs(va).max()
+
+
+# ---------------------------------------------------------------- O step (PAPER.md D1-D2)
+def test_pile_l_coefficients():
+    P, T, dt = 32, 300.0, 0.25e-3
+    om = nm.omegas(P, T)
+    c1, c2 = integrator.pile_l_coefficients(om, 1.0, dt)
+    assert abs(c1[0] - math.exp(-dt / 1.0)) < 1e-16                    # tau_0 = `tau` = 1 ps (L174)
+    for k in (1, 7, 16, 31):
+        tau_k = 1.0 / (2.0 * om[k])                                     # D1 (L466)
+        assert abs(c1[k] - math.exp(-dt / tau_k)) < 1e-15
+    assert np.allclose(c1 ** 2 + c2 ** 2, 1.0, atol=1e-15)
+    # stiffest mode at P=32, 300 K: tau = 0.2 fs, c1 = 0.29 at dt = 0.25 fs (SURVEY C-4)
+    assert abs(1.0 / (2 * om[16]) - 0.199e-3) < 0.002e-3 and abs(c1[16] - 0.285) < 0.01
+
+
+def test_o_step_preserves_maxwell_boltzmann_variance():
+    P, T, dt, N = 4, 300.0, 0.5e-3, 4000
+    masses = np.full(N, 15.9994)
+    om = nm.omegas(P, T)
+    sigma2 = P * C.KB * T / (masses[0] * C.MVV2E)                       # target: n*T (L194)
+    rng = np.random.default_rng(2)
+    v = math.sqrt(sigma2) * rng.standard_normal((P, N, 3))
+    for step in range(3):
+        v = integrator.o_step(v, masses, T, om, 5.0, dt, 99, step)
+    var = v.reshape(P, -1).var(axis=1)
+    assert np.all(np.abs(var / sigma2 - 1.0) < 5.0 * math.sqrt(2.0 / (3 * N)))
+    # from rest, repeated O steps heat every mode to n*T
+    v = np.zeros((P, N, 3))
+    for step in range(400):
+        v = integrator.o_step(v, masses, T, om, 50.0, dt, 7, step)
+    var = v.reshape(P, -1).var(axis=1)
+    assert np.all(np.abs(var / sigma2 - 1.0) < 5.0 * math.sqrt(2.0 / (3 * N)))
+    # gamma0 = 0: NVE, O is the identity for all modes (DESIGN R-4)
+    assert np.array_equal(integrator.o_step(v, masses, T, om, 0.0, dt, 7, 0), v)
+
+
+def test_o_step_uses_the_documented_noise_stream():
+    P, T, dt, N = 4, 300.0, 0.5e-3, 3
+    masses = np.array([15.9994, 1.008, 1.008])
+    om = nm.omegas(P, T)
+    v0 = np.zeros((P, N, 3))
+    v = integrator.o_step(v0, masses, T, om, 1.0, dt, 1234, 5)
+    c1, c2 = integrator.pile_l_coefficients(om, 1.0, dt)
+    for (k, i, a) in [(0, 0, 0), (3, 2, 1), (2, 1, 2)]:
+        eta = float(philox.normal(1234, 5, k, i, a))
+        expect = c2[k] * math.sqrt(P * C.KB * T / (masses[i] * C.MVV2E)) * eta     # D2 (L473)
+        assert abs(v[k, i, a] - expect) < 1e-13 * abs(expect)
+
+
+# ---------------------------------------------------------------- whole step
+def test_p1_reduces_to_classical_langevin_baoab():
+    T, dt, g, N = 300.0, 0.5e-3, 2.0, 5
+    o, omega, ks = _ho(1, T, dt, g, N, bhw=2.0, seed=5)
+    rng = np.random.default_rng(4)
+    x0 = 0.1 * rng.standard_normal((1, N, 3))
+    p0 = 20 * rng.standard_normal((1, N, 3))
+    o.set_model_harmonic(ks)
+    o.set_state(x0, p0)
+    o.step(3)
+    # hand-written classical BAOAB in momentum form
+    m = 1.008
+    x, p = x0[0].copy(), p0[0].copy()
+    for step in range(3):
+        p += 0.5 * dt * (-ks * x) / C.MVV2E
+        x += 0.5 * dt * p / m
+        kk, ii, aa = np.meshgrid([0], np.arange(N), np.arange(3), indexing="ij")
+        eta = philox.normal(5, step, kk, ii, aa)[0]
+        c1 = math.exp(-g * dt)
+        p = c1 * p + math.sqrt(1 - c1 * c1) * math.sqrt(m * C.KB * T / C.MVV2E) * eta
+        x += 0.5 * dt * p / m
+        p += 0.5 * dt * (-ks * x) / C.MVV2E
+    assert np.abs(o.positions()[0] - x).max() < 1e-13
+    assert np.abs(o.momenta()[0] - p).max() < 1e-11
+
+
+def test_nve_energy_is_conserved_with_dt2_scaling():
+    T, P, N = 300.0, 16, 20
+    drift = []
+    for dt, nsteps in ((0.25e-3, 800), (0.125e-3, 1600)):
+        o, omega, ks = _ho(P, T, dt, 0.0, N, bhw=4.0)
+        rng = np.random.default_rng(8)
+        sig_x = math.sqrt(C.KB * T / ks)
+        x0 = sig_x * rng.standard_normal((1, N, 3)) + 0.02 * rng.standard_normal((P, N, 3))
+        p0 = math.sqrt(1.008 * P * C.KB * T / C.MVV2E) * rng.standard_normal((P, N, 3))
+        o.set_model_harmonic(ks)
+        o.set_state(x0, p0)
+        H0 = o.estimators()["H"]
+        dev = 0.0
+        for _ in range(nsteps // 100):
+            o.step(100)
+            dev = max(dev, abs(o.estimators()["H"] - H0) / abs(H0))
+        drift.append(dev)
+    assert drift[0] < 3e-4                                  # bounded fluctuation, no secular drift
+    assert drift[1] < 0.45 * drift[0]                       # ~dt^2
+
+
+def test_estimator_identities_on_random_state():
+    """K_CV in Cartesian form (A9) equals its normal-mode form -1/(2P) sum_{k>=1} x~.f~ + 3NkT/2;
+    T_ring definition; H = K+S+U; K_PR uses the Cartesian springs with 1/P."""
+    P, N, T = 8, 6, 300.0
+    rng = np.random.default_rng(6)
+    masses = rng.uniform(1, 16, N)
+    M, om = nm.nm_matrix(P), nm.omegas(P, T)
+    x, vt, f = rng.standard_normal((P, N, 3)), rng.standard_normal((P, N, 3)), rng.standard_normal((P, N, 3))
+    U = rng.standard_normal(P)
+    e = integrator.estimators(x, vt, f, U, masses, M, om, T)
+    xt, ft = nm.to_nm(M, x), nm.to_nm(M, f)
+    kcv_nm = 1.5 * N * C.KB * T - np.sum(xt[1:] * ft[1:]) / (2 * P)
+    assert abs(e["K_CV"] - kcv_nm) < 1e-13
+    assert abs(e["H"] - (e["K_ring"] + e["S_ring"] + U.sum())) < 1e-13
+    assert abs(e["S_ring"] - e["spring_cart"]) < 1e-12 * e["S_ring"]
+    assert abs(e["K_PR"] - (1.5 * P * N * C.KB * T - e["S_ring"] / P)) < 1e-12
+    assert abs(e["T_ring"] - 2 * e["K_ring"] / (3 * P * N * C.KB)) < 1e-12
+
+
+@pytest.mark.slow
+def test_harmonic_oscillator_matches_finite_P_closed_form():
+    """north_star pin: 3-D HO at P=32.  The sampled ring-polymer distribution gives exactly
+    <K> = <V> = (3 k_B T/2) sum_k w^2/(w^2 + w_k^2) (finite P); the P->inf value
+    (3 hbar w/4) coth(beta hbar w/2) is 0.19 % higher at beta hbar w = 4.  K_PR needs the 1/P of
+    DESIGN R-6: the printed A7 would give tens of eV."""
+    P, T, dt, npart, bhw = 32, 300.0, 0.25e-3, 300, 4.0
+    o, omega, ks = _ho(P, T, dt, 50.0, npart, bhw, seed=2024)
+    om = nm.omegas(P, T)
+    m = 1.008
+    rng = np.random.default_rng(12)
+    # start from the exact stationary Gaussians (temperature P*T) so that no equilibration is needed
+    sig_x = np.sqrt(P * C.KB * T / (m * C.MVV2E * (om ** 2 + omega ** 2)))
+    xt0 = sig_x[:, None, None] * rng.standard_normal((P, npart, 3))
+    vt0 = math.sqrt(P * C.KB * T / (m * C.MVV2E)) * rng.standard_normal((P, npart, 3))
+    o.set_model_harmonic(ks)
+    o.set_state(nm.from_nm(o.M, xt0), m * nm.from_nm(o.M, vt0))
+    kcv, kpr, pot, tring = [], [], [], []
+    for _ in range(1500):
+        o.step(1)
+        e = o.estimators()
+        kcv.append(e["K_CV"] / npart)
+        kpr.append(e["K_PR"] / npart)
+        pot.append(e["U_sum"] / P / npart)
+        tring.append(e["T_ring"])
+    exact_P = 1.5 * C.KB * T * np.sum(omega ** 2 / (omega ** 2 + om ** 2))
+    coth = 0.75 * C.HBAR * omega / math.tanh(0.5 * bhw)
+    assert abs(exact_P / coth - 0.99815) < 2e-4                       # SURVEY C-4 ratio at beta hbar w = 4
+
+    def blocked(a, nb=15):
+        b = np.array(a).reshape(nb, -1).mean(axis=1)
+        return b.mean(), b.std(ddof=1) / math.sqrt(nb)
+    for name, series, floor in (("K_CV", kcv, 2e-4), ("V", pot, 4e-4), ("K_PR", kpr, 1.2e-3)):
+        mean, err = blocked(series)
+        assert abs(mean - exact_P) < max(5 * err, floor), (name, mean, err, exact_P)
+    mean, err = blocked(tring)
+    assert abs(mean / (P * T) - 1.0) < max(5 * err / (P * T), 3e-3)   # ring temperature averages n*T (L194)
