@@ -243,9 +243,11 @@ def energy_forces(x, types, box, model, return_parts=False, row_block=32768):
         at = np.flatnonzero(types == t)
         if at.size == 0:
             continue
-        y, tanhs = _mlp_forward(model.fitnet[t], D[at], _fit_rule)
-        E[at] = y[:, 0]
-        dD[at] = _mlp_backward(model.fitnet[t], tanhs, np.ones((at.size, 1)), _fit_rule)
+        hidden, (W4, b4) = model.fitnet[t][:-1], model.fitnet[t][-1]
+        y, tanhs = _mlp_forward(hidden, D[at], _fit_rule)
+        E[at] = (y @ W4 + b4)[:, 0]                              # last layer is linear: E_i = y3.w4 + b4
+        dy = np.broadcast_to(W4[:, 0], y.shape)                 # dU/dy3 = w4
+        dD[at] = _mlp_backward(hidden, tanhs, dy, _fit_rule)
     dD3 = dD.reshape(N, M1, M2)
     # dT[m,c] = sum_{m2<M2} dD[m,m2] T[m2,c]  +  [m<M2] sum_{m1} dD[m1,m] T[m1,c]
     dT = np.einsum("imn,inc->imc", dD3, T[:, :M2, :])
