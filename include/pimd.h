@@ -1,0 +1,162 @@
+/* pimd.h -- C ABI of libpimd_b200: one ring-polymer PIMD/Langevin BAOAB step for all P beads of an
+ * N-atom system resident on one B200 (sm_100a), with a Deep-Potential se_e2_a force model.
+ *
+ * The calls follow the problem statement of arxiv/paper_2602_13553 ("fix pimd/langevin"), cited as
+ * PAPER.md:Lnnn (= /root/reference/PAPER.md), and BASELINE.json's north_star
+ * ("pimd_create with types, masses, box, P, T, dt, gamma and seed; pimd_set_model with the weights;
+ * pimd_step(n); getters for positions, momenta, forces, virial and estimators").
+ * Readings of garbled / silent passages are DESIGN.md section 3 (R-1 .. R-16).
+ *
+ * Conventions (all calls):
+ *   - Units: Angstrom, ps, eV, g/mol, K (LAMMPS "metal"; the paper's worked constants PAPER.md:L458).
+ *   - Unless a name ends in _dev, every array pointer is a HOST pointer owned by the caller; the
+ *     library copies in / out and is synchronous on return.  _dev variants take DEVICE pointers that
+ *     must stay valid until the call returns; work is issued on the context's stream and the call
+ *     returns after that work is complete.
+ *   - Layout of per-bead per-atom vectors: [P][N][3], C order, double.
+ *   - Return value: 0 (PIMD_OK) or a negative code; the text of the last error of a context is
+ *     available from pimd_last_error().  No C++ exception crosses this boundary.
+ *   - A context is not thread-safe; use one context per host thread.
+ *   - The library runs on the current CUDA device at pimd_create() time.  It has no CPU fallback:
+ *     without a CUDA device pimd_create() returns PIMD_ECUDA.
+ */
+#ifndef PIMD_B200_H
+#define PIMD_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PIMD_OK              0
+#define PIMD_EINVAL         -1   /* bad argument (null pointer, non-positive size, unsupported P, ...) */
+#define PIMD_ENOSTATE       -2   /* pimd_set_state has not been called */
+#define PIMD_ENOMODEL       -3   /* no force model has been set */
+#define PIMD_ESEL_OVERFLOW  -4   /* an atom has more neighbours of one type than sel allows (R-11) */
+#define PIMD_ECUDA          -5   /* CUDA runtime error; see pimd_last_error */
+#define PIMD_ENOMEM         -6   /* the caller-supplied workspace is too small */
+
+typedef struct pimd_ctx pimd_ctx;   /* opaque; owned by the library */
+
+/* se_e2_a architecture (R-11..R-16; BASELINE.json configs[0]). */
+#define PIMD_MAX_TYPES 4
+typedef struct pimd_model_desc {
+    double  rcut;                       /* cutoff radius r_c, Angstrom */
+    double  rcut_smth;                  /* start of the smooth switch r_s */
+    int32_t n_types;
+    int32_t sel[PIMD_MAX_TYPES];        /* max neighbours per neighbour type; N_sel = sum */
+    int32_t embed[3];                   /* embedding widths, each layer out = 2*in after the first: {25,50,100} */
+    int32_t axis_neuron;                /* M2 (16) */
+    int32_t fit[3];                     /* fitting hidden widths, all equal: {240,240,240} */
+} pimd_model_desc;
+
+/* Estimators of PAPER.md Appendix A (L319-365) after the last completed step, in eV (T_ring in K). */
+typedef struct pimd_estimators {
+    double  K_PR;     /* primitive kinetic-energy estimator, Eq. A7 (L354) with R-6 */
+    double  K_CV;     /* centroid-virial kinetic-energy estimator, Eq. A9 (L365) */
+    double  H;        /* total ring-polymer energy sum_k K+S+U, Eq. A6 (L350) */
+    double  K_ring;   /* sum_k K^(k), Eq. A1 (L319) */
+    double  S_ring;   /* sum_k S^(k), Eq. A3 (L330) */
+    double  U_sum;    /* sum_k U^(k), Eq. A5 (L343) */
+    double  T_ring;   /* 2 K_ring / (3 P N k_B); averages P*T (L194, L120) */
+    int64_t step;     /* completed steps since pimd_set_state */
+} pimd_estimators;
+
+/* ---- lifetime ------------------------------------------------------------------------------- */
+
+/* Creates a context for N atoms with P beads (Eq. 1: the ring-polymer Hamiltonian).
+ *   types[N]         atom types 0..n_types-1            masses[n_types]  g/mol
+ *   box[3]           orthorhombic periodic box lengths, Angstrom
+ *   n_beads          P: 1, 2, 4, 8, 16, 32 or 64 (power of two; the transform is an in-register FFT)
+ *   T                target temperature in K; the ring is sampled at P*T (L194)
+ *   dt               time step in ps
+ *   gamma_centroid   centroid friction 1/tau in 1/ps (keyword `tau`, L174); 0 = NVE, no O step (R-4)
+ *   seed             Philox key (R-10)
+ * On success *out holds the context.  Device memory is allocated with cudaMalloc unless
+ * pimd_set_workspace() hands the library a buffer (e.g. from PyTorch's caching allocator). */
+int pimd_create(pimd_ctx** out, int n_atoms, const int32_t* types, int n_types, const double* masses,
+                const double box[3], int n_beads, double T, double dt, double gamma_centroid,
+                uint64_t seed);
+void pimd_destroy(pimd_ctx* ctx);
+const char* pimd_last_error(const pimd_ctx* ctx);   /* never NULL; "" when there was no error */
+
+/* Optional plumbing: the caller lends device memory and a stream (cudaStream_t as void*; NULL = the
+ * legacy default stream).  pimd_workspace_bytes returns the bytes needed for this context including
+ * the buffers of the se_e2_a model `d`.  Must be called before pimd_set_state / pimd_set_model*.  The buffer
+ * (256-byte aligned) stays owned by the caller and must outlive the context. */
+size_t pimd_workspace_bytes(const pimd_ctx* ctx, const pimd_model_desc* d /* NULL: harmonic model only */);
+int pimd_set_workspace(pimd_ctx* ctx, void* workspace_dev, size_t bytes, void* cuda_stream);
+
+/* ---- inputs --------------------------------------------------------------------------------- */
+
+/* x[P][N][3] unwrapped Cartesian bead positions (L202); p[P][N][3] Cartesian bead momenta in
+ * (g/mol) A/ps.  Resets the step counter to 0.  If a model is set, evaluates the initial forces
+ * (BAOAB opens with a B that needs f(x0)). */
+int pimd_set_state(pimd_ctx* ctx, const double* x, const double* p);
+
+/* The se_e2_a Deep-Potential model (PAPER.md:L47, L76 cite it; definition DESIGN.md R-11..R-16).
+ * weights: n_weights doubles, row-major W[in][out] then bias[out] per layer, in the order
+ *   for t_i: for t_j: embedding layers 1..3;  then for t_i: fitting layers 1..4 (last out = 1).
+ * n_weights must equal pimd_model_n_weights(d).  The library converts to FP32 on the device. */
+size_t pimd_model_n_weights(const pimd_model_desc* d);
+int pimd_set_model(pimd_ctx* ctx, const pimd_model_desc* d, const double* weights, size_t n_weights);
+
+/* Test model: U = sum_i 1/2 k |r_i|^2 about the origin on the unwrapped coordinates (FP64), used to
+ * check the integrator alone against closed forms (north_star's harmonic-oscillator check). */
+int pimd_set_model_harmonic(pimd_ctx* ctx, double k_spring /* eV/A^2 */);
+
+/* ---- the hot path --------------------------------------------------------------------------- */
+
+/* n_steps BAOAB steps: B(dt/2) A(dt/2) O(dt) A(dt/2) [force] B(dt/2), with the three
+ * normal-mode transforms of L192 and one force evaluation per step (R-7).  All work runs on the
+ * GPU; there is no host round trip inside the loop. */
+int pimd_step(pimd_ctx* ctx, int64_t n_steps);
+
+/* ---- outputs -------------------------------------------------------------------------------- */
+int pimd_get_positions(pimd_ctx* ctx, double* x /* [P][N][3] A, unwrapped */);
+int pimd_get_momenta(pimd_ctx* ctx, double* p /* [P][N][3] Cartesian, (g/mol) A/ps */);
+int pimd_get_forces(pimd_ctx* ctx, double* f /* [P][N][3] eV/A */);
+int pimd_get_virial(pimd_ctx* ctx, double* xi /* [P][9] eV; Xi_ab = -sum_rows d_a dU/dd_b (L372, R-16) */);
+int pimd_get_energies(pimd_ctx* ctx, double* U /* [P] eV, bead potential energies (A5, L343) */);
+int pimd_get_atom_energies(pimd_ctx* ctx, double* E /* [P][N] eV, E_i of the fitting net */);
+int pimd_get_estimators(pimd_ctx* ctx, pimd_estimators* e);
+/* Estimators of each of the last `n` completed steps of the most recent pimd_step call, oldest first
+ * (configs[1]: "estimators reported every step").  Returns the number written (<= cap) or < 0. */
+int pimd_get_estimator_history(pimd_ctx* ctx, pimd_estimators* e, int cap);
+
+/* Device-pointer variants for callers that keep the state in HBM (bench.py's resident-input leg). */
+int pimd_set_state_dev(pimd_ctx* ctx, const double* x_dev, const double* p_dev);
+int pimd_get_positions_dev(pimd_ctx* ctx, double* x_dev);
+int pimd_get_forces_dev(pimd_ctx* ctx, double* f_dev);
+
+/* ---- parity hooks --------------------------------------------------------------------------- */
+
+/* Neighbour rows of one bead from the most recent force evaluation, in canonical order: for atom i
+ * the rows sorted by (type_j, j, n_x, n_y, n_z).  count[N] receives the rows per atom; j[cap] and
+ * shift[cap][3] (periodic image n of R-11) receive the concatenated rows.  Returns the total number
+ * of rows, or PIMD_EINVAL when cap is too small. */
+int64_t pimd_get_neighbors(pimd_ctx* ctx, int bead, int32_t* count, int32_t* j, int8_t* shift, size_t cap);
+
+/* The four Philox4x32-10 words and the normal eta the O step uses for (step, mode k, atom i,
+ * component alpha) (R-10), evaluated ON THE DEVICE for n entries: idx[n][3] = (k, i, alpha);
+ * words[n][4], eta[n].  */
+int pimd_debug_noise(pimd_ctx* ctx, int64_t step, int n, const int32_t* idx, uint32_t* words, double* eta);
+
+/* Stand-alone timing of kernels (bench.py roofline legs): runs `reps` launches of the fused
+ * integrator kernel (kind 0) on the current state WITHOUT advancing it (output to scratch), and
+ * returns the mean device time per launch in milliseconds through *ms. */
+int pimd_time_kernel(pimd_ctx* ctx, int kind, int reps, double* ms);
+
+/* Mean device milliseconds per step of each phase of the last pimd_step call, when profiling was
+ * enabled with pimd_set_profiling(ctx, 1) (CUDA events on the context's stream):
+ * ms[0] integrator, [1] neighbour+environment, [2] embedding fwd, [3] descriptor+fitting fwd/bwd,
+ * [4] embedding bwd + force/virial, [5] reserved. */
+int pimd_set_profiling(pimd_ctx* ctx, int on);
+int pimd_get_phase_ms(pimd_ctx* ctx, double ms[6]);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PIMD_B200_H */

@@ -1,0 +1,18 @@
+"""paper_2602_13553_b200 -- B200-native hot path of "fix pimd/langevin" (arxiv/paper_2602_13553):
+one ring-polymer PIMD/Langevin BAOAB step for all beads of a water box with an se_e2_a Deep-Potential
+force model, as hand-written CUDA for sm_100a behind the C ABI of include/pimd.h.
+
+This package is argument marshalling only (ctypes); every step of the path runs in the kernels of
+csrc/*.cu.  There is no CPU fallback: importing works without a GPU (so the symbol table can be
+checked), but every compute call needs the compiled library and a CUDA device.
+"""
+from .binding import (  # noqa: F401
+    PIMD_OK, PIMD_EINVAL, PIMD_ENOSTATE, PIMD_ENOMODEL, PIMD_ESEL_OVERFLOW, PIMD_ECUDA, PIMD_ENOMEM,
+    PimdError, ModelDesc, Estimators, lib, library_path,
+    pimd_create, pimd_destroy, pimd_last_error, pimd_workspace_bytes, pimd_set_workspace,
+    pimd_set_state, pimd_set_state_dev, pimd_model_n_weights, pimd_set_model, pimd_set_model_harmonic,
+    pimd_step, pimd_get_positions, pimd_get_momenta, pimd_get_forces, pimd_get_virial, pimd_get_energies,
+    pimd_get_atom_energies, pimd_get_estimators, pimd_get_estimator_history, pimd_get_positions_dev,
+    pimd_get_forces_dev, pimd_get_neighbors, pimd_debug_noise, pimd_time_kernel, pimd_set_profiling,
+    pimd_get_phase_ms, PIMD,
+)

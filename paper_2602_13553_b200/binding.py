@@ -1,0 +1,319 @@
+"""ctypes binding of include/pimd.h -- same names, argument marshalling only.
+
+Host arrays are numpy float64 / int32; `_dev` calls take torch CUDA tensors (or raw device pointers).
+PyTorch is used only to lend device memory (a uint8 workspace tensor from its caching allocator) and
+the current stream to the library (`PIMD(..., torch_workspace=True)`).
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+PIMD_OK, PIMD_EINVAL, PIMD_ENOSTATE, PIMD_ENOMODEL = 0, -1, -2, -3
+PIMD_ESEL_OVERFLOW, PIMD_ECUDA, PIMD_ENOMEM = -4, -5, -6
+PIMD_MAX_TYPES = 4
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def library_path():
+    return os.path.join(_HERE, "libpimd_b200.so")
+
+
+class PimdError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("pimd error %d: %s" % (code, msg))
+        self.code = code
+
+
+class ModelDesc(C.Structure):
+    _fields_ = [("rcut", C.c_double), ("rcut_smth", C.c_double), ("n_types", C.c_int32),
+                ("sel", C.c_int32 * PIMD_MAX_TYPES), ("embed", C.c_int32 * 3), ("axis_neuron", C.c_int32),
+                ("fit", C.c_int32 * 3)]
+
+    @classmethod
+    def from_dict(cls, d):
+        m = cls()
+        m.rcut, m.rcut_smth = float(d["rcut"]), float(d["rcut_smth"])
+        m.n_types = len(d["sel"])
+        for t, s in enumerate(d["sel"]):
+            m.sel[t] = int(s)
+        for l in range(3):
+            m.embed[l] = int(d["embed"][l])
+            m.fit[l] = int(d["fit"][l])
+        m.axis_neuron = int(d["axis"])
+        return m
+
+
+class Estimators(C.Structure):
+    _fields_ = [("K_PR", C.c_double), ("K_CV", C.c_double), ("H", C.c_double), ("K_ring", C.c_double),
+                ("S_ring", C.c_double), ("U_sum", C.c_double), ("T_ring", C.c_double), ("step", C.c_int64)]
+
+    def as_dict(self):
+        return {n: getattr(self, n) for n, _ in self._fields_}
+
+
+_lib = None
+
+_SIGNATURES = {
+    "pimd_create": (C.c_int, [C.POINTER(C.c_void_p), C.c_int, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p,
+                              C.c_int, C.c_double, C.c_double, C.c_double, C.c_uint64]),
+    "pimd_destroy": (None, [C.c_void_p]),
+    "pimd_last_error": (C.c_char_p, [C.c_void_p]),
+    "pimd_workspace_bytes": (C.c_size_t, [C.c_void_p, C.c_void_p]),
+    "pimd_set_workspace": (C.c_int, [C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]),
+    "pimd_set_state": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
+    "pimd_set_state_dev": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
+    "pimd_model_n_weights": (C.c_size_t, [C.c_void_p]),
+    "pimd_set_model": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t]),
+    "pimd_set_model_harmonic": (C.c_int, [C.c_void_p, C.c_double]),
+    "pimd_step": (C.c_int, [C.c_void_p, C.c_int64]),
+    "pimd_get_positions": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "pimd_get_momenta": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "pimd_get_forces": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "pimd_get_virial": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "pimd_get_energies": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "pimd_get_atom_energies": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "pimd_get_estimators": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "pimd_get_estimator_history": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int]),
+    "pimd_get_positions_dev": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "pimd_get_forces_dev": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "pimd_get_neighbors": (C.c_int64, [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t]),
+    "pimd_debug_noise": (C.c_int, [C.c_void_p, C.c_int64, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "pimd_time_kernel": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.POINTER(C.c_double)]),
+    "pimd_set_profiling": (C.c_int, [C.c_void_p, C.c_int]),
+    "pimd_get_phase_ms": (C.c_int, [C.c_void_p, C.c_void_p]),
+}
+
+
+def lib():
+    """Loads libpimd_b200.so (built by paper_2602_13553_b200.build).  Fails loudly if it is missing."""
+    global _lib
+    if _lib is None:
+        path = library_path()
+        if not os.path.exists(path):
+            raise ImportError("%s not found: build it with `python -m paper_2602_13553_b200.build` "
+                              "(there is no CPU fallback)" % path)
+        L = C.CDLL(path)
+        for name, (res, args) in _SIGNATURES.items():
+            fn = getattr(L, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = L
+    return _lib
+
+
+def _check(ctx, rc):
+    if rc < 0:
+        raise PimdError(rc, pimd_last_error(ctx))
+    return rc
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _ptr(a):
+    """numpy array -> host pointer; torch tensor -> device pointer; int -> as is."""
+    if isinstance(a, np.ndarray):
+        return a.ctypes.data
+    if hasattr(a, "data_ptr"):
+        return a.data_ptr()
+    return int(a)
+
+
+# ---- same-name wrappers ------------------------------------------------------------------------
+
+def pimd_create(types, masses, box, n_beads, T, dt, gamma_centroid, seed):
+    types = np.ascontiguousarray(types, dtype=np.int32)
+    masses, box = _f64(masses), _f64(box)
+    ctx = C.c_void_p()
+    rc = lib().pimd_create(C.byref(ctx), types.size, types.ctypes.data, masses.size, masses.ctypes.data,
+                           box.ctypes.data, int(n_beads), float(T), float(dt), float(gamma_centroid),
+                           int(seed) & 0xFFFFFFFFFFFFFFFF)
+    if rc < 0:
+        raise PimdError(rc, "pimd_create failed (no CUDA device?)" if rc == PIMD_ECUDA else "pimd_create: bad argument")
+    return ctx
+
+
+def pimd_destroy(ctx):
+    lib().pimd_destroy(ctx)
+
+
+def pimd_last_error(ctx):
+    return lib().pimd_last_error(ctx).decode()
+
+
+def pimd_workspace_bytes(ctx, desc=None):
+    return lib().pimd_workspace_bytes(ctx, C.byref(desc) if desc is not None else None)
+
+
+def pimd_set_workspace(ctx, workspace_dev, nbytes, cuda_stream=0):
+    return _check(ctx, lib().pimd_set_workspace(ctx, _ptr(workspace_dev), int(nbytes), int(cuda_stream) or None))
+
+
+def pimd_set_state(ctx, x, p):
+    x, p = _f64(x), _f64(p)
+    return _check(ctx, lib().pimd_set_state(ctx, x.ctypes.data, p.ctypes.data))
+
+
+def pimd_set_state_dev(ctx, x_dev, p_dev):
+    return _check(ctx, lib().pimd_set_state_dev(ctx, _ptr(x_dev), _ptr(p_dev)))
+
+
+def pimd_model_n_weights(desc):
+    return lib().pimd_model_n_weights(C.byref(desc))
+
+
+def pimd_set_model(ctx, desc, weights):
+    w = _f64(weights)
+    return _check(ctx, lib().pimd_set_model(ctx, C.byref(desc), w.ctypes.data, w.size))
+
+
+def pimd_set_model_harmonic(ctx, k_spring):
+    return _check(ctx, lib().pimd_set_model_harmonic(ctx, float(k_spring)))
+
+
+def pimd_step(ctx, n_steps=1):
+    return _check(ctx, lib().pimd_step(ctx, int(n_steps)))
+
+
+def _getter(name, ctx, shape):
+    out = np.empty(shape, dtype=np.float64)
+    _check(ctx, getattr(lib(), name)(ctx, out.ctypes.data))
+    return out
+
+
+def pimd_get_positions(ctx, P, N):
+    return _getter("pimd_get_positions", ctx, (P, N, 3))
+
+
+def pimd_get_momenta(ctx, P, N):
+    return _getter("pimd_get_momenta", ctx, (P, N, 3))
+
+
+def pimd_get_forces(ctx, P, N):
+    return _getter("pimd_get_forces", ctx, (P, N, 3))
+
+
+def pimd_get_virial(ctx, P):
+    return _getter("pimd_get_virial", ctx, (P, 3, 3))
+
+
+def pimd_get_energies(ctx, P):
+    return _getter("pimd_get_energies", ctx, (P,))
+
+
+def pimd_get_atom_energies(ctx, P, N):
+    return _getter("pimd_get_atom_energies", ctx, (P, N))
+
+
+def pimd_get_estimators(ctx):
+    e = Estimators()
+    _check(ctx, lib().pimd_get_estimators(ctx, C.byref(e)))
+    return e.as_dict()
+
+
+def pimd_get_estimator_history(ctx, cap):
+    arr = (Estimators * cap)()
+    n = _check(ctx, lib().pimd_get_estimator_history(ctx, arr, cap))
+    return [arr[q].as_dict() for q in range(n)]
+
+
+def pimd_get_positions_dev(ctx, x_dev):
+    return _check(ctx, lib().pimd_get_positions_dev(ctx, _ptr(x_dev)))
+
+
+def pimd_get_forces_dev(ctx, f_dev):
+    return _check(ctx, lib().pimd_get_forces_dev(ctx, _ptr(f_dev)))
+
+
+def pimd_get_neighbors(ctx, bead, N, cap):
+    count = np.empty(N, dtype=np.int32)
+    j = np.empty(cap, dtype=np.int32)
+    shift = np.empty((cap, 3), dtype=np.int8)
+    n = lib().pimd_get_neighbors(ctx, int(bead), count.ctypes.data, j.ctypes.data, shift.ctypes.data, cap)
+    _check(ctx, int(n))
+    return count, j[:n].copy(), shift[:n].copy()
+
+
+def pimd_debug_noise(ctx, step, idx):
+    idx = np.ascontiguousarray(idx, dtype=np.int32).reshape(-1, 3)
+    n = idx.shape[0]
+    words = np.empty((n, 4), dtype=np.uint32)
+    eta = np.empty(n, dtype=np.float64)
+    _check(ctx, lib().pimd_debug_noise(ctx, int(step), n, idx.ctypes.data, words.ctypes.data, eta.ctypes.data))
+    return words, eta
+
+
+def pimd_time_kernel(ctx, kind, reps):
+    ms = C.c_double()
+    _check(ctx, lib().pimd_time_kernel(ctx, int(kind), int(reps), C.byref(ms)))
+    return ms.value
+
+
+def pimd_set_profiling(ctx, on):
+    return _check(ctx, lib().pimd_set_profiling(ctx, int(bool(on))))
+
+
+def pimd_get_phase_ms(ctx):
+    out = np.zeros(6, dtype=np.float64)
+    _check(ctx, lib().pimd_get_phase_ms(ctx, out.ctypes.data))
+    return out
+
+
+class PIMD:
+    """Convenience owner of one context (create .. destroy) with the shapes remembered."""
+
+    def __init__(self, types, masses, box, n_beads, T, dt, gamma_centroid, seed, model_desc=None,
+                 torch_workspace=True):
+        self.N, self.P = int(np.asarray(types).size), int(n_beads)
+        self.ctx = pimd_create(types, masses, box, n_beads, T, dt, gamma_centroid, seed)
+        self.desc = ModelDesc.from_dict(model_desc) if isinstance(model_desc, dict) else model_desc
+        self._ws = None
+        if torch_workspace:
+            import torch
+            nbytes = pimd_workspace_bytes(self.ctx, self.desc)
+            self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device="cuda")   # caching allocator
+            base = (self._ws.data_ptr() + 255) // 256 * 256
+            pimd_set_workspace(self.ctx, base, nbytes, torch.cuda.current_stream().cuda_stream)
+
+    def close(self):
+        if self.ctx is not None:
+            pimd_destroy(self.ctx)
+            self.ctx = None
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_state(self, x, p):
+        if hasattr(x, "data_ptr"):
+            return pimd_set_state_dev(self.ctx, x, p)
+        return pimd_set_state(self.ctx, x, p)
+
+    def set_model(self, weights, desc=None):
+        if desc is not None:
+            self.desc = ModelDesc.from_dict(desc) if isinstance(desc, dict) else desc
+        return pimd_set_model(self.ctx, self.desc, weights)
+
+    def set_model_harmonic(self, k):
+        return pimd_set_model_harmonic(self.ctx, k)
+
+    def step(self, n=1):
+        return pimd_step(self.ctx, n)
+
+    def positions(self): return pimd_get_positions(self.ctx, self.P, self.N)
+    def momenta(self): return pimd_get_momenta(self.ctx, self.P, self.N)
+    def forces(self): return pimd_get_forces(self.ctx, self.P, self.N)
+    def virial(self): return pimd_get_virial(self.ctx, self.P)
+    def energies(self): return pimd_get_energies(self.ctx, self.P)
+    def atom_energies(self): return pimd_get_atom_energies(self.ctx, self.P, self.N)
+    def estimators(self): return pimd_get_estimators(self.ctx)
+    def estimator_history(self, cap=4096): return pimd_get_estimator_history(self.ctx, cap)
+
+    def neighbors(self, bead, cap=None):
+        cap = cap or self.N * 512
+        return pimd_get_neighbors(self.ctx, bead, self.N, cap)

@@ -1,0 +1,699 @@
+// api.cu -- the C ABI of include/pimd.h: context, device-memory arena, model upload, the step driver.
+// Host logic only; every step of the hot path runs in the kernels of integrator.cu, neighbor.cu,
+// embedding.cu and fitting.cu.  No CPU fallback: CUDA errors are returned as PIMD_ECUDA.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include "common.cuh"
+
+using namespace pimd;
+
+struct pimd_ctx {
+    int N = 0, P = 0, ntypes = 0;
+    double box[3] = {0, 0, 0}, T = 0, dt = 0, gamma0 = 0;
+    uint64_t seed = 0;
+    int64_t step = 0;
+    std::vector<int32_t> types;
+    std::vector<double> masses;
+    std::string err;
+    int n_sms = 148;
+
+    // memory arena
+    char* arena = nullptr; size_t arena_bytes = 0, arena_used = 0;    // caller-lent workspace (bump allocator)
+    std::vector<void*> owned;                                          // cudaMalloc'ed buffers otherwise
+    cudaStream_t stream = nullptr;
+
+    // state
+    bool have_state = false;
+    int model_kind = 0;           // 0 none, 1 harmonic, 2 se_e2_a
+    double k_spring = 0;
+    double *x = nullptr, *vt = nullptr, *f = nullptr, *mass_atom = nullptr;
+    double *scratch_a = nullptr, *scratch_b = nullptr;     // [P][N][3] each: momenta staging / timing outputs
+    int* types_d = nullptr;
+    double *U = nullptr, *Xi = nullptr, *Eatom = nullptr;
+    double* est = nullptr;        // [kEstCap + 2][kEstWidth]; slot kEstCap = "current", kEstCap+1 = scratch
+    int est_hist_n = 0;           // valid history slots of the last pimd_step call
+    int64_t est_hist_first_step = 0;
+    ModeConsts mc;
+    Model model;
+
+    // profiling
+    bool profiling = false;
+    cudaEvent_t ev[8] = {};
+    double phase_ms[6] = {0, 0, 0, 0, 0, 0};
+    int64_t phase_steps = 0;
+};
+
+namespace {
+
+int fail(pimd_ctx* c, int code, const std::string& msg) {
+    if (c) c->err = msg;
+    return code;
+}
+#define CK(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e__ = (call);                                                                  \
+        if (e__ != cudaSuccess)                                                                    \
+            return fail(ctx, PIMD_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e__));   \
+    } while (0)
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+template <typename T>
+int arena_alloc(pimd_ctx* ctx, T** out, size_t count) {
+    const size_t bytes = align_up(count * sizeof(T), 256);
+    if (!ctx->arena) {
+        void* p = nullptr;
+        CK(cudaMalloc(&p, bytes));
+        ctx->owned.push_back(p);
+        *out = reinterpret_cast<T*>(p);
+        return PIMD_OK;
+    }
+    if (ctx->arena_used + bytes > ctx->arena_bytes)
+        return fail(ctx, PIMD_ENOMEM, "device arena exhausted (workspace too small)");
+    *out = reinterpret_cast<T*>(ctx->arena + ctx->arena_used);
+    ctx->arena_used += bytes;
+    return PIMD_OK;
+}
+
+size_t base_bytes(const pimd_ctx* c) {
+    const size_t PN3 = (size_t)c->P * c->N * 3;
+    size_t b = 0;
+    b += 5 * align_up(PN3 * 8, 256);                          // x, vt, f, scratch_a, scratch_b
+    b += align_up((size_t)c->N * 8, 256) + align_up((size_t)c->N * 4, 256);
+    b += align_up((size_t)c->P * 8, 256) + align_up((size_t)c->P * 72, 256) + align_up((size_t)c->P * c->N * 8, 256);
+    b += align_up((size_t)(kEstCap + 2) * kEstWidth * 8, 256);
+    return b + 4096;
+}
+
+void cell_grid(const double box[3], double rcut, int ncell[3], int R[3], int* ncells) {
+    *ncells = 1;
+    for (int a = 0; a < 3; ++a) {
+        int nc = (int)std::floor(box[a] / (rcut * (1.0 + 1e-9)));
+        if (nc < 1) nc = 1;
+        ncell[a] = nc;
+        const double w = box[a] / nc;
+        R[a] = (int)std::ceil(rcut / w - 1e-12);
+        if (R[a] < 1) R[a] = 1;
+        *ncells *= nc;
+    }
+}
+
+size_t model_bytes(const pimd_ctx* c, const pimd_model_desc* d) {
+    if (!d) return 0;
+    const size_t PN = (size_t)c->P * c->N;
+    int nsel = 0;
+    for (int t = 0; t < d->n_types; ++t) nsel += d->sel[t];
+    const int M1 = d->embed[2], M2 = d->axis_neuron, NF = d->fit[0], ND = M1 * M2;
+    int ncell[3], R[3], ncells;
+    cell_grid(c->box, d->rcut, ncell, R, &ncells);
+    size_t b = 0;
+    b += align_up((size_t)d->n_types * d->n_types * 8192 * 4, 256);                     // embedding weights (padded)
+    b += (size_t)d->n_types * 2 * (align_up((size_t)ND * NF * 4, 256) + 2 * align_up((size_t)NF * NF * 4, 256) + align_up(NF * 4, 256));
+    b += (size_t)d->n_types * 4 * align_up((size_t)NF * 4, 256);
+    b += 4 * align_up(PN * 4, 256);                                                    // cen_idx,row_of,cell_id,cell_tmp
+    b += 3 * align_up((size_t)c->P * (ncells + 1) * 4, 256);
+    b += align_up(PN * 24, 256) + align_up(PN * 32, 256);
+    b += align_up(PN * d->n_types * 4, 256);
+    b += 2 * align_up(PN * nsel * 16, 256);
+    b += 256;
+    b += 2 * align_up(PN * M1 * 16, 256);
+    b += 2 * align_up(PN * ND * 4, 256);
+    b += 7 * align_up(PN * NF * 4, 256);
+    return b + 65536;
+}
+
+void mode_constants(pimd_ctx* c) {
+    const int P = c->P;
+    const double wP = P * kKB * c->T / kHbar;              // Eq. 2
+    const double h = 0.5 * c->dt;
+    for (int k = 0; k < kMaxBeads; ++k) {
+        c->mc.cosA[k] = 1; c->mc.sinA_w[k] = h; c->mc.msinA_w[k] = 0; c->mc.c1[k] = 1; c->mc.c2[k] = 0; c->mc.om2[k] = 0;
+    }
+    for (int k = 0; k < P; ++k) {
+        const double sk = std::sin(k * M_PI / P);
+        const double lam = 4.0 * sk * sk;                  // Eq. B2
+        const double w = std::sqrt(lam) * wP;              // L469
+        c->mc.om2[k] = w * w;
+        if (k > 0) {
+            c->mc.cosA[k] = std::cos(w * h);
+            c->mc.sinA_w[k] = std::sin(w * h) / w;
+            c->mc.msinA_w[k] = -w * std::sin(w * h);
+        }
+        const double gam = (k == 0) ? c->gamma0 : 2.0 * w;  // Eq. D1; tau_0 = 1/gamma0 (L174)
+        c->mc.c1[k] = std::exp(-c->dt * gam);               // full dt: BAOAB has one O (R-3)
+        c->mc.c2[k] = std::sqrt(1.0 - c->mc.c1[k] * c->mc.c1[k]);
+    }
+}
+
+int alloc_base(pimd_ctx* ctx) {
+    if (ctx->x) return PIMD_OK;
+    const size_t PN3 = (size_t)ctx->P * ctx->N * 3;
+    int rc;
+    if ((rc = arena_alloc(ctx, &ctx->x, PN3))) return rc;
+    if ((rc = arena_alloc(ctx, &ctx->vt, PN3))) return rc;
+    if ((rc = arena_alloc(ctx, &ctx->f, PN3))) return rc;
+    if ((rc = arena_alloc(ctx, &ctx->scratch_a, PN3))) return rc;
+    if ((rc = arena_alloc(ctx, &ctx->scratch_b, PN3))) return rc;
+    if ((rc = arena_alloc(ctx, &ctx->mass_atom, (size_t)ctx->N))) return rc;
+    if ((rc = arena_alloc(ctx, &ctx->types_d, (size_t)ctx->N))) return rc;
+    if ((rc = arena_alloc(ctx, &ctx->U, (size_t)ctx->P))) return rc;
+    if ((rc = arena_alloc(ctx, &ctx->Xi, (size_t)ctx->P * 9))) return rc;
+    if ((rc = arena_alloc(ctx, &ctx->Eatom, (size_t)ctx->P * ctx->N))) return rc;
+    if ((rc = arena_alloc(ctx, &ctx->est, (size_t)(kEstCap + 2) * kEstWidth))) return rc;
+    std::vector<double> ma(ctx->N);
+    for (int i = 0; i < ctx->N; ++i) ma[i] = ctx->masses[ctx->types[i]];
+    CK(cudaMemcpyAsync(ctx->mass_atom, ma.data(), sizeof(double) * ctx->N, cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaMemcpyAsync(ctx->types_d, ctx->types.data(), sizeof(int) * ctx->N, cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaMemsetAsync(ctx->f, 0, PN3 * 8, ctx->stream));
+    CK(cudaMemsetAsync(ctx->U, 0, sizeof(double) * ctx->P, ctx->stream));
+    CK(cudaMemsetAsync(ctx->Xi, 0, sizeof(double) * 9 * ctx->P, ctx->stream));
+    CK(cudaMemsetAsync(ctx->Eatom, 0, sizeof(double) * ctx->P * ctx->N, ctx->stream));
+    CK(cudaMemsetAsync(ctx->est, 0, sizeof(double) * (kEstCap + 2) * kEstWidth, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return PIMD_OK;
+}
+
+void rec(pimd_ctx* ctx, int i) {
+    if (ctx->profiling) cudaEventRecord(ctx->ev[i], ctx->stream);
+}
+
+// one force evaluation at the current x: f, U, Xi, Eatom
+int eval_forces(pimd_ctx* ctx) {
+    if (ctx->model_kind == 1) {
+        launch_harmonic(ctx->P, ctx->N, ctx->k_spring, ctx->x, ctx->f, ctx->U, ctx->Xi, ctx->Eatom, ctx->stream);
+        return PIMD_OK;
+    }
+    ForceArgs a;
+    a.P = ctx->P; a.N = ctx->N; a.ntypes = ctx->ntypes;
+    for (int c = 0; c < 3; ++c) a.box[c] = ctx->box[c];
+    a.x = ctx->x; a.types = ctx->types_d; a.f = ctx->f; a.U = ctx->U; a.Xi = ctx->Xi; a.Eatom = ctx->Eatom;
+    const size_t PN3 = (size_t)ctx->P * ctx->N * 3;
+    cudaMemsetAsync(ctx->f, 0, PN3 * 8, ctx->stream);
+    cudaMemsetAsync(ctx->U, 0, sizeof(double) * ctx->P, ctx->stream);
+    cudaMemsetAsync(ctx->Xi, 0, sizeof(double) * 9 * ctx->P, ctx->stream);
+    rec(ctx, 1);
+    neighbor_build(ctx->model, a, ctx->stream);
+    rec(ctx, 2);
+    embedding_forward(ctx->model, a, ctx->n_sms, ctx->stream);
+    rec(ctx, 3);
+    fitting_forward_backward(ctx->model, a, ctx->stream);
+    rec(ctx, 4);
+    embedding_backward(ctx->model, a, ctx->n_sms, ctx->stream);
+    rec(ctx, 5);
+    return PIMD_OK;
+}
+
+void fill_integrator_args(pimd_ctx* ctx, IntegratorArgs& a, int flags, int64_t step, double* est_slot) {
+    a.N = ctx->N; a.n_dof = 3 * ctx->N; a.flags = flags;
+    a.thermostat = (ctx->gamma0 != 0.0) ? 1 : 0;
+    a.half_dt_mvv = 0.5 * ctx->dt / kMvv2e;
+    a.PkT_mvv = ctx->P * kKB * ctx->T / kMvv2e;
+    a.seed_lo = (uint32_t)ctx->seed; a.seed_hi = (uint32_t)(ctx->seed >> 32);
+    a.step_lo = (uint32_t)(uint64_t)step; a.step_hi = (uint32_t)((uint64_t)step >> 32);
+    a.x_in = ctx->x; a.vt_in = ctx->vt; a.f = ctx->f; a.x_out = ctx->x; a.vt_out = ctx->vt;
+    a.mass = ctx->mass_atom; a.U = ctx->U; a.est = est_slot;
+}
+
+int check_overflow(pimd_ctx* ctx) {
+    if (ctx->model_kind != 2) return PIMD_OK;
+    int flag = 0;
+    CK(cudaMemcpyAsync(&flag, ctx->model.overflow, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    if (flag) {
+        cudaMemsetAsync(ctx->model.overflow, 0, sizeof(int), ctx->stream);
+        return fail(ctx, PIMD_ESEL_OVERFLOW, "an atom has more neighbours of one type than sel allows");
+    }
+    return PIMD_OK;
+}
+
+// forces + estimators of the current (x, v~): used after set_state / set_model
+int refresh(pimd_ctx* ctx) {
+    if (!ctx->have_state || ctx->model_kind == 0) return PIMD_OK;
+    int rc = eval_forces(ctx);
+    if (rc) return rc;
+    double* cur = ctx->est + (size_t)kEstCap * kEstWidth;
+    CK(cudaMemsetAsync(cur, 0, sizeof(double) * kEstWidth, ctx->stream));
+    IntegratorArgs a;
+    fill_integrator_args(ctx, a, I_EST, ctx->step, cur);
+    launch_integrator(ctx->P, a, ctx->mc, ctx->stream);
+    CK(cudaGetLastError());
+    CK(cudaStreamSynchronize(ctx->stream));
+    ctx->est_hist_n = 0;
+    return check_overflow(ctx);
+}
+
+void finalize_est(const pimd_ctx* c, const double raw[kEstWidth], int64_t step, pimd_estimators* e) {
+    const double P = c->P, N = c->N;
+    e->K_ring = raw[0]; e->S_ring = raw[1]; e->U_sum = raw[3];
+    e->H = raw[0] + raw[1] + raw[3];
+    e->K_PR = 1.5 * P * N * kKB * c->T - raw[1] / P;              // A7 with R-6
+    e->K_CV = 1.5 * N * kKB * c->T - raw[2] / (2.0 * P);          // A9
+    e->T_ring = 2.0 * raw[0] / (3.0 * P * N * kKB);
+    e->step = step;
+}
+
+}  // namespace
+
+extern "C" {
+
+int pimd_create(pimd_ctx** out, int n_atoms, const int32_t* types, int n_types, const double* masses,
+                const double box[3], int n_beads, double T, double dt, double gamma_centroid, uint64_t seed) {
+    if (!out) return PIMD_EINVAL;
+    *out = nullptr;
+    if (n_atoms <= 0 || !types || n_types <= 0 || n_types > PIMD_MAX_TYPES || !masses || !box) return PIMD_EINVAL;
+    if (!(n_beads == 1 || n_beads == 2 || n_beads == 4 || n_beads == 8 || n_beads == 16 || n_beads == 32 || n_beads == 64))
+        return PIMD_EINVAL;
+    if (!(T > 0) || !(dt > 0) || gamma_centroid < 0 || !(box[0] > 0 && box[1] > 0 && box[2] > 0)) return PIMD_EINVAL;
+    for (int i = 0; i < n_atoms; ++i)
+        if (types[i] < 0 || types[i] >= n_types) return PIMD_EINVAL;
+    for (int t = 0; t < n_types; ++t)
+        if (!(masses[t] > 0)) return PIMD_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return PIMD_ECUDA;   // no CPU fallback
+    pimd_ctx* ctx = new (std::nothrow) pimd_ctx();
+    if (!ctx) return PIMD_ENOMEM;
+    ctx->N = n_atoms; ctx->P = n_beads; ctx->ntypes = n_types;
+    for (int c = 0; c < 3; ++c) ctx->box[c] = box[c];
+    ctx->T = T; ctx->dt = dt; ctx->gamma0 = gamma_centroid; ctx->seed = seed;
+    ctx->types.assign(types, types + n_atoms);
+    ctx->masses.assign(masses, masses + n_types);
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&ctx->n_sms, cudaDevAttrMultiProcessorCount, dev);
+    mode_constants(ctx);
+    for (int i = 0; i < 8; ++i) cudaEventCreate(&ctx->ev[i]);
+    *out = ctx;
+    return PIMD_OK;
+}
+
+void pimd_destroy(pimd_ctx* ctx) {
+    if (!ctx) return;
+    cudaStreamSynchronize(ctx->stream);
+    for (void* p : ctx->owned) cudaFree(p);
+    for (int i = 0; i < 8; ++i)
+        if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
+    delete ctx;
+}
+
+const char* pimd_last_error(const pimd_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+size_t pimd_workspace_bytes(const pimd_ctx* ctx, const pimd_model_desc* d) {
+    if (!ctx) return 0;
+    return base_bytes(ctx) + model_bytes(ctx, d);
+}
+
+int pimd_set_workspace(pimd_ctx* ctx, void* ws, size_t bytes, void* stream) {
+    if (!ctx) return PIMD_EINVAL;
+    if (ctx->arena || ctx->x) return fail(ctx, PIMD_EINVAL, "workspace must be set before any state or model call");
+    ctx->stream = reinterpret_cast<cudaStream_t>(stream);
+    if (ws) {
+        if (((uintptr_t)ws & 255) != 0) return fail(ctx, PIMD_EINVAL, "workspace must be 256-byte aligned");
+        ctx->arena = reinterpret_cast<char*>(ws);
+        ctx->arena_bytes = bytes; ctx->arena_used = 0;
+    }
+    return PIMD_OK;
+}
+
+size_t pimd_model_n_weights(const pimd_model_desc* d) {
+    if (!d) return 0;
+    size_t ne = 0, nin = 1;
+    for (int l = 0; l < 3; ++l) { ne += nin * d->embed[l] + d->embed[l]; nin = d->embed[l]; }
+    size_t nf = 0;
+    nin = (size_t)d->embed[2] * d->axis_neuron;
+    for (int l = 0; l < 3; ++l) { nf += nin * d->fit[l] + d->fit[l]; nin = d->fit[l]; }
+    nf += nin + 1;
+    return (size_t)d->n_types * d->n_types * ne + (size_t)d->n_types * nf;
+}
+
+int pimd_set_state_dev(pimd_ctx* ctx, const double* x_dev, const double* p_dev) {
+    if (!ctx || !x_dev || !p_dev) return fail(ctx, PIMD_EINVAL, "null argument");
+    int rc;
+    if ((rc = alloc_base(ctx))) return rc;
+    const size_t PN3 = (size_t)ctx->P * ctx->N * 3;
+    CK(cudaMemcpyAsync(ctx->x, x_dev, PN3 * 8, cudaMemcpyDeviceToDevice, ctx->stream));
+    launch_to_nm_velocity(ctx->P, ctx->N, p_dev, ctx->mass_atom, ctx->vt, ctx->stream);
+    CK(cudaGetLastError());
+    ctx->have_state = true;
+    ctx->step = 0;
+    return refresh(ctx);
+}
+
+int pimd_set_state(pimd_ctx* ctx, const double* x, const double* p) {
+    if (!ctx || !x || !p) return fail(ctx, PIMD_EINVAL, "null argument");
+    int rc;
+    if ((rc = alloc_base(ctx))) return rc;
+    const size_t PN3 = (size_t)ctx->P * ctx->N * 3;
+    CK(cudaMemcpyAsync(ctx->scratch_a, x, PN3 * 8, cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaMemcpyAsync(ctx->scratch_b, p, PN3 * 8, cudaMemcpyHostToDevice, ctx->stream));
+    return pimd_set_state_dev(ctx, ctx->scratch_a, ctx->scratch_b);
+}
+
+int pimd_set_model_harmonic(pimd_ctx* ctx, double k_spring) {
+    if (!ctx) return PIMD_EINVAL;
+    int rc;
+    if ((rc = alloc_base(ctx))) return rc;
+    ctx->model_kind = 1;
+    ctx->k_spring = k_spring;
+    return refresh(ctx);
+}
+
+int pimd_set_model(pimd_ctx* ctx, const pimd_model_desc* d, const double* w, size_t n_weights) {
+    if (!ctx || !d || !w) return fail(ctx, PIMD_EINVAL, "null argument");
+    if (d->n_types != ctx->ntypes) return fail(ctx, PIMD_EINVAL, "model n_types differs from the context's");
+    if (n_weights != pimd_model_n_weights(d)) return fail(ctx, PIMD_EINVAL, "weight vector has the wrong length");
+    if (!(d->embed[0] == 25 && d->embed[1] == 50 && d->embed[2] == 100 && d->axis_neuron == 16))
+        return fail(ctx, PIMD_EINVAL, "this build instantiates the embedding kernels for [25,50,100], axis 16 only");
+    if (!(d->fit[0] == d->fit[1] && d->fit[1] == d->fit[2] && d->fit[0] % 16 == 0))
+        return fail(ctx, PIMD_EINVAL, "fitting widths must be equal and a multiple of 16");
+    if (!(d->rcut > d->rcut_smth && d->rcut_smth >= 0)) return fail(ctx, PIMD_EINVAL, "need rcut > rcut_smth >= 0");
+    if (ctx->model.set) return fail(ctx, PIMD_EINVAL, "the model of a context can be set once");
+    int rc;
+    if ((rc = alloc_base(ctx))) return rc;
+    Model& m = ctx->model;
+    m.d = *d;
+    const int nt = d->n_types;
+    m.nsel = 0;
+    for (int t = 0; t < nt; ++t) { m.seloff[t] = m.nsel; m.nsel += d->sel[t]; }
+    for (int t = nt; t <= PIMD_MAX_TYPES; ++t) m.seloff[t] = m.nsel;
+    m.E1 = d->embed[0]; m.E2 = d->embed[1]; m.M1 = d->embed[2]; m.M2 = d->axis_neuron; m.NF = d->fit[0];
+    m.ND = m.M1 * m.M2;
+    cell_grid(ctx->box, d->rcut, m.ncell, m.R, &m.ncells);
+    for (int a = 0; a < 3; ++a)
+        if (m.R[a] > 3) return fail(ctx, PIMD_EINVAL, "box shorter than rcut/3 is not supported");
+    const size_t PN = (size_t)ctx->P * ctx->N;
+    if (ctx->N >= (1 << 23)) return fail(ctx, PIMD_EINVAL, "at most 2^23 - 1 atoms");
+
+    // ---- embedding weights, packed per (t_i, t_j): W1, b1, W2^T (k padded), b2, W3^T, b3 ----
+    const int E1 = m.E1, E2 = m.E2, M1 = m.M1;
+    const int E1p = (E1 + 3) / 4 * 4, E2p = (E2 + 3) / 4 * 4;
+    const int oW1 = 0, ob1 = E1p, oW2t = 2 * E1p, ob2 = oW2t + E2 * E1p, oW3t = ob2 + E2p, ob3 = oW3t + M1 * E2p;
+    m.emb_stride = (ob3 + M1 + 3) / 4 * 4;
+    std::vector<float> ew((size_t)nt * nt * m.emb_stride, 0.f);
+    size_t pos = 0;
+    for (int ti = 0; ti < nt; ++ti)
+        for (int tj = 0; tj < nt; ++tj) {
+            float* o = ew.data() + (size_t)(ti * nt + tj) * m.emb_stride;
+            for (int k = 0; k < E1; ++k) o[oW1 + k] = (float)w[pos + k];
+            pos += E1;
+            for (int k = 0; k < E1; ++k) o[ob1 + k] = (float)w[pos + k];
+            pos += E1;
+            for (int k = 0; k < E1; ++k)
+                for (int n = 0; n < E2; ++n) o[oW2t + n * E1p + k] = (float)w[pos + (size_t)k * E2 + n];
+            pos += (size_t)E1 * E2;
+            for (int n = 0; n < E2; ++n) o[ob2 + n] = (float)w[pos + n];
+            pos += E2;
+            for (int k = 0; k < E2; ++k)
+                for (int n = 0; n < M1; ++n) o[oW3t + n * E2p + k] = (float)w[pos + (size_t)k * M1 + n];
+            pos += (size_t)E2 * M1;
+            for (int n = 0; n < M1; ++n) o[ob3 + n] = (float)w[pos + n];
+            pos += M1;
+        }
+    if ((rc = arena_alloc(ctx, &m.emb_w, ew.size()))) return rc;
+    CK(cudaMemcpyAsync(m.emb_w, ew.data(), ew.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
+
+    // ---- fitting weights: W, W^T, b per layer ----
+    std::vector<std::vector<float>> keep;
+    for (int t = 0; t < nt; ++t) {
+        int nin = m.ND;
+        for (int l = 0; l < 4; ++l) {
+            const int nout = (l < 3) ? m.NF : 1;
+            std::vector<float> W((size_t)nin * nout), WT((size_t)nin * nout), b(nout);
+            for (int k = 0; k < nin; ++k)
+                for (int n = 0; n < nout; ++n) {
+                    const float v = (float)w[pos + (size_t)k * nout + n];
+                    W[(size_t)k * nout + n] = v;
+                    WT[(size_t)n * nin + k] = v;
+                }
+            pos += (size_t)nin * nout;
+            for (int n = 0; n < nout; ++n) b[n] = (float)w[pos + n];
+            pos += nout;
+            if ((rc = arena_alloc(ctx, &m.fit_w[t][l], W.size()))) return rc;
+            if ((rc = arena_alloc(ctx, &m.fit_wT[t][l], WT.size()))) return rc;
+            if ((rc = arena_alloc(ctx, &m.fit_b[t][l], b.size()))) return rc;
+            CK(cudaMemcpyAsync(m.fit_w[t][l], W.data(), W.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
+            CK(cudaMemcpyAsync(m.fit_wT[t][l], WT.data(), WT.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
+            CK(cudaMemcpyAsync(m.fit_b[t][l], b.data(), b.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
+            keep.push_back(std::move(W)); keep.push_back(std::move(WT)); keep.push_back(std::move(b));
+            nin = nout;
+        }
+    }
+
+    // ---- centre order [type][bead][atom of type] ----
+    std::vector<int> cen(PN), rowof(PN);
+    {
+        size_t r = 0;
+        for (int t = 0; t < nt; ++t) {
+            m.type_row0[t] = (int)r;
+            int cnt = 0;
+            for (int k = 0; k < ctx->P; ++k)
+                for (int i = 0; i < ctx->N; ++i)
+                    if (ctx->types[i] == t) { cen[r] = k * ctx->N + i; rowof[(size_t)k * ctx->N + i] = (int)r; ++r; if (k == 0) ++cnt; }
+            m.n_of_type[t] = cnt;
+        }
+        for (int t = nt; t <= PIMD_MAX_TYPES; ++t) m.type_row0[t] = (int)r;
+    }
+    if ((rc = arena_alloc(ctx, &m.cen_idx, PN))) return rc;
+    if ((rc = arena_alloc(ctx, &m.row_of, PN))) return rc;
+    CK(cudaMemcpyAsync(m.cen_idx, cen.data(), PN * 4, cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaMemcpyAsync(m.row_of, rowof.data(), PN * 4, cudaMemcpyHostToDevice, ctx->stream));
+
+    // ---- work buffers ----
+    if ((rc = arena_alloc(ctx, &m.cell_count, (size_t)ctx->P * (m.ncells + 1)))) return rc;
+    if ((rc = arena_alloc(ctx, &m.cell_start, (size_t)ctx->P * (m.ncells + 1)))) return rc;
+    if ((rc = arena_alloc(ctx, &m.cell_fill, (size_t)ctx->P * (m.ncells + 1)))) return rc;
+    if ((rc = arena_alloc(ctx, &m.cell_id, PN))) return rc;
+    if ((rc = arena_alloc(ctx, &m.cell_tmp, PN))) return rc;
+    if ((rc = arena_alloc(ctx, &m.wtmp, PN * 3))) return rc;
+    if ((rc = arena_alloc(ctx, &m.wsorted, PN))) return rc;
+    if ((rc = arena_alloc(ctx, &m.ncount, PN * nt))) return rc;
+    if ((rc = arena_alloc(ctx, &m.slotA, PN * m.nsel))) return rc;
+    if ((rc = arena_alloc(ctx, &m.slotB, PN * m.nsel))) return rc;
+    if ((rc = arena_alloc(ctx, &m.overflow, (size_t)1))) return rc;
+    if ((rc = arena_alloc(ctx, &m.Tm, PN * m.M1 * 4))) return rc;
+    if ((rc = arena_alloc(ctx, &m.dTm, PN * m.M1 * 4))) return rc;
+    if ((rc = arena_alloc(ctx, &m.D, PN * m.ND))) return rc;
+    if ((rc = arena_alloc(ctx, &m.dD, PN * m.ND))) return rc;
+    float** fb[7] = {&m.Y1, &m.T2, &m.Y2, &m.T3, &m.Y3, &m.G1, &m.G2};
+    for (int q = 0; q < 7; ++q)
+        if ((rc = arena_alloc(ctx, fb[q], PN * m.NF))) return rc;
+    CK(cudaMemsetAsync(m.overflow, 0, sizeof(int), ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));     // host staging vectors go out of scope below
+    m.set = true;
+    ctx->model_kind = 2;
+    return refresh(ctx);
+}
+
+int pimd_step(pimd_ctx* ctx, int64_t n_steps) {
+    if (!ctx) return PIMD_EINVAL;
+    if (n_steps < 0) return fail(ctx, PIMD_EINVAL, "n_steps < 0");
+    if (!ctx->have_state) return fail(ctx, PIMD_ENOSTATE, "pimd_set_state has not been called");
+    if (ctx->model_kind == 0) return fail(ctx, PIMD_ENOMODEL, "no force model set");
+    if (n_steps == 0) return PIMD_OK;
+    const int hist = (int)std::min<int64_t>(n_steps, kEstCap);
+    const int64_t first_hist = n_steps - hist;            // steps before this index are not recorded
+    CK(cudaMemsetAsync(ctx->est, 0, sizeof(double) * (size_t)hist * kEstWidth, ctx->stream));
+    double* cur = ctx->est + (size_t)kEstCap * kEstWidth;
+    double* scratch = ctx->est + (size_t)(kEstCap + 1) * kEstWidth;
+    float ms_acc[6] = {0, 0, 0, 0, 0, 0};
+    for (int64_t s = 0; s <= n_steps; ++s) {
+        // launch s: closes step s-1 (B, estimators) and opens step s (B A O A)
+        int flags = 0;
+        double* slot = scratch;
+        if (s > 0) {
+            flags |= I_BCLOSE | I_EST;
+            slot = (s - 1 >= first_hist) ? ctx->est + (size_t)(s - 1 - first_hist) * kEstWidth : scratch;
+        }
+        if (s < n_steps) flags |= I_START;
+        IntegratorArgs a;
+        fill_integrator_args(ctx, a, flags, ctx->step + s, slot);
+        rec(ctx, 0);
+        launch_integrator(ctx->P, a, ctx->mc, ctx->stream);
+        if (s < n_steps) {
+            int rc = eval_forces(ctx);
+            if (rc) return rc;
+            if (ctx->profiling) {
+                rec(ctx, 6);
+                cudaEventSynchronize(ctx->ev[6]);
+                float t;
+                if (ctx->model_kind == 2) {
+                    cudaEventElapsedTime(&t, ctx->ev[0], ctx->ev[1]); ms_acc[0] += t;
+                    for (int q = 1; q < 5; ++q) { cudaEventElapsedTime(&t, ctx->ev[q], ctx->ev[q + 1]); ms_acc[q] += t; }
+                }
+            }
+        }
+    }
+    CK(cudaGetLastError());
+    // the last slot is also "current"
+    CK(cudaMemcpyAsync(cur, ctx->est + (size_t)(hist - 1) * kEstWidth, sizeof(double) * kEstWidth,
+                       cudaMemcpyDeviceToDevice, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    ctx->step += n_steps;
+    ctx->est_hist_n = hist;
+    ctx->est_hist_first_step = ctx->step - hist + 1;
+    if (ctx->profiling) {
+        for (int q = 0; q < 6; ++q) ctx->phase_ms[q] = ms_acc[q] / (double)n_steps;
+        ctx->phase_steps = n_steps;
+    }
+    return check_overflow(ctx);
+}
+
+static int copy_out(pimd_ctx* ctx, const void* dev, void* host, size_t bytes) {
+    if (!ctx || !host) return fail(ctx, PIMD_EINVAL, "null argument");
+    if (!ctx->have_state) return fail(ctx, PIMD_ENOSTATE, "pimd_set_state has not been called");
+    CK(cudaMemcpyAsync(host, dev, bytes, cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return PIMD_OK;
+}
+
+int pimd_get_positions(pimd_ctx* ctx, double* x) {
+    return copy_out(ctx, ctx ? ctx->x : nullptr, x, ctx ? (size_t)ctx->P * ctx->N * 24 : 0);
+}
+int pimd_get_momenta(pimd_ctx* ctx, double* p) {
+    if (!ctx || !p) return fail(ctx, PIMD_EINVAL, "null argument");
+    if (!ctx->have_state) return fail(ctx, PIMD_ENOSTATE, "pimd_set_state has not been called");
+    launch_from_nm_momenta(ctx->P, ctx->N, ctx->vt, ctx->mass_atom, ctx->scratch_a, ctx->stream);
+    return copy_out(ctx, ctx->scratch_a, p, (size_t)ctx->P * ctx->N * 24);
+}
+int pimd_get_forces(pimd_ctx* ctx, double* f) {
+    return copy_out(ctx, ctx ? ctx->f : nullptr, f, ctx ? (size_t)ctx->P * ctx->N * 24 : 0);
+}
+int pimd_get_virial(pimd_ctx* ctx, double* xi) {
+    return copy_out(ctx, ctx ? ctx->Xi : nullptr, xi, ctx ? (size_t)ctx->P * 72 : 0);
+}
+int pimd_get_energies(pimd_ctx* ctx, double* U) {
+    return copy_out(ctx, ctx ? ctx->U : nullptr, U, ctx ? (size_t)ctx->P * 8 : 0);
+}
+int pimd_get_atom_energies(pimd_ctx* ctx, double* E) {
+    return copy_out(ctx, ctx ? ctx->Eatom : nullptr, E, ctx ? (size_t)ctx->P * ctx->N * 8 : 0);
+}
+
+int pimd_get_estimators(pimd_ctx* ctx, pimd_estimators* e) {
+    if (!ctx || !e) return fail(ctx, PIMD_EINVAL, "null argument");
+    if (!ctx->have_state) return fail(ctx, PIMD_ENOSTATE, "pimd_set_state has not been called");
+    if (ctx->model_kind == 0) return fail(ctx, PIMD_ENOMODEL, "no force model set");
+    double raw[kEstWidth];
+    int rc = copy_out(ctx, ctx->est + (size_t)kEstCap * kEstWidth, raw, sizeof(raw));
+    if (rc) return rc;
+    finalize_est(ctx, raw, ctx->step, e);
+    return PIMD_OK;
+}
+
+int pimd_get_estimator_history(pimd_ctx* ctx, pimd_estimators* e, int cap) {
+    if (!ctx || !e || cap < 0) return fail(ctx, PIMD_EINVAL, "bad argument");
+    const int n = std::min(cap, ctx->est_hist_n);
+    if (n == 0) return 0;
+    std::vector<double> raw((size_t)ctx->est_hist_n * kEstWidth);
+    int rc = copy_out(ctx, ctx->est, raw.data(), raw.size() * 8);
+    if (rc) return rc;
+    const int skip = ctx->est_hist_n - n;
+    for (int q = 0; q < n; ++q)
+        finalize_est(ctx, raw.data() + (size_t)(skip + q) * kEstWidth, ctx->est_hist_first_step + skip + q, e + q);
+    return n;
+}
+
+int pimd_get_positions_dev(pimd_ctx* ctx, double* x_dev) {
+    if (!ctx || !x_dev) return fail(ctx, PIMD_EINVAL, "null argument");
+    if (!ctx->have_state) return fail(ctx, PIMD_ENOSTATE, "pimd_set_state has not been called");
+    CK(cudaMemcpyAsync(x_dev, ctx->x, (size_t)ctx->P * ctx->N * 24, cudaMemcpyDeviceToDevice, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return PIMD_OK;
+}
+int pimd_get_forces_dev(pimd_ctx* ctx, double* f_dev) {
+    if (!ctx || !f_dev) return fail(ctx, PIMD_EINVAL, "null argument");
+    if (!ctx->have_state) return fail(ctx, PIMD_ENOSTATE, "pimd_set_state has not been called");
+    CK(cudaMemcpyAsync(f_dev, ctx->f, (size_t)ctx->P * ctx->N * 24, cudaMemcpyDeviceToDevice, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return PIMD_OK;
+}
+
+int64_t pimd_get_neighbors(pimd_ctx* ctx, int bead, int32_t* count, int32_t* jout, int8_t* shift, size_t cap) {
+    if (!ctx || !count || !jout || !shift) return fail(ctx, PIMD_EINVAL, "null argument");
+    if (ctx->model_kind != 2 || !ctx->have_state) return fail(ctx, PIMD_ENOMODEL, "needs an se_e2_a model and a state");
+    if (bead < 0 || bead >= ctx->P) return fail(ctx, PIMD_EINVAL, "bead out of range");
+    const Model& m = ctx->model;
+    const int N = ctx->N, nt = ctx->ntypes;
+    std::vector<int> cnt((size_t)N * nt);
+    std::vector<NeighSlotB> sb((size_t)N * m.nsel);
+    CK(cudaMemcpyAsync(cnt.data(), m.ncount + (size_t)bead * N * nt, cnt.size() * 4, cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaMemcpyAsync(sb.data(), m.slotB + (size_t)bead * N * m.nsel, sb.size() * sizeof(NeighSlotB),
+                       cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    size_t total = 0;
+    struct Row { int t, j, nx, ny, nz; };
+    std::vector<Row> rows;
+    for (int i = 0; i < N; ++i) {
+        rows.clear();
+        for (int t = 0; t < nt; ++t)
+            for (int q = 0; q < cnt[(size_t)i * nt + t]; ++q) {
+                const uint32_t jc = sb[(size_t)i * m.nsel + m.seloff[t] + q].jcode;
+                const uint32_t code = jc >> 23;
+                rows.push_back({t, (int)(jc & 0x7fffffu), (int)(code & 7) - 3, (int)((code >> 3) & 7) - 3, (int)((code >> 6) & 7) - 3});
+            }
+        std::sort(rows.begin(), rows.end(), [](const Row& a, const Row& b) {
+            if (a.t != b.t) return a.t < b.t;
+            if (a.j != b.j) return a.j < b.j;
+            if (a.nx != b.nx) return a.nx < b.nx;
+            if (a.ny != b.ny) return a.ny < b.ny;
+            return a.nz < b.nz;
+        });
+        count[i] = (int32_t)rows.size();
+        if (total + rows.size() > cap) return fail(ctx, PIMD_EINVAL, "cap too small for the neighbour rows");
+        for (const Row& r : rows) {
+            jout[total] = r.j;
+            shift[3 * total] = (int8_t)r.nx; shift[3 * total + 1] = (int8_t)r.ny; shift[3 * total + 2] = (int8_t)r.nz;
+            ++total;
+        }
+    }
+    return (int64_t)total;
+}
+
+int pimd_debug_noise(pimd_ctx* ctx, int64_t step, int n, const int32_t* idx, uint32_t* words, double* eta) {
+    if (!ctx || n <= 0 || !idx || !words || !eta) return fail(ctx, PIMD_EINVAL, "bad argument");
+    int32_t* d_idx = nullptr; uint32_t* d_w = nullptr; double* d_e = nullptr;
+    CK(cudaMalloc(&d_idx, sizeof(int32_t) * 3 * n));
+    CK(cudaMalloc(&d_w, sizeof(uint32_t) * 4 * n));
+    CK(cudaMalloc(&d_e, sizeof(double) * n));
+    CK(cudaMemcpyAsync(d_idx, idx, sizeof(int32_t) * 3 * n, cudaMemcpyHostToDevice, ctx->stream));
+    launch_debug_noise(ctx->seed, (uint64_t)step, n, d_idx, d_w, d_e, ctx->stream);
+    CK(cudaMemcpyAsync(words, d_w, sizeof(uint32_t) * 4 * n, cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaMemcpyAsync(eta, d_e, sizeof(double) * n, cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    cudaFree(d_idx); cudaFree(d_w); cudaFree(d_e);
+    return PIMD_OK;
+}
+
+int pimd_time_kernel(pimd_ctx* ctx, int kind, int reps, double* ms) {
+    if (!ctx || !ms || reps <= 0) return fail(ctx, PIMD_EINVAL, "bad argument");
+    if (!ctx->have_state || ctx->model_kind == 0) return fail(ctx, PIMD_ENOSTATE, "needs a state and a model");
+    if (kind != 0) return fail(ctx, PIMD_EINVAL, "unknown kernel kind");
+    IntegratorArgs a;
+    double* scratch = ctx->est + (size_t)(kEstCap + 1) * kEstWidth;
+    fill_integrator_args(ctx, a, I_BCLOSE | I_EST | I_START, ctx->step, scratch);
+    a.x_out = ctx->scratch_a; a.vt_out = ctx->scratch_b;          // state is not advanced
+    for (int w = 0; w < 3; ++w) launch_integrator(ctx->P, a, ctx->mc, ctx->stream);
+    CK(cudaEventRecord(ctx->ev[6], ctx->stream));
+    for (int r = 0; r < reps; ++r) launch_integrator(ctx->P, a, ctx->mc, ctx->stream);
+    CK(cudaEventRecord(ctx->ev[7], ctx->stream));
+    CK(cudaEventSynchronize(ctx->ev[7]));
+    CK(cudaGetLastError());
+    float t = 0;
+    CK(cudaEventElapsedTime(&t, ctx->ev[6], ctx->ev[7]));
+    *ms = (double)t / reps;
+    return PIMD_OK;
+}
+
+int pimd_set_profiling(pimd_ctx* ctx, int on) {
+    if (!ctx) return PIMD_EINVAL;
+    ctx->profiling = on != 0;
+    return PIMD_OK;
+}
+int pimd_get_phase_ms(pimd_ctx* ctx, double ms[6]) {
+    if (!ctx || !ms) return PIMD_EINVAL;
+    for (int q = 0; q < 6; ++q) ms[q] = ctx->phase_ms[q];
+    return PIMD_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,119 @@
+// common.cuh -- internal declarations shared by the translation units of libpimd_b200.
+// Product code (CUDA, sm_100a).  Shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include <string>
+#include <vector>
+#include "../../include/pimd.h"
+
+namespace pimd {
+
+// Physical constants: PAPER.md:L458 prints h and mvv2e; k_B is DESIGN R-9.
+constexpr double kHPlanck = 4.135667403e-3;                       // eV ps
+constexpr double kHbar    = kHPlanck / (2.0 * 3.14159265358979323846);
+constexpr double kMvv2e   = 1.0364269e-4;                         // eV / ((g/mol)(A/ps)^2)
+constexpr double kKB      = 8.617333262e-5;                       // eV / K
+
+constexpr int kMaxBeads = 64;
+constexpr int kEstCap   = 4096;     // estimator history slots per pimd_step call
+constexpr int kEstWidth = 4;        // K_ring, S_ring, sum x.f - x~0.f~0, U_sum
+
+// integrator launch flags
+enum : int { I_BCLOSE = 1, I_EST = 2, I_START = 4 };
+
+// Per-mode constants of the A and O steps (DESIGN R-3, R-5), kernel parameter.
+struct ModeConsts {
+    double cosA[kMaxBeads];      // cos(omega_k dt/2)
+    double sinA_w[kMaxBeads];    // sin(omega_k dt/2)/omega_k   (k = 0: dt/2)
+    double msinA_w[kMaxBeads];   // -omega_k sin(omega_k dt/2)
+    double c1[kMaxBeads];        // exp(-dt gamma_k)
+    double c2[kMaxBeads];        // sqrt(1 - c1^2)
+    double om2[kMaxBeads];       // omega_k^2
+};
+
+struct IntegratorArgs {
+    int      N;                  // atoms
+    int      n_dof;              // 3N
+    int      flags;
+    int      thermostat;         // 0 = NVE (O step skipped)
+    double   half_dt_mvv;        // (dt/2)/mvv2e : multiply by f~/m to get the B kick
+    double   PkT_mvv;            // P k_B T / mvv2e : sigma_i^2 = this / m_i
+    uint32_t seed_lo, seed_hi, step_lo, step_hi;
+    const double* x_in;  const double* vt_in;  const double* f;
+    double*  x_out;      double* vt_out;
+    const double* mass;          // [N] per atom
+    const double* U;             // [P] bead energies (for the U_sum slot), may be null
+    double*  est;                // [kEstWidth] accumulators of this step's slot, may be null
+};
+
+void launch_integrator(int P, const IntegratorArgs& a, const ModeConsts& mc, cudaStream_t s);
+void launch_to_nm_velocity(int P, int N, const double* p_cart, const double* mass, double* vt, cudaStream_t s);
+void launch_from_nm_momenta(int P, int N, const double* vt, const double* mass, double* p_cart, cudaStream_t s);
+void launch_harmonic(int P, int N, double k_spring, const double* x, double* f, double* U, double* Xi,
+                     double* Eatom, cudaStream_t s);
+void launch_debug_noise(uint64_t seed, uint64_t step, int n, const int32_t* idx_dev, uint32_t* words_dev,
+                        double* eta_dev, cudaStream_t s);
+
+// ---------------------------------------------------------------------------------------------
+// se_e2_a model on the device
+// ---------------------------------------------------------------------------------------------
+struct NeighSlotA { float dx, dy, dz, s; };          // environment row pieces (FP32 from FP64)
+struct NeighSlotB { float ds, rinv; uint32_t jcode; float pad; };   // jcode = j | shiftcode << 23
+
+struct Model {
+    bool     set = false;
+    pimd_model_desc d;
+    int      nsel = 0;
+    int      seloff[PIMD_MAX_TYPES + 1];
+    int      M1 = 0, M2 = 0, E1 = 0, E2 = 0, NF = 0, ND = 0;   // 100,16,25,50,240,1600
+    // geometry of the cell grid
+    int      ncell[3]; int ncells = 0; int R[3];
+    // device buffers
+    float*   emb_w = nullptr;          // [ntypes*ntypes][emb_stride] packed for the kernels
+    int      emb_stride = 0;
+    float*   fit_w[PIMD_MAX_TYPES][4];     // W[in][out] row-major
+    float*   fit_wT[PIMD_MAX_TYPES][4];    // W^T: [out][in] row-major (backward GEMM operand)
+    float*   fit_b[PIMD_MAX_TYPES][4];
+    int*     cen_idx = nullptr;        // [PN] sorted row -> k*N+i  (order [type][bead][atom of type])
+    int*     row_of = nullptr;         // [PN] inverse
+    int      type_row0[PIMD_MAX_TYPES + 1];   // first sorted row of each centre type
+    int      n_of_type[PIMD_MAX_TYPES];
+    int*     cell_count = nullptr;     // [P][ncells+1]
+    int*     cell_start = nullptr;     // [P][ncells+1]
+    int*     cell_fill = nullptr;      // [P][ncells]
+    int*     cell_id = nullptr;        // [PN]
+    int*     cell_tmp = nullptr;       // [PN] unsorted members
+    double*  wtmp = nullptr;           // [PN][3] wrapped coordinates
+    double4* wsorted = nullptr;        // [PN] cell-ordered {w, idx|type}
+    int*     ncount = nullptr;         // [PN][ntypes]
+    NeighSlotA* slotA = nullptr;       // [PN][nsel]
+    NeighSlotB* slotB = nullptr;
+    int*     overflow = nullptr;       // device flag
+    float*   Tm = nullptr;             // [PN rows][M1][4]
+    float*   dTm = nullptr;
+    float*   D = nullptr;              // [rows][ND]
+    float*   dD = nullptr;
+    float*   Y1 = nullptr, *T2 = nullptr, *Y2 = nullptr, *T3 = nullptr, *Y3 = nullptr;   // [rows][NF]
+    float*   G1 = nullptr, *G2 = nullptr;   // backward scratch [rows][NF]
+};
+
+struct ForceArgs {
+    int P, N, ntypes;
+    double box[3];
+    const double* x;      // [P][N][3]
+    const int* types;     // [N]
+    double* f;            // [P][N][3]
+    double* U;            // [P]
+    double* Xi;           // [P][9]
+    double* Eatom;        // [P][N]
+};
+
+void neighbor_build(Model& m, const ForceArgs& a, cudaStream_t s);
+void embedding_forward(Model& m, const ForceArgs& a, int n_sms, cudaStream_t s);
+void fitting_forward_backward(Model& m, const ForceArgs& a, cudaStream_t s);
+void embedding_backward(Model& m, const ForceArgs& a, int n_sms, cudaStream_t s);
+size_t embedding_smem_bytes(const Model& m, int ntypes);
+
+}  // namespace pimd

@@ -1,0 +1,326 @@
+// integrator.cu -- fused FP64 BAOAB / PILE-L kernel I1 (SURVEY 8(a) rows I-a .. I-i).
+//
+// One THREAD owns all P beads of one atom-dimension (with the [P][N][3] layout a
+// warp then reads 32 consecutive doubles of every bead row -> fully coalesced, and the three
+// normal-mode transforms of PAPER.md:L192/L208 become in-register real FFTs with no shuffles).
+//   closing B of step t (needs f~ = M f)
+//   estimators K, S, sum x.f (Appendix A)  -> block reduction -> one atomicAdd per block
+//   opening B, A(dt/2), O(dt), A(dt/2) of step t+1   L165, L190-192, Eq. D1-D2
+//   x = M^T x~                                       Eq. B3
+// reads x, v~, f once and writes x, v~ once: 40 B per bead-atom-dim.
+#include "common.cuh"
+#include "philox.cuh"
+
+namespace pimd {
+
+// cos(2 pi q / 64), q = 0..16
+__device__ constexpr double kCos64[17] = {
+    1.0, 0.99518472667219693, 0.98078528040323043, 0.95694033573220882, 0.92387953251128674,
+    0.88192126434835505, 0.83146961230254524, 0.77301045336273699, 0.70710678118654757,
+    0.63439328416364549, 0.55557023301960229, 0.47139673682599781, 0.38268343236508984,
+    0.29028467725446233, 0.19509032201612833, 0.09801714032956077, 0.0};
+
+// Real-input FFT X_m = sum_j in[j*stride] exp(-2 pi i m j / n), m = 0..n/2, by decimation in time on
+// the half-complex representation.  re[0..n/2], im[1..n/2-1] are written; im[0], im[n/2] are never
+// written nor read (they are zero).  All indices are compile-time so everything stays in registers.
+template <int n, int stride>
+struct RFFT {
+    __device__ __forceinline__ static void run(const double* in, double* re, double* im) {
+        double er[n / 4 + 1], ei[n / 4 + 1], orr[n / 4 + 1], oi[n / 4 + 1];
+        RFFT<n / 2, stride * 2>::run(in, er, ei);
+        RFFT<n / 2, stride * 2>::run(in + stride, orr, oi);
+        re[0] = er[0] + orr[0];
+        re[n / 2] = er[0] - orr[0];
+        re[n / 4] = er[n / 4];
+        im[n / 4] = -orr[n / 4];
+#pragma unroll
+        for (int m = 1; m < n / 4; ++m) {
+            const double wr = kCos64[m * (64 / n)];
+            const double wi = -kCos64[16 - m * (64 / n)];
+            const double tr = wr * orr[m] - wi * oi[m];
+            const double ti = wr * oi[m] + wi * orr[m];
+            re[m] = er[m] + tr;
+            im[m] = ei[m] + ti;
+            re[n / 2 - m] = er[m] - tr;
+            im[n / 2 - m] = ti - ei[m];
+        }
+    }
+};
+template <int stride>
+struct RFFT<2, stride> {
+    __device__ __forceinline__ static void run(const double* in, double* re, double* im) {
+        re[0] = in[0] + in[stride];
+        re[1] = in[0] - in[stride];
+    }
+};
+template <int stride>
+struct RFFT<1, stride> {
+    __device__ __forceinline__ static void run(const double* in, double* re, double* im) { re[0] = in[0]; }
+};
+
+// a~ = M a with M of Eq. B1 (reading DESIGN R-2), in place.
+template <int P>
+__device__ __forceinline__ void nm_forward(double* a) {
+    if constexpr (P == 1) return;
+    double re[P / 2 + 1], im[P / 2 + 1];
+    RFFT<P, 1>::run(a, re, im);
+    const double s0 = rsqrt((double)P), s1 = sqrt(2.0 / (double)P);
+    a[0] = re[0] * s0;
+    a[P / 2] = re[P / 2] * s0;
+#pragma unroll
+    for (int k = 1; k < P / 2; ++k) {
+        a[k] = s1 * re[k];
+        a[P - k] = s1 * im[k];
+    }
+}
+
+// a = M^T a~ (Eq. B3), in place: the transposed real-DFT matrix equals a forward real FFT of the
+// sequence z with z_k + z_{P-k} = sqrt(2/P) a~_k, z_k - z_{P-k} = sqrt(2/P) a~_{P-k}; x_j = Re Z_j + Im Z_j.
+template <int P>
+__device__ __forceinline__ void nm_inverse(double* a) {
+    if constexpr (P == 1) return;
+    double z[P];
+    const double s0 = rsqrt((double)P), s2 = rsqrt(2.0 * (double)P);
+    z[0] = a[0] * s0;
+    z[P / 2] = a[P / 2] * s0;
+#pragma unroll
+    for (int k = 1; k < P / 2; ++k) {
+        z[k] = (a[k] + a[P - k]) * s2;
+        z[P - k] = (a[k] - a[P - k]) * s2;
+    }
+    double re[P / 2 + 1], im[P / 2 + 1];
+    RFFT<P, 1>::run(z, re, im);
+    a[0] = re[0];
+    a[P / 2] = re[P / 2];
+#pragma unroll
+    for (int j = 1; j < P / 2; ++j) {
+        a[j] = re[j] + im[j];
+        a[P - j] = re[j] - im[j];
+    }
+}
+
+constexpr int kIntThreads = 128;
+
+template <int P>
+__global__ void __launch_bounds__(kIntThreads)
+integrator_kernel(const __grid_constant__ IntegratorArgs a, const __grid_constant__ ModeConsts mc) {
+    extern __shared__ double eta_s[];                  // [P][kIntThreads] thermostat normals
+    const int e = blockIdx.x * kIntThreads + threadIdx.x;
+    const bool live = e < a.n_dof;
+    const int ec = live ? e : a.n_dof - 1;             // dead threads shadow the last dof, never store
+    const int i = ec / 3, alpha = ec - 3 * i;
+    const bool start = (a.flags & I_START) != 0;
+    const bool thermo = start && a.thermostat;
+
+    // ---- O-step normals first (few live registers; rolled loop keeps one copy of log/cos) ----
+    if (thermo) {
+#pragma unroll 1
+        for (int k = 0; k < P; ++k) {
+            eta_s[k * kIntThreads + threadIdx.x] =
+                philox_normal(a.seed_lo, a.seed_hi, a.step_lo, a.step_hi, (uint32_t)i, (uint32_t)(4 * k + alpha));
+        }
+    }
+
+    const double m = a.mass[i];
+    const size_t stride = (size_t)a.n_dof;
+    double xt[P], ft[P];
+    double xf = 0.0;
+#pragma unroll
+    for (int k = 0; k < P; ++k) {
+        xt[k] = a.x_in[k * stride + ec];
+        ft[k] = a.f[k * stride + ec];
+    }
+#pragma unroll
+    for (int k = 0; k < P; ++k) xf += xt[k] * ft[k];
+    nm_forward<P>(ft);                                  // f~ = M f      (L192, third transform)
+    nm_forward<P>(xt);                                  // x~ = M x      (first transform)
+
+    const double kick = a.half_dt_mvv / m;              // (dt/2)/(m mvv2e)
+    const double sigma = sqrt(a.PkT_mvv / m);           // sqrt(P k_B T/(m mvv2e))  (Eq. D2)
+    // A9 in normal-mode form: sum_k (r_k - r_c).F_k = sum_{k>=1} x~_k f~_k = sum_j x_j f_j - x~_0 f~_0
+    const double cv_term = xf - xt[0] * ft[0];
+    double accK = 0.0, accS = 0.0;
+#pragma unroll
+    for (int k = 0; k < P; ++k) {
+        double v = a.vt_in[k * stride + ec];
+        if (a.flags & I_BCLOSE) v += kick * ft[k];      // closing B of the previous step
+        if (a.flags & I_EST) {
+            accK += v * v;                               // A1: 1/2 m v~^2
+            accS += mc.om2[k] * xt[k] * xt[k];           // A3: 1/2 m omega_k^2 x~^2
+        }
+        if (start) {
+            v += kick * ft[k];                           // B(dt/2)
+            const double x = xt[k];
+            const double xn = mc.cosA[k] * x + mc.sinA_w[k] * v;    // A(dt/2): exact rotation (R-5)
+            double vn = mc.msinA_w[k] * x + mc.cosA[k] * v;
+            if (thermo) vn = mc.c1[k] * vn + mc.c2[k] * sigma * eta_s[k * kIntThreads + threadIdx.x];   // O(dt)
+            xt[k] = mc.cosA[k] * xn + mc.sinA_w[k] * vn;            // A(dt/2)
+            v = mc.msinA_w[k] * xn + mc.cosA[k] * vn;
+        }
+        if (live && (a.flags & (I_BCLOSE | I_START))) a.vt_out[k * stride + ec] = v;
+    }
+
+    if (a.flags & I_EST) {
+        double r0 = live ? 0.5 * m * accK * kMvv2e : 0.0;     // K_ring share
+        double r1 = live ? 0.5 * m * accS * kMvv2e : 0.0;     // S_ring share
+        double r2 = live ? cv_term : 0.0;
+        __shared__ double red[3][kIntThreads / 32];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            r0 += __shfl_xor_sync(0xffffffffu, r0, o);
+            r1 += __shfl_xor_sync(0xffffffffu, r1, o);
+            r2 += __shfl_xor_sync(0xffffffffu, r2, o);
+        }
+        const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+        if (l == 0) { red[0][w] = r0; red[1][w] = r1; red[2][w] = r2; }
+        __syncthreads();
+        if (threadIdx.x < 3) {
+            double t = 0.0;
+#pragma unroll
+            for (int q = 0; q < kIntThreads / 32; ++q) t += red[threadIdx.x][q];
+            atomicAdd(a.est + threadIdx.x, t);
+        }
+        if (blockIdx.x == 0 && threadIdx.x == 3 && a.U != nullptr) {
+            double u = 0.0;
+            for (int k = 0; k < P; ++k) u += a.U[k];
+            atomicAdd(a.est + 3, u);
+        }
+    }
+
+    if (start) {
+        nm_inverse<P>(xt);                              // x = M^T x~    (second transform)
+        if (live) {
+#pragma unroll
+            for (int k = 0; k < P; ++k) a.x_out[k * stride + ec] = xt[k];
+        }
+    }
+}
+
+template <int P>
+static void launch_int_t(const IntegratorArgs& a, const ModeConsts& mc, cudaStream_t s) {
+    const int blocks = (a.n_dof + kIntThreads - 1) / kIntThreads;
+    const size_t smem = (size_t)P * kIntThreads * sizeof(double);
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaFuncSetAttribute(integrator_kernel<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        attr_done = true;
+    }
+    integrator_kernel<P><<<blocks, kIntThreads, smem, s>>>(a, mc);
+}
+
+void launch_integrator(int P, const IntegratorArgs& a, const ModeConsts& mc, cudaStream_t s) {
+    switch (P) {
+        case 1: launch_int_t<1>(a, mc, s); break;
+        case 2: launch_int_t<2>(a, mc, s); break;
+        case 4: launch_int_t<4>(a, mc, s); break;
+        case 8: launch_int_t<8>(a, mc, s); break;
+        case 16: launch_int_t<16>(a, mc, s); break;
+        case 32: launch_int_t<32>(a, mc, s); break;
+        case 64: launch_int_t<64>(a, mc, s); break;
+        default: break;
+    }
+}
+
+// v~ = M (p/m)  and  p = m M^T v~  (API momenta are Cartesian; PAPER.md:L104 keeps v in NM form inside)
+template <int P, bool kForward>
+__global__ void nm_convert_kernel(int n_dof, const double* __restrict__ in, const double* __restrict__ mass,
+                                  double* __restrict__ out) {
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n_dof) return;
+    const double m = mass[e / 3];
+    double a[P];
+#pragma unroll
+    for (int k = 0; k < P; ++k) a[k] = in[(size_t)k * n_dof + e];
+    if constexpr (kForward) {
+#pragma unroll
+        for (int k = 0; k < P; ++k) a[k] = a[k] / m;
+        nm_forward<P>(a);
+    } else {
+        nm_inverse<P>(a);
+#pragma unroll
+        for (int k = 0; k < P; ++k) a[k] = a[k] * m;
+    }
+#pragma unroll
+    for (int k = 0; k < P; ++k) out[(size_t)k * n_dof + e] = a[k];
+}
+
+template <bool kForward>
+static void launch_conv(int P, int N, const double* in, const double* mass, double* out, cudaStream_t s) {
+    const int n_dof = 3 * N, th = 128, bl = (n_dof + th - 1) / th;
+    switch (P) {
+        case 1: nm_convert_kernel<1, kForward><<<bl, th, 0, s>>>(n_dof, in, mass, out); break;
+        case 2: nm_convert_kernel<2, kForward><<<bl, th, 0, s>>>(n_dof, in, mass, out); break;
+        case 4: nm_convert_kernel<4, kForward><<<bl, th, 0, s>>>(n_dof, in, mass, out); break;
+        case 8: nm_convert_kernel<8, kForward><<<bl, th, 0, s>>>(n_dof, in, mass, out); break;
+        case 16: nm_convert_kernel<16, kForward><<<bl, th, 0, s>>>(n_dof, in, mass, out); break;
+        case 32: nm_convert_kernel<32, kForward><<<bl, th, 0, s>>>(n_dof, in, mass, out); break;
+        case 64: nm_convert_kernel<64, kForward><<<bl, th, 0, s>>>(n_dof, in, mass, out); break;
+        default: break;
+    }
+}
+void launch_to_nm_velocity(int P, int N, const double* p, const double* mass, double* vt, cudaStream_t s) {
+    launch_conv<true>(P, N, p, mass, vt, s);
+}
+void launch_from_nm_momenta(int P, int N, const double* vt, const double* mass, double* p, cudaStream_t s) {
+    launch_conv<false>(P, N, vt, mass, p, s);
+}
+
+// Test model U = sum_i 1/2 k |r_i|^2 (FP64): f = -k x, U^(k), Xi_ab = sum_i x_a f_b.
+__global__ void harmonic_kernel(int N, double ks, const double* __restrict__ x, double* __restrict__ f,
+                                double* __restrict__ U, double* __restrict__ Xi, double* __restrict__ Eatom) {
+    const int k = blockIdx.y;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    double acc[10];
+#pragma unroll
+    for (int q = 0; q < 10; ++q) acc[q] = 0.0;
+    if (i < N) {
+        const size_t o = ((size_t)k * N + i) * 3;
+        const double r[3] = {x[o], x[o + 1], x[o + 2]};
+        double fr[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { fr[c] = -ks * r[c]; f[o + c] = fr[c]; }
+        acc[9] = 0.5 * ks * (r[0] * r[0] + r[1] * r[1] + r[2] * r[2]);
+        Eatom[(size_t)k * N + i] = acc[9];
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+#pragma unroll
+            for (int d = 0; d < 3; ++d) acc[3 * c + d] = r[c] * fr[d];
+    }
+#pragma unroll
+    for (int q = 0; q < 10; ++q)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) acc[q] += __shfl_xor_sync(0xffffffffu, acc[q], o);
+    if ((threadIdx.x & 31) == 0) {
+#pragma unroll
+        for (int q = 0; q < 9; ++q) atomicAdd(Xi + k * 9 + q, acc[q]);
+        atomicAdd(U + k, acc[9]);
+    }
+}
+
+void launch_harmonic(int P, int N, double ks, const double* x, double* f, double* U, double* Xi, double* Eatom,
+                     cudaStream_t s) {
+    cudaMemsetAsync(U, 0, sizeof(double) * P, s);
+    cudaMemsetAsync(Xi, 0, sizeof(double) * 9 * P, s);
+    dim3 grid((N + 127) / 128, P);
+    harmonic_kernel<<<grid, 128, 0, s>>>(N, ks, x, f, U, Xi, Eatom);
+}
+
+__global__ void debug_noise_kernel(uint32_t seed_lo, uint32_t seed_hi, uint32_t step_lo, uint32_t step_hi, int n,
+                                   const int32_t* __restrict__ idx, uint32_t* __restrict__ words,
+                                   double* __restrict__ eta) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n) return;
+    const uint32_t k = idx[3 * t], i = idx[3 * t + 1], al = idx[3 * t + 2];
+    uint32_t w[4];
+    philox4x32_10(step_lo, step_hi, i, 4u * k + al, seed_lo, seed_hi, w);
+    for (int q = 0; q < 4; ++q) words[4 * t + q] = w[q];
+    eta[t] = philox_normal(seed_lo, seed_hi, step_lo, step_hi, i, 4u * k + al);
+}
+
+void launch_debug_noise(uint64_t seed, uint64_t step, int n, const int32_t* idx, uint32_t* words, double* eta,
+                        cudaStream_t s) {
+    debug_noise_kernel<<<(n + 127) / 128, 128, 0, s>>>((uint32_t)seed, (uint32_t)(seed >> 32), (uint32_t)step,
+                                                        (uint32_t)(step >> 32), n, idx, words, eta);
+}
+
+}  // namespace pimd

@@ -1,0 +1,239 @@
+// neighbor.cu -- F1 (wrap + per-bead cell binning) and F2 (neighbour rows + smooth environment matrix)
+// of SURVEY 8(a).  Geometry is FP64 with the exact operation order of DESIGN R-11 (no FMA
+// contraction: __dmul_rn / __dadd_rn), so the neighbour sets are bit-identical to the oracle's.
+//   w = x - L*floor(x/L)                                   PAPER.md:L200-202 (wrap before the force call)
+//   rows (j, n): d = (w_j - w_i) + n*L,  (dx^2+dy^2)+dz^2 < rc^2 strictly, (j,n) != (i,0)    R-11
+//   s(r) smooth switch, R_row = (s, s d/r)                 R-12
+// All images are enumerated (box may be shorter than 2 r_c: configs[0]), by walking cell offsets
+// -R..R with R = ceil(r_c / cell width) and recording the lattice shift n of every wrap-around.
+#include "common.cuh"
+
+namespace pimd {
+
+struct GridGeom {
+    double L[3];
+    double inv_w[3];     // ncell / L
+    int nc[3];
+    int R[3];
+    int ncells;
+};
+
+__global__ void wrap_bin_kernel(int P, int N, GridGeom g, const double* __restrict__ x, double* __restrict__ wtmp,
+                                int* __restrict__ cell_id, int* __restrict__ cell_count) {
+    const int ba = blockIdx.x * blockDim.x + threadIdx.x;
+    if (ba >= P * N) return;
+    const int k = ba / N;
+    int c[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const double xv = x[(size_t)ba * 3 + a];
+        const double w = __dsub_rn(xv, __dmul_rn(g.L[a], floor(__ddiv_rn(xv, g.L[a]))));
+        wtmp[(size_t)ba * 3 + a] = w;
+        int ci = (int)floor(w * g.inv_w[a]);
+        ci = ci < 0 ? 0 : (ci >= g.nc[a] ? g.nc[a] - 1 : ci);
+        c[a] = ci;
+    }
+    const int cid = (c[2] * g.nc[1] + c[1]) * g.nc[0] + c[0];
+    cell_id[ba] = cid;
+    atomicAdd(cell_count + (size_t)k * (g.ncells + 1) + cid, 1);
+}
+
+// exclusive scan of the cell counts of one bead (one block per bead)
+__global__ void cell_scan_kernel(int ncells, const int* __restrict__ cell_count, int* __restrict__ cell_start) {
+    __shared__ int warp_tot[32];
+    __shared__ int carry;
+    const int k = blockIdx.x;
+    const int* cnt = cell_count + (size_t)k * (ncells + 1);
+    int* start = cell_start + (size_t)k * (ncells + 1);
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    for (int base = 0; base < ncells + 1; base += blockDim.x) {
+        const int idx = base + threadIdx.x;
+        const int v = (idx < ncells) ? cnt[idx] : 0;
+        int incl = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, incl, o);
+            if ((threadIdx.x & 31) >= o) incl += t;
+        }
+        if ((threadIdx.x & 31) == 31) warp_tot[threadIdx.x >> 5] = incl;
+        __syncthreads();
+        int woff = 0;
+        for (int q = 0; q < (int)(threadIdx.x >> 5); ++q) woff += warp_tot[q];
+        const int excl = carry + woff + incl - v;
+        if (idx < ncells + 1) start[idx] = excl;
+        __syncthreads();
+        if (threadIdx.x == blockDim.x - 1) carry = excl + v;
+        __syncthreads();
+    }
+}
+
+__global__ void cell_fill_kernel(int P, int N, int ncells, const int* __restrict__ cell_id,
+                                 const int* __restrict__ cell_start, int* __restrict__ cell_fill,
+                                 int* __restrict__ cell_tmp) {
+    const int ba = blockIdx.x * blockDim.x + threadIdx.x;
+    if (ba >= P * N) return;
+    const int k = ba / N, i = ba - k * N;
+    const int cid = cell_id[ba];
+    const int slot = atomicAdd(cell_fill + (size_t)k * ncells + cid, 1);
+    cell_tmp[(size_t)k * N + cell_start[(size_t)k * (ncells + 1) + cid] + slot] = i;
+}
+
+// Deterministic order inside every cell: rank each member by its atom index (one warp per cell).
+__global__ void cell_sort_kernel(int P, int N, int ncells, const int* __restrict__ cell_start,
+                                 const int* __restrict__ cell_tmp, const double* __restrict__ wtmp,
+                                 const int* __restrict__ types, double4* __restrict__ wsorted) {
+    const int wid = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (wid >= P * ncells) return;
+    const int k = wid / ncells, c = wid - k * ncells;
+    const int s0 = cell_start[(size_t)k * (ncells + 1) + c], s1 = cell_start[(size_t)k * (ncells + 1) + c + 1];
+    const int* mem = cell_tmp + (size_t)k * N;
+    for (int q = s0 + lane; q < s1; q += 32) {
+        const int me = mem[q];
+        int rank = 0;
+        for (int t = s0; t < s1; ++t) rank += (mem[t] < me) ? 1 : 0;
+        const size_t ba = (size_t)k * N + me;
+        double4 o;
+        o.x = wtmp[ba * 3]; o.y = wtmp[ba * 3 + 1]; o.z = wtmp[ba * 3 + 2];
+        o.w = __longlong_as_double(((long long)types[me] << 32) | (long long)me);
+        wsorted[(size_t)k * N + s0 + rank] = o;
+    }
+}
+
+struct EnvConsts {
+    double rc, rs, rc2, inv_range;   // inv_range = 1/(rc - rs)
+    int ntypes;
+    int sel[PIMD_MAX_TYPES];
+    int seloff[PIMD_MAX_TYPES + 1];
+    int nsel;
+};
+
+// One warp per centre bead-atom.
+__global__ void __launch_bounds__(128)
+neighbor_env_kernel(int P, int N, GridGeom g, EnvConsts ec, const double* __restrict__ wtmp,
+                    const int* __restrict__ cell_id, const int* __restrict__ cell_start,
+                    const double4* __restrict__ wsorted, int* __restrict__ ncount, NeighSlotA* __restrict__ slotA,
+                    NeighSlotB* __restrict__ slotB, int* __restrict__ overflow) {
+    const int ba = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (ba >= P * N) return;
+    const int k = ba / N, i = ba - k * N;
+    const double wi[3] = {wtmp[(size_t)ba * 3], wtmp[(size_t)ba * 3 + 1], wtmp[(size_t)ba * 3 + 2]};
+    const int cid = cell_id[ba];
+    const int c0 = cid % g.nc[0], c1 = (cid / g.nc[0]) % g.nc[1], c2 = cid / (g.nc[0] * g.nc[1]);
+    const int* cs = cell_start + (size_t)k * (g.ncells + 1);
+    const double4* ws = wsorted + (size_t)k * N;
+    int cnt[PIMD_MAX_TYPES];
+#pragma unroll
+    for (int t = 0; t < PIMD_MAX_TYPES; ++t) cnt[t] = 0;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    const size_t slot0 = (size_t)ba * ec.nsel;
+
+    for (int oz = -g.R[2]; oz <= g.R[2]; ++oz) {
+        const int zz = c2 + oz;
+        const int nz = (zz >= 0) ? zz / g.nc[2] : -((-zz + g.nc[2] - 1) / g.nc[2]);
+        const int cz = zz - nz * g.nc[2];
+        for (int oy = -g.R[1]; oy <= g.R[1]; ++oy) {
+            const int yy = c1 + oy;
+            const int ny = (yy >= 0) ? yy / g.nc[1] : -((-yy + g.nc[1] - 1) / g.nc[1]);
+            const int cy = yy - ny * g.nc[1];
+            for (int ox = -g.R[0]; ox <= g.R[0]; ++ox) {
+                const int xx = c0 + ox;
+                const int nx = (xx >= 0) ? xx / g.nc[0] : -((-xx + g.nc[0] - 1) / g.nc[0]);
+                const int cx = xx - nx * g.nc[0];
+                const int cc = (cz * g.nc[1] + cy) * g.nc[0] + cx;
+                const int s0 = cs[cc], s1 = cs[cc + 1];
+                const double sh[3] = {__dmul_rn((double)nx, g.L[0]), __dmul_rn((double)ny, g.L[1]),
+                                      __dmul_rn((double)nz, g.L[2])};
+                const bool zero_shift = (nx == 0) && (ny == 0) && (nz == 0);
+                for (int q0 = s0; q0 < s1; q0 += 32) {
+                    const int q = q0 + lane;
+                    bool keep = false;
+                    int tj = 0, j = 0;
+                    double d[3] = {0, 0, 0}, r2 = 1.0;
+                    if (q < s1) {
+                        const double4 wj = ws[q];
+                        const long long pk = __double_as_longlong(wj.w);
+                        j = (int)(pk & 0xffffffffll);
+                        tj = (int)(pk >> 32);
+                        d[0] = __dadd_rn(__dsub_rn(wj.x, wi[0]), sh[0]);
+                        d[1] = __dadd_rn(__dsub_rn(wj.y, wi[1]), sh[1]);
+                        d[2] = __dadd_rn(__dsub_rn(wj.z, wi[2]), sh[2]);
+                        r2 = __dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2]));
+                        keep = (r2 < ec.rc2) && !(zero_shift && j == i);
+                    }
+                    int slot = -1;
+                    for (int t = 0; t < ec.ntypes; ++t) {
+                        const unsigned mk = __ballot_sync(0xffffffffu, keep && tj == t);
+                        if (keep && tj == t) slot = cnt[t] + __popc(mk & lt_mask);
+                        cnt[t] += __popc(mk);
+                    }
+                    if (keep) {
+                        if (slot >= ec.sel[tj]) {
+                            atomicMax(overflow, 1);
+                        } else {
+                            // environment row in FP64 (R-12), stored FP32
+                            const double r = sqrt(r2);
+                            double sw = 1.0, dsw = 0.0;
+                            if (r >= ec.rs) {
+                                const double u = (r - ec.rs) * ec.inv_range;
+                                sw = u * u * u * (-6.0 * u * u + 15.0 * u - 10.0) + 1.0;
+                                dsw = -30.0 * u * u * (u - 1.0) * (u - 1.0) * ec.inv_range;
+                            }
+                            const double rinv = 1.0 / r;
+                            const double s = sw * rinv;
+                            const double ds = dsw * rinv - sw * rinv * rinv;
+                            NeighSlotA A;
+                            A.dx = (float)d[0]; A.dy = (float)d[1]; A.dz = (float)d[2]; A.s = (float)s;
+                            NeighSlotB B;
+                            B.ds = (float)ds; B.rinv = (float)rinv;
+                            const uint32_t code = (uint32_t)(nx + 3) | ((uint32_t)(ny + 3) << 3) | ((uint32_t)(nz + 3) << 6);
+                            B.jcode = (uint32_t)j | (code << 23);
+                            B.pad = 0.f;
+                            const size_t o = slot0 + ec.seloff[tj] + slot;
+                            slotA[o] = A;
+                            slotB[o] = B;
+                        }
+                    }
+                }
+            }
+        }
+    }
+    if (lane == 0) {
+        for (int t = 0; t < ec.ntypes; ++t) ncount[(size_t)ba * ec.ntypes + t] = min(cnt[t], ec.sel[t]);
+    }
+}
+
+void neighbor_build(Model& m, const ForceArgs& a, cudaStream_t s) {
+    const int PN = a.P * a.N;
+    GridGeom g;
+    for (int c = 0; c < 3; ++c) {
+        g.L[c] = a.box[c];
+        g.nc[c] = m.ncell[c];
+        g.R[c] = m.R[c];
+        g.inv_w[c] = (double)m.ncell[c] / a.box[c];
+    }
+    g.ncells = m.ncells;
+    EnvConsts ec;
+    ec.rc = m.d.rcut; ec.rs = m.d.rcut_smth; ec.rc2 = m.d.rcut * m.d.rcut;
+    ec.inv_range = 1.0 / (m.d.rcut - m.d.rcut_smth);
+    ec.ntypes = a.ntypes; ec.nsel = m.nsel;
+    for (int t = 0; t < PIMD_MAX_TYPES; ++t) { ec.sel[t] = t < a.ntypes ? m.d.sel[t] : 0; ec.seloff[t] = m.seloff[t]; }
+    ec.seloff[PIMD_MAX_TYPES] = m.nsel;
+
+    cudaMemsetAsync(m.cell_count, 0, sizeof(int) * (size_t)a.P * (m.ncells + 1), s);
+    cudaMemsetAsync(m.cell_fill, 0, sizeof(int) * (size_t)a.P * m.ncells, s);
+    const int th = 128;
+    wrap_bin_kernel<<<(PN + th - 1) / th, th, 0, s>>>(a.P, a.N, g, a.x, m.wtmp, m.cell_id, m.cell_count);
+    cell_scan_kernel<<<a.P, 256, 0, s>>>(m.ncells, m.cell_count, m.cell_start);
+    cell_fill_kernel<<<(PN + th - 1) / th, th, 0, s>>>(a.P, a.N, m.ncells, m.cell_id, m.cell_start, m.cell_fill,
+                                                       m.cell_tmp);
+    const long long nw = (long long)a.P * m.ncells;
+    cell_sort_kernel<<<(unsigned)((nw * 32 + th - 1) / th), th, 0, s>>>(a.P, a.N, m.ncells, m.cell_start, m.cell_tmp,
+                                                                        m.wtmp, a.types, m.wsorted);
+    neighbor_env_kernel<<<(unsigned)(((long long)PN * 32 + th - 1) / th), th, 0, s>>>(
+        a.P, a.N, g, ec, m.wtmp, m.cell_id, m.cell_start, m.wsorted, m.ncount, m.slotA, m.slotB, m.overflow);
+}
+
+}  // namespace pimd

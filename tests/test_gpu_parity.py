@@ -1,0 +1,263 @@
+"""GPU parity: the CUDA path (through the C ABI) against the oracle, element by element, on the same
+seeded inputs.  Tolerances are north_star's: neighbour lists and Philox words bit-exact; force error
+<= 1e-4 relative per component with the bead's F_rms as floor (DESIGN R-17); energy/atom <= 1e-6 eV;
+x, p <= 1e-10 relative (max-norm) after one step with identical FP64 forces (harmonic model) and <= 1e-6
+after 10 steps."""
+import numpy as np
+import pytest
+
+import workloads
+from oracle import philox, se_e2_a
+from oracle.pimd import OraclePIMD
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def pk():
+    import paper_2602_13553_b200 as pk
+    pk.lib()
+    return pk
+
+
+def _rel(a, b):
+    return np.abs(a - b).max() / np.abs(b).max()
+
+
+def _random_system(N, P, seed, T=300.0):
+    rng = np.random.default_rng(seed)
+    types = rng.integers(0, 2, size=N).astype(np.int32)
+    masses = np.array([15.9994, 1.008])
+    x = rng.standard_normal((P, N, 3)) * 0.3
+    p = rng.standard_normal((P, N, 3)) * np.sqrt(masses[types])[None, :, None] * 5.0
+    return types, masses, x, p
+
+
+# ---------------------------------------------------------------------------------------------
+# Philox stream: bit-exact
+# ---------------------------------------------------------------------------------------------
+def test_philox_words_bit_exact_and_normals(pk):
+    sim = pk.PIMD(np.zeros(4, np.int32), [1.0], [10.0] * 3, 4, 300.0, 1e-3, 1.0, seed=0x123456789ABCDEF)
+    rng = np.random.default_rng(3)
+    idx = np.stack([rng.integers(0, 64, 4096), rng.integers(0, 1 << 22, 4096), rng.integers(0, 3, 4096)], axis=1)
+    for step in (0, 1, 12345678901):
+        words, eta = pk.pimd_debug_noise(sim.ctx, step, idx)
+        w = philox.words_for(0x123456789ABCDEF, step, idx[:, 0], idx[:, 1], idx[:, 2])
+        for q in range(4):
+            assert np.array_equal(words[:, q].astype(np.uint64), w[q])
+        ref = philox.normal(0x123456789ABCDEF, step, idx[:, 0], idx[:, 1], idx[:, 2])
+        assert np.abs(eta - ref).max() < 1e-13
+    sim.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# integrator alone (harmonic model: identical FP64 forces on both sides)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("P", [1, 2, 4, 8, 16, 32, 64])
+@pytest.mark.parametrize("gamma", [0.0, 5.0])
+def test_integrator_parity_harmonic(pk, P, gamma):
+    N = 37                                           # 111 dofs: ragged tail of the 128-thread blocks
+    types, masses, x, p = _random_system(N, P, seed=10 + P)
+    ks = 2.5
+    sim = pk.PIMD(types, masses, [30.0] * 3, P, 300.0, 0.25e-3, gamma, seed=99)
+    sim.set_state(x, p)
+    sim.set_model_harmonic(ks)
+    orc = OraclePIMD(types, masses, [30.0] * 3, P, 300.0, 0.25e-3, gamma, seed=99)
+    orc.set_state(x, p)
+    orc.set_model_harmonic(ks)
+    assert _rel(sim.momenta(), orc.momenta()) < 1e-13          # p -> v~ -> p round trip
+    e0, o0 = sim.estimators(), orc.estimators()
+    for key in ("K_PR", "K_CV", "H", "K_ring", "S_ring", "U_sum", "T_ring"):
+        assert abs(e0[key] - o0[key]) <= 1e-11 * max(1.0, abs(o0[key])), key
+    sim.step(1)
+    orc.step(1)
+    assert _rel(sim.positions(), orc.positions()) < 1e-10
+    assert _rel(sim.momenta(), orc.momenta()) < 1e-10
+    sim.step(9)
+    orc.step(9)
+    assert _rel(sim.positions(), orc.positions()) < 1e-6
+    assert _rel(sim.momenta(), orc.momenta()) < 1e-6
+    assert _rel(sim.positions(), orc.positions()) < 1e-11      # what the FP64 kernel actually reaches
+    e, o = sim.estimators(), orc.estimators()
+    assert e["step"] == 10
+    for key in ("K_PR", "K_CV", "H", "K_ring", "S_ring", "U_sum", "T_ring"):
+        assert abs(e[key] - o[key]) <= 1e-9 * max(1.0, abs(o[key])), key
+    assert _rel(sim.forces(), orc.forces()) < 1e-11
+    assert np.abs(sim.virial() - orc.virial()).max() < 1e-9 * np.abs(orc.virial()).max()
+    sim.close()
+
+
+def test_estimator_history_every_step(pk):
+    N, P = 50, 8
+    types, masses, x, p = _random_system(N, P, seed=5)
+    sim = pk.PIMD(types, masses, [30.0] * 3, P, 300.0, 0.25e-3, 2.0, seed=1)
+    sim.set_state(x, p)
+    sim.set_model_harmonic(1.0)
+    orc = OraclePIMD(types, masses, [30.0] * 3, P, 300.0, 0.25e-3, 2.0, seed=1)
+    orc.set_state(x, p)
+    orc.set_model_harmonic(1.0)
+    sim.step(5)
+    hist = sim.estimator_history()
+    assert [h["step"] for h in hist] == [1, 2, 3, 4, 5]
+    for h in hist:
+        orc.step(1)
+        o = orc.estimators()
+        for key in ("K_PR", "K_CV", "H"):
+            assert abs(h[key] - o[key]) <= 1e-9 * max(1.0, abs(o[key]))
+    sim.close()
+
+
+def test_split_calls_equal_one_call_bitwise(pk):
+    """step(3)+step(4) == step(7): the noise is keyed by the absolute step counter (R-10)."""
+    N, P = 20, 4
+    types, masses, x, p = _random_system(N, P, seed=8)
+    outs = []
+    for plan in ((7,), (3, 4)):
+        sim = pk.PIMD(types, masses, [30.0] * 3, P, 300.0, 0.5e-3, 1.0, seed=4)
+        sim.set_state(x, p)
+        sim.set_model_harmonic(3.0)
+        for n in plan:
+            sim.step(n)
+        outs.append((sim.positions(), sim.momenta()))
+        sim.close()
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+
+
+# ---------------------------------------------------------------------------------------------
+# neighbour lists: bit-exact sets
+# ---------------------------------------------------------------------------------------------
+def _oracle_rows(x, types, box, rcut):
+    ri, rj, rn, _ = se_e2_a.neighbours_bruteforce(x, box, rcut)
+    tj = np.asarray(types)[rj]
+    order = np.lexsort((rn[:, 2], rn[:, 1], rn[:, 0], rj, tj, ri))
+    return ri[order], rj[order], rn[order]
+
+
+@pytest.mark.parametrize("cfg_idx,beads", [(0, (0, 1, 2, 3)), (1, (0, 31))])
+def test_neighbour_lists_bit_exact(pk, cfg_idx, beads):
+    cfg, wb, desc, w = workloads.make_config(cfg_idx)
+    sim = pk.PIMD(wb["types"], wb["masses"], wb["box"], cfg["P"], cfg["T"], cfg["dt"], cfg["gamma"], seed=0,
+                  model_desc=desc)
+    sim.set_state(wb["x"], wb["p"])
+    sim.set_model(w)
+    for k in beads:
+        count, j, shift = sim.neighbors(k)
+        ri, rj, rn = _oracle_rows(wb["x"][k], wb["types"], wb["box"], desc["rcut"])
+        assert np.array_equal(count, np.bincount(ri, minlength=sim.N))
+        assert np.array_equal(j, rj)
+        assert np.array_equal(shift.astype(np.int64), rn)
+    if cfg_idx == 0:
+        assert (np.abs(shift).max() == 1)             # multi-image rows exist (box < 2 r_c)
+    sim.close()
+
+
+def test_neighbours_atoms_far_outside_the_box_and_on_faces(pk):
+    """Unwrapped coordinates several boxes away, and atoms exactly on the faces x = 0, x = L."""
+    cfg, wb, desc, w = workloads.make_config(0)
+    x = wb["x"].copy()
+    L = wb["box"][0]
+    x[:, 0::7] += np.array([3 * L, -2 * L, 5 * L])
+    x[0, 3] = [0.0, L, 2 * L]
+    x[0, 4] = [-1e-300, 0.5 * L, 0.25 * L]
+    sim = pk.PIMD(wb["types"], wb["masses"], wb["box"], cfg["P"], cfg["T"], cfg["dt"], cfg["gamma"], seed=0,
+                  model_desc=desc)
+    sim.set_state(x, wb["p"])
+    sim.set_model(w)
+    count, j, shift = sim.neighbors(0)
+    ri, rj, rn = _oracle_rows(x[0], wb["types"], wb["box"], desc["rcut"])
+    assert np.array_equal(count, np.bincount(ri, minlength=sim.N))
+    assert np.array_equal(j, rj) and np.array_equal(shift.astype(np.int64), rn)
+    sim.close()
+
+
+def test_sel_overflow_is_an_error(pk):
+    cfg, wb, desc, w = workloads.make_config(0)
+    small = dict(desc, sel=[8, 16])
+    sim = pk.PIMD(wb["types"], wb["masses"], wb["box"], cfg["P"], cfg["T"], cfg["dt"], cfg["gamma"], seed=0,
+                  model_desc=small)
+    sim.set_state(wb["x"], wb["p"])
+    with pytest.raises(pk.PimdError) as ei:
+        sim.set_model(w, small)
+    assert ei.value.code == pk.PIMD_ESEL_OVERFLOW
+    sim.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# force model
+# ---------------------------------------------------------------------------------------------
+def _force_checks(f, fo, U, Uo, Xi, Xio, E, Eo, N):
+    frms = np.sqrt((fo ** 2).mean(axis=(1, 2), keepdims=True))
+    err = np.abs(f - fo) / np.maximum(np.abs(fo), frms)
+    assert err.max() <= 1e-4, "force error %.3e" % err.max()
+    assert np.abs(U - Uo).max() / N <= 1e-6
+    assert np.abs(E - Eo).max() <= 1e-6
+    assert np.abs(Xi - Xio).max() <= 1e-4 * np.abs(Xio).max()
+    return err.max()
+
+
+@pytest.mark.parametrize("scale", [1.0, 1.0e3])
+def test_force_energy_virial_parity_config0(pk, scale):
+    cfg, wb, desc, _ = workloads.make_config(0)
+    w = workloads.model_weights(desc, cfg["weight_seed"], last_layer_scale=scale)
+    sim = pk.PIMD(wb["types"], wb["masses"], wb["box"], cfg["P"], cfg["T"], cfg["dt"], cfg["gamma"], seed=0,
+                  model_desc=desc)
+    sim.set_state(wb["x"], wb["p"])
+    sim.set_model(w)
+    model = se_e2_a.Model(desc, w)
+    P, N = cfg["P"], sim.N
+    fo, Uo, Xio, Eo = np.zeros((P, N, 3)), np.zeros(P), np.zeros((P, 3, 3)), np.zeros((P, N))
+    for k in range(P):
+        E, F, Xi = se_e2_a.energy_forces(wb["x"][k], wb["types"], wb["box"], model)
+        fo[k], Uo[k], Xio[k], Eo[k] = F, E.sum(), Xi, E
+    tol_scale = scale                                   # energies scale with the last layer
+    f, U, Xi, E = sim.forces(), sim.energies(), sim.virial(), sim.atom_energies()
+    frms = np.sqrt((fo ** 2).mean(axis=(1, 2), keepdims=True))
+    err = np.abs(f - fo) / np.maximum(np.abs(fo), frms)
+    assert err.max() <= 1e-4, "force error %.3e" % err.max()
+    assert np.abs(U - Uo).max() / N <= 1e-6 * tol_scale
+    assert np.abs(E - Eo).max() <= 1e-6 * tol_scale
+    assert np.abs(Xi - Xio).max() <= 1e-4 * np.abs(Xio).max()
+    assert np.abs(f.sum(axis=1)).max() <= 1e-6 * np.abs(fo).max() * N ** 0.5     # Newton's third law
+    sim.close()
+
+
+def test_force_parity_config1_sampled_beads(pk):
+    cfg, wb, desc, w = workloads.make_config(1)
+    sim = pk.PIMD(wb["types"], wb["masses"], wb["box"], cfg["P"], cfg["T"], cfg["dt"], cfg["gamma"], seed=0,
+                  model_desc=desc)
+    sim.set_state(wb["x"], wb["p"])
+    sim.set_model(w)
+    model = se_e2_a.Model(desc, w)
+    f, U, Xi, E = sim.forces(), sim.energies(), sim.virial(), sim.atom_energies()
+    for k in (0, 13, 31):
+        Eo, Fo, Xio = se_e2_a.energy_forces(wb["x"][k], wb["types"], wb["box"], model)
+        _force_checks(f[k:k + 1], Fo[None], U[k:k + 1], np.array([Eo.sum()]), Xi[k:k + 1], Xio[None], E[k], Eo, sim.N)
+    sim.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# the whole step, configs[0]
+# ---------------------------------------------------------------------------------------------
+def test_full_step_parity_config0(pk):
+    cfg, wb, desc, w = workloads.make_config(0)
+    args = (wb["types"], wb["masses"], wb["box"], cfg["P"], cfg["T"], cfg["dt"], cfg["gamma"])
+    sim = pk.PIMD(*args, seed=11, model_desc=desc)
+    sim.set_state(wb["x"], wb["p"])
+    sim.set_model(w)
+    orc = OraclePIMD(*args, seed=11)
+    orc.set_state(wb["x"], wb["p"])
+    orc.set_model(desc, w)
+    sim.step(1)
+    orc.step(1)
+    ex1, ep1 = _rel(sim.positions(), orc.positions()), _rel(sim.momenta(), orc.momenta())
+    assert ex1 <= 1e-10 and ep1 <= 1e-10, (ex1, ep1)
+    sim.step(9)
+    orc.step(9)
+    ex, ep = _rel(sim.positions(), orc.positions()), _rel(sim.momenta(), orc.momenta())
+    assert ex <= 1e-6 and ep <= 1e-6, (ex, ep)
+    e, o = sim.estimators(), orc.estimators()
+    assert e["step"] == 10
+    assert abs(e["K_CV"] - o["K_CV"]) <= 1e-6 * abs(o["K_CV"])
+    assert abs(e["K_PR"] - o["K_PR"]) <= 1e-6 * abs(o["K_PR"])
+    assert abs(e["H"] - o["H"]) <= 1e-6 * sim.N * sim.P
+    sim.close()
