@@ -1,0 +1,339 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the PIMD/Langevin BAOAB hot path (BASELINE.json metric).
+
+    python bench.py --gpus 1 --steps 20 --warmup 5            # this build (CUDA, sm_100a)
+    python bench.py --impl reference --steps 3 --warmup 1     # the oracle on the host cores
+    torchrun ... bench.py --gpus N ...                        # N independent replicas ("replicas only")
+
+A step = one pass of the whole hot path (integrator + force evaluation) over the
+configs[2] workload (1536 atoms x 32 beads, seeded synthetic water box, random-init se_e2_a weights).
+Prints ONE JSON line (rank 0).  See DESIGN.md section 8 for the roofline arithmetic.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import workloads  # noqa: E402
+
+METRIC = "bead-atom-steps/s"
+FP32_LANES_PER_SM = 128          # B200_PROFILING.md / blackwell guide: 4 SMSP x 32 FMA lanes
+
+
+def _peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        d = json.load(open(path))
+        return dict(hbm=d["hbm_gbs"], bf16=d["bf16_tflops"], bf16_sustained=d.get("bf16_tflops_sustained"),
+                    sm_max_mhz=d.get("sm_max_mhz", 1965.0), src="measured")
+    return dict(hbm=6650.0, bf16=1590.0, bf16_sustained=1400.0, sm_max_mhz=1965.0, src="fallback")
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons sampled DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.samples, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.samples.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, smax, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        rows = [l for (t, l) in self.samples if t0 <= t <= t1] or [l for (_, l) in self.samples[-3:]]
+        for line in rows:
+            p = [q.strip() for q in line.split(",")]
+            try:
+                sm.append(float(p[0]))
+                smax = float(p[1])
+            except Exception:
+                continue
+            for n, v in zip(names, p[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": smax, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def _dist():
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+# ------------------------------------------------------------------------------------------------
+# reference arm = the oracle, as it stands, on the host cores
+# ------------------------------------------------------------------------------------------------
+def _oracle_sample(cfg_idx, steps, warmup, n_sample_beads):
+    """Times `steps` oracle steps (after `warmup`) on a bounded sample: the full box and ring of configs
+    [cfg_idx] with the FORCE evaluation restricted to `n_sample_beads` beads (OraclePIMD.only_beads);
+    units = sampled beads x atoms x steps."""
+    from oracle.pimd import OraclePIMD
+    cfg, wb, desc, w = workloads.make_config(cfg_idx)
+    orc = OraclePIMD(wb["types"], wb["masses"], wb["box"], cfg["P"], cfg["T"], cfg["dt"], cfg["gamma"], seed=0)
+    orc.only_beads = list(range(n_sample_beads))
+    orc.set_state(wb["x"], wb["p"])
+    orc.set_model(desc, w)
+    for _ in range(warmup):
+        orc.step(1)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        orc.step(1)
+    dt = time.perf_counter() - t0
+    units = n_sample_beads * orc.N * steps
+    return units / dt, dt / steps, orc.N, cfg["P"]
+
+
+def _cores_used():
+    try:
+        import threadpoolctl
+        n = max([p["num_threads"] for p in threadpoolctl.threadpool_info()] + [1])
+        return int(n)
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def run_reference(args):
+    rank, world, _ = _dist()
+    if rank != 0:
+        return 0
+    value, s_per_step, N, P = _oracle_sample(args.config, args.steps, args.warmup, 1)
+    cores = _cores_used()
+    sample = ("configs[%d] box and ring (%d atoms x %d beads); each step = full FP64 integrator + the force "
+              "evaluation of 1 of the %d beads (%d bead-atoms)" % (args.config, N, P, P, N))
+    out = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": METRIC, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": s_per_step * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workloads.CONFIGS[args.config]["name"], "atoms": N, "beads": P, "sample": sample},
+        "cpu_baseline": {"value": value, "unit": METRIC, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": METRIC, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(out))
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------
+# this build
+# ------------------------------------------------------------------------------------------------
+def algorithmic_work(counts, N, P):
+    """SURVEY 8(d) per-unit figures: useful flops of each force kernel per step."""
+    rows = int(counts.sum())
+    PN = N * P
+    emb_mac = 25 + 1250 + 5000                      # layers 1..3 per row
+    flops = {
+        "embed_fwd": 2.0 * rows * (emb_mac + 400),                    # + G (x) R
+        "embed_bwd": 2.0 * rows * (emb_mac + 400 + 400 + 100),        # backward of the same + dG, dR, ds
+        "fitting": 2.0 * PN * 2 * (1600 * 240 + 2 * 240 * 240) + 2.0 * PN * (1600 * 4 + 2 * 1600 * 4),
+    }
+    return rows, flops
+
+
+def run_ours(args):
+    import torch
+    import paper_2602_13553_b200 as pk
+    pk.lib()                                        # fail loudly if the CUDA library is missing
+    rank, world, local = _dist()
+    if world > 1:
+        import torch.distributed as dist
+        torch.cuda.set_device(local)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    else:
+        torch.cuda.set_device(0)
+    peaks = _peaks()
+
+    cfg, wb, desc, w = workloads.make_config(args.config)
+    P, N = cfg["P"], wb["types"].size
+    # replicas only (north_star: one GPU, no sharding): every rank advances its own copy with its own seed
+    sim = pk.PIMD(wb["types"], wb["masses"], wb["box"], P, cfg["T"], cfg["dt"], cfg["gamma"], seed=1000 + rank,
+                  model_desc=desc)
+    x_host = torch.from_numpy(wb["x"]).pin_memory()
+    p_host = torch.from_numpy(wb["p"]).pin_memory()
+    x_dev, p_dev = x_host.cuda(non_blocking=True), p_host.cuda(non_blocking=True)
+    sim.set_model(w)
+    sim.set_state(x_dev, p_dev)                     # inputs resident in HBM before the timed region
+
+    def barrier():
+        if world > 1:
+            torch.distributed.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing: K steps ----
+    for _ in range(args.warmup):
+        sim.step(1)
+    launches0 = pk.pimd_get_launch_count(sim.ctx)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.25)
+    barrier()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t_wall0 = time.time()
+    ev0.record()
+    for _ in range(args.steps):
+        sim.step(1)
+    ev1.record()
+    barrier()
+    t_wall1 = time.time()
+    ms = ev0.elapsed_time(ev1)
+    launches = pk.pimd_get_launch_count(sim.ctx) - launches0
+    clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
+    if world > 1:
+        t = torch.tensor([ms], device="cuda")
+        torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * P * N * args.steps / (ms * 1e-3)
+
+    # ---- per-phase device times (CUDA events on the library's stream) ----
+    pk.pimd_set_profiling(sim.ctx, 1)
+    sim.step(max(3, min(10, args.steps)))
+    phase = pk.pimd_get_phase_ms(sim.ctx)
+    pk.pimd_set_profiling(sim.ctx, 0)
+    counts = pk.pimd_get_neighbor_counts(sim.ctx, P, N, 2)
+    rows, flops = algorithmic_work(counts, N, P)
+    names = ["integrator", "neighbour_env", "embed_fwd", "fitting", "embed_bwd"]
+    phases = {n: float(phase[q]) for q, n in enumerate(names)}
+    dom = max(("embed_fwd", "fitting", "embed_bwd"), key=lambda n: phases[n])
+    fp32_peak = 148 * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12     # TFLOP/s, CUDA-core FMA
+    achieved = flops[dom] / (phases[dom] * 1e-3) / 1e12
+    roofline = {"kernel": dom, "bound": "alu", "achieved": achieved, "peak": fp32_peak, "unit": "TFLOP/s",
+                "frac": achieved / fp32_peak, "traffic": None,
+                "note": "FP32 CUDA-core path; peak = 148 SM x 128 FMA lanes x 2 x sm_max_mhz (DESIGN.md 8); "
+                        "useful flops (SURVEY 8(d)), recompute not counted"}
+    kernels = {}
+    for n in ("embed_fwd", "fitting", "embed_bwd"):
+        a = flops[n] / (phases[n] * 1e-3) / 1e12
+        kernels[n] = {"ms": phases[n], "useful_tflops": a, "frac_fp32_peak": a / fp32_peak}
+    kernels["integrator"] = {"ms": phases["integrator"], "algorithmic_GBs": 120.0 * P * N / (phases["integrator"] * 1e-3) / 1e9,
+                             "note": "L2-resident at this size (5.9 MB/step); includes 3 memsets"}
+    kernels["neighbour_env"] = {"ms": phases["neighbour_env"]}
+
+    # ---- integrator alone at HBM-bound size (stand-alone leg, harmonic model) ----
+    integ = None
+    if rank == 0 and not args.no_integrator_leg:
+        integ = integrator_leg(pk, peaks)
+
+    # ---- end to end through the C ABI with host buffers ----
+    f_host = torch.empty_like(x_host).pin_memory()
+    xo, po, fo = sim.positions(), sim.momenta(), sim.forces()
+    Uo = sim.energies()
+    x_host.copy_(torch.from_numpy(xo)); p_host.copy_(torch.from_numpy(po)); f_host.copy_(torch.from_numpy(fo))
+    xn, pn, fn = x_host.numpy(), p_host.numpy(), f_host.numpy()
+    step_no = sim.estimators()["step"]
+    e2e_steps = max(3, min(args.steps, 10))
+    barrier()
+    t0 = time.perf_counter()
+    for q in range(e2e_steps):
+        pk.pimd_restore(sim.ctx, xn, pn, fn, Uo, step_no + q)          # H2D: x, p, f (+U)
+        sim.step(1)
+        xo = sim.positions(); po = sim.momenta(); fo = sim.forces()       # D2H
+        Uo = sim.energies()
+        est = sim.estimators()
+        xn[...] = xo; pn[...] = po; fn[...] = fo
+    barrier()
+    e2e_s = (time.perf_counter() - t0) / e2e_steps
+    if world > 1:
+        t = torch.tensor([e2e_s], device="cuda")
+        torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    h2d = 3 * P * N * 24 + P * 8
+    d2h = 3 * P * N * 24 + P * 8 + 32
+
+    out = None
+    if rank == 0:
+        cpu = None
+        if world == 1 and not args.no_cpu_baseline:
+            v, s_step, _, _ = _oracle_sample(args.config, 2, 1, 1)
+            cpu = {"value": v, "unit": METRIC, "cores": _cores_used(), "kind": "oracle",
+                   "sample": "configs[%d] box; 1 warm + 2 timed oracle steps with the force evaluation of 1 of %d beads "
+                             "(%d bead-atoms per step); %.1f s/step" % (args.config, P, N, s_step)}
+        out = {
+            "metric": METRIC, "value": value, "unit": METRIC, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32 network / f64 geometry+integrator", "data": "synthetic",
+            "config": {"workload": cfg["name"], "atoms": N, "beads": P, "bead_atoms": P * N, "neighbour_rows": rows,
+                       "parallelism": "replicas only" if world > 1 else "1 GPU",
+                       "l2": "no flush: per-step working set (neighbour slots, D, dD, activations ~1.5 GB) exceeds the 126 MB L2"},
+            "roofline": roofline, "kernels": kernels, "integrator_hbm": integ, "cpu_baseline": cpu,
+            "e2e": {"value": world * P * N / e2e_s, "unit": METRIC, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "ms_per_step": e2e_s * 1e3, "call": "pimd_restore(host x,p,f,U) + pimd_step(1) + pimd_get_{positions,momenta,forces,energies,estimators}"},
+            "gpu_launches": int(launches), "clocks": clocks, "peaks": peaks,
+            "paper_context": "fix pimd/langevin, 512 H2O x 32 beads: 2.56 M bead-atom-steps/s on 4xA100 (PAPER.md:L252, compressed DP model) -- context, not the target",
+        }
+        print(json.dumps(out))
+    sim.close()
+    if world > 1:
+        torch.distributed.destroy_process_group()
+    return 0
+
+
+def integrator_leg(pk, peaks, n_atoms=1 << 20, P=32):
+    """The fused integrator alone at a size that is HBM-bound: 2^20 atoms x 32 beads, harmonic
+    model, 40 B per bead-atom-dim per launch -> 4.03 GB; the working set exceeds L2 so no flush is needed."""
+    import torch
+    rng = np.random.default_rng(0)
+    types = np.zeros(n_atoms, np.int32)
+    sim = pk.PIMD(types, [1.008], [100.0] * 3, P, 300.0, 0.25e-3, 1.0, seed=5)
+    x = torch.from_numpy(rng.standard_normal((P, n_atoms, 3)) * 0.1).cuda()
+    p = torch.from_numpy(rng.standard_normal((P, n_atoms, 3))).cuda()
+    sim.set_model_harmonic(1.0)
+    sim.set_state(x, p)
+    ms = pk.pimd_time_kernel(sim.ctx, 0, 10)
+    nbytes = 40.0 * 3 * n_atoms * P
+    sim.close()
+    del x, p
+    torch.cuda.empty_cache()
+    gbs = nbytes / (ms * 1e-3) / 1e9
+    return {"kernel": "integrator_kernel<32>", "bound": "hbm", "achieved": gbs, "peak": peaks["hbm"], "unit": "GB/s",
+            "frac": gbs / peaks["hbm"], "ms": ms, "atoms": n_atoms, "beads": P, "bytes": nbytes,
+            "note": "stand-alone: closing B + estimators + B A O A + transforms, thermostat on"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json configs (default: the headline)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-integrator-leg", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

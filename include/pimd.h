@@ -96,6 +96,13 @@ int pimd_set_workspace(pimd_ctx* ctx, void* workspace_dev, size_t bytes, void* c
  * (BAOAB opens with a B that needs f(x0)). */
 int pimd_set_state(pimd_ctx* ctx, const double* x, const double* p);
 
+/* Resume from a checkpoint {x, p, f, U, step} (host arrays; SURVEY section 5 "checkpoint / resume"):
+ * like pimd_set_state, but the forces f[P][N][3] and bead energies U[P] that belong to x are supplied,
+ * so no force evaluation is run, and the step counter (which keys the Philox noise, R-10) is set to
+ * `step`.  Because the noise is counter-based, restore + pimd_step(n) continues a trajectory exactly
+ * as the uninterrupted run would have.  A model must already be set. */
+int pimd_restore(pimd_ctx* ctx, const double* x, const double* p, const double* f, const double* U, int64_t step);
+
 /* The se_e2_a Deep-Potential model (PAPER.md:L47, L76 cite it; definition DESIGN.md R-11..R-16).
  * weights: n_weights doubles, row-major W[in][out] then bias[out] per layer, in the order
  *   for t_i: for t_j: embedding layers 1..3;  then for t_i: fitting layers 1..4 (last out = 1).
@@ -138,6 +145,13 @@ int pimd_get_forces_dev(pimd_ctx* ctx, double* f_dev);
  * shift[cap][3] (periodic image n of R-11) receive the concatenated rows.  Returns the total number
  * of rows, or PIMD_EINVAL when cap is too small. */
 int64_t pimd_get_neighbors(pimd_ctx* ctx, int bead, int32_t* count, int32_t* j, int8_t* shift, size_t cap);
+
+/* Neighbour rows per bead-atom and neighbour type from the most recent force evaluation:
+ * counts[P][N][n_types] (host).  bench.py uses the total to state the algorithmic work. */
+int pimd_get_neighbor_counts(pimd_ctx* ctx, int32_t* counts);
+
+/* Number of kernels of this library launched on the context so far (the bench's gpu_launches). */
+int64_t pimd_get_launch_count(const pimd_ctx* ctx);
 
 /* The four Philox4x32-10 words and the normal eta the O step uses for (step, mode k, atom i,
  * component alpha) (R-10), evaluated ON THE DEVICE for n entries: idx[n][3] = (k, i, alpha);

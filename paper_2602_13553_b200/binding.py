@@ -64,6 +64,9 @@ _SIGNATURES = {
     "pimd_set_workspace": (C.c_int, [C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]),
     "pimd_set_state": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "pimd_set_state_dev": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
+    "pimd_restore": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64]),
+    "pimd_get_neighbor_counts": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "pimd_get_launch_count": (C.c_int64, [C.c_void_p]),
     "pimd_model_n_weights": (C.c_size_t, [C.c_void_p]),
     "pimd_set_model": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t]),
     "pimd_set_model_harmonic": (C.c_int, [C.c_void_p, C.c_double]),
@@ -158,6 +161,21 @@ def pimd_set_state(ctx, x, p):
 
 def pimd_set_state_dev(ctx, x_dev, p_dev):
     return _check(ctx, lib().pimd_set_state_dev(ctx, _ptr(x_dev), _ptr(p_dev)))
+
+
+def pimd_restore(ctx, x, p, f, U, step):
+    x, p, f, U = _f64(x), _f64(p), _f64(f), _f64(U)
+    return _check(ctx, lib().pimd_restore(ctx, x.ctypes.data, p.ctypes.data, f.ctypes.data, U.ctypes.data, int(step)))
+
+
+def pimd_get_neighbor_counts(ctx, P, N, n_types):
+    out = np.empty((P, N, n_types), dtype=np.int32)
+    _check(ctx, lib().pimd_get_neighbor_counts(ctx, out.ctypes.data))
+    return out
+
+
+def pimd_get_launch_count(ctx):
+    return int(lib().pimd_get_launch_count(ctx))
 
 
 def pimd_model_n_weights(desc):

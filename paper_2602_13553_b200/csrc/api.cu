@@ -15,6 +15,7 @@ struct pimd_ctx {
     double box[3] = {0, 0, 0}, T = 0, dt = 0, gamma0 = 0;
     uint64_t seed = 0;
     int64_t step = 0;
+    int64_t launches = 0;
     std::vector<int32_t> types;
     std::vector<double> masses;
     std::string err;
@@ -183,7 +184,7 @@ void rec(pimd_ctx* ctx, int i) {
 // one force evaluation at the current x: f, U, Xi, Eatom
 int eval_forces(pimd_ctx* ctx) {
     if (ctx->model_kind == 1) {
-        launch_harmonic(ctx->P, ctx->N, ctx->k_spring, ctx->x, ctx->f, ctx->U, ctx->Xi, ctx->Eatom, ctx->stream);
+        ctx->launches += launch_harmonic(ctx->P, ctx->N, ctx->k_spring, ctx->x, ctx->f, ctx->U, ctx->Xi, ctx->Eatom, ctx->stream);
         return PIMD_OK;
     }
     ForceArgs a;
@@ -195,13 +196,13 @@ int eval_forces(pimd_ctx* ctx) {
     cudaMemsetAsync(ctx->U, 0, sizeof(double) * ctx->P, ctx->stream);
     cudaMemsetAsync(ctx->Xi, 0, sizeof(double) * 9 * ctx->P, ctx->stream);
     rec(ctx, 1);
-    neighbor_build(ctx->model, a, ctx->stream);
+    ctx->launches += neighbor_build(ctx->model, a, ctx->stream);
     rec(ctx, 2);
-    embedding_forward(ctx->model, a, ctx->n_sms, ctx->stream);
+    ctx->launches += embedding_forward(ctx->model, a, ctx->n_sms, ctx->stream);
     rec(ctx, 3);
-    fitting_forward_backward(ctx->model, a, ctx->stream);
+    ctx->launches += fitting_forward_backward(ctx->model, a, ctx->stream);
     rec(ctx, 4);
-    embedding_backward(ctx->model, a, ctx->n_sms, ctx->stream);
+    ctx->launches += embedding_backward(ctx->model, a, ctx->n_sms, ctx->stream);
     rec(ctx, 5);
     return PIMD_OK;
 }
@@ -238,7 +239,7 @@ int refresh(pimd_ctx* ctx) {
     CK(cudaMemsetAsync(cur, 0, sizeof(double) * kEstWidth, ctx->stream));
     IntegratorArgs a;
     fill_integrator_args(ctx, a, I_EST, ctx->step, cur);
-    launch_integrator(ctx->P, a, ctx->mc, ctx->stream);
+    ctx->launches += launch_integrator(ctx->P, a, ctx->mc, ctx->stream);
     CK(cudaGetLastError());
     CK(cudaStreamSynchronize(ctx->stream));
     ctx->est_hist_n = 0;
@@ -334,7 +335,7 @@ int pimd_set_state_dev(pimd_ctx* ctx, const double* x_dev, const double* p_dev) 
     if ((rc = alloc_base(ctx))) return rc;
     const size_t PN3 = (size_t)ctx->P * ctx->N * 3;
     CK(cudaMemcpyAsync(ctx->x, x_dev, PN3 * 8, cudaMemcpyDeviceToDevice, ctx->stream));
-    launch_to_nm_velocity(ctx->P, ctx->N, p_dev, ctx->mass_atom, ctx->vt, ctx->stream);
+    ctx->launches += launch_to_nm_velocity(ctx->P, ctx->N, p_dev, ctx->mass_atom, ctx->vt, ctx->stream);
     CK(cudaGetLastError());
     ctx->have_state = true;
     ctx->step = 0;
@@ -350,6 +351,41 @@ int pimd_set_state(pimd_ctx* ctx, const double* x, const double* p) {
     CK(cudaMemcpyAsync(ctx->scratch_b, p, PN3 * 8, cudaMemcpyHostToDevice, ctx->stream));
     return pimd_set_state_dev(ctx, ctx->scratch_a, ctx->scratch_b);
 }
+
+int pimd_restore(pimd_ctx* ctx, const double* x, const double* p, const double* f, const double* U, int64_t step) {
+    if (!ctx || !x || !p || !f || !U || step < 0) return fail(ctx, PIMD_EINVAL, "bad argument");
+    if (ctx->model_kind == 0) return fail(ctx, PIMD_ENOMODEL, "set the model before restoring a checkpoint");
+    int rc;
+    if ((rc = alloc_base(ctx))) return rc;
+    const size_t PN3 = (size_t)ctx->P * ctx->N * 3;
+    CK(cudaMemcpyAsync(ctx->x, x, PN3 * 8, cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaMemcpyAsync(ctx->scratch_b, p, PN3 * 8, cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaMemcpyAsync(ctx->f, f, PN3 * 8, cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaMemcpyAsync(ctx->U, U, sizeof(double) * ctx->P, cudaMemcpyHostToDevice, ctx->stream));
+    ctx->launches += launch_to_nm_velocity(ctx->P, ctx->N, ctx->scratch_b, ctx->mass_atom, ctx->vt, ctx->stream);
+    ctx->have_state = true;
+    ctx->step = step;
+    double* cur = ctx->est + (size_t)kEstCap * kEstWidth;
+    CK(cudaMemsetAsync(cur, 0, sizeof(double) * kEstWidth, ctx->stream));
+    IntegratorArgs a;
+    fill_integrator_args(ctx, a, I_EST, ctx->step, cur);
+    ctx->launches += launch_integrator(ctx->P, a, ctx->mc, ctx->stream);
+    CK(cudaGetLastError());
+    CK(cudaStreamSynchronize(ctx->stream));
+    ctx->est_hist_n = 0;
+    return PIMD_OK;
+}
+
+int pimd_get_neighbor_counts(pimd_ctx* ctx, int32_t* counts) {
+    if (!ctx || !counts) return fail(ctx, PIMD_EINVAL, "null argument");
+    if (ctx->model_kind != 2 || !ctx->have_state) return fail(ctx, PIMD_ENOMODEL, "needs an se_e2_a model and a state");
+    CK(cudaMemcpyAsync(counts, ctx->model.ncount, sizeof(int32_t) * (size_t)ctx->P * ctx->N * ctx->ntypes,
+                       cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return PIMD_OK;
+}
+
+int64_t pimd_get_launch_count(const pimd_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
 int pimd_set_model_harmonic(pimd_ctx* ctx, double k_spring) {
     if (!ctx) return PIMD_EINVAL;
@@ -510,7 +546,7 @@ int pimd_step(pimd_ctx* ctx, int64_t n_steps) {
         IntegratorArgs a;
         fill_integrator_args(ctx, a, flags, ctx->step + s, slot);
         rec(ctx, 0);
-        launch_integrator(ctx->P, a, ctx->mc, ctx->stream);
+        ctx->launches += launch_integrator(ctx->P, a, ctx->mc, ctx->stream);
         if (s < n_steps) {
             int rc = eval_forces(ctx);
             if (rc) return rc;
@@ -554,7 +590,7 @@ int pimd_get_positions(pimd_ctx* ctx, double* x) {
 int pimd_get_momenta(pimd_ctx* ctx, double* p) {
     if (!ctx || !p) return fail(ctx, PIMD_EINVAL, "null argument");
     if (!ctx->have_state) return fail(ctx, PIMD_ENOSTATE, "pimd_set_state has not been called");
-    launch_from_nm_momenta(ctx->P, ctx->N, ctx->vt, ctx->mass_atom, ctx->scratch_a, ctx->stream);
+    ctx->launches += launch_from_nm_momenta(ctx->P, ctx->N, ctx->vt, ctx->mass_atom, ctx->scratch_a, ctx->stream);
     return copy_out(ctx, ctx->scratch_a, p, (size_t)ctx->P * ctx->N * 24);
 }
 int pimd_get_forces(pimd_ctx* ctx, double* f) {
@@ -657,7 +693,7 @@ int pimd_debug_noise(pimd_ctx* ctx, int64_t step, int n, const int32_t* idx, uin
     CK(cudaMalloc(&d_w, sizeof(uint32_t) * 4 * n));
     CK(cudaMalloc(&d_e, sizeof(double) * n));
     CK(cudaMemcpyAsync(d_idx, idx, sizeof(int32_t) * 3 * n, cudaMemcpyHostToDevice, ctx->stream));
-    launch_debug_noise(ctx->seed, (uint64_t)step, n, d_idx, d_w, d_e, ctx->stream);
+    ctx->launches += launch_debug_noise(ctx->seed, (uint64_t)step, n, d_idx, d_w, d_e, ctx->stream);
     CK(cudaMemcpyAsync(words, d_w, sizeof(uint32_t) * 4 * n, cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaMemcpyAsync(eta, d_e, sizeof(double) * n, cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
@@ -673,9 +709,9 @@ int pimd_time_kernel(pimd_ctx* ctx, int kind, int reps, double* ms) {
     double* scratch = ctx->est + (size_t)(kEstCap + 1) * kEstWidth;
     fill_integrator_args(ctx, a, I_BCLOSE | I_EST | I_START, ctx->step, scratch);
     a.x_out = ctx->scratch_a; a.vt_out = ctx->scratch_b;          // state is not advanced
-    for (int w = 0; w < 3; ++w) launch_integrator(ctx->P, a, ctx->mc, ctx->stream);
+    for (int w = 0; w < 3; ++w) ctx->launches += launch_integrator(ctx->P, a, ctx->mc, ctx->stream);
     CK(cudaEventRecord(ctx->ev[6], ctx->stream));
-    for (int r = 0; r < reps; ++r) launch_integrator(ctx->P, a, ctx->mc, ctx->stream);
+    for (int r = 0; r < reps; ++r) ctx->launches += launch_integrator(ctx->P, a, ctx->mc, ctx->stream);
     CK(cudaEventRecord(ctx->ev[7], ctx->stream));
     CK(cudaEventSynchronize(ctx->ev[7]));
     CK(cudaGetLastError());

@@ -48,12 +48,12 @@ struct IntegratorArgs {
     double*  est;                // [kEstWidth] accumulators of this step's slot, may be null
 };
 
-void launch_integrator(int P, const IntegratorArgs& a, const ModeConsts& mc, cudaStream_t s);
-void launch_to_nm_velocity(int P, int N, const double* p_cart, const double* mass, double* vt, cudaStream_t s);
-void launch_from_nm_momenta(int P, int N, const double* vt, const double* mass, double* p_cart, cudaStream_t s);
-void launch_harmonic(int P, int N, double k_spring, const double* x, double* f, double* U, double* Xi,
+int launch_integrator(int P, const IntegratorArgs& a, const ModeConsts& mc, cudaStream_t s);
+int launch_to_nm_velocity(int P, int N, const double* p_cart, const double* mass, double* vt, cudaStream_t s);
+int launch_from_nm_momenta(int P, int N, const double* vt, const double* mass, double* p_cart, cudaStream_t s);
+int launch_harmonic(int P, int N, double k_spring, const double* x, double* f, double* U, double* Xi,
                      double* Eatom, cudaStream_t s);
-void launch_debug_noise(uint64_t seed, uint64_t step, int n, const int32_t* idx_dev, uint32_t* words_dev,
+int launch_debug_noise(uint64_t seed, uint64_t step, int n, const int32_t* idx_dev, uint32_t* words_dev,
                         double* eta_dev, cudaStream_t s);
 
 // ---------------------------------------------------------------------------------------------
@@ -110,10 +110,10 @@ struct ForceArgs {
     double* Eatom;        // [P][N]
 };
 
-void neighbor_build(Model& m, const ForceArgs& a, cudaStream_t s);
-void embedding_forward(Model& m, const ForceArgs& a, int n_sms, cudaStream_t s);
-void fitting_forward_backward(Model& m, const ForceArgs& a, cudaStream_t s);
-void embedding_backward(Model& m, const ForceArgs& a, int n_sms, cudaStream_t s);
+int neighbor_build(Model& m, const ForceArgs& a, cudaStream_t s);
+int embedding_forward(Model& m, const ForceArgs& a, int n_sms, cudaStream_t s);
+int fitting_forward_backward(Model& m, const ForceArgs& a, cudaStream_t s);
+int embedding_backward(Model& m, const ForceArgs& a, int n_sms, cudaStream_t s);
 size_t embedding_smem_bytes(const Model& m, int ntypes);
 
 }  // namespace pimd

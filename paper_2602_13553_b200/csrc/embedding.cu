@@ -298,20 +298,22 @@ static size_t bwd_smem(const Model& m, int ntypes) {
 }
 size_t embedding_smem_bytes(const Model& m, int ntypes) { return fwd_smem(m, ntypes); }
 
-void embedding_forward(Model& m, const ForceArgs& fa, int n_sms, cudaStream_t s) {
+int embedding_forward(Model& m, const ForceArgs& fa, int n_sms, cudaStream_t s) {
     EmbArgs a = make_args(m, fa);
     const size_t smem = fwd_smem(m, fa.ntypes);
     cudaFuncSetAttribute(embed_fwd_kernel<25, 50, 100>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     const int grid = min(a.PN, n_sms * 2);
     embed_fwd_kernel<25, 50, 100><<<grid, kEmbThreads, smem, s>>>(a);
+    return 1;
 }
 
-void embedding_backward(Model& m, const ForceArgs& fa, int n_sms, cudaStream_t s) {
+int embedding_backward(Model& m, const ForceArgs& fa, int n_sms, cudaStream_t s) {
     EmbArgs a = make_args(m, fa);
     const size_t smem = bwd_smem(m, fa.ntypes);
     cudaFuncSetAttribute(embed_bwd_kernel<25, 50, 100>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     const int grid = min(a.PN, n_sms * 2);
     embed_bwd_kernel<25, 50, 100><<<grid, kEmbThreads, smem, s>>>(a);
+    return 1;
 }
 
 }  // namespace pimd

@@ -200,13 +200,15 @@ energy_kernel(int row0, int rows, int NF, int N, const float* __restrict__ Y3, c
     }
 }
 
-void fitting_forward_backward(Model& m, const ForceArgs& a, cudaStream_t s) {
+int fitting_forward_backward(Model& m, const ForceArgs& a, cudaStream_t s) {
     const int PN = a.P * a.N;
     const int NF = m.NF, ND = m.ND;
+    int launches = 2;
     descriptor_kernel<100, 16><<<PN, 256, 0, s>>>(PN, m.Tm, m.D);
     for (int t = 0; t < a.ntypes; ++t) {
         const int row0 = m.type_row0[t], rows = m.type_row0[t + 1] - row0;
         if (rows == 0) continue;
+        launches += 7;
         const size_t oF = (size_t)row0 * NF, oD = (size_t)row0 * ND;
         GemmArgs g{};
         // layer 1: Y1 = tanh(D W1 + b1)
@@ -243,6 +245,7 @@ void fitting_forward_backward(Model& m, const ForceArgs& a, cudaStream_t s) {
         launch_gemm<EPI_PLAIN>(g, s);
     }
     dT_kernel<100, 16><<<PN, 128, 0, s>>>(PN, m.Tm, m.dD, m.dTm);
+    return launches;
 }
 
 }  // namespace pimd

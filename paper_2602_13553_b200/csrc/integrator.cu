@@ -208,7 +208,7 @@ static void launch_int_t(const IntegratorArgs& a, const ModeConsts& mc, cudaStre
     integrator_kernel<P><<<blocks, kIntThreads, smem, s>>>(a, mc);
 }
 
-void launch_integrator(int P, const IntegratorArgs& a, const ModeConsts& mc, cudaStream_t s) {
+int launch_integrator(int P, const IntegratorArgs& a, const ModeConsts& mc, cudaStream_t s) {
     switch (P) {
         case 1: launch_int_t<1>(a, mc, s); break;
         case 2: launch_int_t<2>(a, mc, s); break;
@@ -217,8 +217,9 @@ void launch_integrator(int P, const IntegratorArgs& a, const ModeConsts& mc, cud
         case 16: launch_int_t<16>(a, mc, s); break;
         case 32: launch_int_t<32>(a, mc, s); break;
         case 64: launch_int_t<64>(a, mc, s); break;
-        default: break;
+        default: return 0;
     }
+    return 1;
 }
 
 // v~ = M (p/m)  and  p = m M^T v~  (API momenta are Cartesian; PAPER.md:L104 keeps v in NM form inside)
@@ -258,11 +259,13 @@ static void launch_conv(int P, int N, const double* in, const double* mass, doub
         default: break;
     }
 }
-void launch_to_nm_velocity(int P, int N, const double* p, const double* mass, double* vt, cudaStream_t s) {
+int launch_to_nm_velocity(int P, int N, const double* p, const double* mass, double* vt, cudaStream_t s) {
     launch_conv<true>(P, N, p, mass, vt, s);
+    return 1;
 }
-void launch_from_nm_momenta(int P, int N, const double* vt, const double* mass, double* p, cudaStream_t s) {
+int launch_from_nm_momenta(int P, int N, const double* vt, const double* mass, double* p, cudaStream_t s) {
     launch_conv<false>(P, N, vt, mass, p, s);
+    return 1;
 }
 
 // Test model U = sum_i 1/2 k |r_i|^2 (FP64): f = -k x, U^(k), Xi_ab = sum_i x_a f_b.
@@ -297,12 +300,13 @@ __global__ void harmonic_kernel(int N, double ks, const double* __restrict__ x, 
     }
 }
 
-void launch_harmonic(int P, int N, double ks, const double* x, double* f, double* U, double* Xi, double* Eatom,
+int launch_harmonic(int P, int N, double ks, const double* x, double* f, double* U, double* Xi, double* Eatom,
                      cudaStream_t s) {
     cudaMemsetAsync(U, 0, sizeof(double) * P, s);
     cudaMemsetAsync(Xi, 0, sizeof(double) * 9 * P, s);
     dim3 grid((N + 127) / 128, P);
     harmonic_kernel<<<grid, 128, 0, s>>>(N, ks, x, f, U, Xi, Eatom);
+    return 1;
 }
 
 __global__ void debug_noise_kernel(uint32_t seed_lo, uint32_t seed_hi, uint32_t step_lo, uint32_t step_hi, int n,
@@ -317,10 +321,11 @@ __global__ void debug_noise_kernel(uint32_t seed_lo, uint32_t seed_hi, uint32_t 
     eta[t] = philox_normal(seed_lo, seed_hi, step_lo, step_hi, i, 4u * k + al);
 }
 
-void launch_debug_noise(uint64_t seed, uint64_t step, int n, const int32_t* idx, uint32_t* words, double* eta,
+int launch_debug_noise(uint64_t seed, uint64_t step, int n, const int32_t* idx, uint32_t* words, double* eta,
                         cudaStream_t s) {
     debug_noise_kernel<<<(n + 127) / 128, 128, 0, s>>>((uint32_t)seed, (uint32_t)(seed >> 32), (uint32_t)step,
                                                         (uint32_t)(step >> 32), n, idx, words, eta);
+    return 1;
 }
 
 }  // namespace pimd

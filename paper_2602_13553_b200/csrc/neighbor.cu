@@ -205,7 +205,7 @@ neighbor_env_kernel(int P, int N, GridGeom g, EnvConsts ec, const double* __rest
     }
 }
 
-void neighbor_build(Model& m, const ForceArgs& a, cudaStream_t s) {
+int neighbor_build(Model& m, const ForceArgs& a, cudaStream_t s) {
     const int PN = a.P * a.N;
     GridGeom g;
     for (int c = 0; c < 3; ++c) {
@@ -234,6 +234,7 @@ void neighbor_build(Model& m, const ForceArgs& a, cudaStream_t s) {
                                                                         m.wtmp, a.types, m.wsorted);
     neighbor_env_kernel<<<(unsigned)(((long long)PN * 32 + th - 1) / th), th, 0, s>>>(
         a.P, a.N, g, ec, m.wtmp, m.cell_id, m.cell_start, m.wsorted, m.ncount, m.slotA, m.slotB, m.overflow);
+    return 5;
 }
 
 }  // namespace pimd
