@@ -158,6 +158,14 @@ int64_t pimd_get_launch_count(const pimd_ctx* ctx);
  * words[n][4], eta[n].  */
 int pimd_debug_noise(pimd_ctx* ctx, int64_t step, int n, const int32_t* idx, uint32_t* words, double* eta);
 
+/* Fitting-net GEMM path: 1 (default) = tcgen05 tensor cores, 3xTF32 split (fitting_tc.cu); 0 = the FP32
+ * CUDA-core GEMMs kept as the in-tree reference for bisecting.  Both meet the parity tolerances. */
+int pimd_set_fitting_path(pimd_ctx* ctx, int use_tensor_cores);
+
+/* Parity hook for the tensor-core GEMM kernel alone: C[M][N] = A[M][K] Bt[N][K]^T, host FP32 arrays,
+ * N == 240 or N % 160 == 0, K % 16 == 0 (the shapes the fitting net uses). */
+int pimd_debug_gemm(pimd_ctx* ctx, int M, int N, int K, const float* A, const float* Bt, float* C);
+
 /* Stand-alone timing of kernels (bench.py roofline legs): runs `reps` launches of the fused
  * integrator kernel (kind 0) on the current state WITHOUT advancing it (output to scratch), and
  * returns the mean device time per launch in milliseconds through *ms. */

@@ -14,5 +14,6 @@ from .binding import (  # noqa: F401
     pimd_step, pimd_get_positions, pimd_get_momenta, pimd_get_forces, pimd_get_virial, pimd_get_energies,
     pimd_get_atom_energies, pimd_get_estimators, pimd_get_estimator_history, pimd_get_positions_dev,
     pimd_get_forces_dev, pimd_get_neighbors, pimd_debug_noise, pimd_time_kernel, pimd_set_profiling,
-    pimd_get_phase_ms, pimd_restore, pimd_get_neighbor_counts, pimd_get_launch_count, PIMD,
+    pimd_get_phase_ms, pimd_restore, pimd_get_neighbor_counts, pimd_get_launch_count, pimd_set_fitting_path,
+    pimd_debug_gemm, PIMD,
 )

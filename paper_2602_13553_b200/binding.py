@@ -67,6 +67,8 @@ _SIGNATURES = {
     "pimd_restore": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64]),
     "pimd_get_neighbor_counts": (C.c_int, [C.c_void_p, C.c_void_p]),
     "pimd_get_launch_count": (C.c_int64, [C.c_void_p]),
+    "pimd_set_fitting_path": (C.c_int, [C.c_void_p, C.c_int]),
+    "pimd_debug_gemm": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]),
     "pimd_model_n_weights": (C.c_size_t, [C.c_void_p]),
     "pimd_set_model": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t]),
     "pimd_set_model_harmonic": (C.c_int, [C.c_void_p, C.c_double]),
@@ -176,6 +178,20 @@ def pimd_get_neighbor_counts(ctx, P, N, n_types):
 
 def pimd_get_launch_count(ctx):
     return int(lib().pimd_get_launch_count(ctx))
+
+
+def pimd_set_fitting_path(ctx, use_tensor_cores):
+    return _check(ctx, lib().pimd_set_fitting_path(ctx, int(bool(use_tensor_cores))))
+
+
+def pimd_debug_gemm(ctx, A, Bt):
+    A = np.ascontiguousarray(A, dtype=np.float32)
+    Bt = np.ascontiguousarray(Bt, dtype=np.float32)
+    M, K = A.shape
+    N = Bt.shape[0]
+    Cm = np.empty((M, N), dtype=np.float32)
+    _check(ctx, lib().pimd_debug_gemm(ctx, M, N, K, A.ctypes.data, Bt.ctypes.data, Cm.ctypes.data))
+    return Cm
 
 
 def pimd_model_n_weights(desc):

@@ -517,6 +517,7 @@ int pimd_set_model(pimd_ctx* ctx, const pimd_model_desc* d, const double* w, siz
         if ((rc = arena_alloc(ctx, fb[q], PN * m.NF))) return rc;
     CK(cudaMemsetAsync(m.overflow, 0, sizeof(int), ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));     // host staging vectors go out of scope below
+    tc_setup_maps(m, nt);        // tensor-core fitting path (falls back to the CUDA-core GEMMs only if unsupported widths)
     m.set = true;
     ctx->model_kind = 2;
     return refresh(ctx);
@@ -718,6 +719,33 @@ int pimd_time_kernel(pimd_ctx* ctx, int kind, int reps, double* ms) {
     float t = 0;
     CK(cudaEventElapsedTime(&t, ctx->ev[6], ctx->ev[7]));
     *ms = (double)t / reps;
+    return PIMD_OK;
+}
+
+int pimd_set_fitting_path(pimd_ctx* ctx, int use_tensor_cores) {
+    if (!ctx) return PIMD_EINVAL;
+    if (use_tensor_cores && ctx->model.set && !ctx->model.tc_ready)
+        return fail(ctx, PIMD_EINVAL, "tensor-core path unavailable for this architecture (needs fit width 240)");
+    ctx->model.use_tc = use_tensor_cores != 0;
+    return PIMD_OK;
+}
+
+int pimd_debug_gemm(pimd_ctx* ctx, int M, int N, int K, const float* A, const float* Bt, float* C) {
+    if (!ctx || !A || !Bt || !C || M <= 0 || N <= 0 || K <= 0) return fail(ctx, PIMD_EINVAL, "bad argument");
+    float *dA = nullptr, *dB = nullptr, *dC = nullptr;
+    CK(cudaMalloc(&dA, sizeof(float) * (size_t)M * K));
+    CK(cudaMalloc(&dB, sizeof(float) * (size_t)N * K));
+    CK(cudaMalloc(&dC, sizeof(float) * (size_t)M * N));
+    CK(cudaMemcpyAsync(dA, A, sizeof(float) * (size_t)M * K, cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaMemcpyAsync(dB, Bt, sizeof(float) * (size_t)N * K, cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaMemsetAsync(dC, 0xFF, sizeof(float) * (size_t)M * N, ctx->stream));
+    const int rc = debug_tc_gemm(M, N, K, dA, dB, dC, ctx->stream);
+    ctx->launches += 1;
+    cudaError_t e = cudaStreamSynchronize(ctx->stream);
+    if (rc == 0 && e == cudaSuccess) e = cudaMemcpy(C, dC, sizeof(float) * (size_t)M * N, cudaMemcpyDeviceToHost);
+    cudaFree(dA); cudaFree(dB); cudaFree(dC);
+    if (rc != 0) return fail(ctx, PIMD_EINVAL, "debug gemm: unsupported shape or tensor-map failure");
+    if (e != cudaSuccess) return fail(ctx, PIMD_ECUDA, std::string("debug gemm: ") + cudaGetErrorString(e));
     return PIMD_OK;
 }
 

@@ -1,6 +1,7 @@
 // common.cuh -- internal declarations shared by the translation units of libpimd_b200.
 // Product code (CUDA, sm_100a).  Shares nothing with oracle/.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stddef.h>
@@ -97,6 +98,13 @@ struct Model {
     float*   dD = nullptr;
     float*   Y1 = nullptr, *T2 = nullptr, *Y2 = nullptr, *T3 = nullptr, *Y3 = nullptr;   // [rows][NF]
     float*   G1 = nullptr, *G2 = nullptr;   // backward scratch [rows][NF]
+    // tensor-core path (fitting_tc.cu): TMA tensor maps per centre type
+    bool     use_tc = true;
+    bool     tc_ready = false;
+    CUtensorMap mapA_D[PIMD_MAX_TYPES], mapA_Y1[PIMD_MAX_TYPES], mapA_Y2[PIMD_MAX_TYPES], mapA_G1[PIMD_MAX_TYPES],
+                mapA_T3[PIMD_MAX_TYPES];
+    CUtensorMap mapB_fwd[PIMD_MAX_TYPES][3];   // W_l^T  [out][in]
+    CUtensorMap mapB_bwd[PIMD_MAX_TYPES][3];   // W_l    [in][out]
 };
 
 struct ForceArgs {
@@ -115,5 +123,7 @@ int embedding_forward(Model& m, const ForceArgs& a, int n_sms, cudaStream_t s);
 int fitting_forward_backward(Model& m, const ForceArgs& a, cudaStream_t s);
 int embedding_backward(Model& m, const ForceArgs& a, int n_sms, cudaStream_t s);
 size_t embedding_smem_bytes(const Model& m, int ntypes);
+bool tc_setup_maps(Model& m, int ntypes);
+int debug_tc_gemm(int M, int N, int K, const float* A_dev, const float* Bt_dev, float* C_dev, cudaStream_t s);
 
 }  // namespace pimd

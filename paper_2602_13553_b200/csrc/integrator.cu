@@ -9,6 +9,7 @@
 //   x = M^T x~                                       Eq. B3
 // reads x, v~, f once and writes x, v~ once: 40 B per bead-atom-dim.
 #include "common.cuh"
+#include <cuda_pipeline.h>
 #include "philox.cuh"
 
 namespace pimd {
@@ -104,17 +105,30 @@ constexpr int kIntThreads = 128;
 template <int P>
 __global__ void __launch_bounds__(kIntThreads)
 integrator_kernel(const __grid_constant__ IntegratorArgs a, const __grid_constant__ ModeConsts mc) {
-    extern __shared__ double eta_s[];                  // [P][kIntThreads] thermostat normals
+    // dynamic smem: x and f tiles [P][kIntThreads] staged with cp.async (all 2P loads of a thread are in
+    // flight at once, independent of the register budget), then the thermostat normals [P][kIntThreads]
+    extern __shared__ double dyn_s[];
+    double* xs = dyn_s;
+    double* fs = dyn_s + P * kIntThreads;
+    double* eta_s = dyn_s + 2 * P * kIntThreads;
     const int e = blockIdx.x * kIntThreads + threadIdx.x;
     const bool live = e < a.n_dof;
     const int ec = live ? e : a.n_dof - 1;             // dead threads shadow the last dof, never store
     const int i = ec / 3, alpha = ec - 3 * i;
     const bool start = (a.flags & I_START) != 0;
     const bool thermo = start && a.thermostat;
+    const size_t stride = (size_t)a.n_dof;
 
-    // ---- O-step normals first (few live registers; rolled loop keeps one copy of log/cos) ----
+#pragma unroll
+    for (int k = 0; k < P; ++k) {
+        __pipeline_memcpy_async(xs + k * kIntThreads + threadIdx.x, a.x_in + k * stride + ec, sizeof(double));
+        __pipeline_memcpy_async(fs + k * kIntThreads + threadIdx.x, a.f + k * stride + ec, sizeof(double));
+    }
+    __pipeline_commit();
+
+    // ---- O-step normals while the loads fly (rolled loop keeps one copy of log/cos) ----
     if (thermo) {
-#pragma unroll 1
+#pragma unroll 4
         for (int k = 0; k < P; ++k) {
             eta_s[k * kIntThreads + threadIdx.x] =
                 philox_normal(a.seed_lo, a.seed_hi, a.step_lo, a.step_hi, (uint32_t)i, (uint32_t)(4 * k + alpha));
@@ -122,13 +136,13 @@ integrator_kernel(const __grid_constant__ IntegratorArgs a, const __grid_constan
     }
 
     const double m = a.mass[i];
-    const size_t stride = (size_t)a.n_dof;
+    __pipeline_wait_prior(0);
     double xt[P], ft[P];
     double xf = 0.0;
 #pragma unroll
     for (int k = 0; k < P; ++k) {
-        xt[k] = a.x_in[k * stride + ec];
-        ft[k] = a.f[k * stride + ec];
+        xt[k] = xs[k * kIntThreads + threadIdx.x];
+        ft[k] = fs[k * kIntThreads + threadIdx.x];
     }
 #pragma unroll
     for (int k = 0; k < P; ++k) xf += xt[k] * ft[k];
@@ -199,7 +213,7 @@ integrator_kernel(const __grid_constant__ IntegratorArgs a, const __grid_constan
 template <int P>
 static void launch_int_t(const IntegratorArgs& a, const ModeConsts& mc, cudaStream_t s) {
     const int blocks = (a.n_dof + kIntThreads - 1) / kIntThreads;
-    const size_t smem = (size_t)P * kIntThreads * sizeof(double);
+    const size_t smem = (size_t)3 * P * kIntThreads * sizeof(double);
     static bool attr_done = false;
     if (!attr_done) {
         cudaFuncSetAttribute(integrator_kernel<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

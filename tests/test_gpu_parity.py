@@ -261,3 +261,36 @@ def test_full_step_parity_config0(pk):
     assert abs(e["K_PR"] - o["K_PR"]) <= 1e-6 * abs(o["K_PR"])
     assert abs(e["H"] - o["H"]) <= 1e-6 * sim.N * sim.P
     sim.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# tensor-core GEMM kernel alone (3xTF32 on tcgen05) against the FP64 product
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("M,N,K", [(256, 240, 16), (300, 240, 1600), (1000, 240, 240), (417, 1600, 240), (5, 160, 48)])
+def test_tc_gemm_3xtf32_matches_fp64_product(pk, M, N, K):
+    rng = np.random.default_rng(M + N + K)
+    A = rng.standard_normal((M, K)).astype(np.float32)
+    Bt = (rng.standard_normal((N, K)) / np.sqrt(K)).astype(np.float32)
+    sim = pk.PIMD(np.zeros(4, np.int32), [1.0], [10.0] * 3, 4, 300.0, 1e-3, 1.0, seed=0)
+    C = pk.pimd_debug_gemm(sim.ctx, A, Bt)
+    ref = A.astype(np.float64) @ Bt.astype(np.float64).T
+    err = np.abs(C - ref).max() / np.abs(ref).max()
+    assert err < 3e-5, err          # FP32-class (K = 1600: 1.1e-5); single-pass TF32 gives ~1e-3
+    sim.close()
+
+
+def test_tensor_core_and_cuda_core_fitting_paths_agree(pk):
+    cfg, wb, desc, w = workloads.make_config(0)
+    w = workloads.model_weights(desc, cfg["weight_seed"], last_layer_scale=1.0e3)
+    out = []
+    for use_tc in (1, 0):
+        sim = pk.PIMD(wb["types"], wb["masses"], wb["box"], cfg["P"], cfg["T"], cfg["dt"], cfg["gamma"], seed=0,
+                      model_desc=desc)
+        sim.set_model(w)
+        pk.pimd_set_fitting_path(sim.ctx, use_tc)
+        sim.set_state(wb["x"], wb["p"])
+        out.append((sim.forces(), sim.atom_energies()))
+        sim.close()
+    frms = np.sqrt((out[1][0] ** 2).mean())
+    assert np.abs(out[0][0] - out[1][0]).max() <= 2e-5 * frms
+    assert np.abs(out[0][1] - out[1][1]).max() <= 1e-6 * 1e3
