@@ -162,6 +162,11 @@ int pimd_debug_noise(pimd_ctx* ctx, int64_t step, int n, const int32_t* idx, uin
  * CUDA-core GEMMs kept as the in-tree reference for bisecting.  Both meet the parity tolerances. */
 int pimd_set_fitting_path(pimd_ctx* ctx, int use_tensor_cores);
 
+/* Embedding-net path: 1 (default) = tcgen05 tensor cores, 3xTF32, row tiles of one type pair
+ * (embedding_tc.cu); 0 = the FP32 CUDA-core kernels kept as the in-tree reference.  Takes effect at the
+ * next force evaluation (pimd_set_state / pimd_step). */
+int pimd_set_embedding_path(pimd_ctx* ctx, int use_tensor_cores);
+
 /* Parity hook for the tensor-core GEMM kernel alone: C[M][N] = A[M][K] Bt[N][K]^T, host FP32 arrays,
  * N == 240 or N % 160 == 0, K % 16 == 0 (the shapes the fitting net uses). */
 int pimd_debug_gemm(pimd_ctx* ctx, int M, int N, int K, const float* A, const float* Bt, float* C);

@@ -68,6 +68,7 @@ _SIGNATURES = {
     "pimd_get_neighbor_counts": (C.c_int, [C.c_void_p, C.c_void_p]),
     "pimd_get_launch_count": (C.c_int64, [C.c_void_p]),
     "pimd_set_fitting_path": (C.c_int, [C.c_void_p, C.c_int]),
+    "pimd_set_embedding_path": (C.c_int, [C.c_void_p, C.c_int]),
     "pimd_debug_gemm": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]),
     "pimd_model_n_weights": (C.c_size_t, [C.c_void_p]),
     "pimd_set_model": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t]),
@@ -182,6 +183,10 @@ def pimd_get_launch_count(ctx):
 
 def pimd_set_fitting_path(ctx, use_tensor_cores):
     return _check(ctx, lib().pimd_set_fitting_path(ctx, int(bool(use_tensor_cores))))
+
+
+def pimd_set_embedding_path(ctx, use_tensor_cores):
+    return _check(ctx, lib().pimd_set_embedding_path(ctx, int(bool(use_tensor_cores))))
 
 
 def pimd_debug_gemm(ctx, A, Bt):

@@ -123,6 +123,9 @@ size_t model_bytes(const pimd_ctx* c, const pimd_model_desc* d) {
     b += 2 * align_up(PN * M1 * 16, 256);
     b += 2 * align_up(PN * ND * 4, 256);
     b += 7 * align_up(PN * NF * 4, 256);
+    b += align_up((size_t)d->n_types * d->n_types * emb_tc_image_bytes(), 256);               // tensor-core embedding
+    b += align_up((size_t)d->n_types * (PN + 1) * 4, 256) + align_up(PN * nsel * 4, 256);
+    b += align_up((size_t)d->n_types * ((PN + 1023) / 1024) * 4, 256) + align_up(PN * 72, 256);
     return b + 65536;
 }
 
@@ -197,12 +200,16 @@ int eval_forces(pimd_ctx* ctx) {
     cudaMemsetAsync(ctx->Xi, 0, sizeof(double) * 9 * ctx->P, ctx->stream);
     rec(ctx, 1);
     ctx->launches += neighbor_build(ctx->model, a, ctx->stream);
+    const bool tc_emb = ctx->model.use_tc_emb && ctx->model.tc_emb_ready;
+    if (tc_emb) ctx->launches += emb_tc_row_index(ctx->model, a, ctx->stream);
     rec(ctx, 2);
-    ctx->launches += embedding_forward(ctx->model, a, ctx->n_sms, ctx->stream);
+    ctx->launches += tc_emb ? embedding_forward_tc(ctx->model, a, ctx->n_sms, ctx->stream)
+                            : embedding_forward(ctx->model, a, ctx->n_sms, ctx->stream);
     rec(ctx, 3);
     ctx->launches += fitting_forward_backward(ctx->model, a, ctx->stream);
     rec(ctx, 4);
-    ctx->launches += embedding_backward(ctx->model, a, ctx->n_sms, ctx->stream);
+    ctx->launches += tc_emb ? embedding_backward_tc(ctx->model, a, ctx->n_sms, ctx->stream)
+                            : embedding_backward(ctx->model, a, ctx->n_sms, ctx->stream);
     rec(ctx, 5);
     return PIMD_OK;
 }
@@ -429,6 +436,11 @@ int pimd_set_model(pimd_ctx* ctx, const pimd_model_desc* d, const double* w, siz
     m.emb_stride = (ob3 + M1 + 3) / 4 * 4;
     std::vector<float> ew((size_t)nt * nt * m.emb_stride, 0.f);
     size_t pos = 0;
+    std::vector<uint8_t> img((size_t)nt * nt * emb_tc_image_bytes());
+    {
+        const size_t per_pair = (size_t)2 * E1 + (size_t)E1 * E2 + E2 + (size_t)E2 * M1 + M1;
+        for (int q = 0; q < nt * nt; ++q) emb_tc_build_image(w + q * per_pair, img.data() + (size_t)q * emb_tc_image_bytes());
+    }
     for (int ti = 0; ti < nt; ++ti)
         for (int tj = 0; tj < nt; ++tj) {
             float* o = ew.data() + (size_t)(ti * nt + tj) * m.emb_stride;
@@ -449,6 +461,8 @@ int pimd_set_model(pimd_ctx* ctx, const pimd_model_desc* d, const double* w, siz
         }
     if ((rc = arena_alloc(ctx, &m.emb_w, ew.size()))) return rc;
     CK(cudaMemcpyAsync(m.emb_w, ew.data(), ew.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
+    if ((rc = arena_alloc(ctx, &m.emb_img, img.size()))) return rc;
+    CK(cudaMemcpyAsync(m.emb_img, img.data(), img.size(), cudaMemcpyHostToDevice, ctx->stream));
 
     // ---- fitting weights: W, W^T, b per layer ----
     std::vector<std::vector<float>> keep;
@@ -515,6 +529,11 @@ int pimd_set_model(pimd_ctx* ctx, const pimd_model_desc* d, const double* w, siz
     float** fb[7] = {&m.Y1, &m.T2, &m.Y2, &m.T3, &m.Y3, &m.G1, &m.G2};
     for (int q = 0; q < 7; ++q)
         if ((rc = arena_alloc(ctx, fb[q], PN * m.NF))) return rc;
+    if ((rc = arena_alloc(ctx, &m.rowstart, (size_t)nt * (PN + 1)))) return rc;
+    if ((rc = arena_alloc(ctx, &m.rowaddr, PN * m.nsel))) return rc;
+    if ((rc = arena_alloc(ctx, &m.row_bsum, (size_t)nt * ((PN + 1023) / 1024)))) return rc;
+    if ((rc = arena_alloc(ctx, &m.cpart, PN * 9))) return rc;
+    m.tc_emb_ready = true;
     CK(cudaMemsetAsync(m.overflow, 0, sizeof(int), ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));     // host staging vectors go out of scope below
     tc_setup_maps(m, nt);        // tensor-core fitting path (falls back to the CUDA-core GEMMs only if unsupported widths)
@@ -727,6 +746,12 @@ int pimd_set_fitting_path(pimd_ctx* ctx, int use_tensor_cores) {
     if (use_tensor_cores && ctx->model.set && !ctx->model.tc_ready)
         return fail(ctx, PIMD_EINVAL, "tensor-core path unavailable for this architecture (needs fit width 240)");
     ctx->model.use_tc = use_tensor_cores != 0;
+    return PIMD_OK;
+}
+
+int pimd_set_embedding_path(pimd_ctx* ctx, int use_tensor_cores) {
+    if (!ctx) return PIMD_EINVAL;
+    ctx->model.use_tc_emb = use_tensor_cores != 0;
     return PIMD_OK;
 }
 

@@ -105,6 +105,14 @@ struct Model {
                 mapA_T3[PIMD_MAX_TYPES];
     CUtensorMap mapB_fwd[PIMD_MAX_TYPES][3];   // W_l^T  [out][in]
     CUtensorMap mapB_bwd[PIMD_MAX_TYPES][3];   // W_l    [in][out]
+    // tensor-core embedding path (embedding_tc.cu)
+    bool     use_tc_emb = true;
+    bool     tc_emb_ready = false;
+    uint8_t* emb_img = nullptr;        // [ntypes*ntypes][emb_tc_image_bytes()] shared-memory images of the nets
+    int*     rowstart = nullptr;       // [ntypes][PN+1] exclusive scan of ncount[.][tj] over type-sorted centres
+    int*     rowaddr = nullptr;        // [PN*nsel] compact row -> slot index
+    int*     row_bsum = nullptr;       // [ntypes][ceil(PN/1024)] scan block sums
+    double*  cpart = nullptr;          // [PN][9] per-centre virial share
 };
 
 struct ForceArgs {
@@ -124,6 +132,11 @@ int fitting_forward_backward(Model& m, const ForceArgs& a, cudaStream_t s);
 int embedding_backward(Model& m, const ForceArgs& a, int n_sms, cudaStream_t s);
 size_t embedding_smem_bytes(const Model& m, int ntypes);
 bool tc_setup_maps(Model& m, int ntypes);
+size_t emb_tc_image_bytes();
+void emb_tc_build_image(const double* w_pair, uint8_t* img);
+int emb_tc_row_index(Model& m, const ForceArgs& a, cudaStream_t s);
+int embedding_forward_tc(Model& m, const ForceArgs& a, int n_sms, cudaStream_t s);
+int embedding_backward_tc(Model& m, const ForceArgs& a, int n_sms, cudaStream_t s);
 int debug_tc_gemm(int M, int N, int K, const float* A_dev, const float* Bt_dev, float* C_dev, cudaStream_t s);
 
 }  // namespace pimd

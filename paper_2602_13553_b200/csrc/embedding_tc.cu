@@ -1,0 +1,792 @@
+// embedding_tc.cu -- F3 and F5/F6 of SURVEY 8(a) on the 5th-generation tensor cores (tcgen05 + TMEM).
+//
+// Neighbour rows are processed in tiles of 128 rows of ONE ordered type pair (t_i, t_j) -- one weight set,
+// resident in shared memory as ready-made UMMA B operands (hi / lo TF32 split, 128B-swizzled K-major,
+// bias folded in as an extra K row).  One thread owns one row (= one TMEM lane):
+//   h1 = tanh(s W1 + b1)                  CUDA cores (K = 1)
+//   z2 = [h1,1] W2b   (128 x 64 x 32)     tcgen05.mma kind::tf32, 3xTF32: a_hi b_hi + a_lo b_hi + a_hi b_lo
+//   h2 = [h1,h1] + tanh(z2)               epilogue: tcgen05.ld -> registers -> next A operand in smem
+//   z3 = [h2,1] W3b   (128 x 112 x 56)
+//   G  = [h2,h2] + tanh(z3)                                                                    (R-13)
+// Forward:  T_i += (1/N_sel) sum_rows G (x) R  (R-14): G tile through smem, thread <-> (4 m, 26 rows),
+//           red.global.add.v4.f32 on centre change.
+// Backward: forward-mode -- the derivative rows h' = dh/ds go through the same weights (bias column 0):
+//           G' = [h2',h2'] + (1 - tanh^2 z3) z3';  ds = sum_n (dT_n . R) G'_n;  dR_c = sum_n dT_nc G_n;
+//           pair gradient g = dU/dd (R-16), F_j -= g (f64 atomics), F_i and the virial share by a
+//           segmented warp reduction over the rows of one centre.
+// A CTA runs two independent 128-thread contexts (warpgroups), each with its own A-operand region, TMEM
+// columns and mbarrier, so that one context's MMAs overlap the other's tanh / epilogue work.
+#include <cstring>
+#include "common.cuh"
+#include "tc_gemm.cuh"
+
+namespace pimd {
+
+using namespace tc;
+
+namespace etc {
+constexpr int E1 = 25, E2 = 50, M1 = 100;
+constexpr int K2 = 32;                 // layer-2 K: 25 inputs + bias row + zero padding
+constexpr int N2 = 64;                 // layer-2 N: 50 outputs padded
+constexpr int K3 = 56;                 // layer-3 K: 50 inputs + bias row + padding (7 k-steps of 8)
+constexpr int N3 = 112;                // layer-3 N: 100 outputs padded
+// weight image of one (t_i, t_j) pair, bytes
+constexpr int oW2hi = 0, oW2lo = N2 * 128;                       // [64][32] f32, 128 B rows, SW128
+constexpr int kW3blk = N3 * 128;                                 // one K-block of 32: [112][32]
+constexpr int oW3hi = 2 * N2 * 128, oW3lo = oW3hi + 2 * kW3blk;
+constexpr int oW1 = oW3lo + 2 * kW3blk;                          // W1[32], b1[32] plain floats
+constexpr int kImgBytes = oW1 + 256;                             // 73984
+constexpr int kImgPad = (kImgBytes + 1023) / 1024 * 1024;        // 74752
+// per-context shared memory
+constexpr int kABlk = 128 * 128;                                 // one K-block of 32 for 128 rows: 16 KB
+constexpr int oRs = 4 * kABlk;                                   // float4 R[128]
+constexpr int oCen = oRs + 128 * 16;                             // int centre[128]
+constexpr int kCtxBytes = (oCen + 128 * 4 + 1023) / 1024 * 1024; // 68608
+constexpr int kSmemBytes = kImgPad + 2 * kCtxBytes + 64 + 1024;  // + barriers + alignment slack
+constexpr int kThreads = 256;
+constexpr int kScanBlock = 1024;       // centres per scan block
+}  // namespace etc
+
+struct EmbTcArgs {
+    int PN, N, ntypes, nsel;
+    int seloff[PIMD_MAX_TYPES + 1];
+    int type_row0[PIMD_MAX_TYPES + 1];
+    int n_of_type[PIMD_MAX_TYPES];
+    const int* rowstart;       // [ntypes][PN+1]  exclusive scan over type-sorted centres of ncount[.][tj]
+    const int* rowaddr;        // [PN*nsel]       compact row -> slot index (ba*nsel + seloff[tj] + q)
+    const int* row_of;         // [PN]            ba -> type-sorted centre row r
+    const NeighSlotA* slotA;
+    const NeighSlotB* slotB;
+    const uint8_t* wimg;       // [ntypes*ntypes][kImgBytes]
+    float* Tm;                 // [PN][100][4]  (zeroed before the forward kernel)
+    const float* dTm;
+    double* f;                 // [P][N][3]
+    double* cpart;             // [PN][9] per-centre virial share (zeroed before the backward kernel)
+    float inv_nsel;
+};
+
+// -------------------------------------------------------------------------------------------------
+// row bookkeeping: exclusive scan of the neighbour counts in type-sorted centre order, slot index per row
+// -------------------------------------------------------------------------------------------------
+struct SelOff { int v[PIMD_MAX_TYPES + 1]; };
+
+__global__ void __launch_bounds__(256)
+row_block_sums_kernel(int PN, int ntypes, const int* __restrict__ cen_idx, const int* __restrict__ ncount,
+                      int* __restrict__ bsum) {
+    const int tj = blockIdx.y, b = blockIdx.x;
+    int s = 0;
+    for (int q = threadIdx.x; q < etc::kScanBlock; q += 256) {
+        const int r = b * etc::kScanBlock + q;
+        if (r < PN) s += ncount[(size_t)cen_idx[r] * ntypes + tj];
+    }
+    __shared__ int red[8];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int t = 0;
+        for (int w = 0; w < 8; ++w) t += red[w];
+        bsum[tj * gridDim.x + b] = t;
+    }
+}
+
+__global__ void __launch_bounds__(256)
+row_scan_fill_kernel(int PN, int ntypes, int nsel, SelOff so, const int* __restrict__ cen_idx,
+                     const int* __restrict__ ncount, const int* __restrict__ bsum, int* __restrict__ rowstart,
+                     int* __restrict__ rowaddr) {
+    const int* seloff = so.v;
+    const int tj = blockIdx.y, b = blockIdx.x, nblk = gridDim.x;
+    __shared__ int red[8];
+    __shared__ int s_start[etc::kScanBlock], s_cnt[etc::kScanBlock], s_ba[etc::kScanBlock];
+    __shared__ int s_off;
+    // offset of this block = sum of the block sums before it
+    int s = 0;
+    for (int q = threadIdx.x; q < b; q += 256) s += bsum[tj * nblk + q];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int t = 0;
+        for (int w = 0; w < 8; ++w) t += red[w];
+        s_off = t;
+    }
+    __syncthreads();
+    // each thread owns 4 consecutive centres
+    const int r0 = b * etc::kScanBlock + threadIdx.x * 4;
+    int c[4], ba[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const int r = r0 + q;
+        ba[q] = (r < PN) ? cen_idx[r] : 0;
+        c[q] = (r < PN) ? ncount[(size_t)ba[q] * ntypes + tj] : 0;
+    }
+    const int mine = c[0] + c[1] + c[2] + c[3];
+    int incl = mine;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, incl, o);
+        if ((threadIdx.x & 31) >= o) incl += t;
+    }
+    __syncthreads();
+    if ((threadIdx.x & 31) == 31) red[threadIdx.x >> 5] = incl;
+    __syncthreads();
+    int woff = 0;
+    for (int w = 0; w < (int)(threadIdx.x >> 5); ++w) woff += red[w];
+    int run = s_off + woff + incl - mine;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const int r = r0 + q;
+        s_start[threadIdx.x * 4 + q] = run;
+        s_cnt[threadIdx.x * 4 + q] = c[q];
+        s_ba[threadIdx.x * 4 + q] = ba[q];
+        if (r < PN) rowstart[(size_t)tj * (PN + 1) + r] = run;
+        run += c[q];
+        if (r == PN - 1) rowstart[(size_t)tj * (PN + 1) + PN] = run;
+    }
+    __syncthreads();
+    // slot index of every compact row: one warp per centre, coalesced
+    int* out = rowaddr + (size_t)PN * seloff[tj];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (int q = warp; q < etc::kScanBlock; q += 8) {
+        const int n = s_cnt[q];
+        const int base = s_ba[q] * nsel + seloff[tj];
+        for (int e = lane; e < n; e += 32) out[s_start[q] + e] = base + e;
+    }
+}
+
+// fast tanh = 1 - 2 / (1 + e^{2x}); two MUFU ops (ex2, rcp), absolute error ~1e-7
+__device__ __forceinline__ float tanh_fast(float x) {
+    float e, r;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(x * 2.8853900817779268f));
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(e + 1.0f));
+    return fmaf(-2.0f, r, 1.0f);
+}
+
+__device__ __forceinline__ float tf32_hi(float v) { return __uint_as_float(__float_as_uint(v) & 0xFFFFE000u); }
+
+// store 4 consecutive K elements (one 16-byte chunk) of row `row` into the hi and lo copies of a
+// 128B-swizzled K-major operand block (128 rows x 32 floats)
+__device__ __forceinline__ void store_chunk(uint8_t* blk_hi, uint8_t* blk_lo, int row, int chunk, float a, float b,
+                                            float c, float d) {
+    const int off = row * 128 + ((chunk ^ (row & 7)) << 4);
+    const float ah = tf32_hi(a), bh = tf32_hi(b), ch = tf32_hi(c), dh = tf32_hi(d);
+    *reinterpret_cast<float4*>(blk_hi + off) = make_float4(ah, bh, ch, dh);
+    *reinterpret_cast<float4*>(blk_lo + off) = make_float4(a - ah, b - bh, c - ch, d - dh);
+}
+
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+
+__device__ __forceinline__ void red_add_v4(float* addr, float a, float b, float c, float d) {
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
+}
+
+// 3xTF32 product of one A operand (hi/lo blocks) with one B operand (hi/lo blocks) over `nks` k-steps of
+// one 32-float K-block; `first` = this is the first k-step of the accumulation
+__device__ __forceinline__ void mma_block_3x(uint32_t d_tmem, uint32_t a_hi, uint32_t a_lo, uint32_t b_hi, uint32_t b_lo,
+                                             uint32_t idesc, int nks, bool first) {
+    for (int ks = 0; ks < nks; ++ks) {
+        const uint64_t dah = make_smem_desc_kmajor(a_hi + ks * 32, 128), dal = make_smem_desc_kmajor(a_lo + ks * 32, 128);
+        const uint64_t dbh = make_smem_desc_kmajor(b_hi + ks * 32, 128), dbl = make_smem_desc_kmajor(b_lo + ks * 32, 128);
+        umma_tf32(d_tmem, dah, dbh, idesc, (first && ks == 0) ? 0u : 1u);
+        umma_tf32(d_tmem, dal, dbh, idesc, 1u);
+        umma_tf32(d_tmem, dah, dbl, idesc, 1u);
+    }
+}
+
+// per-row inputs, prefetched one tile ahead
+struct RowIn {
+    float dx, dy, dz, s, ds, rinv;
+    uint32_t jcode;
+    int cen;          // type-sorted centre row r, -1 for a row past the end of the pair
+    int ba;           // centre bead-atom k*N + i
+};
+
+__device__ __forceinline__ RowIn load_row(const EmbTcArgs& a, int addr) {
+    RowIn r;
+    if (addr < 0) {
+        r.dx = r.dy = r.dz = r.s = r.ds = 0.f; r.rinv = 1.f; r.jcode = 0u; r.cen = -1; r.ba = 0;
+        return r;
+    }
+    const float4 A = __ldg(reinterpret_cast<const float4*>(a.slotA) + addr);
+    const float4 B = __ldg(reinterpret_cast<const float4*>(a.slotB) + addr);
+    r.dx = A.x; r.dy = A.y; r.dz = A.z; r.s = A.w;
+    r.ds = B.x; r.rinv = B.y; r.jcode = __float_as_uint(B.z);
+    r.ba = addr / a.nsel;
+    r.cen = __ldg(a.row_of + r.ba);
+    return r;
+}
+
+struct CtxSetup {
+    uint8_t* smem;       // 1024-aligned base
+    uint8_t* ctx;        // this context's region
+    uint64_t* mma_bar;
+    uint32_t tmem_base;  // allocation base (all contexts)
+};
+
+// common prologue: barriers, TMEM allocation of `ncols` columns; returns after a CTA-wide sync
+__device__ __forceinline__ CtxSetup ctx_setup(uint8_t* smem_raw, uint32_t ncols) {
+    CtxSetup c;
+    c.smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    const int wg = threadIdx.x >> 7;
+    c.ctx = c.smem + etc::kImgPad + wg * etc::kCtxBytes;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(c.smem + etc::kImgPad + 2 * etc::kCtxBytes);
+    c.mma_bar = bars + wg;
+    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(bars + 2);
+    if (threadIdx.x == 0) {
+        mbar_init(bars, 1);
+        mbar_init(bars + 1, 1);
+        fence_barrier_init();
+    }
+    if ((threadIdx.x >> 5) == 0) tmem_alloc(tmem_ptr, ncols);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    c.tmem_base = *tmem_ptr;
+    return c;
+}
+
+__device__ __forceinline__ void load_weight_image(uint8_t* dst, const uint8_t* src) {
+    const float4* s4 = reinterpret_cast<const float4*>(src);
+    float4* d4 = reinterpret_cast<float4*>(dst);
+    for (int q = threadIdx.x; q < etc::kImgBytes / 16; q += etc::kThreads) d4[q] = __ldg(s4 + q);
+    fence_proxy_async_smem();
+}
+
+// -------------------------------------------------------------------------------------------------
+// F3: embedding forward + T_i
+// -------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(etc::kThreads, 1)
+embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
+    using namespace etc;
+    extern __shared__ uint8_t smem_raw[];
+    const CtxSetup cs = ctx_setup(smem_raw, 256);
+    const int wg = threadIdx.x >> 7, t = threadIdx.x & 127;
+    uint8_t* ctx = cs.ctx;
+    float4* Rs = reinterpret_cast<float4*>(ctx + oRs);
+    int* cen_s = reinterpret_cast<int*>(ctx + oCen);
+    float* Gs = reinterpret_cast<float*>(ctx);
+    const float* W1s = reinterpret_cast<const float*>(cs.smem + oW1);
+    const float* b1s = W1s + 32;
+    const uint32_t tmem_d = cs.tmem_base + wg * 128;
+    const uint32_t lanefield = ((uint32_t)((t >> 5) * 32)) << 16;
+    const uint32_t actx = smem_u32(ctx), wbase = smem_u32(cs.smem);
+    constexpr uint32_t idesc2 = make_idesc_tf32(128, N2), idesc3 = make_idesc_tf32(128, N3);
+    uint32_t phase = 0;
+    const int nt = a.ntypes;
+
+    for (int p = 0; p < nt * nt; ++p) {
+        const int ti = p / nt, tj = p - ti * nt;
+        __syncthreads();                                   // both contexts are done with the previous weights
+        load_weight_image(cs.smem, a.wimg + (size_t)p * kImgBytes);
+        __syncthreads();
+        const int* rs = a.rowstart + (size_t)tj * (a.PN + 1);
+        const int begin = rs[a.type_row0[ti]], end = rs[a.type_row0[ti + 1]];
+        const int ntile = (end - begin + 127) >> 7;
+        const int C = gridDim.x * 2, c = blockIdx.x * 2 + wg;
+        const int tl0 = (int)((long long)ntile * c / C), tl1 = (int)((long long)ntile * (c + 1) / C);
+        if (tl0 >= tl1) continue;
+        const int* raddr = a.rowaddr + (size_t)a.PN * a.seloff[tj];
+        // software pipeline: slot index two tiles ahead, row data one tile ahead
+        auto addr_of = [&](int tile) -> int {
+            const int g = begin + tile * 128 + t;
+            return (tile < tl1 && g < end) ? __ldg(raddr + g) : -1;
+        };
+        RowIn cur = load_row(a, addr_of(tl0));
+        int addr_n1 = addr_of(tl0 + 1);
+
+        for (int tile = tl0; tile < tl1; ++tile) {
+            const int addr_n2 = addr_of(tile + 2);
+            const RowIn nxt = load_row(a, addr_n1);
+            addr_n1 = addr_n2;
+
+            const float s = cur.s, sr = cur.s * cur.rinv;
+            Rs[t] = make_float4(s, sr * cur.dx, sr * cur.dy, sr * cur.dz);
+            cen_s[t] = cur.cen;
+            // ---- layer 1 on CUDA cores, A1 = [h1, 1, 0...] ----
+            float h1[E1];
+#pragma unroll
+            for (int k = 0; k < E1; ++k) h1[k] = tanh_fast(fmaf(s, W1s[k], b1s[k]));
+#pragma unroll
+            for (int ch = 0; ch < 8; ++ch) {
+                float v[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int k = 4 * ch + j;
+                    v[j] = (k < E1) ? h1[k < E1 ? k : 0] : (k == E1 ? 1.f : 0.f);
+                }
+                store_chunk(ctx, ctx + kABlk, t, ch, v[0], v[1], v[2], v[3]);
+            }
+            fence_proxy_async_smem();
+            tc_fence_before();
+            named_bar_sync(1 + wg, 128);
+            if (t == 0) {
+                tc_fence_after();
+                mma_block_3x(tmem_d, actx, actx + kABlk, wbase + oW2hi, wbase + oW2lo, idesc2, 4, true);
+                umma_commit(cs.mma_bar);
+            }
+            mbar_wait(cs.mma_bar, phase);
+            phase ^= 1;
+            tc_fence_after();
+            // ---- epilogue 2: h2 = [h1,h1] + tanh(z2); A2 = [h2, 1, 0...] (two K-blocks; overlays A1) ----
+            float h2[E2];
+#pragma unroll
+            for (int cc = 0; cc < 4; ++cc) {
+                uint32_t v[16];
+                tmem_ld16(tmem_d + lanefield + cc * 16, v);
+                tmem_ld_wait();
+                float o[16];
+#pragma unroll
+                for (int q = 0; q < 16; ++q) {
+                    const int n = cc * 16 + q;
+                    if (n < E2) {
+                        h2[n] = h1[n % E1] + tanh_fast(__uint_as_float(v[q]));
+                        o[q] = h2[n];
+                    } else {
+                        o[q] = (n == E2) ? 1.f : 0.f;
+                    }
+                }
+                uint8_t* bh = ctx + (cc >> 1) * kABlk;
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+                    store_chunk(bh, bh + 2 * kABlk, t, (cc & 1) * 4 + j, o[4 * j], o[4 * j + 1], o[4 * j + 2], o[4 * j + 3]);
+            }
+            fence_proxy_async_smem();
+            tc_fence_before();
+            named_bar_sync(1 + wg, 128);
+            if (t == 0) {
+                tc_fence_after();
+                mma_block_3x(tmem_d, actx, actx + 2 * kABlk, wbase + oW3hi, wbase + oW3lo, idesc3, 4, true);
+                mma_block_3x(tmem_d, actx + kABlk, actx + 3 * kABlk, wbase + oW3hi + kW3blk, wbase + oW3lo + kW3blk, idesc3,
+                             3, false);
+                umma_commit(cs.mma_bar);
+            }
+            mbar_wait(cs.mma_bar, phase);
+            phase ^= 1;
+            tc_fence_after();
+            // ---- epilogue 3: G = [h2,h2] + tanh(z3) -> smem [row][100] (overlays the A region) ----
+#pragma unroll
+            for (int cc = 0; cc < 7; ++cc) {
+                uint32_t v[16];
+                tmem_ld16(tmem_d + lanefield + cc * 16, v);
+                tmem_ld_wait();
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int n = cc * 16 + 4 * j;
+                    if (n < M1) {
+                        float4 gq;
+                        gq.x = h2[n % E2] + tanh_fast(__uint_as_float(v[4 * j]));
+                        gq.y = h2[(n + 1) % E2] + tanh_fast(__uint_as_float(v[4 * j + 1]));
+                        gq.z = h2[(n + 2) % E2] + tanh_fast(__uint_as_float(v[4 * j + 2]));
+                        gq.w = h2[(n + 3) % E2] + tanh_fast(__uint_as_float(v[4 * j + 3]));
+                        *reinterpret_cast<float4*>(Gs + t * M1 + n) = gq;
+                    }
+                }
+            }
+            tc_fence_before();
+            named_bar_sync(1 + wg, 128);
+            // ---- T_i += (1/N_sel) sum_rows G (x) R : thread <-> (4 consecutive m, 26 rows) ----
+            if (t < 125) {
+                const int mq = t % 25, grp = t / 25;
+                const int r_lo = grp * 26, r_hi = min(128, r_lo + 26);
+                float acc[16];
+#pragma unroll
+                for (int q = 0; q < 16; ++q) acc[q] = 0.f;
+                int curc = -1;
+                auto flush = [&]() {
+                    float* dst = a.Tm + ((size_t)curc * M1 + 4 * mq) * 4;
+#pragma unroll
+                    for (int j = 0; j < 4; ++j)
+                        red_add_v4(dst + 4 * j, acc[4 * j] * a.inv_nsel, acc[4 * j + 1] * a.inv_nsel,
+                                   acc[4 * j + 2] * a.inv_nsel, acc[4 * j + 3] * a.inv_nsel);
+                };
+                for (int row = r_lo; row < r_hi; ++row) {
+                    const int cn = cen_s[row];
+                    if (cn != curc) {
+                        if (curc >= 0) flush();
+#pragma unroll
+                        for (int q = 0; q < 16; ++q) acc[q] = 0.f;
+                        curc = cn;
+                    }
+                    if (cn < 0) continue;
+                    const float4 G4 = *reinterpret_cast<const float4*>(Gs + row * M1 + 4 * mq);
+                    const float4 R = Rs[row];
+                    const float gv[4] = {G4.x, G4.y, G4.z, G4.w};
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        acc[4 * j] = fmaf(gv[j], R.x, acc[4 * j]);
+                        acc[4 * j + 1] = fmaf(gv[j], R.y, acc[4 * j + 1]);
+                        acc[4 * j + 2] = fmaf(gv[j], R.z, acc[4 * j + 2]);
+                        acc[4 * j + 3] = fmaf(gv[j], R.w, acc[4 * j + 3]);
+                    }
+                }
+                if (curc >= 0) flush();
+            }
+            named_bar_sync(1 + wg, 128);                   // G / R / centre buffers are free again
+            cur = nxt;
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if ((threadIdx.x >> 5) == 0) tmem_dealloc(cs.tmem_base, 256);
+}
+
+// -------------------------------------------------------------------------------------------------
+// F5 / F6: embedding backward (forward-mode), pair gradient, force and virial
+// -------------------------------------------------------------------------------------------------
+constexpr int kDtStage = 40;          // centres whose dT fits the (free) A region: 40 x 1600 B
+
+__global__ void __launch_bounds__(etc::kThreads, 1)
+embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
+    using namespace etc;
+    extern __shared__ uint8_t smem_raw[];
+    const CtxSetup cs = ctx_setup(smem_raw, 512);
+    const int wg = threadIdx.x >> 7, t = threadIdx.x & 127, lane = threadIdx.x & 31;
+    uint8_t* ctx = cs.ctx;
+    int* cen_s = reinterpret_cast<int*>(ctx + oCen);
+    float4* dTs = reinterpret_cast<float4*>(ctx);
+    const float* W1s = reinterpret_cast<const float*>(cs.smem + oW1);
+    const float* b1s = W1s + 32;
+    const uint32_t tmem_v = cs.tmem_base + wg * 256, tmem_g = tmem_v + N3;     // value / derivative accumulators
+    const uint32_t lanefield = ((uint32_t)((t >> 5) * 32)) << 16;
+    const uint32_t actx = smem_u32(ctx), wbase = smem_u32(cs.smem);
+    constexpr uint32_t idesc2 = make_idesc_tf32(128, N2), idesc3 = make_idesc_tf32(128, N3);
+    uint32_t phase = 0;
+    const int nt = a.ntypes;
+
+    for (int p = 0; p < nt * nt; ++p) {
+        const int ti = p / nt, tj = p - ti * nt;
+        __syncthreads();
+        load_weight_image(cs.smem, a.wimg + (size_t)p * kImgBytes);
+        __syncthreads();
+        const int* rs = a.rowstart + (size_t)tj * (a.PN + 1);
+        const int begin = rs[a.type_row0[ti]], end = rs[a.type_row0[ti + 1]];
+        const int ntile = (end - begin + 127) >> 7;
+        const int C = gridDim.x * 2, c = blockIdx.x * 2 + wg;
+        const int tl0 = (int)((long long)ntile * c / C), tl1 = (int)((long long)ntile * (c + 1) / C);
+        if (tl0 >= tl1) continue;
+        const int* raddr = a.rowaddr + (size_t)a.PN * a.seloff[tj];
+        auto addr_of = [&](int tile) -> int {
+            const int g = begin + tile * 128 + t;
+            return (tile < tl1 && g < end) ? __ldg(raddr + g) : -1;
+        };
+        RowIn cur = load_row(a, addr_of(tl0));
+        int addr_n1 = addr_of(tl0 + 1);
+
+        for (int tile = tl0; tile < tl1; ++tile) {
+            const int addr_n2 = addr_of(tile + 2);
+            const RowIn nxt = load_row(a, addr_n1);
+            addr_n1 = addr_n2;
+
+            const float s = cur.s, sr = cur.s * cur.rinv;
+            const float R0 = s, R1 = sr * cur.dx, R2 = sr * cur.dy, R3 = sr * cur.dz;
+            cen_s[t] = cur.cen;
+            // ---- layer 1 and its s-derivative; A1v = [h1,1,0..], A1d = [h1',0,0..] ----
+            float h1[E1], h1p[E1];
+#pragma unroll
+            for (int k = 0; k < E1; ++k) {
+                const float w = W1s[k];
+                const float th = tanh_fast(fmaf(s, w, b1s[k]));
+                h1[k] = th;
+                h1p[k] = (1.f - th * th) * w;
+            }
+#pragma unroll
+            for (int ch = 0; ch < 8; ++ch) {
+                float v[4], d[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int k = 4 * ch + j;
+                    v[j] = (k < E1) ? h1[k < E1 ? k : 0] : (k == E1 ? 1.f : 0.f);
+                    d[j] = (k < E1) ? h1p[k < E1 ? k : 0] : 0.f;
+                }
+                store_chunk(ctx, ctx + kABlk, t, ch, v[0], v[1], v[2], v[3]);
+                store_chunk(ctx + 2 * kABlk, ctx + 3 * kABlk, t, ch, d[0], d[1], d[2], d[3]);
+            }
+            fence_proxy_async_smem();
+            tc_fence_before();
+            named_bar_sync(1 + wg, 128);
+            if (t == 0) {
+                tc_fence_after();
+                mma_block_3x(tmem_v, actx, actx + kABlk, wbase + oW2hi, wbase + oW2lo, idesc2, 4, true);
+                mma_block_3x(tmem_g, actx + 2 * kABlk, actx + 3 * kABlk, wbase + oW2hi, wbase + oW2lo, idesc2, 4, true);
+                umma_commit(cs.mma_bar);
+            }
+            mbar_wait(cs.mma_bar, phase);
+            phase ^= 1;
+            tc_fence_after();
+            // ---- epilogue 2: h2, h2'; A2v written now, A2d after MMA3v has consumed the region ----
+            float h2[E2], h2p[E2];
+#pragma unroll
+            for (int cc = 0; cc < 4; ++cc) {
+                uint32_t v[16], d[16];
+                tmem_ld16(tmem_v + lanefield + cc * 16, v);
+                tmem_ld16(tmem_g + lanefield + cc * 16, d);
+                tmem_ld_wait();
+                float o[16];
+#pragma unroll
+                for (int q = 0; q < 16; ++q) {
+                    const int n = cc * 16 + q;
+                    if (n < E2) {
+                        const float th = tanh_fast(__uint_as_float(v[q]));
+                        h2[n] = h1[n % E1] + th;
+                        h2p[n] = fmaf(1.f - th * th, __uint_as_float(d[q]), h1p[n % E1]);
+                        o[q] = h2[n];
+                    } else {
+                        o[q] = (n == E2) ? 1.f : 0.f;
+                    }
+                }
+                uint8_t* bh = ctx + (cc >> 1) * kABlk;
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+                    store_chunk(bh, bh + 2 * kABlk, t, (cc & 1) * 4 + j, o[4 * j], o[4 * j + 1], o[4 * j + 2], o[4 * j + 3]);
+            }
+            fence_proxy_async_smem();
+            tc_fence_before();
+            named_bar_sync(1 + wg, 128);
+            if (t == 0) {
+                tc_fence_after();
+                mma_block_3x(tmem_v, actx, actx + 2 * kABlk, wbase + oW3hi, wbase + oW3lo, idesc3, 4, true);
+                mma_block_3x(tmem_v, actx + kABlk, actx + 3 * kABlk, wbase + oW3hi + kW3blk, wbase + oW3lo + kW3blk, idesc3,
+                             3, false);
+                umma_commit(cs.mma_bar);
+            }
+            mbar_wait(cs.mma_bar, phase);                  // the other context works meanwhile
+            phase ^= 1;
+            tc_fence_after();
+#pragma unroll
+            for (int cc = 0; cc < 4; ++cc) {
+                float o[16];
+#pragma unroll
+                for (int q = 0; q < 16; ++q) {
+                    const int n = cc * 16 + q;
+                    o[q] = (n < E2) ? h2p[n < E2 ? n : 0] : 0.f;
+                }
+                uint8_t* bh = ctx + (cc >> 1) * kABlk;
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+                    store_chunk(bh, bh + 2 * kABlk, t, (cc & 1) * 4 + j, o[4 * j], o[4 * j + 1], o[4 * j + 2], o[4 * j + 3]);
+            }
+            fence_proxy_async_smem();
+            tc_fence_before();
+            named_bar_sync(1 + wg, 128);
+            if (t == 0) {
+                tc_fence_after();
+                mma_block_3x(tmem_g, actx, actx + 2 * kABlk, wbase + oW3hi, wbase + oW3lo, idesc3, 4, true);
+                mma_block_3x(tmem_g, actx + kABlk, actx + 3 * kABlk, wbase + oW3hi + kW3blk, wbase + oW3lo + kW3blk, idesc3,
+                             3, false);
+                umma_commit(cs.mma_bar);
+            }
+            mbar_wait(cs.mma_bar, phase);
+            phase ^= 1;
+            tc_fence_after();
+            // ---- stage dT of this tile's centres into the (now free) A region ----
+            const int nvalid = min(128, end - (begin + tile * 128));
+            const int r_lo = cen_s[0], r_hi = cen_s[nvalid - 1];
+            const int nstage = min(r_hi - r_lo + 1, kDtStage);
+            {
+                const float4* src = reinterpret_cast<const float4*>(a.dTm) + (size_t)r_lo * M1;
+                for (int q = t; q < nstage * M1; q += 128) dTs[q] = __ldg(src + q);
+            }
+            named_bar_sync(1 + wg, 128);
+            const int csl = cur.cen - r_lo;
+            const float4* dTp = (cur.cen >= 0 && csl < kDtStage)
+                                    ? dTs + csl * M1
+                                    : reinterpret_cast<const float4*>(a.dTm) + (size_t)max(cur.cen, 0) * M1;
+            // ---- epilogue 3: contract G, G' with dT on the fly ----
+            float ds = 0.f, dR0 = 0.f, dR1 = 0.f, dR2 = 0.f, dR3 = 0.f;
+#pragma unroll
+            for (int cc = 0; cc < 7; ++cc) {
+                uint32_t v[16], d[16];
+                tmem_ld16(tmem_v + lanefield + cc * 16, v);
+                tmem_ld16(tmem_g + lanefield + cc * 16, d);
+                tmem_ld_wait();
+#pragma unroll
+                for (int q = 0; q < 16; ++q) {
+                    const int n = cc * 16 + q;
+                    if (n < M1) {
+                        const float4 dT = dTp[n];
+                        const float th = tanh_fast(__uint_as_float(v[q]));
+                        const float G = h2[n % E2] + th;
+                        const float Gp = fmaf(1.f - th * th, __uint_as_float(d[q]), h2p[n % E2]);
+                        const float dG = fmaf(dT.x, R0, fmaf(dT.y, R1, fmaf(dT.z, R2, dT.w * R3)));
+                        ds = fmaf(dG, Gp, ds);
+                        dR0 = fmaf(dT.x, G, dR0); dR1 = fmaf(dT.y, G, dR1);
+                        dR2 = fmaf(dT.z, G, dR2); dR3 = fmaf(dT.w, G, dR3);
+                    }
+                }
+            }
+            tc_fence_before();
+            // ---- pair gradient g = dU/dd (R-16) ----
+            float red[12];
+            {
+                const float w = (cur.cen >= 0) ? a.inv_nsel : 0.f;
+                ds *= w; dR0 *= w; dR1 *= w; dR2 *= w; dR3 *= w;
+                const float rinv = cur.rinv;
+                const float dot = dR1 * cur.dx + dR2 * cur.dy + dR3 * cur.dz;
+                const float radial = (ds + dR0) * cur.ds + (cur.ds * rinv - s * rinv * rinv) * dot;
+                const float rr = radial * rinv;
+                const float gx = fmaf(rr, cur.dx, sr * dR1), gy = fmaf(rr, cur.dy, sr * dR2), gz = fmaf(rr, cur.dz, sr * dR3);
+                if (cur.cen >= 0) {
+                    const int j = (int)(cur.jcode & 0x7fffffu);
+                    double* fj = a.f + ((size_t)(cur.ba / a.N) * a.N + j) * 3;
+                    atomicAdd(fj, -(double)gx); atomicAdd(fj + 1, -(double)gy); atomicAdd(fj + 2, -(double)gz);
+                }
+                red[0] = gx; red[1] = gy; red[2] = gz;
+                const float dd[3] = {cur.dx, cur.dy, cur.dz}, gg[3] = {gx, gy, gz};
+#pragma unroll
+                for (int u = 0; u < 3; ++u)
+#pragma unroll
+                    for (int w2 = 0; w2 < 3; ++w2) red[3 + 3 * u + w2] = -dd[u] * gg[w2];
+            }
+            // segmented warp reduction over the rows of one centre (rows of a centre are contiguous)
+            const int key = cur.cen;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int ko = __shfl_down_sync(0xffffffffu, key, o);
+                const bool take = (lane + o < 32) && (ko == key);
+#pragma unroll
+                for (int q = 0; q < 12; ++q) {
+                    const float vo = __shfl_down_sync(0xffffffffu, red[q], o);
+                    if (take) red[q] += vo;
+                }
+            }
+            const int kprev = __shfl_up_sync(0xffffffffu, key, 1);
+            if (key >= 0 && (lane == 0 || kprev != key)) {
+                double* fi = a.f + (size_t)cur.ba * 3;
+                atomicAdd(fi, (double)red[0]); atomicAdd(fi + 1, (double)red[1]); atomicAdd(fi + 2, (double)red[2]);
+                double* cp = a.cpart + (size_t)key * 9;
+#pragma unroll
+                for (int q = 0; q < 9; ++q) atomicAdd(cp + q, (double)red[3 + q]);
+            }
+            named_bar_sync(1 + wg, 128);                   // dT stage / centre buffer are free again
+            cur = nxt;
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if ((threadIdx.x >> 5) == 0) tmem_dealloc(cs.tmem_base, 512);
+}
+
+// Xi^(k) = sum of the per-centre virial shares of bead k (one block per bead)
+__global__ void __launch_bounds__(256)
+virial_reduce_kernel(int ntypes, EmbTcArgs a, double* __restrict__ Xi) {
+    const int k = blockIdx.x;
+    double acc[9];
+#pragma unroll
+    for (int q = 0; q < 9; ++q) acc[q] = 0.0;
+    for (int tt = 0; tt < ntypes; ++tt) {
+        const int r0 = a.type_row0[tt] + k * a.n_of_type[tt];
+        for (int r = r0 + threadIdx.x; r < r0 + a.n_of_type[tt]; r += 256) {
+#pragma unroll
+            for (int q = 0; q < 9; ++q) acc[q] += a.cpart[(size_t)r * 9 + q];
+        }
+    }
+    __shared__ double red[8][9];
+#pragma unroll
+    for (int q = 0; q < 9; ++q)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) acc[q] += __shfl_xor_sync(0xffffffffu, acc[q], o);
+    if ((threadIdx.x & 31) == 0)
+        for (int q = 0; q < 9; ++q) red[threadIdx.x >> 5][q] = acc[q];
+    __syncthreads();
+    if (threadIdx.x < 9) {
+        double s = 0.0;
+        for (int w = 0; w < 8; ++w) s += red[w][threadIdx.x];
+        Xi[k * 9 + threadIdx.x] = s;
+    }
+}
+
+// -------------------------------------------------------------------------------------------------
+// host side
+// -------------------------------------------------------------------------------------------------
+size_t emb_tc_image_bytes() { return etc::kImgBytes; }
+
+// Builds the shared-memory image of one (t_i, t_j) embedding net from its packed FP64 weights
+// (W1[1][25], b1[25], W2[25][50], b2[50], W3[50][100], b3[100], row-major in x out).
+void emb_tc_build_image(const double* w, uint8_t* img) {
+    using namespace etc;
+    memset(img, 0, kImgBytes);
+    const double* W1 = w;
+    const double* b1 = W1 + E1;
+    const double* W2 = b1 + E1;
+    const double* b2 = W2 + E1 * E2;
+    const double* W3 = b2 + E2;
+    const double* b3 = W3 + E2 * M1;
+    auto put = [&](int o_hi, int o_lo, int nrows, int n, int k, float v) {
+        const int kb = k / 32, kk = k % 32;
+        const int off = kb * nrows * 128 + n * 128 + (((kk >> 2) ^ (n & 7)) << 4) + (kk & 3) * 4;
+        uint32_t bits;
+        memcpy(&bits, &v, 4);
+        bits &= 0xFFFFE000u;
+        float hi;
+        memcpy(&hi, &bits, 4);
+        const float lo = v - hi;
+        memcpy(img + o_hi + off, &hi, 4);
+        memcpy(img + o_lo + off, &lo, 4);
+    };
+    for (int n = 0; n < E2; ++n) {
+        for (int k = 0; k < E1; ++k) put(oW2hi, oW2lo, N2, n, k, (float)W2[k * E2 + n]);
+        put(oW2hi, oW2lo, N2, n, E1, (float)b2[n]);
+    }
+    for (int n = 0; n < M1; ++n) {
+        for (int k = 0; k < E2; ++k) put(oW3hi, oW3lo, N3, n, k, (float)W3[k * M1 + n]);
+        put(oW3hi, oW3lo, N3, n, E2, (float)b3[n]);
+    }
+    float* l1 = reinterpret_cast<float*>(img + oW1);
+    for (int k = 0; k < E1; ++k) { l1[k] = (float)W1[k]; l1[32 + k] = (float)b1[k]; }
+}
+
+static EmbTcArgs make_tc_args(Model& m, const ForceArgs& fa) {
+    EmbTcArgs a;
+    a.PN = fa.P * fa.N; a.N = fa.N; a.ntypes = fa.ntypes; a.nsel = m.nsel;
+    for (int t = 0; t <= PIMD_MAX_TYPES; ++t) { a.seloff[t] = m.seloff[t]; a.type_row0[t] = m.type_row0[t]; }
+    for (int t = 0; t < PIMD_MAX_TYPES; ++t) a.n_of_type[t] = (t < fa.ntypes) ? m.n_of_type[t] : 0;
+    a.rowstart = m.rowstart; a.rowaddr = m.rowaddr; a.row_of = m.row_of;
+    a.slotA = m.slotA; a.slotB = m.slotB; a.wimg = m.emb_img;
+    a.Tm = m.Tm; a.dTm = m.dTm; a.f = fa.f; a.cpart = m.cpart;
+    a.inv_nsel = 1.0f / (float)m.nsel;
+    return a;
+}
+
+// after neighbor_build: compact-row bookkeeping for the tensor-core embedding kernels
+int emb_tc_row_index(Model& m, const ForceArgs& fa, cudaStream_t s) {
+    const int PN = fa.P * fa.N;
+    const int nblk = (PN + etc::kScanBlock - 1) / etc::kScanBlock;
+    SelOff so;
+    for (int t = 0; t <= PIMD_MAX_TYPES; ++t) so.v[t] = m.seloff[t];
+    dim3 grid(nblk, fa.ntypes);
+    row_block_sums_kernel<<<grid, 256, 0, s>>>(PN, fa.ntypes, m.cen_idx, m.ncount, m.row_bsum);
+    row_scan_fill_kernel<<<grid, 256, 0, s>>>(PN, fa.ntypes, m.nsel, so, m.cen_idx, m.ncount, m.row_bsum, m.rowstart,
+                                              m.rowaddr);
+    return 2;
+}
+
+int embedding_forward_tc(Model& m, const ForceArgs& fa, int n_sms, cudaStream_t s) {
+    EmbTcArgs a = make_tc_args(m, fa);
+    static bool attr = false;
+    if (!attr) {
+        cudaFuncSetAttribute(embed_fwd_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, etc::kSmemBytes);
+        attr = true;
+    }
+    cudaMemsetAsync(m.Tm, 0, sizeof(float) * (size_t)a.PN * etc::M1 * 4, s);
+    embed_fwd_tc_kernel<<<n_sms, etc::kThreads, etc::kSmemBytes, s>>>(a);
+    return 1;
+}
+
+int embedding_backward_tc(Model& m, const ForceArgs& fa, int n_sms, cudaStream_t s) {
+    EmbTcArgs a = make_tc_args(m, fa);
+    static bool attr = false;
+    if (!attr) {
+        cudaFuncSetAttribute(embed_bwd_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, etc::kSmemBytes);
+        attr = true;
+    }
+    cudaMemsetAsync(m.cpart, 0, sizeof(double) * (size_t)a.PN * 9, s);
+    embed_bwd_tc_kernel<<<n_sms, etc::kThreads, etc::kSmemBytes, s>>>(a);
+    virial_reduce_kernel<<<fa.P, 256, 0, s>>>(fa.ntypes, a, fa.Xi);
+    return 2;
+}
+
+}  // namespace pimd

@@ -294,3 +294,23 @@ def test_tensor_core_and_cuda_core_fitting_paths_agree(pk):
     frms = np.sqrt((out[1][0] ** 2).mean())
     assert np.abs(out[0][0] - out[1][0]).max() <= 2e-5 * frms
     assert np.abs(out[0][1] - out[1][1]).max() <= 1e-6 * 1e3
+
+
+def test_tensor_core_and_cuda_core_embedding_paths_agree(pk):
+    """embedding_tc.cu (tcgen05, 3xTF32, fast tanh) against the FP32 CUDA-core embedding kernels: forces, atom
+    energies and virial of configs[0] (multi-image neighbours, ragged last tiles of all four type pairs)."""
+    cfg, wb, desc, w = workloads.make_config(0)
+    w = workloads.model_weights(desc, cfg["weight_seed"], last_layer_scale=1.0e3)
+    out = []
+    for use_tc in (1, 0):
+        sim = pk.PIMD(wb["types"], wb["masses"], wb["box"], cfg["P"], cfg["T"], cfg["dt"], cfg["gamma"], seed=0,
+                      model_desc=desc)
+        sim.set_model(w)
+        pk.pimd_set_embedding_path(sim.ctx, use_tc)
+        sim.set_state(wb["x"], wb["p"])
+        out.append((sim.forces(), sim.atom_energies(), sim.virial()))
+        sim.close()
+    frms = np.sqrt((out[1][0] ** 2).mean())
+    assert np.abs(out[0][0] - out[1][0]).max() <= 5e-5 * frms
+    assert np.abs(out[0][1] - out[1][1]).max() <= 1e-6 * 1e3
+    assert np.abs(out[0][2] - out[1][2]).max() <= 5e-5 * np.abs(out[1][2]).max()
