@@ -225,6 +225,7 @@ def run_ours(args):
     dom = max(("embed_fwd", "fitting", "embed_bwd"), key=lambda n: phases[n])
     # tensor roofline: the path's contractions run as kind::tf32 tcgen05.mma; TF32 dense peak = the measured
     # BF16 cuBLAS figure (sustained: these kernels are timed inside a long step) x the guide's nominal 1/2
+    PN = P * N
     bf16_peak = peaks["bf16_sustained"] or peaks["bf16"]
     tf32_peak = 0.5 * bf16_peak
     mufu_peak = 148 * 16 * peaks["sm_max_mhz"] * 1e6 / 1e12                         # T MUFU op/s

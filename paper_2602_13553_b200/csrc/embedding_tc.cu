@@ -230,7 +230,9 @@ struct CtxSetup {
 // common prologue: barriers, TMEM allocation of `ncols` columns; returns after a CTA-wide sync
 __device__ __forceinline__ CtxSetup ctx_setup(uint8_t* smem_raw, uint32_t ncols) {
     CtxSetup c;
-    c.smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    // pad to 1024 B by pointer arithmetic on the __shared__ array (a uintptr_t round trip loses the address
+    // space and turns every access into a generic LD/ST)
+    c.smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
     const int wg = threadIdx.x >> 7;
     c.ctx = c.smem + etc::kImgPad + wg * etc::kCtxBytes;
     uint64_t* bars = reinterpret_cast<uint64_t*>(c.smem + etc::kImgPad + 2 * etc::kCtxBytes);
@@ -264,7 +266,7 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
     using namespace etc;
     extern __shared__ uint8_t smem_raw[];
     const CtxSetup cs = ctx_setup(smem_raw, 256);
-    const int wg = threadIdx.x >> 7, t = threadIdx.x & 127;
+    const int wg = threadIdx.x >> 7, t = threadIdx.x & 127, lane = threadIdx.x & 31;
     uint8_t* ctx = cs.ctx;
     float4* Rs = reinterpret_cast<float4*>(ctx + oRs);
     int* cen_s = reinterpret_cast<int*>(ctx + oCen);
@@ -387,33 +389,34 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
                 }
             }
             tc_fence_before();
-            named_bar_sync(1 + wg, 128);
-            // ---- T_i += (1/N_sel) sum_rows G (x) R : thread <-> (4 consecutive m, 26 rows) ----
-            if (t < 125) {
-                const int mq = t % 25, grp = t / 25;
-                const int r_lo = grp * 26, r_hi = min(128, r_lo + 26);
+            __syncwarp();
+            // ---- T_i += (1/N_sel) sum_rows G (x) R.  Warp w owns the 32 rows its own lanes just wrote (so a
+            // warp-level sync suffices); lane <-> 4 consecutive m (25 lanes).  All lanes walk the same rows, so
+            // the centre changes are warp-uniform and R / centre reads are broadcasts. ----
+            if (lane < 25) {
+                const int r_lo = t & ~31;
                 float acc[16];
 #pragma unroll
                 for (int q = 0; q < 16; ++q) acc[q] = 0.f;
-                int curc = -1;
-                auto flush = [&]() {
-                    float* dst = a.Tm + ((size_t)curc * M1 + 4 * mq) * 4;
-#pragma unroll
-                    for (int j = 0; j < 4; ++j)
-                        red_add_v4(dst + 4 * j, acc[4 * j] * a.inv_nsel, acc[4 * j + 1] * a.inv_nsel,
-                                   acc[4 * j + 2] * a.inv_nsel, acc[4 * j + 3] * a.inv_nsel);
-                };
-                for (int row = r_lo; row < r_hi; ++row) {
-                    const int cn = cen_s[row];
+                int curc = cen_s[r_lo];
+                const float* gp = Gs + r_lo * M1 + 4 * lane;
+#pragma unroll 4
+                for (int row = 0; row < 32; ++row) {
+                    const int cn = cen_s[r_lo + row];
                     if (cn != curc) {
-                        if (curc >= 0) flush();
+                        if (curc >= 0) {
+                            float* dst = a.Tm + ((size_t)curc * M1 + 4 * lane) * 4;
+#pragma unroll
+                            for (int j = 0; j < 4; ++j)
+                                red_add_v4(dst + 4 * j, acc[4 * j] * a.inv_nsel, acc[4 * j + 1] * a.inv_nsel,
+                                           acc[4 * j + 2] * a.inv_nsel, acc[4 * j + 3] * a.inv_nsel);
+                        }
 #pragma unroll
                         for (int q = 0; q < 16; ++q) acc[q] = 0.f;
                         curc = cn;
                     }
-                    if (cn < 0) continue;
-                    const float4 G4 = *reinterpret_cast<const float4*>(Gs + row * M1 + 4 * mq);
-                    const float4 R = Rs[row];
+                    const float4 G4 = *reinterpret_cast<const float4*>(gp + row * M1);
+                    const float4 R = Rs[r_lo + row];            // rows past the end carry R = 0
                     const float gv[4] = {G4.x, G4.y, G4.z, G4.w};
 #pragma unroll
                     for (int j = 0; j < 4; ++j) {
@@ -423,7 +426,13 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
                         acc[4 * j + 3] = fmaf(gv[j], R.w, acc[4 * j + 3]);
                     }
                 }
-                if (curc >= 0) flush();
+                if (curc >= 0) {
+                    float* dst = a.Tm + ((size_t)curc * M1 + 4 * lane) * 4;
+#pragma unroll
+                    for (int j = 0; j < 4; ++j)
+                        red_add_v4(dst + 4 * j, acc[4 * j] * a.inv_nsel, acc[4 * j + 1] * a.inv_nsel,
+                                   acc[4 * j + 2] * a.inv_nsel, acc[4 * j + 3] * a.inv_nsel);
+                }
             }
             named_bar_sync(1 + wg, 128);                   // G / R / centre buffers are free again
             cur = nxt;
@@ -485,22 +494,20 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
             const float R0 = s, R1 = sr * cur.dx, R2 = sr * cur.dy, R3 = sr * cur.dz;
             cen_s[t] = cur.cen;
             // ---- layer 1 and its s-derivative; A1v = [h1,1,0..], A1d = [h1',0,0..] ----
-            float h1[E1], h1p[E1];
+            // (h1' = (1 - h1^2) W1 is recomputed where it is needed again: keeping it costs 25 registers at
+            // the kernel's pressure peak, epilogue 2)
+            float h1[E1];
 #pragma unroll
-            for (int k = 0; k < E1; ++k) {
-                const float w = W1s[k];
-                const float th = tanh_fast(fmaf(s, w, b1s[k]));
-                h1[k] = th;
-                h1p[k] = (1.f - th * th) * w;
-            }
+            for (int k = 0; k < E1; ++k) h1[k] = tanh_fast(fmaf(s, W1s[k], b1s[k]));
 #pragma unroll
             for (int ch = 0; ch < 8; ++ch) {
                 float v[4], d[4];
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
                     const int k = 4 * ch + j;
-                    v[j] = (k < E1) ? h1[k < E1 ? k : 0] : (k == E1 ? 1.f : 0.f);
-                    d[j] = (k < E1) ? h1p[k < E1 ? k : 0] : 0.f;
+                    const float hv = h1[k < E1 ? k : 0];
+                    v[j] = (k < E1) ? hv : (k == E1 ? 1.f : 0.f);
+                    d[j] = (k < E1) ? (1.f - hv * hv) * W1s[k < E1 ? k : 0] : 0.f;
                 }
                 store_chunk(ctx, ctx + kABlk, t, ch, v[0], v[1], v[2], v[3]);
                 store_chunk(ctx + 2 * kABlk, ctx + 3 * kABlk, t, ch, d[0], d[1], d[2], d[3]);
@@ -531,8 +538,9 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
                     const int n = cc * 16 + q;
                     if (n < E2) {
                         const float th = tanh_fast(__uint_as_float(v[q]));
-                        h2[n] = h1[n % E1] + th;
-                        h2p[n] = fmaf(1.f - th * th, __uint_as_float(d[q]), h1p[n % E1]);
+                        const float hv = h1[n % E1];
+                        h2[n] = hv + th;
+                        h2p[n] = fmaf(1.f - th * th, __uint_as_float(d[q]), (1.f - hv * hv) * W1s[n % E1]);
                         o[q] = h2[n];
                     } else {
                         o[q] = (n == E2) ? 1.f : 0.f;
@@ -591,32 +599,37 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
                 for (int q = t; q < nstage * M1; q += 128) dTs[q] = __ldg(src + q);
             }
             named_bar_sync(1 + wg, 128);
-            const int csl = cur.cen - r_lo;
-            const float4* dTp = (cur.cen >= 0 && csl < kDtStage)
-                                    ? dTs + csl * M1
-                                    : reinterpret_cast<const float4*>(a.dTm) + (size_t)max(cur.cen, 0) * M1;
-            // ---- epilogue 3: contract G, G' with dT on the fly ----
+            // ---- epilogue 3: contract G, G' with dT on the fly.  dT rows come from the staged copy when the
+            // whole tile's centres fit (always, unless a centre has < 4 rows of this pair type); the choice is
+            // tile-uniform so that the common path uses plain shared-memory loads ----
             float ds = 0.f, dR0 = 0.f, dR1 = 0.f, dR2 = 0.f, dR3 = 0.f;
+            auto contract = [&](auto dTp) {
 #pragma unroll
-            for (int cc = 0; cc < 7; ++cc) {
-                uint32_t v[16], d[16];
-                tmem_ld16(tmem_v + lanefield + cc * 16, v);
-                tmem_ld16(tmem_g + lanefield + cc * 16, d);
-                tmem_ld_wait();
+                for (int cc = 0; cc < 7; ++cc) {
+                    uint32_t v[16], d[16];
+                    tmem_ld16(tmem_v + lanefield + cc * 16, v);
+                    tmem_ld16(tmem_g + lanefield + cc * 16, d);
+                    tmem_ld_wait();
 #pragma unroll
-                for (int q = 0; q < 16; ++q) {
-                    const int n = cc * 16 + q;
-                    if (n < M1) {
-                        const float4 dT = dTp[n];
-                        const float th = tanh_fast(__uint_as_float(v[q]));
-                        const float G = h2[n % E2] + th;
-                        const float Gp = fmaf(1.f - th * th, __uint_as_float(d[q]), h2p[n % E2]);
-                        const float dG = fmaf(dT.x, R0, fmaf(dT.y, R1, fmaf(dT.z, R2, dT.w * R3)));
-                        ds = fmaf(dG, Gp, ds);
-                        dR0 = fmaf(dT.x, G, dR0); dR1 = fmaf(dT.y, G, dR1);
-                        dR2 = fmaf(dT.z, G, dR2); dR3 = fmaf(dT.w, G, dR3);
+                    for (int q = 0; q < 16; ++q) {
+                        const int n = cc * 16 + q;
+                        if (n < M1) {
+                            const float4 dT = dTp[n];
+                            const float th = tanh_fast(__uint_as_float(v[q]));
+                            const float G = h2[n % E2] + th;
+                            const float Gp = fmaf(1.f - th * th, __uint_as_float(d[q]), h2p[n % E2]);
+                            const float dG = fmaf(dT.x, R0, fmaf(dT.y, R1, fmaf(dT.z, R2, dT.w * R3)));
+                            ds = fmaf(dG, Gp, ds);
+                            dR0 = fmaf(dT.x, G, dR0); dR1 = fmaf(dT.y, G, dR1);
+                            dR2 = fmaf(dT.z, G, dR2); dR3 = fmaf(dT.w, G, dR3);
+                        }
                     }
                 }
+            };
+            if (r_hi - r_lo < kDtStage) {
+                contract(dTs + max(cur.cen - r_lo, 0) * M1);
+            } else {
+                contract(reinterpret_cast<const float4*>(a.dTm) + (size_t)max(cur.cen, 0) * M1);
             }
             tc_fence_before();
             // ---- pair gradient g = dU/dd (R-16) ----

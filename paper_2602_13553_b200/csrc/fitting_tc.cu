@@ -47,7 +47,7 @@ gemm3xtf32_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
                   const __grid_constant__ TcGemmArgs g) {
     using SM = TcSmem<BN>;
     extern __shared__ uint8_t smem_raw[];
-    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);   // keeps the shared address space
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kTcStages * SM::kStage);
     uint64_t* full = bars;                     // [stages] TMA -> split warps
     uint64_t* ready = bars + kTcStages;        // [stages] split warps -> MMA
