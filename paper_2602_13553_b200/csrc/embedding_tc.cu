@@ -2,21 +2,28 @@
 //
 // Neighbour rows are processed in tiles of 128 rows of ONE ordered type pair (t_i, t_j) -- one weight set,
 // resident in shared memory as ready-made UMMA B operands (hi / lo TF32 split, 128B-swizzled K-major,
-// bias folded in as an extra K row).  One thread owns one row (= one TMEM lane):
-//   h1 = tanh(s W1 + b1)                  CUDA cores (K = 1)
+// bias folded in as an extra K row).  A row is one TMEM lane and is shared by TWO threads (halves A and B,
+// warps w and w+4 of a context: both may touch the same TMEM lane quarter), each owning half of the columns:
+//   h1 = tanh(s W1 + b1)                  CUDA cores (K = 1); 13 of the 26 (25 + 1 dummy) channels per thread
 //   z2 = [h1,1] W2b   (128 x 64 x 32)     tcgen05.mma kind::tf32, 3xTF32: a_hi b_hi + a_lo b_hi + a_hi b_lo
 //   h2 = [h1,h1] + tanh(z2)               epilogue: tcgen05.ld -> registers -> next A operand in smem
-//   z3 = [h2,1] W3b   (128 x 112 x 56)
+//   z3 = [h2,1] W3b   (128 x 128 x 56)
 //   G  = [h2,h2] + tanh(z3)                                                                    (R-13)
-// Forward:  T_i += (1/N_sel) sum_rows G (x) R  (R-14): G tile through smem, thread <-> (4 m, 26 rows),
-//           red.global.add.v4.f32 on centre change.
-// Backward: forward-mode -- the derivative rows h' = dh/ds go through the same weights (bias column 0):
+// The channels are permuted (and padded with zero-weight dummies, 25 -> 26, 50 -> 52, 100 -> 104) so that the
+// skip connections stay thread-local: the thread that owns h1 channel i also owns h2 channels i and i + 25 and
+// G channels i, i + 25, i + 50, i + 75 (see `Perm` below).  Halving the per-thread state is what lets 16 warps
+// (2 contexts x 2 halves x 4 lane quarters) fit the register file: the kernels are bound by MUFU and issue
+// latency, not by the tensor pipe, so they need the extra warps.
+// Forward:  T_i += (1/N_sel) sum_rows G (x) R  (R-14): G tile through smem; the two warps of a lane quarter
+//           split its 32 rows, lane <-> 4 G positions, red.global.add.v4.f32 on (warp-uniform) centre change.
+// Backward: forward-mode -- the derivative rows h' = dh/ds go through the same weights (bias slot 0):
 //           G' = [h2',h2'] + (1 - tanh^2 z3) z3';  ds = sum_n (dT_n . R) G'_n;  dR_c = sum_n dT_nc G_n;
 //           pair gradient g = dU/dd (R-16), F_j -= g (f64 atomics), F_i and the virial share by a
 //           segmented warp reduction over the rows of one centre.
-// A CTA runs two independent 128-thread contexts (warpgroups), each with its own A-operand region, TMEM
-// columns and mbarrier, so that one context's MMAs overlap the other's tanh / epilogue work.
+// A CTA runs two independent contexts, each with its own A-operand region, TMEM columns and mbarrier, so
+// that one context's MMAs overlap the other's tanh / epilogue work.
 #include <cstring>
+#include <type_traits>
 #include "common.cuh"
 #include "tc_gemm.cuh"
 
@@ -26,25 +33,45 @@ using namespace tc;
 
 namespace etc {
 constexpr int E1 = 25, E2 = 50, M1 = 100;
-constexpr int K2 = 32;                 // layer-2 K: 25 inputs + bias row + zero padding
-constexpr int N2 = 64;                 // layer-2 N: 50 outputs padded
-constexpr int K3 = 56;                 // layer-3 K: 50 inputs + bias row + padding (7 k-steps of 8)
-constexpr int N3 = 112;                // layer-3 N: 100 outputs padded
+constexpr int H1 = 13;                 // h1 channels per half (26 = 25 + one zero-weight dummy)
+constexpr int H2 = 26;                 // h2 channels per half
+constexpr int H3 = 52;                 // G channels per half
+constexpr int K2 = 32;                 // layer-2 K: half A at k 0..12, bias at 13, half B at 16..28
+constexpr int N2 = 64;                 // layer-2 N: half A at columns 0..25, half B at 32..57
+constexpr int K3 = 56;                 // layer-3 K: half A at k 0..25, bias at 26, half B at 28..53
+constexpr int N3 = 128;                // layer-3 N: half A at columns 0..51, half B at 64..115
+constexpr int GROW = 108;              // floats per staged G row (104 + pad: conflict-free 16 B stores)
 // weight image of one (t_i, t_j) pair, bytes
 constexpr int oW2hi = 0, oW2lo = N2 * 128;                       // [64][32] f32, 128 B rows, SW128
-constexpr int kW3blk = N3 * 128;                                 // one K-block of 32: [112][32]
+constexpr int kW3blk = N3 * 128;                                 // one K-block of 32: [128][32]
 constexpr int oW3hi = 2 * N2 * 128, oW3lo = oW3hi + 2 * kW3blk;
-constexpr int oW1 = oW3lo + 2 * kW3blk;                          // W1[32], b1[32] plain floats
-constexpr int kImgBytes = oW1 + 256;                             // 73984
-constexpr int kImgPad = (kImgBytes + 1023) / 1024 * 1024;        // 74752
+constexpr int oW1 = oW3lo + 2 * kW3blk;                          // W1[32], b1[32] plain floats (padded h1 index)
+constexpr int kImgBytes = oW1 + 256;                             // 82176
+constexpr int kImgPad = (kImgBytes + 1023) / 1024 * 1024;        // 82944
 // per-context shared memory
 constexpr int kABlk = 128 * 128;                                 // one K-block of 32 for 128 rows: 16 KB
 constexpr int oRs = 4 * kABlk;                                   // float4 R[128]
 constexpr int oCen = oRs + 128 * 16;                             // int centre[128]
-constexpr int kCtxBytes = (oCen + 128 * 4 + 1023) / 1024 * 1024; // 68608
-constexpr int kSmemBytes = kImgPad + 2 * kCtxBytes + 64 + 1024;  // + barriers + alignment slack
-constexpr int kThreads = 256;
+constexpr int oPart = oCen + 128 * 4;                            // float part[128][8]: half B -> half A (bwd)
+constexpr int kCtxBytes = (oPart + 128 * 32 + 1023) / 1024 * 1024;   // 72704
+constexpr int kSmemBytes = kImgPad + 2 * kCtxBytes + 64 + 1024;  // + barriers + alignment slack = 229440
+constexpr int kThreads = 512;
 constexpr int kScanBlock = 1024;       // centres per scan block
+static_assert(128 * GROW * 4 <= 4 * kABlk, "G staging must fit the A region");
+static_assert(kSmemBytes <= 232448, "shared memory budget");
+
+// Channel permutation.  Half h (0/1), local indices:  h1: i in [0,13) -> padded channel c1 = 13 h + i
+// (c1 = 25 is the dummy);  h2: j in [0,26) -> original channel 25 (j / 13) + c1(j % 13);  G: g in [0,52) ->
+// original channel 50 (g / 26) + h2 channel of (g % 26).  Returns -1 for a dummy.
+__host__ __device__ constexpr int h2_orig(int h, int j) { return (13 * h + j % 13 == 25) ? -1 : 25 * (j / 13) + 13 * h + j % 13; }
+__host__ __device__ constexpr int g_orig(int h, int g) { return h2_orig(h, g % 26) < 0 ? -1 : 50 * (g / 26) + h2_orig(h, g % 26); }
+// positions inside the operands / accumulators
+__host__ __device__ constexpr int k2_of(int h, int i) { return 16 * h + i; }       // layer-2 K index of h1 (h, i)
+constexpr int kBias2 = 13;
+__host__ __device__ constexpr int n2_of(int h, int j) { return 32 * h + j; }       // layer-2 output column
+__host__ __device__ constexpr int k3_of(int h, int j) { return 28 * h + j; }       // layer-3 K index of h2 (h, j)
+constexpr int kBias3 = 26;
+__host__ __device__ constexpr int n3_of(int h, int g) { return 64 * h + g; }       // layer-3 output column
 }  // namespace etc
 
 struct EmbTcArgs {
@@ -180,6 +207,22 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
+// MUFU token: the tanh-heavy phases of the two contexts of a CTA are mutually exclusive.  Left alone, the two
+// (identical) contexts phase-lock -- both in a MUFU-bound phase, then both waiting for their MMAs -- and every
+// phase takes twice as long; with the token one context's tanh work overlaps the other's MMA round trips and
+// its T accumulation.  Warp 0 of the context takes the lock, everyone else blocks in the hardware barrier.
+__device__ __forceinline__ void mufu_acquire(uint32_t* lock, int bar_id) {
+    if ((threadIdx.x & 255) < 32) {
+        if ((threadIdx.x & 31) == 0) {
+            while (atomicCAS(lock, 0u, 1u) != 0u) __nanosleep(40);
+        }
+        __syncwarp();
+    }
+    named_bar_sync(bar_id, 256);
+}
+// by ONE thread, after the context barrier that ends the phase
+__device__ __forceinline__ void mufu_release(uint32_t* lock) { atomicExch(lock, 0u); }
+
 __device__ __forceinline__ void red_add_v4(float* addr, float a, float b, float c, float d) {
     asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
 }
@@ -225,6 +268,7 @@ struct CtxSetup {
     uint8_t* ctx;        // this context's region
     uint64_t* mma_bar;
     uint32_t tmem_base;  // allocation base (all contexts)
+    uint32_t* lock;      // MUFU token
 };
 
 // common prologue: barriers, TMEM allocation of `ncols` columns; returns after a CTA-wide sync
@@ -233,12 +277,14 @@ __device__ __forceinline__ CtxSetup ctx_setup(uint8_t* smem_raw, uint32_t ncols)
     // pad to 1024 B by pointer arithmetic on the __shared__ array (a uintptr_t round trip loses the address
     // space and turns every access into a generic LD/ST)
     c.smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
-    const int wg = threadIdx.x >> 7;
+    const int wg = threadIdx.x >> 8;                   // context
     c.ctx = c.smem + etc::kImgPad + wg * etc::kCtxBytes;
     uint64_t* bars = reinterpret_cast<uint64_t*>(c.smem + etc::kImgPad + 2 * etc::kCtxBytes);
     c.mma_bar = bars + wg;
     uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(bars + 2);
+    c.lock = reinterpret_cast<uint32_t*>(bars + 3);
     if (threadIdx.x == 0) {
+        *c.lock = 0u;
         mbar_init(bars, 1);
         mbar_init(bars + 1, 1);
         fence_barrier_init();
@@ -266,19 +312,27 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
     using namespace etc;
     extern __shared__ uint8_t smem_raw[];
     const CtxSetup cs = ctx_setup(smem_raw, 256);
-    const int wg = threadIdx.x >> 7, t = threadIdx.x & 127, lane = threadIdx.x & 31;
+    const int cx = threadIdx.x >> 8, half = (threadIdx.x >> 7) & 1, t = threadIdx.x & 127, lane = threadIdx.x & 31;
+    const int bar_ctx = 1 + cx;
     uint8_t* ctx = cs.ctx;
     float4* Rs = reinterpret_cast<float4*>(ctx + oRs);
     int* cen_s = reinterpret_cast<int*>(ctx + oCen);
     float* Gs = reinterpret_cast<float*>(ctx);
-    const float* W1s = reinterpret_cast<const float*>(cs.smem + oW1);
+    const float* W1s = reinterpret_cast<const float*>(cs.smem + oW1) + H1 * half;
     const float* b1s = W1s + 32;
-    const uint32_t tmem_d = cs.tmem_base + wg * 128;
+    const uint32_t tmem_d = cs.tmem_base + cx * 128;
     const uint32_t lanefield = ((uint32_t)((t >> 5) * 32)) << 16;
     const uint32_t actx = smem_u32(ctx), wbase = smem_u32(cs.smem);
     constexpr uint32_t idesc2 = make_idesc_tf32(128, N2), idesc3 = make_idesc_tf32(128, N3);
     uint32_t phase = 0;
     const int nt = a.ntypes;
+    // T accumulation: lane <-> staged G positions 4 lane .. 4 lane + 3 (26 lanes); their original channels
+    int mo[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const int ps = (4 * lane + j) % (2 * H3);
+        mo[j] = g_orig(ps / H3, ps % H3);
+    }
 
     for (int p = 0; p < nt * nt; ++p) {
         const int ti = p / nt, tj = p - ti * nt;
@@ -288,7 +342,7 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
         const int* rs = a.rowstart + (size_t)tj * (a.PN + 1);
         const int begin = rs[a.type_row0[ti]], end = rs[a.type_row0[ti + 1]];
         const int ntile = (end - begin + 127) >> 7;
-        const int C = gridDim.x * 2, c = blockIdx.x * 2 + wg;
+        const int C = gridDim.x * 2, c = blockIdx.x * 2 + cx;
         const int tl0 = (int)((long long)ntile * c / C), tl1 = (int)((long long)ntile * (c + 1) / C);
         if (tl0 >= tl1) continue;
         const int* raddr = a.rowaddr + (size_t)a.PN * a.seloff[tj];
@@ -305,27 +359,29 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
             const RowIn nxt = load_row(a, addr_n1);
             addr_n1 = addr_n2;
 
-            const float s = cur.s, sr = cur.s * cur.rinv;
-            Rs[t] = make_float4(s, sr * cur.dx, sr * cur.dy, sr * cur.dz);
-            cen_s[t] = cur.cen;
-            // ---- layer 1 on CUDA cores, A1 = [h1, 1, 0...] ----
-            float h1[E1];
+            mufu_acquire(cs.lock, bar_ctx);
+            const float s = cur.s;
+            if (half == 0) {
+                const float sr = cur.s * cur.rinv;
+                Rs[t] = make_float4(s, sr * cur.dx, sr * cur.dy, sr * cur.dz);
+                cen_s[t] = cur.cen;
+            }
+            // ---- layer 1 on CUDA cores: my 13 channels -> K slots 16 half .. 16 half + 15 of A1 ----
+            float h1[H1];
 #pragma unroll
-            for (int k = 0; k < E1; ++k) h1[k] = tanh_fast(fmaf(s, W1s[k], b1s[k]));
-#pragma unroll
-            for (int ch = 0; ch < 8; ++ch) {
-                float v[4];
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const int k = 4 * ch + j;
-                    v[j] = (k < E1) ? h1[k < E1 ? k : 0] : (k == E1 ? 1.f : 0.f);
-                }
-                store_chunk(ctx, ctx + kABlk, t, ch, v[0], v[1], v[2], v[3]);
+            for (int i = 0; i < H1; ++i) h1[i] = tanh_fast(fmaf(s, W1s[i], b1s[i]));
+            {
+                const float one = half ? 0.f : 1.f;        // bias slot (k = 13) lives in half A's range
+                store_chunk(ctx, ctx + kABlk, t, 4 * half + 0, h1[0], h1[1], h1[2], h1[3]);
+                store_chunk(ctx, ctx + kABlk, t, 4 * half + 1, h1[4], h1[5], h1[6], h1[7]);
+                store_chunk(ctx, ctx + kABlk, t, 4 * half + 2, h1[8], h1[9], h1[10], h1[11]);
+                store_chunk(ctx, ctx + kABlk, t, 4 * half + 3, h1[12], one, 0.f, 0.f);
             }
             fence_proxy_async_smem();
             tc_fence_before();
-            named_bar_sync(1 + wg, 128);
-            if (t == 0) {
+            named_bar_sync(bar_ctx, 256);
+            if ((threadIdx.x & 255) == 0) {
+                mufu_release(cs.lock);
                 tc_fence_after();
                 mma_block_3x(tmem_d, actx, actx + kABlk, wbase + oW2hi, wbase + oW2lo, idesc2, 4, true);
                 umma_commit(cs.mma_bar);
@@ -333,33 +389,32 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
             mbar_wait(cs.mma_bar, phase);
             phase ^= 1;
             tc_fence_after();
-            // ---- epilogue 2: h2 = [h1,h1] + tanh(z2); A2 = [h2, 1, 0...] (two K-blocks; overlays A1) ----
-            float h2[E2];
-#pragma unroll
-            for (int cc = 0; cc < 4; ++cc) {
-                uint32_t v[16];
-                tmem_ld16(tmem_d + lanefield + cc * 16, v);
+            mufu_acquire(cs.lock, bar_ctx);
+            // ---- epilogue 2: h2 = [h1,h1] + tanh(z2), my 26 columns; A2 K slots 28 half .. 28 half + 27 ----
+            float h2[H2 + 2];
+            {
+                uint32_t v[H2];
+                const uint32_t col = tmem_d + lanefield + 32 * half;
+                tmem_ld16(col, v);
+                tmem_ld8(col + 16, v + 16);
+                tmem_ld2(col + 24, v + 24);
                 tmem_ld_wait();
-                float o[16];
 #pragma unroll
-                for (int q = 0; q < 16; ++q) {
-                    const int n = cc * 16 + q;
-                    if (n < E2) {
-                        h2[n] = h1[n % E1] + tanh_fast(__uint_as_float(v[q]));
-                        o[q] = h2[n];
-                    } else {
-                        o[q] = (n == E2) ? 1.f : 0.f;
-                    }
+                for (int j = 0; j < H2; ++j) h2[j] = h1[j % H1] + tanh_fast(__uint_as_float(v[j]));
+                h2[H2] = half ? 0.f : 1.f;                 // bias slot (k = 26)
+                h2[H2 + 1] = 0.f;
+#pragma unroll
+                for (int cq = 0; cq < 7; ++cq) {
+                    const int gc = 7 * half + cq, blk = gc >> 3;
+                    uint8_t* bh = ctx + blk * kABlk;
+                    store_chunk(bh, bh + 2 * kABlk, t, gc & 7, h2[4 * cq], h2[4 * cq + 1], h2[4 * cq + 2], h2[4 * cq + 3]);
                 }
-                uint8_t* bh = ctx + (cc >> 1) * kABlk;
-#pragma unroll
-                for (int j = 0; j < 4; ++j)
-                    store_chunk(bh, bh + 2 * kABlk, t, (cc & 1) * 4 + j, o[4 * j], o[4 * j + 1], o[4 * j + 2], o[4 * j + 3]);
             }
             fence_proxy_async_smem();
             tc_fence_before();
-            named_bar_sync(1 + wg, 128);
-            if (t == 0) {
+            named_bar_sync(bar_ctx, 256);
+            if ((threadIdx.x & 255) == 0) {
+                mufu_release(cs.lock);
                 tc_fence_after();
                 mma_block_3x(tmem_d, actx, actx + 2 * kABlk, wbase + oW3hi, wbase + oW3lo, idesc3, 4, true);
                 mma_block_3x(tmem_d, actx + kABlk, actx + 3 * kABlk, wbase + oW3hi + kW3blk, wbase + oW3lo + kW3blk, idesc3,
@@ -369,72 +424,94 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
             mbar_wait(cs.mma_bar, phase);
             phase ^= 1;
             tc_fence_after();
-            // ---- epilogue 3: G = [h2,h2] + tanh(z3) -> smem [row][100] (overlays the A region) ----
-#pragma unroll
-            for (int cc = 0; cc < 7; ++cc) {
-                uint32_t v[16];
-                tmem_ld16(tmem_d + lanefield + cc * 16, v);
+            mufu_acquire(cs.lock, bar_ctx);
+            // ---- epilogue 3: G = [h2,h2] + tanh(z3), my 52 columns -> smem [row][GROW] (overlays the A region) ----
+            {
+                const uint32_t col = tmem_d + lanefield + 64 * half;
+                float* grow = Gs + t * GROW + H3 * half;
+                uint32_t v[32];
+                tmem_ld32(col, v);
                 tmem_ld_wait();
 #pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const int n = cc * 16 + 4 * j;
-                    if (n < M1) {
-                        float4 gq;
-                        gq.x = h2[n % E2] + tanh_fast(__uint_as_float(v[4 * j]));
-                        gq.y = h2[(n + 1) % E2] + tanh_fast(__uint_as_float(v[4 * j + 1]));
-                        gq.z = h2[(n + 2) % E2] + tanh_fast(__uint_as_float(v[4 * j + 2]));
-                        gq.w = h2[(n + 3) % E2] + tanh_fast(__uint_as_float(v[4 * j + 3]));
-                        *reinterpret_cast<float4*>(Gs + t * M1 + n) = gq;
-                    }
+                for (int q = 0; q < 8; ++q) {
+                    float4 gq;
+                    gq.x = h2[(4 * q) % H2] + tanh_fast(__uint_as_float(v[4 * q]));
+                    gq.y = h2[(4 * q + 1) % H2] + tanh_fast(__uint_as_float(v[4 * q + 1]));
+                    gq.z = h2[(4 * q + 2) % H2] + tanh_fast(__uint_as_float(v[4 * q + 2]));
+                    gq.w = h2[(4 * q + 3) % H2] + tanh_fast(__uint_as_float(v[4 * q + 3]));
+                    *reinterpret_cast<float4*>(grow + 4 * q) = gq;
+                }
+                tmem_ld16(col + 32, v);
+                tmem_ld4(col + 48, v + 16);
+                tmem_ld_wait();
+#pragma unroll
+                for (int q = 0; q < 5; ++q) {
+                    const int g = 32 + 4 * q;
+                    float4 gq;
+                    gq.x = h2[g % H2] + tanh_fast(__uint_as_float(v[4 * q]));
+                    gq.y = h2[(g + 1) % H2] + tanh_fast(__uint_as_float(v[4 * q + 1]));
+                    gq.z = h2[(g + 2) % H2] + tanh_fast(__uint_as_float(v[4 * q + 2]));
+                    gq.w = h2[(g + 3) % H2] + tanh_fast(__uint_as_float(v[4 * q + 3]));
+                    *reinterpret_cast<float4*>(grow + g) = gq;
                 }
             }
             tc_fence_before();
-            __syncwarp();
-            // ---- T_i += (1/N_sel) sum_rows G (x) R.  Warp w owns the 32 rows its own lanes just wrote (so a
-            // warp-level sync suffices); lane <-> 4 consecutive m (25 lanes).  All lanes walk the same rows, so
-            // the centre changes are warp-uniform and R / centre reads are broadcasts. ----
-            if (lane < 25) {
-                const int r_lo = t & ~31;
-                float acc[16];
-#pragma unroll
-                for (int q = 0; q < 16; ++q) acc[q] = 0.f;
-                int curc = cen_s[r_lo];
-                const float* gp = Gs + r_lo * M1 + 4 * lane;
-#pragma unroll 4
-                for (int row = 0; row < 32; ++row) {
-                    const int cn = cen_s[r_lo + row];
-                    if (cn != curc) {
-                        if (curc >= 0) {
-                            float* dst = a.Tm + ((size_t)curc * M1 + 4 * lane) * 4;
-#pragma unroll
-                            for (int j = 0; j < 4; ++j)
-                                red_add_v4(dst + 4 * j, acc[4 * j] * a.inv_nsel, acc[4 * j + 1] * a.inv_nsel,
-                                           acc[4 * j + 2] * a.inv_nsel, acc[4 * j + 3] * a.inv_nsel);
-                        }
+            named_bar_sync(bar_ctx, 256);                  // G rows complete
+            if ((threadIdx.x & 255) == 0) mufu_release(cs.lock);
+            // ---- T_i += (1/N_sel) sum_rows G (x) R.  The warp pair owns the 32 rows it just wrote; each warp
+            // takes 16 of them, lane <-> 4 staged G positions (26 lanes).  All lanes walk the same rows, so the
+            // centre changes are warp-uniform and the R / centre reads are broadcasts. ----
+            {
+                const int r_lo = (t & ~31) + 16 * half;
+                // centre boundaries inside my 16 rows (bit r set: row r starts a new centre), warp-uniform
+                const int cme = cen_s[r_lo + (lane & 15)];
+                const int cpv = __shfl_up_sync(0xffffffffu, cme, 1);
+                const uint32_t bnd = __ballot_sync(0xffffffffu, (lane & 15) != 0 && lane < 16 && cme != cpv) & 0xffffu;
+                if (lane < 26) {
+                    const float* gp = Gs + r_lo * GROW + 4 * lane;
+                    int r0 = 0;
+                    while (r0 < 16) {                       // one iteration per centre segment [r0, r1)
+                        const uint32_t rest = bnd >> (r0 + 1);
+                        const int r1 = rest ? r0 + __ffs(rest) : 16;
+                        const int cn = cen_s[r_lo + r0];
+                        if (cn < 0) break;                  // rows past the end of the pair (always at the tail)
+                        float acc[16];
 #pragma unroll
                         for (int q = 0; q < 16; ++q) acc[q] = 0.f;
-                        curc = cn;
-                    }
-                    const float4 G4 = *reinterpret_cast<const float4*>(gp + row * M1);
-                    const float4 R = Rs[r_lo + row];            // rows past the end carry R = 0
-                    const float gv[4] = {G4.x, G4.y, G4.z, G4.w};
+                        auto rows = [&](auto NR, int row) {          // NR rows: all loads first, then the FMAs
+                            constexpr int nr = decltype(NR)::value;
+                            float4 G4[nr], R[nr];
 #pragma unroll
-                    for (int j = 0; j < 4; ++j) {
-                        acc[4 * j] = fmaf(gv[j], R.x, acc[4 * j]);
-                        acc[4 * j + 1] = fmaf(gv[j], R.y, acc[4 * j + 1]);
-                        acc[4 * j + 2] = fmaf(gv[j], R.z, acc[4 * j + 2]);
-                        acc[4 * j + 3] = fmaf(gv[j], R.w, acc[4 * j + 3]);
-                    }
-                }
-                if (curc >= 0) {
-                    float* dst = a.Tm + ((size_t)curc * M1 + 4 * lane) * 4;
+                            for (int u = 0; u < nr; ++u) {
+                                G4[u] = *reinterpret_cast<const float4*>(gp + (row + u) * GROW);
+                                R[u] = Rs[r_lo + row + u];
+                            }
 #pragma unroll
-                    for (int j = 0; j < 4; ++j)
-                        red_add_v4(dst + 4 * j, acc[4 * j] * a.inv_nsel, acc[4 * j + 1] * a.inv_nsel,
-                                   acc[4 * j + 2] * a.inv_nsel, acc[4 * j + 3] * a.inv_nsel);
+                            for (int u = 0; u < nr; ++u) {
+                                const float gv[4] = {G4[u].x, G4[u].y, G4[u].z, G4[u].w};
+#pragma unroll
+                                for (int j = 0; j < 4; ++j) {
+                                    acc[4 * j] = fmaf(gv[j], R[u].x, acc[4 * j]);
+                                    acc[4 * j + 1] = fmaf(gv[j], R[u].y, acc[4 * j + 1]);
+                                    acc[4 * j + 2] = fmaf(gv[j], R[u].z, acc[4 * j + 2]);
+                                    acc[4 * j + 3] = fmaf(gv[j], R[u].w, acc[4 * j + 3]);
+                                }
+                            }
+                        };
+                        int row = r0;
+                        for (; row + 4 <= r1; row += 4) rows(std::integral_constant<int, 4>{}, row);
+                        if (row + 2 <= r1) { rows(std::integral_constant<int, 2>{}, row); row += 2; }
+                        if (row < r1) rows(std::integral_constant<int, 1>{}, row);
+#pragma unroll
+                        for (int j = 0; j < 4; ++j)
+                            if (mo[j] >= 0)
+                                red_add_v4(a.Tm + ((size_t)cn * M1 + mo[j]) * 4, acc[4 * j] * a.inv_nsel,
+                                           acc[4 * j + 1] * a.inv_nsel, acc[4 * j + 2] * a.inv_nsel, acc[4 * j + 3] * a.inv_nsel);
+                        r0 = r1;
+                    }
                 }
             }
-            named_bar_sync(1 + wg, 128);                   // G / R / centre buffers are free again
+            named_bar_sync(bar_ctx, 256);                  // G / R / centre buffers are free again
             cur = nxt;
         }
     }
@@ -453,13 +530,15 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
     using namespace etc;
     extern __shared__ uint8_t smem_raw[];
     const CtxSetup cs = ctx_setup(smem_raw, 512);
-    const int wg = threadIdx.x >> 7, t = threadIdx.x & 127, lane = threadIdx.x & 31;
+    const int cx = threadIdx.x >> 8, half = (threadIdx.x >> 7) & 1, t = threadIdx.x & 127, lane = threadIdx.x & 31;
+    const int bar_ctx = 1 + cx, bar_pair = 3 + cx * 4 + (t >> 5);
     uint8_t* ctx = cs.ctx;
     int* cen_s = reinterpret_cast<int*>(ctx + oCen);
     float4* dTs = reinterpret_cast<float4*>(ctx);
-    const float* W1s = reinterpret_cast<const float*>(cs.smem + oW1);
+    float* part = reinterpret_cast<float*>(ctx + oPart) + t * 8;
+    const float* W1s = reinterpret_cast<const float*>(cs.smem + oW1) + H1 * half;
     const float* b1s = W1s + 32;
-    const uint32_t tmem_v = cs.tmem_base + wg * 256, tmem_g = tmem_v + N3;     // value / derivative accumulators
+    const uint32_t tmem_v = cs.tmem_base + cx * 256, tmem_g = tmem_v + N3;     // value / derivative accumulators
     const uint32_t lanefield = ((uint32_t)((t >> 5) * 32)) << 16;
     const uint32_t actx = smem_u32(ctx), wbase = smem_u32(cs.smem);
     constexpr uint32_t idesc2 = make_idesc_tf32(128, N2), idesc3 = make_idesc_tf32(128, N3);
@@ -474,7 +553,7 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
         const int* rs = a.rowstart + (size_t)tj * (a.PN + 1);
         const int begin = rs[a.type_row0[ti]], end = rs[a.type_row0[ti + 1]];
         const int ntile = (end - begin + 127) >> 7;
-        const int C = gridDim.x * 2, c = blockIdx.x * 2 + wg;
+        const int C = gridDim.x * 2, c = blockIdx.x * 2 + cx;
         const int tl0 = (int)((long long)ntile * c / C), tl1 = (int)((long long)ntile * (c + 1) / C);
         if (tl0 >= tl1) continue;
         const int* raddr = a.rowaddr + (size_t)a.PN * a.seloff[tj];
@@ -482,40 +561,53 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
             const int g = begin + tile * 128 + t;
             return (tile < tl1 && g < end) ? __ldg(raddr + g) : -1;
         };
-        RowIn cur = load_row(a, addr_of(tl0));
-        int addr_n1 = addr_of(tl0 + 1);
+        // software pipeline: slot index two tiles ahead, {d, s} one tile ahead (s feeds layer 1 at once); the
+        // rest of the row is loaded at the top of its tile and first used after the second MMA round trip
+        auto load_A = [&](int addr) -> float4 {
+            return addr >= 0 ? __ldg(reinterpret_cast<const float4*>(a.slotA) + addr) : make_float4(0.f, 0.f, 0.f, 0.f);
+        };
+        int addr_c = addr_of(tl0), addr_n = addr_of(tl0 + 1);
+        float4 curA = load_A(addr_c);
 
         for (int tile = tl0; tile < tl1; ++tile) {
-            const int addr_n2 = addr_of(tile + 2);
-            const RowIn nxt = load_row(a, addr_n1);
-            addr_n1 = addr_n2;
+            RowIn cur;
+            cur.dx = curA.x; cur.dy = curA.y; cur.dz = curA.z; cur.s = curA.w;
+            cur.ds = 0.f; cur.rinv = 1.f; cur.jcode = 0u; cur.cen = -1; cur.ba = 0;
+            if (addr_c >= 0) {
+                const float4 B = __ldg(reinterpret_cast<const float4*>(a.slotB) + addr_c);
+                cur.ds = B.x; cur.rinv = B.y; cur.jcode = __float_as_uint(B.z);
+                cur.ba = addr_c / a.nsel;
+                cur.cen = __ldg(a.row_of + cur.ba);
+            }
+            addr_c = addr_n;
+            curA = load_A(addr_c);
+            addr_n = addr_of(tile + 2);
 
-            const float s = cur.s, sr = cur.s * cur.rinv;
-            const float R0 = s, R1 = sr * cur.dx, R2 = sr * cur.dy, R3 = sr * cur.dz;
-            cen_s[t] = cur.cen;
-            // ---- layer 1 and its s-derivative; A1v = [h1,1,0..], A1d = [h1',0,0..] ----
-            // (h1' = (1 - h1^2) W1 is recomputed where it is needed again: keeping it costs 25 registers at
-            // the kernel's pressure peak, epilogue 2)
-            float h1[E1];
+            const float s = cur.s;
+            // ---- layer 1 and its s-derivative, my 13 channels; A1v = [h1,1,0..], A1d = [h1',0,0..] ----
+            float h1[H1], h1p[H1];
 #pragma unroll
-            for (int k = 0; k < E1; ++k) h1[k] = tanh_fast(fmaf(s, W1s[k], b1s[k]));
+            for (int i = 0; i < H1; ++i) {
+                const float w = W1s[i];
+                const float th = tanh_fast(fmaf(s, w, b1s[i]));
+                h1[i] = th;
+                h1p[i] = (1.f - th * th) * w;
+            }
+            {
+                const float one = half ? 0.f : 1.f;
 #pragma unroll
-            for (int ch = 0; ch < 8; ++ch) {
-                float v[4], d[4];
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const int k = 4 * ch + j;
-                    const float hv = h1[k < E1 ? k : 0];
-                    v[j] = (k < E1) ? hv : (k == E1 ? 1.f : 0.f);
-                    d[j] = (k < E1) ? (1.f - hv * hv) * W1s[k < E1 ? k : 0] : 0.f;
+                for (int cq = 0; cq < 3; ++cq) {
+                    store_chunk(ctx, ctx + kABlk, t, 4 * half + cq, h1[4 * cq], h1[4 * cq + 1], h1[4 * cq + 2], h1[4 * cq + 3]);
+                    store_chunk(ctx + 2 * kABlk, ctx + 3 * kABlk, t, 4 * half + cq, h1p[4 * cq], h1p[4 * cq + 1],
+                                h1p[4 * cq + 2], h1p[4 * cq + 3]);
                 }
-                store_chunk(ctx, ctx + kABlk, t, ch, v[0], v[1], v[2], v[3]);
-                store_chunk(ctx + 2 * kABlk, ctx + 3 * kABlk, t, ch, d[0], d[1], d[2], d[3]);
+                store_chunk(ctx, ctx + kABlk, t, 4 * half + 3, h1[12], one, 0.f, 0.f);
+                store_chunk(ctx + 2 * kABlk, ctx + 3 * kABlk, t, 4 * half + 3, h1p[12], 0.f, 0.f, 0.f);
             }
             fence_proxy_async_smem();
             tc_fence_before();
-            named_bar_sync(1 + wg, 128);
-            if (t == 0) {
+            named_bar_sync(bar_ctx, 256);
+            if ((threadIdx.x & 255) == 0) {
                 tc_fence_after();
                 mma_block_3x(tmem_v, actx, actx + kABlk, wbase + oW2hi, wbase + oW2lo, idesc2, 4, true);
                 mma_block_3x(tmem_g, actx + 2 * kABlk, actx + 3 * kABlk, wbase + oW2hi, wbase + oW2lo, idesc2, 4, true);
@@ -524,37 +616,33 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
             mbar_wait(cs.mma_bar, phase);
             phase ^= 1;
             tc_fence_after();
-            // ---- epilogue 2: h2, h2'; A2v written now, A2d after MMA3v has consumed the region ----
-            float h2[E2], h2p[E2];
-#pragma unroll
-            for (int cc = 0; cc < 4; ++cc) {
-                uint32_t v[16], d[16];
-                tmem_ld16(tmem_v + lanefield + cc * 16, v);
-                tmem_ld16(tmem_g + lanefield + cc * 16, d);
+            // ---- epilogue 2: h2, h2' (my 26 columns); A2v written now, A2d after MMA3v has consumed the region ----
+            float h2[H2 + 2], h2p[H2 + 2];
+            {
+                uint32_t v[H2], d[H2];
+                const uint32_t cv = tmem_v + lanefield + 32 * half, cd = tmem_g + lanefield + 32 * half;
+                tmem_ld16(cv, v); tmem_ld8(cv + 16, v + 16); tmem_ld2(cv + 24, v + 24);
+                tmem_ld16(cd, d); tmem_ld8(cd + 16, d + 16); tmem_ld2(cd + 24, d + 24);
                 tmem_ld_wait();
-                float o[16];
 #pragma unroll
-                for (int q = 0; q < 16; ++q) {
-                    const int n = cc * 16 + q;
-                    if (n < E2) {
-                        const float th = tanh_fast(__uint_as_float(v[q]));
-                        const float hv = h1[n % E1];
-                        h2[n] = hv + th;
-                        h2p[n] = fmaf(1.f - th * th, __uint_as_float(d[q]), (1.f - hv * hv) * W1s[n % E1]);
-                        o[q] = h2[n];
-                    } else {
-                        o[q] = (n == E2) ? 1.f : 0.f;
-                    }
+                for (int j = 0; j < H2; ++j) {
+                    const float th = tanh_fast(__uint_as_float(v[j]));
+                    h2[j] = h1[j % H1] + th;
+                    h2p[j] = fmaf(1.f - th * th, __uint_as_float(d[j]), h1p[j % H1]);
                 }
-                uint8_t* bh = ctx + (cc >> 1) * kABlk;
+                h2[H2] = half ? 0.f : 1.f; h2[H2 + 1] = 0.f;
+                h2p[H2] = 0.f; h2p[H2 + 1] = 0.f;
 #pragma unroll
-                for (int j = 0; j < 4; ++j)
-                    store_chunk(bh, bh + 2 * kABlk, t, (cc & 1) * 4 + j, o[4 * j], o[4 * j + 1], o[4 * j + 2], o[4 * j + 3]);
+                for (int cq = 0; cq < 7; ++cq) {
+                    const int gc = 7 * half + cq, blk = gc >> 3;
+                    uint8_t* bh = ctx + blk * kABlk;
+                    store_chunk(bh, bh + 2 * kABlk, t, gc & 7, h2[4 * cq], h2[4 * cq + 1], h2[4 * cq + 2], h2[4 * cq + 3]);
+                }
             }
             fence_proxy_async_smem();
             tc_fence_before();
-            named_bar_sync(1 + wg, 128);
-            if (t == 0) {
+            named_bar_sync(bar_ctx, 256);
+            if ((threadIdx.x & 255) == 0) {
                 tc_fence_after();
                 mma_block_3x(tmem_v, actx, actx + 2 * kABlk, wbase + oW3hi, wbase + oW3lo, idesc3, 4, true);
                 mma_block_3x(tmem_v, actx + kABlk, actx + 3 * kABlk, wbase + oW3hi + kW3blk, wbase + oW3lo + kW3blk, idesc3,
@@ -565,117 +653,141 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
             phase ^= 1;
             tc_fence_after();
 #pragma unroll
-            for (int cc = 0; cc < 4; ++cc) {
-                float o[16];
-#pragma unroll
-                for (int q = 0; q < 16; ++q) {
-                    const int n = cc * 16 + q;
-                    o[q] = (n < E2) ? h2p[n < E2 ? n : 0] : 0.f;
-                }
-                uint8_t* bh = ctx + (cc >> 1) * kABlk;
-#pragma unroll
-                for (int j = 0; j < 4; ++j)
-                    store_chunk(bh, bh + 2 * kABlk, t, (cc & 1) * 4 + j, o[4 * j], o[4 * j + 1], o[4 * j + 2], o[4 * j + 3]);
+            for (int cq = 0; cq < 7; ++cq) {
+                const int gc = 7 * half + cq, blk = gc >> 3;
+                uint8_t* bh = ctx + blk * kABlk;
+                store_chunk(bh, bh + 2 * kABlk, t, gc & 7, h2p[4 * cq], h2p[4 * cq + 1], h2p[4 * cq + 2], h2p[4 * cq + 3]);
             }
+            if (half == 0) cen_s[t] = cur.cen;
+            const float sr = cur.s * cur.rinv;
+            const float R0 = s, R1 = sr * cur.dx, R2 = sr * cur.dy, R3 = sr * cur.dz;
             fence_proxy_async_smem();
             tc_fence_before();
-            named_bar_sync(1 + wg, 128);
-            if (t == 0) {
+            named_bar_sync(bar_ctx, 256);
+            if ((threadIdx.x & 255) == 0) {
                 tc_fence_after();
                 mma_block_3x(tmem_g, actx, actx + 2 * kABlk, wbase + oW3hi, wbase + oW3lo, idesc3, 4, true);
                 mma_block_3x(tmem_g, actx + kABlk, actx + 3 * kABlk, wbase + oW3hi + kW3blk, wbase + oW3lo + kW3blk, idesc3,
                              3, false);
                 umma_commit(cs.mma_bar);
             }
-            mbar_wait(cs.mma_bar, phase);
-            phase ^= 1;
-            tc_fence_after();
-            // ---- stage dT of this tile's centres into the (now free) A region ----
+            // ---- dT of this tile's centres: fetched into registers while the MMAs run, then staged into the
+            // (by then free) A region ----
             const int nvalid = min(128, end - (begin + tile * 128));
             const int r_lo = cen_s[0], r_hi = cen_s[nvalid - 1];
             const int nstage = min(r_hi - r_lo + 1, kDtStage);
-            {
-                const float4* src = reinterpret_cast<const float4*>(a.dTm) + (size_t)r_lo * M1;
-                for (int q = t; q < nstage * M1; q += 128) dTs[q] = __ldg(src + q);
-            }
-            named_bar_sync(1 + wg, 128);
-            // ---- epilogue 3: contract G, G' with dT on the fly.  dT rows come from the staged copy when the
-            // whole tile's centres fit (always, unless a centre has < 4 rows of this pair type); the choice is
-            // tile-uniform so that the common path uses plain shared-memory loads ----
+            const float4* dsrc = reinterpret_cast<const float4*>(a.dTm) + (size_t)r_lo * M1;
+            const int dq = threadIdx.x & 255;
+            float4 pre[3];
+#pragma unroll
+            for (int i = 0; i < 3; ++i)
+                if (dq + 256 * i < nstage * M1) pre[i] = __ldg(dsrc + dq + 256 * i);
+            mbar_wait(cs.mma_bar, phase);
+            phase ^= 1;
+            tc_fence_after();
+#pragma unroll
+            for (int i = 0; i < 3; ++i)
+                if (dq + 256 * i < nstage * M1) dTs[dq + 256 * i] = pre[i];
+            for (int q = dq + 768; q < nstage * M1; q += 256) dTs[q] = __ldg(dsrc + q);
+            named_bar_sync(bar_ctx, 256);
+            // ---- epilogue 3: contract G, G' (my 52 columns) with dT on the fly.  dT rows come from the staged
+            // copy when the whole tile's centres fit (always, unless a centre has < 4 rows of this pair type);
+            // the choice is tile-uniform so that the common path uses plain shared-memory loads.  Original
+            // channel of my position g: 50 (g / 26) + 25 ((g % 26) / 13) + (g % 26) % 13  + 13 half. ----
             float ds = 0.f, dR0 = 0.f, dR1 = 0.f, dR2 = 0.f, dR3 = 0.f;
             auto contract = [&](auto dTp) {
+                auto piece = [&](auto NV, int g0, const uint32_t* v, const uint32_t* d) {
 #pragma unroll
-                for (int cc = 0; cc < 7; ++cc) {
-                    uint32_t v[16], d[16];
-                    tmem_ld16(tmem_v + lanefield + cc * 16, v);
-                    tmem_ld16(tmem_g + lanefield + cc * 16, d);
-                    tmem_ld_wait();
-#pragma unroll
-                    for (int q = 0; q < 16; ++q) {
-                        const int n = cc * 16 + q;
-                        if (n < M1) {
-                            const float4 dT = dTp[n];
-                            const float th = tanh_fast(__uint_as_float(v[q]));
-                            const float G = h2[n % E2] + th;
-                            const float Gp = fmaf(1.f - th * th, __uint_as_float(d[q]), h2p[n % E2]);
-                            const float dG = fmaf(dT.x, R0, fmaf(dT.y, R1, fmaf(dT.z, R2, dT.w * R3)));
-                            ds = fmaf(dG, Gp, ds);
-                            dR0 = fmaf(dT.x, G, dR0); dR1 = fmaf(dT.y, G, dR1);
-                            dR2 = fmaf(dT.z, G, dR2); dR3 = fmaf(dT.w, G, dR3);
-                        }
+                    for (int q = 0; q < decltype(NV)::value; ++q) {
+                        const int g = g0 + q, j = g % H2;
+                        const bool dummy = (j % H1 == H1 - 1) && half;        // padded channel 25
+                        float4 dT = dTp[50 * (g / H2) + 25 * (j / H1) + j % H1];
+                        if (dummy) dT = make_float4(0.f, 0.f, 0.f, 0.f);
+                        const float th = tanh_fast(__uint_as_float(v[q]));
+                        const float G = h2[j] + th;
+                        const float Gp = fmaf(1.f - th * th, __uint_as_float(d[q]), h2p[j]);
+                        const float dG = fmaf(dT.x, R0, fmaf(dT.y, R1, fmaf(dT.z, R2, dT.w * R3)));
+                        ds = fmaf(dG, Gp, ds);
+                        dR0 = fmaf(dT.x, G, dR0); dR1 = fmaf(dT.y, G, dR1);
+                        dR2 = fmaf(dT.z, G, dR2); dR3 = fmaf(dT.w, G, dR3);
                     }
+                };
+                const uint32_t cv = tmem_v + lanefield + 64 * half, cd = tmem_g + lanefield + 64 * half;
+                uint32_t v[16], d[16];
+#pragma unroll
+                for (int cc = 0; cc < 3; ++cc) {
+                    tmem_ld16(cv + 16 * cc, v);
+                    tmem_ld16(cd + 16 * cc, d);
+                    tmem_ld_wait();
+                    piece(std::integral_constant<int, 16>{}, 16 * cc, v, d);
                 }
+                tmem_ld4(cv + 48, v);
+                tmem_ld4(cd + 48, d);
+                tmem_ld_wait();
+                piece(std::integral_constant<int, 4>{}, 48, v, d);
             };
             if (r_hi - r_lo < kDtStage) {
-                contract(dTs + max(cur.cen - r_lo, 0) * M1);
+                contract(dTs + max(cur.cen - r_lo, 0) * M1 + H1 * half);
             } else {
-                contract(reinterpret_cast<const float4*>(a.dTm) + (size_t)max(cur.cen, 0) * M1);
+                contract(reinterpret_cast<const float4*>(a.dTm) + (size_t)max(cur.cen, 0) * M1 + H1 * half);
             }
             tc_fence_before();
-            // ---- pair gradient g = dU/dd (R-16) ----
-            float red[12];
-            {
-                const float w = (cur.cen >= 0) ? a.inv_nsel : 0.f;
-                ds *= w; dR0 *= w; dR1 *= w; dR2 *= w; dR3 *= w;
-                const float rinv = cur.rinv;
-                const float dot = dR1 * cur.dx + dR2 * cur.dy + dR3 * cur.dz;
-                const float radial = (ds + dR0) * cur.ds + (cur.ds * rinv - s * rinv * rinv) * dot;
-                const float rr = radial * rinv;
-                const float gx = fmaf(rr, cur.dx, sr * dR1), gy = fmaf(rr, cur.dy, sr * dR2), gz = fmaf(rr, cur.dz, sr * dR3);
-                if (cur.cen >= 0) {
-                    const int j = (int)(cur.jcode & 0x7fffffu);
-                    double* fj = a.f + ((size_t)(cur.ba / a.N) * a.N + j) * 3;
-                    atomicAdd(fj, -(double)gx); atomicAdd(fj + 1, -(double)gy); atomicAdd(fj + 2, -(double)gz);
+            // half B hands its partial sums to half A, which finishes the row
+            if (half) {
+                *reinterpret_cast<float4*>(part) = make_float4(dR0, dR1, dR2, dR3);
+                part[4] = ds;
+            }
+            named_bar_sync(bar_pair, 64);
+            if (half == 0) {
+                {
+                    const float4 o = *reinterpret_cast<const float4*>(part);
+                    dR0 += o.x; dR1 += o.y; dR2 += o.z; dR3 += o.w;
+                    ds += part[4];
                 }
-                red[0] = gx; red[1] = gy; red[2] = gz;
-                const float dd[3] = {cur.dx, cur.dy, cur.dz}, gg[3] = {gx, gy, gz};
+                // ---- pair gradient g = dU/dd (R-16) ----
+                float red[12];
+                {
+                    const float w = (cur.cen >= 0) ? a.inv_nsel : 0.f;
+                    ds *= w; dR0 *= w; dR1 *= w; dR2 *= w; dR3 *= w;
+                    const float rinv = cur.rinv;
+                    const float dot = dR1 * cur.dx + dR2 * cur.dy + dR3 * cur.dz;
+                    const float radial = (ds + dR0) * cur.ds + (cur.ds * rinv - s * rinv * rinv) * dot;
+                    const float rr = radial * rinv;
+                    const float gx = fmaf(rr, cur.dx, sr * dR1), gy = fmaf(rr, cur.dy, sr * dR2), gz = fmaf(rr, cur.dz, sr * dR3);
+                    if (cur.cen >= 0) {
+                        const int j = (int)(cur.jcode & 0x7fffffu);
+                        double* fj = a.f + ((size_t)(cur.ba / a.N) * a.N + j) * 3;
+                        atomicAdd(fj, -(double)gx); atomicAdd(fj + 1, -(double)gy); atomicAdd(fj + 2, -(double)gz);
+                    }
+                    red[0] = gx; red[1] = gy; red[2] = gz;
+                    const float dd[3] = {cur.dx, cur.dy, cur.dz}, gg[3] = {gx, gy, gz};
 #pragma unroll
-                for (int u = 0; u < 3; ++u)
+                    for (int u = 0; u < 3; ++u)
 #pragma unroll
-                    for (int w2 = 0; w2 < 3; ++w2) red[3 + 3 * u + w2] = -dd[u] * gg[w2];
-            }
-            // segmented warp reduction over the rows of one centre (rows of a centre are contiguous)
-            const int key = cur.cen;
+                        for (int w2 = 0; w2 < 3; ++w2) red[3 + 3 * u + w2] = -dd[u] * gg[w2];
+                }
+                // segmented warp reduction over the rows of one centre (rows of a centre are contiguous)
+                const int key = cur.cen;
 #pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const int ko = __shfl_down_sync(0xffffffffu, key, o);
-                const bool take = (lane + o < 32) && (ko == key);
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int ko = __shfl_down_sync(0xffffffffu, key, o);
+                    const bool take = (lane + o < 32) && (ko == key);
 #pragma unroll
-                for (int q = 0; q < 12; ++q) {
-                    const float vo = __shfl_down_sync(0xffffffffu, red[q], o);
-                    if (take) red[q] += vo;
+                    for (int q = 0; q < 12; ++q) {
+                        const float vo = __shfl_down_sync(0xffffffffu, red[q], o);
+                        if (take) red[q] += vo;
+                    }
+                }
+                const int kprev = __shfl_up_sync(0xffffffffu, key, 1);
+                if (key >= 0 && (lane == 0 || kprev != key)) {
+                    double* fi = a.f + (size_t)cur.ba * 3;
+                    atomicAdd(fi, (double)red[0]); atomicAdd(fi + 1, (double)red[1]); atomicAdd(fi + 2, (double)red[2]);
+                    double* cp = a.cpart + (size_t)key * 9;
+#pragma unroll
+                    for (int q = 0; q < 9; ++q) atomicAdd(cp + q, (double)red[3 + q]);
                 }
             }
-            const int kprev = __shfl_up_sync(0xffffffffu, key, 1);
-            if (key >= 0 && (lane == 0 || kprev != key)) {
-                double* fi = a.f + (size_t)cur.ba * 3;
-                atomicAdd(fi, (double)red[0]); atomicAdd(fi + 1, (double)red[1]); atomicAdd(fi + 2, (double)red[2]);
-                double* cp = a.cpart + (size_t)key * 9;
-#pragma unroll
-                for (int q = 0; q < 9; ++q) atomicAdd(cp + q, (double)red[3 + q]);
-            }
-            named_bar_sync(1 + wg, 128);                   // dT stage / centre buffer are free again
-            cur = nxt;
+            named_bar_sync(bar_ctx, 256);                  // dT stage / centre / partial buffers are free again
         }
     }
     tc_fence_before();
@@ -718,7 +830,8 @@ virial_reduce_kernel(int ntypes, EmbTcArgs a, double* __restrict__ Xi) {
 size_t emb_tc_image_bytes() { return etc::kImgBytes; }
 
 // Builds the shared-memory image of one (t_i, t_j) embedding net from its packed FP64 weights
-// (W1[1][25], b1[25], W2[25][50], b2[50], W3[50][100], b3[100], row-major in x out).
+// (W1[1][25], b1[25], W2[25][50], b2[50], W3[50][100], b3[100], row-major in x out),
+// with the channel permutation / padding of `etc` applied (dummy channels get zero weights and biases).
 void emb_tc_build_image(const double* w, uint8_t* img) {
     using namespace etc;
     memset(img, 0, kImgBytes);
@@ -740,14 +853,30 @@ void emb_tc_build_image(const double* w, uint8_t* img) {
         memcpy(img + o_hi + off, &hi, 4);
         memcpy(img + o_lo + off, &lo, 4);
     };
-    for (int n = 0; n < E2; ++n) {
-        for (int k = 0; k < E1; ++k) put(oW2hi, oW2lo, N2, n, k, (float)W2[k * E2 + n]);
-        put(oW2hi, oW2lo, N2, n, E1, (float)b2[n]);
-    }
-    for (int n = 0; n < M1; ++n) {
-        for (int k = 0; k < E2; ++k) put(oW3hi, oW3lo, N3, n, k, (float)W3[k * M1 + n]);
-        put(oW3hi, oW3lo, N3, n, E2, (float)b3[n]);
-    }
+    for (int h = 0; h < 2; ++h)
+        for (int j = 0; j < H2; ++j) {
+            const int n_orig = h2_orig(h, j);
+            if (n_orig < 0) continue;
+            const int n = n2_of(h, j);
+            for (int hh = 0; hh < 2; ++hh)
+                for (int i = 0; i < H1; ++i) {
+                    const int c1 = H1 * hh + i;
+                    if (c1 < E1) put(oW2hi, oW2lo, N2, n, k2_of(hh, i), (float)W2[c1 * E2 + n_orig]);
+                }
+            put(oW2hi, oW2lo, N2, n, kBias2, (float)b2[n_orig]);
+        }
+    for (int h = 0; h < 2; ++h)
+        for (int g = 0; g < H3; ++g) {
+            const int n_orig = g_orig(h, g);
+            if (n_orig < 0) continue;
+            const int n = n3_of(h, g);
+            for (int hh = 0; hh < 2; ++hh)
+                for (int j = 0; j < H2; ++j) {
+                    const int k_orig = h2_orig(hh, j);
+                    if (k_orig >= 0) put(oW3hi, oW3lo, N3, n, k3_of(hh, j), (float)W3[k_orig * M1 + n_orig]);
+                }
+            put(oW3hi, oW3lo, N3, n, kBias3, (float)b3[n_orig]);
+        }
     float* l1 = reinterpret_cast<float*>(img + oW1);
     for (int k = 0; k < E1; ++k) { l1[k] = (float)W1[k]; l1[32 + k] = (float)b1[k]; }
 }
