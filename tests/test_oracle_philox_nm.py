@@ -65,11 +65,19 @@ def test_philox_vectorised_equals_scalar():
 
 def test_keying_is_injective_in_every_field():
     base = [int(w) for w in philox.words_for(7, 3, 2, 5, 1)]
-    for other in [(8, 3, 2, 5, 1), (7, 4, 2, 5, 1), (7, 3, 3, 5, 1), (7, 3, 2, 6, 1), (7, 3, 2, 5, 2),
+    for other in [(8, 3, 2, 5, 1), (7, 4, 2, 5, 1), (7, 3, 4, 5, 1), (7, 3, 2, 6, 1), (7, 3, 2, 5, 2),
                   (7 + 2 ** 32, 3, 2, 5, 1), (7, 3 + 2 ** 32, 2, 5, 1)]:
         assert [int(w) for w in philox.words_for(*other)] != base
-    # counter word 3 is 4*k + alpha: (k=1, alpha=0) must differ from (k=0, alpha=3) + 1 etc.
-    assert [int(w) for w in philox.words_for(7, 3, 1, 5, 0)] != [int(w) for w in philox.words_for(7, 3, 0, 5, 3)]
+    # counter word 3 is 4*(k//2) + alpha: (k=2, alpha=0) must differ from (k=0, alpha=3) + 1 etc.
+    assert [int(w) for w in philox.words_for(7, 3, 2, 5, 0)] != [int(w) for w in philox.words_for(7, 3, 0, 5, 3)]
+    # modes 2q and 2q+1 share the draw (same words) and take different Box-Muller branches
+    assert [int(w) for w in philox.words_for(7, 3, 3, 5, 1)] == base
+    e2, e3 = float(philox.normal(7, 3, 2, 5, 1)), float(philox.normal(7, 3, 3, 5, 1))
+    w = base
+    u1 = float(philox.uniform53(w[0], w[1])) + 2.0 ** -53
+    u2 = float(philox.uniform53(w[2], w[3]))
+    assert abs(e2 * e2 + e3 * e3 - (-2.0 * math.log(u1))) < 1e-12          # cos^2 + sin^2 = 1
+    assert abs(math.atan2(e3, e2) % (2 * math.pi) - 2 * math.pi * u2) < 1e-12
 
 
 def test_uniform_grid_and_normal_finite_at_extremes():
@@ -91,6 +99,11 @@ def test_normal_moments():
     # different steps are uncorrelated
     eta2 = philox.normal(1234, 18, k, i, a).ravel()
     assert abs(np.mean(eta * eta2)) < 4.0 / math.sqrt(n)
+    # the two branches of one draw (modes 2q, 2q+1) are uncorrelated, also in their squares
+    ev = philox.normal(1234, 17, k, i, a)
+    c, s_ = ev[0::2].ravel(), ev[1::2].ravel()
+    assert abs(np.mean(c * s_)) < 4.0 / math.sqrt(c.size)
+    assert abs(np.mean((c * c - 1.0) * (s_ * s_ - 1.0))) < 4.0 * 2.0 / math.sqrt(c.size)
 
 
 # ---------------------------------------------------------------- normal modes (PAPER.md B1-B3)
