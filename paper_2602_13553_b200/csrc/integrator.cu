@@ -105,12 +105,15 @@ constexpr int kIntThreads = 128;
 template <int P>
 __global__ void __launch_bounds__(kIntThreads)
 integrator_kernel(const __grid_constant__ IntegratorArgs a, const __grid_constant__ ModeConsts mc) {
-    // dynamic smem: x and f tiles [P][kIntThreads] staged with cp.async (all 2P loads of a thread are in
-    // flight at once, independent of the register budget), then the thermostat normals [P][kIntThreads]
+    // dynamic smem: f, x and v~ tiles [P][kIntThreads], staged with cp.async in that order (all 3P loads of
+    // a thread are in flight at once, independent of the register budget).  Every thread only ever touches
+    // its own column, so no block-level synchronisation is needed and the thermostat normals can overlay
+    // the f tile once f sits in registers.
     extern __shared__ double dyn_s[];
-    double* xs = dyn_s;
-    double* fs = dyn_s + P * kIntThreads;
-    double* eta_s = dyn_s + 2 * P * kIntThreads;
+    double* fs = dyn_s + threadIdx.x;
+    double* xs = fs + P * kIntThreads;
+    double* vs = xs + P * kIntThreads;
+    double* eta_s = fs;
     const int e = blockIdx.x * kIntThreads + threadIdx.x;
     const bool live = e < a.n_dof;
     const int ec = live ? e : a.n_dof - 1;             // dead threads shadow the last dof, never store
@@ -120,34 +123,41 @@ integrator_kernel(const __grid_constant__ IntegratorArgs a, const __grid_constan
     const size_t stride = (size_t)a.n_dof;
 
 #pragma unroll
-    for (int k = 0; k < P; ++k) {
-        __pipeline_memcpy_async(xs + k * kIntThreads + threadIdx.x, a.x_in + k * stride + ec, sizeof(double));
-        __pipeline_memcpy_async(fs + k * kIntThreads + threadIdx.x, a.f + k * stride + ec, sizeof(double));
-    }
+    for (int k = 0; k < P; ++k) __pipeline_memcpy_async(fs + k * kIntThreads, a.f + k * stride + ec, sizeof(double));
+    __pipeline_commit();
+#pragma unroll
+    for (int k = 0; k < P; ++k) __pipeline_memcpy_async(xs + k * kIntThreads, a.x_in + k * stride + ec, sizeof(double));
+    __pipeline_commit();
+#pragma unroll
+    for (int k = 0; k < P; ++k) __pipeline_memcpy_async(vs + k * kIntThreads, a.vt_in + k * stride + ec, sizeof(double));
     __pipeline_commit();
 
-    // ---- O-step normals while the loads fly (rolled loop keeps one copy of log/cos) ----
+    const double m = a.mass[i];
+    double xt[P], ft[P];
+    __pipeline_wait_prior(2);
+#pragma unroll
+    for (int k = 0; k < P; ++k) ft[k] = fs[k * kIntThreads];
+
+    // ---- O-step normals while x and v~ are still in flight: one draw per mode pair (R-10) ----
     if (thermo) {
 #pragma unroll 4
-        for (int k = 0; k < P; ++k) {
-            eta_s[k * kIntThreads + threadIdx.x] =
-                philox_normal(a.seed_lo, a.seed_hi, a.step_lo, a.step_hi, (uint32_t)i, (uint32_t)(4 * k + alpha));
+        for (int q = 0; q < (P + 1) / 2; ++q) {
+            double ee, eo;
+            philox_normal_pair(a.seed_lo, a.seed_hi, a.step_lo, a.step_hi, (uint32_t)i, (uint32_t)(4 * q + alpha), &ee, &eo);
+            eta_s[(2 * q) * kIntThreads] = ee;
+            if (2 * q + 1 < P) eta_s[(2 * q + 1) * kIntThreads] = eo;
         }
     }
 
-    const double m = a.mass[i];
-    __pipeline_wait_prior(0);
-    double xt[P], ft[P];
+    __pipeline_wait_prior(1);
     double xf = 0.0;
 #pragma unroll
-    for (int k = 0; k < P; ++k) {
-        xt[k] = xs[k * kIntThreads + threadIdx.x];
-        ft[k] = fs[k * kIntThreads + threadIdx.x];
-    }
+    for (int k = 0; k < P; ++k) xt[k] = xs[k * kIntThreads];
 #pragma unroll
     for (int k = 0; k < P; ++k) xf += xt[k] * ft[k];
     nm_forward<P>(ft);                                  // f~ = M f      (L192, third transform)
     nm_forward<P>(xt);                                  // x~ = M x      (first transform)
+    __pipeline_wait_prior(0);
 
     const double kick = a.half_dt_mvv / m;              // (dt/2)/(m mvv2e)
     const double sigma = sqrt(a.PkT_mvv / m);           // sqrt(P k_B T/(m mvv2e))  (Eq. D2)
@@ -156,7 +166,7 @@ integrator_kernel(const __grid_constant__ IntegratorArgs a, const __grid_constan
     double accK = 0.0, accS = 0.0;
 #pragma unroll
     for (int k = 0; k < P; ++k) {
-        double v = a.vt_in[k * stride + ec];
+        double v = vs[k * kIntThreads];
         if (a.flags & I_BCLOSE) v += kick * ft[k];      // closing B of the previous step
         if (a.flags & I_EST) {
             accK += v * v;                               // A1: 1/2 m v~^2
@@ -167,7 +177,7 @@ integrator_kernel(const __grid_constant__ IntegratorArgs a, const __grid_constan
             const double x = xt[k];
             const double xn = mc.cosA[k] * x + mc.sinA_w[k] * v;    // A(dt/2): exact rotation (R-5)
             double vn = mc.msinA_w[k] * x + mc.cosA[k] * v;
-            if (thermo) vn = mc.c1[k] * vn + mc.c2[k] * sigma * eta_s[k * kIntThreads + threadIdx.x];   // O(dt)
+            if (thermo) vn = mc.c1[k] * vn + mc.c2[k] * sigma * eta_s[k * kIntThreads];   // O(dt)
             xt[k] = mc.cosA[k] * xn + mc.sinA_w[k] * vn;            // A(dt/2)
             v = mc.msinA_w[k] * xn + mc.cosA[k] * vn;
         }
@@ -330,9 +340,11 @@ __global__ void debug_noise_kernel(uint32_t seed_lo, uint32_t seed_hi, uint32_t 
     if (t >= n) return;
     const uint32_t k = idx[3 * t], i = idx[3 * t + 1], al = idx[3 * t + 2];
     uint32_t w[4];
-    philox4x32_10(step_lo, step_hi, i, 4u * k + al, seed_lo, seed_hi, w);
+    philox4x32_10(step_lo, step_hi, i, 4u * (k >> 1) + al, seed_lo, seed_hi, w);
     for (int q = 0; q < 4; ++q) words[4 * t + q] = w[q];
-    eta[t] = philox_normal(seed_lo, seed_hi, step_lo, step_hi, i, 4u * k + al);
+    double ee, eo;
+    philox_normal_pair(seed_lo, seed_hi, step_lo, step_hi, i, 4u * (k >> 1) + al, &ee, &eo);
+    eta[t] = (k & 1u) ? eo : ee;
 }
 
 int launch_debug_noise(uint64_t seed, uint64_t step, int n, const int32_t* idx, uint32_t* words, double* eta,

@@ -18,17 +18,29 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-// eta = sqrt(-2 ln u1) cos(2 pi u2), u1 = (n1 + 1) 2^-53 in (0,1], u2 = n2 2^-53 in [0,1),
-// n = (w_a >> 5) 2^26 + (w_b >> 6)  (Box-Muller, cosine branch; DESIGN R-10; Eq. D2's eta)
-__device__ __forceinline__ double philox_normal(uint32_t seed_lo, uint32_t seed_hi, uint32_t step_lo,
-                                                uint32_t step_hi, uint32_t atom, uint32_t kdim) {
+// 53-bit grid uniform ((wa >> 5) 2^26 + (wb >> 6) + add) 2^-53, exact: the two pieces are turned into doubles
+// by the 2^52 exponent trick (no 64-bit integer conversion), both products and the sum are exact.
+__device__ __forceinline__ double philox_u53(uint32_t wa, uint32_t wb, uint32_t add) {
+    const double dh = __hiloint2double(0x43300000, (int)(wa >> 5)) - 4503599627370496.0;
+    const double dl = __hiloint2double(0x43300000, (int)((wb >> 6) + add)) - 4503599627370496.0;
+    return fma(dh, 0x1p-27, dl * 0x1p-53);
+}
+
+// Thermostat normals of the mode pair (2q, 2q+1) of atom `atom`, component alpha (DESIGN R-10; Eq. D2's eta,
+// PAPER.md:L476): one draw, counter word 3 = 4q + alpha; u1 in (0,1], u2 in [0,1);
+// r = sqrt(-2 ln u1); eta_even = r cos(2 pi u2), eta_odd = r sin(2 pi u2)  (Box-Muller, both branches).
+__device__ __forceinline__ void philox_normal_pair(uint32_t seed_lo, uint32_t seed_hi, uint32_t step_lo,
+                                                   uint32_t step_hi, uint32_t atom, uint32_t qdim, double* eta_even,
+                                                   double* eta_odd) {
     uint32_t w[4];
-    philox4x32_10(step_lo, step_hi, atom, kdim, seed_lo, seed_hi, w);
-    const uint64_t n1 = ((uint64_t)(w[0] >> 5) << 26) + (uint64_t)(w[1] >> 6);
-    const uint64_t n2 = ((uint64_t)(w[2] >> 5) << 26) + (uint64_t)(w[3] >> 6);
-    const double u1 = (double)n1 * 0x1p-53 + 0x1p-53;     // exact
-    const double u2 = (double)n2 * 0x1p-53;
-    return sqrt(-2.0 * log(u1)) * cospi(2.0 * u2);
+    philox4x32_10(step_lo, step_hi, atom, qdim, seed_lo, seed_hi, w);
+    const double u1 = philox_u53(w[0], w[1], 1u);
+    const double u2 = philox_u53(w[2], w[3], 0u);
+    const double r = sqrt(-2.0 * log(u1));
+    double sn, cs;
+    sincospi(2.0 * u2, &sn, &cs);
+    *eta_even = r * cs;
+    *eta_odd = r * sn;
 }
 
 }  // namespace pimd
