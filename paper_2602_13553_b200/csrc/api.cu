@@ -112,7 +112,7 @@ size_t model_bytes(const pimd_ctx* c, const pimd_model_desc* d) {
     cell_grid(c->box, d->rcut, ncell, R, &ncells);
     size_t b = 0;
     b += align_up((size_t)d->n_types * d->n_types * 8192 * 4, 256);                     // embedding weights (padded)
-    b += (size_t)d->n_types * 2 * (align_up((size_t)ND * NF * 4, 256) + 2 * align_up((size_t)NF * NF * 4, 256) + align_up(NF * 4, 256));
+    b += (size_t)d->n_types * 6 * (align_up((size_t)ND * NF * 4, 256) + 2 * align_up((size_t)NF * NF * 4, 256) + align_up(NF * 4, 256));
     b += (size_t)d->n_types * 4 * align_up((size_t)NF * 4, 256);
     b += 4 * align_up(PN * 4, 256);                                                    // cen_idx,row_of,cell_id,cell_tmp
     b += 3 * align_up((size_t)c->P * (ncells + 1) * 4, 256);
@@ -486,6 +486,14 @@ int pimd_set_model(pimd_ctx* ctx, const pimd_model_desc* d, const double* w, siz
             CK(cudaMemcpyAsync(m.fit_w[t][l], W.data(), W.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
             CK(cudaMemcpyAsync(m.fit_wT[t][l], WT.data(), WT.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
             CK(cudaMemcpyAsync(m.fit_b[t][l], b.data(), b.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
+            if (l < 3) {          // TF32 hi / lo images of W and W^T for the tensor-core GEMMs
+                if ((rc = arena_alloc(ctx, &m.fit_w_hi[t][l], W.size()))) return rc;
+                if ((rc = arena_alloc(ctx, &m.fit_w_lo[t][l], W.size()))) return rc;
+                if ((rc = arena_alloc(ctx, &m.fit_wT_hi[t][l], W.size()))) return rc;
+                if ((rc = arena_alloc(ctx, &m.fit_wT_lo[t][l], W.size()))) return rc;
+                tc_split_weights(W.size(), m.fit_w[t][l], m.fit_w_hi[t][l], m.fit_w_lo[t][l], ctx->stream);
+                tc_split_weights(W.size(), m.fit_wT[t][l], m.fit_wT_hi[t][l], m.fit_wT_lo[t][l], ctx->stream);
+            }
             keep.push_back(std::move(W)); keep.push_back(std::move(WT)); keep.push_back(std::move(b));
             nin = nout;
         }

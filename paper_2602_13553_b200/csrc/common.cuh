@@ -103,8 +103,10 @@ struct Model {
     bool     tc_ready = false;
     CUtensorMap mapA_D[PIMD_MAX_TYPES], mapA_Y1[PIMD_MAX_TYPES], mapA_Y2[PIMD_MAX_TYPES], mapA_G1[PIMD_MAX_TYPES],
                 mapA_T3[PIMD_MAX_TYPES];
-    CUtensorMap mapB_fwd[PIMD_MAX_TYPES][3];   // W_l^T  [out][in]
-    CUtensorMap mapB_bwd[PIMD_MAX_TYPES][3];   // W_l    [in][out]
+    CUtensorMap mapB_fwd_hi[PIMD_MAX_TYPES][3], mapB_fwd_lo[PIMD_MAX_TYPES][3];   // W_l^T  [out][in], TF32 hi / lo
+    CUtensorMap mapB_bwd_hi[PIMD_MAX_TYPES][3], mapB_bwd_lo[PIMD_MAX_TYPES][3];   // W_l    [in][out]
+    float*   fit_w_hi[PIMD_MAX_TYPES][3], *fit_w_lo[PIMD_MAX_TYPES][3];           // pre-split weights (layers 1..3)
+    float*   fit_wT_hi[PIMD_MAX_TYPES][3], *fit_wT_lo[PIMD_MAX_TYPES][3];
     // tensor-core embedding path (embedding_tc.cu)
     bool     use_tc_emb = true;
     bool     tc_emb_ready = false;
@@ -132,6 +134,8 @@ int fitting_forward_backward(Model& m, const ForceArgs& a, cudaStream_t s);
 int embedding_backward(Model& m, const ForceArgs& a, int n_sms, cudaStream_t s);
 size_t embedding_smem_bytes(const Model& m, int ntypes);
 bool tc_setup_maps(Model& m, int ntypes);
+void tc_split_weights(size_t n, const float* w, float* hi, float* lo, cudaStream_t s);
+int fitting_chain_tc(Model& m, const ForceArgs& a, cudaStream_t s);
 size_t emb_tc_image_bytes();
 void emb_tc_build_image(const double* w_pair, uint8_t* img);
 int emb_tc_row_index(Model& m, const ForceArgs& a, cudaStream_t s);

@@ -200,26 +200,21 @@ energy_kernel(int row0, int rows, int NF, int N, const float* __restrict__ Y3, c
     }
 }
 
-int fitting_gemms_tc(Model& m, int t, cudaStream_t s);
-int fitting_gemms_tc_bwd(Model& m, int t, cudaStream_t s);
-
 int fitting_forward_backward(Model& m, const ForceArgs& a, cudaStream_t s) {
     const int PN = a.P * a.N;
     const int NF = m.NF, ND = m.ND;
     int launches = 2;
     descriptor_kernel<100, 16><<<PN, 256, 0, s>>>(PN, m.Tm, m.D);
+    if (m.use_tc && m.tc_ready) {
+        launches += fitting_chain_tc(m, a, s);           // all centre types per launch; energy fused into layer 3
+        dT_kernel<100, 16><<<PN, 128, 0, s>>>(PN, m.Tm, m.dD, m.dTm);
+        return launches;
+    }
     for (int t = 0; t < a.ntypes; ++t) {
         const int row0 = m.type_row0[t], rows = m.type_row0[t + 1] - row0;
         if (rows == 0) continue;
         launches += 7;
         const size_t oF = (size_t)row0 * NF, oD = (size_t)row0 * ND;
-        if (m.use_tc && m.tc_ready) {
-            fitting_gemms_tc(m, t, s);
-            energy_kernel<<<(rows * 32 + 127) / 128, 128, 0, s>>>(row0, rows, NF, a.N, m.Y3, m.T3, m.fit_w[t][3],
-                                                                  m.fit_b[t][3], m.cen_idx, a.Eatom, a.U, m.G1, m.G2);
-            fitting_gemms_tc_bwd(m, t, s);
-            continue;
-        }
         GemmArgs g{};
         // layer 1: Y1 = tanh(D W1 + b1)
         g.M = rows; g.N = NF; g.K = ND; g.A = m.D + oD; g.lda = ND; g.B = m.fit_w[t][0]; g.ldb = NF;

@@ -1,16 +1,18 @@
 // fitting_tc.cu -- the fitting-net GEMMs of F4 on the 5th-generation tensor cores.
+// One launch per layer covers the rows of all centre types (tiles numbered type by type).
 //
 //   C[M x N] = epilogue( A[M x K] . Bt[N x K]^T ),  FP32 in / FP32 out, computed as 3xTF32:
 //   a = a_hi + a_lo, b = b_hi + b_lo (hi = top 10 mantissa bits, lo = exact remainder)
 //   a.b ~= a_hi.b_hi + a_lo.b_hi + a_hi.b_lo     (FP32 accumulate in TMEM; dropped term ~2^-22)
 // which keeps the force error at the FP32 level (single-pass TF32 fails north_star's 1e-4).
 //
-// One CTA computes a 256 x BN tile (two M = 128 accumulators, 2 x BN <= 512 TMEM columns) so that every
-// weight tile is used for 256 rows.  Warp roles (192 threads):
-//   warp 0   TMA producer: raw FP32 A (2 boxes 16 x 128) and B (box 16 x BN) tiles, SWIZZLE_64B, 3 stages
-//   warp 1   TMEM allocation + single-thread tcgen05.mma issue (12 MMAs of 128 x BN x 8 per stage)
-//   warps 2-5 split hi/lo in shared memory (elementwise, so the swizzled layout is preserved), then the
-//            epilogue: tcgen05.ld accumulators -> bias / tanh / skip / derivative -> global
+// One CTA computes a (128 NH) x BN tile (NH accumulators of M = 128 in TMEM).  Warp roles (192 threads):
+//   warp 0   TMA producer: raw FP32 A (NH boxes 16 x 128) and the PRE-SPLIT weights B_hi, B_lo (boxes 16 x BN),
+//            SWIZZLE_64B, ST stages
+//   warp 1   TMEM allocation + single-thread tcgen05.mma issue (6 NH MMAs of 128 x BN x 8 per stage)
+//   warps 2-5 split A into hi/lo in shared memory (elementwise, so the swizzled layout is preserved), then
+//            the epilogue: tcgen05.ld accumulators -> bias / tanh / skip / derivative / energy -> global
+// Two CTAs share an SM (2 x 256 TMEM columns, 2 x 2 stages), so one CTA's epilogue runs under the other's MMAs.
 #include "common.cuh"
 #include "tc_gemm.cuh"
 
@@ -18,55 +20,78 @@ namespace pimd {
 
 using namespace tc;
 
-enum : int { TEPI_TANH_BIAS = 0, TEPI_TANH_BIAS_SKIP = 1, TEPI_BWD = 2, TEPI_BWD_FIRST = 3, TEPI_PLAIN = 4 };
+enum : int { TEPI_TANH_BIAS = 0, TEPI_TANH_BIAS_SKIP = 1, TEPI_BWD_VEC = 2, TEPI_BWD_FIRST = 3, TEPI_PLAIN = 4, TEPI_L3E = 5 };
+
+constexpr int kMaxT = PIMD_MAX_TYPES;
+
+// one launch covers the rows of ALL centre types: M tiles are numbered type by type
+struct TcMaps {
+    CUtensorMap A[kMaxT];       // activations of type t: [rows_t][K], box 16 x 128
+    CUtensorMap Bhi[kMaxT];     // weights of type t, TF32 hi part: [N][K] (K-major), box 16 x BN
+    CUtensorMap Blo[kMaxT];     // exact remainder
+};
 
 struct TcGemmArgs {
-    int M, N, K;               // N = logical columns of C (multiple of BN chunks handled by grid.x)
-    const float* bias;
-    const float* add; int ldadd;
+    int ntypes, N, K;               // N = logical columns of C (grid.x chunks of BN)
+    int tile0[kMaxT + 1];           // first M tile of each type
+    int row0[kMaxT + 1];            // first (type-sorted) row of each type
+    const float* bias[kMaxT];
+    const float* vec[kMaxT];        // TEPI_L3E: w4 ; TEPI_BWD_VEC: dy3 = w4 (a row vector)
+    const float* b4[kMaxT];
+    const float* add; int ldadd;    // matrices indexed by the global (type-sorted) row
     const float* tt; int ldtt;
     float* out0; float* out1; int ldo;
+    const int* cen_idx; double* Eatom; double* U; int natoms;    // TEPI_L3E
 };
 
 constexpr int kTcThreads = 192;
-constexpr int kTcStages = 3;
 constexpr int kTcBK = 16;                 // floats per K block = 64 B rows (SWIZZLE_64B)
 
-template <int BN>
+template <int BN, int NH, int ST>
 struct TcSmem {
     static constexpr int kABytes = 128 * 64;                      // one 128-row half
     static constexpr int kBBytes = BN * 64;
-    static constexpr int oAhi = 0, oAlo = 2 * kABytes, oBhi = 4 * kABytes, oBlo = 4 * kABytes + kBBytes;
-    static constexpr int kStage = 4 * kABytes + 2 * kBBytes;
-    static constexpr int kTotal = kTcStages * kStage + 1024 /*align slack*/ + 256 /*barriers*/;
+    static constexpr int oAhi = 0, oAlo = NH * kABytes, oBhi = 2 * NH * kABytes, oBlo = 2 * NH * kABytes + kBBytes;
+    static constexpr int kStage = 2 * NH * kABytes + 2 * kBBytes;
+    static constexpr int kTotal = ST * kStage + 1024 /*align slack*/ + 256 /*barriers*/;
+    static constexpr int kTmemCols = (NH * BN <= 256) ? 256 : 512;
 };
 
-template <int BN, int EPI>
-__global__ void __launch_bounds__(kTcThreads, 1)
-gemm3xtf32_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constant__ CUtensorMap mapB,
-                  const __grid_constant__ TcGemmArgs g) {
-    using SM = TcSmem<BN>;
+// BN: N tile; EPI: epilogue; NH: 128-row halves per CTA; ST: pipeline stages; OCC: CTAs per SM
+template <int BN, int EPI, int NH, int ST, int OCC>
+__global__ void __launch_bounds__(kTcThreads, OCC)
+gemm3xtf32_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ TcGemmArgs g) {
+    using SM = TcSmem<BN, NH, ST>;
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);   // keeps the shared address space
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kTcStages * SM::kStage);
-    uint64_t* full = bars;                     // [stages] TMA -> split warps
-    uint64_t* ready = bars + kTcStages;        // [stages] split warps -> MMA
-    uint64_t* empty = bars + 2 * kTcStages;    // [stages] MMA -> TMA
-    uint64_t* tmem_full = bars + 3 * kTcStages;
-    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(bars + 3 * kTcStages + 1);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + ST * SM::kStage);
+    uint64_t* full = bars;                     // [stages] TMA -> split warps (A) and MMA (B)
+    uint64_t* ready = bars + ST;               // [stages] split warps -> MMA
+    uint64_t* empty = bars + 2 * ST;           // [stages] MMA -> TMA
+    uint64_t* tmem_full = bars + 3 * ST;
+    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(bars + 3 * ST + 1);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int m0 = blockIdx.y * 256, n0 = blockIdx.x * BN;
+    int ty = 0;
+#pragma unroll
+    for (int t = 1; t < kMaxT; ++t)
+        if (t < g.ntypes && (int)blockIdx.y >= g.tile0[t]) ty = t;
+    const int m0 = ((int)blockIdx.y - g.tile0[ty]) * (128 * NH), n0 = blockIdx.x * BN;
+    const int rows_t = g.row0[ty + 1] - g.row0[ty];
     const int nk = g.K / kTcBK;
+    const CUtensorMap* mapA = &maps.A[ty];
+    const CUtensorMap* mapBhi = &maps.Bhi[ty];
+    const CUtensorMap* mapBlo = &maps.Blo[ty];
 
     if (warp == 0 && lane == 0) {
-        tma_prefetch_desc(&mapA);
-        tma_prefetch_desc(&mapB);
-        for (int s = 0; s < kTcStages; ++s) { mbar_init(full + s, 1); mbar_init(ready + s, 128); mbar_init(empty + s, 1); }
+        tma_prefetch_desc(mapA);
+        tma_prefetch_desc(mapBhi);
+        tma_prefetch_desc(mapBlo);
+        for (int s = 0; s < ST; ++s) { mbar_init(full + s, 1); mbar_init(ready + s, 128); mbar_init(empty + s, 1); }
         mbar_init(tmem_full, 1);
         fence_barrier_init();
     }
-    if (warp == 1) tmem_alloc(tmem_ptr, 512);
+    if (warp == 1) tmem_alloc(tmem_ptr, SM::kTmemCols);
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
@@ -75,25 +100,26 @@ gemm3xtf32_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
     if (warp == 0) {
         if (lane == 0) {
             for (int kb = 0; kb < nk; ++kb) {
-                const int s = kb % kTcStages, ph = (kb / kTcStages) & 1;
+                const int s = kb % ST, ph = (kb / ST) & 1;
                 mbar_wait(empty + s, ph ^ 1);
                 uint8_t* st = smem + s * SM::kStage;
-                mbar_arrive_expect_tx(full + s, 2 * SM::kABytes + SM::kBBytes);
-                tma_load_2d(st + SM::oAhi, &mapA, full + s, kb * kTcBK, m0);
-                tma_load_2d(st + SM::oAhi + SM::kABytes, &mapA, full + s, kb * kTcBK, m0 + 128);
-                tma_load_2d(st + SM::oBhi, &mapB, full + s, kb * kTcBK, n0);
+                mbar_arrive_expect_tx(full + s, NH * SM::kABytes + 2 * SM::kBBytes);
+#pragma unroll
+                for (int h = 0; h < NH; ++h) tma_load_2d(st + SM::oAhi + h * SM::kABytes, mapA, full + s, kb * kTcBK, m0 + 128 * h);
+                tma_load_2d(st + SM::oBhi, mapBhi, full + s, kb * kTcBK, n0);
+                tma_load_2d(st + SM::oBlo, mapBlo, full + s, kb * kTcBK, n0);
             }
         }
     } else if (warp == 1) {
         if (lane == 0) {
             constexpr uint32_t idesc = make_idesc_tf32(128, BN);
             for (int kb = 0; kb < nk; ++kb) {
-                const int s = kb % kTcStages, ph = (kb / kTcStages) & 1;
+                const int s = kb % ST, ph = (kb / ST) & 1;
                 mbar_wait(ready + s, ph);
                 tc_fence_after();
                 const uint32_t st = smem_u32(smem + s * SM::kStage);
 #pragma unroll
-                for (int h = 0; h < 2; ++h) {
+                for (int h = 0; h < NH; ++h) {
                     const uint32_t d = tmem_base + h * 256;
 #pragma unroll
                     for (int ks = 0; ks < 2; ++ks) {
@@ -111,16 +137,17 @@ gemm3xtf32_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
             umma_commit(tmem_full);
         }
     } else {
-        // ---- split hi / lo in place (128 threads) ----
+        // ---- split A into hi / lo in place (128 threads; elementwise, so the swizzled layout is preserved;
+        //      the weights arrive pre-split) ----
         const int t = threadIdx.x - 64;
         for (int kb = 0; kb < nk; ++kb) {
-            const int s = kb % kTcStages, ph = (kb / kTcStages) & 1;
+            const int s = kb % ST, ph = (kb / ST) & 1;
             mbar_wait(full + s, ph);
             uint8_t* st = smem + s * SM::kStage;
             float4* a_hi = reinterpret_cast<float4*>(st + SM::oAhi);
             float4* a_lo = reinterpret_cast<float4*>(st + SM::oAlo);
 #pragma unroll
-            for (int q = 0; q < (2 * SM::kABytes / 16) / 128; ++q) {
+            for (int q = 0; q < (NH * SM::kABytes / 16) / 128; ++q) {
                 const int idx = t + q * 128;
                 const float4 v = a_hi[idx];
                 float4 hi, lo;
@@ -131,29 +158,19 @@ gemm3xtf32_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
                 a_hi[idx] = hi;
                 a_lo[idx] = lo;
             }
-            float4* b_hi = reinterpret_cast<float4*>(st + SM::oBhi);
-            float4* b_lo = reinterpret_cast<float4*>(st + SM::oBlo);
-            for (int idx = t; idx < SM::kBBytes / 16; idx += 128) {
-                const float4 v = b_hi[idx];
-                float4 hi, lo;
-                hi.x = __uint_as_float(__float_as_uint(v.x) & 0xFFFFE000u); lo.x = v.x - hi.x;
-                hi.y = __uint_as_float(__float_as_uint(v.y) & 0xFFFFE000u); lo.y = v.y - hi.y;
-                hi.z = __uint_as_float(__float_as_uint(v.z) & 0xFFFFE000u); lo.z = v.z - hi.z;
-                hi.w = __uint_as_float(__float_as_uint(v.w) & 0xFFFFE000u); lo.w = v.w - hi.w;
-                b_hi[idx] = hi;
-                b_lo[idx] = lo;
-            }
             fence_proxy_async_smem();
             mbar_arrive(ready + s);
         }
-        // ---- epilogue ----
+        // ---- epilogue: one thread per row ----
         mbar_wait(tmem_full, 0);
         tc_fence_after();
         const int quarter = warp & 3;                      // TMEM lane quarter this warp may access
 #pragma unroll 1
-        for (int h = 0; h < 2; ++h) {
-            const int m = m0 + h * 128 + quarter * 32 + lane;
-            const bool row_ok = m < g.M;
+        for (int h = 0; h < NH; ++h) {
+            const int ml = m0 + h * 128 + quarter * 32 + lane;     // row inside the type
+            const bool row_ok = ml < rows_t;
+            const size_t m = (size_t)(g.row0[ty] + ml);            // type-sorted global row
+            float e_acc = 0.f;
 #pragma unroll 1
             for (int c = 0; c < BN / 16; ++c) {
                 uint32_t v[16];
@@ -164,42 +181,75 @@ gemm3xtf32_kernel(const __grid_constant__ CUtensorMap mapA, const __grid_constan
                 float r[16];
 #pragma unroll
                 for (int q = 0; q < 16; ++q) r[q] = __uint_as_float(v[q]);
-                if (EPI == TEPI_TANH_BIAS || EPI == TEPI_TANH_BIAS_SKIP) {
+                if (EPI == TEPI_TANH_BIAS || EPI == TEPI_TANH_BIAS_SKIP || EPI == TEPI_L3E) {
+                    const float* bias = g.bias[ty] + n;
 #pragma unroll
-                    for (int q = 0; q < 16; ++q) r[q] = tanhf(r[q] + __ldg(g.bias + n + q));
+                    for (int q = 0; q < 16; ++q) r[q] = tanhf(r[q] + __ldg(bias + q));
                 }
-                float4* o0 = (g.out0 != nullptr) ? reinterpret_cast<float4*>(g.out0 + (size_t)m * g.ldo + n) : nullptr;
-                float4* o1 = (g.out1 != nullptr) ? reinterpret_cast<float4*>(g.out1 + (size_t)m * g.ldo + n) : nullptr;
+                float4* o0 = (g.out0 != nullptr) ? reinterpret_cast<float4*>(g.out0 + m * g.ldo + n) : nullptr;
+                float4* o1 = (g.out1 != nullptr) ? reinterpret_cast<float4*>(g.out1 + m * g.ldo + n) : nullptr;
                 if (EPI == TEPI_TANH_BIAS || EPI == TEPI_PLAIN) {
 #pragma unroll
                     for (int q = 0; q < 4; ++q) o0[q] = make_float4(r[4 * q], r[4 * q + 1], r[4 * q + 2], r[4 * q + 3]);
                 } else if (EPI == TEPI_TANH_BIAS_SKIP) {
-                    const float4* ad = reinterpret_cast<const float4*>(g.add + (size_t)m * g.ldadd + n);
+                    const float4* ad = reinterpret_cast<const float4*>(g.add + m * g.ldadd + n);
 #pragma unroll
                     for (int q = 0; q < 4; ++q) {
                         o0[q] = make_float4(r[4 * q], r[4 * q + 1], r[4 * q + 2], r[4 * q + 3]);
                         const float4 a4 = ad[q];
                         o1[q] = make_float4(r[4 * q] + a4.x, r[4 * q + 1] + a4.y, r[4 * q + 2] + a4.z, r[4 * q + 3] + a4.w);
                     }
-                } else {   // TEPI_BWD, TEPI_BWD_FIRST
-                    const float4* ad = reinterpret_cast<const float4*>(g.add + (size_t)m * g.ldadd + n);
-                    const float4* tt = reinterpret_cast<const float4*>(g.tt + (size_t)m * g.ldtt + n);
+                } else if (EPI == TEPI_L3E) {
+                    // y3 = y2 + t3 ; E_i += y3 . w4 ; seed of the backward pass da3 = w4 o (1 - t3^2) -> out1
+                    const float4* ad = reinterpret_cast<const float4*>(g.add + m * g.ldadd + n);
+                    const float4* w4 = reinterpret_cast<const float4*>(g.vec[ty] + n);
 #pragma unroll
                     for (int q = 0; q < 4; ++q) {
-                        const float4 a4 = ad[q], t4 = tt[q];
+                        const float4 a4 = ad[q], w = __ldg(w4 + q);
+                        e_acc = fmaf(a4.x + r[4 * q], w.x, e_acc);
+                        e_acc = fmaf(a4.y + r[4 * q + 1], w.y, e_acc);
+                        e_acc = fmaf(a4.z + r[4 * q + 2], w.z, e_acc);
+                        e_acc = fmaf(a4.w + r[4 * q + 3], w.w, e_acc);
+                        o1[q] = make_float4(w.x * (1.f - r[4 * q] * r[4 * q]), w.y * (1.f - r[4 * q + 1] * r[4 * q + 1]),
+                                            w.z * (1.f - r[4 * q + 2] * r[4 * q + 2]), w.w * (1.f - r[4 * q + 3] * r[4 * q + 3]));
+                    }
+                } else {   // TEPI_BWD_VEC, TEPI_BWD_FIRST
+                    const float4* tt = reinterpret_cast<const float4*>(g.tt + m * g.ldtt + n);
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        const float4 a4 = (EPI == TEPI_BWD_VEC) ? __ldg(reinterpret_cast<const float4*>(g.vec[ty] + n) + q)
+                                                                : reinterpret_cast<const float4*>(g.add + m * g.ldadd + n)[q];
+                        const float4 t4 = tt[q];
                         float4 y = make_float4(r[4 * q] + a4.x, r[4 * q + 1] + a4.y, r[4 * q + 2] + a4.z, r[4 * q + 3] + a4.w);
-                        if (EPI == TEPI_BWD) o0[q] = y;
+                        if (EPI == TEPI_BWD_VEC) o0[q] = y;
                         y.x *= (1.f - t4.x * t4.x); y.y *= (1.f - t4.y * t4.y);
                         y.z *= (1.f - t4.z * t4.z); y.w *= (1.f - t4.w * t4.w);
                         o1[q] = y;
                     }
                 }
             }
+            if (EPI == TEPI_L3E) {
+                // E_i = y3 . w4 + b4 ; U^(bead) += E_i : one atomic per warp when its rows share the bead
+                const int ba = row_ok ? g.cen_idx[m] : 0;
+                const double e = row_ok ? (double)(e_acc + __ldg(g.b4[ty])) : 0.0;
+                if (row_ok) g.Eatom[ba] = e;
+                const int bead = row_ok ? ba / g.natoms : -1;
+                const int bead0 = __shfl_sync(0xffffffffu, bead, 0);
+                const bool uniform = __all_sync(0xffffffffu, bead == bead0 || bead < 0);
+                if (uniform) {
+                    double sum = e;
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+                    if (lane == 0 && bead0 >= 0) atomicAdd(g.U + bead0, sum);
+                } else if (row_ok) {
+                    atomicAdd(g.U + bead, e);
+                }
+            }
         }
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == 1) tmem_dealloc(tmem_base, 512);
+    if (warp == 1) tmem_dealloc(tmem_base, SM::kTmemCols);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -234,110 +284,159 @@ bool tc_make_map(CUtensorMap* map, const float* base, uint64_t rows, uint64_t co
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// w = hi + lo, hi = top 10 mantissa bits (what kind::tf32 reads), lo the exact remainder
+__global__ void split_hi_lo_kernel(size_t n, const float* __restrict__ w, float* __restrict__ hi, float* __restrict__ lo) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float v = w[i];
+    const float h = __uint_as_float(__float_as_uint(v) & 0xFFFFE000u);
+    hi[i] = h;
+    lo[i] = v - h;
+}
+void tc_split_weights(size_t n, const float* w, float* hi, float* lo, cudaStream_t s) {
+    split_hi_lo_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(n, w, hi, lo);
+}
+
+constexpr int kNH = 1, kST = 2, kOCC = 2;     // 128-row tiles, 2 stages, 2 CTAs per SM (one's epilogue under the other's MMAs)
+
 template <int BN, int EPI>
-static cudaError_t launch_tc(const CUtensorMap& mapA, const CUtensorMap& mapB, const TcGemmArgs& g, cudaStream_t s) {
-    using SM = TcSmem<BN>;
+static cudaError_t launch_tc(const TcMaps& maps, const TcGemmArgs& g, int mtiles, cudaStream_t s) {
+    using SM = TcSmem<BN, kNH, kST>;
     static bool attr = false;
     if (!attr) {
-        cudaError_t e = cudaFuncSetAttribute(gemm3xtf32_kernel<BN, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM::kTotal);
+        cudaError_t e = cudaFuncSetAttribute(gemm3xtf32_kernel<BN, EPI, kNH, kST, kOCC>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM::kTotal);
         if (e != cudaSuccess) return e;
         attr = true;
     }
-    dim3 grid((g.N + BN - 1) / BN, (g.M + 255) / 256);
-    gemm3xtf32_kernel<BN, EPI><<<grid, kTcThreads, SM::kTotal, s>>>(mapA, mapB, g);
+    dim3 grid((g.N + BN - 1) / BN, mtiles);
+    gemm3xtf32_kernel<BN, EPI, kNH, kST, kOCC><<<grid, kTcThreads, SM::kTotal, s>>>(maps, g);
     return cudaGetLastError();
 }
 
-// C = epi(A Bt^T): A [M][K] (lda), Bt [N][K] (ldb) row-major FP32.  bn = 240 (N == 240) or 160 (N % 160 == 0).
-cudaError_t tc_gemm(int epi, int bn, const CUtensorMap& mapA, const CUtensorMap& mapB, const TcGemmArgs& g, cudaStream_t s) {
+// C = epi(A Bt^T) for all centre types at once.  bn = 240 (N == 240) or 160 (N % 160 == 0).
+static cudaError_t tc_gemm(int epi, int bn, const TcMaps& maps, const TcGemmArgs& g, int mtiles, cudaStream_t s) {
     if (bn == 240) {
         switch (epi) {
-            case TEPI_TANH_BIAS: return launch_tc<240, TEPI_TANH_BIAS>(mapA, mapB, g, s);
-            case TEPI_TANH_BIAS_SKIP: return launch_tc<240, TEPI_TANH_BIAS_SKIP>(mapA, mapB, g, s);
-            case TEPI_BWD: return launch_tc<240, TEPI_BWD>(mapA, mapB, g, s);
-            case TEPI_BWD_FIRST: return launch_tc<240, TEPI_BWD_FIRST>(mapA, mapB, g, s);
-            case TEPI_PLAIN: return launch_tc<240, TEPI_PLAIN>(mapA, mapB, g, s);
+            case TEPI_TANH_BIAS: return launch_tc<240, TEPI_TANH_BIAS>(maps, g, mtiles, s);
+            case TEPI_TANH_BIAS_SKIP: return launch_tc<240, TEPI_TANH_BIAS_SKIP>(maps, g, mtiles, s);
+            case TEPI_L3E: return launch_tc<240, TEPI_L3E>(maps, g, mtiles, s);
+            case TEPI_BWD_VEC: return launch_tc<240, TEPI_BWD_VEC>(maps, g, mtiles, s);
+            case TEPI_BWD_FIRST: return launch_tc<240, TEPI_BWD_FIRST>(maps, g, mtiles, s);
+            case TEPI_PLAIN: return launch_tc<240, TEPI_PLAIN>(maps, g, mtiles, s);
         }
     } else if (bn == 160) {
-        if (epi == TEPI_PLAIN) return launch_tc<160, TEPI_PLAIN>(mapA, mapB, g, s);
+        if (epi == TEPI_PLAIN) return launch_tc<160, TEPI_PLAIN>(maps, g, mtiles, s);
     }
     return cudaErrorInvalidValue;
 }
 
+// tile / row bookkeeping shared by all launches of a model
+static int fill_types(const Model& m, int ntypes, TcGemmArgs& g) {
+    g.ntypes = ntypes;
+    int tiles = 0;
+    for (int t = 0; t <= kMaxT; ++t) {
+        g.tile0[t] = tiles;
+        g.row0[t] = m.type_row0[t < ntypes ? t : ntypes];
+        if (t < ntypes) tiles += (m.type_row0[t + 1] - m.type_row0[t] + 128 * kNH - 1) / (128 * kNH);
+    }
+    return tiles;
+}
 
 bool tc_setup_maps(Model& m, int ntypes) {
     const int NF = m.NF, ND = m.ND;
     if (NF != 240 || ND % 160 != 0) return false;
+    bool ok = true;
     for (int t = 0; t < ntypes; ++t) {
-        const uint64_t row0 = m.type_row0[t], rows = m.type_row0[t + 1] - m.type_row0[t];
-        if (rows == 0) continue;
-        bool ok = true;
+        const uint64_t row0 = m.type_row0[t];
+        uint64_t rows = m.type_row0[t + 1] - m.type_row0[t];
+        if (rows == 0) rows = 1;                          // keep the descriptor valid; no tile ever uses it
         ok &= tc_make_map(&m.mapA_D[t], m.D + row0 * ND, rows, ND, ND, 128);
         ok &= tc_make_map(&m.mapA_Y1[t], m.Y1 + row0 * NF, rows, NF, NF, 128);
         ok &= tc_make_map(&m.mapA_Y2[t], m.Y2 + row0 * NF, rows, NF, NF, 128);
         ok &= tc_make_map(&m.mapA_G1[t], m.G1 + row0 * NF, rows, NF, NF, 128);
         ok &= tc_make_map(&m.mapA_T3[t], m.T3 + row0 * NF, rows, NF, NF, 128);
-        ok &= tc_make_map(&m.mapB_fwd[t][0], m.fit_wT[t][0], NF, ND, ND, 240);
-        ok &= tc_make_map(&m.mapB_fwd[t][1], m.fit_wT[t][1], NF, NF, NF, 240);
-        ok &= tc_make_map(&m.mapB_fwd[t][2], m.fit_wT[t][2], NF, NF, NF, 240);
-        ok &= tc_make_map(&m.mapB_bwd[t][0], m.fit_w[t][0], ND, NF, NF, 160);
-        ok &= tc_make_map(&m.mapB_bwd[t][1], m.fit_w[t][1], NF, NF, NF, 240);
-        ok &= tc_make_map(&m.mapB_bwd[t][2], m.fit_w[t][2], NF, NF, NF, 240);
-        if (!ok) return false;
+        for (int l = 0; l < 3; ++l) {
+            const uint64_t nin = (l == 0) ? ND : NF;
+            // forward: Bt = W_l^T [out][in];  backward: Bt = W_l [in][out]
+            ok &= tc_make_map(&m.mapB_fwd_hi[t][l], m.fit_wT_hi[t][l], NF, nin, nin, 240);
+            ok &= tc_make_map(&m.mapB_fwd_lo[t][l], m.fit_wT_lo[t][l], NF, nin, nin, 240);
+            ok &= tc_make_map(&m.mapB_bwd_hi[t][l], m.fit_w_hi[t][l], nin, NF, NF, l == 0 ? 160 : 240);
+            ok &= tc_make_map(&m.mapB_bwd_lo[t][l], m.fit_w_lo[t][l], nin, NF, NF, l == 0 ? 160 : 240);
+        }
     }
+    if (!ok) return false;
     m.tc_ready = true;
     return true;
 }
 
-// the six GEMMs of one centre type on the tensor cores; same buffers and epilogues as the CUDA-core path
-int fitting_gemms_tc(Model& m, int t, cudaStream_t s) {
-    const int NF = m.NF, ND = m.ND;
-    const int row0 = m.type_row0[t], rows = m.type_row0[t + 1] - row0;
-    const size_t oF = (size_t)row0 * NF, oD = (size_t)row0 * ND;
-    TcGemmArgs g{};
-    g.M = rows; g.N = NF; g.K = ND; g.bias = m.fit_b[t][0]; g.out0 = m.Y1 + oF; g.ldo = NF;
-    tc_gemm(TEPI_TANH_BIAS, 240, m.mapA_D[t], m.mapB_fwd[t][0], g, s);
-    g = TcGemmArgs{};
-    g.M = rows; g.N = NF; g.K = NF; g.bias = m.fit_b[t][1]; g.add = m.Y1 + oF; g.ldadd = NF;
-    g.out0 = m.T2 + oF; g.out1 = m.Y2 + oF; g.ldo = NF;
-    tc_gemm(TEPI_TANH_BIAS_SKIP, 240, m.mapA_Y1[t], m.mapB_fwd[t][1], g, s);
-    g = TcGemmArgs{};
-    g.M = rows; g.N = NF; g.K = NF; g.bias = m.fit_b[t][2]; g.add = m.Y2 + oF; g.ldadd = NF;
-    g.out0 = m.T3 + oF; g.out1 = m.Y3 + oF; g.ldo = NF;
-    tc_gemm(TEPI_TANH_BIAS_SKIP, 240, m.mapA_Y2[t], m.mapB_fwd[t][2], g, s);
-    return 3;
+static void gather_maps(TcMaps& mp, const CUtensorMap* A, const CUtensorMap (*Bhi)[3], const CUtensorMap (*Blo)[3], int l, int ntypes) {
+    for (int t = 0; t < ntypes; ++t) { mp.A[t] = A[t]; mp.Bhi[t] = Bhi[t][l]; mp.Blo[t] = Blo[t][l]; }
+    for (int t = ntypes; t < kMaxT; ++t) { mp.A[t] = A[0]; mp.Bhi[t] = Bhi[0][l]; mp.Blo[t] = Blo[0][l]; }
 }
-int fitting_gemms_tc_bwd(Model& m, int t, cudaStream_t s) {
-    const int NF = m.NF, ND = m.ND;
-    const int row0 = m.type_row0[t], rows = m.type_row0[t + 1] - row0;
-    const size_t oF = (size_t)row0 * NF, oD = (size_t)row0 * ND;
+
+// the whole fitting chain of all centre types on the tensor cores: 3 forward GEMMs (the third also yields
+// E_i, U and the seed of the backward pass), 3 backward GEMMs.  Returns the number of launches.
+int fitting_chain_tc(Model& m, const ForceArgs& fa, cudaStream_t s) {
+    const int NF = m.NF, ND = m.ND, nt = fa.ntypes;
     TcGemmArgs g{};
-    // dy2 = dy3 + da3 W3^T -> Y3 ; da2 = dy2 o (1 - t2^2) -> T3       (A = G1 = da3)
-    g.M = rows; g.N = NF; g.K = NF; g.add = m.G2 + oF; g.ldadd = NF; g.tt = m.T2 + oF; g.ldtt = NF;
-    g.out0 = m.Y3 + oF; g.out1 = m.T3 + oF; g.ldo = NF;
-    tc_gemm(TEPI_BWD, 240, m.mapA_G1[t], m.mapB_bwd[t][2], g, s);
+    TcMaps mp;
+    const int tiles = fill_types(m, nt, g);
+    auto base = [&]() { TcGemmArgs q{}; fill_types(m, nt, q); return q; };
+    // layer 1: Y1 = tanh(D W1 + b1)
+    g = base(); g.N = NF; g.K = ND; g.out0 = m.Y1; g.ldo = NF;
+    for (int t = 0; t < nt; ++t) g.bias[t] = m.fit_b[t][0];
+    gather_maps(mp, m.mapA_D, m.mapB_fwd_hi, m.mapB_fwd_lo, 0, nt);
+    tc_gemm(TEPI_TANH_BIAS, 240, mp, g, tiles, s);
+    // layer 2: T2 = tanh(Y1 W2 + b2); Y2 = Y1 + T2
+    g = base(); g.N = NF; g.K = NF; g.add = m.Y1; g.ldadd = NF; g.out0 = m.T2; g.out1 = m.Y2; g.ldo = NF;
+    for (int t = 0; t < nt; ++t) g.bias[t] = m.fit_b[t][1];
+    gather_maps(mp, m.mapA_Y1, m.mapB_fwd_hi, m.mapB_fwd_lo, 1, nt);
+    tc_gemm(TEPI_TANH_BIAS_SKIP, 240, mp, g, tiles, s);
+    // layer 3 + energy: t3 = tanh(Y2 W3 + b3); y3 = Y2 + t3; E_i = y3.w4 + b4; da3 = w4 o (1 - t3^2) -> G1
+    g = base(); g.N = NF; g.K = NF; g.add = m.Y2; g.ldadd = NF; g.out1 = m.G1; g.ldo = NF;
+    g.cen_idx = m.cen_idx; g.Eatom = fa.Eatom; g.U = fa.U; g.natoms = fa.N;
+    for (int t = 0; t < nt; ++t) { g.bias[t] = m.fit_b[t][2]; g.vec[t] = m.fit_w[t][3]; g.b4[t] = m.fit_b[t][3]; }
+    gather_maps(mp, m.mapA_Y2, m.mapB_fwd_hi, m.mapB_fwd_lo, 2, nt);
+    tc_gemm(TEPI_L3E, 240, mp, g, tiles, s);
+    // dy2 = dy3 + da3 W3^T -> Y3 ; da2 = dy2 o (1 - t2^2) -> T3       (A = G1 = da3, dy3 = w4)
+    g = base(); g.N = NF; g.K = NF; g.tt = m.T2; g.ldtt = NF; g.out0 = m.Y3; g.out1 = m.T3; g.ldo = NF;
+    for (int t = 0; t < nt; ++t) g.vec[t] = m.fit_w[t][3];
+    gather_maps(mp, m.mapA_G1, m.mapB_bwd_hi, m.mapB_bwd_lo, 2, nt);
+    tc_gemm(TEPI_BWD_VEC, 240, mp, g, tiles, s);
     // dy1 = dy2 + da2 W2^T ; da1 = dy1 o (1 - y1^2) -> G1                (A = T3 = da2)
-    g = TcGemmArgs{};
-    g.M = rows; g.N = NF; g.K = NF; g.add = m.Y3 + oF; g.ldadd = NF; g.tt = m.Y1 + oF; g.ldtt = NF;
-    g.out1 = m.G1 + oF; g.ldo = NF;
-    tc_gemm(TEPI_BWD_FIRST, 240, m.mapA_T3[t], m.mapB_bwd[t][1], g, s);
+    g = base(); g.N = NF; g.K = NF; g.add = m.Y3; g.ldadd = NF; g.tt = m.Y1; g.ldtt = NF; g.out1 = m.G1; g.ldo = NF;
+    gather_maps(mp, m.mapA_T3, m.mapB_bwd_hi, m.mapB_bwd_lo, 1, nt);
+    tc_gemm(TEPI_BWD_FIRST, 240, mp, g, tiles, s);
     // dD = da1 W1^T                                                     (A = G1 = da1)
-    g = TcGemmArgs{};
-    g.M = rows; g.N = ND; g.K = NF; g.out0 = m.dD + oD; g.ldo = ND;
-    tc_gemm(TEPI_PLAIN, 160, m.mapA_G1[t], m.mapB_bwd[t][0], g, s);
-    return 3;
+    g = base(); g.N = ND; g.K = NF; g.out0 = m.dD; g.ldo = ND;
+    gather_maps(mp, m.mapA_G1, m.mapB_bwd_hi, m.mapB_bwd_lo, 0, nt);
+    tc_gemm(TEPI_PLAIN, 160, mp, g, tiles, s);
+    return 6;
 }
 
 // parity hook: C[M][N] = A[M][K] Bt[N][K]^T through the tensor-core kernel (N == 240 or N % 160 == 0, K % 16 == 0)
 int debug_tc_gemm(int M, int N, int K, const float* A, const float* Bt, float* C, cudaStream_t s) {
     const int bn = (N == 240) ? 240 : 160;
     if ((bn == 160 && N % 160 != 0) || K % 16 != 0) return -1;
-    CUtensorMap ma, mb;
-    if (!tc_make_map(&ma, A, M, K, K, 128)) return -2;
-    if (!tc_make_map(&mb, Bt, N, K, K, bn)) return -2;
-    TcGemmArgs g{};
-    g.M = M; g.N = N; g.K = K; g.out0 = C; g.ldo = N;
-    return tc_gemm(TEPI_PLAIN, bn, ma, mb, g, s) == cudaSuccess ? 0 : -3;
+    float *hi = nullptr, *lo = nullptr;
+    if (cudaMalloc(&hi, sizeof(float) * (size_t)N * K) != cudaSuccess) return -4;
+    if (cudaMalloc(&lo, sizeof(float) * (size_t)N * K) != cudaSuccess) { cudaFree(hi); return -4; }
+    tc_split_weights((size_t)N * K, Bt, hi, lo, s);
+    TcMaps mp;
+    CUtensorMap ma, mh, ml;
+    int rc = 0;
+    if (!tc_make_map(&ma, A, M, K, K, 128) || !tc_make_map(&mh, hi, N, K, K, bn) || !tc_make_map(&ml, lo, N, K, K, bn)) rc = -2;
+    if (rc == 0) {
+        for (int t = 0; t < kMaxT; ++t) { mp.A[t] = ma; mp.Bhi[t] = mh; mp.Blo[t] = ml; }
+        TcGemmArgs g{};
+        g.ntypes = 1; g.N = N; g.K = K; g.out0 = C; g.ldo = N;
+        const int tiles = (M + 128 * kNH - 1) / (128 * kNH);
+        for (int t = 0; t <= kMaxT; ++t) { g.tile0[t] = t == 0 ? 0 : tiles; g.row0[t] = t == 0 ? 0 : M; }
+        rc = tc_gemm(TEPI_PLAIN, bn, mp, g, tiles, s) == cudaSuccess ? 0 : -3;
+    }
+    cudaStreamSynchronize(s);
+    cudaFree(hi); cudaFree(lo);
+    return rc;
 }
 
 }  // namespace pimd
