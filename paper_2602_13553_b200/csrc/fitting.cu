@@ -206,8 +206,7 @@ int fitting_forward_backward(Model& m, const ForceArgs& a, cudaStream_t s) {
     int launches = 2;
     descriptor_kernel<100, 16><<<PN, 256, 0, s>>>(PN, m.Tm, m.D);
     if (m.use_tc && m.tc_ready) {
-        launches += fitting_chain_tc(m, a, s);           // all centre types per launch; energy fused into layer 3
-        dT_kernel<100, 16><<<PN, 128, 0, s>>>(PN, m.Tm, m.dD, m.dTm);
+        launches += fitting_chain_tc(m, a, s) - 1;       // all centre types per launch; energy fused into layer 3; dD -> dT fused
         return launches;
     }
     for (int t = 0; t < a.ntypes; ++t) {

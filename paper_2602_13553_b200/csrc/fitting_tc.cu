@@ -253,6 +253,194 @@ gemm3xtf32_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ T
 }
 
 // ---------------------------------------------------------------------------------------------
+// dD = da1 W1^T fused with the descriptor backward (F4 -> F5 hand-over): dD (rows x 1600, 315 MB at
+// configs[2]) never reaches HBM.  One CTA owns 128 rows and walks the 10 column chunks of 160 = 10 m1 x 16 m2;
+// the epilogue thread of row i contracts each accumulator chunk with T_i on the fly (R-14):
+//   dT[i][m][c] = sum_{m2<16} dD[i][m,m2] T[i][m2][c]  +  [m<16] sum_{m1} dD[i][m1,m] T[i][m1][c]
+// first term: complete inside a chunk, stored at once; second term: 16 x 4 register accumulators over all
+// chunks, added to the rows m < 16 at the end (same thread, program order).  T[i][0:16] sits in shared memory.
+// ---------------------------------------------------------------------------------------------
+struct DdDtArgs {
+    int ntypes, K, nchunks;
+    int tile0[kMaxT + 1];
+    int row0[kMaxT + 1];
+    const float* Tm;      // [rows][100][4]
+    float* dTm;           // [rows][100][4]
+    int M1;               // 100
+};
+
+constexpr int kDdBN = 160, kDdST = 2;
+struct DdSmem {
+    static constexpr int kABytes = 128 * 64, kBBytes = kDdBN * 64;
+    static constexpr int oAhi = 0, oAlo = kABytes, oBhi = 2 * kABytes, oBlo = 2 * kABytes + kBBytes;
+    static constexpr int kStage = 2 * kABytes + 2 * kBBytes;               // 36864
+    static constexpr int oT2 = kDdST * kStage;                             // float4 [16][128]
+    static constexpr int oBars = oT2 + 16 * 128 * 16;
+    static constexpr int kTotal = oBars + 256 + 1024;
+};
+
+__global__ void __launch_bounds__(kTcThreads, 2)
+dd_dt_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ DdDtArgs g) {
+    using SM = DdSmem;
+    constexpr int ST = kDdST, BN = kDdBN;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + SM::oBars);
+    uint64_t* full = bars;
+    uint64_t* ready = bars + ST;
+    uint64_t* empty = bars + 2 * ST;
+    uint64_t* tmem_full = bars + 3 * ST;
+    uint64_t* tmem_empty = bars + 3 * ST + 1;
+    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(bars + 3 * ST + 2);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    int ty = 0;
+#pragma unroll
+    for (int t = 1; t < kMaxT; ++t)
+        if (t < g.ntypes && (int)blockIdx.x >= g.tile0[t]) ty = t;
+    const int m0 = ((int)blockIdx.x - g.tile0[ty]) * 128;
+    const int rows_t = g.row0[ty + 1] - g.row0[ty];
+    const int nk = g.K / kTcBK, nch = g.nchunks;
+    const CUtensorMap* mapA = &maps.A[ty];
+    const CUtensorMap* mapBhi = &maps.Bhi[ty];
+    const CUtensorMap* mapBlo = &maps.Blo[ty];
+
+    if (warp == 0 && lane == 0) {
+        tma_prefetch_desc(mapA);
+        tma_prefetch_desc(mapBhi);
+        tma_prefetch_desc(mapBlo);
+        for (int s = 0; s < ST; ++s) { mbar_init(full + s, 1); mbar_init(ready + s, 128); mbar_init(empty + s, 1); }
+        mbar_init(tmem_full, 1);
+        mbar_init(tmem_empty, 128);
+        fence_barrier_init();
+    }
+    if (warp == 1) tmem_alloc(tmem_ptr, 256);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_ptr;
+
+    if (warp == 0) {
+        if (lane == 0) {
+            for (int it = 0; it < nch * nk; ++it) {
+                const int nc = it / nk, kb = it - nc * nk;
+                const int s = it % ST, ph = (it / ST) & 1;
+                mbar_wait(empty + s, ph ^ 1);
+                uint8_t* st = smem + s * SM::kStage;
+                mbar_arrive_expect_tx(full + s, SM::kABytes + 2 * SM::kBBytes);
+                tma_load_2d(st + SM::oAhi, mapA, full + s, kb * kTcBK, m0);
+                tma_load_2d(st + SM::oBhi, mapBhi, full + s, kb * kTcBK, nc * BN);
+                tma_load_2d(st + SM::oBlo, mapBlo, full + s, kb * kTcBK, nc * BN);
+            }
+        }
+    } else if (warp == 1) {
+        if (lane == 0) {
+            constexpr uint32_t idesc = make_idesc_tf32(128, BN);
+            for (int nc = 0; nc < nch; ++nc) {
+                if (nc > 0) {                      // the epilogue has drained the previous chunk's accumulators
+                    mbar_wait(tmem_empty, (nc - 1) & 1);
+                    tc_fence_after();
+                }
+                for (int kb = 0; kb < nk; ++kb) {
+                    const int it = nc * nk + kb;
+                    const int s = it % ST, ph = (it / ST) & 1;
+                    mbar_wait(ready + s, ph);
+                    tc_fence_after();
+                    const uint32_t st = smem_u32(smem + s * SM::kStage);
+#pragma unroll
+                    for (int ks = 0; ks < 2; ++ks) {
+                        const uint64_t a_hi = make_smem_desc_kmajor(st + SM::oAhi + ks * 32, 64);
+                        const uint64_t a_lo = make_smem_desc_kmajor(st + SM::oAlo + ks * 32, 64);
+                        const uint64_t b_hi = make_smem_desc_kmajor(st + SM::oBhi + ks * 32, 64);
+                        const uint64_t b_lo = make_smem_desc_kmajor(st + SM::oBlo + ks * 32, 64);
+                        umma_tf32(tmem_base, a_hi, b_hi, idesc, (kb | ks) ? 1u : 0u);
+                        umma_tf32(tmem_base, a_lo, b_hi, idesc, 1u);
+                        umma_tf32(tmem_base, a_hi, b_lo, idesc, 1u);
+                    }
+                    umma_commit(empty + s);
+                }
+                umma_commit(tmem_full);
+            }
+        }
+    } else {
+        const int t = threadIdx.x - 64;
+        const int quarter = warp & 3;
+        const int ml = m0 + quarter * 32 + lane;               // my row inside the type (TMEM lane)
+        const bool row_ok = ml < rows_t;
+        const size_t m = (size_t)(g.row0[ty] + (row_ok ? ml : 0));
+        const float4* Trow = reinterpret_cast<const float4*>(g.Tm) + m * g.M1;
+        float4* dTrow = reinterpret_cast<float4*>(g.dTm) + m * g.M1;
+        // T[i][0:16] of my row -> shared memory, [m2][thread] (conflict-free 16 B accesses)
+        float4* T2s = reinterpret_cast<float4*>(smem + SM::oT2) + (quarter * 32 + lane);
+#pragma unroll
+        for (int m2 = 0; m2 < 16; ++m2) T2s[m2 * 128] = row_ok ? __ldg(Trow + m2) : make_float4(0.f, 0.f, 0.f, 0.f);
+        float4 accB[16];
+#pragma unroll
+        for (int m2 = 0; m2 < 16; ++m2) accB[m2] = make_float4(0.f, 0.f, 0.f, 0.f);
+
+        for (int nc = 0; nc < nch; ++nc) {
+            for (int kb = 0; kb < nk; ++kb) {
+                const int it = nc * nk + kb;
+                const int s = it % ST, ph = (it / ST) & 1;
+                mbar_wait(full + s, ph);
+                uint8_t* st = smem + s * SM::kStage;
+                float4* a_hi = reinterpret_cast<float4*>(st + SM::oAhi);
+                float4* a_lo = reinterpret_cast<float4*>(st + SM::oAlo);
+#pragma unroll
+                for (int q = 0; q < (SM::kABytes / 16) / 128; ++q) {
+                    const int idx = t + q * 128;
+                    const float4 v = a_hi[idx];
+                    float4 hi, lo;
+                    hi.x = __uint_as_float(__float_as_uint(v.x) & 0xFFFFE000u); lo.x = v.x - hi.x;
+                    hi.y = __uint_as_float(__float_as_uint(v.y) & 0xFFFFE000u); lo.y = v.y - hi.y;
+                    hi.z = __uint_as_float(__float_as_uint(v.z) & 0xFFFFE000u); lo.z = v.z - hi.z;
+                    hi.w = __uint_as_float(__float_as_uint(v.w) & 0xFFFFE000u); lo.w = v.w - hi.w;
+                    a_hi[idx] = hi;
+                    a_lo[idx] = lo;
+                }
+                fence_proxy_async_smem();
+                mbar_arrive(ready + s);
+            }
+            // ---- epilogue of chunk nc: m1 = 10 nc .. 10 nc + 9 ----
+            mbar_wait(tmem_full, nc & 1);
+            tc_fence_after();
+#pragma unroll 2
+            for (int j = 0; j < BN / 16; ++j) {
+                uint32_t v[16];
+                tmem_ld16(tmem_base + ((uint32_t)(quarter * 32) << 16) + j * 16, v);
+                const int m1 = nc * (BN / 16) + j;
+                const float4 T1 = row_ok ? __ldg(Trow + m1) : make_float4(0.f, 0.f, 0.f, 0.f);
+                tmem_ld_wait();
+                float4 accA = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+                for (int m2 = 0; m2 < 16; ++m2) {
+                    const float d = __uint_as_float(v[m2]);
+                    const float4 T2 = T2s[m2 * 128];
+                    accA.x = fmaf(d, T2.x, accA.x); accA.y = fmaf(d, T2.y, accA.y);
+                    accA.z = fmaf(d, T2.z, accA.z); accA.w = fmaf(d, T2.w, accA.w);
+                    accB[m2].x = fmaf(d, T1.x, accB[m2].x); accB[m2].y = fmaf(d, T1.y, accB[m2].y);
+                    accB[m2].z = fmaf(d, T1.z, accB[m2].z); accB[m2].w = fmaf(d, T1.w, accB[m2].w);
+                }
+                if (row_ok) dTrow[m1] = accA;
+            }
+            tc_fence_before();
+            mbar_arrive(tmem_empty);
+        }
+        if (row_ok) {
+#pragma unroll
+            for (int m2 = 0; m2 < 16; ++m2) {
+                float4 o = dTrow[m2];
+                o.x += accB[m2].x; o.y += accB[m2].y; o.z += accB[m2].z; o.w += accB[m2].w;
+                dTrow[m2] = o;
+            }
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) tmem_dealloc(tmem_base, 256);
+}
+
+// ---------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
@@ -407,10 +595,19 @@ int fitting_chain_tc(Model& m, const ForceArgs& fa, cudaStream_t s) {
     g = base(); g.N = NF; g.K = NF; g.add = m.Y3; g.ldadd = NF; g.tt = m.Y1; g.ldtt = NF; g.out1 = m.G1; g.ldo = NF;
     gather_maps(mp, m.mapA_T3, m.mapB_bwd_hi, m.mapB_bwd_lo, 1, nt);
     tc_gemm(TEPI_BWD_FIRST, 240, mp, g, tiles, s);
-    // dD = da1 W1^T                                                     (A = G1 = da1)
-    g = base(); g.N = ND; g.K = NF; g.out0 = m.dD; g.ldo = ND;
-    gather_maps(mp, m.mapA_G1, m.mapB_bwd_hi, m.mapB_bwd_lo, 0, nt);
-    tc_gemm(TEPI_PLAIN, 160, mp, g, tiles, s);
+    // dD = da1 W1^T contracted with T on the fly -> dT                   (A = G1 = da1)
+    {
+        DdDtArgs d{};
+        d.ntypes = nt; d.K = NF; d.nchunks = ND / kDdBN; d.Tm = m.Tm; d.dTm = m.dTm; d.M1 = m.M1;
+        for (int t = 0; t <= kMaxT; ++t) { d.tile0[t] = g.tile0[t]; d.row0[t] = g.row0[t]; }
+        gather_maps(mp, m.mapA_G1, m.mapB_bwd_hi, m.mapB_bwd_lo, 0, nt);
+        static bool attr = false;
+        if (!attr) {
+            cudaFuncSetAttribute(dd_dt_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, DdSmem::kTotal);
+            attr = true;
+        }
+        dd_dt_kernel<<<tiles, kTcThreads, DdSmem::kTotal, s>>>(mp, d);
+    }
     return 6;
 }
 
