@@ -204,11 +204,12 @@ int fitting_forward_backward(Model& m, const ForceArgs& a, cudaStream_t s) {
     const int PN = a.P * a.N;
     const int NF = m.NF, ND = m.ND;
     int launches = 2;
-    descriptor_kernel<100, 16><<<PN, 256, 0, s>>>(PN, m.Tm, m.D);
-    if (m.use_tc && m.tc_ready) {
-        launches += fitting_chain_tc(m, a, s) - 1;       // all centre types per launch; energy fused into layer 3; dD -> dT fused
+    if (m.use_tc && m.tc_ready && m.M1 == 100 && m.M2 == 16) {
+        // one launch per layer for all centre types; descriptor fused into layer 1, energy into layer 3, dD -> dT
+        launches = fitting_chain_tc(m, a, s);
         return launches;
     }
+    descriptor_kernel<100, 16><<<PN, 256, 0, s>>>(PN, m.Tm, m.D);
     for (int t = 0; t < a.ntypes; ++t) {
         const int row0 = m.type_row0[t], rows = m.type_row0[t + 1] - row0;
         if (rows == 0) continue;

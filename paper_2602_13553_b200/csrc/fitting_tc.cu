@@ -253,6 +253,163 @@ gemm3xtf32_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ T
 }
 
 // ---------------------------------------------------------------------------------------------
+// Layer 1 fused with the descriptor (F3 -> F4 hand-over): Y1 = tanh(D W1 + b1) with
+// D[i][16 m1 + m2] = T[i][m1] . T[i][m2] (R-14) produced on the fly -- K block kb of the A operand is exactly
+// m1 = kb, so the producer thread of row i needs T[i][kb] (one float4 per K block) and T[i][0:16] (registers).
+// D (rows x 1600, 315 MB at configs[2]) is neither written nor read.  The weights arrive pre-split by TMA.
+// ---------------------------------------------------------------------------------------------
+struct L1Args {
+    int ntypes, K;
+    int tile0[kMaxT + 1];
+    int row0[kMaxT + 1];
+    const float* bias[kMaxT];
+    const float* Tm;      // [rows][100][4]
+    float* out; int ldo;  // Y1
+    int M1;
+};
+
+constexpr int kL1BN = 240, kL1ST = 2;
+struct L1Smem {
+    static constexpr int kABytes = 128 * 64, kBBytes = kL1BN * 64;
+    static constexpr int oAhi = 0, oAlo = kABytes, oBhi = 2 * kABytes, oBlo = 2 * kABytes + kBBytes;
+    static constexpr int kStage = 2 * kABytes + 2 * kBBytes;               // 47104
+    static constexpr int oBars = kL1ST * kStage;
+    static constexpr int kTotal = oBars + 256 + 1024;
+};
+
+__global__ void __launch_bounds__(kTcThreads, 2)
+l1_desc_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ L1Args g) {
+    using SM = L1Smem;
+    constexpr int ST = kL1ST, BN = kL1BN;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + SM::oBars);
+    uint64_t* full = bars;                     // TMA (weights) -> MMA
+    uint64_t* ready = bars + ST;               // producer threads (A = D block) -> MMA
+    uint64_t* empty = bars + 2 * ST;           // MMA -> TMA and producers
+    uint64_t* tmem_full = bars + 3 * ST;
+    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(bars + 3 * ST + 1);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    int ty = 0;
+#pragma unroll
+    for (int t = 1; t < kMaxT; ++t)
+        if (t < g.ntypes && (int)blockIdx.x >= g.tile0[t]) ty = t;
+    const int m0 = ((int)blockIdx.x - g.tile0[ty]) * 128;
+    const int rows_t = g.row0[ty + 1] - g.row0[ty];
+    const int nk = g.K / kTcBK;
+    const CUtensorMap* mapBhi = &maps.Bhi[ty];
+    const CUtensorMap* mapBlo = &maps.Blo[ty];
+
+    if (warp == 0 && lane == 0) {
+        tma_prefetch_desc(mapBhi);
+        tma_prefetch_desc(mapBlo);
+        for (int s = 0; s < ST; ++s) { mbar_init(full + s, 1); mbar_init(ready + s, 128); mbar_init(empty + s, 1); }
+        mbar_init(tmem_full, 1);
+        fence_barrier_init();
+    }
+    if (warp == 1) tmem_alloc(tmem_ptr, 256);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_ptr;
+
+    if (warp == 0) {
+        if (lane == 0) {
+            for (int kb = 0; kb < nk; ++kb) {
+                const int s = kb % ST, ph = (kb / ST) & 1;
+                mbar_wait(empty + s, ph ^ 1);
+                uint8_t* st = smem + s * SM::kStage;
+                mbar_arrive_expect_tx(full + s, 2 * SM::kBBytes);
+                tma_load_2d(st + SM::oBhi, mapBhi, full + s, kb * kTcBK, 0);
+                tma_load_2d(st + SM::oBlo, mapBlo, full + s, kb * kTcBK, 0);
+            }
+        }
+    } else if (warp == 1) {
+        if (lane == 0) {
+            constexpr uint32_t idesc = make_idesc_tf32(128, BN);
+            for (int kb = 0; kb < nk; ++kb) {
+                const int s = kb % ST, ph = (kb / ST) & 1;
+                mbar_wait(full + s, ph);
+                mbar_wait(ready + s, ph);
+                tc_fence_after();
+                const uint32_t st = smem_u32(smem + s * SM::kStage);
+#pragma unroll
+                for (int ks = 0; ks < 2; ++ks) {
+                    const uint64_t a_hi = make_smem_desc_kmajor(st + SM::oAhi + ks * 32, 64);
+                    const uint64_t a_lo = make_smem_desc_kmajor(st + SM::oAlo + ks * 32, 64);
+                    const uint64_t b_hi = make_smem_desc_kmajor(st + SM::oBhi + ks * 32, 64);
+                    const uint64_t b_lo = make_smem_desc_kmajor(st + SM::oBlo + ks * 32, 64);
+                    umma_tf32(tmem_base, a_hi, b_hi, idesc, (kb | ks) ? 1u : 0u);
+                    umma_tf32(tmem_base, a_lo, b_hi, idesc, 1u);
+                    umma_tf32(tmem_base, a_hi, b_lo, idesc, 1u);
+                }
+                umma_commit(empty + s);
+            }
+            umma_commit(tmem_full);
+        }
+    } else {
+        const int quarter = warp & 3;
+        const int row = quarter * 32 + lane;                   // tile row = TMEM lane
+        const int ml = m0 + row;
+        const bool row_ok = ml < rows_t;
+        const size_t m = (size_t)(g.row0[ty] + (row_ok ? ml : 0));
+        const float4* Trow = reinterpret_cast<const float4*>(g.Tm) + m * g.M1;
+        const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
+        float4 T2[16];
+#pragma unroll
+        for (int m2 = 0; m2 < 16; ++m2) T2[m2] = row_ok ? __ldg(Trow + m2) : zero4;
+        // SWIZZLE_64B K-major block: 64 B rows, 16 B chunk index XOR ((row >> 1) & 3)
+        const int rbase = row * 64, sw = (row >> 1) & 3;
+        float4 T1 = row_ok ? __ldg(Trow) : zero4;
+        for (int kb = 0; kb < nk; ++kb) {
+            const int s = kb % ST, ph = (kb / ST) & 1;
+            const float4 T1n = (row_ok && kb + 1 < nk) ? __ldg(Trow + kb + 1) : zero4;
+            float d[16];
+#pragma unroll
+            for (int m2 = 0; m2 < 16; ++m2) d[m2] = T1.x * T2[m2].x + T1.y * T2[m2].y + T1.z * T2[m2].z + T1.w * T2[m2].w;
+            mbar_wait(empty + s, ph ^ 1);                       // the MMAs that read this stage have retired
+            uint8_t* st = smem + s * SM::kStage;
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                float4 hi, lo;
+                hi.x = __uint_as_float(__float_as_uint(d[4 * c]) & 0xFFFFE000u); lo.x = d[4 * c] - hi.x;
+                hi.y = __uint_as_float(__float_as_uint(d[4 * c + 1]) & 0xFFFFE000u); lo.y = d[4 * c + 1] - hi.y;
+                hi.z = __uint_as_float(__float_as_uint(d[4 * c + 2]) & 0xFFFFE000u); lo.z = d[4 * c + 2] - hi.z;
+                hi.w = __uint_as_float(__float_as_uint(d[4 * c + 3]) & 0xFFFFE000u); lo.w = d[4 * c + 3] - hi.w;
+                const int off = rbase + ((c ^ sw) << 4);
+                *reinterpret_cast<float4*>(st + SM::oAhi + off) = hi;
+                *reinterpret_cast<float4*>(st + SM::oAlo + off) = lo;
+            }
+            fence_proxy_async_smem();
+            mbar_arrive(ready + s);
+            T1 = T1n;
+        }
+        // ---- epilogue: Y1 = tanh(acc + b1) ----
+        mbar_wait(tmem_full, 0);
+        tc_fence_after();
+        float* orow = g.out + m * g.ldo;
+#pragma unroll 1
+        for (int c = 0; c < BN / 16; ++c) {
+            uint32_t v[16];
+            tmem_ld16(tmem_base + ((uint32_t)(quarter * 32) << 16) + c * 16, v);
+            tmem_ld_wait();
+            if (!row_ok) continue;
+            const float* bias = g.bias[ty] + c * 16;
+            float r[16];
+#pragma unroll
+            for (int q = 0; q < 16; ++q) r[q] = tanhf(__uint_as_float(v[q]) + __ldg(bias + q));
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                reinterpret_cast<float4*>(orow + c * 16)[q] = make_float4(r[4 * q], r[4 * q + 1], r[4 * q + 2], r[4 * q + 3]);
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) tmem_dealloc(tmem_base, 256);
+}
+
+// ---------------------------------------------------------------------------------------------
 // dD = da1 W1^T fused with the descriptor backward (F4 -> F5 hand-over): dD (rows x 1600, 315 MB at
 // configs[2]) never reaches HBM.  One CTA owns 128 rows and walks the 10 column chunks of 160 = 10 m1 x 16 m2;
 // the epilogue thread of row i contracts each accumulator chunk with T_i on the fly (R-14):
@@ -570,11 +727,20 @@ int fitting_chain_tc(Model& m, const ForceArgs& fa, cudaStream_t s) {
     TcMaps mp;
     const int tiles = fill_types(m, nt, g);
     auto base = [&]() { TcGemmArgs q{}; fill_types(m, nt, q); return q; };
-    // layer 1: Y1 = tanh(D W1 + b1)
-    g = base(); g.N = NF; g.K = ND; g.out0 = m.Y1; g.ldo = NF;
-    for (int t = 0; t < nt; ++t) g.bias[t] = m.fit_b[t][0];
-    gather_maps(mp, m.mapA_D, m.mapB_fwd_hi, m.mapB_fwd_lo, 0, nt);
-    tc_gemm(TEPI_TANH_BIAS, 240, mp, g, tiles, s);
+    // layer 1: Y1 = tanh(D W1 + b1), D produced on the fly from T
+    {
+        L1Args a1{};
+        a1.ntypes = nt; a1.K = ND; a1.Tm = m.Tm; a1.out = m.Y1; a1.ldo = NF; a1.M1 = m.M1;
+        for (int t = 0; t <= kMaxT; ++t) { a1.tile0[t] = g.tile0[t]; a1.row0[t] = g.row0[t]; }
+        for (int t = 0; t < nt; ++t) a1.bias[t] = m.fit_b[t][0];
+        gather_maps(mp, m.mapA_D, m.mapB_fwd_hi, m.mapB_fwd_lo, 0, nt);
+        static bool attr = false;
+        if (!attr) {
+            cudaFuncSetAttribute(l1_desc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, L1Smem::kTotal);
+            attr = true;
+        }
+        l1_desc_kernel<<<tiles, kTcThreads, L1Smem::kTotal, s>>>(mp, a1);
+    }
     // layer 2: T2 = tanh(Y1 W2 + b2); Y2 = Y1 + T2
     g = base(); g.N = NF; g.K = NF; g.add = m.Y1; g.ldadd = NF; g.out0 = m.T2; g.out1 = m.Y2; g.ldo = NF;
     for (int t = 0; t < nt; ++t) g.bias[t] = m.fit_b[t][1];
