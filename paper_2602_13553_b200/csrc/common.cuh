@@ -102,7 +102,7 @@ struct Model {
     bool     use_tc = true;
     bool     tc_ready = false;
     CUtensorMap mapA_D[PIMD_MAX_TYPES], mapA_Y1[PIMD_MAX_TYPES], mapA_Y2[PIMD_MAX_TYPES], mapA_G1[PIMD_MAX_TYPES],
-                mapA_T3[PIMD_MAX_TYPES];
+                mapA_T3[PIMD_MAX_TYPES], mapA_G2[PIMD_MAX_TYPES];
     CUtensorMap mapB_fwd_hi[PIMD_MAX_TYPES][3], mapB_fwd_lo[PIMD_MAX_TYPES][3];   // W_l^T  [out][in], TF32 hi / lo
     CUtensorMap mapB_bwd_hi[PIMD_MAX_TYPES][3], mapB_bwd_lo[PIMD_MAX_TYPES][3];   // W_l    [in][out]
     float*   fit_w_hi[PIMD_MAX_TYPES][3], *fit_w_lo[PIMD_MAX_TYPES][3];           // pre-split weights (layers 1..3)

@@ -224,7 +224,17 @@ gemm3xtf32_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ T
                         if (EPI == TEPI_BWD_VEC) o0[q] = y;
                         y.x *= (1.f - t4.x * t4.x); y.y *= (1.f - t4.y * t4.y);
                         y.z *= (1.f - t4.z * t4.z); y.w *= (1.f - t4.w * t4.w);
-                        o1[q] = y;
+                        if (EPI == TEPI_BWD_FIRST) {     // da1 feeds dd_dt_kernel only: written pre-split (hi -> out1, lo -> out0)
+                            float4 hi;
+                            hi.x = __uint_as_float(__float_as_uint(y.x) & 0xFFFFE000u);
+                            hi.y = __uint_as_float(__float_as_uint(y.y) & 0xFFFFE000u);
+                            hi.z = __uint_as_float(__float_as_uint(y.z) & 0xFFFFE000u);
+                            hi.w = __uint_as_float(__float_as_uint(y.w) & 0xFFFFE000u);
+                            o1[q] = hi;
+                            o0[q] = make_float4(y.x - hi.x, y.y - hi.y, y.z - hi.z, y.w - hi.w);
+                        } else {
+                            o1[q] = y;
+                        }
                     }
                 }
             }
@@ -268,7 +278,7 @@ struct L1Args {
     int M1;
 };
 
-constexpr int kL1BN = 240, kL1ST = 2;
+constexpr int kL1BN = 240, kL1ST = 4;
 struct L1Smem {
     static constexpr int kABytes = 128 * 64, kBBytes = kL1BN * 64;
     static constexpr int oAhi = 0, oAlo = kABytes, oBhi = 2 * kABytes, oBlo = 2 * kABytes + kBBytes;
@@ -277,7 +287,7 @@ struct L1Smem {
     static constexpr int kTotal = oBars + 256 + 1024;
 };
 
-__global__ void __launch_bounds__(kTcThreads, 2)
+__global__ void __launch_bounds__(kTcThreads, 1)
 l1_desc_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ L1Args g) {
     using SM = L1Smem;
     constexpr int ST = kL1ST, BN = kL1BN;
@@ -426,7 +436,14 @@ struct DdDtArgs {
     int M1;               // 100
 };
 
-constexpr int kDdBN = 160, kDdST = 2;
+// A (= da1) arrives pre-split as well (the producing epilogue writes hi and lo), so nothing stands between TMA
+// and MMA: warps 0 / 1 run ahead through the chunks, alternating between two TMEM accumulator buffers, while
+// the four epilogue warps contract the previous chunk.
+struct DdMaps {
+    CUtensorMap Ahi[kMaxT], Alo[kMaxT], Bhi[kMaxT], Blo[kMaxT];
+};
+
+constexpr int kDdBN = 160, kDdST = 5;
 struct DdSmem {
     static constexpr int kABytes = 128 * 64, kBBytes = kDdBN * 64;
     static constexpr int oAhi = 0, oAlo = kABytes, oBhi = 2 * kABytes, oBlo = 2 * kABytes + kBBytes;
@@ -436,19 +453,18 @@ struct DdSmem {
     static constexpr int kTotal = oBars + 256 + 1024;
 };
 
-__global__ void __launch_bounds__(kTcThreads, 2)
-dd_dt_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ DdDtArgs g) {
+__global__ void __launch_bounds__(kTcThreads, 1)
+dd_dt_kernel(const __grid_constant__ DdMaps maps, const __grid_constant__ DdDtArgs g) {
     using SM = DdSmem;
     constexpr int ST = kDdST, BN = kDdBN;
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + SM::oBars);
-    uint64_t* full = bars;
-    uint64_t* ready = bars + ST;
-    uint64_t* empty = bars + 2 * ST;
-    uint64_t* tmem_full = bars + 3 * ST;
-    uint64_t* tmem_empty = bars + 3 * ST + 1;
-    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(bars + 3 * ST + 2);
+    uint64_t* full = bars;                     // [ST] TMA -> MMA
+    uint64_t* empty = bars + ST;               // [ST] MMA -> TMA
+    uint64_t* tmem_full = bars + 2 * ST;       // [2]  MMA -> epilogue
+    uint64_t* tmem_empty = bars + 2 * ST + 2;  // [2]  epilogue -> MMA
+    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(bars + 2 * ST + 4);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     int ty = 0;
@@ -458,20 +474,17 @@ dd_dt_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ DdDtAr
     const int m0 = ((int)blockIdx.x - g.tile0[ty]) * 128;
     const int rows_t = g.row0[ty + 1] - g.row0[ty];
     const int nk = g.K / kTcBK, nch = g.nchunks;
-    const CUtensorMap* mapA = &maps.A[ty];
-    const CUtensorMap* mapBhi = &maps.Bhi[ty];
-    const CUtensorMap* mapBlo = &maps.Blo[ty];
 
     if (warp == 0 && lane == 0) {
-        tma_prefetch_desc(mapA);
-        tma_prefetch_desc(mapBhi);
-        tma_prefetch_desc(mapBlo);
-        for (int s = 0; s < ST; ++s) { mbar_init(full + s, 1); mbar_init(ready + s, 128); mbar_init(empty + s, 1); }
-        mbar_init(tmem_full, 1);
-        mbar_init(tmem_empty, 128);
+        tma_prefetch_desc(&maps.Ahi[ty]);
+        tma_prefetch_desc(&maps.Alo[ty]);
+        tma_prefetch_desc(&maps.Bhi[ty]);
+        tma_prefetch_desc(&maps.Blo[ty]);
+        for (int s = 0; s < ST; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, 1); }
+        for (int b = 0; b < 2; ++b) { mbar_init(tmem_full + b, 1); mbar_init(tmem_empty + b, 128); }
         fence_barrier_init();
     }
-    if (warp == 1) tmem_alloc(tmem_ptr, 256);
+    if (warp == 1) tmem_alloc(tmem_ptr, 512);
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
@@ -484,24 +497,27 @@ dd_dt_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ DdDtAr
                 const int s = it % ST, ph = (it / ST) & 1;
                 mbar_wait(empty + s, ph ^ 1);
                 uint8_t* st = smem + s * SM::kStage;
-                mbar_arrive_expect_tx(full + s, SM::kABytes + 2 * SM::kBBytes);
-                tma_load_2d(st + SM::oAhi, mapA, full + s, kb * kTcBK, m0);
-                tma_load_2d(st + SM::oBhi, mapBhi, full + s, kb * kTcBK, nc * BN);
-                tma_load_2d(st + SM::oBlo, mapBlo, full + s, kb * kTcBK, nc * BN);
+                mbar_arrive_expect_tx(full + s, 2 * SM::kABytes + 2 * SM::kBBytes);
+                tma_load_2d(st + SM::oAhi, &maps.Ahi[ty], full + s, kb * kTcBK, m0);
+                tma_load_2d(st + SM::oAlo, &maps.Alo[ty], full + s, kb * kTcBK, m0);
+                tma_load_2d(st + SM::oBhi, &maps.Bhi[ty], full + s, kb * kTcBK, nc * BN);
+                tma_load_2d(st + SM::oBlo, &maps.Blo[ty], full + s, kb * kTcBK, nc * BN);
             }
         }
     } else if (warp == 1) {
         if (lane == 0) {
             constexpr uint32_t idesc = make_idesc_tf32(128, BN);
             for (int nc = 0; nc < nch; ++nc) {
-                if (nc > 0) {                      // the epilogue has drained the previous chunk's accumulators
-                    mbar_wait(tmem_empty, (nc - 1) & 1);
+                const int buf = nc & 1;
+                if (nc >= 2) {                     // the epilogue has drained this buffer (chunk nc - 2)
+                    mbar_wait(tmem_empty + buf, ((nc >> 1) - 1) & 1);
                     tc_fence_after();
                 }
+                const uint32_t dcol = tmem_base + buf * 256;
                 for (int kb = 0; kb < nk; ++kb) {
                     const int it = nc * nk + kb;
                     const int s = it % ST, ph = (it / ST) & 1;
-                    mbar_wait(ready + s, ph);
+                    mbar_wait(full + s, ph);
                     tc_fence_after();
                     const uint32_t st = smem_u32(smem + s * SM::kStage);
 #pragma unroll
@@ -510,78 +526,64 @@ dd_dt_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ DdDtAr
                         const uint64_t a_lo = make_smem_desc_kmajor(st + SM::oAlo + ks * 32, 64);
                         const uint64_t b_hi = make_smem_desc_kmajor(st + SM::oBhi + ks * 32, 64);
                         const uint64_t b_lo = make_smem_desc_kmajor(st + SM::oBlo + ks * 32, 64);
-                        umma_tf32(tmem_base, a_hi, b_hi, idesc, (kb | ks) ? 1u : 0u);
-                        umma_tf32(tmem_base, a_lo, b_hi, idesc, 1u);
-                        umma_tf32(tmem_base, a_hi, b_lo, idesc, 1u);
+                        umma_tf32(dcol, a_hi, b_hi, idesc, (kb | ks) ? 1u : 0u);
+                        umma_tf32(dcol, a_lo, b_hi, idesc, 1u);
+                        umma_tf32(dcol, a_hi, b_lo, idesc, 1u);
                     }
                     umma_commit(empty + s);
                 }
-                umma_commit(tmem_full);
+                umma_commit(tmem_full + buf);
             }
         }
     } else {
-        const int t = threadIdx.x - 64;
         const int quarter = warp & 3;
         const int ml = m0 + quarter * 32 + lane;               // my row inside the type (TMEM lane)
         const bool row_ok = ml < rows_t;
         const size_t m = (size_t)(g.row0[ty] + (row_ok ? ml : 0));
         const float4* Trow = reinterpret_cast<const float4*>(g.Tm) + m * g.M1;
         float4* dTrow = reinterpret_cast<float4*>(g.dTm) + m * g.M1;
+        const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
         // T[i][0:16] of my row -> shared memory, [m2][thread] (conflict-free 16 B accesses)
         float4* T2s = reinterpret_cast<float4*>(smem + SM::oT2) + (quarter * 32 + lane);
 #pragma unroll
-        for (int m2 = 0; m2 < 16; ++m2) T2s[m2 * 128] = row_ok ? __ldg(Trow + m2) : make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int m2 = 0; m2 < 16; ++m2) T2s[m2 * 128] = row_ok ? __ldg(Trow + m2) : zero4;
         float4 accB[16];
 #pragma unroll
-        for (int m2 = 0; m2 < 16; ++m2) accB[m2] = make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int m2 = 0; m2 < 16; ++m2) accB[m2] = zero4;
+        float4 T1[BN / 16];                                     // T[i][m1] of the chunk, fetched one chunk ahead
+#pragma unroll
+        for (int j = 0; j < BN / 16; ++j) T1[j] = row_ok ? __ldg(Trow + j) : zero4;
 
         for (int nc = 0; nc < nch; ++nc) {
-            for (int kb = 0; kb < nk; ++kb) {
-                const int it = nc * nk + kb;
-                const int s = it % ST, ph = (it / ST) & 1;
-                mbar_wait(full + s, ph);
-                uint8_t* st = smem + s * SM::kStage;
-                float4* a_hi = reinterpret_cast<float4*>(st + SM::oAhi);
-                float4* a_lo = reinterpret_cast<float4*>(st + SM::oAlo);
+            const int buf = nc & 1;
+            float4 T1n[BN / 16];
 #pragma unroll
-                for (int q = 0; q < (SM::kABytes / 16) / 128; ++q) {
-                    const int idx = t + q * 128;
-                    const float4 v = a_hi[idx];
-                    float4 hi, lo;
-                    hi.x = __uint_as_float(__float_as_uint(v.x) & 0xFFFFE000u); lo.x = v.x - hi.x;
-                    hi.y = __uint_as_float(__float_as_uint(v.y) & 0xFFFFE000u); lo.y = v.y - hi.y;
-                    hi.z = __uint_as_float(__float_as_uint(v.z) & 0xFFFFE000u); lo.z = v.z - hi.z;
-                    hi.w = __uint_as_float(__float_as_uint(v.w) & 0xFFFFE000u); lo.w = v.w - hi.w;
-                    a_hi[idx] = hi;
-                    a_lo[idx] = lo;
-                }
-                fence_proxy_async_smem();
-                mbar_arrive(ready + s);
-            }
-            // ---- epilogue of chunk nc: m1 = 10 nc .. 10 nc + 9 ----
-            mbar_wait(tmem_full, nc & 1);
+            for (int j = 0; j < BN / 16; ++j)
+                T1n[j] = (row_ok && nc + 1 < nch) ? __ldg(Trow + (nc + 1) * (BN / 16) + j) : zero4;
+            mbar_wait(tmem_full + buf, (nc >> 1) & 1);
             tc_fence_after();
-#pragma unroll 2
+            const uint32_t dcol = tmem_base + ((uint32_t)(quarter * 32) << 16) + buf * 256;
+#pragma unroll
             for (int j = 0; j < BN / 16; ++j) {
                 uint32_t v[16];
-                tmem_ld16(tmem_base + ((uint32_t)(quarter * 32) << 16) + j * 16, v);
-                const int m1 = nc * (BN / 16) + j;
-                const float4 T1 = row_ok ? __ldg(Trow + m1) : make_float4(0.f, 0.f, 0.f, 0.f);
+                tmem_ld16(dcol + j * 16, v);
                 tmem_ld_wait();
-                float4 accA = make_float4(0.f, 0.f, 0.f, 0.f);
+                float4 accA = zero4;
 #pragma unroll
                 for (int m2 = 0; m2 < 16; ++m2) {
                     const float d = __uint_as_float(v[m2]);
                     const float4 T2 = T2s[m2 * 128];
                     accA.x = fmaf(d, T2.x, accA.x); accA.y = fmaf(d, T2.y, accA.y);
                     accA.z = fmaf(d, T2.z, accA.z); accA.w = fmaf(d, T2.w, accA.w);
-                    accB[m2].x = fmaf(d, T1.x, accB[m2].x); accB[m2].y = fmaf(d, T1.y, accB[m2].y);
-                    accB[m2].z = fmaf(d, T1.z, accB[m2].z); accB[m2].w = fmaf(d, T1.w, accB[m2].w);
+                    accB[m2].x = fmaf(d, T1[j].x, accB[m2].x); accB[m2].y = fmaf(d, T1[j].y, accB[m2].y);
+                    accB[m2].z = fmaf(d, T1[j].z, accB[m2].z); accB[m2].w = fmaf(d, T1[j].w, accB[m2].w);
                 }
-                if (row_ok) dTrow[m1] = accA;
+                if (row_ok) dTrow[nc * (BN / 16) + j] = accA;
             }
             tc_fence_before();
-            mbar_arrive(tmem_empty);
+            mbar_arrive(tmem_empty + buf);
+#pragma unroll
+            for (int j = 0; j < BN / 16; ++j) T1[j] = T1n[j];
         }
         if (row_ok) {
 #pragma unroll
@@ -594,7 +596,7 @@ dd_dt_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ DdDtAr
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == 1) tmem_dealloc(tmem_base, 256);
+    if (warp == 1) tmem_dealloc(tmem_base, 512);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -642,7 +644,7 @@ void tc_split_weights(size_t n, const float* w, float* hi, float* lo, cudaStream
     split_hi_lo_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(n, w, hi, lo);
 }
 
-constexpr int kNH = 1, kST = 2, kOCC = 2;     // 128-row tiles, 2 stages, 2 CTAs per SM (one's epilogue under the other's MMAs)
+constexpr int kNH = 1, kST = 4, kOCC = 1;     // 128-row tiles, 2 stages, 2 CTAs per SM (one's epilogue under the other's MMAs)
 
 template <int BN, int EPI>
 static cudaError_t launch_tc(const TcMaps& maps, const TcGemmArgs& g, int mtiles, cudaStream_t s) {
@@ -699,6 +701,7 @@ bool tc_setup_maps(Model& m, int ntypes) {
         ok &= tc_make_map(&m.mapA_Y1[t], m.Y1 + row0 * NF, rows, NF, NF, 128);
         ok &= tc_make_map(&m.mapA_Y2[t], m.Y2 + row0 * NF, rows, NF, NF, 128);
         ok &= tc_make_map(&m.mapA_G1[t], m.G1 + row0 * NF, rows, NF, NF, 128);
+        ok &= tc_make_map(&m.mapA_G2[t], m.G2 + row0 * NF, rows, NF, NF, 128);
         ok &= tc_make_map(&m.mapA_T3[t], m.T3 + row0 * NF, rows, NF, NF, 128);
         for (int l = 0; l < 3; ++l) {
             const uint64_t nin = (l == 0) ? ND : NF;
@@ -758,7 +761,7 @@ int fitting_chain_tc(Model& m, const ForceArgs& fa, cudaStream_t s) {
     gather_maps(mp, m.mapA_G1, m.mapB_bwd_hi, m.mapB_bwd_lo, 2, nt);
     tc_gemm(TEPI_BWD_VEC, 240, mp, g, tiles, s);
     // dy1 = dy2 + da2 W2^T ; da1 = dy1 o (1 - y1^2) -> G1                (A = T3 = da2)
-    g = base(); g.N = NF; g.K = NF; g.add = m.Y3; g.ldadd = NF; g.tt = m.Y1; g.ldtt = NF; g.out1 = m.G1; g.ldo = NF;
+    g = base(); g.N = NF; g.K = NF; g.add = m.Y3; g.ldadd = NF; g.tt = m.Y1; g.ldtt = NF; g.out1 = m.G1; g.out0 = m.G2; g.ldo = NF;
     gather_maps(mp, m.mapA_T3, m.mapB_bwd_hi, m.mapB_bwd_lo, 1, nt);
     tc_gemm(TEPI_BWD_FIRST, 240, mp, g, tiles, s);
     // dD = da1 W1^T contracted with T on the fly -> dT                   (A = G1 = da1)
@@ -766,13 +769,18 @@ int fitting_chain_tc(Model& m, const ForceArgs& fa, cudaStream_t s) {
         DdDtArgs d{};
         d.ntypes = nt; d.K = NF; d.nchunks = ND / kDdBN; d.Tm = m.Tm; d.dTm = m.dTm; d.M1 = m.M1;
         for (int t = 0; t <= kMaxT; ++t) { d.tile0[t] = g.tile0[t]; d.row0[t] = g.row0[t]; }
-        gather_maps(mp, m.mapA_G1, m.mapB_bwd_hi, m.mapB_bwd_lo, 0, nt);
+        DdMaps dm;
+        for (int t = 0; t < kMaxT; ++t) {
+            const int q = t < nt ? t : 0;
+            dm.Ahi[t] = m.mapA_G1[q]; dm.Alo[t] = m.mapA_G2[q];
+            dm.Bhi[t] = m.mapB_bwd_hi[q][0]; dm.Blo[t] = m.mapB_bwd_lo[q][0];
+        }
         static bool attr = false;
         if (!attr) {
             cudaFuncSetAttribute(dd_dt_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, DdSmem::kTotal);
             attr = true;
         }
-        dd_dt_kernel<<<tiles, kTcThreads, DdSmem::kTotal, s>>>(mp, d);
+        dd_dt_kernel<<<tiles, kTcThreads, DdSmem::kTotal, s>>>(dm, d);
     }
     return 6;
 }
