@@ -183,14 +183,6 @@ row_scan_fill_kernel(int PN, int ntypes, int nsel, SelOff so, const int* __restr
     }
 }
 
-// fast tanh = 1 - 2 / (1 + e^{2x}); two MUFU ops (ex2, rcp), absolute error ~1e-7
-__device__ __forceinline__ float tanh_fast(float x) {
-    float e, r;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(x * 2.8853900817779268f));
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(e + 1.0f));
-    return fmaf(-2.0f, r, 1.0f);
-}
-
 __device__ __forceinline__ float tf32_hi(float v) { return __uint_as_float(__float_as_uint(v) & 0xFFFFE000u); }
 
 // store 4 consecutive K elements (one 16-byte chunk) of row `row` into the hi and lo copies of a

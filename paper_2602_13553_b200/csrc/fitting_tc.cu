@@ -161,30 +161,55 @@ gemm3xtf32_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ T
             fence_proxy_async_smem();
             mbar_arrive(ready + s);
         }
-        // ---- epilogue: one thread per row ----
+        // ---- epilogue: one thread per row; the row's `add` / `tt` operands are fetched one chunk ahead ----
         mbar_wait(tmem_full, 0);
         tc_fence_after();
         const int quarter = warp & 3;                      // TMEM lane quarter this warp may access
+        constexpr bool kAdd = (EPI == TEPI_TANH_BIAS_SKIP || EPI == TEPI_L3E || EPI == TEPI_BWD_FIRST);
+        constexpr bool kTt = (EPI == TEPI_BWD_VEC || EPI == TEPI_BWD_FIRST);
+        constexpr bool kTanh = (EPI == TEPI_TANH_BIAS || EPI == TEPI_TANH_BIAS_SKIP || EPI == TEPI_L3E);
 #pragma unroll 1
         for (int h = 0; h < NH; ++h) {
             const int ml = m0 + h * 128 + quarter * 32 + lane;     // row inside the type
             const bool row_ok = ml < rows_t;
-            const size_t m = (size_t)(g.row0[ty] + ml);            // type-sorted global row
+            const size_t m = (size_t)(g.row0[ty] + (row_ok ? ml : 0));   // type-sorted global row
             float e_acc = 0.f;
+            const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
+            const float4* adp = kAdd ? reinterpret_cast<const float4*>(g.add + m * g.ldadd + n0) : nullptr;
+            const float4* ttp = kTt ? reinterpret_cast<const float4*>(g.tt + m * g.ldtt + n0) : nullptr;
+            float4 adn[4], ttn[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                adn[q] = (kAdd && row_ok) ? adp[q] : zero4;
+                ttn[q] = (kTt && row_ok) ? ttp[q] : zero4;
+            }
 #pragma unroll 1
             for (int c = 0; c < BN / 16; ++c) {
                 uint32_t v[16];
                 tmem_ld16(tmem_base + ((uint32_t)(quarter * 32) << 16) + h * 256 + c * 16, v);
-                tmem_ld_wait();
+                float4 ad[4], t4[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) { ad[q] = adn[q]; t4[q] = ttn[q]; }
                 const int n = n0 + c * 16;
+                const bool more = row_ok && (c + 1 < BN / 16) && (n + 16 < g.N);
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    if (kAdd) adn[q] = more ? adp[4 * (c + 1) + q] : zero4;
+                    if (kTt) ttn[q] = more ? ttp[4 * (c + 1) + q] : zero4;
+                }
+                tmem_ld_wait();
                 if (!row_ok || n >= g.N) continue;
                 float r[16];
 #pragma unroll
                 for (int q = 0; q < 16; ++q) r[q] = __uint_as_float(v[q]);
-                if (EPI == TEPI_TANH_BIAS || EPI == TEPI_TANH_BIAS_SKIP || EPI == TEPI_L3E) {
-                    const float* bias = g.bias[ty] + n;
+                if (kTanh) {
+                    const float4* bias = reinterpret_cast<const float4*>(g.bias[ty] + n);
 #pragma unroll
-                    for (int q = 0; q < 16; ++q) r[q] = tanhf(r[q] + __ldg(bias + q));
+                    for (int q = 0; q < 4; ++q) {
+                        const float4 b4 = __ldg(bias + q);
+                        r[4 * q] = tanh_fast(r[4 * q] + b4.x); r[4 * q + 1] = tanh_fast(r[4 * q + 1] + b4.y);
+                        r[4 * q + 2] = tanh_fast(r[4 * q + 2] + b4.z); r[4 * q + 3] = tanh_fast(r[4 * q + 3] + b4.w);
+                    }
                 }
                 float4* o0 = (g.out0 != nullptr) ? reinterpret_cast<float4*>(g.out0 + m * g.ldo + n) : nullptr;
                 float4* o1 = (g.out1 != nullptr) ? reinterpret_cast<float4*>(g.out1 + m * g.ldo + n) : nullptr;
@@ -192,7 +217,6 @@ gemm3xtf32_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ T
 #pragma unroll
                     for (int q = 0; q < 4; ++q) o0[q] = make_float4(r[4 * q], r[4 * q + 1], r[4 * q + 2], r[4 * q + 3]);
                 } else if (EPI == TEPI_TANH_BIAS_SKIP) {
-                    const float4* ad = reinterpret_cast<const float4*>(g.add + m * g.ldadd + n);
 #pragma unroll
                     for (int q = 0; q < 4; ++q) {
                         o0[q] = make_float4(r[4 * q], r[4 * q + 1], r[4 * q + 2], r[4 * q + 3]);
@@ -201,7 +225,6 @@ gemm3xtf32_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ T
                     }
                 } else if (EPI == TEPI_L3E) {
                     // y3 = y2 + t3 ; E_i += y3 . w4 ; seed of the backward pass da3 = w4 o (1 - t3^2) -> out1
-                    const float4* ad = reinterpret_cast<const float4*>(g.add + m * g.ldadd + n);
                     const float4* w4 = reinterpret_cast<const float4*>(g.vec[ty] + n);
 #pragma unroll
                     for (int q = 0; q < 4; ++q) {
@@ -214,16 +237,14 @@ gemm3xtf32_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ T
                                             w.z * (1.f - r[4 * q + 2] * r[4 * q + 2]), w.w * (1.f - r[4 * q + 3] * r[4 * q + 3]));
                     }
                 } else {   // TEPI_BWD_VEC, TEPI_BWD_FIRST
-                    const float4* tt = reinterpret_cast<const float4*>(g.tt + m * g.ldtt + n);
 #pragma unroll
                     for (int q = 0; q < 4; ++q) {
-                        const float4 a4 = (EPI == TEPI_BWD_VEC) ? __ldg(reinterpret_cast<const float4*>(g.vec[ty] + n) + q)
-                                                                : reinterpret_cast<const float4*>(g.add + m * g.ldadd + n)[q];
-                        const float4 t4 = tt[q];
+                        const float4 a4 = (EPI == TEPI_BWD_VEC) ? __ldg(reinterpret_cast<const float4*>(g.vec[ty] + n) + q) : ad[q];
+                        const float4 tq = t4[q];
                         float4 y = make_float4(r[4 * q] + a4.x, r[4 * q + 1] + a4.y, r[4 * q + 2] + a4.z, r[4 * q + 3] + a4.w);
                         if (EPI == TEPI_BWD_VEC) o0[q] = y;
-                        y.x *= (1.f - t4.x * t4.x); y.y *= (1.f - t4.y * t4.y);
-                        y.z *= (1.f - t4.z * t4.z); y.w *= (1.f - t4.w * t4.w);
+                        y.x *= (1.f - tq.x * tq.x); y.y *= (1.f - tq.y * tq.y);
+                        y.z *= (1.f - tq.z * tq.z); y.w *= (1.f - tq.w * tq.w);
                         if (EPI == TEPI_BWD_FIRST) {     // da1 feeds dd_dt_kernel only: written pre-split (hi -> out1, lo -> out0)
                             float4 hi;
                             hi.x = __uint_as_float(__float_as_uint(y.x) & 0xFFFFE000u);
@@ -408,7 +429,7 @@ l1_desc_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ L1Ar
             const float* bias = g.bias[ty] + c * 16;
             float r[16];
 #pragma unroll
-            for (int q = 0; q < 16; ++q) r[q] = tanhf(__uint_as_float(v[q]) + __ldg(bias + q));
+            for (int q = 0; q < 16; ++q) r[q] = tanh_fast(__uint_as_float(v[q]) + __ldg(bias + q));
 #pragma unroll
             for (int q = 0; q < 4; ++q)
                 reinterpret_cast<float4*>(orow + c * 16)[q] = make_float4(r[4 * q], r[4 * q + 1], r[4 * q + 2], r[4 * q + 3]);

@@ -143,4 +143,13 @@ __device__ __forceinline__ void umma_commit(uint64_t* bar) {
 }
 
 }  // namespace tc
+
+// fast tanh = 1 - 2 / (1 + e^{2x}); two MUFU ops (ex2, rcp), absolute error ~1e-7
+__device__ __forceinline__ float tanh_fast(float x) {
+    float e, r;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(x * 2.8853900817779268f));
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(e + 1.0f));
+    return fmaf(-2.0f, r, 1.0f);
+}
+
 }  // namespace pimd
