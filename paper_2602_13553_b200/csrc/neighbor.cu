@@ -130,73 +130,95 @@ neighbor_env_kernel(int P, int N, GridGeom g, EnvConsts ec, const double* __rest
     const unsigned lt_mask = (1u << lane) - 1u;
     const size_t slot0 = (size_t)ba * ec.nsel;
 
-    for (int oz = -g.R[2]; oz <= g.R[2]; ++oz) {
-        const int zz = c2 + oz;
-        const int nz = (zz >= 0) ? zz / g.nc[2] : -((-zz + g.nc[2] - 1) / g.nc[2]);
-        const int cz = zz - nz * g.nc[2];
-        for (int oy = -g.R[1]; oy <= g.R[1]; ++oy) {
-            const int yy = c1 + oy;
-            const int ny = (yy >= 0) ? yy / g.nc[1] : -((-yy + g.nc[1] - 1) / g.nc[1]);
-            const int cy = yy - ny * g.nc[1];
-            for (int ox = -g.R[0]; ox <= g.R[0]; ++ox) {
-                const int xx = c0 + ox;
+    // The (2R+1)^3 neighbour cells are walked in the order (oz, oy, ox), ox fastest.  Lane l of a batch looks up
+    // cell l's range and periodic image first (27 independent loads instead of 27 dependent ones); the cells are
+    // then processed one by one with the first 32 candidates of the NEXT cell already in flight.
+    const int nx_c = 2 * g.R[0] + 1, ny_c = 2 * g.R[1] + 1, nz_c = 2 * g.R[2] + 1;
+    const int ncl = nx_c * ny_c * nz_c;
+    for (int base = 0; base < ncl; base += 32) {
+        int my_s0 = 0, my_s1 = 0, my_code = 0;
+        {
+            const int idx = base + lane;
+            if (idx < ncl) {
+                const int ox = idx % nx_c - g.R[0], oy = (idx / nx_c) % ny_c - g.R[1], oz = idx / (nx_c * ny_c) - g.R[2];
+                const int xx = c0 + ox, yy = c1 + oy, zz = c2 + oz;
                 const int nx = (xx >= 0) ? xx / g.nc[0] : -((-xx + g.nc[0] - 1) / g.nc[0]);
-                const int cx = xx - nx * g.nc[0];
-                const int cc = (cz * g.nc[1] + cy) * g.nc[0] + cx;
-                const int s0 = cs[cc], s1 = cs[cc + 1];
-                const double sh[3] = {__dmul_rn((double)nx, g.L[0]), __dmul_rn((double)ny, g.L[1]),
-                                      __dmul_rn((double)nz, g.L[2])};
-                const bool zero_shift = (nx == 0) && (ny == 0) && (nz == 0);
-                for (int q0 = s0; q0 < s1; q0 += 32) {
-                    const int q = q0 + lane;
-                    bool keep = false;
-                    int tj = 0, j = 0;
-                    double d[3] = {0, 0, 0}, r2 = 1.0;
-                    if (q < s1) {
-                        const double4 wj = ws[q];
-                        const long long pk = __double_as_longlong(wj.w);
-                        j = (int)(pk & 0xffffffffll);
-                        tj = (int)(pk >> 32);
-                        d[0] = __dadd_rn(__dsub_rn(wj.x, wi[0]), sh[0]);
-                        d[1] = __dadd_rn(__dsub_rn(wj.y, wi[1]), sh[1]);
-                        d[2] = __dadd_rn(__dsub_rn(wj.z, wi[2]), sh[2]);
-                        r2 = __dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2]));
-                        keep = (r2 < ec.rc2) && !(zero_shift && j == i);
+                const int ny = (yy >= 0) ? yy / g.nc[1] : -((-yy + g.nc[1] - 1) / g.nc[1]);
+                const int nz = (zz >= 0) ? zz / g.nc[2] : -((-zz + g.nc[2] - 1) / g.nc[2]);
+                const int cc = ((zz - nz * g.nc[2]) * g.nc[1] + (yy - ny * g.nc[1])) * g.nc[0] + (xx - nx * g.nc[0]);
+                my_s0 = cs[cc]; my_s1 = cs[cc + 1];
+                my_code = (nx + 3) | ((ny + 3) << 3) | ((nz + 3) << 6);
+            }
+        }
+        const int nb = min(32, ncl - base);
+        double4 wnext = make_double4(0, 0, 0, 0);
+        {
+            const int f0 = __shfl_sync(0xffffffffu, my_s0, 0), f1 = __shfl_sync(0xffffffffu, my_s1, 0);
+            if (f0 + lane < f1) wnext = ws[f0 + lane];
+        }
+        for (int c = 0; c < nb; ++c) {
+            const int s0 = __shfl_sync(0xffffffffu, my_s0, c), s1 = __shfl_sync(0xffffffffu, my_s1, c);
+            const int code = __shfl_sync(0xffffffffu, my_code, c);
+            const int nx = (code & 7) - 3, ny = ((code >> 3) & 7) - 3, nz = ((code >> 6) & 7) - 3;
+            const double4 wfirst = wnext;
+            if (c + 1 < nb) {
+                const int f0 = __shfl_sync(0xffffffffu, my_s0, c + 1), f1 = __shfl_sync(0xffffffffu, my_s1, c + 1);
+                if (f0 + lane < f1) wnext = ws[f0 + lane];
+            }
+            const double sh[3] = {__dmul_rn((double)nx, g.L[0]), __dmul_rn((double)ny, g.L[1]),
+                                  __dmul_rn((double)nz, g.L[2])};
+            const bool zero_shift = (nx == 0) && (ny == 0) && (nz == 0);
+            for (int q0 = s0; q0 < s1; q0 += 32) {
+                const int q = q0 + lane;
+                double4 wj = wfirst;
+                if (q0 != s0 && q < s1) wj = ws[q];
+            bool keep = false;
+            int tj = 0, j = 0;
+            double d[3] = {0, 0, 0}, r2 = 1.0;
+            if (q < s1) {
+                const long long pk = __double_as_longlong(wj.w);
+                j = (int)(pk & 0xffffffffll);
+                tj = (int)(pk >> 32);
+                d[0] = __dadd_rn(__dsub_rn(wj.x, wi[0]), sh[0]);
+                d[1] = __dadd_rn(__dsub_rn(wj.y, wi[1]), sh[1]);
+                d[2] = __dadd_rn(__dsub_rn(wj.z, wi[2]), sh[2]);
+                r2 = __dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2]));
+                keep = (r2 < ec.rc2) && !(zero_shift && j == i);
+            }
+            int slot = -1;
+            for (int t = 0; t < ec.ntypes; ++t) {
+                const unsigned mk = __ballot_sync(0xffffffffu, keep && tj == t);
+                if (keep && tj == t) slot = cnt[t] + __popc(mk & lt_mask);
+                cnt[t] += __popc(mk);
+            }
+            if (keep) {
+                if (slot >= ec.sel[tj]) {
+                    atomicMax(overflow, 1);
+                } else {
+                    // environment row in FP64 (R-12), stored FP32
+                    const double r = sqrt(r2);
+                    double sw = 1.0, dsw = 0.0;
+                    if (r >= ec.rs) {
+                        const double u = (r - ec.rs) * ec.inv_range;
+                        sw = u * u * u * (-6.0 * u * u + 15.0 * u - 10.0) + 1.0;
+                        dsw = -30.0 * u * u * (u - 1.0) * (u - 1.0) * ec.inv_range;
                     }
-                    int slot = -1;
-                    for (int t = 0; t < ec.ntypes; ++t) {
-                        const unsigned mk = __ballot_sync(0xffffffffu, keep && tj == t);
-                        if (keep && tj == t) slot = cnt[t] + __popc(mk & lt_mask);
-                        cnt[t] += __popc(mk);
-                    }
-                    if (keep) {
-                        if (slot >= ec.sel[tj]) {
-                            atomicMax(overflow, 1);
-                        } else {
-                            // environment row in FP64 (R-12), stored FP32
-                            const double r = sqrt(r2);
-                            double sw = 1.0, dsw = 0.0;
-                            if (r >= ec.rs) {
-                                const double u = (r - ec.rs) * ec.inv_range;
-                                sw = u * u * u * (-6.0 * u * u + 15.0 * u - 10.0) + 1.0;
-                                dsw = -30.0 * u * u * (u - 1.0) * (u - 1.0) * ec.inv_range;
-                            }
-                            const double rinv = 1.0 / r;
-                            const double s = sw * rinv;
-                            const double ds = dsw * rinv - sw * rinv * rinv;
-                            NeighSlotA A;
-                            A.dx = (float)d[0]; A.dy = (float)d[1]; A.dz = (float)d[2]; A.s = (float)s;
-                            NeighSlotB B;
-                            B.ds = (float)ds; B.rinv = (float)rinv;
-                            const uint32_t code = (uint32_t)(nx + 3) | ((uint32_t)(ny + 3) << 3) | ((uint32_t)(nz + 3) << 6);
-                            B.jcode = (uint32_t)j | (code << 23);
-                            B.pad = 0.f;
-                            const size_t o = slot0 + ec.seloff[tj] + slot;
-                            slotA[o] = A;
-                            slotB[o] = B;
-                        }
-                    }
+                    const double rinv = 1.0 / r;
+                    const double s = sw * rinv;
+                    const double ds = dsw * rinv - sw * rinv * rinv;
+                    NeighSlotA A;
+                    A.dx = (float)d[0]; A.dy = (float)d[1]; A.dz = (float)d[2]; A.s = (float)s;
+                    NeighSlotB B;
+                    B.ds = (float)ds; B.rinv = (float)rinv;
+                    const uint32_t code = (uint32_t)(nx + 3) | ((uint32_t)(ny + 3) << 3) | ((uint32_t)(nz + 3) << 6);
+                    B.jcode = (uint32_t)j | (code << 23);
+                    B.pad = 0.f;
+                    const size_t o = slot0 + ec.seloff[tj] + slot;
+                    slotA[o] = A;
+                    slotB[o] = B;
                 }
+            }
+
             }
         }
     }
