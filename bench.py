@@ -26,6 +26,9 @@ if ROOT not in sys.path:
 import workloads  # noqa: E402
 
 METRIC = "bead-atom-steps/s"
+# dram__bytes_read.sum + dram__bytes_write.sum per launch at configs[2], from the committed ncu --set full capture
+# (profiles/r1c_README.md); None where the phase is several kernels
+NCU_DRAM_BYTES = {"embed_fwd": 275.95e6 + 76.92e6, "embed_bwd": 308.27e6 + 10.72e6, "fitting": None}
 
 
 def _peaks():
@@ -230,14 +233,14 @@ def run_ours(args):
     tf32_peak = 0.5 * bf16_peak
     mufu_peak = 148 * 16 * peaks["sm_max_mhz"] * 1e6 / 1e12                         # T MUFU op/s
     issued = {                                                                       # padded tiles, 3xTF32 passes
-        "embed_fwd": 2.0 * rows * 3 * (32 * 64 + 56 * 112),
-        "embed_bwd": 2.0 * rows * 3 * 2 * (32 * 64 + 56 * 112),                     # value + derivative rows
+        "embed_fwd": 2.0 * rows * 3 * (32 * 64 + 56 * 128),                         # K2 x N2 + K3 x N3 of embedding_tc.cu
+        "embed_bwd": 2.0 * rows * 3 * 2 * (32 * 64 + 56 * 128),                     # value + derivative rows
         "fitting": 3 * 2.0 * PN * 2 * (1600 * 240 + 2 * 240 * 240),
     }
     mufu_ops = {"embed_fwd": 2.0 * rows * 175, "embed_bwd": 2.0 * rows * 175, "fitting": 0.0}
     achieved = flops[dom] / (phases[dom] * 1e-3) / 1e12
     roofline = {"kernel": dom, "bound": "tensor", "achieved": achieved, "peak": tf32_peak, "unit": "TFLOP/s",
-                "frac": achieved / tf32_peak, "traffic": None,
+                "frac": achieved / tf32_peak, "traffic": NCU_DRAM_BYTES.get(dom),
                 "issued_tflops": issued[dom] / (phases[dom] * 1e-3) / 1e12,
                 "note": "achieved = USEFUL flops (SURVEY 8(d): no recompute, no 3xTF32 extra passes) / live CUDA-event "
                         "time of the phase; peak = TF32 dense = %s BF16 %.0f TFLOP/s x 1/2 (guide's nominal ratio); "
@@ -300,7 +303,7 @@ def run_ours(args):
             "vs_baseline": None, "dtype": "f32 network / f64 geometry+integrator", "data": "synthetic",
             "config": {"workload": cfg["name"], "atoms": N, "beads": P, "bead_atoms": P * N, "neighbour_rows": rows,
                        "parallelism": "replicas only" if world > 1 else "1 GPU",
-                       "l2": "no flush: per-step working set (neighbour slots, D, dD, activations ~1.5 GB) exceeds the 126 MB L2"},
+                       "l2": "no flush: per-step working set (neighbour rows 135 MB, T and dT 157 MB, fitting activations ~380 MB) exceeds the 126 MB L2"},
             "roofline": roofline, "kernels": kernels, "integrator_hbm": integ, "cpu_baseline": cpu,
             "e2e": {"value": world * P * N / e2e_s, "unit": METRIC, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": e2e_s * 1e3, "call": "pimd_restore(host x,p,f,U) + pimd_step(1) + pimd_get_{positions,momenta,forces,energies,estimators}"},
@@ -345,10 +348,17 @@ def main():
     ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json configs (default: the headline)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-integrator-leg", action="store_true")
+    ap.add_argument("--integrator-only", action="store_true",
+                    help="only the stand-alone integrator leg (2^20 atoms x 32 beads, HBM-bound size); prints its JSON")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         return run_reference(args)
+    if args.integrator_only:
+        import paper_2602_13553_b200 as pk
+        pk.lib()
+        print(json.dumps(integrator_leg(pk, _peaks())))
+        return 0
     return run_ours(args)
 
 
