@@ -85,6 +85,21 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
+def max_over_ranks(value, world, device):
+    """Whole-job time = the slowest rank's (replicas only: no data-path collective)."""
+    if world <= 1:
+        return float(value)
+    import torch
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_throughput(units_per_rank, world, ms_max):
+    """bead-atom-steps/s of the whole job: every rank advanced its own replica by `units_per_rank`."""
+    return world * units_per_rank / (ms_max * 1e-3)
+
+
 def _dist():
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -210,11 +225,8 @@ def run_ours(args):
     ms = ev0.elapsed_time(ev1)
     launches = pk.pimd_get_launch_count(sim.ctx) - launches0
     clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
-    if world > 1:
-        t = torch.tensor([ms], device="cuda")
-        torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * P * N * args.steps / (ms * 1e-3)
+    ms = max_over_ranks(ms, world, "cuda")
+    value = job_throughput(P * N * args.steps, world, ms)
 
     # ---- per-phase device times (CUDA events on the library's stream) ----
     pk.pimd_set_profiling(sim.ctx, 1)
@@ -269,6 +281,9 @@ def run_ours(args):
     Uo = sim.energies()
     x_host.copy_(torch.from_numpy(xo)); p_host.copy_(torch.from_numpy(po)); f_host.copy_(torch.from_numpy(fo))
     xn, pn, fn = x_host.numpy(), p_host.numpy(), f_host.numpy()
+    # device -> host results land in pinned buffers of their own (then become the next step's inputs)
+    xo_h, po_h, fo_h = (torch.empty_like(x_host).pin_memory() for _ in range(3))
+    xon, pon, fon = xo_h.numpy(), po_h.numpy(), fo_h.numpy()
     step_no = sim.estimators()["step"]
     e2e_steps = max(3, min(args.steps, 10))
     barrier()
@@ -276,16 +291,13 @@ def run_ours(args):
     for q in range(e2e_steps):
         pk.pimd_restore(sim.ctx, xn, pn, fn, Uo, step_no + q)          # H2D: x, p, f (+U)
         sim.step(1)
-        xo = sim.positions(); po = sim.momenta(); fo = sim.forces()       # D2H
+        sim.positions(out=xon); sim.momenta(out=pon); sim.forces(out=fon)   # D2H
         Uo = sim.energies()
         est = sim.estimators()
-        xn[...] = xo; pn[...] = po; fn[...] = fo
+        xn, xon = xon, xn; pn, pon = pon, pn; fn, fon = fon, fn            # results are the next step's inputs
     barrier()
     e2e_s = (time.perf_counter() - t0) / e2e_steps
-    if world > 1:
-        t = torch.tensor([e2e_s], device="cuda")
-        torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = max_over_ranks(e2e_s, world, "cuda")
     h2d = 3 * P * N * 24 + P * 8
     d2h = 3 * P * N * 24 + P * 8 + 32
 

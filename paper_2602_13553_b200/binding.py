@@ -216,22 +216,27 @@ def pimd_step(ctx, n_steps=1):
     return _check(ctx, lib().pimd_step(ctx, int(n_steps)))
 
 
-def _getter(name, ctx, shape):
-    out = np.empty(shape, dtype=np.float64)
+def _getter(name, ctx, shape, out=None):
+    """`out`: optional C-contiguous float64 array of `shape` to receive the copy (e.g. a view of pinned memory,
+    which makes the device->host copy a direct DMA); a fresh array otherwise."""
+    if out is None:
+        out = np.empty(shape, dtype=np.float64)
+    elif out.dtype != np.float64 or tuple(out.shape) != tuple(shape) or not out.flags["C_CONTIGUOUS"]:
+        raise ValueError("out must be a C-contiguous float64 array of shape %r" % (tuple(shape),))
     _check(ctx, getattr(lib(), name)(ctx, out.ctypes.data))
     return out
 
 
-def pimd_get_positions(ctx, P, N):
-    return _getter("pimd_get_positions", ctx, (P, N, 3))
+def pimd_get_positions(ctx, P, N, out=None):
+    return _getter("pimd_get_positions", ctx, (P, N, 3), out)
 
 
-def pimd_get_momenta(ctx, P, N):
-    return _getter("pimd_get_momenta", ctx, (P, N, 3))
+def pimd_get_momenta(ctx, P, N, out=None):
+    return _getter("pimd_get_momenta", ctx, (P, N, 3), out)
 
 
-def pimd_get_forces(ctx, P, N):
-    return _getter("pimd_get_forces", ctx, (P, N, 3))
+def pimd_get_forces(ctx, P, N, out=None):
+    return _getter("pimd_get_forces", ctx, (P, N, 3), out)
 
 
 def pimd_get_virial(ctx, P):
@@ -344,9 +349,9 @@ class PIMD:
     def step(self, n=1):
         return pimd_step(self.ctx, n)
 
-    def positions(self): return pimd_get_positions(self.ctx, self.P, self.N)
-    def momenta(self): return pimd_get_momenta(self.ctx, self.P, self.N)
-    def forces(self): return pimd_get_forces(self.ctx, self.P, self.N)
+    def positions(self, out=None): return pimd_get_positions(self.ctx, self.P, self.N, out)
+    def momenta(self, out=None): return pimd_get_momenta(self.ctx, self.P, self.N, out)
+    def forces(self, out=None): return pimd_get_forces(self.ctx, self.P, self.N, out)
     def virial(self): return pimd_get_virial(self.ctx, self.P)
     def energies(self): return pimd_get_energies(self.ctx, self.P)
     def atom_energies(self): return pimd_get_atom_energies(self.ctx, self.P, self.N)

@@ -235,6 +235,26 @@ def test_force_parity_config1_sampled_beads(pk):
     sim.close()
 
 
+def test_force_parity_config2_headline_size_sampled_beads(pk):
+    """BASELINE.json's headline configuration (1536 atoms x 32 beads), in the launch configuration bench.py
+    times; the oracle evaluates two sampled beads (a few seconds each)."""
+    cfg, wb, desc, w = workloads.make_config(2)
+    sim = pk.PIMD(wb["types"], wb["masses"], wb["box"], cfg["P"], cfg["T"], cfg["dt"], cfg["gamma"], seed=0,
+                  model_desc=desc)
+    sim.set_state(wb["x"], wb["p"])
+    sim.set_model(w)
+    model = se_e2_a.Model(desc, w)
+    f, U, Xi, E = sim.forces(), sim.energies(), sim.virial(), sim.atom_energies()
+    for k in (0, 31):
+        Eo, Fo, Xio = se_e2_a.energy_forces(wb["x"][k], wb["types"], wb["box"], model)
+        _force_checks(f[k:k + 1], Fo[None], U[k:k + 1], np.array([Eo.sum()]), Xi[k:k + 1], Xio[None], E[k], Eo, sim.N)
+    # properties that hold for every bead at any size: Newton's third law, symmetric virial
+    assert np.abs(f.sum(axis=1)).max() <= 1e-6 * np.abs(f).max() * sim.N ** 0.5
+    X3 = Xi.reshape(-1, 3, 3)
+    assert np.abs(X3 - np.swapaxes(X3, 1, 2)).max() <= 1e-5 * np.abs(X3).max()
+    sim.close()
+
+
 # ---------------------------------------------------------------------------------------------
 # the whole step, configs[0]
 # ---------------------------------------------------------------------------------------------
