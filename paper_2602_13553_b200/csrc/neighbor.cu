@@ -185,14 +185,20 @@ neighbor_env_kernel(int P, int N, GridGeom g, EnvConsts ec, const double* __rest
                 r2 = __dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2]));
                 keep = (r2 < ec.rc2) && !(zero_shift && j == i);
             }
-            int slot = -1;
-            for (int t = 0; t < ec.ntypes; ++t) {
-                const unsigned mk = __ballot_sync(0xffffffffu, keep && tj == t);
-                if (keep && tj == t) slot = cnt[t] + __popc(mk & lt_mask);
-                cnt[t] += __popc(mk);
+            // slot inside the type partition; fully unrolled over the (at most PIMD_MAX_TYPES) types so that the
+            // counters stay in registers and sel / seloff are constant-bank operands
+            int slot = -1, sel_t = 0, seloff_t = 0;
+#pragma unroll
+            for (int t = 0; t < PIMD_MAX_TYPES; ++t) {
+                if (t < ec.ntypes) {
+                    const bool mine = keep && tj == t;
+                    const unsigned mk = __ballot_sync(0xffffffffu, mine);
+                    if (mine) { slot = cnt[t] + __popc(mk & lt_mask); sel_t = ec.sel[t]; seloff_t = ec.seloff[t]; }
+                    cnt[t] += __popc(mk);
+                }
             }
             if (keep) {
-                if (slot >= ec.sel[tj]) {
+                if (slot >= sel_t) {
                     atomicMax(overflow, 1);
                 } else {
                     // environment row in FP64 (R-12), stored FP32
@@ -213,7 +219,7 @@ neighbor_env_kernel(int P, int N, GridGeom g, EnvConsts ec, const double* __rest
                     const uint32_t code = (uint32_t)(nx + 3) | ((uint32_t)(ny + 3) << 3) | ((uint32_t)(nz + 3) << 6);
                     B.jcode = (uint32_t)j | (code << 23);
                     B.pad = 0.f;
-                    const size_t o = slot0 + ec.seloff[tj] + slot;
+                    const size_t o = slot0 + seloff_t + slot;
                     slotA[o] = A;
                     slotB[o] = B;
                 }
@@ -223,7 +229,9 @@ neighbor_env_kernel(int P, int N, GridGeom g, EnvConsts ec, const double* __rest
         }
     }
     if (lane == 0) {
-        for (int t = 0; t < ec.ntypes; ++t) ncount[(size_t)ba * ec.ntypes + t] = min(cnt[t], ec.sel[t]);
+#pragma unroll
+        for (int t = 0; t < PIMD_MAX_TYPES; ++t)
+            if (t < ec.ntypes) ncount[(size_t)ba * ec.ntypes + t] = min(cnt[t], ec.sel[t]);
     }
 }
 
