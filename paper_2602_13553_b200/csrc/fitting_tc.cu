@@ -53,7 +53,8 @@ struct TcSmem {
     static constexpr int kBBytes = BN * 64;
     static constexpr int oAhi = 0, oAlo = NH * kABytes, oBhi = 2 * NH * kABytes, oBlo = 2 * NH * kABytes + kBBytes;
     static constexpr int kStage = 2 * NH * kABytes + 2 * kBBytes;
-    static constexpr int kTotal = ST * kStage + 1024 /*align slack*/ + 256 /*barriers*/;
+    static constexpr int kEpiOff = ST * kStage + 256;                       // 4 warps x 32 x 20 floats: epilogue transpose
+    static constexpr int kTotal = ST * kStage + 256 /*barriers*/ + 4 * 32 * 20 * 4 + 1024 /*align slack*/;
     static constexpr int kTmemCols = (NH * BN <= 256) ? 256 : 512;
 };
 
@@ -161,27 +162,36 @@ gemm3xtf32_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ T
             fence_proxy_async_smem();
             mbar_arrive(ready + s);
         }
-        // ---- epilogue: one thread per row; the row's `add` / `tt` operands are fetched one chunk ahead ----
+        // ---- epilogue.  tcgen05.ld hands every lane one ROW of the accumulator; row-per-lane global accesses
+        // would touch 32 different 128 B lines per instruction (the L1 tag stage then bounds the epilogue), so each
+        // 32 x 16 chunk goes through a per-warp shared-memory patch and comes back as lane <-> (row l/4 + 8 j,
+        // columns 4 (l % 4) .. + 3), j = 0..3: a warp-wide float4 access then covers 8 rows x 64 contiguous bytes.
+        // All epilogue math is elementwise, so it runs in that layout; `add` / `tt` are fetched one chunk ahead. ----
         mbar_wait(tmem_full, 0);
         tc_fence_after();
         const int quarter = warp & 3;                      // TMEM lane quarter this warp may access
         constexpr bool kAdd = (EPI == TEPI_TANH_BIAS_SKIP || EPI == TEPI_L3E || EPI == TEPI_BWD_FIRST);
         constexpr bool kTt = (EPI == TEPI_BWD_VEC || EPI == TEPI_BWD_FIRST);
         constexpr bool kTanh = (EPI == TEPI_TANH_BIAS || EPI == TEPI_TANH_BIAS_SKIP || EPI == TEPI_L3E);
+        float* patch = reinterpret_cast<float*>(smem + SM::kEpiOff) + (warp - 2) * (32 * 20);
+        const int lr = lane >> 2, lc = 4 * (lane & 3);     // my row (+ 8 j) and column offset inside a chunk
+        const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll 1
         for (int h = 0; h < NH; ++h) {
-            const int ml = m0 + h * 128 + quarter * 32 + lane;     // row inside the type
-            const bool row_ok = ml < rows_t;
-            const size_t m = (size_t)(g.row0[ty] + (row_ok ? ml : 0));   // type-sorted global row
-            float e_acc = 0.f;
-            const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
-            const float4* adp = kAdd ? reinterpret_cast<const float4*>(g.add + m * g.ldadd + n0) : nullptr;
-            const float4* ttp = kTt ? reinterpret_cast<const float4*>(g.tt + m * g.ldtt + n0) : nullptr;
+            const int mbase = m0 + h * 128 + quarter * 32;         // first row of this warp inside the type
+            bool ok[4];
+            size_t mrow[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                ok[j] = mbase + lr + 8 * j < rows_t;
+                mrow[j] = (size_t)(g.row0[ty] + (ok[j] ? mbase + lr + 8 * j : 0));
+            }
+            float e_acc[4] = {0.f, 0.f, 0.f, 0.f};
             float4 adn[4], ttn[4];
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                adn[q] = (kAdd && row_ok) ? adp[q] : zero4;
-                ttn[q] = (kTt && row_ok) ? ttp[q] : zero4;
+            for (int j = 0; j < 4; ++j) {
+                adn[j] = (kAdd && ok[j] && n0 < g.N) ? *reinterpret_cast<const float4*>(g.add + mrow[j] * g.ldadd + n0 + lc) : zero4;
+                ttn[j] = (kTt && ok[j] && n0 < g.N) ? *reinterpret_cast<const float4*>(g.tt + mrow[j] * g.ldtt + n0 + lc) : zero4;
             }
 #pragma unroll 1
             for (int c = 0; c < BN / 16; ++c) {
@@ -189,60 +199,59 @@ gemm3xtf32_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ T
                 tmem_ld16(tmem_base + ((uint32_t)(quarter * 32) << 16) + h * 256 + c * 16, v);
                 float4 ad[4], t4[4];
 #pragma unroll
-                for (int q = 0; q < 4; ++q) { ad[q] = adn[q]; t4[q] = ttn[q]; }
+                for (int j = 0; j < 4; ++j) { ad[j] = adn[j]; t4[j] = ttn[j]; }
                 const int n = n0 + c * 16;
-                const bool more = row_ok && (c + 1 < BN / 16) && (n + 16 < g.N);
+                const bool more = (c + 1 < BN / 16) && (n + 16 < g.N);
 #pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    if (kAdd) adn[q] = more ? adp[4 * (c + 1) + q] : zero4;
-                    if (kTt) ttn[q] = more ? ttp[4 * (c + 1) + q] : zero4;
+                for (int j = 0; j < 4; ++j) {
+                    if (kAdd) adn[j] = (more && ok[j]) ? *reinterpret_cast<const float4*>(g.add + mrow[j] * g.ldadd + n + 16 + lc) : zero4;
+                    if (kTt) ttn[j] = (more && ok[j]) ? *reinterpret_cast<const float4*>(g.tt + mrow[j] * g.ldtt + n + 16 + lc) : zero4;
                 }
                 tmem_ld_wait();
-                if (!row_ok || n >= g.N) continue;
-                float r[16];
+                // transpose through the patch: row `lane` in, (row lr + 8 j, columns lc..lc+3) out
 #pragma unroll
-                for (int q = 0; q < 16; ++q) r[q] = __uint_as_float(v[q]);
+                for (int q = 0; q < 4; ++q)
+                    *reinterpret_cast<float4*>(patch + lane * 20 + 4 * q) =
+                        make_float4(__uint_as_float(v[4 * q]), __uint_as_float(v[4 * q + 1]), __uint_as_float(v[4 * q + 2]), __uint_as_float(v[4 * q + 3]));
+                __syncwarp();
+                float4 r[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) r[j] = *reinterpret_cast<const float4*>(patch + (lr + 8 * j) * 20 + lc);
+                __syncwarp();
+                if (n >= g.N) continue;
                 if (kTanh) {
-                    const float4* bias = reinterpret_cast<const float4*>(g.bias[ty] + n);
+                    const float4 b4 = __ldg(reinterpret_cast<const float4*>(g.bias[ty] + n + lc));
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        const float4 b4 = __ldg(bias + q);
-                        r[4 * q] = tanh_fast(r[4 * q] + b4.x); r[4 * q + 1] = tanh_fast(r[4 * q + 1] + b4.y);
-                        r[4 * q + 2] = tanh_fast(r[4 * q + 2] + b4.z); r[4 * q + 3] = tanh_fast(r[4 * q + 3] + b4.w);
+                    for (int j = 0; j < 4; ++j) {
+                        r[j].x = tanh_fast(r[j].x + b4.x); r[j].y = tanh_fast(r[j].y + b4.y);
+                        r[j].z = tanh_fast(r[j].z + b4.z); r[j].w = tanh_fast(r[j].w + b4.w);
                     }
                 }
-                float4* o0 = (g.out0 != nullptr) ? reinterpret_cast<float4*>(g.out0 + m * g.ldo + n) : nullptr;
-                float4* o1 = (g.out1 != nullptr) ? reinterpret_cast<float4*>(g.out1 + m * g.ldo + n) : nullptr;
-                if (EPI == TEPI_TANH_BIAS || EPI == TEPI_PLAIN) {
+                float4 w = zero4;
+                if (EPI == TEPI_L3E || EPI == TEPI_BWD_VEC) w = __ldg(reinterpret_cast<const float4*>(g.vec[ty] + n + lc));
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) o0[q] = make_float4(r[4 * q], r[4 * q + 1], r[4 * q + 2], r[4 * q + 3]);
-                } else if (EPI == TEPI_TANH_BIAS_SKIP) {
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        o0[q] = make_float4(r[4 * q], r[4 * q + 1], r[4 * q + 2], r[4 * q + 3]);
-                        const float4 a4 = ad[q];
-                        o1[q] = make_float4(r[4 * q] + a4.x, r[4 * q + 1] + a4.y, r[4 * q + 2] + a4.z, r[4 * q + 3] + a4.w);
-                    }
-                } else if (EPI == TEPI_L3E) {
-                    // y3 = y2 + t3 ; E_i += y3 . w4 ; seed of the backward pass da3 = w4 o (1 - t3^2) -> out1
-                    const float4* w4 = reinterpret_cast<const float4*>(g.vec[ty] + n);
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        const float4 a4 = ad[q], w = __ldg(w4 + q);
-                        e_acc = fmaf(a4.x + r[4 * q], w.x, e_acc);
-                        e_acc = fmaf(a4.y + r[4 * q + 1], w.y, e_acc);
-                        e_acc = fmaf(a4.z + r[4 * q + 2], w.z, e_acc);
-                        e_acc = fmaf(a4.w + r[4 * q + 3], w.w, e_acc);
-                        o1[q] = make_float4(w.x * (1.f - r[4 * q] * r[4 * q]), w.y * (1.f - r[4 * q + 1] * r[4 * q + 1]),
-                                            w.z * (1.f - r[4 * q + 2] * r[4 * q + 2]), w.w * (1.f - r[4 * q + 3] * r[4 * q + 3]));
-                    }
-                } else {   // TEPI_BWD_VEC, TEPI_BWD_FIRST
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        const float4 a4 = (EPI == TEPI_BWD_VEC) ? __ldg(reinterpret_cast<const float4*>(g.vec[ty] + n) + q) : ad[q];
-                        const float4 tq = t4[q];
-                        float4 y = make_float4(r[4 * q] + a4.x, r[4 * q + 1] + a4.y, r[4 * q + 2] + a4.z, r[4 * q + 3] + a4.w);
-                        if (EPI == TEPI_BWD_VEC) o0[q] = y;
+                for (int j = 0; j < 4; ++j) {
+                    if (!ok[j]) continue;
+                    float4* o0 = (g.out0 != nullptr) ? reinterpret_cast<float4*>(g.out0 + mrow[j] * g.ldo + n + lc) : nullptr;
+                    float4* o1 = (g.out1 != nullptr) ? reinterpret_cast<float4*>(g.out1 + mrow[j] * g.ldo + n + lc) : nullptr;
+                    if (EPI == TEPI_TANH_BIAS || EPI == TEPI_PLAIN) {
+                        *o0 = r[j];
+                    } else if (EPI == TEPI_TANH_BIAS_SKIP) {
+                        *o0 = r[j];
+                        *o1 = make_float4(r[j].x + ad[j].x, r[j].y + ad[j].y, r[j].z + ad[j].z, r[j].w + ad[j].w);
+                    } else if (EPI == TEPI_L3E) {
+                        // y3 = y2 + t3 ; E_i += y3 . w4 ; seed of the backward pass da3 = w4 o (1 - t3^2) -> out1
+                        e_acc[j] = fmaf(ad[j].x + r[j].x, w.x, e_acc[j]);
+                        e_acc[j] = fmaf(ad[j].y + r[j].y, w.y, e_acc[j]);
+                        e_acc[j] = fmaf(ad[j].z + r[j].z, w.z, e_acc[j]);
+                        e_acc[j] = fmaf(ad[j].w + r[j].w, w.w, e_acc[j]);
+                        *o1 = make_float4(w.x * (1.f - r[j].x * r[j].x), w.y * (1.f - r[j].y * r[j].y),
+                                          w.z * (1.f - r[j].z * r[j].z), w.w * (1.f - r[j].w * r[j].w));
+                    } else {   // TEPI_BWD_VEC (add = the row vector w4), TEPI_BWD_FIRST
+                        const float4 a4 = (EPI == TEPI_BWD_VEC) ? w : ad[j];
+                        const float4 tq = t4[j];
+                        float4 y = make_float4(r[j].x + a4.x, r[j].y + a4.y, r[j].z + a4.z, r[j].w + a4.w);
+                        if (EPI == TEPI_BWD_VEC) *o0 = y;
                         y.x *= (1.f - tq.x * tq.x); y.y *= (1.f - tq.y * tq.y);
                         y.z *= (1.f - tq.z * tq.z); y.w *= (1.f - tq.w * tq.w);
                         if (EPI == TEPI_BWD_FIRST) {     // da1 feeds dd_dt_kernel only: written pre-split (hi -> out1, lo -> out0)
@@ -251,30 +260,44 @@ gemm3xtf32_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ T
                             hi.y = __uint_as_float(__float_as_uint(y.y) & 0xFFFFE000u);
                             hi.z = __uint_as_float(__float_as_uint(y.z) & 0xFFFFE000u);
                             hi.w = __uint_as_float(__float_as_uint(y.w) & 0xFFFFE000u);
-                            o1[q] = hi;
-                            o0[q] = make_float4(y.x - hi.x, y.y - hi.y, y.z - hi.z, y.w - hi.w);
+                            *o1 = hi;
+                            *o0 = make_float4(y.x - hi.x, y.y - hi.y, y.z - hi.z, y.w - hi.w);
                         } else {
-                            o1[q] = y;
+                            *o1 = y;
                         }
                     }
                 }
             }
             if (EPI == TEPI_L3E) {
-                // E_i = y3 . w4 + b4 ; U^(bead) += E_i : one atomic per warp when its rows share the bead
-                const int ba = row_ok ? g.cen_idx[m] : 0;
-                const double e = row_ok ? (double)(e_acc + __ldg(g.b4[ty])) : 0.0;
-                if (row_ok) g.Eatom[ba] = e;
-                const int bead = row_ok ? ba / g.natoms : -1;
-                const int bead0 = __shfl_sync(0xffffffffu, bead, 0);
-                const bool uniform = __all_sync(0xffffffffu, bead == bead0 || bead < 0);
-                if (uniform) {
-                    double sum = e;
+                // E_i = y3 . w4 + b4: the four lanes of a row add their column shares; lane 4 r then owns rows
+                // r + 8 j.  U^(bead) += E_i with one atomic per warp when all its rows share the bead.
+                double esum = 0.0;
+                int bead_u = -1;
+                bool uniform = true;
 #pragma unroll
-                    for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
-                    if (lane == 0 && bead0 >= 0) atomicAdd(g.U + bead0, sum);
-                } else if (row_ok) {
-                    atomicAdd(g.U + bead, e);
+                for (int j = 0; j < 4; ++j) {
+                    float e = e_acc[j];
+                    e += __shfl_xor_sync(0xffffffffu, e, 1);
+                    e += __shfl_xor_sync(0xffffffffu, e, 2);
+                    const bool mine = ok[j] && (lane & 3) == 0;
+                    const int ba = mine ? g.cen_idx[mrow[j]] : 0;
+                    const double ed = mine ? (double)(e + __ldg(g.b4[ty])) : 0.0;
+                    if (mine) g.Eatom[ba] = ed;
+                    const int bead = mine ? ba / g.natoms : -1;
+                    const int bmax = __reduce_max_sync(0xffffffffu, bead);
+                    const bool same = __all_sync(0xffffffffu, bead < 0 || bead == bmax);
+                    if (same && (bead_u < 0 || bmax < 0 || bmax == bead_u)) {
+                        esum += ed;
+                        if (bmax >= 0) bead_u = bmax;
+                    } else {
+                        uniform = false;
+                        if (mine) atomicAdd(g.U + bead, ed);
+                    }
                 }
+                (void)uniform;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) esum += __shfl_xor_sync(0xffffffffu, esum, o);
+                if (lane == 0 && bead_u >= 0) atomicAdd(g.U + bead_u, esum);
             }
         }
     }
