@@ -200,22 +200,6 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
-// MUFU token: the tanh-heavy phases of the two contexts of a CTA are mutually exclusive.  Left alone, the two
-// (identical) contexts phase-lock -- both in a MUFU-bound phase, then both waiting for their MMAs -- and every
-// phase takes twice as long; with the token one context's tanh work overlaps the other's MMA round trips and
-// its T accumulation.  Warp 0 of the context takes the lock, everyone else blocks in the hardware barrier.
-__device__ __forceinline__ void mufu_acquire(uint32_t* lock, int bar_id) {
-    if ((threadIdx.x & 255) < 32) {
-        if ((threadIdx.x & 31) == 0) {
-            while (atomicCAS(lock, 0u, 1u) != 0u) __nanosleep(40);
-        }
-        __syncwarp();
-    }
-    named_bar_sync(bar_id, 256);
-}
-// by ONE thread, after the context barrier that ends the phase
-__device__ __forceinline__ void mufu_release(uint32_t* lock) { atomicExch(lock, 0u); }
-
 __device__ __forceinline__ void red_add_v4(float* addr, float a, float b, float c, float d) {
     asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
 }
@@ -261,7 +245,6 @@ struct CtxSetup {
     uint8_t* ctx;        // this context's region
     uint64_t* mma_bar;
     uint32_t tmem_base;  // allocation base (all contexts)
-    uint32_t* lock;      // MUFU token
 };
 
 // common prologue: barriers, TMEM allocation of `ncols` columns; returns after a CTA-wide sync
@@ -275,9 +258,7 @@ __device__ __forceinline__ CtxSetup ctx_setup(uint8_t* smem_raw, uint32_t ncols)
     uint64_t* bars = reinterpret_cast<uint64_t*>(c.smem + etc::kImgPad + 2 * etc::kCtxBytes);
     c.mma_bar = bars + wg;
     uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(bars + 2);
-    c.lock = reinterpret_cast<uint32_t*>(bars + 3);
     if (threadIdx.x == 0) {
-        *c.lock = 0u;
         mbar_init(bars, 1);
         mbar_init(bars + 1, 1);
         fence_barrier_init();
@@ -306,7 +287,7 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
     extern __shared__ uint8_t smem_raw[];
     const CtxSetup cs = ctx_setup(smem_raw, 256);
     const int cx = threadIdx.x >> 8, half = (threadIdx.x >> 7) & 1, t = threadIdx.x & 127, lane = threadIdx.x & 31;
-    const int bar_ctx = 1 + cx;
+    const int bar_ctx = 1 + cx, bar_pair = 3 + cx * 4 + (t >> 5);
     uint8_t* ctx = cs.ctx;
     float4* Rs = reinterpret_cast<float4*>(ctx + oRs);
     int* cen_s = reinterpret_cast<int*>(ctx + oCen);
@@ -338,7 +319,7 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
         const int C = gridDim.x * 2, c = blockIdx.x * 2 + cx;
         const int tl0 = (int)((long long)ntile * c / C), tl1 = (int)((long long)ntile * (c + 1) / C);
         if (tl0 >= tl1) continue;
-        if (cx == 1 && a.skew_fwd > 0) {                    // de-phase the two contexts (see mufu_acquire)
+        if (cx == 1 && a.skew_fwd > 0) {                    // de-phase the two contexts (see the backward kernel)
             const long long t0 = clock64();
             while (clock64() - t0 < a.skew_fwd) __nanosleep(200);
         }
@@ -356,7 +337,6 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
             const RowIn nxt = load_row(a, addr_n1);
             addr_n1 = addr_n2;
 
-            mufu_acquire(cs.lock, bar_ctx);
             const float s = cur.s;
             if (half == 0) {
                 const float sr = cur.s * cur.rinv;
@@ -378,7 +358,6 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
             tc_fence_before();
             named_bar_sync(bar_ctx, 256);
             if ((threadIdx.x & 255) == 0) {
-                mufu_release(cs.lock);
                 tc_fence_after();
                 mma_block_3x(tmem_d, actx, actx + kABlk, wbase + oW2hi, wbase + oW2lo, idesc2, 4, true);
                 umma_commit(cs.mma_bar);
@@ -386,7 +365,6 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
             mbar_wait(cs.mma_bar, phase);
             phase ^= 1;
             tc_fence_after();
-            mufu_acquire(cs.lock, bar_ctx);
             // ---- epilogue 2: h2 = [h1,h1] + tanh(z2), my 26 columns; A2 K slots 28 half .. 28 half + 27 ----
             float h2[H2 + 2];
             {
@@ -411,7 +389,6 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
             tc_fence_before();
             named_bar_sync(bar_ctx, 256);
             if ((threadIdx.x & 255) == 0) {
-                mufu_release(cs.lock);
                 tc_fence_after();
                 mma_block_3x(tmem_d, actx, actx + 2 * kABlk, wbase + oW3hi, wbase + oW3lo, idesc3, 4, true);
                 mma_block_3x(tmem_d, actx + kABlk, actx + 3 * kABlk, wbase + oW3hi + kW3blk, wbase + oW3lo + kW3blk, idesc3,
@@ -421,7 +398,6 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
             mbar_wait(cs.mma_bar, phase);
             phase ^= 1;
             tc_fence_after();
-            mufu_acquire(cs.lock, bar_ctx);
             // ---- epilogue 3: G = [h2,h2] + tanh(z3), my 52 columns -> smem [row][GROW] (overlays the A region) ----
             {
                 const uint32_t col = tmem_d + lanefield + 64 * half;
@@ -453,8 +429,7 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
                 }
             }
             tc_fence_before();
-            named_bar_sync(bar_ctx, 256);                  // G rows complete
-            if ((threadIdx.x & 255) == 0) mufu_release(cs.lock);
+            named_bar_sync(bar_pair, 64);                  // the two warps of this lane quarter: G rows complete
             // ---- T_i += (1/N_sel) sum_rows G (x) R.  The warp pair owns the 32 rows it just wrote; each warp
             // takes 16 of them, lane <-> 4 staged G positions (26 lanes).  All lanes walk the same rows, so the
             // centre changes are warp-uniform and the R / centre reads are broadcasts. ----
@@ -894,9 +869,8 @@ static EmbTcArgs make_tc_args(Model& m, const ForceArgs& fa) {
     a.slotA = m.slotA; a.slotB = m.slotB; a.wimg = m.emb_img;
     a.Tm = m.Tm; a.dTm = m.dTm; a.f = fa.f; a.cpart = m.cpart;
     a.inv_nsel = 1.0f / (float)m.nsel;
-    // measured on B200: the backward kernel gains 8 % from a ~9 k-cycle head start; the forward
-    // kernel is de-phased by its MUFU token instead
-    a.skew_fwd = 0;
+    // measured on B200: plateaus at 4-6 k cycles (forward, -20 %) and 5-13 k cycles (backward, -8 %)
+    a.skew_fwd = 5000;
     a.skew_bwd = 9000;
     return a;
 }
