@@ -51,7 +51,7 @@ def pile_l_coefficients(om, gamma0, h):
     return c1, c2
 
 
-def o_step(vt, masses, T, om, gamma0, h, seed, step):
+def o_step(vt, masses, T, om, gamma0, h, seed, step, half=0):
     """O: PILE_L thermostat, Eq. D2 verbatim:
       v~_k <- c1_k v~_k + c2_k sqrt(n/(m_i beta)) eta,   eta(seed; step, k, i, alpha) from Philox.
     sqrt(n k_B T / m_i) is converted to A/ps with mvv2e.  gamma0 == 0 means NVE: the whole O step
@@ -61,7 +61,7 @@ def o_step(vt, masses, T, om, gamma0, h, seed, step):
     P, N, _ = vt.shape
     c1, c2 = pile_l_coefficients(om, gamma0, h)
     kk, ii, aa = np.meshgrid(np.arange(P), np.arange(N), np.arange(3), indexing="ij")
-    eta = philox.normal(seed, step, kk, ii, aa)
+    eta = philox.normal(seed, step, kk, ii, aa, half)
     sigma = np.sqrt(P * KB * T / (masses * MVV2E))            # [N]
     return c1[:, None, None] * vt + c2[:, None, None] * sigma[None, :, None] * eta
 
@@ -85,6 +85,26 @@ def baoab_finish(vt, f, masses, M, dt):
     (PAPER.md:L192), then the closing B(dt/2).  Returns (v~, f~)."""
     ft = nm.to_nm(M, f)
     vt = b_step(vt, ft, masses, 0.5 * dt)
+    return vt, ft
+
+
+def obabo_positions_half(x, vt, ft, masses, M, om, T, gamma0, dt, seed, step):
+    """First part of one OBABO step (PAPER.md:L165 lists OBABO as the default Trotter splitting; L84):
+    O(dt/2), B(dt/2), transform x, A(dt), inverse transform.  Each of the two O's of the step takes dt/2
+    (DESIGN R-3) and its own normals (`half` = 0 here, 1 in obabo_finish)."""
+    vt = o_step(vt, masses, T, om, gamma0, 0.5 * dt, seed, step, half=0)
+    vt = b_step(vt, ft, masses, 0.5 * dt)
+    xt = nm.to_nm(M, x)
+    xt, vt = a_step(xt, vt, om, dt)
+    x = nm.from_nm(M, xt)
+    return x, vt
+
+
+def obabo_finish(vt, f, masses, M, om, T, gamma0, dt, seed, step):
+    """Second part: transform of the new forces, B(dt/2), O(dt/2).  Returns (v~, f~)."""
+    ft = nm.to_nm(M, f)
+    vt = b_step(vt, ft, masses, 0.5 * dt)
+    vt = o_step(vt, masses, T, om, gamma0, 0.5 * dt, seed, step, half=1)
     return vt, ft
 
 

@@ -36,16 +36,18 @@ def philox4x32_10(c0, c1, c2, c3, k0, k1):
     return c0, c1, c2, c3
 
 
-def words_for(seed, step, k, i, alpha):
+def words_for(seed, step, k, i, alpha, half=0):
     """The four Philox words behind thermostat normal (step, mode k, atom i, component alpha).
     DESIGN R-10: key = (seed_lo32, seed_hi32); counter = (step_lo32, step_hi32, i, 4*(k//2) + alpha):
-    modes 2q and 2q+1 share one call and take the two Box-Muller branches (see `normal`)."""
+    modes 2q and 2q+1 share one call and take the two Box-Muller branches (see `normal`).
+    `half` = 1 selects the second thermostat half-step of an OBABO step (bit 31 of counter word 1;
+    steps are < 2**63); BAOAB's single O uses half = 0."""
     seed = int(seed) & 0xFFFFFFFFFFFFFFFF
     step = int(step) & 0xFFFFFFFFFFFFFFFF
     k = np.asarray(k, dtype=np.uint64)
     i = np.asarray(i, dtype=np.uint64)
     alpha = np.asarray(alpha, dtype=np.uint64)
-    return philox4x32_10(step & 0xFFFFFFFF, step >> 32, i, np.uint64(4) * (k >> np.uint64(1)) + alpha,
+    return philox4x32_10(step & 0xFFFFFFFF, (step >> 32) | (int(half) << 31), i, np.uint64(4) * (k >> np.uint64(1)) + alpha,
                          seed & 0xFFFFFFFF, seed >> 32)
 
 
@@ -58,13 +60,13 @@ def uniform53(wa, wb):
     return n.astype(np.float64) * (2.0 ** -53)
 
 
-def normal(seed, step, k, i, alpha):
+def normal(seed, step, k, i, alpha, half=0):
     """eta ~ N(0,1) of Eq. D2 by Box-Muller (DESIGN R-10):
     u1 = uniform53(w0,w1) + 2^-53 in (0,1] (so the logarithm is finite; the sum is exact),
     u2 = uniform53(w2,w3) in [0,1);  r = sqrt(-2 ln u1);
     eta = r cos(2 pi u2) for even k, r sin(2 pi u2) for odd k -- the two branches of one draw are
     independent standard normals, so one Philox call serves the mode pair (2q, 2q+1)."""
-    w0, w1, w2, w3 = words_for(seed, step, k, i, alpha)
+    w0, w1, w2, w3 = words_for(seed, step, k, i, alpha, half)
     u1 = uniform53(w0, w1) + 2.0 ** -53
     u2 = uniform53(w2, w3)
     r = np.sqrt(-2.0 * np.log(u1))

@@ -13,7 +13,7 @@ from . import nm, integrator, se_e2_a
 
 
 class OraclePIMD:
-    def __init__(self, types, masses_per_type, box, n_beads, T, dt, gamma_centroid, seed):
+    def __init__(self, types, masses_per_type, box, n_beads, T, dt, gamma_centroid, seed, integrator="baoab"):
         self.types = np.asarray(types, dtype=np.int64)
         self.N = self.types.size
         self.masses = np.asarray(masses_per_type, dtype=np.float64)[self.types]   # per atom
@@ -23,6 +23,8 @@ class OraclePIMD:
         self.dt = float(dt)
         self.gamma0 = float(gamma_centroid)
         self.seed = int(seed)
+        assert integrator in ("baoab", "obabo")
+        self.integrator = integrator
         self.M = nm.nm_matrix(self.P)
         self.om = nm.omegas(self.P, self.T)
         self.step_count = 0
@@ -76,6 +78,15 @@ class OraclePIMD:
 
     def step(self, n_steps=1):
         for _ in range(int(n_steps)):
+            if self.integrator == "obabo":
+                self.x, self.vt = integrator.obabo_positions_half(
+                    self.x, self.vt, self.ft, self.masses, self.M, self.om, self.T, self.gamma0,
+                    self.dt, self.seed, self.step_count)
+                self._forces()
+                self.vt, _ = integrator.obabo_finish(self.vt, self.f, self.masses, self.M, self.om, self.T,
+                                                     self.gamma0, self.dt, self.seed, self.step_count)
+                self.step_count += 1
+                continue
             self.x, self.vt = integrator.baoab_positions_half(
                 self.x, self.vt, self.ft, self.masses, self.M, self.om, self.T, self.gamma0,
                 self.dt, self.seed, self.step_count)

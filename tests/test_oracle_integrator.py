@@ -9,11 +9,11 @@ from oracle import integrator, nm, philox
 from oracle.pimd import OraclePIMD
 
 
-def _ho(P, T, dt, gamma0, n_part, bhw, seed=11, mass=1.008):
+def _ho(P, T, dt, gamma0, n_part, bhw, seed=11, mass=1.008, integ="baoab"):
     """n_part independent 3-D harmonic oscillators (one 'type'), beta*hbar*omega = bhw."""
     omega = bhw * C.KB * T / C.HBAR
     k_spring = mass * C.MVV2E * omega ** 2
-    o = OraclePIMD(np.zeros(n_part, dtype=int), [mass], [100.0, 100.0, 100.0], P, T, dt, gamma0, seed)
+    o = OraclePIMD(np.zeros(n_part, dtype=int), [mass], [100.0, 100.0, 100.0], P, T, dt, gamma0, seed, integrator=integ)
     return o, omega, k_spring
 
 
@@ -138,6 +138,57 @@ def test_p1_reduces_to_classical_langevin_baoab():
     assert np.abs(o.momenta()[0] - p).max() < 1e-11
 
 
+def test_obabo_is_the_documented_splitting_p1_by_hand():
+    """OBABO (the default splitting) at P = 1 against a hand-written classical
+    O(dt/2) B(dt/2) A(dt) B(dt/2) O(dt/2) in momentum form; the two O's of a step draw different normals
+    (`half` = 0 / 1, DESIGN R-10) and use c1 = exp(-gamma dt/2) (R-3)."""
+    T, dt, g, N = 300.0, 0.5e-3, 2.0, 5
+    o, omega, ks = _ho(1, T, dt, g, N, bhw=2.0, seed=5, integ="obabo")
+    rng = np.random.default_rng(4)
+    x0 = 0.1 * rng.standard_normal((1, N, 3))
+    p0 = 20 * rng.standard_normal((1, N, 3))
+    o.set_model_harmonic(ks)
+    o.set_state(x0, p0)
+    o.step(3)
+    m = 1.008
+    x, p = x0[0].copy(), p0[0].copy()
+    kk, ii, aa = np.meshgrid([0], np.arange(N), np.arange(3), indexing="ij")
+    c1 = math.exp(-g * 0.5 * dt)
+    amp = math.sqrt(1 - c1 * c1) * math.sqrt(m * C.KB * T / C.MVV2E)
+    for step in range(3):
+        p = c1 * p + amp * philox.normal(5, step, kk, ii, aa, 0)[0]
+        p += 0.5 * dt * (-ks * x) / C.MVV2E
+        x += dt * p / m
+        p += 0.5 * dt * (-ks * x) / C.MVV2E
+        p = c1 * p + amp * philox.normal(5, step, kk, ii, aa, 1)[0]
+    assert np.abs(o.positions()[0] - x).max() < 1e-13
+    assert np.abs(o.momenta()[0] - p).max() < 1e-11
+    # the two half-step streams differ from each other and from the next step's
+    e0, e1 = philox.normal(5, 0, kk, ii, aa, 0), philox.normal(5, 0, kk, ii, aa, 1)
+    assert np.abs(e0 - e1).min() > 0 and np.abs(e1 - philox.normal(5, 2 ** 31, kk, ii, aa, 0)).min() > 0
+
+
+def test_obabo_equals_baoab_without_thermostat_and_composes_the_o_steps():
+    """gamma = 0: both splittings are B(dt/2) A(dt) B(dt/2) (A(dt/2)A(dt/2) = A(dt), pinned above), so the
+    trajectories coincide; and c1(dt/2)^2 = c1(dt): two half O's damp like BAOAB's single O."""
+    P, T, dt, N = 8, 300.0, 0.25e-3, 6
+    rng = np.random.default_rng(3)
+    x0, p0 = 0.05 * rng.standard_normal((P, N, 3)), 30 * rng.standard_normal((P, N, 3))
+    res = []
+    for integ in ("baoab", "obabo"):
+        o, omega, ks = _ho(P, T, dt, 0.0, N, bhw=4.0, integ=integ)
+        o.set_model_harmonic(ks)
+        o.set_state(x0, p0)
+        o.step(20)
+        res.append((o.positions(), o.momenta()))
+    assert np.abs(res[0][0] - res[1][0]).max() < 1e-12 * np.abs(res[0][0]).max()
+    assert np.abs(res[0][1] - res[1][1]).max() < 1e-12 * np.abs(res[0][1]).max()
+    om = nm.omegas(P, T)
+    c1h, _ = integrator.pile_l_coefficients(om, 3.0, 0.5 * dt)
+    c1f, _ = integrator.pile_l_coefficients(om, 3.0, dt)
+    assert np.abs(c1h * c1h - c1f).max() < 1e-15
+
+
 def test_nve_energy_is_conserved_with_dt2_scaling():
     T, P, N = 300.0, 16, 20
     drift = []
@@ -179,13 +230,14 @@ def test_estimator_identities_on_random_state():
 
 
 @pytest.mark.slow
-def test_harmonic_oscillator_matches_finite_P_closed_form():
+@pytest.mark.parametrize("integ", ["baoab", "obabo"])
+def test_harmonic_oscillator_matches_finite_P_closed_form(integ):
     """north_star pin: 3-D HO at P=32.  The sampled ring-polymer distribution gives exactly
     <K> = <V> = (3 k_B T/2) sum_k w^2/(w^2 + w_k^2) (finite P); the P->inf value
     (3 hbar w/4) coth(beta hbar w/2) is 0.19 % higher at beta hbar w = 4.  K_PR needs the 1/P of
     DESIGN R-6: the printed A7 would give tens of eV."""
     P, T, dt, npart, bhw = 32, 300.0, 0.25e-3, 300, 4.0
-    o, omega, ks = _ho(P, T, dt, 50.0, npart, bhw, seed=2024)
+    o, omega, ks = _ho(P, T, dt, 50.0, npart, bhw, seed=2024, integ=integ)
     om = nm.omegas(P, T)
     m = 1.008
     rng = np.random.default_rng(12)
