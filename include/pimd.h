@@ -158,6 +158,15 @@ int64_t pimd_get_launch_count(const pimd_ctx* ctx);
  * words[n][4], eta[n].  */
 int pimd_debug_noise(pimd_ctx* ctx, int64_t step, int n, const int32_t* idx, uint32_t* words, double* eta);
 
+/* Trotter splitting of the step ("integrator"): PIMD_BAOAB (default here; north_star's path) or
+ * PIMD_OBABO (the fix's own default): O(dt/2) B(dt/2) A(dt) B(dt/2) O(dt/2), each O with c1 = exp(-gamma_k dt/2)
+ * and its own normals (bit 31 of Philox counter word 1 marks the second half-step; DESIGN R-3, R-10).  Both run
+ * in the same fused kernel, one launch per step.  Returns PIMD_EINVAL for an unknown kind.  May be changed
+ * between pimd_step calls. */
+#define PIMD_BAOAB 0
+#define PIMD_OBABO 1
+int pimd_set_integrator(pimd_ctx* ctx, int kind);
+
 /* Fitting-net GEMM path: 1 (default) = tcgen05 tensor cores, 3xTF32 split (fitting_tc.cu); 0 = the FP32
  * CUDA-core GEMMs kept as the in-tree reference for bisecting.  Both meet the parity tolerances. */
 int pimd_set_fitting_path(pimd_ctx* ctx, int use_tensor_cores);

@@ -68,6 +68,7 @@ _SIGNATURES = {
     "pimd_get_neighbor_counts": (C.c_int, [C.c_void_p, C.c_void_p]),
     "pimd_get_launch_count": (C.c_int64, [C.c_void_p]),
     "pimd_set_fitting_path": (C.c_int, [C.c_void_p, C.c_int]),
+    "pimd_set_integrator": (C.c_int, [C.c_void_p, C.c_int]),
     "pimd_set_embedding_path": (C.c_int, [C.c_void_p, C.c_int]),
     "pimd_debug_gemm": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]),
     "pimd_model_n_weights": (C.c_size_t, [C.c_void_p]),
@@ -179,6 +180,16 @@ def pimd_get_neighbor_counts(ctx, P, N, n_types):
 
 def pimd_get_launch_count(ctx):
     return int(lib().pimd_get_launch_count(ctx))
+
+
+PIMD_BAOAB, PIMD_OBABO = 0, 1
+
+
+def pimd_set_integrator(ctx, kind):
+    """kind: PIMD_BAOAB / PIMD_OBABO or the strings "baoab" / "obabo"."""
+    if isinstance(kind, str):
+        kind = {"baoab": PIMD_BAOAB, "obabo": PIMD_OBABO}[kind.lower()]
+    return _check(ctx, lib().pimd_set_integrator(ctx, int(kind)))
 
 
 def pimd_set_fitting_path(ctx, use_tensor_cores):
@@ -309,9 +320,11 @@ class PIMD:
     """Convenience owner of one context (create .. destroy) with the shapes remembered."""
 
     def __init__(self, types, masses, box, n_beads, T, dt, gamma_centroid, seed, model_desc=None,
-                 torch_workspace=True):
+                 torch_workspace=True, integrator="baoab"):
         self.N, self.P = int(np.asarray(types).size), int(n_beads)
         self.ctx = pimd_create(types, masses, box, n_beads, T, dt, gamma_centroid, seed)
+        if integrator != "baoab":
+            pimd_set_integrator(self.ctx, integrator)
         self.desc = ModelDesc.from_dict(model_desc) if isinstance(model_desc, dict) else model_desc
         self._ws = None
         if torch_workspace:

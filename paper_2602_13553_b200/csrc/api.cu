@@ -16,6 +16,7 @@ struct pimd_ctx {
     uint64_t seed = 0;
     int64_t step = 0;
     int64_t launches = 0;
+    int integrator = PIMD_BAOAB;
     std::vector<int32_t> types;
     std::vector<double> masses;
     std::string err;
@@ -132,7 +133,10 @@ size_t model_bytes(const pimd_ctx* c, const pimd_model_desc* d) {
 void mode_constants(pimd_ctx* c) {
     const int P = c->P;
     const double wP = P * kKB * c->T / kHbar;              // Eq. 2
-    const double h = 0.5 * c->dt;
+    // BAOAB: A(dt/2) twice, O(dt) once; OBABO: A(dt) once, O(dt/2) twice (R-3)
+    const bool obabo = c->integrator == PIMD_OBABO;
+    const double h = obabo ? c->dt : 0.5 * c->dt;
+    const double ho = obabo ? 0.5 * c->dt : c->dt;
     for (int k = 0; k < kMaxBeads; ++k) {
         c->mc.cosA[k] = 1; c->mc.sinA_w[k] = h; c->mc.msinA_w[k] = 0; c->mc.c1[k] = 1; c->mc.c2[k] = 0; c->mc.om2[k] = 0;
     }
@@ -147,7 +151,7 @@ void mode_constants(pimd_ctx* c) {
             c->mc.msinA_w[k] = -w * std::sin(w * h);
         }
         const double gam = (k == 0) ? c->gamma0 : 2.0 * w;  // Eq. D1; tau_0 = 1/gamma0 (L174)
-        c->mc.c1[k] = std::exp(-c->dt * gam);               // full dt: BAOAB has one O (R-3)
+        c->mc.c1[k] = std::exp(-ho * gam);
         c->mc.c2[k] = std::sqrt(1.0 - c->mc.c1[k] * c->mc.c1[k]);
     }
 }
@@ -221,6 +225,8 @@ void fill_integrator_args(pimd_ctx* ctx, IntegratorArgs& a, int flags, int64_t s
     a.PkT_mvv = ctx->P * kKB * ctx->T / kMvv2e;
     a.seed_lo = (uint32_t)ctx->seed; a.seed_hi = (uint32_t)(ctx->seed >> 32);
     a.step_lo = (uint32_t)(uint64_t)step; a.step_hi = (uint32_t)((uint64_t)step >> 32);
+    { const uint64_t cs = (uint64_t)(step - 1); a.cstep_lo = (uint32_t)cs; a.cstep_hi = (uint32_t)(cs >> 32) | 0x80000000u; }
+    if (ctx->integrator == PIMD_OBABO) a.flags |= I_OBABO;
     a.x_in = ctx->x; a.vt_in = ctx->vt; a.f = ctx->f; a.x_out = ctx->x; a.vt_out = ctx->vt;
     a.mass = ctx->mass_atom; a.U = ctx->U; a.est = est_slot;
 }
@@ -393,6 +399,14 @@ int pimd_get_neighbor_counts(pimd_ctx* ctx, int32_t* counts) {
 }
 
 int64_t pimd_get_launch_count(const pimd_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int pimd_set_integrator(pimd_ctx* ctx, int kind) {
+    if (!ctx) return PIMD_EINVAL;
+    if (kind != PIMD_BAOAB && kind != PIMD_OBABO) return fail(ctx, PIMD_EINVAL, "unknown integrator kind");
+    ctx->integrator = kind;
+    mode_constants(ctx);
+    return PIMD_OK;
+}
 
 int pimd_set_model_harmonic(pimd_ctx* ctx, double k_spring) {
     if (!ctx) return PIMD_EINVAL;

@@ -22,7 +22,7 @@ constexpr int kEstCap   = 4096;     // estimator history slots per pimd_step cal
 constexpr int kEstWidth = 4;        // K_ring, S_ring, sum x.f - x~0.f~0, U_sum
 
 // integrator launch flags
-enum : int { I_BCLOSE = 1, I_EST = 2, I_START = 4 };
+enum : int { I_BCLOSE = 1, I_EST = 2, I_START = 4, I_OBABO = 8 };
 
 // Per-mode constants of the A and O steps (DESIGN R-3, R-5), kernel parameter.
 struct ModeConsts {
@@ -41,7 +41,8 @@ struct IntegratorArgs {
     int      thermostat;         // 0 = NVE (O step skipped)
     double   half_dt_mvv;        // (dt/2)/mvv2e : multiply by f~/m to get the B kick
     double   PkT_mvv;            // P k_B T / mvv2e : sigma_i^2 = this / m_i
-    uint32_t seed_lo, seed_hi, step_lo, step_hi;
+    uint32_t seed_lo, seed_hi, step_lo, step_hi;   // step = the step this launch OPENS
+    uint32_t cstep_lo, cstep_hi;                   // OBABO: the step this launch CLOSES, bit 31 of word 1 set (second O)
     const double* x_in;  const double* vt_in;  const double* f;
     double*  x_out;      double* vt_out;
     const double* mass;          // [N] per atom

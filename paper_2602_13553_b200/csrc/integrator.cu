@@ -102,7 +102,7 @@ __device__ __forceinline__ void nm_inverse(double* a) {
 
 constexpr int kIntThreads = 128;
 
-template <int P>
+template <int P, bool kObabo>
 __global__ void __launch_bounds__(kIntThreads)
 integrator_kernel(const __grid_constant__ IntegratorArgs a, const __grid_constant__ ModeConsts mc) {
     // dynamic smem: f, x and v~ tiles [P][kIntThreads], staged with cp.async in that order (all 3P loads of
@@ -138,15 +138,23 @@ integrator_kernel(const __grid_constant__ IntegratorArgs a, const __grid_constan
 #pragma unroll
     for (int k = 0; k < P; ++k) ft[k] = fs[k * kIntThreads];
 
-    // ---- O-step normals while x and v~ are still in flight: one draw per mode pair (R-10) ----
-    if (thermo) {
+    // ---- O-step normals while x and v~ are still in flight: one draw per mode pair (R-10).  BAOAB: the O of
+    //      the step this launch opens; OBABO: first the closing O(dt/2) of the previous step (its second half-step
+    //      stream), the opening O's normals are generated between the two mode loops below ----
+    auto gen_normals = [&](uint32_t s_lo, uint32_t s_hi) {
 #pragma unroll 4
         for (int q = 0; q < (P + 1) / 2; ++q) {
             double ee, eo;
-            philox_normal_pair(a.seed_lo, a.seed_hi, a.step_lo, a.step_hi, (uint32_t)i, (uint32_t)(4 * q + alpha), &ee, &eo);
+            philox_normal_pair(a.seed_lo, a.seed_hi, s_lo, s_hi, (uint32_t)i, (uint32_t)(4 * q + alpha), &ee, &eo);
             eta_s[(2 * q) * kIntThreads] = ee;
             if (2 * q + 1 < P) eta_s[(2 * q + 1) * kIntThreads] = eo;
         }
+    };
+    const bool thermo_close = kObabo && a.thermostat && (a.flags & I_BCLOSE);
+    if (kObabo) {
+        if (thermo_close) gen_normals(a.cstep_lo, a.cstep_hi);
+    } else if (thermo) {
+        gen_normals(a.step_lo, a.step_hi);
     }
 
     __pipeline_wait_prior(1);
@@ -164,24 +172,55 @@ integrator_kernel(const __grid_constant__ IntegratorArgs a, const __grid_constan
     // A9 in normal-mode form: sum_k (r_k - r_c).F_k = sum_{k>=1} x~_k f~_k = sum_j x_j f_j - x~_0 f~_0
     const double cv_term = xf - xt[0] * ft[0];
     double accK = 0.0, accS = 0.0;
+    if constexpr (!kObabo) {
 #pragma unroll
-    for (int k = 0; k < P; ++k) {
-        double v = vs[k * kIntThreads];
-        if (a.flags & I_BCLOSE) v += kick * ft[k];      // closing B of the previous step
-        if (a.flags & I_EST) {
-            accK += v * v;                               // A1: 1/2 m v~^2
-            accS += mc.om2[k] * xt[k] * xt[k];           // A3: 1/2 m omega_k^2 x~^2
+        for (int k = 0; k < P; ++k) {
+            double v = vs[k * kIntThreads];
+            if (a.flags & I_BCLOSE) v += kick * ft[k];      // closing B of the previous step
+            if (a.flags & I_EST) {
+                accK += v * v;                               // A1: 1/2 m v~^2
+                accS += mc.om2[k] * xt[k] * xt[k];           // A3: 1/2 m omega_k^2 x~^2
+            }
+            if (start) {
+                v += kick * ft[k];                           // B(dt/2)
+                const double x = xt[k];
+                const double xn = mc.cosA[k] * x + mc.sinA_w[k] * v;    // A(dt/2): exact rotation (R-5)
+                double vn = mc.msinA_w[k] * x + mc.cosA[k] * v;
+                if (thermo) vn = mc.c1[k] * vn + mc.c2[k] * sigma * eta_s[k * kIntThreads];   // O(dt)
+                xt[k] = mc.cosA[k] * xn + mc.sinA_w[k] * vn;            // A(dt/2)
+                v = mc.msinA_w[k] * xn + mc.cosA[k] * vn;
+            }
+            if (live && (a.flags & (I_BCLOSE | I_START))) a.vt_out[k * stride + ec] = v;
         }
-        if (start) {
-            v += kick * ft[k];                           // B(dt/2)
-            const double x = xt[k];
-            const double xn = mc.cosA[k] * x + mc.sinA_w[k] * v;    // A(dt/2): exact rotation (R-5)
-            double vn = mc.msinA_w[k] * x + mc.cosA[k] * v;
-            if (thermo) vn = mc.c1[k] * vn + mc.c2[k] * sigma * eta_s[k * kIntThreads];   // O(dt)
-            xt[k] = mc.cosA[k] * xn + mc.sinA_w[k] * vn;            // A(dt/2)
-            v = mc.msinA_w[k] * xn + mc.cosA[k] * vn;
+    } else {
+        // OBABO: close the previous step with B(dt/2) O(dt/2), then estimators ...
+#pragma unroll
+        for (int k = 0; k < P; ++k) {
+            double v = vs[k * kIntThreads];
+            if (a.flags & I_BCLOSE) {
+                v += kick * ft[k];
+                if (thermo_close) v = mc.c1[k] * v + mc.c2[k] * sigma * eta_s[k * kIntThreads];
+            }
+            if (a.flags & I_EST) {
+                accK += v * v;
+                accS += mc.om2[k] * xt[k] * xt[k];
+            }
+            vs[k * kIntThreads] = v;
         }
-        if (live && (a.flags & (I_BCLOSE | I_START))) a.vt_out[k * stride + ec] = v;
+        // ... and open the next one with O(dt/2) B(dt/2) A(dt) (mc holds cos/sin for dt and c1, c2 for dt/2)
+        if (thermo) gen_normals(a.step_lo, a.step_hi);
+#pragma unroll
+        for (int k = 0; k < P; ++k) {
+            double v = vs[k * kIntThreads];
+            if (start) {
+                if (thermo) v = mc.c1[k] * v + mc.c2[k] * sigma * eta_s[k * kIntThreads];
+                v += kick * ft[k];
+                const double x = xt[k];
+                xt[k] = mc.cosA[k] * x + mc.sinA_w[k] * v;
+                v = mc.msinA_w[k] * x + mc.cosA[k] * v;
+            }
+            if (live && (a.flags & (I_BCLOSE | I_START))) a.vt_out[k * stride + ec] = v;
+        }
     }
 
     if (a.flags & I_EST) {
@@ -226,10 +265,12 @@ static void launch_int_t(const IntegratorArgs& a, const ModeConsts& mc, cudaStre
     const size_t smem = (size_t)3 * P * kIntThreads * sizeof(double);
     static bool attr_done = false;
     if (!attr_done) {
-        cudaFuncSetAttribute(integrator_kernel<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaFuncSetAttribute(integrator_kernel<P, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaFuncSetAttribute(integrator_kernel<P, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         attr_done = true;
     }
-    integrator_kernel<P><<<blocks, kIntThreads, smem, s>>>(a, mc);
+    if (a.flags & I_OBABO) integrator_kernel<P, true><<<blocks, kIntThreads, smem, s>>>(a, mc);
+    else integrator_kernel<P, false><<<blocks, kIntThreads, smem, s>>>(a, mc);
 }
 
 int launch_integrator(int P, const IntegratorArgs& a, const ModeConsts& mc, cudaStream_t s) {

@@ -87,6 +87,65 @@ def test_integrator_parity_harmonic(pk, P, gamma):
     sim.close()
 
 
+@pytest.mark.parametrize("P", [1, 4, 32, 64])
+@pytest.mark.parametrize("gamma", [0.0, 5.0])
+def test_integrator_parity_harmonic_obabo(pk, P, gamma):
+    """OBABO splitting in the same fused kernel: two half-step O's per
+    launch, each with its own Philox stream; also split calls and a switch of the splitting mid-run."""
+    N = 37
+    types, masses, x, p = _random_system(N, P, seed=20 + P)
+    ks = 2.5
+    sim = pk.PIMD(types, masses, [30.0] * 3, P, 300.0, 0.25e-3, gamma, seed=99, integrator="obabo")
+    sim.set_state(x, p)
+    sim.set_model_harmonic(ks)
+    orc = OraclePIMD(types, masses, [30.0] * 3, P, 300.0, 0.25e-3, gamma, seed=99, integrator="obabo")
+    orc.set_state(x, p)
+    orc.set_model_harmonic(ks)
+    sim.step(1)
+    orc.step(1)
+    assert _rel(sim.positions(), orc.positions()) < 1e-10
+    assert _rel(sim.momenta(), orc.momenta()) < 1e-10
+    sim.step(4)
+    sim.step(5)
+    orc.step(9)
+    assert _rel(sim.positions(), orc.positions()) < 1e-11
+    assert _rel(sim.momenta(), orc.momenta()) < 1e-10
+    e, o = sim.estimators(), orc.estimators()
+    assert e["step"] == 10
+    for key in ("K_PR", "K_CV", "H", "K_ring", "S_ring", "U_sum", "T_ring"):
+        assert abs(e[key] - o[key]) <= 1e-9 * max(1.0, abs(o[key])), key
+    # back to BAOAB for two steps: the oracle follows
+    pk.pimd_set_integrator(sim.ctx, "baoab")
+    orc.integrator = "baoab"
+    sim.step(2)
+    orc.step(2)
+    assert _rel(sim.positions(), orc.positions()) < 1e-11
+    assert _rel(sim.momenta(), orc.momenta()) < 1e-10
+    with pytest.raises(pk.PimdError):
+        pk.pimd_set_integrator(sim.ctx, 7)
+    sim.close()
+
+
+def test_full_step_parity_config0_obabo(pk):
+    cfg, wb, desc, w = workloads.make_config(0)
+    args = (wb["types"], wb["masses"], wb["box"], cfg["P"], cfg["T"], cfg["dt"], cfg["gamma"])
+    sim = pk.PIMD(*args, seed=11, model_desc=desc, integrator="obabo")
+    sim.set_state(wb["x"], wb["p"])
+    sim.set_model(w)
+    orc = OraclePIMD(*args, seed=11, integrator="obabo")
+    orc.set_state(wb["x"], wb["p"])
+    orc.set_model(desc, w)
+    sim.step(1)
+    orc.step(1)
+    ex1, ep1 = _rel(sim.positions(), orc.positions()), _rel(sim.momenta(), orc.momenta())
+    assert ex1 <= 1e-10 and ep1 <= 1e-10, (ex1, ep1)
+    sim.step(4)
+    orc.step(4)
+    ex, ep = _rel(sim.positions(), orc.positions()), _rel(sim.momenta(), orc.momenta())
+    assert ex <= 1e-6 and ep <= 1e-6, (ex, ep)
+    sim.close()
+
+
 def test_estimator_history_every_step(pk):
     N, P = 50, 8
     types, masses, x, p = _random_system(N, P, seed=5)
