@@ -108,6 +108,16 @@ def obabo_finish(vt, f, masses, M, om, T, gamma0, dt, seed, step):
     return vt, ft
 
 
+def remove_centroid_com(vt, masses):
+    """`fixcom yes`: "the center-of-mass velocity is removed in every timestep for the
+    centroid mode" (nmpimd).  v~_0,i <- v~_0,i - sum_j m_j v~_0,j / sum_j m_j, per Cartesian component;
+    applied once per step after its last velocity update (DESIGN R-19: the paper does not say where)."""
+    out = vt.copy()
+    vcom = np.sum(masses[:, None] * vt[0], axis=0) / np.sum(masses)
+    out[0] = vt[0] - vcom[None, :]
+    return out
+
+
 def estimators(x, vt, f, U, masses, M, om, T):
     """Appendix A outputs that the hot path reports, on unwrapped coordinates
     (L202).  x, f Cartesian [P,N,3]; vt normal-mode velocities; U[P] bead potential energies.

@@ -13,7 +13,7 @@ from . import nm, integrator, se_e2_a
 
 
 class OraclePIMD:
-    def __init__(self, types, masses_per_type, box, n_beads, T, dt, gamma_centroid, seed, integrator="baoab"):
+    def __init__(self, types, masses_per_type, box, n_beads, T, dt, gamma_centroid, seed, integrator="baoab", fixcom=False):
         self.types = np.asarray(types, dtype=np.int64)
         self.N = self.types.size
         self.masses = np.asarray(masses_per_type, dtype=np.float64)[self.types]   # per atom
@@ -25,6 +25,7 @@ class OraclePIMD:
         self.seed = int(seed)
         assert integrator in ("baoab", "obabo")
         self.integrator = integrator
+        self.fixcom = bool(fixcom)
         self.M = nm.nm_matrix(self.P)
         self.om = nm.omegas(self.P, self.T)
         self.step_count = 0
@@ -85,6 +86,8 @@ class OraclePIMD:
                 self._forces()
                 self.vt, _ = integrator.obabo_finish(self.vt, self.f, self.masses, self.M, self.om, self.T,
                                                      self.gamma0, self.dt, self.seed, self.step_count)
+                if self.fixcom:
+                    self.vt = integrator.remove_centroid_com(self.vt, self.masses)
                 self.step_count += 1
                 continue
             self.x, self.vt = integrator.baoab_positions_half(
@@ -92,6 +95,8 @@ class OraclePIMD:
                 self.dt, self.seed, self.step_count)
             self._forces()                                   # one force evaluation per step
             self.vt, _ = integrator.baoab_finish(self.vt, self.f, self.masses, self.M, self.dt)
+            if self.fixcom:
+                self.vt = integrator.remove_centroid_com(self.vt, self.masses)
             self.step_count += 1
 
     # ---- outputs ----

@@ -189,6 +189,38 @@ def test_obabo_equals_baoab_without_thermostat_and_composes_the_o_steps():
     assert np.abs(c1h * c1h - c1f).max() < 1e-15
 
 
+@pytest.mark.parametrize("integ", ["baoab", "obabo"])
+def test_fixcom_removes_exactly_the_centroid_momentum(integ):
+    """fixcom: after every step the total momentum of the centroid mode vanishes, the
+    relative velocities and all other modes are untouched, and a second removal is a no-op."""
+    P, T, dt, N = 4, 300.0, 0.5e-3, 7
+    rng = np.random.default_rng(9)
+    masses_t = [15.9994, 1.008]
+    types = rng.integers(0, 2, N)
+    o = OraclePIMD(types, masses_t, [50.0] * 3, P, T, dt, 5.0, 3, integrator=integ, fixcom=True)
+    ref = OraclePIMD(types, masses_t, [50.0] * 3, P, T, dt, 5.0, 3, integrator=integ, fixcom=False)
+    x0, p0 = 0.1 * rng.standard_normal((P, N, 3)), 20 * rng.standard_normal((P, N, 3))
+    for sim in (o, ref):
+        sim.set_model_harmonic(1.5)
+        sim.set_state(x0, p0)
+        sim.step(1)
+    m = o.masses
+    pc = np.sum(m[:, None] * o.vt[0], axis=0)
+    assert np.abs(pc).max() < 1e-12 * np.abs(m[:, None] * o.vt[0]).max()
+    # one step: identical except for a uniform shift of the centroid velocities
+    shift = ref.vt[0] - o.vt[0]
+    assert np.abs(shift - shift[0]).max() < 1e-12 * np.abs(ref.vt[0]).max()
+    assert np.abs(shift[0] - np.sum(m[:, None] * ref.vt[0], axis=0) / m.sum()).max() < 1e-12 * np.abs(ref.vt[0]).max()
+    assert np.array_equal(o.vt[1:], ref.vt[1:]) and np.array_equal(o.x, ref.x)
+    again = integrator.remove_centroid_com(o.vt, m)
+    assert np.abs(again - o.vt).max() < 1e-13 * np.abs(o.vt).max()
+    # Cartesian view: sum over beads and atoms of the bead momenta is sqrt(P) times the centroid-mode momentum
+    ptot = o.momenta().sum(axis=(0, 1))
+    assert np.abs(ptot).max() < 1e-11 * np.abs(o.momenta()).max()
+    o.step(5)
+    assert np.abs(np.sum(m[:, None] * o.vt[0], axis=0)).max() < 1e-12 * np.abs(m[:, None] * o.vt[0]).max()
+
+
 def test_nve_energy_is_conserved_with_dt2_scaling():
     T, P, N = 300.0, 16, 20
     drift = []
