@@ -167,6 +167,12 @@ int pimd_debug_noise(pimd_ctx* ctx, int64_t step, int n, const int32_t* idx, uin
 #define PIMD_OBABO 1
 int pimd_set_integrator(pimd_ctx* ctx, int kind);
 
+/* `fixcom`: when on, the centre-of-mass velocity of the centroid mode is removed once per step,
+ * after the step's last velocity update and before its estimators (DESIGN R-19).  Off by default (north_star's
+ * create() list has no such argument).  The removal needs a reduction over all atoms between the closing and the
+ * opening half of the fused integrator launch, so a step then costs two integrator launches instead of one. */
+int pimd_set_fixcom(pimd_ctx* ctx, int on);
+
 /* Fitting-net GEMM path: 1 (default) = tcgen05 tensor cores, 3xTF32 split (fitting_tc.cu); 0 = the FP32
  * CUDA-core GEMMs kept as the in-tree reference for bisecting.  Both meet the parity tolerances. */
 int pimd_set_fitting_path(pimd_ctx* ctx, int use_tensor_cores);

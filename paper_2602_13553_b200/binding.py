@@ -69,6 +69,7 @@ _SIGNATURES = {
     "pimd_get_launch_count": (C.c_int64, [C.c_void_p]),
     "pimd_set_fitting_path": (C.c_int, [C.c_void_p, C.c_int]),
     "pimd_set_integrator": (C.c_int, [C.c_void_p, C.c_int]),
+    "pimd_set_fixcom": (C.c_int, [C.c_void_p, C.c_int]),
     "pimd_set_embedding_path": (C.c_int, [C.c_void_p, C.c_int]),
     "pimd_debug_gemm": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]),
     "pimd_model_n_weights": (C.c_size_t, [C.c_void_p]),
@@ -190,6 +191,10 @@ def pimd_set_integrator(ctx, kind):
     if isinstance(kind, str):
         kind = {"baoab": PIMD_BAOAB, "obabo": PIMD_OBABO}[kind.lower()]
     return _check(ctx, lib().pimd_set_integrator(ctx, int(kind)))
+
+
+def pimd_set_fixcom(ctx, on):
+    return _check(ctx, lib().pimd_set_fixcom(ctx, int(bool(on))))
 
 
 def pimd_set_fitting_path(ctx, use_tensor_cores):
@@ -320,11 +325,13 @@ class PIMD:
     """Convenience owner of one context (create .. destroy) with the shapes remembered."""
 
     def __init__(self, types, masses, box, n_beads, T, dt, gamma_centroid, seed, model_desc=None,
-                 torch_workspace=True, integrator="baoab"):
+                 torch_workspace=True, integrator="baoab", fixcom=False):
         self.N, self.P = int(np.asarray(types).size), int(n_beads)
         self.ctx = pimd_create(types, masses, box, n_beads, T, dt, gamma_centroid, seed)
         if integrator != "baoab":
             pimd_set_integrator(self.ctx, integrator)
+        if fixcom:
+            pimd_set_fixcom(self.ctx, True)
         self.desc = ModelDesc.from_dict(model_desc) if isinstance(model_desc, dict) else model_desc
         self._ws = None
         if torch_workspace:

@@ -17,6 +17,9 @@ struct pimd_ctx {
     int64_t step = 0;
     int64_t launches = 0;
     int integrator = PIMD_BAOAB;
+    bool fixcom = false;
+    double* com = nullptr;        // [3] device: centroid COM momentum (fixcom)
+    double inv_mtot = 0;
     std::vector<int32_t> types;
     std::vector<double> masses;
     std::string err;
@@ -87,7 +90,7 @@ size_t base_bytes(const pimd_ctx* c) {
     b += align_up((size_t)c->N * 8, 256) + align_up((size_t)c->N * 4, 256);
     b += align_up((size_t)c->P * 8, 256) + align_up((size_t)c->P * 72, 256) + align_up((size_t)c->P * c->N * 8, 256);
     b += align_up((size_t)(kEstCap + 2) * kEstWidth * 8, 256);
-    return b + 4096;
+    return b + 4096 + 256;
 }
 
 void cell_grid(const double box[3], double rcut, int ncell[3], int R[3], int* ncells) {
@@ -171,8 +174,11 @@ int alloc_base(pimd_ctx* ctx) {
     if ((rc = arena_alloc(ctx, &ctx->Xi, (size_t)ctx->P * 9))) return rc;
     if ((rc = arena_alloc(ctx, &ctx->Eatom, (size_t)ctx->P * ctx->N))) return rc;
     if ((rc = arena_alloc(ctx, &ctx->est, (size_t)(kEstCap + 2) * kEstWidth))) return rc;
+    if ((rc = arena_alloc(ctx, &ctx->com, (size_t)4))) return rc;
     std::vector<double> ma(ctx->N);
-    for (int i = 0; i < ctx->N; ++i) ma[i] = ctx->masses[ctx->types[i]];
+    double mtot = 0;
+    for (int i = 0; i < ctx->N; ++i) { ma[i] = ctx->masses[ctx->types[i]]; mtot += ma[i]; }
+    ctx->inv_mtot = 1.0 / mtot;
     CK(cudaMemcpyAsync(ctx->mass_atom, ma.data(), sizeof(double) * ctx->N, cudaMemcpyHostToDevice, ctx->stream));
     CK(cudaMemcpyAsync(ctx->types_d, ctx->types.data(), sizeof(int) * ctx->N, cudaMemcpyHostToDevice, ctx->stream));
     CK(cudaMemsetAsync(ctx->f, 0, PN3 * 8, ctx->stream));
@@ -229,6 +235,7 @@ void fill_integrator_args(pimd_ctx* ctx, IntegratorArgs& a, int flags, int64_t s
     if (ctx->integrator == PIMD_OBABO) a.flags |= I_OBABO;
     a.x_in = ctx->x; a.vt_in = ctx->vt; a.f = ctx->f; a.x_out = ctx->x; a.vt_out = ctx->vt;
     a.mass = ctx->mass_atom; a.U = ctx->U; a.est = est_slot;
+    a.com = ctx->com; a.inv_mtot = ctx->inv_mtot;
 }
 
 int check_overflow(pimd_ctx* ctx) {
@@ -399,6 +406,12 @@ int pimd_get_neighbor_counts(pimd_ctx* ctx, int32_t* counts) {
 }
 
 int64_t pimd_get_launch_count(const pimd_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int pimd_set_fixcom(pimd_ctx* ctx, int on) {
+    if (!ctx) return PIMD_EINVAL;
+    ctx->fixcom = on != 0;
+    return PIMD_OK;
+}
 
 int pimd_set_integrator(pimd_ctx* ctx, int kind) {
     if (!ctx) return PIMD_EINVAL;
@@ -586,8 +599,16 @@ int pimd_step(pimd_ctx* ctx, int64_t n_steps) {
         }
         if (s < n_steps) flags |= I_START;
         IntegratorArgs a;
-        fill_integrator_args(ctx, a, flags, ctx->step + s, slot);
         rec(ctx, 0);
+        if (ctx->fixcom && s > 0) {
+            // fixcom (R-19): the removal needs sum_i m_i v~_0,i over ALL atoms after the closing half,
+            // so the launch splits: close + accumulate, then subtract + estimators (+ open)
+            cudaMemsetAsync(ctx->com, 0, sizeof(double) * 3, ctx->stream);
+            fill_integrator_args(ctx, a, I_BCLOSE | I_COMACC, ctx->step + s, scratch);
+            ctx->launches += launch_integrator(ctx->P, a, ctx->mc, ctx->stream);
+            flags = (flags & ~I_BCLOSE) | I_COMSUB;
+        }
+        fill_integrator_args(ctx, a, flags, ctx->step + s, slot);
         ctx->launches += launch_integrator(ctx->P, a, ctx->mc, ctx->stream);
         if (s < n_steps) {
             int rc = eval_forces(ctx);

@@ -22,7 +22,7 @@ constexpr int kEstCap   = 4096;     // estimator history slots per pimd_step cal
 constexpr int kEstWidth = 4;        // K_ring, S_ring, sum x.f - x~0.f~0, U_sum
 
 // integrator launch flags
-enum : int { I_BCLOSE = 1, I_EST = 2, I_START = 4, I_OBABO = 8 };
+enum : int { I_BCLOSE = 1, I_EST = 2, I_START = 4, I_OBABO = 8, I_COMACC = 16, I_COMSUB = 32 };
 
 // Per-mode constants of the A and O steps (DESIGN R-3, R-5), kernel parameter.
 struct ModeConsts {
@@ -48,6 +48,8 @@ struct IntegratorArgs {
     const double* mass;          // [N] per atom
     const double* U;             // [P] bead energies (for the U_sum slot), may be null
     double*  est;                // [kEstWidth] accumulators of this step's slot, may be null
+    double*  com;                // [3] fixcom: sum_i m_i v~_0,i per component (I_COMACC adds, I_COMSUB reads)
+    double   inv_mtot;           // 1 / sum_i m_i
 };
 
 int launch_integrator(int P, const IntegratorArgs& a, const ModeConsts& mc, cudaStream_t s);

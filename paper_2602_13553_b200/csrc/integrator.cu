@@ -166,17 +166,19 @@ integrator_kernel(const __grid_constant__ IntegratorArgs a, const __grid_constan
     nm_forward<P>(ft);                                  // f~ = M f      (L192, third transform)
     nm_forward<P>(xt);                                  // x~ = M x      (first transform)
     __pipeline_wait_prior(0);
+    if (a.flags & I_COMSUB) vs[0] -= a.com[alpha] * a.inv_mtot;     // fixcom (L180, R-19): centroid COM velocity
 
     const double kick = a.half_dt_mvv / m;              // (dt/2)/(m mvv2e)
     const double sigma = sqrt(a.PkT_mvv / m);           // sqrt(P k_B T/(m mvv2e))  (Eq. D2)
     // A9 in normal-mode form: sum_k (r_k - r_c).F_k = sum_{k>=1} x~_k f~_k = sum_j x_j f_j - x~_0 f~_0
     const double cv_term = xf - xt[0] * ft[0];
-    double accK = 0.0, accS = 0.0;
+    double accK = 0.0, accS = 0.0, v0c = 0.0;
     if constexpr (!kObabo) {
 #pragma unroll
         for (int k = 0; k < P; ++k) {
             double v = vs[k * kIntThreads];
             if (a.flags & I_BCLOSE) v += kick * ft[k];      // closing B of the previous step
+            if (k == 0) v0c = v;
             if (a.flags & I_EST) {
                 accK += v * v;                               // A1: 1/2 m v~^2
                 accS += mc.om2[k] * xt[k] * xt[k];           // A3: 1/2 m omega_k^2 x~^2
@@ -190,7 +192,7 @@ integrator_kernel(const __grid_constant__ IntegratorArgs a, const __grid_constan
                 xt[k] = mc.cosA[k] * xn + mc.sinA_w[k] * vn;            // A(dt/2)
                 v = mc.msinA_w[k] * xn + mc.cosA[k] * vn;
             }
-            if (live && (a.flags & (I_BCLOSE | I_START))) a.vt_out[k * stride + ec] = v;
+            if (live && (a.flags & (I_BCLOSE | I_START | I_COMSUB))) a.vt_out[k * stride + ec] = v;
         }
     } else {
         // OBABO: close the previous step with B(dt/2) O(dt/2), then estimators ...
@@ -201,6 +203,7 @@ integrator_kernel(const __grid_constant__ IntegratorArgs a, const __grid_constan
                 v += kick * ft[k];
                 if (thermo_close) v = mc.c1[k] * v + mc.c2[k] * sigma * eta_s[k * kIntThreads];
             }
+            if (k == 0) v0c = v;
             if (a.flags & I_EST) {
                 accK += v * v;
                 accS += mc.om2[k] * xt[k] * xt[k];
@@ -219,8 +222,21 @@ integrator_kernel(const __grid_constant__ IntegratorArgs a, const __grid_constan
                 xt[k] = mc.cosA[k] * x + mc.sinA_w[k] * v;
                 v = mc.msinA_w[k] * x + mc.cosA[k] * v;
             }
-            if (live && (a.flags & (I_BCLOSE | I_START))) a.vt_out[k * stride + ec] = v;
+            if (live && (a.flags & (I_BCLOSE | I_START | I_COMSUB))) a.vt_out[k * stride + ec] = v;
         }
+    }
+
+    if (a.flags & I_COMACC) {                                // fixcom: sum_i m_i v~_0,i per component
+        double c3[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) c3[c] = (live && alpha == c) ? m * v0c : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) c3[c] += __shfl_xor_sync(0xffffffffu, c3[c], o);
+        if ((threadIdx.x & 31) == 0)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) atomicAdd(a.com + c, c3[c]);
     }
 
     if (a.flags & I_EST) {

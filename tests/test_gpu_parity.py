@@ -126,6 +126,40 @@ def test_integrator_parity_harmonic_obabo(pk, P, gamma):
     sim.close()
 
 
+@pytest.mark.parametrize("integ", ["baoab", "obabo"])
+@pytest.mark.parametrize("P", [1, 8, 32])
+def test_fixcom_parity_and_zero_centroid_momentum(pk, integ, P):
+    """fixcom (DESIGN R-19): two integrator launches per step (close + accumulate, subtract +
+    estimators + open); trajectories follow the oracle and the total bead momentum vanishes after every step."""
+    N = 301                                          # several 128-thread blocks and a ragged tail
+    types, masses, x, p = _random_system(N, P, seed=40 + P)
+    ks = 2.5
+    args = (types, masses, [30.0] * 3, P, 300.0, 0.25e-3, 5.0)
+    sim = pk.PIMD(*args, seed=7, integrator=integ, fixcom=True)
+    sim.set_state(x, p)
+    sim.set_model_harmonic(ks)
+    orc = OraclePIMD(*args, seed=7, integrator=integ, fixcom=True)
+    orc.set_state(x, p)
+    orc.set_model_harmonic(ks)
+    sim.step(1)
+    orc.step(1)
+    assert _rel(sim.positions(), orc.positions()) < 1e-10
+    assert _rel(sim.momenta(), orc.momenta()) < 1e-10
+    ptot = sim.momenta().sum(axis=(0, 1))
+    assert np.abs(ptot).max() < 1e-10 * np.abs(sim.momenta()).max() * N ** 0.5
+    sim.step(3)
+    sim.step(2)
+    orc.step(5)
+    assert _rel(sim.positions(), orc.positions()) < 1e-10
+    assert _rel(sim.momenta(), orc.momenta()) < 1e-9
+    ptot = sim.momenta().sum(axis=(0, 1))
+    assert np.abs(ptot).max() < 1e-10 * np.abs(sim.momenta()).max() * N ** 0.5
+    e, o = sim.estimators(), orc.estimators()
+    for key in ("K_PR", "K_CV", "H", "K_ring", "S_ring", "U_sum", "T_ring"):
+        assert abs(e[key] - o[key]) <= 1e-9 * max(1.0, abs(o[key])), key
+    sim.close()
+
+
 def test_full_step_parity_config0_obabo(pk):
     cfg, wb, desc, w = workloads.make_config(0)
     args = (wb["types"], wb["masses"], wb["box"], cfg["P"], cfg["T"], cfg["dt"], cfg["gamma"])
