@@ -263,6 +263,40 @@ def test_neighbours_atoms_far_outside_the_box_and_on_faces(pk):
     sim.close()
 
 
+def test_isolated_atoms_empty_pair_types_and_single_atom_beads(pk):
+    """Degenerate inputs of the force path: atoms with no neighbour at all (energy = the fitting net at D = 0,
+    zero force), a centre type with no rows of one neighbour type, row tiles that are almost empty, P = 1."""
+    desc = workloads.model_desc()
+    w = workloads.model_weights(desc, 3, last_layer_scale=50.0)
+    model = se_e2_a.Model(desc, w)
+    box = np.array([60.0, 60.0, 60.0])
+    # one water (3 atoms inside r_c of each other), one O-O pair, three isolated atoms (H, H, O)
+    x1 = np.array([[5.0, 5.0, 5.0], [5.9, 5.2, 5.0], [4.8, 5.9, 5.1],
+                   [30.0, 30.0, 30.0], [32.5, 30.0, 30.5],
+                   [50.0, 10.0, 10.0], [10.0, 50.0, 10.0], [10.0, 10.0, 50.0]])
+    types = np.array([0, 1, 1, 0, 0, 1, 1, 0], dtype=np.int32)
+    for P in (1, 4):
+        rng = np.random.default_rng(P)
+        x = x1[None] + 0.01 * rng.standard_normal((P, 8, 3))
+        p = rng.standard_normal((P, 8, 3))
+        sim = pk.PIMD(types, [15.9994, 1.008], box, P, 300.0, 0.5e-3, 1.0, seed=1, model_desc=desc)
+        sim.set_state(x, p)
+        sim.set_model(w)
+        f, U, E = sim.forces(), sim.energies(), sim.atom_energies()
+        for k in range(P):
+            Eo, Fo, Xio = se_e2_a.energy_forces(x[k], types, box, model)
+            assert np.abs(E[k] - Eo).max() <= 1e-6 * 50.0
+            assert abs(U[k] - Eo.sum()) / 8 <= 1e-6 * 50.0
+            scale = max(np.abs(Fo).max(), 1e-30)
+            assert np.abs(f[k] - Fo).max() <= 1e-4 * scale
+            assert np.all(f[k, 5:] == 0.0) and np.all(Fo[5:] == 0.0)          # isolated atoms feel nothing
+        count, j, shift = sim.neighbors(0)
+        assert list(count) == [2, 2, 2, 1, 1, 0, 0, 0]
+        sim.step(2)                                                          # and the step runs on it
+        assert np.all(np.isfinite(sim.positions()))
+        sim.close()
+
+
 def test_sel_overflow_is_an_error(pk):
     cfg, wb, desc, w = workloads.make_config(0)
     small = dict(desc, sel=[8, 16])
