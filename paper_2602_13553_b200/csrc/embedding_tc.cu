@@ -39,7 +39,7 @@ constexpr int H3 = 52;                 // G channels per half
 constexpr int K2 = 32;                 // layer-2 K: half A at k 0..12, bias at 13, half B at 16..28
 constexpr int N2 = 64;                 // layer-2 N: half A at columns 0..25, half B at 32..57
 constexpr int K3 = 56;                 // layer-3 K: half A at k 0..25, bias at 26, half B at 28..53
-constexpr int N3 = 128;                // layer-3 N: half A at columns 0..51, half B at 64..115
+constexpr int N3 = 112;                // layer-3 N: half A at columns 0..51, half B at 56..107
 constexpr int GROW = 108;              // floats per staged G row (104 + pad: conflict-free 16 B stores)
 // weight image of one (t_i, t_j) pair, bytes
 constexpr int oW2hi = 0, oW2lo = N2 * 128;                       // [64][32] f32, 128 B rows, SW128
@@ -71,7 +71,7 @@ constexpr int kBias2 = 13;
 __host__ __device__ constexpr int n2_of(int h, int j) { return 32 * h + j; }       // layer-2 output column
 __host__ __device__ constexpr int k3_of(int h, int j) { return 28 * h + j; }       // layer-3 K index of h2 (h, j)
 constexpr int kBias3 = 26;
-__host__ __device__ constexpr int n3_of(int h, int g) { return 64 * h + g; }       // layer-3 output column
+__host__ __device__ constexpr int n3_of(int h, int g) { return 56 * h + g; }       // layer-3 output column
 }  // namespace etc
 
 struct EmbTcArgs {
@@ -400,10 +400,11 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
             tc_fence_after();
             // ---- epilogue 3: G = [h2,h2] + tanh(z3), my 52 columns -> smem [row][GROW] (overlays the A region) ----
             {
-                const uint32_t col = tmem_d + lanefield + 64 * half;
+                const uint32_t col = tmem_d + lanefield + 56 * half;
                 float* grow = Gs + t * GROW + H3 * half;
                 uint32_t v[32];
-                tmem_ld32(col, v);
+                tmem_ld16(col, v);
+                tmem_ld16(col + 16, v + 16);
                 tmem_ld_wait();
 #pragma unroll
                 for (int q = 0; q < 8; ++q) {
@@ -510,7 +511,7 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
     float* part = reinterpret_cast<float*>(ctx + oPart) + t * 8;
     const float* W1s = reinterpret_cast<const float*>(cs.smem + oW1) + H1 * half;
     const float* b1s = W1s + 32;
-    const uint32_t tmem_v = cs.tmem_base + cx * 256, tmem_g = tmem_v + N3;     // value / derivative accumulators
+    const uint32_t tmem_v = cs.tmem_base + cx * 256, tmem_g = tmem_v + 128;     // value / derivative accumulators
     const uint32_t lanefield = ((uint32_t)((t >> 5) * 32)) << 16;
     const uint32_t actx = smem_u32(ctx), wbase = smem_u32(cs.smem);
     constexpr uint32_t idesc2 = make_idesc_tf32(128, N2), idesc3 = make_idesc_tf32(128, N3);
@@ -691,7 +692,7 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
                         dR2 = fmaf(dT.z, G, dR2); dR3 = fmaf(dT.w, G, dR3);
                     }
                 };
-                const uint32_t cv = tmem_v + lanefield + 64 * half, cd = tmem_g + lanefield + 64 * half;
+                const uint32_t cv = tmem_v + lanefield + 56 * half, cd = tmem_g + lanefield + 56 * half;
                 uint32_t v[16], d[16];
 #pragma unroll
                 for (int cc = 0; cc < 3; ++cc) {
