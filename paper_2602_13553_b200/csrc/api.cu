@@ -313,6 +313,14 @@ int pimd_create(pimd_ctx** out, int n_atoms, const int32_t* types, int n_types, 
 void pimd_destroy(pimd_ctx* ctx) {
     if (!ctx) return;
     cudaStreamSynchronize(ctx->stream);
+    if (ctx->model.aux_stream[0]) {
+        for (int q = 0; q < Model::kChainStreams - 1; ++q) {
+            cudaStreamSynchronize(ctx->model.aux_stream[q]);
+            cudaStreamDestroy(ctx->model.aux_stream[q]);
+            cudaEventDestroy(ctx->model.ev_join[q]);
+        }
+        cudaEventDestroy(ctx->model.ev_fork);
+    }
     for (void* p : ctx->owned) cudaFree(p);
     for (int i = 0; i < 8; ++i)
         if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);

@@ -68,6 +68,9 @@ struct NeighSlotB { float ds, rinv; uint32_t jcode; float pad; };   // jcode = j
 
 struct Model {
     bool     set = false;
+    static constexpr int kChainStreams = 3; // tile ranges of the fitting chain run on this many streams (fitting_tc.cu)
+    cudaStream_t aux_stream[kChainStreams - 1] = {};
+    cudaEvent_t  ev_fork = nullptr, ev_join[kChainStreams - 1] = {};
     pimd_model_desc d;
     int      nsel = 0;
     int      seloff[PIMD_MAX_TYPES + 1];

@@ -32,6 +32,7 @@ struct TcMaps {
 };
 
 struct TcGemmArgs {
+    int tile_off;                   // first M tile of this launch (the chain runs in tile ranges on two streams)
     int ntypes, N, K;               // N = logical columns of C (grid.x chunks of BN)
     int tile0[kMaxT + 1];           // first M tile of each type
     int row0[kMaxT + 1];            // first (type-sorted) row of each type
@@ -73,11 +74,12 @@ gemm3xtf32_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ T
     uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(bars + 3 * ST + 1);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int tile = (int)blockIdx.y + g.tile_off;
     int ty = 0;
 #pragma unroll
     for (int t = 1; t < kMaxT; ++t)
-        if (t < g.ntypes && (int)blockIdx.y >= g.tile0[t]) ty = t;
-    const int m0 = ((int)blockIdx.y - g.tile0[ty]) * (128 * NH), n0 = blockIdx.x * BN;
+        if (t < g.ntypes && tile >= g.tile0[t]) ty = t;
+    const int m0 = (tile - g.tile0[ty]) * (128 * NH), n0 = blockIdx.x * BN;
     const int rows_t = g.row0[ty + 1] - g.row0[ty];
     const int nk = g.K / kTcBK;
     const CUtensorMap* mapA = &maps.A[ty];
@@ -313,6 +315,7 @@ gemm3xtf32_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ T
 // D (rows x 1600, 315 MB at configs[2]) is neither written nor read.  The weights arrive pre-split by TMA.
 // ---------------------------------------------------------------------------------------------
 struct L1Args {
+    int tile_off;
     int ntypes, K;
     int tile0[kMaxT + 1];
     int row0[kMaxT + 1];
@@ -345,11 +348,12 @@ l1_desc_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ L1Ar
     uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(bars + 3 * ST + 1);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int tile = (int)blockIdx.x + g.tile_off;
     int ty = 0;
 #pragma unroll
     for (int t = 1; t < kMaxT; ++t)
-        if (t < g.ntypes && (int)blockIdx.x >= g.tile0[t]) ty = t;
-    const int m0 = ((int)blockIdx.x - g.tile0[ty]) * 128;
+        if (t < g.ntypes && tile >= g.tile0[t]) ty = t;
+    const int m0 = (tile - g.tile0[ty]) * 128;
     const int rows_t = g.row0[ty + 1] - g.row0[ty];
     const int nk = g.K / kTcBK;
     const CUtensorMap* mapBhi = &maps.Bhi[ty];
@@ -472,6 +476,7 @@ l1_desc_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ L1Ar
 // chunks, added to the rows m < 16 at the end (same thread, program order).  T[i][0:16] sits in shared memory.
 // ---------------------------------------------------------------------------------------------
 struct DdDtArgs {
+    int tile_off;
     int ntypes, K, nchunks;
     int tile0[kMaxT + 1];
     int row0[kMaxT + 1];
@@ -511,11 +516,12 @@ dd_dt_kernel(const __grid_constant__ DdMaps maps, const __grid_constant__ DdDtAr
     uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(bars + 2 * ST + 4);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int tile = (int)blockIdx.x + g.tile_off;
     int ty = 0;
 #pragma unroll
     for (int t = 1; t < kMaxT; ++t)
-        if (t < g.ntypes && (int)blockIdx.x >= g.tile0[t]) ty = t;
-    const int m0 = ((int)blockIdx.x - g.tile0[ty]) * 128;
+        if (t < g.ntypes && tile >= g.tile0[t]) ty = t;
+    const int m0 = (tile - g.tile0[ty]) * 128;
     const int rows_t = g.row0[ty + 1] - g.row0[ty];
     const int nk = g.K / kTcBK, nch = g.nchunks;
 
@@ -768,49 +774,47 @@ static void gather_maps(TcMaps& mp, const CUtensorMap* A, const CUtensorMap (*Bh
 
 // the whole fitting chain of all centre types on the tensor cores: 3 forward GEMMs (the third also yields
 // E_i, U and the seed of the backward pass), 3 backward GEMMs.  Returns the number of launches.
-int fitting_chain_tc(Model& m, const ForceArgs& fa, cudaStream_t s) {
+// tiles [t0, t0 + nt_) of the chain on stream s
+static void chain_range(Model& m, const ForceArgs& fa, int t0, int ntl, cudaStream_t s) {
     const int NF = m.NF, ND = m.ND, nt = fa.ntypes;
     TcGemmArgs g{};
     TcMaps mp;
-    const int tiles = fill_types(m, nt, g);
-    auto base = [&]() { TcGemmArgs q{}; fill_types(m, nt, q); return q; };
+    fill_types(m, nt, g);
+    auto base = [&]() { TcGemmArgs q{}; fill_types(m, nt, q); q.tile_off = t0; return q; };
     // layer 1: Y1 = tanh(D W1 + b1), D produced on the fly from T
     {
         L1Args a1{};
+        a1.tile_off = t0;
         a1.ntypes = nt; a1.K = ND; a1.Tm = m.Tm; a1.out = m.Y1; a1.ldo = NF; a1.M1 = m.M1;
         for (int t = 0; t <= kMaxT; ++t) { a1.tile0[t] = g.tile0[t]; a1.row0[t] = g.row0[t]; }
         for (int t = 0; t < nt; ++t) a1.bias[t] = m.fit_b[t][0];
         gather_maps(mp, m.mapA_D, m.mapB_fwd_hi, m.mapB_fwd_lo, 0, nt);
-        static bool attr = false;
-        if (!attr) {
-            cudaFuncSetAttribute(l1_desc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, L1Smem::kTotal);
-            attr = true;
-        }
-        l1_desc_kernel<<<tiles, kTcThreads, L1Smem::kTotal, s>>>(mp, a1);
+        l1_desc_kernel<<<ntl, kTcThreads, L1Smem::kTotal, s>>>(mp, a1);
     }
     // layer 2: T2 = tanh(Y1 W2 + b2); Y2 = Y1 + T2
     g = base(); g.N = NF; g.K = NF; g.add = m.Y1; g.ldadd = NF; g.out0 = m.T2; g.out1 = m.Y2; g.ldo = NF;
     for (int t = 0; t < nt; ++t) g.bias[t] = m.fit_b[t][1];
     gather_maps(mp, m.mapA_Y1, m.mapB_fwd_hi, m.mapB_fwd_lo, 1, nt);
-    tc_gemm(TEPI_TANH_BIAS_SKIP, 240, mp, g, tiles, s);
+    tc_gemm(TEPI_TANH_BIAS_SKIP, 240, mp, g, ntl, s);
     // layer 3 + energy: t3 = tanh(Y2 W3 + b3); y3 = Y2 + t3; E_i = y3.w4 + b4; da3 = w4 o (1 - t3^2) -> G1
     g = base(); g.N = NF; g.K = NF; g.add = m.Y2; g.ldadd = NF; g.out1 = m.G1; g.ldo = NF;
     g.cen_idx = m.cen_idx; g.Eatom = fa.Eatom; g.U = fa.U; g.natoms = fa.N;
     for (int t = 0; t < nt; ++t) { g.bias[t] = m.fit_b[t][2]; g.vec[t] = m.fit_w[t][3]; g.b4[t] = m.fit_b[t][3]; }
     gather_maps(mp, m.mapA_Y2, m.mapB_fwd_hi, m.mapB_fwd_lo, 2, nt);
-    tc_gemm(TEPI_L3E, 240, mp, g, tiles, s);
+    tc_gemm(TEPI_L3E, 240, mp, g, ntl, s);
     // dy2 = dy3 + da3 W3^T -> Y3 ; da2 = dy2 o (1 - t2^2) -> T3       (A = G1 = da3, dy3 = w4)
     g = base(); g.N = NF; g.K = NF; g.tt = m.T2; g.ldtt = NF; g.out0 = m.Y3; g.out1 = m.T3; g.ldo = NF;
     for (int t = 0; t < nt; ++t) g.vec[t] = m.fit_w[t][3];
     gather_maps(mp, m.mapA_G1, m.mapB_bwd_hi, m.mapB_bwd_lo, 2, nt);
-    tc_gemm(TEPI_BWD_VEC, 240, mp, g, tiles, s);
+    tc_gemm(TEPI_BWD_VEC, 240, mp, g, ntl, s);
     // dy1 = dy2 + da2 W2^T ; da1 = dy1 o (1 - y1^2) -> G1                (A = T3 = da2)
     g = base(); g.N = NF; g.K = NF; g.add = m.Y3; g.ldadd = NF; g.tt = m.Y1; g.ldtt = NF; g.out1 = m.G1; g.out0 = m.G2; g.ldo = NF;
     gather_maps(mp, m.mapA_T3, m.mapB_bwd_hi, m.mapB_bwd_lo, 1, nt);
-    tc_gemm(TEPI_BWD_FIRST, 240, mp, g, tiles, s);
+    tc_gemm(TEPI_BWD_FIRST, 240, mp, g, ntl, s);
     // dD = da1 W1^T contracted with T on the fly -> dT                   (A = G1 = da1)
     {
         DdDtArgs d{};
+        d.tile_off = t0;
         d.ntypes = nt; d.K = NF; d.nchunks = ND / kDdBN; d.Tm = m.Tm; d.dTm = m.dTm; d.M1 = m.M1;
         for (int t = 0; t <= kMaxT; ++t) { d.tile0[t] = g.tile0[t]; d.row0[t] = g.row0[t]; }
         DdMaps dm;
@@ -819,14 +823,44 @@ int fitting_chain_tc(Model& m, const ForceArgs& fa, cudaStream_t s) {
             dm.Ahi[t] = m.mapA_G1[q]; dm.Alo[t] = m.mapA_G2[q];
             dm.Bhi[t] = m.mapB_bwd_hi[q][0]; dm.Blo[t] = m.mapB_bwd_lo[q][0];
         }
-        static bool attr = false;
-        if (!attr) {
-            cudaFuncSetAttribute(dd_dt_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, DdSmem::kTotal);
-            attr = true;
-        }
-        dd_dt_kernel<<<tiles, kTcThreads, DdSmem::kTotal, s>>>(dm, d);
+        dd_dt_kernel<<<ntl, kTcThreads, DdSmem::kTotal, s>>>(dm, d);
     }
-    return 6;
+}
+
+// The whole fitting chain of all centre types on the tensor cores: 6 kernels per tile range.  Every kernel of
+// the chain is row-local, so the tiles are cut into ranges that run on separate streams: the tail wave of one
+// range's kernel (384 tiles on 148 SMs are 2.6 waves) is filled by the other range's kernels.
+int fitting_chain_tc(Model& m, const ForceArgs& fa, cudaStream_t s) {
+    TcGemmArgs g{};
+    const int tiles = fill_types(m, fa.ntypes, g);
+    static bool attr = false;
+    if (!attr) {
+        cudaFuncSetAttribute(l1_desc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, L1Smem::kTotal);
+        cudaFuncSetAttribute(dd_dt_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, DdSmem::kTotal);
+        attr = true;
+    }
+    constexpr int NR = Model::kChainStreams;
+    if (!m.aux_stream[0]) {
+        for (int q = 0; q < NR - 1; ++q) {
+            cudaStreamCreateWithFlags(&m.aux_stream[q], cudaStreamNonBlocking);
+            cudaEventCreateWithFlags(&m.ev_join[q], cudaEventDisableTiming);
+        }
+        cudaEventCreateWithFlags(&m.ev_fork, cudaEventDisableTiming);
+    }
+    if (tiles < 2 * NR) {
+        chain_range(m, fa, 0, tiles, s);
+        return 6;
+    }
+    cudaEventRecord(m.ev_fork, s);
+    for (int q = 0; q < NR; ++q) {
+        const int t0 = (int)((long long)tiles * q / NR), t1 = (int)((long long)tiles * (q + 1) / NR);
+        cudaStream_t sq = (q == 0) ? s : m.aux_stream[q - 1];
+        if (q > 0) cudaStreamWaitEvent(sq, m.ev_fork, 0);
+        chain_range(m, fa, t0, t1 - t0, sq);
+        if (q > 0) cudaEventRecord(m.ev_join[q - 1], sq);
+    }
+    for (int q = 1; q < NR; ++q) cudaStreamWaitEvent(s, m.ev_join[q - 1], 0);
+    return 6 * NR;
 }
 
 // parity hook: C[M][N] = A[M][K] Bt[N][K]^T through the tensor-core kernel (N == 240 or N % 160 == 0, K % 16 == 0)
