@@ -201,31 +201,54 @@ neighbor_env_kernel(int P, int N, GridGeom g, EnvConsts ec, const double* __rest
                 if (slot >= sel_t) {
                     atomicMax(overflow, 1);
                 } else {
-                    // environment row in FP64 (R-12), stored FP32
-                    const double r = sqrt(r2);
-                    double sw = 1.0, dsw = 0.0;
-                    if (r >= ec.rs) {
-                        const double u = (r - ec.rs) * ec.inv_range;
-                        sw = u * u * u * (-6.0 * u * u + 15.0 * u - 10.0) + 1.0;
-                        dsw = -30.0 * u * u * (u - 1.0) * (u - 1.0) * ec.inv_range;
-                    }
-                    const double rinv = 1.0 / r;
-                    const double s = sw * rinv;
-                    const double ds = dsw * rinv - sw * rinv * rinv;
-                    NeighSlotA A;
-                    A.dx = (float)d[0]; A.dy = (float)d[1]; A.dz = (float)d[2]; A.s = (float)s;
-                    NeighSlotB B;
-                    B.ds = (float)ds; B.rinv = (float)rinv;
+                    // queue the accepted candidate in its final slot: {j | image code, index into the cell-sorted
+                    // positions}.  The FP64 environment arithmetic runs afterwards over the compact slots with all
+                    // lanes busy (inside this loop only ~13 % of the lanes would be active).
                     const uint32_t code = (uint32_t)(nx + 3) | ((uint32_t)(ny + 3) << 3) | ((uint32_t)(nz + 3) << 6);
+                    NeighSlotB B;
+                    B.ds = 0.f; B.rinv = 0.f;
                     B.jcode = (uint32_t)j | (code << 23);
-                    B.pad = 0.f;
-                    const size_t o = slot0 + seloff_t + slot;
-                    slotA[o] = A;
-                    slotB[o] = B;
+                    B.pad = __int_as_float(q);
+                    slotB[slot0 + seloff_t + slot] = B;
                 }
             }
 
             }
+        }
+    }
+    __syncwarp();
+    // environment rows in FP64 (R-12), stored FP32: same operation order as the distance test above, so d and r2
+    // are reproduced bit for bit
+#pragma unroll
+    for (int t = 0; t < PIMD_MAX_TYPES; ++t) {
+        if (t >= ec.ntypes) continue;
+        const int n = min(cnt[t], ec.sel[t]);
+        for (int e = lane; e < n; e += 32) {
+            const size_t o = slot0 + ec.seloff[t] + e;
+            NeighSlotB B = slotB[o];
+            const uint32_t code = B.jcode >> 23;
+            const int nx = (int)(code & 7) - 3, ny = (int)((code >> 3) & 7) - 3, nz = (int)((code >> 6) & 7) - 3;
+            const double4 wj = ws[__float_as_int(B.pad)];
+            double d[3];
+            d[0] = __dadd_rn(__dsub_rn(wj.x, wi[0]), __dmul_rn((double)nx, g.L[0]));
+            d[1] = __dadd_rn(__dsub_rn(wj.y, wi[1]), __dmul_rn((double)ny, g.L[1]));
+            d[2] = __dadd_rn(__dsub_rn(wj.z, wi[2]), __dmul_rn((double)nz, g.L[2]));
+            const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2]));
+            const double r = sqrt(r2);
+            double sw = 1.0, dsw = 0.0;
+            if (r >= ec.rs) {
+                const double u = (r - ec.rs) * ec.inv_range;
+                sw = u * u * u * (-6.0 * u * u + 15.0 * u - 10.0) + 1.0;
+                dsw = -30.0 * u * u * (u - 1.0) * (u - 1.0) * ec.inv_range;
+            }
+            const double rinv = 1.0 / r;
+            const double sv = sw * rinv;
+            const double ds = dsw * rinv - sw * rinv * rinv;
+            NeighSlotA A;
+            A.dx = (float)d[0]; A.dy = (float)d[1]; A.dz = (float)d[2]; A.s = (float)sv;
+            B.ds = (float)ds; B.rinv = (float)rinv; B.pad = 0.f;
+            slotA[o] = A;
+            slotB[o] = B;
         }
     }
     if (lane == 0) {
