@@ -147,22 +147,40 @@ neighbor_env_kernel(int P, int N, GridGeom g, EnvConsts ec, const double* __rest
                 const int nz = (zz >= 0) ? zz / g.nc[2] : -((-zz + g.nc[2] - 1) / g.nc[2]);
                 const int cc = ((zz - nz * g.nc[2]) * g.nc[1] + (yy - ny * g.nc[1])) * g.nc[0] + (xx - nx * g.nc[0]);
                 my_s0 = cs[cc]; my_s1 = cs[cc + 1];
+                // prune cells that lie entirely outside the cutoff sphere (about a third of the 27): distance from
+                // the centre to the cell's box in the unwrapped cell frame, with a 1e-6 relative margin on r^2 that
+                // dwarfs the rounding of the binning, so no candidate the exact test would accept is dropped
+                const int un[3] = {xx, yy, zz};
+                double dm2 = 0.0;
+#pragma unroll
+                for (int ax = 0; ax < 3; ++ax) {
+                    const double wc = 1.0 / g.inv_w[ax];
+                    const double lo = un[ax] * wc - wi[ax], hi = wi[ax] - (un[ax] + 1) * wc;
+                    const double dd = fmax(fmax(lo, hi), 0.0);
+                    dm2 += dd * dd;
+                }
+                if (dm2 > ec.rc2 * (1.0 + 1e-6)) my_s1 = my_s0;
                 my_code = (nx + 3) | ((ny + 3) << 3) | ((nz + 3) << 6);
             }
         }
-        const int nb = min(32, ncl - base);
+        // walk only the cells that still have candidates, in the same (oz, oy, ox) order
+        unsigned todo = __ballot_sync(0xffffffffu, my_s1 > my_s0);
         double4 wnext = make_double4(0, 0, 0, 0);
-        {
-            const int f0 = __shfl_sync(0xffffffffu, my_s0, 0), f1 = __shfl_sync(0xffffffffu, my_s1, 0);
+        if (todo) {
+            const int c = __ffs(todo) - 1;
+            const int f0 = __shfl_sync(0xffffffffu, my_s0, c), f1 = __shfl_sync(0xffffffffu, my_s1, c);
             if (f0 + lane < f1) wnext = ws[f0 + lane];
         }
-        for (int c = 0; c < nb; ++c) {
+        while (todo) {
+            const int c = __ffs(todo) - 1;
+            todo &= todo - 1;
             const int s0 = __shfl_sync(0xffffffffu, my_s0, c), s1 = __shfl_sync(0xffffffffu, my_s1, c);
             const int code = __shfl_sync(0xffffffffu, my_code, c);
             const int nx = (code & 7) - 3, ny = ((code >> 3) & 7) - 3, nz = ((code >> 6) & 7) - 3;
             const double4 wfirst = wnext;
-            if (c + 1 < nb) {
-                const int f0 = __shfl_sync(0xffffffffu, my_s0, c + 1), f1 = __shfl_sync(0xffffffffu, my_s1, c + 1);
+            if (todo) {
+                const int cn = __ffs(todo) - 1;
+                const int f0 = __shfl_sync(0xffffffffu, my_s0, cn), f1 = __shfl_sync(0xffffffffu, my_s1, cn);
                 if (f0 + lane < f1) wnext = ws[f0 + lane];
             }
             const double sh[3] = {__dmul_rn((double)nx, g.L[0]), __dmul_rn((double)ny, g.L[1]),
