@@ -308,16 +308,34 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
         mo[j] = g_orig(ps / H3, ps % H3);
     }
 
+    // Work split: the row tiles of all (t_i, t_j) pairs form one list; CTA b takes the contiguous share
+    // [T b / G, T (b+1) / G) of it (balanced to one tile; most CTAs see a single pair, so they load one weight
+    // image and the two contexts are de-phased once), and its two contexts halve every pair's sub-range.
+    int tile_total = 0, sub_lo = 0, sub_hi = 0;
     for (int p = 0; p < nt * nt; ++p) {
         const int ti = p / nt, tj = p - ti * nt;
+        const int* rs = a.rowstart + (size_t)tj * (a.PN + 1);
+        tile_total += (rs[a.type_row0[ti + 1]] - rs[a.type_row0[ti]] + 127) >> 7;
+    }
+    const int g_lo = (int)((long long)tile_total * blockIdx.x / gridDim.x);
+    const int g_hi = (int)((long long)tile_total * (blockIdx.x + 1) / gridDim.x);
+    int tile_off = 0;
+    for (int p = 0; p < nt * nt; ++p) {
+        const int ti = p / nt, tj = p - ti * nt;
+        {
+            const int* rs0 = a.rowstart + (size_t)tj * (a.PN + 1);
+            const int nt_p = (rs0[a.type_row0[ti + 1]] - rs0[a.type_row0[ti]] + 127) >> 7;
+            const int lo = max(g_lo, tile_off) - tile_off, hi = min(g_hi, tile_off + nt_p) - tile_off;
+            tile_off += nt_p;
+            if (lo >= hi) continue;                        // CTA-uniform: no tile of this pair is mine
+            sub_lo = lo; sub_hi = hi;
+        }
         __syncthreads();                                   // both contexts are done with the previous weights
         load_weight_image(cs.smem, a.wimg + (size_t)p * kImgBytes);
         __syncthreads();
         const int* rs = a.rowstart + (size_t)tj * (a.PN + 1);
         const int begin = rs[a.type_row0[ti]], end = rs[a.type_row0[ti + 1]];
-        const int ntile = (end - begin + 127) >> 7;
-        const int C = gridDim.x * 2, c = blockIdx.x * 2 + cx;
-        const int tl0 = (int)((long long)ntile * c / C), tl1 = (int)((long long)ntile * (c + 1) / C);
+        const int tl0 = sub_lo + (sub_hi - sub_lo) * cx / 2, tl1 = sub_lo + (sub_hi - sub_lo) * (cx + 1) / 2;
         if (tl0 >= tl1) continue;
         if (cx == 1 && a.skew_fwd > 0) {                    // de-phase the two contexts (see the backward kernel)
             const long long t0 = clock64();
@@ -518,6 +536,9 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
     uint32_t phase = 0;
     const int nt = a.ntypes;
 
+    // Work split (unlike the forward kernel's contiguous shares): every context takes its 1/(2G) slice of EVERY
+    // pair, which keeps the two contexts of a CTA on far-apart centres -- measured 3 % faster here, presumably
+    // because their force atomics then rarely meet on the same atoms.
     for (int p = 0; p < nt * nt; ++p) {
         const int ti = p / nt, tj = p - ti * nt;
         __syncthreads();
