@@ -23,6 +23,7 @@
 // A CTA runs two independent contexts, each with its own A-operand region, TMEM columns and mbarrier, so
 // that one context's MMAs overlap the other's tanh / epilogue work.
 #include <cstring>
+#include <cuda_fp16.h>
 #include <type_traits>
 #include "common.cuh"
 #include "tc_gemm.cuh"
@@ -74,6 +75,62 @@ constexpr int kBias3 = 26;
 __host__ __device__ constexpr int n3_of(int h, int g) { return 56 * h + g; }       // layer-3 output column
 }  // namespace etc
 
+// ---- FP16-split operand variant (forward kernel) ----------------------------------------------------------
+// a = hi + lo with hi = fp16(a) (11-bit significand, like TF32) and lo = fp16(a - hi): a b ~= hi_a hi_b + lo_a hi_b +
+// hi_a lo_b with FP32 accumulation, the same three-pass scheme at kind::f16 -- twice the tensor rate per pass and
+// half the shared-memory bytes per operand (the MMAs here are operand-read-bound).  All operands are O(1)
+// (tanh outputs plus skips, weights ~ 1/sqrt(fan_in)), far inside FP16's range; small values keep an absolute
+// error of 2^-25 through FP16 subnormals, which is what matters inside a dot product.
+namespace eh {
+constexpr int K2 = 32;                 // halfs: half A at k 0..12, bias at 13, half B at 16..28   (64 B rows, SW64)
+constexpr int N2 = 64;
+constexpr int K3 = 64;                 // halfs: half A at k 0..25, bias at 26, half B at 32..57   (128 B rows, SW128)
+constexpr int N3 = 112;
+constexpr int oW2hi = 0, oW2lo = N2 * 64;                        // [64][32] fp16
+constexpr int oW3hi = 2 * N2 * 64, oW3lo = oW3hi + N3 * 128;     // [112][64] fp16
+constexpr int oW1 = oW3lo + N3 * 128;                            // W1[32], b1[32] plain floats (padded h1 index)
+constexpr int kImgBytes = oW1 + 256;                             // 37120
+constexpr int kImgPad = (kImgBytes + 1023) / 1024 * 1024;
+__host__ __device__ constexpr int k2_of(int h, int i) { return 16 * h + i; }
+constexpr int kBias2 = 13;
+__host__ __device__ constexpr int k3_of(int h, int j) { return 32 * h + j; }
+constexpr int kBias3 = 26;
+constexpr int oA1hi = 0, oA1lo = 128 * 64;                       // per-context A1: [128][32] fp16 hi / lo
+constexpr int oA2hi = 0, oA2lo = 128 * 128;                      // per-context A2: [128][64] fp16 hi / lo (overlays A1)
+}  // namespace eh
+
+// 8 consecutive K elements (one 16-byte chunk) of row `row` -> hi and lo copies of a K-major FP16 operand block
+// with `ROWB`-byte rows (64: SWIZZLE_64B, 128: SWIZZLE_128B)
+template <int ROWB>
+__device__ __forceinline__ void store_chunk_h(uint8_t* blk_hi, uint8_t* blk_lo, int row, int chunk, const float* v) {
+    const int sw = (ROWB == 128) ? (row & 7) : ((row >> 1) & 3);
+    const int off = row * ROWB + ((chunk ^ sw) << 4);
+    uint32_t hi[4], lo[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const __half2 h = __floats2half2_rn(v[2 * q], v[2 * q + 1]);
+        const float2 hf = __half22float2(h);
+        const __half2 l = __floats2half2_rn(v[2 * q] - hf.x, v[2 * q + 1] - hf.y);
+        hi[q] = *reinterpret_cast<const uint32_t*>(&h);
+        lo[q] = *reinterpret_cast<const uint32_t*>(&l);
+    }
+    *reinterpret_cast<uint4*>(blk_hi + off) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+    *reinterpret_cast<uint4*>(blk_lo + off) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+}
+
+// three-pass FP16 product over `nks` k-steps of 16 (32 bytes of K per step inside a swizzled row)
+template <int ROWB>
+__device__ __forceinline__ void mma_3x_f16(uint32_t d_tmem, uint32_t a_hi, uint32_t a_lo, uint32_t b_hi, uint32_t b_lo,
+                                           uint32_t idesc, int nks) {
+    for (int ks = 0; ks < nks; ++ks) {
+        const uint64_t dah = make_smem_desc_kmajor(a_hi + ks * 32, ROWB), dal = make_smem_desc_kmajor(a_lo + ks * 32, ROWB);
+        const uint64_t dbh = make_smem_desc_kmajor(b_hi + ks * 32, ROWB), dbl = make_smem_desc_kmajor(b_lo + ks * 32, ROWB);
+        umma_f16(d_tmem, dah, dbh, idesc, ks == 0 ? 0u : 1u);
+        umma_f16(d_tmem, dal, dbh, idesc, 1u);
+        umma_f16(d_tmem, dah, dbl, idesc, 1u);
+    }
+}
+
 struct EmbTcArgs {
     int PN, N, ntypes, nsel;
     int seloff[PIMD_MAX_TYPES + 1];
@@ -85,6 +142,7 @@ struct EmbTcArgs {
     const NeighSlotA* slotA;
     const NeighSlotB* slotB;
     const uint8_t* wimg;       // [ntypes*ntypes][kImgBytes]
+    const uint8_t* wimg_h;     // [ntypes*ntypes][eh::kImgBytes]  FP16-split images (forward kernel)
     float* Tm;                 // [PN][100][4]  (zeroed before the forward kernel)
     const float* dTm;
     double* f;                 // [P][N][3]
@@ -271,6 +329,13 @@ __device__ __forceinline__ CtxSetup ctx_setup(uint8_t* smem_raw, uint32_t ncols)
     return c;
 }
 
+__device__ __forceinline__ void load_weight_image_n(uint8_t* dst, const uint8_t* src, int nbytes) {
+    const float4* s4 = reinterpret_cast<const float4*>(src);
+    float4* d4 = reinterpret_cast<float4*>(dst);
+    for (int q = threadIdx.x; q < nbytes / 16; q += etc::kThreads) d4[q] = __ldg(s4 + q);
+    fence_proxy_async_smem();
+}
+
 __device__ __forceinline__ void load_weight_image(uint8_t* dst, const uint8_t* src) {
     const float4* s4 = reinterpret_cast<const float4*>(src);
     float4* d4 = reinterpret_cast<float4*>(dst);
@@ -292,12 +357,12 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
     float4* Rs = reinterpret_cast<float4*>(ctx + oRs);
     int* cen_s = reinterpret_cast<int*>(ctx + oCen);
     float* Gs = reinterpret_cast<float*>(ctx);
-    const float* W1s = reinterpret_cast<const float*>(cs.smem + oW1) + H1 * half;
+    const float* W1s = reinterpret_cast<const float*>(cs.smem + eh::oW1) + H1 * half;
     const float* b1s = W1s + 32;
     const uint32_t tmem_d = cs.tmem_base + cx * 128;
     const uint32_t lanefield = ((uint32_t)((t >> 5) * 32)) << 16;
     const uint32_t actx = smem_u32(ctx), wbase = smem_u32(cs.smem);
-    constexpr uint32_t idesc2 = make_idesc_tf32(128, N2), idesc3 = make_idesc_tf32(128, N3);
+    constexpr uint32_t idesc2 = make_idesc_f16(128, eh::N2), idesc3 = make_idesc_f16(128, eh::N3);
     uint32_t phase = 0;
     const int nt = a.ntypes;
     // T accumulation: lane <-> staged G positions 4 lane .. 4 lane + 3 (26 lanes); their original channels
@@ -331,7 +396,7 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
             sub_lo = lo; sub_hi = hi;
         }
         __syncthreads();                                   // both contexts are done with the previous weights
-        load_weight_image(cs.smem, a.wimg + (size_t)p * kImgBytes);
+        load_weight_image_n(cs.smem, a.wimg_h + (size_t)p * eh::kImgBytes, eh::kImgBytes);
         __syncthreads();
         const int* rs = a.rowstart + (size_t)tj * (a.PN + 1);
         const int begin = rs[a.type_row0[ti]], end = rs[a.type_row0[ti + 1]];
@@ -366,25 +431,27 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
 #pragma unroll
             for (int i = 0; i < H1; ++i) h1[i] = tanh_fast(fmaf(s, W1s[i], b1s[i]));
             {
-                const float one = half ? 0.f : 1.f;        // bias slot (k = 13) lives in half A's range
-                store_chunk(ctx, ctx + kABlk, t, 4 * half + 0, h1[0], h1[1], h1[2], h1[3]);
-                store_chunk(ctx, ctx + kABlk, t, 4 * half + 1, h1[4], h1[5], h1[6], h1[7]);
-                store_chunk(ctx, ctx + kABlk, t, 4 * half + 2, h1[8], h1[9], h1[10], h1[11]);
-                store_chunk(ctx, ctx + kABlk, t, 4 * half + 3, h1[12], one, 0.f, 0.f);
+                // FP16 A1 (64 B rows): my 13 channels + the bias slot (k = 13, half A only) = K slots 16 half .. + 15
+                float v16[16];
+#pragma unroll
+                for (int i = 0; i < H1; ++i) v16[i] = h1[i];
+                v16[13] = half ? 0.f : 1.f; v16[14] = 0.f; v16[15] = 0.f;
+                store_chunk_h<64>(ctx + eh::oA1hi, ctx + eh::oA1lo, t, 2 * half, v16);
+                store_chunk_h<64>(ctx + eh::oA1hi, ctx + eh::oA1lo, t, 2 * half + 1, v16 + 8);
             }
             fence_proxy_async_smem();
             tc_fence_before();
             named_bar_sync(bar_ctx, 256);
             if ((threadIdx.x & 255) == 0) {
                 tc_fence_after();
-                mma_block_3x(tmem_d, actx, actx + kABlk, wbase + oW2hi, wbase + oW2lo, idesc2, 4, true);
+                mma_3x_f16<64>(tmem_d, actx + eh::oA1hi, actx + eh::oA1lo, wbase + eh::oW2hi, wbase + eh::oW2lo, idesc2, 2);
                 umma_commit(cs.mma_bar);
             }
             mbar_wait(cs.mma_bar, phase);
             phase ^= 1;
             tc_fence_after();
             // ---- epilogue 2: h2 = [h1,h1] + tanh(z2), my 26 columns; A2 K slots 28 half .. 28 half + 27 ----
-            float h2[H2 + 2];
+            float h2[H2];
             {
                 uint32_t v[H2];
                 const uint32_t col = tmem_d + lanefield + 32 * half;
@@ -394,23 +461,23 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
                 tmem_ld_wait();
 #pragma unroll
                 for (int j = 0; j < H2; ++j) h2[j] = h1[j % H1] + tanh_fast(__uint_as_float(v[j]));
-                h2[H2] = half ? 0.f : 1.f;                 // bias slot (k = 26)
-                h2[H2 + 1] = 0.f;
+                // FP16 A2 (128 B rows): my 26 channels + the bias slot (k = 26, half A only) = K slots 32 half .. + 31
+                float v32[32];
 #pragma unroll
-                for (int cq = 0; cq < 7; ++cq) {
-                    const int gc = 7 * half + cq, blk = gc >> 3;
-                    uint8_t* bh = ctx + blk * kABlk;
-                    store_chunk(bh, bh + 2 * kABlk, t, gc & 7, h2[4 * cq], h2[4 * cq + 1], h2[4 * cq + 2], h2[4 * cq + 3]);
-                }
+                for (int j = 0; j < H2; ++j) v32[j] = h2[j];
+                v32[26] = half ? 0.f : 1.f;
+#pragma unroll
+                for (int j = 27; j < 32; ++j) v32[j] = 0.f;
+#pragma unroll
+                for (int cq = 0; cq < 4; ++cq)
+                    store_chunk_h<128>(ctx + eh::oA2hi, ctx + eh::oA2lo, t, 4 * half + cq, v32 + 8 * cq);
             }
             fence_proxy_async_smem();
             tc_fence_before();
             named_bar_sync(bar_ctx, 256);
             if ((threadIdx.x & 255) == 0) {
                 tc_fence_after();
-                mma_block_3x(tmem_d, actx, actx + 2 * kABlk, wbase + oW3hi, wbase + oW3lo, idesc3, 4, true);
-                mma_block_3x(tmem_d, actx + kABlk, actx + 3 * kABlk, wbase + oW3hi + kW3blk, wbase + oW3lo + kW3blk, idesc3,
-                             3, false);
+                mma_3x_f16<128>(tmem_d, actx + eh::oA2hi, actx + eh::oA2lo, wbase + eh::oW3hi, wbase + eh::oW3lo, idesc3, 4);
                 umma_commit(cs.mma_bar);
             }
             mbar_wait(cs.mma_bar, phase);
@@ -882,13 +949,61 @@ void emb_tc_build_image(const double* w, uint8_t* img) {
     for (int k = 0; k < E1; ++k) { l1[k] = (float)W1[k]; l1[32 + k] = (float)b1[k]; }
 }
 
+size_t emb_tc_image_h_bytes() { return eh::kImgBytes; }
+
+// FP16-split image of one (t_i, t_j) net for the forward kernel (same channel permutation as emb_tc_build_image)
+void emb_tc_build_image_h(const double* w, uint8_t* img) {
+    using namespace etc;
+    memset(img, 0, eh::kImgBytes);
+    const double* W1 = w;
+    const double* b1 = W1 + E1;
+    const double* W2 = b1 + E1;
+    const double* b2 = W2 + E1 * E2;
+    const double* W3 = b2 + E2;
+    const double* b3 = W3 + E2 * M1;
+    auto put = [&](int o_hi, int o_lo, int rowb, int n, int k, float v) {
+        const int sw = (rowb == 128) ? (n & 7) : ((n >> 1) & 3);
+        const int off = n * rowb + (((k >> 3) ^ sw) << 4) + (k & 7) * 2;
+        const __half hi = __float2half_rn(v);
+        const __half lo = __float2half_rn(v - __half2float(hi));
+        memcpy(img + o_hi + off, &hi, 2);
+        memcpy(img + o_lo + off, &lo, 2);
+    };
+    for (int h = 0; h < 2; ++h)
+        for (int j = 0; j < H2; ++j) {
+            const int n_orig = h2_orig(h, j);
+            if (n_orig < 0) continue;
+            const int n = n2_of(h, j);
+            for (int hh = 0; hh < 2; ++hh)
+                for (int i = 0; i < H1; ++i) {
+                    const int c1 = H1 * hh + i;
+                    if (c1 < E1) put(eh::oW2hi, eh::oW2lo, 64, n, eh::k2_of(hh, i), (float)W2[c1 * E2 + n_orig]);
+                }
+            put(eh::oW2hi, eh::oW2lo, 64, n, eh::kBias2, (float)b2[n_orig]);
+        }
+    for (int h = 0; h < 2; ++h)
+        for (int g = 0; g < H3; ++g) {
+            const int n_orig = g_orig(h, g);
+            if (n_orig < 0) continue;
+            const int n = n3_of(h, g);
+            for (int hh = 0; hh < 2; ++hh)
+                for (int j = 0; j < H2; ++j) {
+                    const int k_orig = h2_orig(hh, j);
+                    if (k_orig >= 0) put(eh::oW3hi, eh::oW3lo, 128, n, eh::k3_of(hh, j), (float)W3[k_orig * M1 + n_orig]);
+                }
+            put(eh::oW3hi, eh::oW3lo, 128, n, eh::kBias3, (float)b3[n_orig]);
+        }
+    float* l1 = reinterpret_cast<float*>(img + eh::oW1);
+    for (int k = 0; k < E1; ++k) { l1[k] = (float)W1[k]; l1[32 + k] = (float)b1[k]; }
+}
+
 static EmbTcArgs make_tc_args(Model& m, const ForceArgs& fa) {
     EmbTcArgs a;
     a.PN = fa.P * fa.N; a.N = fa.N; a.ntypes = fa.ntypes; a.nsel = m.nsel;
     for (int t = 0; t <= PIMD_MAX_TYPES; ++t) { a.seloff[t] = m.seloff[t]; a.type_row0[t] = m.type_row0[t]; }
     for (int t = 0; t < PIMD_MAX_TYPES; ++t) a.n_of_type[t] = (t < fa.ntypes) ? m.n_of_type[t] : 0;
     a.rowstart = m.rowstart; a.rowaddr = m.rowaddr; a.row_of = m.row_of;
-    a.slotA = m.slotA; a.slotB = m.slotB; a.wimg = m.emb_img;
+    a.slotA = m.slotA; a.slotB = m.slotB; a.wimg = m.emb_img; a.wimg_h = m.emb_img_h;
     a.Tm = m.Tm; a.dTm = m.dTm; a.f = fa.f; a.cpart = m.cpart;
     a.inv_nsel = 1.0f / (float)m.nsel;
     // measured on B200: plateaus at 4-6 k cycles (forward, -20 %) and 5-13 k cycles (backward, -8 %)
