@@ -594,12 +594,15 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
     int* cen_s = reinterpret_cast<int*>(ctx + oCen);
     float4* dTs = reinterpret_cast<float4*>(ctx);
     float* part = reinterpret_cast<float*>(ctx + oPart) + t * 8;
-    const float* W1s = reinterpret_cast<const float*>(cs.smem + oW1) + H1 * half;
+    const float* W1s = reinterpret_cast<const float*>(cs.smem + eh::oW1) + H1 * half;
     const float* b1s = W1s + 32;
     const uint32_t tmem_v = cs.tmem_base + cx * 256, tmem_g = tmem_v + 128;     // value / derivative accumulators
     const uint32_t lanefield = ((uint32_t)((t >> 5) * 32)) << 16;
     const uint32_t actx = smem_u32(ctx), wbase = smem_u32(cs.smem);
-    constexpr uint32_t idesc2 = make_idesc_tf32(128, N2), idesc3 = make_idesc_tf32(128, N3);
+    constexpr uint32_t idesc2 = make_idesc_f16(128, eh::N2), idesc3 = make_idesc_f16(128, eh::N3);
+    // FP16-split operands (see namespace eh): region X = ctx + 0 (32 KB): A1v | A1d, later A2v; region Y = ctx + 32 KB: A2d.
+    // Value and derivative operands have their own storage, so both layer-3 products go out in one MMA round trip.
+    constexpr int oY = 2 * kABlk;
     uint32_t phase = 0;
     const int nt = a.ntypes;
 
@@ -609,7 +612,7 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
     for (int p = 0; p < nt * nt; ++p) {
         const int ti = p / nt, tj = p - ti * nt;
         __syncthreads();
-        load_weight_image(cs.smem, a.wimg + (size_t)p * kImgBytes);
+        load_weight_image_n(cs.smem, a.wimg_h + (size_t)p * eh::kImgBytes, eh::kImgBytes);
         __syncthreads();
         const int* rs = a.rowstart + (size_t)tj * (a.PN + 1);
         const int begin = rs[a.type_row0[ti]], end = rs[a.type_row0[ti + 1]];
@@ -662,30 +665,32 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
                 h1p[i] = (1.f - th * th) * w;
             }
             {
-                const float one = half ? 0.f : 1.f;
+                // A1v = [h1, 1 (bias slot, half A), 0, 0], A1d = [h1', 0, 0, 0]: K slots 16 half .. + 15 (64 B rows)
+                float vv[16], vd[16];
 #pragma unroll
-                for (int cq = 0; cq < 3; ++cq) {
-                    store_chunk(ctx, ctx + kABlk, t, 4 * half + cq, h1[4 * cq], h1[4 * cq + 1], h1[4 * cq + 2], h1[4 * cq + 3]);
-                    store_chunk(ctx + 2 * kABlk, ctx + 3 * kABlk, t, 4 * half + cq, h1p[4 * cq], h1p[4 * cq + 1],
-                                h1p[4 * cq + 2], h1p[4 * cq + 3]);
+                for (int i = 0; i < H1; ++i) { vv[i] = h1[i]; vd[i] = h1p[i]; }
+                vv[13] = half ? 0.f : 1.f; vv[14] = 0.f; vv[15] = 0.f;
+                vd[13] = 0.f; vd[14] = 0.f; vd[15] = 0.f;
+#pragma unroll
+                for (int cq = 0; cq < 2; ++cq) {
+                    store_chunk_h<64>(ctx, ctx + 8192, t, 2 * half + cq, vv + 8 * cq);
+                    store_chunk_h<64>(ctx + 16384, ctx + 24576, t, 2 * half + cq, vd + 8 * cq);
                 }
-                store_chunk(ctx, ctx + kABlk, t, 4 * half + 3, h1[12], one, 0.f, 0.f);
-                store_chunk(ctx + 2 * kABlk, ctx + 3 * kABlk, t, 4 * half + 3, h1p[12], 0.f, 0.f, 0.f);
             }
             fence_proxy_async_smem();
             tc_fence_before();
             named_bar_sync(bar_ctx, 256);
             if ((threadIdx.x & 255) == 0) {
                 tc_fence_after();
-                mma_block_3x(tmem_v, actx, actx + kABlk, wbase + oW2hi, wbase + oW2lo, idesc2, 4, true);
-                mma_block_3x(tmem_g, actx + 2 * kABlk, actx + 3 * kABlk, wbase + oW2hi, wbase + oW2lo, idesc2, 4, true);
+                mma_3x_f16<64>(tmem_v, actx, actx + 8192, wbase + eh::oW2hi, wbase + eh::oW2lo, idesc2, 2);
+                mma_3x_f16<64>(tmem_g, actx + 16384, actx + 24576, wbase + eh::oW2hi, wbase + eh::oW2lo, idesc2, 2);
                 umma_commit(cs.mma_bar);
             }
             mbar_wait(cs.mma_bar, phase);
             phase ^= 1;
             tc_fence_after();
-            // ---- epilogue 2: h2, h2' (my 26 columns); A2v written now, A2d after MMA3v has consumed the region ----
-            float h2[H2 + 2], h2p[H2 + 2];
+            // ---- epilogue 2: h2, h2' (my 26 columns) -> A2v and A2d ----
+            float h2[H2], h2p[H2];
             {
                 uint32_t v[H2], d[H2];
                 const uint32_t cv = tmem_v + lanefield + 32 * half, cd = tmem_g + lanefield + 32 * half;
@@ -698,33 +703,18 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
                     h2[j] = h1[j % H1] + th;
                     h2p[j] = fmaf(1.f - th * th, __uint_as_float(d[j]), h1p[j % H1]);
                 }
-                h2[H2] = half ? 0.f : 1.f; h2[H2 + 1] = 0.f;
-                h2p[H2] = 0.f; h2p[H2 + 1] = 0.f;
+                // A2v (region X) = [h2, 1 (bias slot, half A), 0..]; A2d (region Y) = [h2', 0..]: K slots 32 half .. + 31
+                float vv[32], vd[32];
 #pragma unroll
-                for (int cq = 0; cq < 7; ++cq) {
-                    const int gc = 7 * half + cq, blk = gc >> 3;
-                    uint8_t* bh = ctx + blk * kABlk;
-                    store_chunk(bh, bh + 2 * kABlk, t, gc & 7, h2[4 * cq], h2[4 * cq + 1], h2[4 * cq + 2], h2[4 * cq + 3]);
+                for (int j = 0; j < H2; ++j) { vv[j] = h2[j]; vd[j] = h2p[j]; }
+                vv[26] = half ? 0.f : 1.f; vd[26] = 0.f;
+#pragma unroll
+                for (int j = 27; j < 32; ++j) { vv[j] = 0.f; vd[j] = 0.f; }
+#pragma unroll
+                for (int cq = 0; cq < 4; ++cq) {
+                    store_chunk_h<128>(ctx, ctx + 16384, t, 4 * half + cq, vv + 8 * cq);
+                    store_chunk_h<128>(ctx + oY, ctx + oY + 16384, t, 4 * half + cq, vd + 8 * cq);
                 }
-            }
-            fence_proxy_async_smem();
-            tc_fence_before();
-            named_bar_sync(bar_ctx, 256);
-            if ((threadIdx.x & 255) == 0) {
-                tc_fence_after();
-                mma_block_3x(tmem_v, actx, actx + 2 * kABlk, wbase + oW3hi, wbase + oW3lo, idesc3, 4, true);
-                mma_block_3x(tmem_v, actx + kABlk, actx + 3 * kABlk, wbase + oW3hi + kW3blk, wbase + oW3lo + kW3blk, idesc3,
-                             3, false);
-                umma_commit(cs.mma_bar);
-            }
-            mbar_wait(cs.mma_bar, phase);                  // the other context works meanwhile
-            phase ^= 1;
-            tc_fence_after();
-#pragma unroll
-            for (int cq = 0; cq < 7; ++cq) {
-                const int gc = 7 * half + cq, blk = gc >> 3;
-                uint8_t* bh = ctx + blk * kABlk;
-                store_chunk(bh, bh + 2 * kABlk, t, gc & 7, h2p[4 * cq], h2p[4 * cq + 1], h2p[4 * cq + 2], h2p[4 * cq + 3]);
             }
             if (half == 0) cen_s[t] = cur.cen;
             const float sr = cur.s * cur.rinv;
@@ -734,9 +724,8 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
             named_bar_sync(bar_ctx, 256);
             if ((threadIdx.x & 255) == 0) {
                 tc_fence_after();
-                mma_block_3x(tmem_g, actx, actx + 2 * kABlk, wbase + oW3hi, wbase + oW3lo, idesc3, 4, true);
-                mma_block_3x(tmem_g, actx + kABlk, actx + 3 * kABlk, wbase + oW3hi + kW3blk, wbase + oW3lo + kW3blk, idesc3,
-                             3, false);
+                mma_3x_f16<128>(tmem_v, actx, actx + 16384, wbase + eh::oW3hi, wbase + eh::oW3lo, idesc3, 4);
+                mma_3x_f16<128>(tmem_g, actx + oY, actx + oY + 16384, wbase + eh::oW3hi, wbase + eh::oW3lo, idesc3, 4);
                 umma_commit(cs.mma_bar);
             }
             // ---- dT of this tile's centres: fetched into registers while the MMAs run, then staged into the
