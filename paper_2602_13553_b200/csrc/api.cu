@@ -116,6 +116,7 @@ size_t model_bytes(const pimd_ctx* c, const pimd_model_desc* d) {
     cell_grid(c->box, d->rcut, ncell, R, &ncells);
     size_t b = 0;
     b += align_up((size_t)d->n_types * d->n_types * 8192 * 4, 256);                     // embedding weights (padded)
+    b += (size_t)d->n_types * 4 * align_up((size_t)ND * NF * 2, 256);                  // FP16-split layer-1 images
     b += (size_t)d->n_types * 6 * (align_up((size_t)ND * NF * 4, 256) + 2 * align_up((size_t)NF * NF * 4, 256) + align_up(NF * 4, 256));
     b += (size_t)d->n_types * 4 * align_up((size_t)NF * 4, 256);
     b += 4 * align_up(PN * 4, 256);                                                    // cen_idx,row_of,cell_id,cell_tmp
@@ -536,12 +537,33 @@ int pimd_set_model(pimd_ctx* ctx, const pimd_model_desc* d, const double* w, siz
                 if ((rc = arena_alloc(ctx, &m.fit_wT_lo[t][l], W.size()))) return rc;
                 tc_split_weights(W.size(), m.fit_w[t][l], m.fit_w_hi[t][l], m.fit_w_lo[t][l], ctx->stream);
                 tc_split_weights(W.size(), m.fit_wT[t][l], m.fit_wT_hi[t][l], m.fit_wT_lo[t][l], ctx->stream);
+                if (l == 0) {     // FP16-split images of layer 1 (fitting_tc.cu: l1_desc_kernel, dd_dt_kernel)
+                    if ((rc = arena_alloc(ctx, &m.w1_h_hi[t], W.size()))) return rc;
+                    if ((rc = arena_alloc(ctx, &m.w1_h_lo[t], W.size()))) return rc;
+                    if ((rc = arena_alloc(ctx, &m.w1T_h_hi[t], W.size()))) return rc;
+                    if ((rc = arena_alloc(ctx, &m.w1T_h_lo[t], W.size()))) return rc;
+                    tc_split_weights_h(W.size(), m.fit_w[t][l], 64.f, m.w1_h_hi[t], m.w1_h_lo[t], ctx->stream);
+                    tc_split_weights_h(W.size(), m.fit_wT[t][l], 64.f, m.w1T_h_hi[t], m.w1T_h_lo[t], ctx->stream);
+                }
             }
             keep.push_back(std::move(W)); keep.push_back(std::move(WT)); keep.push_back(std::move(b));
             nin = nout;
         }
     }
 
+    {   // backward activations start at dy3 = w4: scale them by a power of two so that max |w4| lands in [8, 16)
+        float wmax = 0.f;
+        size_t q = (size_t)nt * nt * ((size_t)2 * E1 + (size_t)E1 * E2 + E2 + (size_t)E2 * M1 + M1);
+        for (int t = 0; t < nt; ++t) {
+            size_t nin = m.ND;
+            for (int l = 0; l < 3; ++l) { q += nin * m.NF + m.NF; nin = m.NF; }
+            for (int k = 0; k < m.NF; ++k) wmax = std::max(wmax, (float)std::fabs(w[q + k]));
+            q += m.NF + 1;
+        }
+        int ex = 0;
+        if (wmax > 0.f) std::frexp(wmax, &ex);            // wmax = f 2^ex, f in [0.5, 1)
+        m.bwd_scale = std::ldexp(1.f, 4 - ex);
+    }
     // ---- centre order [type][bead][atom of type] ----
     std::vector<int> cen(PN), rowof(PN);
     {

@@ -113,6 +113,13 @@ struct Model {
     CUtensorMap mapB_bwd_hi[PIMD_MAX_TYPES][3], mapB_bwd_lo[PIMD_MAX_TYPES][3];   // W_l    [in][out]
     float*   fit_w_hi[PIMD_MAX_TYPES][3], *fit_w_lo[PIMD_MAX_TYPES][3];           // pre-split weights (layers 1..3)
     float*   fit_wT_hi[PIMD_MAX_TYPES][3], *fit_wT_lo[PIMD_MAX_TYPES][3];
+    // FP16-split images of the first fitting layer (x kW1Scale) for the two K = 1600 / N = 1600 kernels
+    uint16_t* w1T_h_hi[PIMD_MAX_TYPES], *w1T_h_lo[PIMD_MAX_TYPES];   // W1^T [240][1600]
+    uint16_t* w1_h_hi[PIMD_MAX_TYPES], *w1_h_lo[PIMD_MAX_TYPES];     // W1   [1600][240]
+    CUtensorMap mapBh_l1_hi[PIMD_MAX_TYPES], mapBh_l1_lo[PIMD_MAX_TYPES];     // layer-1 forward B
+    CUtensorMap mapBh_dd_hi[PIMD_MAX_TYPES], mapBh_dd_lo[PIMD_MAX_TYPES];     // dD GEMM B
+    CUtensorMap mapAh_G1[PIMD_MAX_TYPES], mapAh_G2[PIMD_MAX_TYPES];           // da1 as FP16 hi / lo (x bwd_scale)
+    float    bwd_scale = 1.f;          // power of two that brings the backward activations to O(1..16)
     // tensor-core embedding path (embedding_tc.cu)
     bool     use_tc_emb = true;
     bool     tc_emb_ready = false;
@@ -142,6 +149,7 @@ int embedding_backward(Model& m, const ForceArgs& a, int n_sms, cudaStream_t s);
 size_t embedding_smem_bytes(const Model& m, int ntypes);
 bool tc_setup_maps(Model& m, int ntypes);
 void tc_split_weights(size_t n, const float* w, float* hi, float* lo, cudaStream_t s);
+void tc_split_weights_h(size_t n, const float* w, float scale, uint16_t* hi, uint16_t* lo, cudaStream_t s);
 int fitting_chain_tc(Model& m, const ForceArgs& a, cudaStream_t s);
 size_t emb_tc_image_bytes();
 size_t emb_tc_image_h_bytes();

@@ -13,6 +13,7 @@
 //   warps 2-5 split A into hi/lo in shared memory (elementwise, so the swizzled layout is preserved), then
 //            the epilogue: tcgen05.ld accumulators -> bias / tanh / skip / derivative / energy -> global
 // Two CTAs share an SM (2 x 256 TMEM columns, 2 x 2 stages), so one CTA's epilogue runs under the other's MMAs.
+#include <cuda_fp16.h>
 #include "common.cuh"
 #include "tc_gemm.cuh"
 
@@ -325,9 +326,14 @@ struct L1Args {
     int M1;
 };
 
+// FP16-split operands (kind::f16, three passes, FP32 accumulate; see embedding_tc.cu): D is scaled by 256 and W1 by
+// 64 (exact powers of two) so that hi and lo stay in FP16's normal range -- |D| <= 4 (3 x 1.2)^2 ~ 52 by
+// construction (|G| <= 3, |R| <= ~1.2, at most N_sel rows), so 256 |D| < 65504 -- and the epilogue multiplies the
+// accumulator by 2^-14.  A stage holds K = 32 (two m1 values): 50 stages of 6 MMAs instead of 100.
 constexpr int kL1BN = 240, kL1ST = 4;
+constexpr float kL1DScale = 256.f, kW1Scale = 64.f;
 struct L1Smem {
-    static constexpr int kABytes = 128 * 64, kBBytes = kL1BN * 64;
+    static constexpr int kABytes = 128 * 64, kBBytes = kL1BN * 64;        // 64 B rows = 32 halfs, SWIZZLE_64B
     static constexpr int oAhi = 0, oAlo = kABytes, oBhi = 2 * kABytes, oBlo = 2 * kABytes + kBBytes;
     static constexpr int kStage = 2 * kABytes + 2 * kBBytes;               // 47104
     static constexpr int oBars = kL1ST * kStage;
@@ -355,7 +361,7 @@ l1_desc_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ L1Ar
         if (t < g.ntypes && tile >= g.tile0[t]) ty = t;
     const int m0 = (tile - g.tile0[ty]) * 128;
     const int rows_t = g.row0[ty + 1] - g.row0[ty];
-    const int nk = g.K / kTcBK;
+    const int nk = g.K / 32;                   // K = 16 m1: two m1 per stage
     const CUtensorMap* mapBhi = &maps.Bhi[ty];
     const CUtensorMap* mapBlo = &maps.Blo[ty];
 
@@ -379,13 +385,13 @@ l1_desc_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ L1Ar
                 mbar_wait(empty + s, ph ^ 1);
                 uint8_t* st = smem + s * SM::kStage;
                 mbar_arrive_expect_tx(full + s, 2 * SM::kBBytes);
-                tma_load_2d(st + SM::oBhi, mapBhi, full + s, kb * kTcBK, 0);
-                tma_load_2d(st + SM::oBlo, mapBlo, full + s, kb * kTcBK, 0);
+                tma_load_2d(st + SM::oBhi, mapBhi, full + s, kb * 32, 0);
+                tma_load_2d(st + SM::oBlo, mapBlo, full + s, kb * 32, 0);
             }
         }
     } else if (warp == 1) {
         if (lane == 0) {
-            constexpr uint32_t idesc = make_idesc_tf32(128, BN);
+            constexpr uint32_t idesc = make_idesc_f16(128, BN);
             for (int kb = 0; kb < nk; ++kb) {
                 const int s = kb % ST, ph = (kb / ST) & 1;
                 mbar_wait(full + s, ph);
@@ -398,9 +404,9 @@ l1_desc_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ L1Ar
                     const uint64_t a_lo = make_smem_desc_kmajor(st + SM::oAlo + ks * 32, 64);
                     const uint64_t b_hi = make_smem_desc_kmajor(st + SM::oBhi + ks * 32, 64);
                     const uint64_t b_lo = make_smem_desc_kmajor(st + SM::oBlo + ks * 32, 64);
-                    umma_tf32(tmem_base, a_hi, b_hi, idesc, (kb | ks) ? 1u : 0u);
-                    umma_tf32(tmem_base, a_lo, b_hi, idesc, 1u);
-                    umma_tf32(tmem_base, a_hi, b_lo, idesc, 1u);
+                    umma_f16(tmem_base, a_hi, b_hi, idesc, (kb | ks) ? 1u : 0u);
+                    umma_f16(tmem_base, a_lo, b_hi, idesc, 1u);
+                    umma_f16(tmem_base, a_hi, b_lo, idesc, 1u);
                 }
                 umma_commit(empty + s);
             }
@@ -416,37 +422,47 @@ l1_desc_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ L1Ar
         const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
         float4 T2[16];
 #pragma unroll
-        for (int m2 = 0; m2 < 16; ++m2) T2[m2] = row_ok ? __ldg(Trow + m2) : zero4;
-        // SWIZZLE_64B K-major block: 64 B rows, 16 B chunk index XOR ((row >> 1) & 3)
+        for (int m2 = 0; m2 < 16; ++m2) {
+            T2[m2] = row_ok ? __ldg(Trow + m2) : zero4;
+            T2[m2].x *= kL1DScale; T2[m2].y *= kL1DScale; T2[m2].z *= kL1DScale; T2[m2].w *= kL1DScale;   // D x 256
+        }
+        // SWIZZLE_64B K-major block: 64 B rows (32 halfs), 16 B chunk index XOR ((row >> 1) & 3)
         const int rbase = row * 64, sw = (row >> 1) & 3;
-        float4 T1 = row_ok ? __ldg(Trow) : zero4;
+        float4 T1a = row_ok ? __ldg(Trow) : zero4, T1b = row_ok ? __ldg(Trow + 1) : zero4;
         for (int kb = 0; kb < nk; ++kb) {
             const int s = kb % ST, ph = (kb / ST) & 1;
-            const float4 T1n = (row_ok && kb + 1 < nk) ? __ldg(Trow + kb + 1) : zero4;
-            float d[16];
+            const bool more = row_ok && kb + 1 < nk;
+            const float4 T1an = more ? __ldg(Trow + 2 * kb + 2) : zero4, T1bn = more ? __ldg(Trow + 2 * kb + 3) : zero4;
+            uint32_t hi[16], lo[16];                            // 32 halfs each, packed in pairs
 #pragma unroll
-            for (int m2 = 0; m2 < 16; ++m2) d[m2] = T1.x * T2[m2].x + T1.y * T2[m2].y + T1.z * T2[m2].z + T1.w * T2[m2].w;
+            for (int q = 0; q < 16; ++q) {                      // K index 2q, 2q+1: m1 = 2 kb + (q >> 3), m2 = 2 (q & 7) ..
+                const float4 T1 = (q < 8) ? T1a : T1b;
+                const int m2 = 2 * (q & 7);
+                const float d0 = T1.x * T2[m2].x + T1.y * T2[m2].y + T1.z * T2[m2].z + T1.w * T2[m2].w;
+                const float d1 = T1.x * T2[m2 + 1].x + T1.y * T2[m2 + 1].y + T1.z * T2[m2 + 1].z + T1.w * T2[m2 + 1].w;
+                const __half2 h = __floats2half2_rn(d0, d1);
+                const float2 hf = __half22float2(h);
+                const __half2 l = __floats2half2_rn(d0 - hf.x, d1 - hf.y);
+                hi[q] = *reinterpret_cast<const uint32_t*>(&h);
+                lo[q] = *reinterpret_cast<const uint32_t*>(&l);
+            }
             mbar_wait(empty + s, ph ^ 1);                       // the MMAs that read this stage have retired
             uint8_t* st = smem + s * SM::kStage;
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
-                float4 hi, lo;
-                hi.x = __uint_as_float(__float_as_uint(d[4 * c]) & 0xFFFFE000u); lo.x = d[4 * c] - hi.x;
-                hi.y = __uint_as_float(__float_as_uint(d[4 * c + 1]) & 0xFFFFE000u); lo.y = d[4 * c + 1] - hi.y;
-                hi.z = __uint_as_float(__float_as_uint(d[4 * c + 2]) & 0xFFFFE000u); lo.z = d[4 * c + 2] - hi.z;
-                hi.w = __uint_as_float(__float_as_uint(d[4 * c + 3]) & 0xFFFFE000u); lo.w = d[4 * c + 3] - hi.w;
                 const int off = rbase + ((c ^ sw) << 4);
-                *reinterpret_cast<float4*>(st + SM::oAhi + off) = hi;
-                *reinterpret_cast<float4*>(st + SM::oAlo + off) = lo;
+                *reinterpret_cast<uint4*>(st + SM::oAhi + off) = make_uint4(hi[4 * c], hi[4 * c + 1], hi[4 * c + 2], hi[4 * c + 3]);
+                *reinterpret_cast<uint4*>(st + SM::oAlo + off) = make_uint4(lo[4 * c], lo[4 * c + 1], lo[4 * c + 2], lo[4 * c + 3]);
             }
             fence_proxy_async_smem();
             mbar_arrive(ready + s);
-            T1 = T1n;
+            T1a = T1an; T1b = T1bn;
         }
-        // ---- epilogue: Y1 = tanh(acc + b1) ----
+        // ---- epilogue: Y1 = tanh(acc 2^-14 + b1) ----
         mbar_wait(tmem_full, 0);
         tc_fence_after();
         float* orow = g.out + m * g.ldo;
+        constexpr float kInv = 1.f / (kL1DScale * kW1Scale);
 #pragma unroll 1
         for (int c = 0; c < BN / 16; ++c) {
             uint32_t v[16];
@@ -456,7 +472,7 @@ l1_desc_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ L1Ar
             const float* bias = g.bias[ty] + c * 16;
             float r[16];
 #pragma unroll
-            for (int q = 0; q < 16; ++q) r[q] = tanh_fast(__uint_as_float(v[q]) + __ldg(bias + q));
+            for (int q = 0; q < 16; ++q) r[q] = tanh_fast(fmaf(__uint_as_float(v[q]), kInv, __ldg(bias + q)));
 #pragma unroll
             for (int q = 0; q < 4; ++q)
                 reinterpret_cast<float4*>(orow + c * 16)[q] = make_float4(r[4 * q], r[4 * q + 1], r[4 * q + 2], r[4 * q + 3]);
@@ -681,6 +697,35 @@ bool tc_make_map(CUtensorMap* map, const float* base, uint64_t rows, uint64_t co
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// row-major FP16 matrix [rows][cols] with leading dimension ld (halfs); box = 32 halfs x box_rows, SWIZZLE_64B;
+// columns past `cols` read as zero (the K = 240 operands are walked in 8 blocks of 32)
+bool tc_make_map_h(CUtensorMap* map, const uint16_t* base, uint64_t rows, uint64_t cols, uint64_t ld, uint32_t box_rows) {
+    EncodeTiledFn enc = get_encode();
+    if (!enc) return false;
+    cuuint64_t dims[2] = {cols, rows};
+    cuuint64_t strides[1] = {ld * 2};
+    cuuint32_t box[2] = {32, box_rows};
+    cuuint32_t estr[2] = {1, 1};
+    return enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, const_cast<uint16_t*>(base), dims, strides, box, estr,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// FP16 split of scale * w: hi = fp16(v), lo = fp16(v - hi)
+__global__ void split_hi_lo_h_kernel(size_t n, const float* __restrict__ w, float scale, __half* __restrict__ hi,
+                                     __half* __restrict__ lo) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float v = w[i] * scale;
+    const __half h = __float2half_rn(v);
+    hi[i] = h;
+    lo[i] = __float2half_rn(v - __half2float(h));
+}
+void tc_split_weights_h(size_t n, const float* w, float scale, uint16_t* hi, uint16_t* lo, cudaStream_t s) {
+    split_hi_lo_h_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(n, w, scale, reinterpret_cast<__half*>(hi),
+                                                                      reinterpret_cast<__half*>(lo));
+}
+
 // w = hi + lo, hi = top 10 mantissa bits (what kind::tf32 reads), lo the exact remainder
 __global__ void split_hi_lo_kernel(size_t n, const float* __restrict__ w, float* __restrict__ hi, float* __restrict__ lo) {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -752,6 +797,12 @@ bool tc_setup_maps(Model& m, int ntypes) {
         ok &= tc_make_map(&m.mapA_Y2[t], m.Y2 + row0 * NF, rows, NF, NF, 128);
         ok &= tc_make_map(&m.mapA_G1[t], m.G1 + row0 * NF, rows, NF, NF, 128);
         ok &= tc_make_map(&m.mapA_G2[t], m.G2 + row0 * NF, rows, NF, NF, 128);
+        ok &= tc_make_map_h(&m.mapAh_G1[t], reinterpret_cast<const uint16_t*>(m.G1) + row0 * NF, rows, NF, NF, 128);
+        ok &= tc_make_map_h(&m.mapAh_G2[t], reinterpret_cast<const uint16_t*>(m.G2) + row0 * NF, rows, NF, NF, 128);
+        ok &= tc_make_map_h(&m.mapBh_l1_hi[t], m.w1T_h_hi[t], NF, ND, ND, 240);
+        ok &= tc_make_map_h(&m.mapBh_l1_lo[t], m.w1T_h_lo[t], NF, ND, ND, 240);
+        ok &= tc_make_map_h(&m.mapBh_dd_hi[t], m.w1_h_hi[t], ND, NF, NF, 160);
+        ok &= tc_make_map_h(&m.mapBh_dd_lo[t], m.w1_h_lo[t], ND, NF, NF, 160);
         ok &= tc_make_map(&m.mapA_T3[t], m.T3 + row0 * NF, rows, NF, NF, 128);
         for (int l = 0; l < 3; ++l) {
             const uint64_t nin = (l == 0) ? ND : NF;
@@ -788,7 +839,7 @@ static void chain_range(Model& m, const ForceArgs& fa, int t0, int ntl, cudaStre
         a1.ntypes = nt; a1.K = ND; a1.Tm = m.Tm; a1.out = m.Y1; a1.ldo = NF; a1.M1 = m.M1;
         for (int t = 0; t <= kMaxT; ++t) { a1.tile0[t] = g.tile0[t]; a1.row0[t] = g.row0[t]; }
         for (int t = 0; t < nt; ++t) a1.bias[t] = m.fit_b[t][0];
-        gather_maps(mp, m.mapA_D, m.mapB_fwd_hi, m.mapB_fwd_lo, 0, nt);
+        for (int t = 0; t < kMaxT; ++t) { const int q = t < nt ? t : 0; mp.A[t] = m.mapA_D[q]; mp.Bhi[t] = m.mapBh_l1_hi[q]; mp.Blo[t] = m.mapBh_l1_lo[q]; }
         l1_desc_kernel<<<ntl, kTcThreads, L1Smem::kTotal, s>>>(mp, a1);
     }
     // layer 2: T2 = tanh(Y1 W2 + b2); Y2 = Y1 + T2
