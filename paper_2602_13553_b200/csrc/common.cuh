@@ -119,6 +119,7 @@ struct Model {
     CUtensorMap mapBh_l1_hi[PIMD_MAX_TYPES], mapBh_l1_lo[PIMD_MAX_TYPES];     // layer-1 forward B
     CUtensorMap mapBh_dd_hi[PIMD_MAX_TYPES], mapBh_dd_lo[PIMD_MAX_TYPES];     // dD GEMM B
     CUtensorMap mapAh_G1[PIMD_MAX_TYPES], mapAh_G2[PIMD_MAX_TYPES];           // da1 as FP16 hi / lo (x bwd_scale)
+    uint16_t* da1_h_hi = nullptr, *da1_h_lo = nullptr;   // [rows][240] halfs, carved out of D
     float    bwd_scale = 1.f;          // power of two that brings the backward activations to O(1..16)
     // tensor-core embedding path (embedding_tc.cu)
     bool     use_tc_emb = true;

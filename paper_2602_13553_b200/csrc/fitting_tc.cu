@@ -44,6 +44,7 @@ struct TcGemmArgs {
     const float* tt; int ldtt;
     float* out0; float* out1; int ldo;
     const int* cen_idx; double* Eatom; double* U; int natoms;    // TEPI_L3E
+    float scale;                    // TEPI_BWD_FIRST: da1 is stored as FP16 hi / lo of scale * da1
 };
 
 constexpr int kTcThreads = 192;
@@ -257,14 +258,18 @@ gemm3xtf32_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ T
                         if (EPI == TEPI_BWD_VEC) *o0 = y;
                         y.x *= (1.f - tq.x * tq.x); y.y *= (1.f - tq.y * tq.y);
                         y.z *= (1.f - tq.z * tq.z); y.w *= (1.f - tq.w * tq.w);
-                        if (EPI == TEPI_BWD_FIRST) {     // da1 feeds dd_dt_kernel only: written pre-split (hi -> out1, lo -> out0)
-                            float4 hi;
-                            hi.x = __uint_as_float(__float_as_uint(y.x) & 0xFFFFE000u);
-                            hi.y = __uint_as_float(__float_as_uint(y.y) & 0xFFFFE000u);
-                            hi.z = __uint_as_float(__float_as_uint(y.z) & 0xFFFFE000u);
-                            hi.w = __uint_as_float(__float_as_uint(y.w) & 0xFFFFE000u);
-                            *o1 = hi;
-                            *o0 = make_float4(y.x - hi.x, y.y - hi.y, y.z - hi.z, y.w - hi.w);
+                        if (EPI == TEPI_BWD_FIRST) {
+                            // da1 feeds dd_dt_kernel only: stored as FP16 hi (-> out1) / lo (-> out0) of scale * da1,
+                            // [rows][240] halfs (the power-of-two scale keeps the values in FP16's normal range)
+                            const __half2 h01 = __floats2half2_rn(y.x * g.scale, y.y * g.scale);
+                            const __half2 h23 = __floats2half2_rn(y.z * g.scale, y.w * g.scale);
+                            const float2 f01 = __half22float2(h01), f23 = __half22float2(h23);
+                            const __half2 l01 = __floats2half2_rn(y.x * g.scale - f01.x, y.y * g.scale - f01.y);
+                            const __half2 l23 = __floats2half2_rn(y.z * g.scale - f23.x, y.w * g.scale - f23.y);
+                            __half* ph = reinterpret_cast<__half*>(g.out1) + mrow[j] * g.ldo + n + lc;
+                            __half* pl = reinterpret_cast<__half*>(g.out0) + mrow[j] * g.ldo + n + lc;
+                            *reinterpret_cast<uint2*>(ph) = make_uint2(*reinterpret_cast<const uint32_t*>(&h01), *reinterpret_cast<const uint32_t*>(&h23));
+                            *reinterpret_cast<uint2*>(pl) = make_uint2(*reinterpret_cast<const uint32_t*>(&l01), *reinterpret_cast<const uint32_t*>(&l23));
                         } else {
                             *o1 = y;
                         }
@@ -499,6 +504,7 @@ struct DdDtArgs {
     const float* Tm;      // [rows][100][4]
     float* dTm;           // [rows][100][4]
     int M1;               // 100
+    float inv_scale;      // 1 / (bwd_scale x W1 scale): the operands are FP16-split images of scaled values
 };
 
 // A (= da1) arrives pre-split as well (the producing epilogue writes hi and lo), so nothing stands between TMA
@@ -539,7 +545,7 @@ dd_dt_kernel(const __grid_constant__ DdMaps maps, const __grid_constant__ DdDtAr
         if (t < g.ntypes && tile >= g.tile0[t]) ty = t;
     const int m0 = (tile - g.tile0[ty]) * 128;
     const int rows_t = g.row0[ty + 1] - g.row0[ty];
-    const int nk = g.K / kTcBK, nch = g.nchunks;
+    const int nk = (g.K + 31) / 32, nch = g.nchunks;    // K blocks of 32 halfs; the last one is zero-filled past K
 
     if (warp == 0 && lane == 0) {
         tma_prefetch_desc(&maps.Ahi[ty]);
@@ -564,15 +570,15 @@ dd_dt_kernel(const __grid_constant__ DdMaps maps, const __grid_constant__ DdDtAr
                 mbar_wait(empty + s, ph ^ 1);
                 uint8_t* st = smem + s * SM::kStage;
                 mbar_arrive_expect_tx(full + s, 2 * SM::kABytes + 2 * SM::kBBytes);
-                tma_load_2d(st + SM::oAhi, &maps.Ahi[ty], full + s, kb * kTcBK, m0);
-                tma_load_2d(st + SM::oAlo, &maps.Alo[ty], full + s, kb * kTcBK, m0);
-                tma_load_2d(st + SM::oBhi, &maps.Bhi[ty], full + s, kb * kTcBK, nc * BN);
-                tma_load_2d(st + SM::oBlo, &maps.Blo[ty], full + s, kb * kTcBK, nc * BN);
+                tma_load_2d(st + SM::oAhi, &maps.Ahi[ty], full + s, kb * 32, m0);
+                tma_load_2d(st + SM::oAlo, &maps.Alo[ty], full + s, kb * 32, m0);
+                tma_load_2d(st + SM::oBhi, &maps.Bhi[ty], full + s, kb * 32, nc * BN);
+                tma_load_2d(st + SM::oBlo, &maps.Blo[ty], full + s, kb * 32, nc * BN);
             }
         }
     } else if (warp == 1) {
         if (lane == 0) {
-            constexpr uint32_t idesc = make_idesc_tf32(128, BN);
+            constexpr uint32_t idesc = make_idesc_f16(128, BN);
             for (int nc = 0; nc < nch; ++nc) {
                 const int buf = nc & 1;
                 if (nc >= 2) {                     // the epilogue has drained this buffer (chunk nc - 2)
@@ -592,9 +598,9 @@ dd_dt_kernel(const __grid_constant__ DdMaps maps, const __grid_constant__ DdDtAr
                         const uint64_t a_lo = make_smem_desc_kmajor(st + SM::oAlo + ks * 32, 64);
                         const uint64_t b_hi = make_smem_desc_kmajor(st + SM::oBhi + ks * 32, 64);
                         const uint64_t b_lo = make_smem_desc_kmajor(st + SM::oBlo + ks * 32, 64);
-                        umma_tf32(dcol, a_hi, b_hi, idesc, (kb | ks) ? 1u : 0u);
-                        umma_tf32(dcol, a_lo, b_hi, idesc, 1u);
-                        umma_tf32(dcol, a_hi, b_lo, idesc, 1u);
+                        umma_f16(dcol, a_hi, b_hi, idesc, (kb | ks) ? 1u : 0u);
+                        umma_f16(dcol, a_lo, b_hi, idesc, 1u);
+                        umma_f16(dcol, a_hi, b_lo, idesc, 1u);
                     }
                     umma_commit(empty + s);
                 }
@@ -637,7 +643,7 @@ dd_dt_kernel(const __grid_constant__ DdMaps maps, const __grid_constant__ DdDtAr
                 float4 accA = zero4;
 #pragma unroll
                 for (int m2 = 0; m2 < 16; ++m2) {
-                    const float d = __uint_as_float(v[m2]);
+                    const float d = __uint_as_float(v[m2]) * g.inv_scale;
                     const float4 T2 = T2s[m2 * 128];
                     accA.x = fmaf(d, T2.x, accA.x); accA.y = fmaf(d, T2.y, accA.y);
                     accA.z = fmaf(d, T2.z, accA.z); accA.w = fmaf(d, T2.w, accA.w);
@@ -788,6 +794,13 @@ bool tc_setup_maps(Model& m, int ntypes) {
     const int NF = m.NF, ND = m.ND;
     if (NF != 240 || ND % 160 != 0) return false;
     bool ok = true;
+    {   // da1 as FP16 hi / lo lives in D's storage (D is not materialised on this path); buffers of its own, because
+        // the tile ranges of the chain run on different streams and a half-precision row r does not alias row r of
+        // a float buffer
+        const size_t S = (size_t)m.type_row0[ntypes] * NF;
+        m.da1_h_hi = reinterpret_cast<uint16_t*>(m.D);
+        m.da1_h_lo = m.da1_h_hi + S;
+    }
     for (int t = 0; t < ntypes; ++t) {
         const uint64_t row0 = m.type_row0[t];
         uint64_t rows = m.type_row0[t + 1] - m.type_row0[t];
@@ -797,8 +810,8 @@ bool tc_setup_maps(Model& m, int ntypes) {
         ok &= tc_make_map(&m.mapA_Y2[t], m.Y2 + row0 * NF, rows, NF, NF, 128);
         ok &= tc_make_map(&m.mapA_G1[t], m.G1 + row0 * NF, rows, NF, NF, 128);
         ok &= tc_make_map(&m.mapA_G2[t], m.G2 + row0 * NF, rows, NF, NF, 128);
-        ok &= tc_make_map_h(&m.mapAh_G1[t], reinterpret_cast<const uint16_t*>(m.G1) + row0 * NF, rows, NF, NF, 128);
-        ok &= tc_make_map_h(&m.mapAh_G2[t], reinterpret_cast<const uint16_t*>(m.G2) + row0 * NF, rows, NF, NF, 128);
+        ok &= tc_make_map_h(&m.mapAh_G1[t], m.da1_h_hi + row0 * NF, rows, NF, NF, 128);
+        ok &= tc_make_map_h(&m.mapAh_G2[t], m.da1_h_lo + row0 * NF, rows, NF, NF, 128);
         ok &= tc_make_map_h(&m.mapBh_l1_hi[t], m.w1T_h_hi[t], NF, ND, ND, 240);
         ok &= tc_make_map_h(&m.mapBh_l1_lo[t], m.w1T_h_lo[t], NF, ND, ND, 240);
         ok &= tc_make_map_h(&m.mapBh_dd_hi[t], m.w1_h_hi[t], ND, NF, NF, 160);
@@ -859,20 +872,20 @@ static void chain_range(Model& m, const ForceArgs& fa, int t0, int ntl, cudaStre
     gather_maps(mp, m.mapA_G1, m.mapB_bwd_hi, m.mapB_bwd_lo, 2, nt);
     tc_gemm(TEPI_BWD_VEC, 240, mp, g, ntl, s);
     // dy1 = dy2 + da2 W2^T ; da1 = dy1 o (1 - y1^2) -> G1                (A = T3 = da2)
-    g = base(); g.N = NF; g.K = NF; g.add = m.Y3; g.ldadd = NF; g.tt = m.Y1; g.ldtt = NF; g.out1 = m.G1; g.out0 = m.G2; g.ldo = NF;
+    g = base(); g.N = NF; g.K = NF; g.add = m.Y3; g.ldadd = NF; g.tt = m.Y1; g.ldtt = NF; g.out1 = reinterpret_cast<float*>(m.da1_h_hi); g.out0 = reinterpret_cast<float*>(m.da1_h_lo); g.ldo = NF; g.scale = m.bwd_scale;
     gather_maps(mp, m.mapA_T3, m.mapB_bwd_hi, m.mapB_bwd_lo, 1, nt);
     tc_gemm(TEPI_BWD_FIRST, 240, mp, g, ntl, s);
     // dD = da1 W1^T contracted with T on the fly -> dT                   (A = G1 = da1)
     {
         DdDtArgs d{};
         d.tile_off = t0;
-        d.ntypes = nt; d.K = NF; d.nchunks = ND / kDdBN; d.Tm = m.Tm; d.dTm = m.dTm; d.M1 = m.M1;
+        d.ntypes = nt; d.K = NF; d.nchunks = ND / kDdBN; d.Tm = m.Tm; d.dTm = m.dTm; d.M1 = m.M1; d.inv_scale = 1.f / (m.bwd_scale * kW1Scale);
         for (int t = 0; t <= kMaxT; ++t) { d.tile0[t] = g.tile0[t]; d.row0[t] = g.row0[t]; }
         DdMaps dm;
         for (int t = 0; t < kMaxT; ++t) {
             const int q = t < nt ? t : 0;
-            dm.Ahi[t] = m.mapA_G1[q]; dm.Alo[t] = m.mapA_G2[q];
-            dm.Bhi[t] = m.mapB_bwd_hi[q][0]; dm.Blo[t] = m.mapB_bwd_lo[q][0];
+            dm.Ahi[t] = m.mapAh_G1[q]; dm.Alo[t] = m.mapAh_G2[q];
+            dm.Bhi[t] = m.mapBh_dd_hi[q]; dm.Blo[t] = m.mapBh_dd_lo[q];
         }
         dd_dt_kernel<<<ntl, kTcThreads, DdSmem::kTotal, s>>>(dm, d);
     }
