@@ -128,7 +128,6 @@ size_t model_bytes(const pimd_ctx* c, const pimd_model_desc* d) {
     b += 2 * align_up(PN * M1 * 16, 256);
     b += 2 * align_up(PN * ND * 4, 256);
     b += 7 * align_up(PN * NF * 4, 256);
-    b += align_up((size_t)d->n_types * d->n_types * emb_tc_image_bytes(), 256);               // tensor-core embedding
     b += align_up((size_t)d->n_types * d->n_types * emb_tc_image_h_bytes(), 256);
     b += align_up((size_t)d->n_types * (PN + 1) * 4, 256) + align_up(PN * nsel * 4, 256);
     b += align_up((size_t)d->n_types * ((PN + 1023) / 1024) * 4, 256) + align_up(PN * 72, 256);
@@ -473,11 +472,6 @@ int pimd_set_model(pimd_ctx* ctx, const pimd_model_desc* d, const double* w, siz
     m.emb_stride = (ob3 + M1 + 3) / 4 * 4;
     std::vector<float> ew((size_t)nt * nt * m.emb_stride, 0.f);
     size_t pos = 0;
-    std::vector<uint8_t> img((size_t)nt * nt * emb_tc_image_bytes());
-    {
-        const size_t per_pair = (size_t)2 * E1 + (size_t)E1 * E2 + E2 + (size_t)E2 * M1 + M1;
-        for (int q = 0; q < nt * nt; ++q) emb_tc_build_image(w + q * per_pair, img.data() + (size_t)q * emb_tc_image_bytes());
-    }
     for (int ti = 0; ti < nt; ++ti)
         for (int tj = 0; tj < nt; ++tj) {
             float* o = ew.data() + (size_t)(ti * nt + tj) * m.emb_stride;
@@ -498,8 +492,6 @@ int pimd_set_model(pimd_ctx* ctx, const pimd_model_desc* d, const double* w, siz
         }
     if ((rc = arena_alloc(ctx, &m.emb_w, ew.size()))) return rc;
     CK(cudaMemcpyAsync(m.emb_w, ew.data(), ew.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
-    if ((rc = arena_alloc(ctx, &m.emb_img, img.size()))) return rc;
-    CK(cudaMemcpyAsync(m.emb_img, img.data(), img.size(), cudaMemcpyHostToDevice, ctx->stream));
     std::vector<uint8_t> img_h((size_t)nt * nt * emb_tc_image_h_bytes());
     {
         const size_t per_pair = (size_t)2 * E1 + (size_t)E1 * E2 + E2 + (size_t)E2 * M1 + M1;

@@ -124,8 +124,7 @@ struct Model {
     // tensor-core embedding path (embedding_tc.cu)
     bool     use_tc_emb = true;
     bool     tc_emb_ready = false;
-    uint8_t* emb_img_h = nullptr;      // [ntypes*ntypes][emb_tc_image_h_bytes()] FP16-split images (forward kernel)
-    uint8_t* emb_img = nullptr;        // [ntypes*ntypes][emb_tc_image_bytes()] shared-memory images of the nets
+    uint8_t* emb_img_h = nullptr;      // [ntypes*ntypes][emb_tc_image_h_bytes()] FP16-split shared-memory images of the nets
     int*     rowstart = nullptr;       // [ntypes][PN+1] exclusive scan of ncount[.][tj] over type-sorted centres
     int*     rowaddr = nullptr;        // [PN*nsel] compact row -> slot index
     int*     row_bsum = nullptr;       // [ntypes][ceil(PN/1024)] scan block sums
@@ -152,10 +151,8 @@ bool tc_setup_maps(Model& m, int ntypes);
 void tc_split_weights(size_t n, const float* w, float* hi, float* lo, cudaStream_t s);
 void tc_split_weights_h(size_t n, const float* w, float scale, uint16_t* hi, uint16_t* lo, cudaStream_t s);
 int fitting_chain_tc(Model& m, const ForceArgs& a, cudaStream_t s);
-size_t emb_tc_image_bytes();
 size_t emb_tc_image_h_bytes();
 void emb_tc_build_image_h(const double* w_pair, uint8_t* img);
-void emb_tc_build_image(const double* w_pair, uint8_t* img);
 int emb_tc_row_index(Model& m, const ForceArgs& a, cudaStream_t s);
 int embedding_forward_tc(Model& m, const ForceArgs& a, int n_sms, cudaStream_t s);
 int embedding_backward_tc(Model& m, const ForceArgs& a, int n_sms, cudaStream_t s);
