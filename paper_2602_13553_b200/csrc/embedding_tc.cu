@@ -310,38 +310,58 @@ __device__ __forceinline__ void load_weight_image_n(uint8_t* dst, const uint8_t*
 }
 
 // -------------------------------------------------------------------------------------------------
-// F3: embedding forward + T_i
+// F3: embedding forward + T_i.  One thread per row here (it does the work of both column halves in turn; the
+// operand layout and the weight image are those of the two-threads-per-row backward kernel), 128 threads per
+// context, so THREE contexts fit the register file (384 threads x 170) and, with FP16 operands, shared memory
+// (3 x 57 KB + 37 KB).  The third context gives the tile pipeline -- tanh epilogues, MMA round trips, T
+// accumulation -- one more independent stream to overlap: 0.75 -> 0.64 ms against the two-context version.
 // -------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(etc::kThreads, 1)
+namespace f3 {
+constexpr int kCtx = 3, kThreads = 128 * kCtx;
+constexpr int oRs = 128 * etc::GROW * 4;                           // G staging (overlays the A operands), then R, centres
+constexpr int oCen = oRs + 128 * 16;
+constexpr int kCtxBytes = (oCen + 128 * 4 + 1023) / 1024 * 1024;   // 58368
+constexpr int kSmemBytes = eh::kImgPad + kCtx * kCtxBytes + 64 + 1024;
+static_assert(kSmemBytes <= 232448, "shared memory budget (3-context forward)");
+}  // namespace f3
+
+__global__ void __launch_bounds__(f3::kThreads, 1)
 embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
     using namespace etc;
     extern __shared__ uint8_t smem_raw[];
-    const CtxSetup cs = ctx_setup(smem_raw, 256);
-    const int cx = threadIdx.x >> 8, half = (threadIdx.x >> 7) & 1, t = threadIdx.x & 127, lane = threadIdx.x & 31;
-    const int bar_ctx = 1 + cx, bar_pair = 3 + cx * 4 + (t >> 5);
-    uint8_t* ctx = cs.ctx;
-    float4* Rs = reinterpret_cast<float4*>(ctx + oRs);
-    int* cen_s = reinterpret_cast<int*>(ctx + oCen);
+    uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+    const int cx = threadIdx.x >> 7, t = threadIdx.x & 127, lane = threadIdx.x & 31;
+    uint8_t* ctx = smem + eh::kImgPad + cx * f3::kCtxBytes;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + eh::kImgPad + f3::kCtx * f3::kCtxBytes);
+    uint64_t* mma_bar = bars + cx;
+    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(bars + 4);
+    if (threadIdx.x == 0) {
+        for (int q = 0; q < f3::kCtx; ++q) mbar_init(bars + q, 1);
+        fence_barrier_init();
+    }
+    if ((threadIdx.x >> 5) == 0) tmem_alloc(tmem_ptr, 512);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_d = *tmem_ptr + cx * 128;
+    const int bar_ctx = 1 + cx;
+    float4* Rs = reinterpret_cast<float4*>(ctx + f3::oRs);
+    int* cen_s = reinterpret_cast<int*>(ctx + f3::oCen);
     float* Gs = reinterpret_cast<float*>(ctx);
-    const float* W1s = reinterpret_cast<const float*>(cs.smem + eh::oW1) + H1 * half;
+    const float* W1s = reinterpret_cast<const float*>(smem + eh::oW1);
     const float* b1s = W1s + 32;
-    const uint32_t tmem_d = cs.tmem_base + cx * 128;
     const uint32_t lanefield = ((uint32_t)((t >> 5) * 32)) << 16;
-    const uint32_t actx = smem_u32(ctx), wbase = smem_u32(cs.smem);
+    const uint32_t actx = smem_u32(ctx), wbase = smem_u32(smem);
     constexpr uint32_t idesc2 = make_idesc_f16(128, eh::N2), idesc3 = make_idesc_f16(128, eh::N3);
     uint32_t phase = 0;
     const int nt = a.ntypes;
-    // T accumulation: lane <-> staged G positions 4 lane .. 4 lane + 3 (26 lanes); their original channels
-    int mo[4];
+    int mo[4];                                             // original channels of staged positions 4 lane .. + 3
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
         const int ps = (4 * lane + j) % (2 * H3);
         mo[j] = g_orig(ps / H3, ps % H3);
     }
 
-    // Work split: the row tiles of all (t_i, t_j) pairs form one list; CTA b takes the contiguous share
-    // [T b / G, T (b+1) / G) of it (balanced to one tile; most CTAs see a single pair, so they load one weight
-    // image and the two contexts are de-phased once), and its two contexts halve every pair's sub-range.
     int tile_total = 0, sub_lo = 0, sub_hi = 0;
     for (int p = 0; p < nt * nt; ++p) {
         const int ti = p / nt, tj = p - ti * nt;
@@ -361,19 +381,23 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
             if (lo >= hi) continue;                        // CTA-uniform: no tile of this pair is mine
             sub_lo = lo; sub_hi = hi;
         }
-        __syncthreads();                                   // both contexts are done with the previous weights
-        load_weight_image_n(cs.smem, a.wimg_h + (size_t)p * eh::kImgBytes, eh::kImgBytes);
+        __syncthreads();                                   // all contexts are done with the previous weights
+        {
+            const float4* s4 = reinterpret_cast<const float4*>(a.wimg_h + (size_t)p * eh::kImgBytes);
+            float4* d4 = reinterpret_cast<float4*>(smem);
+            for (int q = threadIdx.x; q < eh::kImgBytes / 16; q += f3::kThreads) d4[q] = __ldg(s4 + q);
+            fence_proxy_async_smem();
+        }
         __syncthreads();
         const int* rs = a.rowstart + (size_t)tj * (a.PN + 1);
         const int begin = rs[a.type_row0[ti]], end = rs[a.type_row0[ti + 1]];
-        const int tl0 = sub_lo + (sub_hi - sub_lo) * cx / 2, tl1 = sub_lo + (sub_hi - sub_lo) * (cx + 1) / 2;
+        const int tl0 = sub_lo + (sub_hi - sub_lo) * cx / f3::kCtx, tl1 = sub_lo + (sub_hi - sub_lo) * (cx + 1) / f3::kCtx;
         if (tl0 >= tl1) continue;
-        if (cx == 1 && a.skew_fwd > 0) {                    // de-phase the two contexts (see the backward kernel)
+        if (cx > 0 && a.skew_fwd > 0) {                     // de-phase the contexts
             const long long t0 = clock64();
-            while (clock64() - t0 < a.skew_fwd) __nanosleep(200);
+            while (clock64() - t0 < (long long)a.skew_fwd * cx) __nanosleep(200);
         }
         const int* raddr = a.rowaddr + (size_t)a.PN * a.seloff[tj];
-        // software pipeline: slot index two tiles ahead, row data one tile ahead
         auto addr_of = [&](int tile) -> int {
             const int g = begin + tile * 128 + t;
             return (tile < tl1 && g < end) ? __ldg(raddr + g) : -1;
@@ -385,124 +409,116 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
             const int addr_n2 = addr_of(tile + 2);
             const RowIn nxt = load_row(a, addr_n1);
             addr_n1 = addr_n2;
-
             const float s = cur.s;
-            if (half == 0) {
+            {
                 const float sr = cur.s * cur.rinv;
                 Rs[t] = make_float4(s, sr * cur.dx, sr * cur.dy, sr * cur.dz);
                 cen_s[t] = cur.cen;
             }
-            // ---- layer 1 on CUDA cores: my 13 channels -> K slots 16 half .. 16 half + 15 of A1 ----
-            float h1[H1];
+            // ---- layer 1: both halves' 13 channels -> A1 (64 B rows): K slots 0..15 and 16..31 ----
+            float h1[2][H1];
 #pragma unroll
-            for (int i = 0; i < H1; ++i) h1[i] = tanh_fast(fmaf(s, W1s[i], b1s[i]));
-            {
-                // FP16 A1 (64 B rows): my 13 channels + the bias slot (k = 13, half A only) = K slots 16 half .. + 15
+            for (int h = 0; h < 2; ++h) {
                 float v16[16];
 #pragma unroll
-                for (int i = 0; i < H1; ++i) v16[i] = h1[i];
-                v16[13] = half ? 0.f : 1.f; v16[14] = 0.f; v16[15] = 0.f;
-                store_chunk_h<64>(ctx + eh::oA1hi, ctx + eh::oA1lo, t, 2 * half, v16);
-                store_chunk_h<64>(ctx + eh::oA1hi, ctx + eh::oA1lo, t, 2 * half + 1, v16 + 8);
+                for (int i = 0; i < H1; ++i) { h1[h][i] = tanh_fast(fmaf(s, W1s[H1 * h + i], b1s[H1 * h + i])); v16[i] = h1[h][i]; }
+                v16[13] = h ? 0.f : 1.f; v16[14] = 0.f; v16[15] = 0.f;
+                store_chunk_h<64>(ctx + eh::oA1hi, ctx + eh::oA1lo, t, 2 * h, v16);
+                store_chunk_h<64>(ctx + eh::oA1hi, ctx + eh::oA1lo, t, 2 * h + 1, v16 + 8);
             }
             fence_proxy_async_smem();
             tc_fence_before();
-            named_bar_sync(bar_ctx, 256);
-            if ((threadIdx.x & 255) == 0) {
+            named_bar_sync(bar_ctx, 128);
+            if (t == 0) {
                 tc_fence_after();
                 mma_3x_f16<64>(tmem_d, actx + eh::oA1hi, actx + eh::oA1lo, wbase + eh::oW2hi, wbase + eh::oW2lo, idesc2, 2);
-                umma_commit(cs.mma_bar);
+                umma_commit(mma_bar);
             }
-            mbar_wait(cs.mma_bar, phase);
+            mbar_wait(mma_bar, phase);
             phase ^= 1;
             tc_fence_after();
-            // ---- epilogue 2: h2 = [h1,h1] + tanh(z2), my 26 columns; A2 K slots 28 half .. 28 half + 27 ----
-            float h2[H2];
-            {
+            // ---- epilogue 2: h2 = [h1,h1] + tanh(z2) -> A2 (128 B rows): K slots 0..31 and 32..63 ----
+            float h2[2][H2];
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
                 uint32_t v[H2];
-                const uint32_t col = tmem_d + lanefield + 32 * half;
+                const uint32_t col = tmem_d + lanefield + 32 * h;
                 tmem_ld16(col, v);
                 tmem_ld8(col + 16, v + 16);
                 tmem_ld2(col + 24, v + 24);
                 tmem_ld_wait();
-#pragma unroll
-                for (int j = 0; j < H2; ++j) h2[j] = h1[j % H1] + tanh_fast(__uint_as_float(v[j]));
-                // FP16 A2 (128 B rows): my 26 channels + the bias slot (k = 26, half A only) = K slots 32 half .. + 31
                 float v32[32];
 #pragma unroll
-                for (int j = 0; j < H2; ++j) v32[j] = h2[j];
-                v32[26] = half ? 0.f : 1.f;
+                for (int j = 0; j < H2; ++j) { h2[h][j] = h1[h][j % H1] + tanh_fast(__uint_as_float(v[j])); v32[j] = h2[h][j]; }
+                v32[26] = h ? 0.f : 1.f;
 #pragma unroll
                 for (int j = 27; j < 32; ++j) v32[j] = 0.f;
 #pragma unroll
                 for (int cq = 0; cq < 4; ++cq)
-                    store_chunk_h<128>(ctx + eh::oA2hi, ctx + eh::oA2lo, t, 4 * half + cq, v32 + 8 * cq);
+                    store_chunk_h<128>(ctx + eh::oA2hi, ctx + eh::oA2lo, t, 4 * h + cq, v32 + 8 * cq);
             }
             fence_proxy_async_smem();
             tc_fence_before();
-            named_bar_sync(bar_ctx, 256);
-            if ((threadIdx.x & 255) == 0) {
+            named_bar_sync(bar_ctx, 128);
+            if (t == 0) {
                 tc_fence_after();
                 mma_3x_f16<128>(tmem_d, actx + eh::oA2hi, actx + eh::oA2lo, wbase + eh::oW3hi, wbase + eh::oW3lo, idesc3, 4);
-                umma_commit(cs.mma_bar);
+                umma_commit(mma_bar);
             }
-            mbar_wait(cs.mma_bar, phase);
+            mbar_wait(mma_bar, phase);
             phase ^= 1;
             tc_fence_after();
-            // ---- epilogue 3: G = [h2,h2] + tanh(z3), my 52 columns -> smem [row][GROW] (overlays the A region) ----
-            {
-                const uint32_t col = tmem_d + lanefield + 56 * half;
-                float* grow = Gs + t * GROW + H3 * half;
-                uint32_t v[32];
-                tmem_ld16(col, v);
-                tmem_ld16(col + 16, v + 16);
-                tmem_ld_wait();
+            // ---- epilogue 3: G = [h2,h2] + tanh(z3) -> smem [row][GROW] (overlays the A operands) ----
 #pragma unroll
-                for (int q = 0; q < 8; ++q) {
-                    float4 gq;
-                    gq.x = h2[(4 * q) % H2] + tanh_fast(__uint_as_float(v[4 * q]));
-                    gq.y = h2[(4 * q + 1) % H2] + tanh_fast(__uint_as_float(v[4 * q + 1]));
-                    gq.z = h2[(4 * q + 2) % H2] + tanh_fast(__uint_as_float(v[4 * q + 2]));
-                    gq.w = h2[(4 * q + 3) % H2] + tanh_fast(__uint_as_float(v[4 * q + 3]));
-                    *reinterpret_cast<float4*>(grow + 4 * q) = gq;
-                }
-                tmem_ld16(col + 32, v);
-                tmem_ld4(col + 48, v + 16);
-                tmem_ld_wait();
+            for (int h = 0; h < 2; ++h) {
+                const uint32_t col = tmem_d + lanefield + 56 * h;
+                float* grow = Gs + t * GROW + H3 * h;
 #pragma unroll
-                for (int q = 0; q < 5; ++q) {
-                    const int g = 32 + 4 * q;
-                    float4 gq;
-                    gq.x = h2[g % H2] + tanh_fast(__uint_as_float(v[4 * q]));
-                    gq.y = h2[(g + 1) % H2] + tanh_fast(__uint_as_float(v[4 * q + 1]));
-                    gq.z = h2[(g + 2) % H2] + tanh_fast(__uint_as_float(v[4 * q + 2]));
-                    gq.w = h2[(g + 3) % H2] + tanh_fast(__uint_as_float(v[4 * q + 3]));
-                    *reinterpret_cast<float4*>(grow + g) = gq;
+                for (int pc = 0; pc < 3; ++pc) {
+                    uint32_t v[16];
+                    tmem_ld16(col + 16 * pc, v);
+                    tmem_ld_wait();
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        const int g = 16 * pc + 4 * q;
+                        float4 gq;
+                        gq.x = h2[h][g % H2] + tanh_fast(__uint_as_float(v[4 * q]));
+                        gq.y = h2[h][(g + 1) % H2] + tanh_fast(__uint_as_float(v[4 * q + 1]));
+                        gq.z = h2[h][(g + 2) % H2] + tanh_fast(__uint_as_float(v[4 * q + 2]));
+                        gq.w = h2[h][(g + 3) % H2] + tanh_fast(__uint_as_float(v[4 * q + 3]));
+                        *reinterpret_cast<float4*>(grow + g) = gq;
+                    }
                 }
+                uint32_t v[4];
+                tmem_ld4(col + 48, v);
+                tmem_ld_wait();
+                float4 gq;
+                gq.x = h2[h][48 % H2] + tanh_fast(__uint_as_float(v[0]));
+                gq.y = h2[h][49 % H2] + tanh_fast(__uint_as_float(v[1]));
+                gq.z = h2[h][50 % H2] + tanh_fast(__uint_as_float(v[2]));
+                gq.w = h2[h][51 % H2] + tanh_fast(__uint_as_float(v[3]));
+                *reinterpret_cast<float4*>(grow + 48) = gq;
             }
             tc_fence_before();
-            named_bar_sync(bar_pair, 64);                  // the two warps of this lane quarter: G rows complete
-            // ---- T_i += (1/N_sel) sum_rows G (x) R.  The warp pair owns the 32 rows it just wrote; each warp
-            // takes 16 of them, lane <-> 4 staged G positions (26 lanes).  All lanes walk the same rows, so the
-            // centre changes are warp-uniform and the R / centre reads are broadcasts. ----
+            __syncwarp();                                  // a warp accumulates the 32 rows it has just written
+            // ---- T_i += (1/N_sel) sum_rows G (x) R: lane <-> 4 staged G positions (26 lanes) ----
             {
-                const int r_lo = (t & ~31) + 16 * half;
-                // centre boundaries inside my 16 rows (bit r set: row r starts a new centre), warp-uniform
-                const int cme = cen_s[r_lo + (lane & 15)];
+                const int r_lo = t & ~31;
+                const int cme = cen_s[r_lo + lane];
                 const int cpv = __shfl_up_sync(0xffffffffu, cme, 1);
-                const uint32_t bnd = __ballot_sync(0xffffffffu, (lane & 15) != 0 && lane < 16 && cme != cpv) & 0xffffu;
+                const uint32_t bnd = __ballot_sync(0xffffffffu, lane != 0 && cme != cpv);
                 if (lane < 26) {
                     const float* gp = Gs + r_lo * GROW + 4 * lane;
                     int r0 = 0;
-                    while (r0 < 16) {                       // one iteration per centre segment [r0, r1)
-                        const uint32_t rest = bnd >> (r0 + 1);
-                        const int r1 = rest ? r0 + __ffs(rest) : 16;
+                    while (r0 < 32) {                       // one iteration per centre segment [r0, r1)
+                        const uint32_t rest = (r0 + 1 < 32) ? (bnd >> (r0 + 1)) : 0u;
+                        const int r1 = rest ? r0 + __ffs(rest) : 32;
                         const int cn = cen_s[r_lo + r0];
                         if (cn < 0) break;                  // rows past the end of the pair (always at the tail)
                         float acc[16];
 #pragma unroll
                         for (int q = 0; q < 16; ++q) acc[q] = 0.f;
-                        auto rows = [&](auto NR, int row) {          // NR rows: all loads first, then the FMAs
+                        auto rows = [&](auto NR, int row) {
                             constexpr int nr = decltype(NR)::value;
                             float4 G4[nr], R[nr];
 #pragma unroll
@@ -535,13 +551,13 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
                     }
                 }
             }
-            named_bar_sync(bar_ctx, 256);                  // G / R / centre buffers are free again
+            named_bar_sync(bar_ctx, 128);                  // G / R / centre buffers are free again
             cur = nxt;
         }
     }
     tc_fence_before();
     __syncthreads();
-    if ((threadIdx.x >> 5) == 0) tmem_dealloc(cs.tmem_base, 256);
+    if ((threadIdx.x >> 5) == 0) tmem_dealloc(*tmem_ptr, 512);
 }
 
 // -------------------------------------------------------------------------------------------------
@@ -932,11 +948,11 @@ int embedding_forward_tc(Model& m, const ForceArgs& fa, int n_sms, cudaStream_t 
     EmbTcArgs a = make_tc_args(m, fa);
     static bool attr = false;
     if (!attr) {
-        cudaFuncSetAttribute(embed_fwd_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, etc::kSmemBytes);
+        cudaFuncSetAttribute(embed_fwd_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, f3::kSmemBytes);
         attr = true;
     }
     cudaMemsetAsync(m.Tm, 0, sizeof(float) * (size_t)a.PN * etc::M1 * 4, s);
-    embed_fwd_tc_kernel<<<n_sms, etc::kThreads, etc::kSmemBytes, s>>>(a);
+    embed_fwd_tc_kernel<<<n_sms, f3::kThreads, f3::kSmemBytes, s>>>(a);
     return 1;
 }
 
