@@ -27,8 +27,8 @@ import workloads  # noqa: E402
 
 METRIC = "bead-atom-steps/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch at configs[2], from the committed ncu --set full capture
-# (profiles/r1c_README.md); None where the phase is several kernels
-NCU_DRAM_BYTES = {"embed_fwd": 275.95e6 + 76.92e6, "embed_bwd": 308.27e6 + 10.72e6, "fitting": None}
+# (profiles/r1f_README.md); None where the phase is several kernels
+NCU_DRAM_BYTES = {"embed_fwd": 284.17e6 + 75.11e6, "embed_bwd": 309.36e6 + 11.71e6, "fitting": None}
 
 
 def _peaks():
@@ -238,32 +238,40 @@ def run_ours(args):
     names = ["integrator", "neighbour_env", "embed_fwd", "fitting", "embed_bwd"]
     phases = {n: float(phase[q]) for q, n in enumerate(names)}
     dom = max(("embed_fwd", "fitting", "embed_bwd"), key=lambda n: phases[n])
-    # tensor roofline: the path's contractions run as kind::tf32 tcgen05.mma; TF32 dense peak = the measured
-    # BF16 cuBLAS figure (sustained: these kernels are timed inside a long step) x the guide's nominal 1/2
+    # tensor roofline.  The embedding kernels and the two big fitting kernels (K = 1600 / N = 1600) run as three-pass
+    # FP16-split kind::f16 tcgen05.mma, the four 240 x 240 fitting GEMMs as 3xTF32 kind::tf32.  Peaks: FP16 dense = the
+    # measured BF16 cuBLAS figure (same tensor rate; sustained: these kernels are timed inside a long step), TF32
+    # dense = 1/2 of it (the guide's nominal ratio).
     PN = P * N
-    bf16_peak = peaks["bf16_sustained"] or peaks["bf16"]
-    tf32_peak = 0.5 * bf16_peak
+    f16_peak = peaks["bf16_sustained"] or peaks["bf16"]
+    tf32_peak = 0.5 * f16_peak
     mufu_peak = 148 * 16 * peaks["sm_max_mhz"] * 1e6 / 1e12                         # T MUFU op/s
-    issued = {                                                                       # padded tiles, 3xTF32 passes
-        "embed_fwd": 2.0 * rows * 3 * (32 * 64 + 56 * 128),                         # K2 x N2 + K3 x N3 of embedding_tc.cu
-        "embed_bwd": 2.0 * rows * 3 * 2 * (32 * 64 + 56 * 128),                     # value + derivative rows
-        "fitting": 3 * 2.0 * PN * 2 * (1600 * 240 + 2 * 240 * 240),
+    emb_issue = 2.0 * rows * 3 * (32 * 64 + 64 * 112)                               # K2 x N2 + K3 x N3 of embedding_tc.cu, 3 passes
+    issued = {   # (flops issued on padded tiles incl. the 3 passes, peak of that dtype)
+        "embed_fwd": [(emb_issue, f16_peak)],
+        "embed_bwd": [(2.0 * emb_issue, f16_peak)],                                 # value + derivative rows
+        "fitting": [(3 * 2.0 * PN * (1600 * 240 + 256 * 1600), f16_peak),           # l1_desc, dd_dt (K padded to 256)
+                    (3 * 2.0 * PN * 4 * 240 * 240, tf32_peak)],
     }
-    mufu_ops = {"embed_fwd": 2.0 * rows * 175, "embed_bwd": 2.0 * rows * 175, "fitting": 0.0}
+    mufu_ops = {"embed_fwd": 2.0 * rows * 182, "embed_bwd": 2.0 * rows * 182, "fitting": 0.0}   # incl. padded channels
+    dom_peak = f16_peak
     achieved = flops[dom] / (phases[dom] * 1e-3) / 1e12
-    roofline = {"kernel": dom, "bound": "tensor", "achieved": achieved, "peak": tf32_peak, "unit": "TFLOP/s",
-                "frac": achieved / tf32_peak, "traffic": NCU_DRAM_BYTES.get(dom),
-                "issued_tflops": issued[dom] / (phases[dom] * 1e-3) / 1e12,
-                "note": "achieved = USEFUL flops (SURVEY 8(d): no recompute, no 3xTF32 extra passes) / live CUDA-event "
-                        "time of the phase; peak = TF32 dense = %s BF16 %.0f TFLOP/s x 1/2 (guide's nominal ratio); "
-                        "issued_tflops counts the 3 TF32 passes on padded tiles" % (
-                            "measured sustained" if peaks["bf16_sustained"] else "measured burst", bf16_peak)}
+    dom_issued = sum(f for f, _ in issued[dom]) / (phases[dom] * 1e-3) / 1e12
+    roofline = {"kernel": dom, "bound": "tensor", "achieved": achieved, "peak": dom_peak, "unit": "TFLOP/s",
+                "frac": achieved / dom_peak, "traffic": NCU_DRAM_BYTES.get(dom),
+                "issued_tflops": dom_issued,
+                "note": "achieved = USEFUL flops (SURVEY 8(d): no recompute, no extra hi/lo passes, no padding) / live "
+                        "CUDA-event time of the phase; peak = FP16 dense = %s BF16 %.0f TFLOP/s (kind::f16 runs at the "
+                        "BF16 rate); issued_tflops counts the 3 passes on padded tiles" % (
+                            "measured sustained" if peaks["bf16_sustained"] else "measured burst", f16_peak)}
     kernels = {}
     for n in ("embed_fwd", "fitting", "embed_bwd"):
         sec = phases[n] * 1e-3
-        kernels[n] = {"ms": phases[n], "useful_tflops": flops[n] / sec / 1e12, "issued_tf32_tflops": issued[n] / sec / 1e12,
-                      "frac_tf32_peak_useful": flops[n] / sec / 1e12 / tf32_peak,
-                      "frac_tf32_peak_issued": issued[n] / sec / 1e12 / tf32_peak}
+        t_at_peak = sum(f / (pk_ * 1e12) for f, pk_ in issued[n])
+        kernels[n] = {"ms": phases[n], "useful_tflops": flops[n] / sec / 1e12,
+                      "issued_tflops": sum(f for f, _ in issued[n]) / sec / 1e12,
+                      "frac_tensor_peak_issued": t_at_peak / sec,
+                      "frac_tensor_peak_useful": flops[n] / sec / 1e12 / (f16_peak if n != "fitting" else f16_peak)}
         if mufu_ops[n]:
             kernels[n]["frac_mufu_peak"] = mufu_ops[n] / sec / 1e12 / mufu_peak
     kernels["integrator"] = {"ms": phases["integrator"], "algorithmic_GBs": 120.0 * P * N / (phases["integrator"] * 1e-3) / 1e9,
@@ -312,7 +320,7 @@ def run_ours(args):
         out = {
             "metric": METRIC, "value": value, "unit": METRIC, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f32 network / f64 geometry+integrator", "data": "synthetic",
+            "vs_baseline": None, "dtype": "f16-split (3-pass hi/lo, f32 accumulate) network ~ f32 / f64 geometry+integrator", "data": "synthetic",
             "config": {"workload": cfg["name"], "atoms": N, "beads": P, "bead_atoms": P * N, "neighbour_rows": rows,
                        "parallelism": "replicas only" if world > 1 else "1 GPU",
                        "l2": "no flush: per-step working set (neighbour rows 135 MB, T and dT 157 MB, fitting activations ~380 MB) exceeds the 126 MB L2"},
