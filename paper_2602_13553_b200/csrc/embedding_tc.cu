@@ -24,6 +24,7 @@
 // that one context's MMAs overlap the other's tanh / epilogue work.
 #include <cstring>
 #include <cuda_fp16.h>
+#include <cuda_pipeline.h>
 #include <type_traits>
 #include "common.cuh"
 #include "tc_gemm.cuh"
@@ -53,6 +54,8 @@ constexpr int kSmemBytes = kImgPad + 2 * kCtxBytes + 64 + 1024;  // + barriers +
 // The backward kernel keeps its contexts where they were before the weight image shrank (73 KB into the block) and
 // the largest carve-out: measured 6 % faster than the compact layout (the forward kernel is 5 % faster compact).
 constexpr int kImgPadBwd = 74752;
+constexpr int kDtBufBytes = (kImgPadBwd - kImgPad) / 2;          // per context, between the weight image and the contexts
+static_assert(kDtBufBytes >= 11 * 1600, "dT buffer");
 constexpr int kSmemBytesBwd = kImgPadBwd + 2 * kCtxBytes + 64 + 1024;
 constexpr int kThreads = 512;
 constexpr int kScanBlock = 1024;       // centres per scan block
@@ -563,7 +566,7 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
 // -------------------------------------------------------------------------------------------------
 // F5 / F6: embedding backward (forward-mode), pair gradient, force and virial
 // -------------------------------------------------------------------------------------------------
-constexpr int kDtStage = 40;          // centres whose dT fits the (free) A region: 40 x 1600 B
+constexpr int kDtStage = 11;          // centres whose dT fits the dedicated buffer: 11 x 1600 B (a tile spans 3-6)
 
 __global__ void __launch_bounds__(etc::kThreads, 1)
 embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
@@ -574,7 +577,7 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
     const int bar_ctx = 1 + cx, bar_pair = 3 + cx * 4 + (t >> 5);
     uint8_t* ctx = cs.ctx;
     int* cen_s = reinterpret_cast<int*>(ctx + oCen);
-    float4* dTs = reinterpret_cast<float4*>(ctx);
+    float4* dTs = reinterpret_cast<float4*>(cs.smem + kImgPad + cx * kDtBufBytes);   // dedicated dT buffer (cp.async target)
     float* part = reinterpret_cast<float*>(ctx + oPart) + t * 8;
     const float* W1s = reinterpret_cast<const float*>(cs.smem + eh::oW1) + H1 * half;
     const float* b1s = W1s + 32;
@@ -619,22 +622,21 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
         auto load_A = [&](int addr) -> float4 {
             return addr >= 0 ? __ldg(reinterpret_cast<const float4*>(a.slotA) + addr) : make_float4(0.f, 0.f, 0.f, 0.f);
         };
-        int addr_c = addr_of(tl0), addr_n = addr_of(tl0 + 1);
-        float4 curA = load_A(addr_c);
+        auto load_cen = [&](int addr) -> int { return addr >= 0 ? __ldg(a.row_of + addr / a.nsel) : -1; };
+        int addr_nx = addr_of(tl0), addr_n2 = addr_of(tl0 + 1);
+        float4 nxtA = load_A(addr_nx);
+        int nxtCen = load_cen(addr_nx);
 
         for (int tile = tl0; tile < tl1; ++tile) {
+            // {d, s} and the centre of my row were fetched one tile ahead; {s', 1/r, j} follow under the layer-3 MMAs
             RowIn cur;
-            cur.dx = curA.x; cur.dy = curA.y; cur.dz = curA.z; cur.s = curA.w;
-            cur.ds = 0.f; cur.rinv = 1.f; cur.jcode = 0u; cur.cen = -1; cur.ba = 0;
-            if (addr_c >= 0) {
-                const float4 B = __ldg(reinterpret_cast<const float4*>(a.slotB) + addr_c);
-                cur.ds = B.x; cur.rinv = B.y; cur.jcode = __float_as_uint(B.z);
-                cur.ba = addr_c / a.nsel;
-                cur.cen = __ldg(a.row_of + cur.ba);
-            }
-            addr_c = addr_n;
-            curA = load_A(addr_c);
-            addr_n = addr_of(tile + 2);
+            const int addr_c = addr_nx;
+            cur.dx = nxtA.x; cur.dy = nxtA.y; cur.dz = nxtA.z; cur.s = nxtA.w;
+            cur.cen = nxtCen; cur.ba = addr_c >= 0 ? addr_c / a.nsel : 0;
+            addr_nx = addr_n2;
+            nxtA = load_A(addr_nx);
+            nxtCen = load_cen(addr_nx);
+            addr_n2 = addr_of(tile + 2);
 
             const float s = cur.s;
             // ---- layer 1 and its s-derivative, my 13 channels; A1v = [h1,1,0..], A1d = [h1',0,0..] ----
@@ -699,8 +701,6 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
                 }
             }
             if (half == 0) cen_s[t] = cur.cen;
-            const float sr = cur.s * cur.rinv;
-            const float R0 = s, R1 = sr * cur.dx, R2 = sr * cur.dy, R3 = sr * cur.dz;
             fence_proxy_async_smem();
             tc_fence_before();
             named_bar_sync(bar_ctx, 256);
@@ -710,24 +710,28 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
                 mma_3x_f16<128>(tmem_g, actx + oY, actx + oY + 16384, wbase + eh::oW3hi, wbase + eh::oW3lo, idesc3, 4);
                 umma_commit(cs.mma_bar);
             }
-            // ---- dT of this tile's centres: fetched into registers while the MMAs run, then staged into the
-            // (by then free) A region ----
+            // ---- while the MMAs run: dT of this tile's centres goes global -> shared by cp.async (no registers in
+            // between), and the rest of my row arrives ----
             const int nvalid = min(128, end - (begin + tile * 128));
             const int r_lo = cen_s[0], r_hi = cen_s[nvalid - 1];
-            const int nstage = min(r_hi - r_lo + 1, kDtStage);
-            const float4* dsrc = reinterpret_cast<const float4*>(a.dTm) + (size_t)r_lo * M1;
-            const int dq = threadIdx.x & 255;
-            float4 pre[3];
-#pragma unroll
-            for (int i = 0; i < 3; ++i)
-                if (dq + 256 * i < nstage * M1) pre[i] = __ldg(dsrc + dq + 256 * i);
+            const bool staged = r_hi - r_lo < kDtStage;
+            if (staged) {
+                const float4* dsrc = reinterpret_cast<const float4*>(a.dTm) + (size_t)r_lo * M1;
+                const int nq = (r_hi - r_lo + 1) * M1;
+                for (int q = threadIdx.x & 255; q < nq; q += 256) __pipeline_memcpy_async(dTs + q, dsrc + q, 16);
+            }
+            __pipeline_commit();
+            cur.ds = 0.f; cur.rinv = 1.f; cur.jcode = 0u;
+            if (addr_c >= 0) {
+                const float4 B = __ldg(reinterpret_cast<const float4*>(a.slotB) + addr_c);
+                cur.ds = B.x; cur.rinv = B.y; cur.jcode = __float_as_uint(B.z);
+            }
+            const float sr = cur.s * cur.rinv;
+            const float R0 = s, R1 = sr * cur.dx, R2 = sr * cur.dy, R3 = sr * cur.dz;
             mbar_wait(cs.mma_bar, phase);
             phase ^= 1;
             tc_fence_after();
-#pragma unroll
-            for (int i = 0; i < 3; ++i)
-                if (dq + 256 * i < nstage * M1) dTs[dq + 256 * i] = pre[i];
-            for (int q = dq + 768; q < nstage * M1; q += 256) dTs[q] = __ldg(dsrc + q);
+            __pipeline_wait_prior(0);
             named_bar_sync(bar_ctx, 256);
             // ---- epilogue 3: contract G, G' (my 52 columns) with dT on the fly.  dT rows come from the staged
             // copy when the whole tile's centres fit (always, unless a centre has < 4 rows of this pair type);
@@ -765,7 +769,7 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
                 tmem_ld_wait();
                 piece(std::integral_constant<int, 4>{}, 48, v, d);
             };
-            if (r_hi - r_lo < kDtStage) {
+            if (staged) {
                 contract(dTs + max(cur.cen - r_lo, 0) * M1 + H1 * half);
             } else {
                 contract(reinterpret_cast<const float4*>(a.dTm) + (size_t)max(cur.cen, 0) * M1 + H1 * half);

@@ -297,6 +297,40 @@ def test_isolated_atoms_empty_pair_types_and_single_atom_beads(pk):
         sim.close()
 
 
+def test_dilute_gas_many_centres_per_row_tile(pk):
+    """A dilute system (about 4 neighbours per atom): a 128-row tile of the embedding kernels then spans ~30 centres,
+    which takes the backward kernel's un-staged dT path and many short centre segments in the forward kernel."""
+    desc = workloads.model_desc()
+    w = workloads.model_weights(desc, 5)
+    model = se_e2_a.Model(desc, w)
+    rng = np.random.default_rng(17)
+    N, L = 320, 40.0
+    pts = []
+    while len(pts) < N:                                  # random positions at least 1.1 A apart
+        c = rng.uniform(0, L, 3)
+        if all(np.linalg.norm((c - q + L / 2) % L - L / 2) > 1.1 for q in pts):
+            pts.append(c)
+    x1 = np.array(pts)
+    types = (np.arange(N) % 3 != 0).astype(np.int32)     # O, H, H, ...
+    P = 2
+    x = x1[None] + 0.01 * rng.standard_normal((P, N, 3))
+    p = rng.standard_normal((P, N, 3))
+    box = np.array([L, L, L])
+    sim = pk.PIMD(types, [15.9994, 1.008], box, P, 300.0, 0.5e-3, 1.0, seed=1, model_desc=desc)
+    sim.set_state(x, p)
+    sim.set_model(w)
+    f, U, E = sim.forces(), sim.energies(), sim.atom_energies()
+    counts = pk.pimd_get_neighbor_counts(sim.ctx, P, N, 2)
+    assert counts.sum() / (P * N) < 12                   # dilute indeed
+    for k in range(P):
+        Eo, Fo, Xio = se_e2_a.energy_forces(x[k], types, box, model)
+        frms = np.sqrt((Fo ** 2).mean())
+        assert (np.abs(f[k] - Fo) / np.maximum(np.abs(Fo), frms)).max() <= 1e-4
+        assert np.abs(E[k] - Eo).max() <= 1e-6
+        assert abs(U[k] - Eo.sum()) / N <= 1e-6
+    sim.close()
+
+
 def test_sel_overflow_is_an_error(pk):
     cfg, wb, desc, w = workloads.make_config(0)
     small = dict(desc, sel=[8, 16])
