@@ -12,6 +12,8 @@ Pin status (see tests/test_oracle_*.py):
   nm.py          pinned   orthogonality, diagonalises the ring Laplacian (PAPER.md B1-B3)
   integrator.py  pinned   closed-form harmonic propagation, variance preservation, finite-P
                           harmonic-oscillator <K>,<V>, NVE energy conservation, P=1 limit
+  barostat.py    pinned   E1 = quadrature of the cell force over the kick, E4/E5 = numerical ODE, NpH enthalpy
+                          (A17) conserved to second order, A12 = A11 at n = 1, closed forms, E7 variance
   se_e2_a.py     backward pinned (finite differences, torch autograd, invariances, virial =
                  -dU/d(strain), continuity at r_c);  forward architecture: PARITY UNPINNED
                  against physics -- the paper prints no equation for the Deep-Potential

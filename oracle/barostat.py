@@ -1,0 +1,111 @@
+"""Isotropic BZP barostat of the oracle (test infrastructure; see oracle/__init__.py).
+
+Sources: PAPER.md:L196 (NpH = atoms + cell with conserved enthalpy A17; NpT = white-noise Langevin
+on the barostat velocity plus PILE_L on the atoms), Appendix A Eq. A10-A17 (L370-411), Appendix E
+Eq. E1, E4-E7 (L488-522).  Readings of garbled / silent passages are DESIGN R-20 .. R-25 and are
+named where they are used.  Everything is FP64 numpy, one statement per printed term.
+
+Conventions as oracle/integrator.py: x[P,N,3] Cartesian, vt/ft[P,N,3] normal-mode velocities and
+forces, mode 0 = centroid mode (x~_0 = sum_k x_k / sqrt(n)).  Pressures are eV/A^3 inside; the
+`iso` keyword (metal units: bar) is converted with BAR_PER_EV_A3 (DESIGN R-25).
+"""
+import numpy as np
+
+from .constants import KB, MVV2E
+from . import nm, philox
+
+BAR_PER_EV_A3 = 1.602176634e6      # 1 eV/A^3 in bar (elementary charge, exact SI value; DESIGN R-25)
+
+
+def barostat_mass(P, N, T, tau_p):
+    """W = 3 n N k_B T tau_P^2 (under Eq. A13)."""
+    return 3.0 * P * N * KB * T * tau_p * tau_p
+
+
+def centroid_sums(x, vt, ft, masses):
+    """The four sums over atoms that Eq. A12 and Eq. E1 are built from:
+      S_kin = sum_i m_i v~_i^(0)2            (eV, via mvv2e)      A12 first term
+      S_cv  = sum_k sum_i (r_i^(k) - r_i^c).F_i^(k)   (eV)        A12 second term
+      S_fv  = sum_i F~_i^(0).v~_i^(0)        (eV/ps)              E1 third term
+      S_ff  = sum_i |F~_i^(0)|^2 / m_i       (eV/ps^2, via mvv2e) E1 fourth term"""
+    P = x.shape[0]
+    m = masses[:, None]
+    f = nm.from_nm(nm.nm_matrix(P), ft)
+    rc = np.mean(x, axis=0, keepdims=True)
+    S_kin = float(np.sum(m * vt[0] * vt[0]) * MVV2E)
+    S_cv = float(np.sum((x - rc) * f))
+    S_fv = float(np.sum(ft[0] * vt[0]))
+    S_ff = float(np.sum(ft[0] * ft[0] / (m * MVV2E)))
+    return S_kin, S_cv, S_fv, S_ff
+
+
+def p_cv(x, vt, ft, Xi, masses, V):
+    """Eq. A12: P_CV = [S_kin - S_cv + sum_k Tr Xi^(k)] / (3 n V), eV/A^3."""
+    P = x.shape[0]
+    S_kin, S_cv, _, _ = centroid_sums(x, vt, ft, masses)
+    return (S_kin - S_cv + float(np.trace(Xi, axis1=1, axis2=2).sum())) / (3.0 * P * V)
+
+
+def press_v_step(vW, x, vt, ft, Xi, masses, V, T, W, p_ext, h):
+    """Eq. E1 over a time h:
+      v_W += (3h/W) [ n V (P_CV - P_ext) + n k_B T ] + (h^2/W) sum F~0.v~0 + (h^3/(3W)) sum |F~0|^2/m.
+    DESIGN R-20: the bracket's second term is printed "1/(n k_B T)"; only n k_B T is an energy, and
+    it is the term that makes A17 (with J_W = -n k_B T ln V, A16) a constant of the motion -- pinned by
+    the NpH enthalpy test.  The velocities are those BEFORE the B kick of the same length that follows
+    (the h^2 and h^3 terms are that kick's contribution to the kinetic part integrated over h)."""
+    P = x.shape[0]
+    _, _, S_fv, S_ff = centroid_sums(x, vt, ft, masses)
+    pcv = p_cv(x, vt, ft, Xi, masses, V)
+    vW = vW + (3.0 * h / W) * (P * V * (pcv - p_ext) + P * KB * T)
+    vW = vW + (h * h / W) * S_fv
+    vW = vW + (h * h * h / (3.0 * W)) * S_ff
+    return vW
+
+
+def sinh_over(vW, h):
+    """(e^{h v_W} - e^{-h v_W}) / (2 v_W) of Eq. E4, with its limit h for v_W -> 0 (DESIGN R-22:
+    below |h v_W| = 1e-4 the series h (1 + (h v_W)^2/6 + (h v_W)^4/120), exact to 1e-30)."""
+    a = h * vW
+    if abs(a) < 1e-4:
+        return h * (1.0 + a * a / 6.0 + a * a * a * a / 120.0)
+    return (np.exp(a) - np.exp(-a)) / (2.0 * vW)
+
+
+def qc_step(xt, vt, box, vW, h):
+    """Eq. E4-E6 over a time h, on the CENTROID mode only (DESIGN R-21: E4/E5 carry no
+    bead index; P_CV and E1 are built from centroid quantities alone, i.e. the cell scales the centroids and
+    the internal modes follow the free ring-polymer A step):
+      x~_0 <- e^{h v_W} x~_0 + sinh(h v_W)/v_W v~_0 ;  v~_0 <- e^{-h v_W} v~_0 ;  L <- e^{h v_W} L."""
+    xt = xt.copy()
+    vt = vt.copy()
+    e = np.exp(h * vW)
+    xt[0] = e * xt[0] + sinh_over(vW, h) * vt[0]
+    vt[0] = np.exp(-h * vW) * vt[0]
+    return xt, vt, np.asarray(box, dtype=np.float64) * e
+
+
+def press_o_step(vW, P, N, T, W, gamma0, h, seed, step):
+    """Eq. E7: v_W <- c1 v_W + c2 sqrt(n k_B T / W) eta, c1 = exp(-h/tau_0), c2 = sqrt(1-c1^2).
+    DESIGN R-23: the printed "m_i" under the root is the barostat mass W (v_W is 1/time: n k_B T / W is
+    1/time^2); tau_0 is the centroid damping time 1/gamma0 as printed.  eta is the Philox normal keyed as
+    mode 0, component 0 of the atom index N (one past the last atom) of this step (DESIGN R-10)."""
+    c1 = np.exp(-h * gamma0)
+    c2 = np.sqrt(1.0 - c1 * c1)
+    eta = float(philox.normal(seed, step, 0, N, 0))
+    return c1 * vW + c2 * np.sqrt(P * KB * T / W) * eta
+
+
+def extended_terms(vW, V, P, T, W, p_ext):
+    """K_W = W v_W^2 / 2 (A13), U_W = n P_ext V (A15), J_W = -n k_B T ln V (A16)."""
+    return 0.5 * W * vW * vW, P * p_ext * V, -P * KB * T * np.log(V)
+
+
+def p_pr(S_ring, P, N, T, V):
+    """Eq. A10: (1/3V)(3 n N k_B T - sum m omega_n^2 |r^(k)-r^(k+1)|^2) with the square on
+    omega_n as in A7 (DESIGN R-6): the sum is twice the spring energy S_ring."""
+    return (3.0 * P * N * KB * T - 2.0 * S_ring) / (3.0 * V)
+
+
+def p_md(K_ring, Xi, V):
+    """Eq. A11: (1/3V) sum_k (sum_i m v~^(k)2 + Tr Xi^(k)); sum m v~^2 = 2 K_ring."""
+    return (2.0 * K_ring + float(np.trace(Xi, axis1=1, axis2=2).sum())) / (3.0 * V)

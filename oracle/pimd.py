@@ -9,7 +9,7 @@ after the closing B with x, f consistent.
 import numpy as np
 
 from .constants import KB, MVV2E
-from . import nm, integrator, se_e2_a
+from . import nm, integrator, se_e2_a, barostat
 
 
 class OraclePIMD:
@@ -38,6 +38,10 @@ class OraclePIMD:
         self.U = np.zeros(self.P)
         self.Xi = np.zeros((self.P, 3, 3))
         self.only_beads = None       # bench.py's bounded cpu_baseline sample: evaluate these beads only
+        self.baro = False            # isotropic BZP barostat (NpH; NpT when gamma0 > 0)
+        self.vW = 0.0
+        self.p_ext = 0.0
+        self.W = 0.0
 
     # ---- inputs ----
     def set_state(self, x, p):
@@ -62,6 +66,15 @@ class OraclePIMD:
         if self.x is not None:
             self._forces()
 
+    def set_barostat(self, p_ext_bar, tau_p):
+        """`iso p_ext barostat BZP taup tau_p`: isotropic target pressure in bar,
+        barostat mass W = 3 n N k_B T tau_p^2 (L389); v_W starts at 0.  BAOAB only (DESIGN R-24)."""
+        assert self.integrator == "baoab"
+        self.baro = True
+        self.p_ext = float(p_ext_bar) / barostat.BAR_PER_EV_A3
+        self.W = barostat.barostat_mass(self.P, self.N, self.T, float(tau_p))
+        self.vW = 0.0
+
     # ---- the path ----
     def _forces(self):
         f = np.zeros((self.P, self.N, 3))
@@ -77,8 +90,43 @@ class OraclePIMD:
         self.f = f
         self.ft = nm.to_nm(self.M, f)
 
+    def _drift_half(self, xt, h):
+        """A(h) with the cell: centroid by Eq. E4-E6, modes k >= 1 by the free ring-polymer rotation (R-21)."""
+        xq, vq, self.box = barostat.qc_step(xt, self.vt, self.box, self.vW, h)
+        xa, va = integrator.a_step(xt, self.vt, self.om, h)
+        xa[0], va[0] = xq[0], vq[0]
+        self.vt = va
+        return xa
+
+    def _npt_step(self):
+        """One BAOAB step with the BZP barostat (DESIGN R-24; the paper prints the sub-steps, Appendix E, but not
+        their order): [E1(dt/2), B(dt/2)], [E4-E6 + A](dt/2), [O(dt), E7(dt)], [E4-E6 + A](dt/2), forces at the new
+        positions and cell, [E1(dt/2), B(dt/2)] -- every barostat sub-step sits next to the atomic sub-step of
+        the same letter and takes its length."""
+        h = 0.5 * self.dt
+        self.vW = barostat.press_v_step(self.vW, self.x, self.vt, self.ft, self.Xi, self.masses,
+                                        float(np.prod(self.box)), self.T, self.W, self.p_ext, h)
+        self.vt = integrator.b_step(self.vt, self.ft, self.masses, h)
+        xt = nm.to_nm(self.M, self.x)
+        xt = self._drift_half(xt, h)
+        self.vt = integrator.o_step(self.vt, self.masses, self.T, self.om, self.gamma0, self.dt, self.seed,
+                                    self.step_count)
+        if self.gamma0 != 0.0:
+            self.vW = barostat.press_o_step(self.vW, self.P, self.N, self.T, self.W, self.gamma0, self.dt,
+                                            self.seed, self.step_count)
+        xt = self._drift_half(xt, h)
+        self.x = nm.from_nm(self.M, xt)
+        self._forces()
+        self.vW = barostat.press_v_step(self.vW, self.x, self.vt, self.ft, self.Xi, self.masses,
+                                        float(np.prod(self.box)), self.T, self.W, self.p_ext, h)
+        self.vt = integrator.b_step(self.vt, self.ft, self.masses, h)
+        self.step_count += 1
+
     def step(self, n_steps=1):
         for _ in range(int(n_steps)):
+            if self.baro:
+                self._npt_step()
+                continue
             if self.integrator == "obabo":
                 self.x, self.vt = integrator.obabo_positions_half(
                     self.x, self.vt, self.ft, self.masses, self.M, self.om, self.T, self.gamma0,
@@ -120,3 +168,17 @@ class OraclePIMD:
         e = integrator.estimators(self.x, self.vt, self.f, self.U, self.masses, self.M, self.om, self.T)
         e["step"] = self.step_count
         return e
+
+    def barostat_state(self):
+        """Outputs 8-15 of Appendix A; pressures in bar."""
+        e = self.estimators()
+        V = float(np.prod(self.box))
+        KW, UW, JW = barostat.extended_terms(self.vW, V, self.P, self.T, self.W, self.p_ext)
+        bar = barostat.BAR_PER_EV_A3
+        return {
+            "v_W": self.vW, "box": self.box.copy(), "V": V,
+            "P_CV": barostat.p_cv(self.x, self.vt, self.ft, self.Xi, self.masses, V) * bar,
+            "P_PR": barostat.p_pr(e["S_ring"], self.P, self.N, self.T, V) * bar,
+            "P_MD": barostat.p_md(e["K_ring"], self.Xi, V) * bar,
+            "K_W": KW, "U_W": UW, "J_W": JW, "enthalpy": e["H"] + KW + UW + JW,     # A17
+        }
