@@ -173,6 +173,35 @@ int pimd_set_integrator(pimd_ctx* ctx, int kind);
  * opening half of the fused integrator launch, so a step then costs two integrator launches instead of one. */
 int pimd_set_fixcom(pimd_ctx* ctx, int on);
 
+/* Isotropic BZP barostat (Appendix E Eq. E1, E4-E7, L488-522; keywords `iso`, `barostat BZP`, `taup`,
+ * L176-179): the cell gets one velocity v_W with mass W = 3 n N k_B T tau_p^2 (L389), driven by the centroid-virial
+ * pressure P_CV (Eq. A12) against p_ext_bar (bar; 1 eV/A^3 = 1.602176634e6 bar, DESIGN R-25).  With
+ * gamma_centroid = 0 this is the NpH ensemble (the enthalpy of Eq. A17 is conserved); with gamma_centroid > 0 the
+ * cell velocity is thermostatted by Eq. E7 next to PILE_L on the atoms: NpT.  Sub-step order DESIGN R-24; the
+ * centroids scale with the cell, internal modes do not (R-21).  v_W starts at 0 and is reset by every call.  The
+ * cell then lives on the device and is rescaled every step (Eq. E6); the neighbour list is rebuilt from the
+ * current cell at every force evaluation.  BAOAB only: returns PIMD_EINVAL under PIMD_OBABO or with fixcom on
+ * (and pimd_set_integrator / pimd_set_fixcom refuse those while a barostat is on), and for tau_p <= 0.
+ * If the cell shrinks by more than a few per cent inside ONE pimd_step call so that r_c no longer fits the cell
+ * grid chosen at the start of the call, the call returns PIMD_ESEL_OVERFLOW (call with fewer steps). */
+int pimd_set_barostat(pimd_ctx* ctx, double p_ext_bar, double tau_p);
+
+/* Barostat outputs after the last completed step (Appendix A outputs 8-15); pressures in bar,
+ * energies in eV, lengths in Angstrom.  PIMD_EINVAL when no barostat is set. */
+typedef struct pimd_barostat_state {
+    double v_W;       /* cell velocity, 1/ps (output 11) */
+    double box[3];    /* current cell lengths (Eq. E6) */
+    double V;         /* box[0] box[1] box[2] */
+    double P_CV;      /* centroid-virial pressure, Eq. A12 */
+    double P_PR;      /* primitive pressure, Eq. A10 (omega_n squared as in A7, R-6) */
+    double P_MD;      /* pressure of the extended classical system, Eq. A11 */
+    double K_W;       /* W v_W^2 / 2, Eq. A13 */
+    double U_W;       /* n P_ext V, Eq. A15 */
+    double J_W;       /* -n k_B T ln V, Eq. A16 */
+    double enthalpy;  /* H + K_W + U_W + J_W, Eq. A17 */
+} pimd_barostat_state;
+int pimd_get_barostat(pimd_ctx* ctx, pimd_barostat_state* b);
+
 /* Fitting-net GEMM path: 1 (default) = tcgen05 tensor cores, 3xTF32 split (fitting_tc.cu); 0 = the FP32
  * CUDA-core GEMMs kept as the in-tree reference for bisecting.  Both meet the parity tolerances. */
 int pimd_set_fitting_path(pimd_ctx* ctx, int use_tensor_cores);

@@ -53,6 +53,17 @@ class Estimators(C.Structure):
         return {n: getattr(self, n) for n, _ in self._fields_}
 
 
+class BarostatState(C.Structure):
+    _fields_ = [("v_W", C.c_double), ("box", C.c_double * 3), ("V", C.c_double), ("P_CV", C.c_double),
+                ("P_PR", C.c_double), ("P_MD", C.c_double), ("K_W", C.c_double), ("U_W", C.c_double),
+                ("J_W", C.c_double), ("enthalpy", C.c_double)]
+
+    def as_dict(self):
+        d = {n: getattr(self, n) for n, _ in self._fields_}
+        d["box"] = np.array(list(self.box))
+        return d
+
+
 _lib = None
 
 _SIGNATURES = {
@@ -70,6 +81,8 @@ _SIGNATURES = {
     "pimd_set_fitting_path": (C.c_int, [C.c_void_p, C.c_int]),
     "pimd_set_integrator": (C.c_int, [C.c_void_p, C.c_int]),
     "pimd_set_fixcom": (C.c_int, [C.c_void_p, C.c_int]),
+    "pimd_set_barostat": (C.c_int, [C.c_void_p, C.c_double, C.c_double]),
+    "pimd_get_barostat": (C.c_int, [C.c_void_p, C.c_void_p]),
     "pimd_set_embedding_path": (C.c_int, [C.c_void_p, C.c_int]),
     "pimd_debug_gemm": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]),
     "pimd_model_n_weights": (C.c_size_t, [C.c_void_p]),
@@ -273,6 +286,16 @@ def pimd_get_estimators(ctx):
     return e.as_dict()
 
 
+def pimd_set_barostat(ctx, p_ext_bar, tau_p):
+    return _check(ctx, lib().pimd_set_barostat(ctx, float(p_ext_bar), float(tau_p)))
+
+
+def pimd_get_barostat(ctx):
+    b = BarostatState()
+    _check(ctx, lib().pimd_get_barostat(ctx, C.byref(b)))
+    return b.as_dict()
+
+
 def pimd_get_estimator_history(ctx, cap):
     arr = (Estimators * cap)()
     n = _check(ctx, lib().pimd_get_estimator_history(ctx, arr, cap))
@@ -376,6 +399,8 @@ class PIMD:
     def energies(self): return pimd_get_energies(self.ctx, self.P)
     def atom_energies(self): return pimd_get_atom_energies(self.ctx, self.P, self.N)
     def estimators(self): return pimd_get_estimators(self.ctx)
+    def set_barostat(self, p_ext_bar, tau_p): return pimd_set_barostat(self.ctx, p_ext_bar, tau_p)
+    def barostat_state(self): return pimd_get_barostat(self.ctx)
     def estimator_history(self, cap=4096): return pimd_get_estimator_history(self.ctx, cap)
 
     def neighbors(self, bead, cap=None):

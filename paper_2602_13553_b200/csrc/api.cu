@@ -20,6 +20,9 @@ struct pimd_ctx {
     bool fixcom = false;
     double* com = nullptr;        // [3] device: centroid COM momentum (fixcom)
     double inv_mtot = 0;
+    bool baro = false;            // isotropic BZP barostat (Appendix E)
+    double p_ext = 0, baro_W = 0; // eV/A^3, eV ps^2
+    double* baro_state = nullptr; // [BS_WIDTH] device
     std::vector<int32_t> types;
     std::vector<double> masses;
     std::string err;
@@ -90,6 +93,7 @@ size_t base_bytes(const pimd_ctx* c) {
     b += align_up((size_t)c->N * 8, 256) + align_up((size_t)c->N * 4, 256);
     b += align_up((size_t)c->P * 8, 256) + align_up((size_t)c->P * 72, 256) + align_up((size_t)c->P * c->N * 8, 256);
     b += align_up((size_t)(kEstCap + 2) * kEstWidth * 8, 256);
+    b += align_up(barostat_state_doubles(3 * c->N) * 8, 256);
     return b + 4096 + 256;
 }
 
@@ -204,6 +208,7 @@ int eval_forces(pimd_ctx* ctx) {
     ForceArgs a;
     a.P = ctx->P; a.N = ctx->N; a.ntypes = ctx->ntypes;
     for (int c = 0; c < 3; ++c) a.box[c] = ctx->box[c];
+    a.box_dev = ctx->baro ? ctx->baro_state + BS_LX : nullptr;
     a.x = ctx->x; a.types = ctx->types_d; a.f = ctx->f; a.U = ctx->U; a.Xi = ctx->Xi; a.Eatom = ctx->Eatom;
     const size_t PN3 = (size_t)ctx->P * ctx->N * 3;
     cudaMemsetAsync(ctx->f, 0, PN3 * 8, ctx->stream);
@@ -237,6 +242,42 @@ void fill_integrator_args(pimd_ctx* ctx, IntegratorArgs& a, int flags, int64_t s
     a.x_in = ctx->x; a.vt_in = ctx->vt; a.f = ctx->f; a.x_out = ctx->x; a.vt_out = ctx->vt;
     a.mass = ctx->mass_atom; a.U = ctx->U; a.est = est_slot;
     a.com = ctx->com; a.inv_mtot = ctx->inv_mtot;
+    a.baro = ctx->baro ? ctx->baro_state : nullptr;
+}
+
+constexpr double kBarPerEvA3 = 1.602176634e6;    // DESIGN R-25
+
+// the barostat's share of launch s (barostat.cu): closing E1 of the step that ends, opening E1 / E4-E7 of the next
+int run_barostat(pimd_ctx* ctx, bool close, bool start, int64_t step) {
+    BaroArgs b;
+    b.P = ctx->P; b.N = ctx->N; b.n_dof = 3 * ctx->N;
+    b.close = close; b.start = start; b.thermostat = (ctx->gamma0 != 0.0) ? 1 : 0;
+    b.h = 0.5 * ctx->dt; b.W = ctx->baro_W; b.p_ext = ctx->p_ext;
+    b.nkT = ctx->P * kKB * ctx->T;
+    b.c1 = std::exp(-ctx->dt * ctx->gamma0);
+    b.c2sig = std::sqrt(1.0 - b.c1 * b.c1) * std::sqrt(b.nkT / ctx->baro_W);
+    b.seed_lo = (uint32_t)ctx->seed; b.seed_hi = (uint32_t)(ctx->seed >> 32);
+    b.step_lo = (uint32_t)(uint64_t)step; b.step_hi = (uint32_t)((uint64_t)step >> 32);
+    b.x = ctx->x; b.vt = ctx->vt; b.f = ctx->f; b.mass = ctx->mass_atom; b.Xi = ctx->Xi;
+    b.state = ctx->baro_state; b.partial = ctx->baro_state + BS_WIDTH;
+    return launch_barostat(b, ctx->stream);
+}
+
+// under a barostat the cell changes on the device: fetch it once per API call and refit the walk range of the
+// (fixed) cell grid with a 3 % margin for the shrinkage inside the call (neighbor.cu flags a violation)
+int sync_box(pimd_ctx* ctx) {
+    if (!ctx->baro) return PIMD_OK;
+    CK(cudaMemcpyAsync(ctx->box, ctx->baro_state + BS_LX, 3 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    if (ctx->model_kind == 2) {
+        Model& m = ctx->model;
+        for (int a = 0; a < 3; ++a) {
+            const double w = ctx->box[a] / m.ncell[a];
+            m.R[a] = std::max(1, (int)std::ceil(m.d.rcut * 1.03 / w - 1e-12));
+            if (m.R[a] > 3) return fail(ctx, PIMD_EINVAL, "cell shrank below rcut/3 per grid cell");
+        }
+    }
+    return PIMD_OK;
 }
 
 int check_overflow(pimd_ctx* ctx) {
@@ -246,6 +287,8 @@ int check_overflow(pimd_ctx* ctx) {
     CK(cudaStreamSynchronize(ctx->stream));
     if (flag) {
         cudaMemsetAsync(ctx->model.overflow, 0, sizeof(int), ctx->stream);
+        if (flag & 2)
+            return fail(ctx, PIMD_ESEL_OVERFLOW, "the cell shrank past the cell-grid margin inside one pimd_step call; use fewer steps per call");
         return fail(ctx, PIMD_ESEL_OVERFLOW, "an atom has more neighbours of one type than sel allows");
     }
     return PIMD_OK;
@@ -254,8 +297,11 @@ int check_overflow(pimd_ctx* ctx) {
 // forces + estimators of the current (x, v~): used after set_state / set_model
 int refresh(pimd_ctx* ctx) {
     if (!ctx->have_state || ctx->model_kind == 0) return PIMD_OK;
-    int rc = eval_forces(ctx);
+    int rc = sync_box(ctx);
     if (rc) return rc;
+    rc = eval_forces(ctx);
+    if (rc) return rc;
+    if (ctx->baro) ctx->launches += run_barostat(ctx, false, false, ctx->step);     // P_CV of the current state
     double* cur = ctx->est + (size_t)kEstCap * kEstWidth;
     CK(cudaMemsetAsync(cur, 0, sizeof(double) * kEstWidth, ctx->stream));
     IntegratorArgs a;
@@ -416,8 +462,50 @@ int pimd_get_neighbor_counts(pimd_ctx* ctx, int32_t* counts) {
 
 int64_t pimd_get_launch_count(const pimd_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
+int pimd_set_barostat(pimd_ctx* ctx, double p_ext_bar, double tau_p) {
+    if (!ctx) return PIMD_EINVAL;
+    if (!(tau_p > 0)) return fail(ctx, PIMD_EINVAL, "tau_p must be positive");
+    if (ctx->integrator != PIMD_BAOAB || ctx->fixcom)
+        return fail(ctx, PIMD_EINVAL, "the barostat is implemented for BAOAB without fixcom (DESIGN R-24)");
+    if (!ctx->baro_state) {
+        int rc = arena_alloc(ctx, &ctx->baro_state, barostat_state_doubles(3 * ctx->N));
+        if (rc) return rc;
+    }
+    double st[BS_WIDTH] = {0};
+    if (ctx->baro) { int rc = sync_box(ctx); if (rc) return rc; }     // keep the current cell
+    for (int c = 0; c < 3; ++c) st[BS_LX + c] = ctx->box[c];
+    CK(cudaMemcpyAsync(ctx->baro_state, st, sizeof(st), cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    ctx->baro = true;
+    ctx->p_ext = p_ext_bar / kBarPerEvA3;
+    ctx->baro_W = 3.0 * ctx->P * ctx->N * kKB * ctx->T * tau_p * tau_p;
+    return refresh(ctx);
+}
+
+int pimd_get_barostat(pimd_ctx* ctx, pimd_barostat_state* b) {
+    if (!ctx || !b) return fail(ctx, PIMD_EINVAL, "null argument");
+    if (!ctx->baro) return fail(ctx, PIMD_EINVAL, "no barostat set");
+    double st[BS_WIDTH], raw[kEstWidth];
+    CK(cudaMemcpyAsync(st, ctx->baro_state, sizeof(st), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaMemcpyAsync(raw, ctx->est + (size_t)kEstCap * kEstWidth, sizeof(raw), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    const double n = ctx->P, N = ctx->N;
+    b->v_W = st[BS_VW];
+    for (int c = 0; c < 3; ++c) b->box[c] = st[BS_LX + c];
+    b->V = st[BS_LX] * st[BS_LY] * st[BS_LZ];
+    b->P_CV = st[BS_PCV] * kBarPerEvA3;
+    b->P_PR = (3.0 * n * N * kKB * ctx->T - 2.0 * raw[1]) / (3.0 * b->V) * kBarPerEvA3;    // A10
+    b->P_MD = (2.0 * raw[0] + st[BS_TRXI]) / (3.0 * b->V) * kBarPerEvA3;                   // A11
+    b->K_W = 0.5 * ctx->baro_W * b->v_W * b->v_W;                                          // A13
+    b->U_W = n * ctx->p_ext * b->V;                                                        // A15
+    b->J_W = -n * kKB * ctx->T * std::log(b->V);                                           // A16
+    b->enthalpy = raw[0] + raw[1] + raw[3] + b->K_W + b->U_W + b->J_W;                     // A17
+    return PIMD_OK;
+}
+
 int pimd_set_fixcom(pimd_ctx* ctx, int on) {
     if (!ctx) return PIMD_EINVAL;
+    if (on && ctx->baro) return fail(ctx, PIMD_EINVAL, "fixcom is not available with the barostat (DESIGN R-24)");
     ctx->fixcom = on != 0;
     return PIMD_OK;
 }
@@ -425,6 +513,7 @@ int pimd_set_fixcom(pimd_ctx* ctx, int on) {
 int pimd_set_integrator(pimd_ctx* ctx, int kind) {
     if (!ctx) return PIMD_EINVAL;
     if (kind != PIMD_BAOAB && kind != PIMD_OBABO) return fail(ctx, PIMD_EINVAL, "unknown integrator kind");
+    if (kind != PIMD_BAOAB && ctx->baro) return fail(ctx, PIMD_EINVAL, "the barostat is implemented for BAOAB (DESIGN R-24)");
     ctx->integrator = kind;
     mode_constants(ctx);
     return PIMD_OK;
@@ -613,6 +702,7 @@ int pimd_step(pimd_ctx* ctx, int64_t n_steps) {
     if (!ctx->have_state) return fail(ctx, PIMD_ENOSTATE, "pimd_set_state has not been called");
     if (ctx->model_kind == 0) return fail(ctx, PIMD_ENOMODEL, "no force model set");
     if (n_steps == 0) return PIMD_OK;
+    { int rc = sync_box(ctx); if (rc) return rc; }
     const int hist = (int)std::min<int64_t>(n_steps, kEstCap);
     const int64_t first_hist = n_steps - hist;            // steps before this index are not recorded
     CK(cudaMemsetAsync(ctx->est, 0, sizeof(double) * (size_t)hist * kEstWidth, ctx->stream));
@@ -630,6 +720,7 @@ int pimd_step(pimd_ctx* ctx, int64_t n_steps) {
         if (s < n_steps) flags |= I_START;
         IntegratorArgs a;
         rec(ctx, 0);
+        if (ctx->baro) ctx->launches += run_barostat(ctx, s > 0, s < n_steps, ctx->step + s);
         if (ctx->fixcom && s > 0) {
             // fixcom (R-19): the removal needs sum_i m_i v~_0,i over ALL atoms after the closing half,
             // so the launch splits: close + accumulate, then subtract + estimators (+ open)

@@ -50,7 +50,27 @@ struct IntegratorArgs {
     double*  est;                // [kEstWidth] accumulators of this step's slot, may be null
     double*  com;                // [3] fixcom: sum_i m_i v~_0,i per component (I_COMACC adds, I_COMSUB reads)
     double   inv_mtot;           // 1 / sum_i m_i
+    const double* baro;          // barostat state (BaroSlot layout) or null: centroid drift by Eq. E4/E5
 };
+
+// Barostat state on the device (Appendix E; DESIGN R-20..R-25), doubles:
+enum BaroSlot { BS_VW = 0, BS_LX = 1, BS_LY = 2, BS_LZ = 3, BS_PCV = 4, BS_TRXI = 5,
+                BS_EA1 = 6, BS_SH1 = 7, BS_EM1 = 8, BS_EA2 = 9, BS_SH2 = 10, BS_EM2 = 11,
+                BS_SKIN = 12, BS_SCV = 13, BS_SFV = 14, BS_SFF = 15, BS_WIDTH = 16 };
+struct BaroArgs {
+    int P, N, n_dof;
+    int close, start, thermostat;
+    double h;                    // dt/2
+    double W, p_ext;             // barostat mass (eV ps^2), target pressure (eV/A^3)
+    double nkT;                  // n k_B T
+    double c1, c2sig;            // E7 over dt: exp(-dt gamma0), sqrt(1-c1^2) sqrt(n k_B T / W)
+    uint32_t seed_lo, seed_hi, step_lo, step_hi;
+    const double* x; const double* vt; const double* f; const double* mass; const double* Xi;
+    double* state;               // [BS_WIDTH]
+    double* partial;             // [blocks][4] block partials of the four sums
+};
+int launch_barostat(const BaroArgs& a, cudaStream_t s);
+size_t barostat_state_doubles(int n_dof);    // BS_WIDTH + the partials
 
 int launch_integrator(int P, const IntegratorArgs& a, const ModeConsts& mc, cudaStream_t s);
 int launch_to_nm_velocity(int P, int N, const double* p_cart, const double* mass, double* vt, cudaStream_t s);
@@ -134,6 +154,7 @@ struct Model {
 struct ForceArgs {
     int P, N, ntypes;
     double box[3];
+    const double* box_dev; // barostat: the cell lives on the device ([3] doubles) and box[] is ignored; else null
     const double* x;      // [P][N][3]
     const int* types;     // [N]
     double* f;            // [P][N][3]

@@ -186,11 +186,21 @@ integrator_kernel(const __grid_constant__ IntegratorArgs a, const __grid_constan
             if (start) {
                 v += kick * ft[k];                           // B(dt/2)
                 const double x = xt[k];
-                const double xn = mc.cosA[k] * x + mc.sinA_w[k] * v;    // A(dt/2): exact rotation (R-5)
-                double vn = mc.msinA_w[k] * x + mc.cosA[k] * v;
-                if (thermo) vn = mc.c1[k] * vn + mc.c2[k] * sigma * eta_s[k * kIntThreads];   // O(dt)
-                xt[k] = mc.cosA[k] * xn + mc.sinA_w[k] * vn;            // A(dt/2)
-                v = mc.msinA_w[k] * xn + mc.cosA[k] * vn;
+                if (k == 0 && a.baro != nullptr) {
+                    // BZP barostat (Eq. E4/E5, L507-512; R-21: centroid mode only): the two half drifts with the
+                    // cell velocity before and after its own thermostat step (barostat.cu prepared the factors)
+                    const double xn = a.baro[BS_EA1] * x + a.baro[BS_SH1] * v;
+                    double vn = a.baro[BS_EM1] * v;
+                    if (thermo) vn = mc.c1[k] * vn + mc.c2[k] * sigma * eta_s[k * kIntThreads];
+                    xt[k] = a.baro[BS_EA2] * xn + a.baro[BS_SH2] * vn;
+                    v = a.baro[BS_EM2] * vn;
+                } else {
+                    const double xn = mc.cosA[k] * x + mc.sinA_w[k] * v;    // A(dt/2): exact rotation (R-5)
+                    double vn = mc.msinA_w[k] * x + mc.cosA[k] * v;
+                    if (thermo) vn = mc.c1[k] * vn + mc.c2[k] * sigma * eta_s[k * kIntThreads];   // O(dt)
+                    xt[k] = mc.cosA[k] * xn + mc.sinA_w[k] * vn;            // A(dt/2)
+                    v = mc.msinA_w[k] * xn + mc.cosA[k] * vn;
+                }
             }
             if (live && (a.flags & (I_BCLOSE | I_START | I_COMSUB))) a.vt_out[k * stride + ec] = v;
         }

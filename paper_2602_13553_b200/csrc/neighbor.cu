@@ -16,20 +16,39 @@ struct GridGeom {
     int nc[3];
     int R[3];
     int ncells;
+    const double* boxp;  // barostat (PAPER.md Eq. E6): the cell is rescaled on the device every step; null = use L
+    double rc;
+    int* overflow;
 };
+
+// cell lengths and inverse cell widths of this launch: kernel arguments, or the device-resident cell under a barostat
+__device__ __forceinline__ void load_geom(const GridGeom& g, double L[3], double inv_w[3]) {
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        L[a] = g.boxp ? g.boxp[a] : g.L[a];
+        inv_w[a] = g.boxp ? (double)g.nc[a] / L[a] : g.inv_w[a];
+    }
+}
 
 __global__ void wrap_bin_kernel(int P, int N, GridGeom g, const double* __restrict__ x, double* __restrict__ wtmp,
                                 int* __restrict__ cell_id, int* __restrict__ cell_count) {
     const int ba = blockIdx.x * blockDim.x + threadIdx.x;
     if (ba >= P * N) return;
     const int k = ba / N;
+    double gL[3], ginv_w[3];
+    load_geom(g, gL, ginv_w);
+    if (g.boxp && ba == 0) {
+        // the cell shrank so far inside one pimd_step call that rc spans more than R cells: neighbours would be missed
+        for (int a = 0; a < 3; ++a)
+            if (g.rc * ginv_w[a] > (double)g.R[a]) atomicOr(g.overflow, 2);
+    }
     int c[3];
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
         const double xv = x[(size_t)ba * 3 + a];
-        const double w = __dsub_rn(xv, __dmul_rn(g.L[a], floor(__ddiv_rn(xv, g.L[a]))));
+        const double w = __dsub_rn(xv, __dmul_rn(gL[a], floor(__ddiv_rn(xv, gL[a]))));
         wtmp[(size_t)ba * 3 + a] = w;
-        int ci = (int)floor(w * g.inv_w[a]);
+        int ci = (int)floor(w * ginv_w[a]);
         ci = ci < 0 ? 0 : (ci >= g.nc[a] ? g.nc[a] - 1 : ci);
         c[a] = ci;
     }
@@ -119,6 +138,8 @@ neighbor_env_kernel(int P, int N, GridGeom g, EnvConsts ec, const double* __rest
     const int lane = threadIdx.x & 31;
     if (ba >= P * N) return;
     const int k = ba / N, i = ba - k * N;
+    double gL[3], ginv_w[3];
+    load_geom(g, gL, ginv_w);
     const double wi[3] = {wtmp[(size_t)ba * 3], wtmp[(size_t)ba * 3 + 1], wtmp[(size_t)ba * 3 + 2]};
     const int cid = cell_id[ba];
     const int c0 = cid % g.nc[0], c1 = (cid / g.nc[0]) % g.nc[1], c2 = cid / (g.nc[0] * g.nc[1]);
@@ -154,7 +175,7 @@ neighbor_env_kernel(int P, int N, GridGeom g, EnvConsts ec, const double* __rest
                 double dm2 = 0.0;
 #pragma unroll
                 for (int ax = 0; ax < 3; ++ax) {
-                    const double wc = 1.0 / g.inv_w[ax];
+                    const double wc = 1.0 / ginv_w[ax];
                     const double lo = un[ax] * wc - wi[ax], hi = wi[ax] - (un[ax] + 1) * wc;
                     const double dd = fmax(fmax(lo, hi), 0.0);
                     dm2 += dd * dd;
@@ -183,8 +204,8 @@ neighbor_env_kernel(int P, int N, GridGeom g, EnvConsts ec, const double* __rest
                 const int f0 = __shfl_sync(0xffffffffu, my_s0, cn), f1 = __shfl_sync(0xffffffffu, my_s1, cn);
                 if (f0 + lane < f1) wnext = ws[f0 + lane];
             }
-            const double sh[3] = {__dmul_rn((double)nx, g.L[0]), __dmul_rn((double)ny, g.L[1]),
-                                  __dmul_rn((double)nz, g.L[2])};
+            const double sh[3] = {__dmul_rn((double)nx, gL[0]), __dmul_rn((double)ny, gL[1]),
+                                  __dmul_rn((double)nz, gL[2])};
             const bool zero_shift = (nx == 0) && (ny == 0) && (nz == 0);
             for (int q0 = s0; q0 < s1; q0 += 32) {
                 const int q = q0 + lane;
@@ -248,9 +269,9 @@ neighbor_env_kernel(int P, int N, GridGeom g, EnvConsts ec, const double* __rest
             const int nx = (int)(code & 7) - 3, ny = (int)((code >> 3) & 7) - 3, nz = (int)((code >> 6) & 7) - 3;
             const double4 wj = ws[__float_as_int(B.pad)];
             double d[3];
-            d[0] = __dadd_rn(__dsub_rn(wj.x, wi[0]), __dmul_rn((double)nx, g.L[0]));
-            d[1] = __dadd_rn(__dsub_rn(wj.y, wi[1]), __dmul_rn((double)ny, g.L[1]));
-            d[2] = __dadd_rn(__dsub_rn(wj.z, wi[2]), __dmul_rn((double)nz, g.L[2]));
+            d[0] = __dadd_rn(__dsub_rn(wj.x, wi[0]), __dmul_rn((double)nx, gL[0]));
+            d[1] = __dadd_rn(__dsub_rn(wj.y, wi[1]), __dmul_rn((double)ny, gL[1]));
+            d[2] = __dadd_rn(__dsub_rn(wj.z, wi[2]), __dmul_rn((double)nz, gL[2]));
             const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2]));
             const double r = sqrt(r2);
             double sw = 1.0, dsw = 0.0;
@@ -286,6 +307,7 @@ int neighbor_build(Model& m, const ForceArgs& a, cudaStream_t s) {
         g.inv_w[c] = (double)m.ncell[c] / a.box[c];
     }
     g.ncells = m.ncells;
+    g.boxp = a.box_dev; g.rc = m.d.rcut; g.overflow = m.overflow;
     EnvConsts ec;
     ec.rc = m.d.rcut; ec.rs = m.d.rcut_smth; ec.rc2 = m.d.rcut * m.d.rcut;
     ec.inv_range = 1.0 / (m.d.rcut - m.d.rcut_smth);
