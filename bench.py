@@ -118,6 +118,8 @@ def _oracle_sample(cfg_idx, steps, warmup, n_sample_beads):
     cfg, wb, desc, w = workloads.make_config(cfg_idx)
     orc = OraclePIMD(wb["types"], wb["masses"], wb["box"], cfg["P"], cfg["T"], cfg["dt"], cfg["gamma"], seed=0)
     orc.only_beads = list(range(n_sample_beads))
+    if "p_ext_bar" in cfg:
+        orc.set_barostat(cfg["p_ext_bar"], cfg["tau_p"])
     orc.set_state(wb["x"], wb["p"])
     orc.set_model(desc, w)
     for _ in range(warmup):
@@ -199,6 +201,8 @@ def run_ours(args):
     x_dev, p_dev = x_host.cuda(non_blocking=True), p_host.cuda(non_blocking=True)
     sim.set_model(w)
     sim.set_state(x_dev, p_dev)                     # inputs resident in HBM before the timed region
+    if "p_ext_bar" in cfg:                          # configs[4]: NpT, isotropic BZP barostat
+        sim.set_barostat(cfg["p_ext_bar"], cfg["tau_p"])
 
     def barrier():
         if world > 1:
@@ -323,6 +327,7 @@ def run_ours(args):
             "vs_baseline": None, "dtype": "f16-split (3-pass hi/lo, f32 accumulate) network ~ f32 / f64 geometry+integrator", "data": "synthetic",
             "config": {"workload": cfg["name"], "atoms": N, "beads": P, "bead_atoms": P * N, "neighbour_rows": rows,
                        "parallelism": "replicas only" if world > 1 else "1 GPU",
+                       "ensemble": ("NpT %g bar, BZP barostat tau_p %g ps" % (cfg["p_ext_bar"], cfg["tau_p"])) if "p_ext_bar" in cfg else "NVT",
                        "l2": "no flush: per-step working set (neighbour rows 135 MB, T and dT 157 MB, fitting activations ~380 MB) exceeds the 126 MB L2"},
             "roofline": roofline, "kernels": kernels, "integrator_hbm": integ, "cpu_baseline": cpu,
             "e2e": {"value": world * P * N / e2e_s, "unit": METRIC, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,

@@ -7,6 +7,7 @@ import numpy as np
 import pytest
 
 import workloads
+from oracle import barostat, nm, se_e2_a
 from oracle.constants import KB, MVV2E
 from oracle.pimd import OraclePIMD
 
@@ -155,6 +156,109 @@ def test_full_npt_step_parity_config0(pk):
     assert bo["V"] != float(np.prod(wb["box"]))
     pressures_close(bs, bo)
     assert abs(bs["enthalpy"] - bo["enthalpy"]) <= 1e-6 * sim.N * sim.P
+    sim.close()
+
+
+@pytest.mark.parametrize("squeeze", [False, True])
+def test_neighbour_lists_bit_exact_in_the_rescaled_cell(pk, squeeze):
+    """After the barostat has moved the cell (expanding at 1 bar under the random-weight model's pressure, or
+    squeezed by a target far above it), the neighbour rows of the last force evaluation are exactly the brute-force
+    rows of the oracle at the positions and cell the getters return (wrap, images and cutoff all use the new L)."""
+    cfg, wb, desc, w = workloads.make_config(0)
+    sim = pk.PIMD(wb["types"], wb["masses"], wb["box"], cfg["P"], cfg["T"], cfg["dt"], cfg["gamma"], seed=2,
+                  model_desc=desc)
+    sim.set_state(wb["x"], wb["p"])
+    sim.set_model(w)
+    sim.set_barostat(1.0, 0.02)
+    if squeeze:
+        sim.set_barostat(sim.barostat_state()["P_CV"] + 1.0e5, 0.02)
+    for _ in range(12):                               # stop between 0.5 % and a few % of linear change
+        sim.step(2)
+        bs = sim.barostat_state()
+        if abs(bs["box"][0] / wb["box"][0] - 1.0) > 5e-3:
+            break
+    assert (bs["box"][0] < wb["box"][0] * 0.995) if squeeze else (bs["box"][0] > wb["box"][0] * 1.005)
+    x = sim.positions()
+    for k in (0, 3):
+        count, j, shift = sim.neighbors(k)
+        ri, rj, rn, _ = se_e2_a.neighbours_bruteforce(x[k], bs["box"], desc["rcut"])
+        tj = np.asarray(wb["types"])[rj]
+        order = np.lexsort((rn[:, 2], rn[:, 1], rn[:, 0], rj, tj, ri))
+        assert np.array_equal(count, np.bincount(ri, minlength=sim.N))
+        assert np.array_equal(j, rj[order])
+        assert np.array_equal(shift.astype(np.int64), rn[order])
+    sim.close()
+
+
+def _squeezed_config1(pk, seed):
+    cfg, wb, desc, w = workloads.make_config(1, n_beads=4)      # L = 12.42: two cells of 6.21 A per side, R = 1
+    sim = pk.PIMD(wb["types"], wb["masses"], wb["box"], 4, cfg["T"], cfg["dt"], cfg["gamma"], seed=seed, model_desc=desc)
+    sim.set_state(wb["x"], wb["p"])
+    sim.set_model(w)
+    sim.set_barostat(1.0, 0.02)
+    sim.set_barostat(sim.barostat_state()["P_CV"] + 1.0e5, 0.02)
+    return sim, wb, desc
+
+
+def test_cell_grid_follows_a_shrinking_cell_across_calls(pk):
+    """The cell grid is fixed at pimd_set_model; once the cell is below 2 x 6 A the walk range must grow to two
+    cells (refit at every API call): rows stay bit-exact."""
+    sim, wb, desc = _squeezed_config1(pk, 3)
+    for _ in range(200):
+        sim.step(2)
+        bs = sim.barostat_state()
+        if bs["box"][0] < 11.9:
+            break
+    assert bs["box"][0] < 11.9
+    x = sim.positions()
+    count, j, shift = sim.neighbors(1)
+    ri, rj, rn, _ = se_e2_a.neighbours_bruteforce(x[1], bs["box"], desc["rcut"])
+    order = np.lexsort((rn[:, 2], rn[:, 1], rn[:, 0], rj, np.asarray(wb["types"])[rj], ri))
+    assert np.array_equal(count, np.bincount(ri, minlength=sim.N))
+    assert np.array_equal(j, rj[order]) and np.array_equal(shift.astype(np.int64), rn[order])
+    sim.close()
+
+
+def test_cell_shrinking_past_the_grid_margin_inside_one_call_is_an_error(pk):
+    sim, wb, desc = _squeezed_config1(pk, 3)
+    with pytest.raises(pk.PimdError, match="cell shrank|more neighbours"):
+        sim.step(400)
+    sim.close()
+
+
+def test_npt_config4_full_size_sampled(pk):
+    """BASELINE.json configs[4] (6144 atoms x 64 beads, NpT) in the launch configuration bench.py times, with a
+    fast cell (tau_p 0.02 ps) so that it moves in three steps.  The oracle cannot step this size; it (a) recomputes
+    Eq. A12 from the state the getters return, (b) evaluates one sampled bead at the RESCALED cell."""
+    cfg, wb, desc, w = workloads.make_config(4)
+    P = cfg["P"]
+    sim = pk.PIMD(wb["types"], wb["masses"], wb["box"], P, cfg["T"], cfg["dt"], cfg["gamma"], seed=0, model_desc=desc)
+    sim.set_state(wb["x"], wb["p"])
+    sim.set_model(w)
+    sim.set_barostat(cfg["p_ext_bar"], 0.02)
+    sim.step(3)
+    bs = sim.barostat_state()
+    assert abs(bs["box"][0] / wb["box"][0] - 1.0) > 1e-5 and np.isfinite(bs["enthalpy"])
+    np.testing.assert_allclose(bs["V"], np.prod(bs["box"]), rtol=1e-15)
+    x, p, f, Xi = sim.positions(), sim.momenta(), sim.forces(), sim.virial().reshape(P, 3, 3)
+    m = wb["masses"][wb["types"]]
+    M = nm.nm_matrix(P)
+    vt, ft = nm.to_nm(M, p / m[None, :, None]), nm.to_nm(M, f)
+    pcv = barostat.p_cv(x, vt, ft, Xi, m, bs["V"]) * BAR
+    big = abs(np.trace(Xi, axis1=1, axis2=2).sum()) / (3.0 * P * bs["V"]) * BAR
+    assert abs(bs["P_CV"] - pcv) <= 1e-9 * max(big, abs(pcv)), (bs["P_CV"], pcv, big)
+    e = sim.estimators()
+    assert abs(bs["P_MD"] - barostat.p_md(e["K_ring"], Xi, bs["V"]) * BAR) <= 1e-9 * max(big * P, abs(bs["P_MD"]))
+    assert abs(bs["P_PR"] - barostat.p_pr(e["S_ring"], P, sim.N, cfg["T"], bs["V"]) * BAR) <= 1e-9 * abs(bs["P_PR"])
+    # forces and virial of a sampled bead at the cell the barostat produced
+    model = se_e2_a.Model(desc, w)
+    k = 37
+    Eo, Fo, Xio = se_e2_a.energy_forces(x[k], wb["types"], bs["box"], model)
+    frms = np.sqrt((Fo ** 2).mean())
+    err = np.abs(f[k] - Fo) / np.maximum(np.abs(Fo), frms)
+    assert err.max() <= 1e-4, "force error %.3e" % err.max()
+    assert np.abs(Xi[k] - Xio).max() <= 1e-4 * np.abs(Xio).max()
+    assert abs(sim.energies()[k] - Eo.sum()) / sim.N <= 1e-6
     sim.close()
 
 

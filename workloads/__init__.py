@@ -30,7 +30,7 @@ CONFIGS = [
     dict(name="c3_4096h2o_p32", n_mol=4096, box=49.67, P=32, T=300.0, dt=0.25e-3, gamma=1.0, lattice="sc",
          steps=50, geom_seed=3, weight_seed=1),
     dict(name="c4_2048h2o_p64_npt", n_mol=2048, box=39.42, P=64, T=300.0, dt=0.25e-3, gamma=1.0,
-         lattice="fcc", steps=50, geom_seed=4, weight_seed=1),
+         lattice="fcc", steps=50, geom_seed=4, weight_seed=1, p_ext_bar=1.0, tau_p=0.5),   # NpT: PAPER.md:L76
 ]
 
 
