@@ -98,6 +98,38 @@ def test_nph_enthalpy_is_conserved_on_the_gpu(pk):
     sim.close()
 
 
+def test_npt_ideal_gas_samples_the_isobaric_volume_distribution(pk):
+    """Free particles (harmonic model with k = 0) under NpT: the cell force is sum m v~0^2 - 3 n V P_ext + 3 n k_B T,
+    whose stationary volume distribution is V^N exp(-P_ext V / k_B T), so <V> = (N + 1) k_B T / P_ext and
+    <K_W> = n k_B T / 2 -- a statistical check of E1's n k_B T term (R-20), E4-E7 and the thermostats together
+    (N rather than N + 1 would be 12.5 % off at N = 8; the tolerance is 4 sigma of the measured block error)."""
+    N, P, T = 8, 4, 300.0
+    rng = np.random.default_rng(0)
+    types = np.zeros(N, dtype=np.int32)
+    masses = np.array([15.9994])
+    x = rng.uniform(0.0, 10.0, size=(1, N, 3)) + 0.05 * rng.standard_normal((P, N, 3))
+    p = rng.standard_normal((P, N, 3)) * np.sqrt(P * KB * T * masses[0] / MVV2E)
+    p_ext = (N + 1) * KB * T / 1000.0                                  # eV/A^3: <V> = 1000 A^3
+    sim = pk.PIMD(types, masses, [10.0] * 3, P, T, 2.0e-3, 20.0, seed=7)
+    sim.set_state(x, p)
+    sim.set_model_harmonic(0.0)
+    sim.set_barostat(p_ext * BAR, 0.05)
+    sim.step(2000)
+    V, KW = [], []
+    for _ in range(3000):
+        sim.step(100)
+        b = sim.barostat_state()
+        V.append(b["V"]); KW.append(b["K_W"])
+    V, KW = np.asarray(V), np.asarray(KW)
+    blocks = V.reshape(30, 100).mean(axis=1)
+    err = blocks.std(ddof=1) / np.sqrt(len(blocks))
+    assert err < 0.02 * 1000.0
+    assert abs(V.mean() - 1000.0) < 4.0 * err, (V.mean(), err)
+    kb = KW.reshape(30, 100).mean(axis=1)
+    assert abs(KW.mean() - 0.5 * P * KB * T) < 4.0 * kb.std(ddof=1) / np.sqrt(len(kb)), KW.mean()
+    sim.close()
+
+
 def test_split_calls_agree_with_one_call_under_the_barostat(pk):
     """step(6) against step(1)+step(2)+step(3).  Not bitwise: a call boundary re-reads the kicked velocities where
     the single call advances the two velocity sums analytically (barostat.cu), a rounding-level difference."""
