@@ -84,14 +84,15 @@ def qc_step(xt, vt, box, vW, h):
     return xt, vt, np.asarray(box, dtype=np.float64) * e
 
 
-def press_o_step(vW, P, N, T, W, gamma0, h, seed, step):
+def press_o_step(vW, P, N, T, W, gamma0, h, seed, step, half=0):
     """Eq. E7: v_W <- c1 v_W + c2 sqrt(n k_B T / W) eta, c1 = exp(-h/tau_0), c2 = sqrt(1-c1^2).
     DESIGN R-23: the printed "m_i" under the root is the barostat mass W (v_W is 1/time: n k_B T / W is
     1/time^2); tau_0 is the centroid damping time 1/gamma0 as printed.  eta is the Philox normal keyed as
-    mode 0, component 0 of the atom index N (one past the last atom) of this step (DESIGN R-10)."""
+    mode 0, component 0 of the atom index N (one past the last atom) of this step (DESIGN R-10); `half` = 1
+    selects the second thermostat half-step of an OBABO step, as for the atoms."""
     c1 = np.exp(-h * gamma0)
     c2 = np.sqrt(1.0 - c1 * c1)
-    eta = float(philox.normal(seed, step, 0, N, 0))
+    eta = float(philox.normal(seed, step, 0, N, 0, half))
     return c1 * vW + c2 * np.sqrt(P * KB * T / W) * eta
 
 

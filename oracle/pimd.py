@@ -68,8 +68,8 @@ class OraclePIMD:
 
     def set_barostat(self, p_ext_bar, tau_p):
         """`iso p_ext barostat BZP taup tau_p`: isotropic target pressure in bar,
-        barostat mass W = 3 n N k_B T tau_p^2 (L389); v_W starts at 0.  BAOAB only (DESIGN R-24)."""
-        assert self.integrator == "baoab"
+        barostat mass W = 3 n N k_B T tau_p^2 (L389); v_W starts at 0.  Sub-step order: DESIGN R-24."""
+        assert not self.fixcom
         self.baro = True
         self.p_ext = float(p_ext_bar) / barostat.BAR_PER_EV_A3
         self.W = barostat.barostat_mass(self.P, self.N, self.T, float(tau_p))
@@ -91,7 +91,7 @@ class OraclePIMD:
         self.ft = nm.to_nm(self.M, f)
 
     def _drift_half(self, xt, h):
-        """A(h) with the cell: centroid by Eq. E4-E6, modes k >= 1 by the free ring-polymer rotation (R-21)."""
+        """A(h) (h = dt/2 in BAOAB, dt in OBABO) with the cell: centroid by Eq. E4-E6, modes k >= 1 by the free ring-polymer rotation (R-21)."""
         xq, vq, self.box = barostat.qc_step(xt, self.vt, self.box, self.vW, h)
         xa, va = integrator.a_step(xt, self.vt, self.om, h)
         xa[0], va[0] = xq[0], vq[0]
@@ -122,10 +122,39 @@ class OraclePIMD:
         self.vt = integrator.b_step(self.vt, self.ft, self.masses, h)
         self.step_count += 1
 
+    def _npt_step_obabo(self):
+        """One OBABO step (the fix's default splitting, PAPER.md:L82-84 runs it with `ensemble npt`) with the BZP
+        barostat, DESIGN R-24: [O, E7](dt/2), [E1, B](dt/2), [E4-E6 + A](dt), forces, [E1, B](dt/2), [O, E7](dt/2)."""
+        h = 0.5 * self.dt
+        self.vt = integrator.o_step(self.vt, self.masses, self.T, self.om, self.gamma0, h, self.seed,
+                                    self.step_count, half=0)
+        if self.gamma0 != 0.0:
+            self.vW = barostat.press_o_step(self.vW, self.P, self.N, self.T, self.W, self.gamma0, h,
+                                            self.seed, self.step_count, half=0)
+        self.vW = barostat.press_v_step(self.vW, self.x, self.vt, self.ft, self.Xi, self.masses,
+                                        float(np.prod(self.box)), self.T, self.W, self.p_ext, h)
+        self.vt = integrator.b_step(self.vt, self.ft, self.masses, h)
+        xt = nm.to_nm(self.M, self.x)
+        xt = self._drift_half(xt, self.dt)
+        self.x = nm.from_nm(self.M, xt)
+        self._forces()
+        self.vW = barostat.press_v_step(self.vW, self.x, self.vt, self.ft, self.Xi, self.masses,
+                                        float(np.prod(self.box)), self.T, self.W, self.p_ext, h)
+        self.vt = integrator.b_step(self.vt, self.ft, self.masses, h)
+        self.vt = integrator.o_step(self.vt, self.masses, self.T, self.om, self.gamma0, h, self.seed,
+                                    self.step_count, half=1)
+        if self.gamma0 != 0.0:
+            self.vW = barostat.press_o_step(self.vW, self.P, self.N, self.T, self.W, self.gamma0, h,
+                                            self.seed, self.step_count, half=1)
+        self.step_count += 1
+
     def step(self, n_steps=1):
         for _ in range(int(n_steps)):
             if self.baro:
-                self._npt_step()
+                if self.integrator == "obabo":
+                    self._npt_step_obabo()
+                else:
+                    self._npt_step()
                 continue
             if self.integrator == "obabo":
                 self.x, self.vt = integrator.obabo_positions_half(

@@ -81,14 +81,14 @@ def test_E4_group_property():
     np.testing.assert_allclose(L2, L3, rtol=1e-15)
 
 
-def _nph(dt, n_steps, P=4, N=6, gamma=0.0, seed=3):
+def _nph(dt, n_steps, P=4, N=6, gamma=0.0, seed=3, integ="baoab"):
     masses_t = [15.9994, 1.008]
     rng = np.random.default_rng(seed)
     types = rng.integers(0, 2, size=N)
     m = np.asarray(masses_t)[types]
     x = 0.23 * rng.standard_normal((1, N, 3)) + 0.05 * rng.standard_normal((P, N, 3))   # thermal width of the trap
     p = rng.standard_normal((P, N, 3)) * np.sqrt(P * KB * 300.0 * m[None, :, None] / MVV2E)   # (g/mol) A/ps
-    sim = OraclePIMD(types, masses_t, [10.0, 10.0, 10.0], P, 300.0, dt, gamma, 11)
+    sim = OraclePIMD(types, masses_t, [10.0, 10.0, 10.0], P, 300.0, dt, gamma, 11, integrator=integ)
     sim.set_barostat(KB * 300.0 / 1000.0 * barostat.BAR_PER_EV_A3, 0.05)   # trapped gas: <V> = k_B T / P_ext
     sim.set_state(x, p)
     sim.set_model_harmonic(0.5)
@@ -100,9 +100,26 @@ def _nph(dt, n_steps, P=4, N=6, gamma=0.0, seed=3):
     return sim, np.asarray(hs)
 
 
-def test_nph_conserves_the_enthalpy_A17_to_second_order():
-    sim1, d1 = _nph(1.0e-3, 400)
-    sim2, d2 = _nph(0.5e-3, 800)
+def test_obabo_equals_baoab_in_nph():
+    """Without thermostats both splittings are B A B with the same cell sub-steps: A(dt) = A(dt/2) A(dt/2) and
+    E4-E6 compose (group property), so the trajectories agree to rounding."""
+    a, _ = _nph(1.0e-3, 20, integ="baoab")
+    b, _ = _nph(1.0e-3, 20, integ="obabo")
+    np.testing.assert_allclose(a.positions(), b.positions(), rtol=0, atol=1e-11)
+    assert a.vW == pytest.approx(b.vW, rel=1e-10)
+    np.testing.assert_allclose(a.box, b.box, rtol=1e-13)
+
+
+def test_obabo_npt_draws_both_half_step_streams():
+    sim, _ = _nph(1.0e-3, 3, gamma=20.0, integ="obabo")
+    ref, _ = _nph(1.0e-3, 3, gamma=20.0, integ="baoab")
+    assert np.isfinite(sim.barostat_state()["enthalpy"]) and sim.vW != ref.vW
+
+
+@pytest.mark.parametrize("integ", ["baoab", "obabo"])
+def test_nph_conserves_the_enthalpy_A17_to_second_order(integ):
+    sim1, d1 = _nph(1.0e-3, 400, integ=integ)
+    sim2, d2 = _nph(0.5e-3, 800, integ=integ)
     st = sim1.barostat_state()
     assert abs(st["V"] / 1000.0 - 1.0) > 0.02 and abs(st["v_W"]) > 0           # the cell really moved
     assert np.abs(d1).max() < 5e-4 * abs(st["enthalpy"])
