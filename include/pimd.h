@@ -180,8 +180,9 @@ int pimd_set_fixcom(pimd_ctx* ctx, int on);
  * cell velocity is thermostatted by Eq. E7 next to PILE_L on the atoms: NpT.  Sub-step order DESIGN R-24; the
  * centroids scale with the cell, internal modes do not (R-21).  v_W starts at 0 and is reset by every call.  The
  * cell then lives on the device and is rescaled every step (Eq. E6); the neighbour list is rebuilt from the
- * current cell at every force evaluation.  BAOAB only: returns PIMD_EINVAL under PIMD_OBABO or with fixcom on
- * (and pimd_set_integrator / pimd_set_fixcom refuse those while a barostat is on), and for tau_p <= 0.
+ * current cell at every force evaluation.  Works with both splittings (PIMD_OBABO + npt is the paper's own example,
+ * L82): the cell's sub-steps sit next to the atomic sub-steps of the same letter.  Returns PIMD_EINVAL with fixcom
+ * on (and pimd_set_fixcom refuses while a barostat is on), and for tau_p <= 0.
  * If the cell shrinks by more than a few per cent inside ONE pimd_step call so that r_c no longer fits the cell
  * grid chosen at the start of the call, the call returns PIMD_ESEL_OVERFLOW (call with fewer steps). */
 int pimd_set_barostat(pimd_ctx* ctx, double p_ext_bar, double tau_p);

@@ -252,12 +252,17 @@ int run_barostat(pimd_ctx* ctx, bool close, bool start, int64_t step) {
     BaroArgs b;
     b.P = ctx->P; b.N = ctx->N; b.n_dof = 3 * ctx->N;
     b.close = close; b.start = start; b.thermostat = (ctx->gamma0 != 0.0) ? 1 : 0;
+    b.obabo = ctx->integrator == PIMD_OBABO;
     b.h = 0.5 * ctx->dt; b.W = ctx->baro_W; b.p_ext = ctx->p_ext;
     b.nkT = ctx->P * kKB * ctx->T;
-    b.c1 = std::exp(-ctx->dt * ctx->gamma0);
-    b.c2sig = std::sqrt(1.0 - b.c1 * b.c1) * std::sqrt(b.nkT / ctx->baro_W);
+    b.c1 = std::exp(-(b.obabo ? 0.5 * ctx->dt : ctx->dt) * ctx->gamma0);
+    b.c2 = std::sqrt(1.0 - b.c1 * b.c1);
+    b.c2sig = b.c2 * std::sqrt(b.nkT / ctx->baro_W);
+    b.half_dt_mvv = 0.5 * ctx->dt / kMvv2e;
+    b.PkT_mvv = ctx->P * kKB * ctx->T / kMvv2e;
     b.seed_lo = (uint32_t)ctx->seed; b.seed_hi = (uint32_t)(ctx->seed >> 32);
     b.step_lo = (uint32_t)(uint64_t)step; b.step_hi = (uint32_t)((uint64_t)step >> 32);
+    { const uint64_t cs = (uint64_t)(step - 1); b.cstep_lo = (uint32_t)cs; b.cstep_hi = (uint32_t)(cs >> 32) | 0x80000000u; }
     b.x = ctx->x; b.vt = ctx->vt; b.f = ctx->f; b.mass = ctx->mass_atom; b.Xi = ctx->Xi;
     b.state = ctx->baro_state; b.partial = ctx->baro_state + BS_WIDTH;
     return launch_barostat(b, ctx->stream);
@@ -465,8 +470,7 @@ int64_t pimd_get_launch_count(const pimd_ctx* ctx) { return ctx ? ctx->launches 
 int pimd_set_barostat(pimd_ctx* ctx, double p_ext_bar, double tau_p) {
     if (!ctx) return PIMD_EINVAL;
     if (!(tau_p > 0)) return fail(ctx, PIMD_EINVAL, "tau_p must be positive");
-    if (ctx->integrator != PIMD_BAOAB || ctx->fixcom)
-        return fail(ctx, PIMD_EINVAL, "the barostat is implemented for BAOAB without fixcom (DESIGN R-24)");
+    if (ctx->fixcom) return fail(ctx, PIMD_EINVAL, "the barostat is not available with fixcom (DESIGN R-24)");
     if (!ctx->baro_state) {
         int rc = arena_alloc(ctx, &ctx->baro_state, barostat_state_doubles(3 * ctx->N));
         if (rc) return rc;
@@ -513,7 +517,6 @@ int pimd_set_fixcom(pimd_ctx* ctx, int on) {
 int pimd_set_integrator(pimd_ctx* ctx, int kind) {
     if (!ctx) return PIMD_EINVAL;
     if (kind != PIMD_BAOAB && kind != PIMD_OBABO) return fail(ctx, PIMD_EINVAL, "unknown integrator kind");
-    if (kind != PIMD_BAOAB && ctx->baro) return fail(ctx, PIMD_EINVAL, "the barostat is implemented for BAOAB (DESIGN R-24)");
     ctx->integrator = kind;
     mode_constants(ctx);
     return PIMD_OK;

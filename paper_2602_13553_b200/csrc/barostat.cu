@@ -22,7 +22,7 @@ constexpr int kBaroThreads = 128;
 __global__ void __launch_bounds__(kBaroThreads)
 baro_sums_kernel(const __grid_constant__ BaroArgs a) {
     const int e = blockIdx.x * kBaroThreads + threadIdx.x;
-    double r[4] = {0.0, 0.0, 0.0, 0.0};
+    double r[kBaroSums] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
     if (e < a.n_dof) {
         const size_t stride = (size_t)a.n_dof;
         const double m = a.mass[e / 3];
@@ -38,22 +38,44 @@ baro_sums_kernel(const __grid_constant__ BaroArgs a) {
         r[1] = xf - (sx / (double)a.P) * sf;            // sum_k (r_k - r_c) F_k
         r[2] = f0 * v0;                                 // E1 third term
         r[3] = f0 * f0 / (m * kMvv2e);                  // E1 fourth term
+        if (a.obabo) {
+            // OBABO puts the centroid's thermostat between the closing and the opening E1, so the velocity sums of the
+            // opening E1 are not a function of the closing ones: replay kick and O steps of the centroid mode here
+            // (the normals are counter-based: the same ones the integrator kernel draws for mode 0)
+            const int i = e / 3, alpha = e - 3 * i;
+            const double sigma = sqrt(a.PkT_mvv / m);
+            double v = v0, ee, eo;
+            if (a.close) {
+                v += (a.half_dt_mvv / m) * f0;
+                if (a.thermostat) {
+                    philox_normal_pair(a.seed_lo, a.seed_hi, a.cstep_lo, a.cstep_hi, (uint32_t)i, (uint32_t)alpha, &ee, &eo);
+                    v = a.c1 * v + a.c2 * sigma * ee;
+                }
+            }
+            r[4] = m * v * v * kMvv2e;                  // what the estimators' P_CV sees
+            if (a.start && a.thermostat) {
+                philox_normal_pair(a.seed_lo, a.seed_hi, a.step_lo, a.step_hi, (uint32_t)i, (uint32_t)alpha, &ee, &eo);
+                v = a.c1 * v + a.c2 * sigma * ee;
+            }
+            r[5] = m * v * v * kMvv2e;
+            r[6] = f0 * v;
+        }
     }
-    __shared__ double red[4][kBaroThreads / 32];
+    __shared__ double red[kBaroSums][kBaroThreads / 32];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1)
 #pragma unroll
-        for (int q = 0; q < 4; ++q) r[q] += __shfl_xor_sync(0xffffffffu, r[q], o);
+        for (int q = 0; q < kBaroSums; ++q) r[q] += __shfl_xor_sync(0xffffffffu, r[q], o);
     const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
     if (l == 0)
 #pragma unroll
-        for (int q = 0; q < 4; ++q) red[q][w] = r[q];
+        for (int q = 0; q < kBaroSums; ++q) red[q][w] = r[q];
     __syncthreads();
-    if (threadIdx.x < 4) {
+    if (threadIdx.x < kBaroSums) {
         double t = 0.0;
 #pragma unroll
         for (int q = 0; q < kBaroThreads / 32; ++q) t += red[threadIdx.x][q];
-        a.partial[4 * blockIdx.x + threadIdx.x] = t;    // no atomics: the sums steer the dynamics, keep them reproducible
+        a.partial[kBaroSums * blockIdx.x + threadIdx.x] = t;    // no atomics: the sums steer the dynamics, keep them reproducible
     }
 }
 
@@ -66,15 +88,15 @@ __device__ __forceinline__ double sinh_over(double vW, double h) {
 
 __global__ void baro_update_kernel(const __grid_constant__ BaroArgs a) {
     // the block partials of the four sums, in a fixed order: lane-strided, then a shuffle tree
-    double sum4[4] = {0.0, 0.0, 0.0, 0.0};
+    double sum4[kBaroSums] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
     const int nblk = (a.n_dof + kBaroThreads - 1) / kBaroThreads;
     for (int b = threadIdx.x; b < nblk; b += 32)
 #pragma unroll
-        for (int q = 0; q < 4; ++q) sum4[q] += a.partial[4 * b + q];
+        for (int q = 0; q < kBaroSums; ++q) sum4[q] += a.partial[kBaroSums * b + q];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1)
 #pragma unroll
-        for (int q = 0; q < 4; ++q) sum4[q] += __shfl_xor_sync(0xffffffffu, sum4[q], o);
+        for (int q = 0; q < kBaroSums; ++q) sum4[q] += __shfl_xor_sync(0xffffffffu, sum4[q], o);
     if (threadIdx.x != 0) return;
     double* st = a.state;
     double vW = st[BS_VW];
@@ -96,6 +118,31 @@ __global__ void baro_update_kernel(const __grid_constant__ BaroArgs a) {
         Skin = Skin + 2.0 * h * Sfv + h * h * Sff;
         Sfv = Sfv + h * Sff;
     };
+    auto press_o = [&](uint32_t s_lo, uint32_t s_hi) {      // E7 (R-23), eta keyed (mode 0, atom N, dim 0)
+        double ee, eo;
+        philox_normal_pair(a.seed_lo, a.seed_hi, s_lo, s_hi, (uint32_t)a.N, 0u, &ee, &eo);
+        vW = a.c1 * vW + a.c2sig * ee;
+    };
+    if (a.obabo) {
+        // [E1, B](h) [O, E7](h) | [O, E7](h) [E1, B](h) [E4-E6 + A](dt)      (R-24)
+        if (a.close) {
+            press_v();
+            if (a.thermostat) press_o(a.cstep_lo, a.cstep_hi);
+        }
+        st[BS_PCV] = (sum4[4] - Scv + tr) / (3.0 * nP * V);
+        st[BS_TRXI] = tr;
+        if (a.start) {
+            if (a.thermostat) press_o(a.step_lo, a.step_hi);
+            Skin = sum4[5]; Sfv = sum4[6];
+            press_v();
+            const double dt = 2.0 * h, e1 = exp(dt * vW);
+            st[BS_EA1] = e1; st[BS_SH1] = sinh_over(vW, dt); st[BS_EM1] = exp(-dt * vW);
+            st[BS_EA2] = 1.0; st[BS_SH2] = 0.0; st[BS_EM2] = 1.0;
+            st[BS_LX] = L[0] * e1; st[BS_LY] = L[1] * e1; st[BS_LZ] = L[2] * e1;
+        }
+        st[BS_VW] = vW;
+        return;
+    }
     if (a.close) { press_v(); b_kick(); }
     st[BS_PCV] = (Skin - Scv + tr) / (3.0 * nP * V);       // A12 of the state the estimators see
     st[BS_TRXI] = tr;
@@ -104,11 +151,7 @@ __global__ void baro_update_kernel(const __grid_constant__ BaroArgs a) {
         const double e1 = exp(h * vW);
         st[BS_EA1] = e1; st[BS_SH1] = sinh_over(vW, h); st[BS_EM1] = exp(-h * vW);
         for (int c = 0; c < 3; ++c) L[c] *= e1;             // E6
-        if (a.thermostat) {                                 // E7 over dt (R-23), eta keyed (mode 0, atom N, dim 0)
-            double ee, eo;
-            philox_normal_pair(a.seed_lo, a.seed_hi, a.step_lo, a.step_hi, (uint32_t)a.N, 0u, &ee, &eo);
-            vW = a.c1 * vW + a.c2sig * ee;
-        }
+        if (a.thermostat) press_o(a.step_lo, a.step_hi);    // E7 over dt
         const double e2 = exp(h * vW);
         st[BS_EA2] = e2; st[BS_SH2] = sinh_over(vW, h); st[BS_EM2] = exp(-h * vW);
         for (int c = 0; c < 3; ++c) L[c] *= e2;
@@ -123,6 +166,6 @@ int launch_barostat(const BaroArgs& a, cudaStream_t s) {
     return 2;
 }
 
-size_t barostat_state_doubles(int n_dof) { return (size_t)BS_WIDTH + 4 * (size_t)((n_dof + kBaroThreads - 1) / kBaroThreads); }
+size_t barostat_state_doubles(int n_dof) { return (size_t)BS_WIDTH + kBaroSums * (size_t)((n_dof + kBaroThreads - 1) / kBaroThreads); }
 
 }  // namespace pimd

@@ -60,15 +60,20 @@ enum BaroSlot { BS_VW = 0, BS_LX = 1, BS_LY = 2, BS_LZ = 3, BS_PCV = 4, BS_TRXI 
 struct BaroArgs {
     int P, N, n_dof;
     int close, start, thermostat;
+    int obabo;                   // OBABO: O(dt/2) twice around the kicks, one drift of dt (R-24)
     double h;                    // dt/2
     double W, p_ext;             // barostat mass (eV ps^2), target pressure (eV/A^3)
     double nkT;                  // n k_B T
-    double c1, c2sig;            // E7 over dt: exp(-dt gamma0), sqrt(1-c1^2) sqrt(n k_B T / W)
+    double c1, c2sig;            // E7 over the O step's length (dt, OBABO dt/2): exp(-l gamma0), sqrt(1-c1^2) sqrt(n k_B T / W)
+    double c2;                   // sqrt(1-c1^2): the centroid mode's own O coefficients are the same c1, c2 (tau_0)
+    double half_dt_mvv, PkT_mvv; // as IntegratorArgs
     uint32_t seed_lo, seed_hi, step_lo, step_hi;
+    uint32_t cstep_lo, cstep_hi; // OBABO: the step this launch closes, bit 31 of word 1 set
     const double* x; const double* vt; const double* f; const double* mass; const double* Xi;
     double* state;               // [BS_WIDTH]
-    double* partial;             // [blocks][4] block partials of the four sums
+    double* partial;             // [blocks][kBaroSums] block partials of the sums
 };
+constexpr int kBaroSums = 7;     // S_kin, S_cv, S_fv, S_ff, and (OBABO) S_kin after kick + closing O, S_kin and S_fv after the opening O
 int launch_barostat(const BaroArgs& a, cudaStream_t s);
 size_t barostat_state_doubles(int n_dof);    // BS_WIDTH + the partials
 

@@ -229,8 +229,13 @@ integrator_kernel(const __grid_constant__ IntegratorArgs a, const __grid_constan
                 if (thermo) v = mc.c1[k] * v + mc.c2[k] * sigma * eta_s[k * kIntThreads];
                 v += kick * ft[k];
                 const double x = xt[k];
-                xt[k] = mc.cosA[k] * x + mc.sinA_w[k] * v;
-                v = mc.msinA_w[k] * x + mc.cosA[k] * v;
+                if (k == 0 && a.baro != nullptr) {           // BZP barostat: Eq. E4/E5 over dt on the centroid mode
+                    xt[k] = a.baro[BS_EA1] * x + a.baro[BS_SH1] * v;
+                    v = a.baro[BS_EM1] * v;
+                } else {
+                    xt[k] = mc.cosA[k] * x + mc.sinA_w[k] * v;
+                    v = mc.msinA_w[k] * x + mc.cosA[k] * v;
+                }
             }
             if (live && (a.flags & (I_BCLOSE | I_START | I_COMSUB))) a.vt_out[k * stride + ec] = v;
         }

@@ -45,19 +45,20 @@ def _compare_state(bs, bo, tol):
     assert _rel(bs["box"], bo["box"]) <= tol
 
 
+@pytest.mark.parametrize("integ", ["baoab", "obabo"])
 @pytest.mark.parametrize("P", [1, 4, 32, 64])
 @pytest.mark.parametrize("gamma", [0.0, 20.0])
-def test_barostat_parity_harmonic(pk, P, gamma):
+def test_barostat_parity_harmonic(pk, P, gamma, integ):
     N = 43                                           # 129 dofs: one full 128-thread block and a tail of one
     types, masses, x, p = _trap_system(N, P, seed=20 + P)
     box = [10.0, 11.0, 12.0]
     p_ext = 2.0 * KB * 300.0 / 1320.0 * BAR
     args = (types, masses, box, P, 300.0, 1.0e-3, gamma)
-    sim = pk.PIMD(*args, seed=5)
+    sim = pk.PIMD(*args, seed=5, integrator=integ)
     sim.set_state(x, p)
     sim.set_model_harmonic(0.5)
     sim.set_barostat(p_ext, 0.05)
-    orc = OraclePIMD(*args, seed=5)
+    orc = OraclePIMD(*args, seed=5, integrator=integ)
     orc.set_barostat(p_ext, 0.05)
     orc.set_state(x, p)
     orc.set_model_harmonic(0.5)
@@ -80,11 +81,12 @@ def test_barostat_parity_harmonic(pk, P, gamma):
     sim.close()
 
 
-def test_nph_enthalpy_is_conserved_on_the_gpu(pk):
+@pytest.mark.parametrize("integ", ["baoab", "obabo"])
+def test_nph_enthalpy_is_conserved_on_the_gpu(pk, integ):
     """Eq. A17 over 2000 steps of the CUDA path alone (a property that holds at any size)."""
     P, N = 8, 64
     types, masses, x, p = _trap_system(N, P, seed=3)
-    sim = pk.PIMD(types, masses, [10.0] * 3, P, 300.0, 0.5e-3, 0.0, seed=1)
+    sim = pk.PIMD(types, masses, [10.0] * 3, P, 300.0, 0.5e-3, 0.0, seed=1, integrator=integ)
     sim.set_state(x, p)
     sim.set_model_harmonic(0.5)
     sim.set_barostat(KB * 300.0 / 1000.0 * BAR, 0.05)
@@ -98,7 +100,8 @@ def test_nph_enthalpy_is_conserved_on_the_gpu(pk):
     sim.close()
 
 
-def test_npt_ideal_gas_samples_the_isobaric_volume_distribution(pk):
+@pytest.mark.parametrize("integ", ["baoab", "obabo"])
+def test_npt_ideal_gas_samples_the_isobaric_volume_distribution(pk, integ):
     """Free particles (harmonic model with k = 0) under NpT: the cell force is sum m v~0^2 - 3 n V P_ext + 3 n k_B T,
     whose stationary volume distribution is V^N exp(-P_ext V / k_B T), so <V> = (N + 1) k_B T / P_ext and
     <K_W> = n k_B T / 2 -- a statistical check of E1's n k_B T term (R-20), E4-E7 and the thermostats together
@@ -110,7 +113,7 @@ def test_npt_ideal_gas_samples_the_isobaric_volume_distribution(pk):
     x = rng.uniform(0.0, 10.0, size=(1, N, 3)) + 0.05 * rng.standard_normal((P, N, 3))
     p = rng.standard_normal((P, N, 3)) * np.sqrt(P * KB * T * masses[0] / MVV2E)
     p_ext = (N + 1) * KB * T / 1000.0                                  # eV/A^3: <V> = 1000 A^3
-    sim = pk.PIMD(types, masses, [10.0] * 3, P, T, 2.0e-3, 20.0, seed=7)
+    sim = pk.PIMD(types, masses, [10.0] * 3, P, T, 2.0e-3, 20.0, seed=7, integrator=integ)
     sim.set_state(x, p)
     sim.set_model_harmonic(0.0)
     sim.set_barostat(p_ext * BAR, 0.05)
@@ -150,16 +153,18 @@ def test_split_calls_agree_with_one_call_under_the_barostat(pk):
     assert _rel(out[0][2]["box"], out[1][2]["box"]) < 1e-14
 
 
-def test_full_npt_step_parity_config0(pk):
+@pytest.mark.parametrize("integ", ["baoab", "obabo"])
+def test_full_npt_step_parity_config0(pk, integ):
     """configs[0] geometry and model under NpT at 1 bar (configs[4]'s ensemble at the size the oracle finishes):
-    multi-image neighbours from a cell that changes every step."""
+    multi-image neighbours from a cell that changes every step.  OBABO + npt is the paper's own example command
+    (PAPER.md:L82)."""
     cfg, wb, desc, w = workloads.make_config(0)
     args = (wb["types"], wb["masses"], wb["box"], cfg["P"], cfg["T"], cfg["dt"], cfg["gamma"])
-    sim = pk.PIMD(*args, seed=11, model_desc=desc)
+    sim = pk.PIMD(*args, seed=11, model_desc=desc, integrator=integ)
     sim.set_state(wb["x"], wb["p"])
     sim.set_model(w)
     sim.set_barostat(1.0, 0.02)
-    orc = OraclePIMD(*args, seed=11)
+    orc = OraclePIMD(*args, seed=11, integrator=integ)
     orc.set_barostat(1.0, 0.02)
     orc.set_state(wb["x"], wb["p"])
     orc.set_model(desc, w)
@@ -303,11 +308,9 @@ def test_barostat_argument_errors(pk):
         sim.set_barostat(1.0, 0.0)                   # tau_p <= 0
     sim.set_barostat(1.0, 0.1)
     with pytest.raises(pk.PimdError):
-        pk.pimd_set_integrator(sim.ctx, "obabo")     # BAOAB only (R-24)
-    with pytest.raises(pk.PimdError):
-        pk.pimd_set_fixcom(sim.ctx, True)
+        pk.pimd_set_fixcom(sim.ctx, True)            # not with a barostat (R-24)
     sim.close()
-    sim = pk.PIMD(types, masses, [10.0] * 3, 4, 300.0, 1e-3, 0.0, seed=1, integrator="obabo")
+    sim = pk.PIMD(types, masses, [10.0] * 3, 4, 300.0, 1e-3, 0.0, seed=1, fixcom=True)
     with pytest.raises(pk.PimdError):
         sim.set_barostat(1.0, 0.1)
     sim.close()
