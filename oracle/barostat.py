@@ -97,8 +97,68 @@ def press_o_step(vW, P, N, T, W, gamma0, h, seed, step, half=0):
 
 
 def extended_terms(vW, V, P, T, W, p_ext):
-    """K_W = W v_W^2 / 2 (A13), U_W = n P_ext V (A15), J_W = -n k_B T ln V (A16)."""
-    return 0.5 * W * vW * vW, P * p_ext * V, -P * KB * T * np.log(V)
+    """K_W = W v_W^2 / 2 (A13; A14 = the sum over the three v_W,alpha when vW is an array), U_W = n P_ext V (A15),
+    J_W = -n k_B T ln V (A16)."""
+    return float(np.sum(0.5 * W * np.asarray(vW) ** 2)), P * p_ext * V, -P * KB * T * np.log(V)
+
+
+# ---- anisotropic variant (PAPER.md:L176 `aniso`; Eq. A14, E2, E3) ---------------------------------------------
+
+def barostat_mass_aniso(P, N, T, tau_p):
+    """W = n N k_B T tau_P^2 (under Eq. A14)."""
+    return P * N * KB * T * tau_p * tau_p
+
+
+def centroid_sums_diag(x, vt, ft, masses):
+    """The sums of `centroid_sums`, kept per Cartesian component alpha (arrays of 3): the pieces of Eq. E2/E3."""
+    P = x.shape[0]
+    m = masses[:, None]
+    f = nm.from_nm(nm.nm_matrix(P), ft)
+    rc = np.mean(x, axis=0, keepdims=True)
+    S_kin = np.sum(m * vt[0] * vt[0], axis=0) * MVV2E
+    S_cv = np.sum((x - rc) * f, axis=(0, 1))
+    S_fv = np.sum(ft[0] * vt[0], axis=0)
+    S_ff = np.sum(ft[0] * ft[0] / (m * MVV2E), axis=0)
+    return S_kin, S_cv, S_fv, S_ff
+
+
+def p_cv_diag(x, vt, ft, Xi, masses, V):
+    """Diagonal of the centroid-virial stress tensor, Eq. E3:
+    P_CV^aa = [sum m v~0_a^2 - sum_k sum_i (r_a - r^c_a) F_a + sum_k Xi_aa] / (n V); its mean is A12."""
+    P = x.shape[0]
+    S_kin, S_cv, _, _ = centroid_sums_diag(x, vt, ft, masses)
+    return (S_kin - S_cv + np.einsum("kaa->a", Xi)) / (P * V)
+
+
+def press_v_step_aniso(vW, x, vt, ft, Xi, masses, V, T, W, p_ext, h):
+    """Eq. E2 over a time h, per component alpha (R-20 for the bracket's second term):
+      v_Wa += (h/W) [ n V (P_CV^aa - P_ext) + n k_B T ] + (h^2/W) sum F~0_a v~0_a + (h^3/(3W)) sum F~0_a^2/m."""
+    P = x.shape[0]
+    _, _, S_fv, S_ff = centroid_sums_diag(x, vt, ft, masses)
+    pd = p_cv_diag(x, vt, ft, Xi, masses, V)
+    vW = np.asarray(vW, dtype=np.float64) + (h / W) * (P * V * (pd - p_ext) + P * KB * T)
+    vW = vW + (h * h / W) * S_fv
+    vW = vW + (h * h * h / (3.0 * W)) * S_ff
+    return vW
+
+
+def qc_step_aniso(xt, vt, box, vW, h):
+    """Eq. E4-E6 with one v_W,alpha per Cartesian component (centroid mode only, R-21)."""
+    xt = xt.copy()
+    vt = vt.copy()
+    e = np.exp(h * vW)
+    so = np.array([sinh_over(vW[a], h) for a in range(3)])
+    xt[0] = e[None, :] * xt[0] + so[None, :] * vt[0]
+    vt[0] = np.exp(-h * vW)[None, :] * vt[0]
+    return xt, vt, np.asarray(box, dtype=np.float64) * e
+
+
+def press_o_step_aniso(vW, P, N, T, W, gamma0, h, seed, step, half=0):
+    """Eq. E7 per component: eta_alpha = the Philox normal of (mode 0, atom index N, component alpha) (R-23)."""
+    c1 = np.exp(-h * gamma0)
+    c2 = np.sqrt(1.0 - c1 * c1)
+    eta = np.array([float(philox.normal(seed, step, 0, N, a, half)) for a in range(3)])
+    return c1 * np.asarray(vW) + c2 * np.sqrt(P * KB * T / W) * eta
 
 
 def p_pr(S_ring, P, N, T, V):

@@ -39,6 +39,7 @@ class OraclePIMD:
         self.Xi = np.zeros((self.P, 3, 3))
         self.only_beads = None       # bench.py's bounded cpu_baseline sample: evaluate these beads only
         self.baro = False            # isotropic BZP barostat (NpH; NpT when gamma0 > 0)
+        self.aniso = False
         self.vW = 0.0
         self.p_ext = 0.0
         self.W = 0.0
@@ -66,14 +67,29 @@ class OraclePIMD:
         if self.x is not None:
             self._forces()
 
-    def set_barostat(self, p_ext_bar, tau_p):
+    def set_barostat(self, p_ext_bar, tau_p, aniso=False):
         """`iso p_ext barostat BZP taup tau_p`: isotropic target pressure in bar,
         barostat mass W = 3 n N k_B T tau_p^2 (L389); v_W starts at 0.  Sub-step order: DESIGN R-24."""
         assert not self.fixcom
         self.baro = True
         self.p_ext = float(p_ext_bar) / barostat.BAR_PER_EV_A3
-        self.W = barostat.barostat_mass(self.P, self.N, self.T, float(tau_p))
-        self.vW = 0.0
+        self.aniso = bool(aniso)                     # PAPER.md:L176 `aniso`: one v_W per cell vector (Eq. E2-E3, A14)
+        if self.aniso:
+            self.W = barostat.barostat_mass_aniso(self.P, self.N, self.T, float(tau_p))
+            self.vW = np.zeros(3)
+        else:
+            self.W = barostat.barostat_mass(self.P, self.N, self.T, float(tau_p))
+            self.vW = 0.0
+
+    def _press_v(self, h):
+        fn = barostat.press_v_step_aniso if self.aniso else barostat.press_v_step
+        self.vW = fn(self.vW, self.x, self.vt, self.ft, self.Xi, self.masses, float(np.prod(self.box)), self.T,
+                     self.W, self.p_ext, h)
+
+    def _press_o(self, h, half=0):
+        if self.gamma0 != 0.0:
+            fn = barostat.press_o_step_aniso if self.aniso else barostat.press_o_step
+            self.vW = fn(self.vW, self.P, self.N, self.T, self.W, self.gamma0, h, self.seed, self.step_count, half)
 
     # ---- the path ----
     def _forces(self):
@@ -92,7 +108,7 @@ class OraclePIMD:
 
     def _drift_half(self, xt, h):
         """A(h) (h = dt/2 in BAOAB, dt in OBABO) with the cell: centroid by Eq. E4-E6, modes k >= 1 by the free ring-polymer rotation (R-21)."""
-        xq, vq, self.box = barostat.qc_step(xt, self.vt, self.box, self.vW, h)
+        xq, vq, self.box = (barostat.qc_step_aniso if self.aniso else barostat.qc_step)(xt, self.vt, self.box, self.vW, h)
         xa, va = integrator.a_step(xt, self.vt, self.om, h)
         xa[0], va[0] = xq[0], vq[0]
         self.vt = va
@@ -104,21 +120,17 @@ class OraclePIMD:
         positions and cell, [E1(dt/2), B(dt/2)] -- every barostat sub-step sits next to the atomic sub-step of
         the same letter and takes its length."""
         h = 0.5 * self.dt
-        self.vW = barostat.press_v_step(self.vW, self.x, self.vt, self.ft, self.Xi, self.masses,
-                                        float(np.prod(self.box)), self.T, self.W, self.p_ext, h)
+        self._press_v(h)
         self.vt = integrator.b_step(self.vt, self.ft, self.masses, h)
         xt = nm.to_nm(self.M, self.x)
         xt = self._drift_half(xt, h)
         self.vt = integrator.o_step(self.vt, self.masses, self.T, self.om, self.gamma0, self.dt, self.seed,
                                     self.step_count)
-        if self.gamma0 != 0.0:
-            self.vW = barostat.press_o_step(self.vW, self.P, self.N, self.T, self.W, self.gamma0, self.dt,
-                                            self.seed, self.step_count)
+        self._press_o(self.dt)
         xt = self._drift_half(xt, h)
         self.x = nm.from_nm(self.M, xt)
         self._forces()
-        self.vW = barostat.press_v_step(self.vW, self.x, self.vt, self.ft, self.Xi, self.masses,
-                                        float(np.prod(self.box)), self.T, self.W, self.p_ext, h)
+        self._press_v(h)
         self.vt = integrator.b_step(self.vt, self.ft, self.masses, h)
         self.step_count += 1
 
@@ -128,24 +140,18 @@ class OraclePIMD:
         h = 0.5 * self.dt
         self.vt = integrator.o_step(self.vt, self.masses, self.T, self.om, self.gamma0, h, self.seed,
                                     self.step_count, half=0)
-        if self.gamma0 != 0.0:
-            self.vW = barostat.press_o_step(self.vW, self.P, self.N, self.T, self.W, self.gamma0, h,
-                                            self.seed, self.step_count, half=0)
-        self.vW = barostat.press_v_step(self.vW, self.x, self.vt, self.ft, self.Xi, self.masses,
-                                        float(np.prod(self.box)), self.T, self.W, self.p_ext, h)
+        self._press_o(h, half=0)
+        self._press_v(h)
         self.vt = integrator.b_step(self.vt, self.ft, self.masses, h)
         xt = nm.to_nm(self.M, self.x)
         xt = self._drift_half(xt, self.dt)
         self.x = nm.from_nm(self.M, xt)
         self._forces()
-        self.vW = barostat.press_v_step(self.vW, self.x, self.vt, self.ft, self.Xi, self.masses,
-                                        float(np.prod(self.box)), self.T, self.W, self.p_ext, h)
+        self._press_v(h)
         self.vt = integrator.b_step(self.vt, self.ft, self.masses, h)
         self.vt = integrator.o_step(self.vt, self.masses, self.T, self.om, self.gamma0, h, self.seed,
                                     self.step_count, half=1)
-        if self.gamma0 != 0.0:
-            self.vW = barostat.press_o_step(self.vW, self.P, self.N, self.T, self.W, self.gamma0, h,
-                                            self.seed, self.step_count, half=1)
+        self._press_o(h, half=1)
         self.step_count += 1
 
     def step(self, n_steps=1):
@@ -205,7 +211,8 @@ class OraclePIMD:
         KW, UW, JW = barostat.extended_terms(self.vW, V, self.P, self.T, self.W, self.p_ext)
         bar = barostat.BAR_PER_EV_A3
         return {
-            "v_W": self.vW, "box": self.box.copy(), "V": V,
+            "v_W": float(np.mean(self.vW)), "v_W3": np.broadcast_to(self.vW, (3,)).copy(), "box": self.box.copy(), "V": V,
+            "P_CV3": barostat.p_cv_diag(self.x, self.vt, self.ft, self.Xi, self.masses, V) * bar,
             "P_CV": barostat.p_cv(self.x, self.vt, self.ft, self.Xi, self.masses, V) * bar,
             "P_PR": barostat.p_pr(e["S_ring"], self.P, self.N, self.T, V) * bar,
             "P_MD": barostat.p_md(e["K_ring"], self.Xi, V) * bar,

@@ -81,7 +81,7 @@ def test_E4_group_property():
     np.testing.assert_allclose(L2, L3, rtol=1e-15)
 
 
-def _nph(dt, n_steps, P=4, N=6, gamma=0.0, seed=3, integ="baoab"):
+def _nph(dt, n_steps, P=4, N=6, gamma=0.0, seed=3, integ="baoab", aniso=False):
     masses_t = [15.9994, 1.008]
     rng = np.random.default_rng(seed)
     types = rng.integers(0, 2, size=N)
@@ -89,7 +89,7 @@ def _nph(dt, n_steps, P=4, N=6, gamma=0.0, seed=3, integ="baoab"):
     x = 0.23 * rng.standard_normal((1, N, 3)) + 0.05 * rng.standard_normal((P, N, 3))   # thermal width of the trap
     p = rng.standard_normal((P, N, 3)) * np.sqrt(P * KB * 300.0 * m[None, :, None] / MVV2E)   # (g/mol) A/ps
     sim = OraclePIMD(types, masses_t, [10.0, 10.0, 10.0], P, 300.0, dt, gamma, 11, integrator=integ)
-    sim.set_barostat(KB * 300.0 / 1000.0 * barostat.BAR_PER_EV_A3, 0.05)   # trapped gas: <V> = k_B T / P_ext
+    sim.set_barostat(KB * 300.0 / 1000.0 * barostat.BAR_PER_EV_A3, 0.05, aniso=aniso)   # trapped gas: <V> = k_B T / P_ext
     sim.set_state(x, p)
     sim.set_model_harmonic(0.5)
     h0 = sim.barostat_state()["enthalpy"]
@@ -196,3 +196,61 @@ def test_npt_run_is_finite_and_thermostats_the_cell():
     st = sim.barostat_state()
     assert np.isfinite(st["enthalpy"]) and st["V"] > 0
     assert st["P_CV"] != st["P_MD"] and np.isfinite(st["P_PR"])
+
+
+# ---- anisotropic variant (Eq. A14, E2, E3) ----------------------------------------------------------------------
+
+def test_E3_diagonal_averages_to_A12_and_mass_A14():
+    P, N = 4, 7
+    masses, x, v = _state(P, N, 21)
+    M = nm.nm_matrix(P)
+    vt = nm.to_nm(M, v)
+    f = np.random.default_rng(22).standard_normal(x.shape)
+    ft = nm.to_nm(M, f)
+    Xi = np.random.default_rng(23).standard_normal((P, 3, 3))
+    d = barostat.p_cv_diag(x, vt, ft, Xi, masses, 300.0)
+    assert d.mean() == pytest.approx(barostat.p_cv(x, vt, ft, Xi, masses, 300.0), rel=1e-13)
+    assert len(set(np.round(d, 12))) == 3
+    assert barostat.barostat_mass_aniso(4, 10, 300.0, 0.5) == pytest.approx(barostat.barostat_mass(4, 10, 300.0, 0.5) / 3)
+
+
+def test_E2_is_the_integral_of_the_cell_force_per_component():
+    P, N = 4, 7
+    masses, x, v = _state(P, N, 31)
+    M = nm.nm_matrix(P)
+    vt = nm.to_nm(M, v)
+    f = -0.8 * x * np.array([1.0, 0.5, 2.0])
+    ft = nm.to_nm(M, f)
+    Xi = np.stack([x[k].T @ f[k] for k in range(P)])
+    V, T, W, p_ext, h = 512.0, 300.0, 2.1, 2.0e-5, 0.013
+    vW0 = np.array([0.02, -0.01, 0.005])
+    got = barostat.press_v_step_aniso(vW0, x, vt, ft, Xi, masses, V, T, W, p_ext, h)
+    rc = x.mean(axis=0, keepdims=True)
+    ts, ws = np.polynomial.legendre.leggauss(8)
+    ts = 0.5 * h * (ts + 1.0)
+    ws = 0.5 * h * ws
+    for a in range(3):
+        const = -np.sum(((x - rc) * f)[:, :, a]) + Xi[:, a, a].sum() - P * V * p_ext + P * KB * T
+        integral = sum(w * (np.sum(masses * (vt[0][:, a] + t * ft[0][:, a] / (masses * MVV2E)) ** 2) * MVV2E + const)
+                       for t, w in zip(ts, ws))
+        assert got[a] == pytest.approx(vW0[a] + integral / W, rel=1e-13)
+
+
+@pytest.mark.parametrize("integ", ["baoab", "obabo"])
+def test_anisotropic_nph_conserves_the_enthalpy_with_A14(integ):
+    sim1, d1 = _nph(1.0e-3, 400, integ=integ, aniso=True)
+    sim2, d2 = _nph(0.5e-3, 800, integ=integ, aniso=True)
+    st = sim1.barostat_state()
+    assert np.ptp(st["box"]) > 0.05 and np.ptp(st["v_W3"]) > 0            # the three cell vectors went their own ways
+    assert np.abs(d1).max() < 5e-4 * abs(st["enthalpy"])
+    assert np.abs(d2).max() < 0.3 * np.abs(d1).max()
+
+
+def test_anisotropic_E7_draws_one_normal_per_component():
+    P, N, T, W, g, h, seed = 4, 12, 300.0, 3.0, 5.0, 0.01, 77
+    c1 = np.exp(-h * g)
+    v1 = barostat.press_o_step_aniso(np.array([0.4, 0.1, -0.2]), P, N, T, W, g, h, seed, 5, half=1)
+    eta = np.array([float(philox.normal(seed, 5, 0, N, a, 1)) for a in range(3)])
+    np.testing.assert_allclose(v1, c1 * np.array([0.4, 0.1, -0.2]) + np.sqrt(1 - c1 * c1) * np.sqrt(P * KB * T / W) * eta,
+                               rtol=1e-14)
+    assert len(set(eta)) == 3
