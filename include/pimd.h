@@ -187,6 +187,12 @@ int pimd_set_fixcom(pimd_ctx* ctx, int on);
  * grid chosen at the start of the call, the call returns PIMD_ESEL_OVERFLOW (call with fewer steps). */
 int pimd_set_barostat(pimd_ctx* ctx, double p_ext_bar, double tau_p);
 
+/* Anisotropic variant (keyword `aniso`; Eq. E2-E3; Eq. A14): one cell velocity v_W,alpha
+ * per Cartesian component, each driven by its own diagonal element of the centroid-virial stress tensor against the
+ * same p_ext_bar, barostat mass W = n N k_B T tau_p^2 (L397), one thermostat normal per component (E7).  The cell
+ * stays orthorhombic.  Same rules and errors as pimd_set_barostat; the later of the two calls wins. */
+int pimd_set_barostat_aniso(pimd_ctx* ctx, double p_ext_bar, double tau_p);
+
 /* Barostat outputs after the last completed step (Appendix A outputs 8-15); pressures in bar,
  * energies in eV, lengths in Angstrom.  PIMD_EINVAL when no barostat is set. */
 typedef struct pimd_barostat_state {
@@ -196,10 +202,12 @@ typedef struct pimd_barostat_state {
     double P_CV;      /* centroid-virial pressure, Eq. A12 */
     double P_PR;      /* primitive pressure, Eq. A10 (omega_n squared as in A7, R-6) */
     double P_MD;      /* pressure of the extended classical system, Eq. A11 */
-    double K_W;       /* W v_W^2 / 2, Eq. A13 */
+    double K_W;       /* W v_W^2 / 2, Eq. A13; anisotropic: sum over the three components, Eq. A14 */
     double U_W;       /* n P_ext V, Eq. A15 */
     double J_W;       /* -n k_B T ln V, Eq. A16 */
     double enthalpy;  /* H + K_W + U_W + J_W, Eq. A17 */
+    double v_W3[3];   /* cell velocity per component (all equal to v_W in isotropic mode; v_W is their mean) */
+    double P_CV3[3];  /* diagonal of the centroid-virial stress tensor, Eq. E3 (P_CV is its mean) */
 } pimd_barostat_state;
 int pimd_get_barostat(pimd_ctx* ctx, pimd_barostat_state* b);
 

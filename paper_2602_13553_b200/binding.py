@@ -56,11 +56,12 @@ class Estimators(C.Structure):
 class BarostatState(C.Structure):
     _fields_ = [("v_W", C.c_double), ("box", C.c_double * 3), ("V", C.c_double), ("P_CV", C.c_double),
                 ("P_PR", C.c_double), ("P_MD", C.c_double), ("K_W", C.c_double), ("U_W", C.c_double),
-                ("J_W", C.c_double), ("enthalpy", C.c_double)]
+                ("J_W", C.c_double), ("enthalpy", C.c_double), ("v_W3", C.c_double * 3), ("P_CV3", C.c_double * 3)]
 
     def as_dict(self):
         d = {n: getattr(self, n) for n, _ in self._fields_}
-        d["box"] = np.array(list(self.box))
+        for key in ("box", "v_W3", "P_CV3"):
+            d[key] = np.array(list(getattr(self, key)))
         return d
 
 
@@ -82,6 +83,7 @@ _SIGNATURES = {
     "pimd_set_integrator": (C.c_int, [C.c_void_p, C.c_int]),
     "pimd_set_fixcom": (C.c_int, [C.c_void_p, C.c_int]),
     "pimd_set_barostat": (C.c_int, [C.c_void_p, C.c_double, C.c_double]),
+    "pimd_set_barostat_aniso": (C.c_int, [C.c_void_p, C.c_double, C.c_double]),
     "pimd_get_barostat": (C.c_int, [C.c_void_p, C.c_void_p]),
     "pimd_set_embedding_path": (C.c_int, [C.c_void_p, C.c_int]),
     "pimd_debug_gemm": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]),
@@ -290,6 +292,10 @@ def pimd_set_barostat(ctx, p_ext_bar, tau_p):
     return _check(ctx, lib().pimd_set_barostat(ctx, float(p_ext_bar), float(tau_p)))
 
 
+def pimd_set_barostat_aniso(ctx, p_ext_bar, tau_p):
+    return _check(ctx, lib().pimd_set_barostat_aniso(ctx, float(p_ext_bar), float(tau_p)))
+
+
 def pimd_get_barostat(ctx):
     b = BarostatState()
     _check(ctx, lib().pimd_get_barostat(ctx, C.byref(b)))
@@ -399,7 +405,9 @@ class PIMD:
     def energies(self): return pimd_get_energies(self.ctx, self.P)
     def atom_energies(self): return pimd_get_atom_energies(self.ctx, self.P, self.N)
     def estimators(self): return pimd_get_estimators(self.ctx)
-    def set_barostat(self, p_ext_bar, tau_p): return pimd_set_barostat(self.ctx, p_ext_bar, tau_p)
+    def set_barostat(self, p_ext_bar, tau_p, aniso=False):
+        return (pimd_set_barostat_aniso if aniso else pimd_set_barostat)(self.ctx, p_ext_bar, tau_p)
+
     def barostat_state(self): return pimd_get_barostat(self.ctx)
     def estimator_history(self, cap=4096): return pimd_get_estimator_history(self.ctx, cap)
 

@@ -20,7 +20,8 @@ struct pimd_ctx {
     bool fixcom = false;
     double* com = nullptr;        // [3] device: centroid COM momentum (fixcom)
     double inv_mtot = 0;
-    bool baro = false;            // isotropic BZP barostat (Appendix E)
+    bool baro = false;            // BZP barostat (Appendix E)
+    bool baro_aniso = false;      // Eq. E2-E3: one cell velocity per component
     double p_ext = 0, baro_W = 0; // eV/A^3, eV ps^2
     double* baro_state = nullptr; // [BS_WIDTH] device
     std::vector<int32_t> types;
@@ -252,7 +253,7 @@ int run_barostat(pimd_ctx* ctx, bool close, bool start, int64_t step) {
     BaroArgs b;
     b.P = ctx->P; b.N = ctx->N; b.n_dof = 3 * ctx->N;
     b.close = close; b.start = start; b.thermostat = (ctx->gamma0 != 0.0) ? 1 : 0;
-    b.obabo = ctx->integrator == PIMD_OBABO;
+    b.obabo = ctx->integrator == PIMD_OBABO; b.aniso = ctx->baro_aniso;
     b.h = 0.5 * ctx->dt; b.W = ctx->baro_W; b.p_ext = ctx->p_ext;
     b.nkT = ctx->P * kKB * ctx->T;
     b.c1 = std::exp(-(b.obabo ? 0.5 * ctx->dt : ctx->dt) * ctx->gamma0);
@@ -467,7 +468,7 @@ int pimd_get_neighbor_counts(pimd_ctx* ctx, int32_t* counts) {
 
 int64_t pimd_get_launch_count(const pimd_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
-int pimd_set_barostat(pimd_ctx* ctx, double p_ext_bar, double tau_p) {
+static int set_barostat(pimd_ctx* ctx, double p_ext_bar, double tau_p, bool aniso) {
     if (!ctx) return PIMD_EINVAL;
     if (!(tau_p > 0)) return fail(ctx, PIMD_EINVAL, "tau_p must be positive");
     if (ctx->fixcom) return fail(ctx, PIMD_EINVAL, "the barostat is not available with fixcom (DESIGN R-24)");
@@ -481,10 +482,15 @@ int pimd_set_barostat(pimd_ctx* ctx, double p_ext_bar, double tau_p) {
     CK(cudaMemcpyAsync(ctx->baro_state, st, sizeof(st), cudaMemcpyHostToDevice, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
     ctx->baro = true;
+    ctx->baro_aniso = aniso;
     ctx->p_ext = p_ext_bar / kBarPerEvA3;
-    ctx->baro_W = 3.0 * ctx->P * ctx->N * kKB * ctx->T * tau_p * tau_p;
+    // W = 3 n N k_B T tau_p^2, anisotropic n N k_B T tau_p^2 (L397)
+    ctx->baro_W = (aniso ? 1.0 : 3.0) * ctx->P * ctx->N * kKB * ctx->T * tau_p * tau_p;
     return refresh(ctx);
 }
+
+int pimd_set_barostat(pimd_ctx* ctx, double p_ext_bar, double tau_p) { return set_barostat(ctx, p_ext_bar, tau_p, false); }
+int pimd_set_barostat_aniso(pimd_ctx* ctx, double p_ext_bar, double tau_p) { return set_barostat(ctx, p_ext_bar, tau_p, true); }
 
 int pimd_get_barostat(pimd_ctx* ctx, pimd_barostat_state* b) {
     if (!ctx || !b) return fail(ctx, PIMD_EINVAL, "null argument");
@@ -494,13 +500,19 @@ int pimd_get_barostat(pimd_ctx* ctx, pimd_barostat_state* b) {
     CK(cudaMemcpyAsync(raw, ctx->est + (size_t)kEstCap * kEstWidth, sizeof(raw), cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
     const double n = ctx->P, N = ctx->N;
-    b->v_W = st[BS_VW];
-    for (int c = 0; c < 3; ++c) b->box[c] = st[BS_LX + c];
+    b->K_W = 0.0;
+    for (int c = 0; c < 3; ++c) {
+        b->box[c] = st[BS_LX + c];
+        b->v_W3[c] = st[BS_VW + c];
+        b->P_CV3[c] = st[BS_PCV + c] * kBarPerEvA3;                                        // E3 diagonal
+        if (ctx->baro_aniso) b->K_W += 0.5 * ctx->baro_W * st[BS_VW + c] * st[BS_VW + c];  // A14
+    }
+    b->v_W = (st[BS_VW] + st[BS_VW + 1] + st[BS_VW + 2]) / 3.0;
+    if (!ctx->baro_aniso) b->K_W = 0.5 * ctx->baro_W * st[BS_VW] * st[BS_VW];              // A13
     b->V = st[BS_LX] * st[BS_LY] * st[BS_LZ];
-    b->P_CV = st[BS_PCV] * kBarPerEvA3;
+    b->P_CV = (st[BS_PCV] + st[BS_PCV + 1] + st[BS_PCV + 2]) / 3.0 * kBarPerEvA3;          // A12 = the mean of E3's diagonal
     b->P_PR = (3.0 * n * N * kKB * ctx->T - 2.0 * raw[1]) / (3.0 * b->V) * kBarPerEvA3;    // A10
     b->P_MD = (2.0 * raw[0] + st[BS_TRXI]) / (3.0 * b->V) * kBarPerEvA3;                   // A11
-    b->K_W = 0.5 * ctx->baro_W * b->v_W * b->v_W;                                          // A13
     b->U_W = n * ctx->p_ext * b->V;                                                        // A15
     b->J_W = -n * kKB * ctx->T * std::log(b->V);                                           // A16
     b->enthalpy = raw[0] + raw[1] + raw[3] + b->K_W + b->U_W + b->J_W;                     // A17

@@ -54,12 +54,14 @@ struct IntegratorArgs {
 };
 
 // Barostat state on the device (Appendix E; DESIGN R-20..R-25), doubles:
-enum BaroSlot { BS_VW = 0, BS_LX = 1, BS_LY = 2, BS_LZ = 3, BS_PCV = 4, BS_TRXI = 5,
-                BS_EA1 = 6, BS_SH1 = 7, BS_EM1 = 8, BS_EA2 = 9, BS_SH2 = 10, BS_EM2 = 11,
-                BS_SKIN = 12, BS_SCV = 13, BS_SFV = 14, BS_SFF = 15, BS_WIDTH = 16 };
+enum BaroSlot { BS_VW = 0 /* [3], equal in isotropic mode */, BS_LX = 3, BS_LY = 4, BS_LZ = 5,
+                BS_PCV = 6 /* [3] diagonal of Eq. E3, eV/A^3 */, BS_TRXI = 9,
+                BS_FAC = 10 /* [3][6]: e^{h v}, sinh(h v)/v, e^{-h v} of the first and the second half drift */,
+                BS_WIDTH = 32 };
 struct BaroArgs {
     int P, N, n_dof;
     int close, start, thermostat;
+    int aniso;                   // one cell velocity per Cartesian component (Eq. E2-E3) instead of one (E1)
     int obabo;                   // OBABO: O(dt/2) twice around the kicks, one drift of dt (R-24)
     double h;                    // dt/2
     double W, p_ext;             // barostat mass (eV ps^2), target pressure (eV/A^3)
@@ -71,7 +73,7 @@ struct BaroArgs {
     uint32_t cstep_lo, cstep_hi; // OBABO: the step this launch closes, bit 31 of word 1 set
     const double* x; const double* vt; const double* f; const double* mass; const double* Xi;
     double* state;               // [BS_WIDTH]
-    double* partial;             // [blocks][kBaroSums] block partials of the sums
+    double* partial;             // [blocks][3][kBaroSums] block partials of the sums, per Cartesian component
 };
 constexpr int kBaroSums = 7;     // S_kin, S_cv, S_fv, S_ff, and (OBABO) S_kin after kick + closing O, S_kin and S_fv after the opening O
 int launch_barostat(const BaroArgs& a, cudaStream_t s);

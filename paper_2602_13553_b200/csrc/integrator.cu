@@ -189,11 +189,12 @@ integrator_kernel(const __grid_constant__ IntegratorArgs a, const __grid_constan
                 if (k == 0 && a.baro != nullptr) {
                     // BZP barostat (Eq. E4/E5, L507-512; R-21: centroid mode only): the two half drifts with the
                     // cell velocity before and after its own thermostat step (barostat.cu prepared the factors)
-                    const double xn = a.baro[BS_EA1] * x + a.baro[BS_SH1] * v;
-                    double vn = a.baro[BS_EM1] * v;
+                    const double* bf = a.baro + BS_FAC + 6 * alpha;
+                    const double xn = bf[0] * x + bf[1] * v;
+                    double vn = bf[2] * v;
                     if (thermo) vn = mc.c1[k] * vn + mc.c2[k] * sigma * eta_s[k * kIntThreads];
-                    xt[k] = a.baro[BS_EA2] * xn + a.baro[BS_SH2] * vn;
-                    v = a.baro[BS_EM2] * vn;
+                    xt[k] = bf[3] * xn + bf[4] * vn;
+                    v = bf[5] * vn;
                 } else {
                     const double xn = mc.cosA[k] * x + mc.sinA_w[k] * v;    // A(dt/2): exact rotation (R-5)
                     double vn = mc.msinA_w[k] * x + mc.cosA[k] * v;
@@ -230,8 +231,9 @@ integrator_kernel(const __grid_constant__ IntegratorArgs a, const __grid_constan
                 v += kick * ft[k];
                 const double x = xt[k];
                 if (k == 0 && a.baro != nullptr) {           // BZP barostat: Eq. E4/E5 over dt on the centroid mode
-                    xt[k] = a.baro[BS_EA1] * x + a.baro[BS_SH1] * v;
-                    v = a.baro[BS_EM1] * v;
+                    const double* bf = a.baro + BS_FAC + 6 * alpha;
+                    xt[k] = bf[0] * x + bf[1] * v;
+                    v = bf[2] * v;
                 } else {
                     xt[k] = mc.cosA[k] * x + mc.sinA_w[k] * v;
                     v = mc.msinA_w[k] * x + mc.cosA[k] * v;

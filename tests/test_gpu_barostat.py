@@ -43,12 +43,15 @@ def _compare_state(bs, bo, tol):
         scale = max(abs(bo[key]), abs(bo["P_MD"]) if key.startswith("P_") else 0.0, 1e-3 if key == "v_W" else 0.0)
         assert abs(bs[key] - bo[key]) <= tol * max(scale, 1e-12), (key, bs[key], bo[key])
     assert _rel(bs["box"], bo["box"]) <= tol
+    assert np.abs(bs["v_W3"] - bo["v_W3"]).max() <= tol * max(np.abs(bo["v_W3"]).max(), 1e-3)
+    assert np.abs(bs["P_CV3"] - bo["P_CV3"]).max() <= tol * max(np.abs(bo["P_CV3"]).max(), abs(bo["P_MD"]))
 
 
+@pytest.mark.parametrize("aniso", [False, True])
 @pytest.mark.parametrize("integ", ["baoab", "obabo"])
 @pytest.mark.parametrize("P", [1, 4, 32, 64])
 @pytest.mark.parametrize("gamma", [0.0, 20.0])
-def test_barostat_parity_harmonic(pk, P, gamma, integ):
+def test_barostat_parity_harmonic(pk, P, gamma, integ, aniso):
     N = 43                                           # 129 dofs: one full 128-thread block and a tail of one
     types, masses, x, p = _trap_system(N, P, seed=20 + P)
     box = [10.0, 11.0, 12.0]
@@ -57,9 +60,9 @@ def test_barostat_parity_harmonic(pk, P, gamma, integ):
     sim = pk.PIMD(*args, seed=5, integrator=integ)
     sim.set_state(x, p)
     sim.set_model_harmonic(0.5)
-    sim.set_barostat(p_ext, 0.05)
+    sim.set_barostat(p_ext, 0.05, aniso=aniso)
     orc = OraclePIMD(*args, seed=5, integrator=integ)
-    orc.set_barostat(p_ext, 0.05)
+    orc.set_barostat(p_ext, 0.05, aniso=aniso)
     orc.set_state(x, p)
     orc.set_model_harmonic(0.5)
     _compare_state(sim.barostat_state(), orc.barostat_state(), 1e-11)
@@ -75,21 +78,23 @@ def test_barostat_parity_harmonic(pk, P, gamma, integ):
     bs, bo = sim.barostat_state(), orc.barostat_state()
     _compare_state(bs, bo, 1e-9)
     assert abs(bo["V"] / 1320.0 - 1.0) > 1e-3 and bo["v_W"] != 0.0          # the cell really moved
+    assert (np.ptp(bo["v_W3"]) > 0) == aniso
     e, o = sim.estimators(), orc.estimators()
     for key in ("K_PR", "K_CV", "H", "K_ring", "S_ring", "U_sum"):
         assert abs(e[key] - o[key]) <= 1e-9 * max(1.0, abs(o[key])), key
     sim.close()
 
 
+@pytest.mark.parametrize("aniso", [False, True])
 @pytest.mark.parametrize("integ", ["baoab", "obabo"])
-def test_nph_enthalpy_is_conserved_on_the_gpu(pk, integ):
+def test_nph_enthalpy_is_conserved_on_the_gpu(pk, integ, aniso):
     """Eq. A17 over 2000 steps of the CUDA path alone (a property that holds at any size)."""
     P, N = 8, 64
     types, masses, x, p = _trap_system(N, P, seed=3)
     sim = pk.PIMD(types, masses, [10.0] * 3, P, 300.0, 0.5e-3, 0.0, seed=1, integrator=integ)
     sim.set_state(x, p)
     sim.set_model_harmonic(0.5)
-    sim.set_barostat(KB * 300.0 / 1000.0 * BAR, 0.05)
+    sim.set_barostat(KB * 300.0 / 1000.0 * BAR, 0.05, aniso=aniso)
     h0 = sim.barostat_state()["enthalpy"]
     dev = []
     for _ in range(20):
@@ -153,8 +158,8 @@ def test_split_calls_agree_with_one_call_under_the_barostat(pk):
     assert _rel(out[0][2]["box"], out[1][2]["box"]) < 1e-14
 
 
-@pytest.mark.parametrize("integ", ["baoab", "obabo"])
-def test_full_npt_step_parity_config0(pk, integ):
+@pytest.mark.parametrize("integ,aniso", [("baoab", False), ("obabo", False), ("baoab", True), ("obabo", True)])
+def test_full_npt_step_parity_config0(pk, integ, aniso):
     """configs[0] geometry and model under NpT at 1 bar (configs[4]'s ensemble at the size the oracle finishes):
     multi-image neighbours from a cell that changes every step.  OBABO + npt is the paper's own example command
     (PAPER.md:L82)."""
@@ -163,9 +168,9 @@ def test_full_npt_step_parity_config0(pk, integ):
     sim = pk.PIMD(*args, seed=11, model_desc=desc, integrator=integ)
     sim.set_state(wb["x"], wb["p"])
     sim.set_model(w)
-    sim.set_barostat(1.0, 0.02)
+    sim.set_barostat(1.0, 0.02, aniso=aniso)
     orc = OraclePIMD(*args, seed=11, integrator=integ)
-    orc.set_barostat(1.0, 0.02)
+    orc.set_barostat(1.0, 0.02, aniso=aniso)
     orc.set_state(wb["x"], wb["p"])
     orc.set_model(desc, w)
 
@@ -175,6 +180,7 @@ def test_full_npt_step_parity_config0(pk, integ):
         big = abs(trXi) / (3.0 * bo["V"]) * BAR
         for key in ("P_CV", "P_MD"):
             assert abs(bs[key] - bo[key]) <= 1e-4 * max(big, abs(bo[key])), (key, bs[key], bo[key], big)
+        assert np.abs(bs["P_CV3"] - bo["P_CV3"]).max() <= 1e-4 * max(big, np.abs(bo["P_CV3"]).max())
         assert abs(bs["P_PR"] - bo["P_PR"]) <= 1e-6 * abs(bo["P_PR"])
 
     pressures_close(sim.barostat_state(), orc.barostat_state())
@@ -190,7 +196,8 @@ def test_full_npt_step_parity_config0(pk, integ):
     # the cell integrates the FP32-level virial: its bar is that of the positions it scales
     assert _rel(bs["box"], bo["box"]) <= 1e-6
     assert abs(bs["v_W"] - bo["v_W"]) <= 1e-4 * max(abs(bo["v_W"]), 1e-3)
-    assert bo["V"] != float(np.prod(wb["box"]))
+    assert np.abs(bs["v_W3"] - bo["v_W3"]).max() <= 1e-4 * max(np.abs(bo["v_W3"]).max(), 1e-3)
+    assert bo["V"] != float(np.prod(wb["box"])) and (np.ptp(bo["box"]) > 0) == aniso
     pressures_close(bs, bo)
     assert abs(bs["enthalpy"] - bo["enthalpy"]) <= 1e-6 * sim.N * sim.P
     sim.close()
