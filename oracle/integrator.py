@@ -108,6 +108,58 @@ def obabo_finish(vt, f, masses, M, om, T, gamma0, dt, seed, step):
     return vt, ft
 
 
+# ---- `method pimd`: integration in Cartesian coordinates (Eq. D3) ------------------------
+
+def spring_force_cart(x, masses, wP):
+    """-dS/dx of the ring springs of Eq. 1 (omega_n squared by DESIGN R-1), Cartesian:
+    F^spring_k = -m omega_n^2 (2 x_k - x_{k-1} - x_{k+1}), beads cyclic; eV/A via mvv2e."""
+    m = masses[None, :, None]
+    return -m * wP * wP * MVV2E * (2.0 * x - np.roll(x, 1, axis=0) - np.roll(x, -1, axis=0))
+
+
+def o_step_cart(v, masses, T, wP, gamma0, h, seed, step, half=0):
+    """Eq. D3: v_k <- c1 v_k + c2 sqrt(n/(m beta)) eta for EVERY bead k with the same
+    c1 = exp(-h/tau_0), tau_0 = 1/(2 omega_n) (L478: "the default damping time is tau_k = 1/(2 omega_n),
+    k = 0..n-1"; DESIGN R-27: the `tau` keyword does not enter, gamma0 == 0 still means no thermostat).
+    eta(seed; step, k, i, alpha) is the stream of Eq. D2 with the bead index in place of the mode index."""
+    if gamma0 == 0.0:
+        return v.copy()
+    P, N, _ = v.shape
+    c1 = np.exp(-h * 2.0 * wP)
+    c2 = np.sqrt(1.0 - c1 * c1)
+    kk, ii, aa = np.meshgrid(np.arange(P), np.arange(N), np.arange(3), indexing="ij")
+    eta = philox.normal(seed, step, kk, ii, aa, half)
+    sigma = np.sqrt(P * KB * T / (masses * MVV2E))
+    return c1 * v + c2 * sigma[None, :, None] * eta
+
+
+def cart_kick(v, x, f, masses, wP, h):
+    """B in Cartesian coordinates: the bead force plus the ring-spring force (both terms of Eq. 1's potential)."""
+    return v + h * (f + spring_force_cart(x, masses, wP)) / (masses[None, :, None] * MVV2E)
+
+
+def cart_positions_half(x, v, f, masses, T, wP, gamma0, dt, seed, step, obabo):
+    """First part of one Cartesian step (DESIGN R-27; A is the plain drift x += h v, L165 "position update"):
+    BAOAB: B(dt/2) A(dt/2) O(dt) A(dt/2);  OBABO: O(dt/2) B(dt/2) A(dt)."""
+    if obabo:
+        v = o_step_cart(v, masses, T, wP, gamma0, 0.5 * dt, seed, step, half=0)
+        v = cart_kick(v, x, f, masses, wP, 0.5 * dt)
+        return x + dt * v, v
+    v = cart_kick(v, x, f, masses, wP, 0.5 * dt)
+    x = x + 0.5 * dt * v
+    v = o_step_cart(v, masses, T, wP, gamma0, dt, seed, step)
+    x = x + 0.5 * dt * v
+    return x, v
+
+
+def cart_finish(x, v, f, masses, T, wP, gamma0, dt, seed, step, obabo):
+    """Second part: B(dt/2) with the new bead forces and the springs at the new positions (+ O(dt/2) for OBABO)."""
+    v = cart_kick(v, x, f, masses, wP, 0.5 * dt)
+    if obabo:
+        v = o_step_cart(v, masses, T, wP, gamma0, 0.5 * dt, seed, step, half=1)
+    return v
+
+
 def remove_centroid_com(vt, masses):
     """`fixcom yes`: "the center-of-mass velocity is removed in every timestep for the
     centroid mode" (nmpimd).  v~_0,i <- v~_0,i - sum_j m_j v~_0,j / sum_j m_j, per Cartesian component;

@@ -13,7 +13,8 @@ from . import nm, integrator, se_e2_a, barostat
 
 
 class OraclePIMD:
-    def __init__(self, types, masses_per_type, box, n_beads, T, dt, gamma_centroid, seed, integrator="baoab", fixcom=False):
+    def __init__(self, types, masses_per_type, box, n_beads, T, dt, gamma_centroid, seed, integrator="baoab", fixcom=False,
+                 method="nmpimd"):
         self.types = np.asarray(types, dtype=np.int64)
         self.N = self.types.size
         self.masses = np.asarray(masses_per_type, dtype=np.float64)[self.types]   # per atom
@@ -26,6 +27,9 @@ class OraclePIMD:
         assert integrator in ("baoab", "obabo")
         self.integrator = integrator
         self.fixcom = bool(fixcom)
+        assert method in ("nmpimd", "pimd")
+        self.method = method                             # PAPER.md:L164; "pimd" = Cartesian (DESIGN R-27)
+        assert not (self.method == "pimd" and self.fixcom)
         self.M = nm.nm_matrix(self.P)
         self.om = nm.omegas(self.P, self.T)
         self.step_count = 0
@@ -50,7 +54,7 @@ class OraclePIMD:
         Internally v~ = M (p/m) (velocities live in normal-mode form)."""
         self.x = np.array(x, dtype=np.float64).reshape(self.P, self.N, 3)
         v = np.asarray(p, dtype=np.float64).reshape(self.P, self.N, 3) / self.masses[None, :, None]
-        self.vt = nm.to_nm(self.M, v)
+        self.vt = v.copy() if self.method == "pimd" else nm.to_nm(self.M, v)     # `pimd`: vt holds Cartesian v
         self.step_count = 0
         if self.model is not None or self.k_spring is not None:
             self._forces()
@@ -70,7 +74,7 @@ class OraclePIMD:
     def set_barostat(self, p_ext_bar, tau_p, aniso=False):
         """`iso p_ext barostat BZP taup tau_p`: isotropic target pressure in bar,
         barostat mass W = 3 n N k_B T tau_p^2 (L389); v_W starts at 0.  Sub-step order: DESIGN R-24."""
-        assert not self.fixcom
+        assert not self.fixcom and self.method == "nmpimd"
         self.baro = True
         self.p_ext = float(p_ext_bar) / barostat.BAR_PER_EV_A3
         self.aniso = bool(aniso)                     # PAPER.md:L176 `aniso`: one v_W per cell vector (Eq. E2-E3, A14)
@@ -154,8 +158,21 @@ class OraclePIMD:
         self._press_o(h, half=1)
         self.step_count += 1
 
+    def _cart_step(self):
+        wP = nm.omega_P(self.P, self.T)
+        ob = self.integrator == "obabo"
+        self.x, self.vt = integrator.cart_positions_half(self.x, self.vt, self.f, self.masses, self.T, wP,
+                                                         self.gamma0, self.dt, self.seed, self.step_count, ob)
+        self._forces()
+        self.vt = integrator.cart_finish(self.x, self.vt, self.f, self.masses, self.T, wP, self.gamma0, self.dt,
+                                         self.seed, self.step_count, ob)
+        self.step_count += 1
+
     def step(self, n_steps=1):
         for _ in range(int(n_steps)):
+            if self.method == "pimd":
+                self._cart_step()
+                continue
             if self.baro:
                 if self.integrator == "obabo":
                     self._npt_step_obabo()
@@ -188,6 +205,8 @@ class OraclePIMD:
 
     def momenta(self):
         """Cartesian bead momenta p = m M^T v~."""
+        if self.method == "pimd":
+            return self.vt * self.masses[None, :, None]
         return nm.from_nm(self.M, self.vt) * self.masses[None, :, None]
 
     def forces(self):
@@ -200,7 +219,8 @@ class OraclePIMD:
         return self.U.copy()
 
     def estimators(self):
-        e = integrator.estimators(self.x, self.vt, self.f, self.U, self.masses, self.M, self.om, self.T)
+        vt = nm.to_nm(self.M, self.vt) if self.method == "pimd" else self.vt      # Appendix A is written in v~
+        e = integrator.estimators(self.x, vt, self.f, self.U, self.masses, self.M, self.om, self.T)
         e["step"] = self.step_count
         return e
 

@@ -299,3 +299,100 @@ def test_harmonic_oscillator_matches_finite_P_closed_form(integ):
         assert abs(mean - exact_P) < max(5 * err, floor), (name, mean, err, exact_P)
     mean, err = blocked(tring)
     assert abs(mean / (P * T) - 1.0) < max(5 * err / (P * T), 3e-3)   # ring temperature averages n*T (L194)
+
+
+# ---------------------------------------------------------------- `method pimd` (Cartesian, Eq. D3)
+def _cart_pair(P, N, dt, gamma0, integ="baoab", seed=5):
+    """The same harmonic system under `nmpimd` and `pimd`."""
+    T, mass = 300.0, 1.008
+    omega = 4.0 * C.KB * T / C.HBAR
+    ks = mass * C.MVV2E * omega ** 2
+    rng = np.random.default_rng(seed)
+    x0 = math.sqrt(C.KB * T / ks) * rng.standard_normal((1, N, 3)) + 0.02 * rng.standard_normal((P, N, 3))
+    p0 = math.sqrt(mass * P * C.KB * T / C.MVV2E) * rng.standard_normal((P, N, 3))
+    sims = []
+    for method in ("nmpimd", "pimd"):
+        o = OraclePIMD(np.zeros(N, dtype=int), [mass], [100.0] * 3, P, T, dt, gamma0, 9, integrator=integ, method=method)
+        o.set_model_harmonic(ks)
+        o.set_state(x0, p0)
+        sims.append(o)
+    return sims
+
+
+def test_cartesian_spring_force_is_minus_the_gradient_of_A3():
+    P, N, T = 8, 3, 300.0
+    rng = np.random.default_rng(1)
+    masses = np.array([15.9994, 1.008, 1.008])
+    x = rng.standard_normal((P, N, 3))
+    wP = nm.omega_P(P, T)
+
+    def S(xx):
+        dr = xx - np.roll(xx, -1, axis=0)
+        return 0.5 * np.sum(masses[None, :, None] * wP * wP * dr * dr) * C.MVV2E
+
+    F = integrator.spring_force_cart(x, masses, wP)
+    for (k, i, a) in [(0, 0, 0), (3, 1, 2), (7, 2, 1)]:
+        xp, xm = x.copy(), x.copy()
+        xp[k, i, a] += 1e-5
+        xm[k, i, a] -= 1e-5
+        assert F[k, i, a] == pytest.approx(-(S(xp) - S(xm)) / 2e-5, rel=1e-7)
+    np.testing.assert_allclose(F.sum(axis=0), 0.0, atol=1e-9 * np.abs(F).max())      # internal forces
+
+
+@pytest.mark.parametrize("integ", ["baoab", "obabo"])
+def test_cartesian_and_normal_mode_integration_converge_to_each_other(integ):
+    """Both integrate Eq. 1; `nmpimd` treats the springs exactly, `pimd` by the kick-drift splitting, so at
+    gamma = 0 their trajectories differ by O(dt^2) after a fixed time (pins sign and size of the spring term)."""
+    diffs = []
+    for dt, n in ((1.0e-4, 100), (0.5e-4, 200)):
+        a, b = _cart_pair(4, 5, dt, 0.0, integ)
+        a.step(n)
+        b.step(n)
+        diffs.append(np.abs(a.positions() - b.positions()).max() / np.abs(a.positions()).max())
+        np.testing.assert_allclose(a.momenta(), b.momenta(), rtol=0, atol=50 * diffs[-1] * np.abs(a.momenta()).max())
+    assert diffs[0] < 2e-3 and diffs[1] < 0.3 * diffs[0]
+
+
+def test_cartesian_nve_conserves_A6_and_obabo_equals_baoab():
+    drift = []
+    for dt, n in ((1.0e-4, 400), (0.5e-4, 800)):
+        _, b = _cart_pair(8, 6, dt, 0.0)
+        H0 = b.estimators()["H"]
+        dev = 0.0
+        for _ in range(n // 50):
+            b.step(50)
+            dev = max(dev, abs(b.estimators()["H"] - H0) / abs(H0))
+        drift.append(dev)
+    assert drift[0] < 1e-3 and drift[1] < 0.45 * drift[0]                    # ~dt^2
+    _, b1 = _cart_pair(4, 5, 1e-4, 0.0, "baoab")
+    _, b2 = _cart_pair(4, 5, 1e-4, 0.0, "obabo")
+    b1.step(20)
+    b2.step(20)
+    np.testing.assert_allclose(b1.positions(), b2.positions(), rtol=0, atol=1e-12)
+
+
+def test_D3_thermostat_is_the_same_for_every_bead_and_uses_the_bead_keyed_stream():
+    P, N, T, h, seed = 4, 3, 300.0, 1e-3, 21
+    masses = np.array([15.9994, 1.008, 1.008])
+    wP = nm.omega_P(P, T)
+    v = np.random.default_rng(2).standard_normal((P, N, 3))
+    out = integrator.o_step_cart(v, masses, T, wP, 1.0, h, seed, 7, half=1)
+    c1 = math.exp(-h * 2.0 * wP)                                    # tau = 1/(2 omega_n), L478
+    kk, ii, aa = np.meshgrid(np.arange(P), np.arange(N), np.arange(3), indexing="ij")
+    eta = philox.normal(seed, 7, kk, ii, aa, 1)
+    sig = np.sqrt(P * C.KB * T / (masses * C.MVV2E))
+    np.testing.assert_allclose(out, c1 * v + math.sqrt(1 - c1 * c1) * sig[None, :, None] * eta, rtol=1e-14)
+    np.testing.assert_array_equal(integrator.o_step_cart(v, masses, T, wP, 0.0, h, seed, 7), v)     # NVE
+
+
+def test_cartesian_thermostat_samples_the_ring_temperature():
+    """<K_ring> = 3 n N (n k_B T) / 2 under D3 alone plus free-ring dynamics (T_ring averages n T, L194)."""
+    P, N = 4, 16
+    _, b = _cart_pair(P, N, 2.0e-4, 1.0)
+    b.set_model_harmonic(0.0)
+    b.step(300)
+    acc = []
+    for _ in range(120):
+        b.step(10)
+        acc.append(b.estimators()["T_ring"])
+    assert np.mean(acc) == pytest.approx(P * 300.0, rel=0.06)
