@@ -167,6 +167,16 @@ int pimd_debug_noise(pimd_ctx* ctx, int64_t step, int n, const int32_t* idx, uin
 #define PIMD_OBABO 1
 int pimd_set_integrator(pimd_ctx* ctx, int kind);
 
+/* Coordinate system of the integration (keyword `method`).  PIMD_NMPIMD (default): normal modes, the
+ * north_star path.  PIMD_CART (`method pimd`): Cartesian coordinates -- B kicks with the bead force plus the ring-spring
+ * force of Eq. 1, A is the drift x += h v, and the thermostat is Eq. D3 (L478-484): the same tau = 1/(2 omega_n) on
+ * every bead, normals keyed by the bead index (DESIGN R-27); both splittings; estimators as in Appendix A.  Call it
+ * BEFORE pimd_set_state: a change of method drops the state (the stored velocities change representation).
+ * PIMD_EINVAL for an unknown method, or for PIMD_CART with fixcom or a barostat on (and those refuse under PIMD_CART). */
+#define PIMD_NMPIMD 0
+#define PIMD_CART 1
+int pimd_set_method(pimd_ctx* ctx, int method);
+
 /* `fixcom`: when on, the centre-of-mass velocity of the centroid mode is removed once per step,
  * after the step's last velocity update and before its estimators (DESIGN R-19).  Off by default (north_star's
  * create() list has no such argument).  The removal needs a reduction over all atoms between the closing and the

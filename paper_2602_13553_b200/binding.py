@@ -82,6 +82,7 @@ _SIGNATURES = {
     "pimd_set_fitting_path": (C.c_int, [C.c_void_p, C.c_int]),
     "pimd_set_integrator": (C.c_int, [C.c_void_p, C.c_int]),
     "pimd_set_fixcom": (C.c_int, [C.c_void_p, C.c_int]),
+    "pimd_set_method": (C.c_int, [C.c_void_p, C.c_int]),
     "pimd_set_barostat": (C.c_int, [C.c_void_p, C.c_double, C.c_double]),
     "pimd_set_barostat_aniso": (C.c_int, [C.c_void_p, C.c_double, C.c_double]),
     "pimd_get_barostat": (C.c_int, [C.c_void_p, C.c_void_p]),
@@ -206,6 +207,15 @@ def pimd_set_integrator(ctx, kind):
     if isinstance(kind, str):
         kind = {"baoab": PIMD_BAOAB, "obabo": PIMD_OBABO}[kind.lower()]
     return _check(ctx, lib().pimd_set_integrator(ctx, int(kind)))
+
+
+PIMD_NMPIMD, PIMD_CART = 0, 1
+
+
+def pimd_set_method(ctx, method):
+    if isinstance(method, str):
+        method = {"nmpimd": PIMD_NMPIMD, "pimd": PIMD_CART}[method]
+    return _check(ctx, lib().pimd_set_method(ctx, int(method)))
 
 
 def pimd_set_fixcom(ctx, on):
@@ -354,11 +364,13 @@ class PIMD:
     """Convenience owner of one context (create .. destroy) with the shapes remembered."""
 
     def __init__(self, types, masses, box, n_beads, T, dt, gamma_centroid, seed, model_desc=None,
-                 torch_workspace=True, integrator="baoab", fixcom=False):
+                 torch_workspace=True, integrator="baoab", fixcom=False, method="nmpimd"):
         self.N, self.P = int(np.asarray(types).size), int(n_beads)
         self.ctx = pimd_create(types, masses, box, n_beads, T, dt, gamma_centroid, seed)
         if integrator != "baoab":
             pimd_set_integrator(self.ctx, integrator)
+        if method != "nmpimd":
+            pimd_set_method(self.ctx, method)
         if fixcom:
             pimd_set_fixcom(self.ctx, True)
         self.desc = ModelDesc.from_dict(model_desc) if isinstance(model_desc, dict) else model_desc

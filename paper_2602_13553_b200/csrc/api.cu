@@ -18,6 +18,7 @@ struct pimd_ctx {
     int64_t launches = 0;
     int integrator = PIMD_BAOAB;
     bool fixcom = false;
+    int method = PIMD_NMPIMD;
     double* com = nullptr;        // [3] device: centroid COM momentum (fixcom)
     double inv_mtot = 0;
     bool baro = false;            // BZP barostat (Appendix E)
@@ -159,7 +160,8 @@ void mode_constants(pimd_ctx* c) {
             c->mc.sinA_w[k] = std::sin(w * h) / w;
             c->mc.msinA_w[k] = -w * std::sin(w * h);
         }
-        const double gam = (k == 0) ? c->gamma0 : 2.0 * w;  // Eq. D1; tau_0 = 1/gamma0 (L174)
+        double gam = (k == 0) ? c->gamma0 : 2.0 * w;  // Eq. D1; tau_0 = 1/gamma0 (L174)
+        if (c->method == PIMD_CART) gam = 2.0 * wP;   // Eq. D3: tau = 1/(2 omega_n) for every bead (R-27)
         c->mc.c1[k] = std::exp(-ho * gam);
         c->mc.c2[k] = std::sqrt(1.0 - c->mc.c1[k] * c->mc.c1[k]);
     }
@@ -244,6 +246,8 @@ void fill_integrator_args(pimd_ctx* ctx, IntegratorArgs& a, int flags, int64_t s
     a.mass = ctx->mass_atom; a.U = ctx->U; a.est = est_slot;
     a.com = ctx->com; a.inv_mtot = ctx->inv_mtot;
     a.baro = ctx->baro ? ctx->baro_state : nullptr;
+    { const double wP = ctx->P * kKB * ctx->T / kHbar; a.wP2 = wP * wP; }
+    if (ctx->method == PIMD_CART) a.flags |= I_CART;
 }
 
 constexpr double kBarPerEvA3 = 1.602176634e6;    // DESIGN R-25
@@ -416,7 +420,9 @@ int pimd_set_state_dev(pimd_ctx* ctx, const double* x_dev, const double* p_dev) 
     if ((rc = alloc_base(ctx))) return rc;
     const size_t PN3 = (size_t)ctx->P * ctx->N * 3;
     CK(cudaMemcpyAsync(ctx->x, x_dev, PN3 * 8, cudaMemcpyDeviceToDevice, ctx->stream));
-    ctx->launches += launch_to_nm_velocity(ctx->P, ctx->N, p_dev, ctx->mass_atom, ctx->vt, ctx->stream);
+    ctx->launches += ctx->method == PIMD_CART
+        ? launch_cart_convert(ctx->P, ctx->N, p_dev, ctx->mass_atom, ctx->vt, 1, ctx->stream)
+        : launch_to_nm_velocity(ctx->P, ctx->N, p_dev, ctx->mass_atom, ctx->vt, ctx->stream);
     CK(cudaGetLastError());
     ctx->have_state = true;
     ctx->step = 0;
@@ -443,7 +449,9 @@ int pimd_restore(pimd_ctx* ctx, const double* x, const double* p, const double* 
     CK(cudaMemcpyAsync(ctx->scratch_b, p, PN3 * 8, cudaMemcpyHostToDevice, ctx->stream));
     CK(cudaMemcpyAsync(ctx->f, f, PN3 * 8, cudaMemcpyHostToDevice, ctx->stream));
     CK(cudaMemcpyAsync(ctx->U, U, sizeof(double) * ctx->P, cudaMemcpyHostToDevice, ctx->stream));
-    ctx->launches += launch_to_nm_velocity(ctx->P, ctx->N, ctx->scratch_b, ctx->mass_atom, ctx->vt, ctx->stream);
+    ctx->launches += ctx->method == PIMD_CART
+        ? launch_cart_convert(ctx->P, ctx->N, ctx->scratch_b, ctx->mass_atom, ctx->vt, 1, ctx->stream)
+        : launch_to_nm_velocity(ctx->P, ctx->N, ctx->scratch_b, ctx->mass_atom, ctx->vt, ctx->stream);
     ctx->have_state = true;
     ctx->step = step;
     double* cur = ctx->est + (size_t)kEstCap * kEstWidth;
@@ -472,6 +480,7 @@ static int set_barostat(pimd_ctx* ctx, double p_ext_bar, double tau_p, bool anis
     if (!ctx) return PIMD_EINVAL;
     if (!(tau_p > 0)) return fail(ctx, PIMD_EINVAL, "tau_p must be positive");
     if (ctx->fixcom) return fail(ctx, PIMD_EINVAL, "the barostat is not available with fixcom (DESIGN R-24)");
+    if (ctx->method == PIMD_CART) return fail(ctx, PIMD_EINVAL, "the barostat needs the normal-mode method (DESIGN R-27)");
     if (!ctx->baro_state) {
         int rc = arena_alloc(ctx, &ctx->baro_state, barostat_state_doubles(3 * ctx->N));
         if (rc) return rc;
@@ -519,8 +528,20 @@ int pimd_get_barostat(pimd_ctx* ctx, pimd_barostat_state* b) {
     return PIMD_OK;
 }
 
+int pimd_set_method(pimd_ctx* ctx, int method) {
+    if (!ctx) return PIMD_EINVAL;
+    if (method != PIMD_NMPIMD && method != PIMD_CART) return fail(ctx, PIMD_EINVAL, "unknown method");
+    if (method == PIMD_CART && (ctx->baro || ctx->fixcom))
+        return fail(ctx, PIMD_EINVAL, "the Cartesian method is implemented without barostat and fixcom (DESIGN R-27)");
+    if (method != ctx->method) ctx->have_state = false;      // the stored velocities change representation
+    ctx->method = method;
+    mode_constants(ctx);
+    return PIMD_OK;
+}
+
 int pimd_set_fixcom(pimd_ctx* ctx, int on) {
     if (!ctx) return PIMD_EINVAL;
+    if (on && ctx->method == PIMD_CART) return fail(ctx, PIMD_EINVAL, "fixcom is not available with the Cartesian method (DESIGN R-27)");
     if (on && ctx->baro) return fail(ctx, PIMD_EINVAL, "fixcom is not available with the barostat (DESIGN R-24)");
     ctx->fixcom = on != 0;
     return PIMD_OK;
@@ -789,7 +810,9 @@ int pimd_get_positions(pimd_ctx* ctx, double* x) {
 int pimd_get_momenta(pimd_ctx* ctx, double* p) {
     if (!ctx || !p) return fail(ctx, PIMD_EINVAL, "null argument");
     if (!ctx->have_state) return fail(ctx, PIMD_ENOSTATE, "pimd_set_state has not been called");
-    ctx->launches += launch_from_nm_momenta(ctx->P, ctx->N, ctx->vt, ctx->mass_atom, ctx->scratch_a, ctx->stream);
+    ctx->launches += ctx->method == PIMD_CART
+        ? launch_cart_convert(ctx->P, ctx->N, ctx->vt, ctx->mass_atom, ctx->scratch_a, 0, ctx->stream)
+        : launch_from_nm_momenta(ctx->P, ctx->N, ctx->vt, ctx->mass_atom, ctx->scratch_a, ctx->stream);
     return copy_out(ctx, ctx->scratch_a, p, (size_t)ctx->P * ctx->N * 24);
 }
 int pimd_get_forces(pimd_ctx* ctx, double* f) {

@@ -22,7 +22,7 @@ constexpr int kEstCap   = 4096;     // estimator history slots per pimd_step cal
 constexpr int kEstWidth = 4;        // K_ring, S_ring, sum x.f - x~0.f~0, U_sum
 
 // integrator launch flags
-enum : int { I_BCLOSE = 1, I_EST = 2, I_START = 4, I_OBABO = 8, I_COMACC = 16, I_COMSUB = 32 };
+enum : int { I_BCLOSE = 1, I_EST = 2, I_START = 4, I_OBABO = 8, I_COMACC = 16, I_COMSUB = 32, I_CART = 64 };
 
 // Per-mode constants of the A and O steps (DESIGN R-3, R-5), kernel parameter.
 struct ModeConsts {
@@ -50,6 +50,7 @@ struct IntegratorArgs {
     double*  est;                // [kEstWidth] accumulators of this step's slot, may be null
     double*  com;                // [3] fixcom: sum_i m_i v~_0,i per component (I_COMACC adds, I_COMSUB reads)
     double   inv_mtot;           // 1 / sum_i m_i
+    double   wP2;                // omega_n^2 (Cartesian method: ring-spring force)
     const double* baro;          // barostat state (BaroSlot layout) or null: centroid drift by Eq. E4/E5
 };
 
@@ -80,6 +81,7 @@ int launch_barostat(const BaroArgs& a, cudaStream_t s);
 size_t barostat_state_doubles(int n_dof);    // BS_WIDTH + the partials
 
 int launch_integrator(int P, const IntegratorArgs& a, const ModeConsts& mc, cudaStream_t s);
+int launch_cart_convert(int P, int N, const double* in, const double* mass, double* out, int forward, cudaStream_t s);
 int launch_to_nm_velocity(int P, int N, const double* p_cart, const double* mass, double* vt, cudaStream_t s);
 int launch_from_nm_momenta(int P, int N, const double* vt, const double* mass, double* p_cart, cudaStream_t s);
 int launch_harmonic(int P, int N, double k_spring, const double* x, double* f, double* U, double* Xi,

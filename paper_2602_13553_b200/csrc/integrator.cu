@@ -306,7 +306,166 @@ static void launch_int_t(const IntegratorArgs& a, const ModeConsts& mc, cudaStre
     else integrator_kernel<P, false><<<blocks, kIntThreads, smem, s>>>(a, mc);
 }
 
+// ---------------------------------------------------------------------------------------------
+// `method pimd` (Eq. D3; DESIGN R-27): the same fused launch in Cartesian coordinates.
+// No transforms: v is the Cartesian bead velocity, B kicks with the bead force plus the ring-spring force
+// -m omega_n^2 (2 x_k - x_{k-1} - x_{k+1}) (Eq. 1), A is the drift x += h v, O is Eq. D3 with the same
+// c1 = exp(-l 2 omega_n) on every bead (mc.c1[0], mc.c2[0]; mc.sinA_w[0] = the drift length).  Not the headline
+// path: plain coalesced loads, the normals of all beads staged in shared memory.
+// ---------------------------------------------------------------------------------------------
+template <int P, bool kObabo>
+__global__ void __launch_bounds__(kIntThreads)
+integrator_cart_kernel(const __grid_constant__ IntegratorArgs a, const __grid_constant__ ModeConsts mc) {
+    extern __shared__ double dyn_s[];
+    double* eta_s = dyn_s + threadIdx.x;
+    const int e = blockIdx.x * kIntThreads + threadIdx.x;
+    const bool live = e < a.n_dof;
+    const int ec = live ? e : a.n_dof - 1;
+    const int i = ec / 3, alpha = ec - 3 * i;
+    const bool start = (a.flags & I_START) != 0;
+    const bool close = (a.flags & I_BCLOSE) != 0;
+    const bool thermo = start && a.thermostat;
+    const size_t stride = (size_t)a.n_dof;
+    const double m = a.mass[i];
+    double x[P], v[P], g[P];             // g: total acceleration-kick h (f + f_spring)/(m mvv2e)
+#pragma unroll
+    for (int k = 0; k < P; ++k) { x[k] = a.x_in[k * stride + ec]; v[k] = a.vt_in[k * stride + ec]; g[k] = a.f[k * stride + ec]; }
+    auto gen_normals = [&](uint32_t s_lo, uint32_t s_hi) {
+#pragma unroll 4
+        for (int q = 0; q < (P + 1) / 2; ++q) {
+            double ee, eo;
+            philox_normal_pair(a.seed_lo, a.seed_hi, s_lo, s_hi, (uint32_t)i, (uint32_t)(4 * q + alpha), &ee, &eo);
+            eta_s[(2 * q) * kIntThreads] = ee;
+            if (2 * q + 1 < P) eta_s[(2 * q + 1) * kIntThreads] = eo;
+        }
+    };
+    const double kick = a.half_dt_mvv / m;
+    const double hh = a.half_dt_mvv * kMvv2e;          // dt/2
+    const double sigma = sqrt(a.PkT_mvv / m);
+    double sx = 0.0, sf = 0.0, xf = 0.0, accS = 0.0;
+#pragma unroll
+    for (int k = 0; k < P; ++k) { sx += x[k]; sf += g[k]; xf += x[k] * g[k]; }
+#pragma unroll
+    for (int k = 0; k < P; ++k) {
+        const double dr = x[k] - x[(k + 1) % P];
+        accS += dr * dr;                                 // A3 in Cartesian form: 1/2 m omega_n^2 |r_k - r_{k+1}|^2
+    }
+#pragma unroll
+    for (int k = 0; k < P; ++k) {
+        const double lap = (P == 1) ? 0.0 : 2.0 * x[k] - x[(k + P - 1) % P] - x[(k + 1) % P];
+        g[k] = kick * g[k] - hh * a.wP2 * lap;
+    }
+    const double cv_term = xf - (sx / (double)P) * sf;   // A9: sum_k (r_k - r_c).F_k
+    if (close) {
+#pragma unroll
+        for (int k = 0; k < P; ++k) v[k] += g[k];        // closing B(dt/2)
+        if (kObabo && a.thermostat) {                    // closing O(dt/2), second half-step stream
+            gen_normals(a.cstep_lo, a.cstep_hi);
+#pragma unroll
+            for (int k = 0; k < P; ++k) v[k] = mc.c1[0] * v[k] + mc.c2[0] * sigma * eta_s[k * kIntThreads];
+        }
+    }
+    double accK = 0.0;
+#pragma unroll
+    for (int k = 0; k < P; ++k) accK += v[k] * v[k];
+    if (start) {
+        const double hd = mc.sinA_w[0];                  // drift length: dt/2 (BAOAB), dt (OBABO)
+        if (thermo) gen_normals(a.step_lo, a.step_hi);
+        if (kObabo) {
+#pragma unroll
+            for (int k = 0; k < P; ++k) {
+                if (thermo) v[k] = mc.c1[0] * v[k] + mc.c2[0] * sigma * eta_s[k * kIntThreads];
+                v[k] += g[k];
+                x[k] += hd * v[k];
+            }
+        } else {
+#pragma unroll
+            for (int k = 0; k < P; ++k) {
+                v[k] += g[k];
+                x[k] += hd * v[k];
+                if (thermo) v[k] = mc.c1[0] * v[k] + mc.c2[0] * sigma * eta_s[k * kIntThreads];
+                x[k] += hd * v[k];
+            }
+        }
+    }
+    if (live && (close || start)) {
+#pragma unroll
+        for (int k = 0; k < P; ++k) a.vt_out[k * stride + ec] = v[k];
+    }
+    if (live && start) {
+#pragma unroll
+        for (int k = 0; k < P; ++k) a.x_out[k * stride + ec] = x[k];
+    }
+    if (a.flags & I_EST) {
+        double r0 = live ? 0.5 * m * accK * kMvv2e : 0.0;
+        double r1 = live ? 0.5 * m * a.wP2 * accS * kMvv2e : 0.0;
+        double r2 = live ? cv_term : 0.0;
+        __shared__ double red[3][kIntThreads / 32];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            r0 += __shfl_xor_sync(0xffffffffu, r0, o);
+            r1 += __shfl_xor_sync(0xffffffffu, r1, o);
+            r2 += __shfl_xor_sync(0xffffffffu, r2, o);
+        }
+        const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+        if (l == 0) { red[0][w] = r0; red[1][w] = r1; red[2][w] = r2; }
+        __syncthreads();
+        if (threadIdx.x < 3) {
+            double t = 0.0;
+#pragma unroll
+            for (int q = 0; q < kIntThreads / 32; ++q) t += red[threadIdx.x][q];
+            atomicAdd(a.est + threadIdx.x, t);
+        }
+        if (blockIdx.x == 0 && threadIdx.x == 3 && a.U != nullptr) {
+            double u = 0.0;
+            for (int k = 0; k < P; ++k) u += a.U[k];
+            atomicAdd(a.est + 3, u);
+        }
+    }
+}
+
+template <int P>
+static void launch_cart_t(const IntegratorArgs& a, const ModeConsts& mc, cudaStream_t s) {
+    const int blocks = (a.n_dof + kIntThreads - 1) / kIntThreads;
+    const size_t smem = (size_t)P * kIntThreads * sizeof(double);
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaFuncSetAttribute(integrator_cart_kernel<P, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaFuncSetAttribute(integrator_cart_kernel<P, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        attr_done = true;
+    }
+    if (a.flags & I_OBABO) integrator_cart_kernel<P, true><<<blocks, kIntThreads, smem, s>>>(a, mc);
+    else integrator_cart_kernel<P, false><<<blocks, kIntThreads, smem, s>>>(a, mc);
+}
+
+// v = p/m and p = m v per bead (the Cartesian method keeps v as it crosses the API)
+__global__ void cart_convert_kernel(size_t n, int n_dof, const double* __restrict__ in, const double* __restrict__ mass,
+                                    double* __restrict__ out, int forward) {
+    const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n) return;
+    const double m = mass[(t % n_dof) / 3];
+    out[t] = forward ? in[t] / m : in[t] * m;
+}
+int launch_cart_convert(int P, int N, const double* in, const double* mass, double* out, int forward, cudaStream_t s) {
+    const size_t n = (size_t)P * N * 3;
+    cart_convert_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(n, 3 * N, in, mass, out, forward);
+    return 1;
+}
+
 int launch_integrator(int P, const IntegratorArgs& a, const ModeConsts& mc, cudaStream_t s) {
+    if (a.flags & I_CART) {
+        switch (P) {
+            case 1: launch_cart_t<1>(a, mc, s); break;
+            case 2: launch_cart_t<2>(a, mc, s); break;
+            case 4: launch_cart_t<4>(a, mc, s); break;
+            case 8: launch_cart_t<8>(a, mc, s); break;
+            case 16: launch_cart_t<16>(a, mc, s); break;
+            case 32: launch_cart_t<32>(a, mc, s); break;
+            case 64: launch_cart_t<64>(a, mc, s); break;
+            default: return 0;
+        }
+        return 1;
+    }
     switch (P) {
         case 1: launch_int_t<1>(a, mc, s); break;
         case 2: launch_int_t<2>(a, mc, s); break;

@@ -495,3 +495,81 @@ def test_tensor_core_and_cuda_core_embedding_paths_agree(pk):
     assert np.abs(out[0][0] - out[1][0]).max() <= 5e-5 * frms
     assert np.abs(out[0][1] - out[1][1]).max() <= 1e-6 * 1e3
     assert np.abs(out[0][2] - out[1][2]).max() <= 5e-5 * np.abs(out[1][2]).max()
+
+
+# ---------------------------------------------------------------------------------------------
+# `method pimd`: integration in Cartesian coordinates (Eq. D3)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("integ", ["baoab", "obabo"])
+@pytest.mark.parametrize("P", [1, 2, 8, 32, 64])
+@pytest.mark.parametrize("gamma", [0.0, 5.0])
+def test_cartesian_method_parity_harmonic(pk, P, gamma, integ):
+    N = 37
+    types, masses, x, p = _random_system(N, P, seed=40 + P)
+    ks = 2.5
+    args = (types, masses, [30.0] * 3, P, 300.0, 0.1e-3, gamma)
+    sim = pk.PIMD(*args, seed=99, integrator=integ, method="pimd")
+    sim.set_state(x, p)
+    sim.set_model_harmonic(ks)
+    orc = OraclePIMD(*args, seed=99, integrator=integ, method="pimd")
+    orc.set_state(x, p)
+    orc.set_model_harmonic(ks)
+    assert _rel(sim.momenta(), orc.momenta()) < 1e-15
+    e0, o0 = sim.estimators(), orc.estimators()
+    for key in ("K_PR", "K_CV", "H", "K_ring", "S_ring", "U_sum", "T_ring"):
+        assert abs(e0[key] - o0[key]) <= 1e-11 * max(1.0, abs(o0[key])), key
+    sim.step(1)
+    orc.step(1)
+    assert _rel(sim.positions(), orc.positions()) < 1e-10
+    assert _rel(sim.momenta(), orc.momenta()) < 1e-10
+    sim.step(9)
+    orc.step(9)
+    assert _rel(sim.positions(), orc.positions()) < 1e-10
+    assert _rel(sim.momenta(), orc.momenta()) < 1e-9
+    e, o = sim.estimators(), orc.estimators()
+    assert e["step"] == 10
+    for key in ("K_PR", "K_CV", "H", "K_ring", "S_ring", "U_sum", "T_ring"):
+        assert abs(e[key] - o[key]) <= 1e-9 * max(1.0, abs(o[key])), key
+    sim.close()
+
+
+def test_cartesian_method_full_step_parity_config0(pk):
+    cfg, wb, desc, w = workloads.make_config(0)
+    args = (wb["types"], wb["masses"], wb["box"], cfg["P"], cfg["T"], 0.1e-3, cfg["gamma"])
+    sim = pk.PIMD(*args, seed=11, model_desc=desc, method="pimd")
+    sim.set_state(wb["x"], wb["p"])
+    sim.set_model(w)
+    orc = OraclePIMD(*args, seed=11, method="pimd")
+    orc.set_state(wb["x"], wb["p"])
+    orc.set_model(desc, w)
+    sim.step(1)
+    orc.step(1)
+    ex1, ep1 = _rel(sim.positions(), orc.positions()), _rel(sim.momenta(), orc.momenta())
+    assert ex1 <= 1e-10 and ep1 <= 1e-10, (ex1, ep1)
+    sim.step(9)
+    orc.step(9)
+    ex, ep = _rel(sim.positions(), orc.positions()), _rel(sim.momenta(), orc.momenta())
+    assert ex <= 1e-6 and ep <= 1e-6, (ex, ep)
+    e, o = sim.estimators(), orc.estimators()
+    assert abs(e["K_CV"] - o["K_CV"]) <= 1e-6 * abs(o["K_CV"])
+    assert abs(e["H"] - o["H"]) <= 1e-6 * sim.N * sim.P
+    sim.close()
+
+
+def test_cartesian_method_argument_rules(pk):
+    types, masses, x, p = _random_system(5, 4, seed=1)
+    sim = pk.PIMD(types, masses, [30.0] * 3, 4, 300.0, 1e-4, 1.0, seed=1)
+    sim.set_state(x, p)
+    sim.set_model_harmonic(1.0)
+    pk.pimd_set_method(sim.ctx, "pimd")
+    with pytest.raises(pk.PimdError):
+        sim.step(1)                                  # the change of representation dropped the state
+    with pytest.raises(pk.PimdError):
+        pk.pimd_set_fixcom(sim.ctx, True)
+    with pytest.raises(pk.PimdError):
+        sim.set_barostat(1.0, 0.1)
+    with pytest.raises(pk.PimdError):
+        pk.pimd_set_method(sim.ctx, 7)
+    sim.set_state(x, p)
+    sim.step(2)
+    sim.close()
