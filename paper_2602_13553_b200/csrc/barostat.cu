@@ -102,18 +102,28 @@ __global__ void baro_update_kernel(const __grid_constant__ BaroArgs a) {
 #pragma unroll
     for (int c = 0; c < 3; ++c)
 #pragma unroll
-        for (int q = 0; q < kBaroSums; ++q) {
-            double t = 0.0;
-            for (int b = threadIdx.x; b < nblk; b += 32) t += a.partial[kBaroPart * b + c * kBaroSums + q];
+        for (int q = 0; q < kBaroSums; ++q) S[c][q] = 0.0;
+    for (int b = threadIdx.x; b < nblk; b += 32) {          // a block's 21 partials are contiguous: independent loads
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
-            S[c][q] = t;
-        }
+        for (int c = 0; c < 3; ++c)
+#pragma unroll
+            for (int q = 0; q < kBaroSums; ++q) S[c][q] += a.partial[kBaroPart * b + c * kBaroSums + q];
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+#pragma unroll
+            for (int q = 0; q < kBaroSums; ++q) S[c][q] += __shfl_xor_sync(0xffffffffu, S[c][q], o);
+    double tr[3] = {0.0, 0.0, 0.0};
+    for (int k = threadIdx.x; k < a.P; k += 32) { tr[0] += a.Xi[9 * k]; tr[1] += a.Xi[9 * k + 4]; tr[2] += a.Xi[9 * k + 8]; }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) tr[c] += __shfl_xor_sync(0xffffffffu, tr[c], o);
     if (threadIdx.x != 0) return;
     double* st = a.state;
     const double L[3] = {st[BS_LX], st[BS_LY], st[BS_LZ]};
-    double tr[3] = {0.0, 0.0, 0.0};
-    for (int k = 0; k < a.P; ++k) { tr[0] += a.Xi[9 * k]; tr[1] += a.Xi[9 * k + 4]; tr[2] += a.Xi[9 * k + 8]; }
     const double V = L[0] * L[1] * L[2];
     const double h = a.h, nP = (double)a.P;
     st[BS_TRXI] = tr[0] + tr[1] + tr[2];
