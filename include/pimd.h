@@ -203,6 +203,14 @@ int pimd_set_barostat(pimd_ctx* ctx, double p_ext_bar, double tau_p);
  * stays orthorhombic.  Same rules and errors as pimd_set_barostat; the later of the two calls wins. */
 int pimd_set_barostat_aniso(pimd_ctx* ctx, double p_ext_bar, double tau_p);
 
+/* Checkpoint / resume under a barostat: restores the cell lengths, the cell velocities (three equal values in
+ * isotropic mode) and the bead virials xi[P][9] that belong to the checkpointed positions (the first E1 of the next
+ * step needs them; pimd_restore carries x, p, f, U and the step counter).  Call after pimd_set_barostat[_aniso]
+ * and around pimd_restore; restore + pimd_step(n) then continues the trajectory as the uninterrupted run would,
+ * up to the rounding noted at pimd_step (a call boundary re-reads the kicked velocities).  PIMD_EINVAL without a
+ * barostat or for a non-positive length. */
+int pimd_restore_cell(pimd_ctx* ctx, const double box[3], const double v_W[3], const double* xi);
+
 /* Barostat outputs after the last completed step (Appendix A outputs 8-15); pressures in bar,
  * energies in eV, lengths in Angstrom.  PIMD_EINVAL when no barostat is set. */
 typedef struct pimd_barostat_state {

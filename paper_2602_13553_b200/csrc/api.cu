@@ -454,6 +454,7 @@ int pimd_restore(pimd_ctx* ctx, const double* x, const double* p, const double* 
         : launch_to_nm_velocity(ctx->P, ctx->N, ctx->scratch_b, ctx->mass_atom, ctx->vt, ctx->stream);
     ctx->have_state = true;
     ctx->step = step;
+    if (ctx->baro) ctx->launches += run_barostat(ctx, false, false, ctx->step);     // P_CV of the restored state
     double* cur = ctx->est + (size_t)kEstCap * kEstWidth;
     CK(cudaMemsetAsync(cur, 0, sizeof(double) * kEstWidth, ctx->stream));
     IntegratorArgs a;
@@ -500,6 +501,24 @@ static int set_barostat(pimd_ctx* ctx, double p_ext_bar, double tau_p, bool anis
 
 int pimd_set_barostat(pimd_ctx* ctx, double p_ext_bar, double tau_p) { return set_barostat(ctx, p_ext_bar, tau_p, false); }
 int pimd_set_barostat_aniso(pimd_ctx* ctx, double p_ext_bar, double tau_p) { return set_barostat(ctx, p_ext_bar, tau_p, true); }
+
+int pimd_restore_cell(pimd_ctx* ctx, const double box[3], const double v_W[3], const double* xi) {
+    if (!ctx || !box || !v_W || !xi) return fail(ctx, PIMD_EINVAL, "null argument");
+    if (!ctx->baro) return fail(ctx, PIMD_EINVAL, "no barostat set");
+    if (!(box[0] > 0 && box[1] > 0 && box[2] > 0)) return fail(ctx, PIMD_EINVAL, "cell lengths must be positive");
+    int rc;
+    if ((rc = alloc_base(ctx))) return rc;
+    double st[6] = {v_W[0], v_W[1], v_W[2], box[0], box[1], box[2]};     // BS_VW .. BS_LZ
+    CK(cudaMemcpyAsync(ctx->baro_state + BS_VW, st, sizeof(st), cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaMemcpyAsync(ctx->Xi, xi, sizeof(double) * 9 * ctx->P, cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    for (int c = 0; c < 3; ++c) ctx->box[c] = box[c];
+    if (ctx->have_state && ctx->model_kind != 0) {
+        ctx->launches += run_barostat(ctx, false, false, ctx->step);     // P_CV of the restored state
+        CK(cudaStreamSynchronize(ctx->stream));
+    }
+    return PIMD_OK;
+}
 
 int pimd_get_barostat(pimd_ctx* ctx, pimd_barostat_state* b) {
     if (!ctx || !b) return fail(ctx, PIMD_EINVAL, "null argument");

@@ -306,6 +306,37 @@ def test_npt_config4_full_size_sampled(pk):
     sim.close()
 
 
+@pytest.mark.parametrize("aniso", [False, True])
+def test_checkpoint_resume_under_the_barostat(pk, aniso):
+    """{x, p, f, U, step} + {cell, v_W, virials} restored into a fresh context continue the NpT trajectory (to the
+    rounding of a call boundary): counter-based noise for atoms and cell alike."""
+    N, P = 50, 8
+    types, masses, x, p = _trap_system(N, P, seed=9)
+    args = (types, masses, [10.0, 10.5, 11.0], P, 300.0, 1e-3, 20.0)
+    ref = pk.PIMD(*args, seed=4)
+    ref.set_state(x, p)
+    ref.set_model_harmonic(0.5)
+    ref.set_barostat(40.0, 0.05, aniso=aniso)
+    ref.step(3)
+    ck = dict(x=ref.positions(), p=ref.momenta(), f=ref.forces(), U=ref.energies(), xi=ref.virial(),
+              b=ref.barostat_state())
+    ref.step(3)
+    sim = pk.PIMD(*args, seed=4)
+    sim.set_model_harmonic(0.5)
+    sim.set_barostat(40.0, 0.05, aniso=aniso)
+    sim.restore_cell(ck["b"]["box"], ck["b"]["v_W3"], ck["xi"])
+    pk.pimd_restore(sim.ctx, ck["x"], ck["p"], ck["f"], ck["U"], 3)
+    b0 = sim.barostat_state()
+    assert abs(b0["P_CV"] - ck["b"]["P_CV"]) <= 1e-12 * abs(ck["b"]["P_MD"])
+    assert abs(b0["enthalpy"] - ck["b"]["enthalpy"]) <= 1e-12 * abs(ck["b"]["enthalpy"])
+    sim.step(3)
+    assert _rel(sim.positions(), ref.positions()) < 1e-12 and _rel(sim.momenta(), ref.momenta()) < 1e-12
+    bs, br = sim.barostat_state(), ref.barostat_state()
+    assert _rel(bs["box"], br["box"]) < 1e-14 and np.abs(bs["v_W3"] - br["v_W3"]).max() < 1e-12 * np.abs(br["v_W3"]).max()
+    assert sim.estimators()["step"] == 6
+    ref.close(); sim.close()
+
+
 def test_barostat_argument_errors(pk):
     types, masses, x, p = _trap_system(5, 4, seed=1)
     sim = pk.PIMD(types, masses, [10.0] * 3, 4, 300.0, 1e-3, 0.0, seed=1)
