@@ -573,3 +573,48 @@ def test_cartesian_method_argument_rules(pk):
     sim.set_state(x, p)
     sim.step(2)
     sim.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# the largest configuration: outputs of sampled atoms, one by one
+# ---------------------------------------------------------------------------------------------
+def _cluster_energy_force(xb, types, box, model, i, rcut):
+    """E_i and F_i of atom i of one bead from the oracle on the cluster of all atom images within 2 r_c of it
+    (E_j of every j within r_c of i then has its complete environment, so F_i = -dU/dx_i is exact), placed in
+    the middle of a huge non-periodic cell."""
+    L = np.asarray(box, dtype=np.float64)
+    w = xb - L * np.floor(xb / L)
+    shifts = np.array([(a, b, c) for a in (-1, 0, 1) for b in (-1, 0, 1) for c in (-1, 0, 1)], dtype=np.float64) * L
+    rel = (w[:, None, :] - w[i][None, None, :]) + shifts[None, :, :]          # [N, 27, 3]
+    r2 = (rel ** 2).sum(axis=2)
+    jj, ss = np.nonzero(r2 < (2.0 * rcut) ** 2)
+    order = np.argsort(r2[jj, ss], kind="stable")                              # the centre itself (r = 0) first
+    jj, ss = jj[order], ss[order]
+    assert jj[0] == i and r2[jj[0], ss[0]] == 0.0
+    E, F, _ = se_e2_a.energy_forces(rel[jj, ss] + 500.0, np.asarray(types)[jj], [1000.0] * 3, model)
+    return E[0], F[0], len(jj)
+
+
+def test_force_parity_config3_largest_size_sampled_atoms(pk):
+    """BASELINE.json configs[3] (12288 atoms x 32 beads = 393,216 bead-atoms, the largest NVT configuration, in the
+    launch configuration bench.py --config 3 times): E_i and F_i of sampled atoms of two beads against the oracle."""
+    cfg, wb, desc, w = workloads.make_config(3)
+    sim = pk.PIMD(wb["types"], wb["masses"], wb["box"], cfg["P"], cfg["T"], cfg["dt"], cfg["gamma"], seed=0,
+                  model_desc=desc)
+    sim.set_state(wb["x"], wb["p"])
+    sim.set_model(w)
+    model = se_e2_a.Model(desc, w)
+    f, E = sim.forces(), sim.atom_energies()
+    rng = np.random.default_rng(3)
+    for k in (0, 31):
+        frms = np.sqrt((f[k] ** 2).mean())
+        for i in rng.choice(sim.N, size=4, replace=False):
+            Eo, Fo, n_cluster = _cluster_energy_force(wb["x"][k], wb["types"], wb["box"], model, int(i), desc["rcut"])
+            assert n_cluster > 500
+            assert abs(E[k, i] - Eo) <= 1e-6
+            err = np.abs(f[k, i] - Fo) / np.maximum(np.abs(Fo), frms)
+            assert err.max() <= 1e-4, "force error %.3e" % err.max()
+    assert np.abs(f.sum(axis=1)).max() <= 1e-6 * np.abs(f).max() * sim.N ** 0.5     # Newton's third law, every bead
+    X3 = sim.virial().reshape(-1, 3, 3)
+    assert np.abs(X3 - np.swapaxes(X3, 1, 2)).max() <= 1e-5 * np.abs(X3).max()
+    sim.close()
