@@ -262,7 +262,7 @@ def run_ours(args):
     achieved = flops[dom] / (phases[dom] * 1e-3) / 1e12
     dom_issued = sum(f for f, _ in issued[dom]) / (phases[dom] * 1e-3) / 1e12
     roofline = {"kernel": dom, "bound": "tensor", "achieved": achieved, "peak": dom_peak, "unit": "TFLOP/s",
-                "frac": achieved / dom_peak, "traffic": NCU_DRAM_BYTES.get(dom),
+                "frac": achieved / dom_peak, "traffic": NCU_DRAM_BYTES.get(dom) if args.config == 2 else None,
                 "issued_tflops": dom_issued,
                 "note": "achieved = USEFUL flops (SURVEY 8(d): no recompute, no extra hi/lo passes, no padding) / live "
                         "CUDA-event time of the phase; peak = FP16 dense = %s BF16 %.0f TFLOP/s (kind::f16 runs at the "
@@ -328,7 +328,9 @@ def run_ours(args):
             "config": {"workload": cfg["name"], "atoms": N, "beads": P, "bead_atoms": P * N, "neighbour_rows": rows,
                        "parallelism": "replicas only" if world > 1 else "1 GPU",
                        "ensemble": ("NpT %g bar, BZP barostat tau_p %g ps" % (cfg["p_ext_bar"], cfg["tau_p"])) if "p_ext_bar" in cfg else "NVT",
-                       "l2": "no flush: per-step working set (neighbour rows 135 MB, T and dT 157 MB, fitting activations ~380 MB) exceeds the 126 MB L2"},
+                       "l2": "no flush: per-step working set (neighbour rows %.0f MB, T and dT %.0f MB, fitting activations ~%.0f MB)%s" % (
+                           rows * 32 / 1e6, 2 * P * N * 1600 / 1e6, P * N * 7740 / 1e6,
+                           " exceeds the 126 MB L2" if rows * 32 + P * N * 3200 > 126e6 else " -- fits the 126 MB L2: small-case config, not a bench line")},
             "roofline": roofline, "kernels": kernels, "integrator_hbm": integ, "cpu_baseline": cpu,
             "e2e": {"value": world * P * N / e2e_s, "unit": METRIC, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": e2e_s * 1e3, "call": "pimd_restore(host x,p,f,U) + pimd_step(1) + pimd_get_{positions,momenta,forces,energies,estimators}"},
