@@ -14,6 +14,8 @@ Pin status (see tests/test_oracle_*.py):
                           harmonic-oscillator <K>,<V>, NVE energy conservation, P=1 limit
   barostat.py    pinned   E1 = quadrature of the cell force over the kick, E4/E5 = numerical ODE, NpH enthalpy
                           (A17) conserved to second order, A12 = A11 at n = 1, closed forms, E7 variance
+  compress.py    pinned   node conditions of the quintic Hermite table, 6th-order convergence, forces = -grad of
+                          the compressed energy, distance to the MLP (no CUDA counterpart yet: NEXT-3)
   se_e2_a.py     backward pinned (finite differences, torch autograd, invariances, virial =
                  -dU/d(strain), continuity at r_c);  forward architecture: PARITY UNPINNED
                  against physics -- the paper prints no equation for the Deep-Potential

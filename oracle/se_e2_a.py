@@ -55,6 +55,7 @@ class Model:
             self.fitnet.append(layers)
         if pos != w.size:
             raise ValueError("weight vector has %d entries, the architecture needs %d" % (w.size, pos))
+        self.tables = None       # set by oracle.compress.compress(): tabulated embedding
 
     @staticmethod
     def n_weights(desc):
@@ -230,8 +231,12 @@ def energy_forces(x, types, box, model, return_parts=False, row_block=32768):
         for p in range(model.ntypes ** 2):
             sel_rows = np.flatnonzero(pair_id[b0:b1] == p)
             if sel_rows.size:
-                G[sel_rows], _ = _mlp_forward(model.emb[(p // model.ntypes, p % model.ntypes)],
-                                              s[b0:b1][sel_rows, None], _embed_rule)
+                pair = (p // model.ntypes, p % model.ntypes)
+                if model.tables is not None:
+                    from . import compress
+                    G[sel_rows], _ = compress.table_eval(model.tables[pair], s[b0:b1][sel_rows])
+                else:
+                    G[sel_rows], _ = _mlp_forward(model.emb[pair], s[b0:b1][sel_rows, None], _embed_rule)
         T += _segment_sum(G[:, :, None] * R[b0:b1, None, :], ri[b0:b1], N)
     T *= inv_nsel
 
@@ -267,7 +272,13 @@ def energy_forces(x, types, box, model, return_parts=False, row_block=32768):
         for p in range(model.ntypes ** 2):
             sel_rows = np.flatnonzero(pair_id[b0:b1] == p)
             if sel_rows.size:
-                layers = model.emb[(p // model.ntypes, p % model.ntypes)]
+                pair = (p // model.ntypes, p % model.ntypes)
+                if model.tables is not None:
+                    from . import compress
+                    G[sel_rows], Gp = compress.table_eval(model.tables[pair], sb[sel_rows])
+                    dsG[sel_rows] = np.einsum("rm,rm->r", dG[sel_rows], Gp)
+                    continue
+                layers = model.emb[pair]
                 G[sel_rows], tanhs = _mlp_forward(layers, sb[sel_rows, None], _embed_rule)
                 dsG[sel_rows] = _mlp_backward(layers, tanhs, dG[sel_rows], _embed_rule)[:, 0]
         dR = np.einsum("rmc,rm->rc", dTi, G) * inv_nsel          # [rows, 4]
