@@ -227,13 +227,28 @@ neighbor_env_kernel(int P, int N, GridGeom g, EnvConsts ec, const double* __rest
             // slot inside the type partition; fully unrolled over the (at most PIMD_MAX_TYPES) types so that the
             // counters stay in registers and sel / seloff are constant-bank operands
             int slot = -1, sel_t = 0, seloff_t = 0;
+            if (ec.ntypes == 2) {
+                // the water case: two ballots instead of one per possible type
+                const unsigned mk_all = __ballot_sync(0xffffffffu, keep);
+                const unsigned mk0 = __ballot_sync(0xffffffffu, keep && tj == 0);
+                const unsigned mk1 = mk_all & ~mk0;
+                if (keep) {
+                    const bool t0 = tj == 0;
+                    slot = t0 ? cnt[0] + __popc(mk0 & lt_mask) : cnt[1] + __popc(mk1 & lt_mask);
+                    sel_t = t0 ? ec.sel[0] : ec.sel[1];
+                    seloff_t = t0 ? ec.seloff[0] : ec.seloff[1];
+                }
+                cnt[0] += __popc(mk0);
+                cnt[1] += __popc(mk1);
+            } else {
 #pragma unroll
-            for (int t = 0; t < PIMD_MAX_TYPES; ++t) {
-                if (t < ec.ntypes) {
-                    const bool mine = keep && tj == t;
-                    const unsigned mk = __ballot_sync(0xffffffffu, mine);
-                    if (mine) { slot = cnt[t] + __popc(mk & lt_mask); sel_t = ec.sel[t]; seloff_t = ec.seloff[t]; }
-                    cnt[t] += __popc(mk);
+                for (int t = 0; t < PIMD_MAX_TYPES; ++t) {
+                    if (t < ec.ntypes) {
+                        const bool mine = keep && tj == t;
+                        const unsigned mk = __ballot_sync(0xffffffffu, mine);
+                        if (mine) { slot = cnt[t] + __popc(mk & lt_mask); sel_t = ec.sel[t]; seloff_t = ec.seloff[t]; }
+                        cnt[t] += __popc(mk);
+                    }
                 }
             }
             if (keep) {
