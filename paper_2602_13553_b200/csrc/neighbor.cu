@@ -151,9 +151,9 @@ neighbor_env_kernel(int P, int N, GridGeom g, EnvConsts ec, const double* __rest
     const unsigned lt_mask = (1u << lane) - 1u;
     const size_t slot0 = (size_t)ba * ec.nsel;
 
-    // The (2R+1)^3 neighbour cells are walked in the order (oz, oy, ox), ox fastest.  Lane l of a batch looks up
-    // cell l's range and periodic image first (27 independent loads instead of 27 dependent ones); the cells are
-    // then processed one by one with the first 32 candidates of the NEXT cell already in flight.
+    // The (2R+1)^3 neighbour cells are taken in the order (oz, oy, ox), ox fastest.  Lane l of a batch looks up
+    // cell l's range and periodic image first (27 independent loads instead of 27 dependent ones); the candidates
+    // of all cells of the batch are then walked as one flat list, 32 at a time.
     const int nx_c = 2 * g.R[0] + 1, ny_c = 2 * g.R[1] + 1, nz_c = 2 * g.R[2] + 1;
     const int ncl = nx_c * ny_c * nz_c;
     for (int base = 0; base < ncl; base += 32) {
@@ -184,48 +184,61 @@ neighbor_env_kernel(int P, int N, GridGeom g, EnvConsts ec, const double* __rest
                 my_code = (nx + 3) | ((ny + 3) << 3) | ((nz + 3) << 6);
             }
         }
-        // walk only the cells that still have candidates, in the same (oz, oy, ox) order
-        unsigned todo = __ballot_sync(0xffffffffu, my_s1 > my_s0);
-        double4 wnext = make_double4(0, 0, 0, 0);
-        if (todo) {
-            const int c = __ffs(todo) - 1;
-            const int f0 = __shfl_sync(0xffffffffu, my_s0, c), f1 = __shfl_sync(0xffffffffu, my_s1, c);
-            if (f0 + lane < f1) wnext = ws[f0 + lane];
+        // The candidates of the non-pruned cells form one flat list in the same (oz, oy, ox) / in-cell order; it is
+        // walked 32 at a time with every lane busy (cells hold ~24 atoms, so a batch per cell left a quarter of the
+        // lanes idle and paid a per-cell header).  Lane l finds the cell of candidate g by a binary search over the
+        // inclusive prefix sums of the cell lengths, which live one per lane.
+        const int my_len = max(my_s1 - my_s0, 0);
+        int pre = my_len;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, pre, o);
+            if (lane >= o) pre += t;
         }
-        while (todo) {
-            const int c = __ffs(todo) - 1;
-            todo &= todo - 1;
-            const int s0 = __shfl_sync(0xffffffffu, my_s0, c), s1 = __shfl_sync(0xffffffffu, my_s1, c);
-            const int code = __shfl_sync(0xffffffffu, my_code, c);
-            const int nx = (code & 7) - 3, ny = ((code >> 3) & 7) - 3, nz = ((code >> 6) & 7) - 3;
-            const double4 wfirst = wnext;
-            if (todo) {
-                const int cn = __ffs(todo) - 1;
-                const int f0 = __shfl_sync(0xffffffffu, my_s0, cn), f1 = __shfl_sync(0xffffffffu, my_s1, cn);
-                if (f0 + lane < f1) wnext = ws[f0 + lane];
+        const int total = __shfl_sync(0xffffffffu, pre, 31);
+        const int my_beg = pre - my_len;
+        auto locate = [&](int gi, int& q, int& code) {
+            int c = 0;
+#pragma unroll
+            for (int step = 16; step > 0; step >>= 1) {
+                const int probe = __shfl_sync(0xffffffffu, pre, c + step - 1);
+                if (probe <= gi) c += step;
             }
-            const double sh[3] = {__dmul_rn((double)nx, gL[0]), __dmul_rn((double)ny, gL[1]),
-                                  __dmul_rn((double)nz, gL[2])};
-            const bool zero_shift = (nx == 0) && (ny == 0) && (nz == 0);
-            for (int q0 = s0; q0 < s1; q0 += 32) {
-                const int q = q0 + lane;
-                double4 wj = wfirst;
-                if (q0 != s0 && q < s1) wj = ws[q];
+            c = min(c, 31);
+            const int cbeg = __shfl_sync(0xffffffffu, my_beg, c), cs0 = __shfl_sync(0xffffffffu, my_s0, c);
+            code = __shfl_sync(0xffffffffu, my_code, c);
+            q = cs0 + (gi - cbeg);
+        };
+        int qn = 0, coden = 0;
+        double4 wn = make_double4(0, 0, 0, 0);
+        if (total > 0) {
+            locate(lane, qn, coden);
+            if (lane < total) wn = ws[qn];
+        }
+        for (int g0 = 0; g0 < total; g0 += 32) {
+            const int q = qn, code = coden;
+            const double4 wj = wn;
+            const bool act = g0 + lane < total;
+            if (g0 + 32 < total) {                              // next batch in flight while this one is tested
+                locate(g0 + 32 + lane, qn, coden);
+                if (g0 + 32 + lane < total) wn = ws[qn];
+            }
+            const int nx = (code & 7) - 3, ny = ((code >> 3) & 7) - 3, nz = ((code >> 6) & 7) - 3;
             bool keep = false;
             int tj = 0, j = 0;
-            double d[3] = {0, 0, 0}, r2 = 1.0;
-            if (q < s1) {
+            if (act) {
+                const double sh[3] = {__dmul_rn((double)nx, gL[0]), __dmul_rn((double)ny, gL[1]),
+                                      __dmul_rn((double)nz, gL[2])};
                 const long long pk = __double_as_longlong(wj.w);
                 j = (int)(pk & 0xffffffffll);
                 tj = (int)(pk >> 32);
-                d[0] = __dadd_rn(__dsub_rn(wj.x, wi[0]), sh[0]);
-                d[1] = __dadd_rn(__dsub_rn(wj.y, wi[1]), sh[1]);
-                d[2] = __dadd_rn(__dsub_rn(wj.z, wi[2]), sh[2]);
-                r2 = __dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2]));
-                keep = (r2 < ec.rc2) && !(zero_shift && j == i);
+                const double d0 = __dadd_rn(__dsub_rn(wj.x, wi[0]), sh[0]);
+                const double d1 = __dadd_rn(__dsub_rn(wj.y, wi[1]), sh[1]);
+                const double d2 = __dadd_rn(__dsub_rn(wj.z, wi[2]), sh[2]);
+                const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(d0, d0), __dmul_rn(d1, d1)), __dmul_rn(d2, d2));
+                keep = (r2 < ec.rc2) && !(code == (3 | (3 << 3) | (3 << 6)) && j == i);
             }
-            // slot inside the type partition; fully unrolled over the (at most PIMD_MAX_TYPES) types so that the
-            // counters stay in registers and sel / seloff are constant-bank operands
+            // slot inside the type partition
             int slot = -1, sel_t = 0, seloff_t = 0;
             if (ec.ntypes == 2) {
                 // the water case: two ballots instead of one per possible type
@@ -257,16 +270,13 @@ neighbor_env_kernel(int P, int N, GridGeom g, EnvConsts ec, const double* __rest
                 } else {
                     // queue the accepted candidate in its final slot: {j | image code, index into the cell-sorted
                     // positions}.  The FP64 environment arithmetic runs afterwards over the compact slots with all
-                    // lanes busy (inside this loop only ~13 % of the lanes would be active).
-                    const uint32_t code = (uint32_t)(nx + 3) | ((uint32_t)(ny + 3) << 3) | ((uint32_t)(nz + 3) << 6);
+                    // lanes busy (inside this loop only ~20 % of the lanes would be active).
                     NeighSlotB B;
                     B.ds = 0.f; B.rinv = 0.f;
-                    B.jcode = (uint32_t)j | (code << 23);
+                    B.jcode = (uint32_t)j | ((uint32_t)code << 23);
                     B.pad = __int_as_float(q);
                     slotB[slot0 + seloff_t + slot] = B;
                 }
-            }
-
             }
         }
     }
