@@ -13,6 +13,8 @@ namespace pimd {
 struct GridGeom {
     double L[3];
     double inv_w[3];     // ncell / L
+    double cw[3];        // cell width L / ncell
+    double inv_nc[3];    // 1 / ncell
     int nc[3];
     int R[3];
     int ncells;
@@ -28,6 +30,11 @@ __device__ __forceinline__ void load_geom(const GridGeom& g, double L[3], double
         L[a] = g.boxp ? g.boxp[a] : g.L[a];
         inv_w[a] = g.boxp ? (double)g.nc[a] / L[a] : g.inv_w[a];
     }
+}
+// cell widths (only the pruning test uses them: its 1e-6 margin dwarfs the rounding of L * (1/nc))
+__device__ __forceinline__ void load_widths(const GridGeom& g, const double L[3], double cw[3]) {
+#pragma unroll
+    for (int a = 0; a < 3; ++a) cw[a] = g.boxp ? L[a] * g.inv_nc[a] : g.cw[a];
 }
 
 __global__ void wrap_bin_kernel(int P, int N, GridGeom g, const double* __restrict__ x, double* __restrict__ wtmp,
@@ -138,8 +145,9 @@ neighbor_env_kernel(int P, int N, GridGeom g, EnvConsts ec, const double* __rest
     const int lane = threadIdx.x & 31;
     if (ba >= P * N) return;
     const int k = ba / N, i = ba - k * N;
-    double gL[3], ginv_w[3];
+    double gL[3], ginv_w[3], gcw[3];
     load_geom(g, gL, ginv_w);
+    load_widths(g, gL, gcw);
     const double wi[3] = {wtmp[(size_t)ba * 3], wtmp[(size_t)ba * 3 + 1], wtmp[(size_t)ba * 3 + 2]};
     const int cid = cell_id[ba];
     const int c0 = cid % g.nc[0], c1 = (cid / g.nc[0]) % g.nc[1], c2 = cid / (g.nc[0] * g.nc[1]);
@@ -156,17 +164,27 @@ neighbor_env_kernel(int P, int N, GridGeom g, EnvConsts ec, const double* __rest
     // of all cells of the batch are then walked as one flat list, 32 at a time.
     const int nx_c = 2 * g.R[0] + 1, ny_c = 2 * g.R[1] + 1, nz_c = 2 * g.R[2] + 1;
     const int ncl = nx_c * ny_c * nz_c;
+    const int mag_x = 65536 / nx_c + 1, mag_y = 65536 / ny_c + 1;     // exact for numerators < 343 and divisors <= 7
     for (int base = 0; base < ncl; base += 32) {
         int my_s0 = 0, my_s1 = 0, my_code = 0;
         {
             const int idx = base + lane;
             if (idx < ncl) {
-                const int ox = idx % nx_c - g.R[0], oy = (idx / nx_c) % ny_c - g.R[1], oz = idx / (nx_c * ny_c) - g.R[2];
+                // idx -> (ox, oy, oz) and the periodic image of each coordinate without integer divisions: idx < 343
+                // (R <= 3), so a 16-bit reciprocal is exact; |offset| <= R <= 3 cells, so the image is found by at
+                // most three conditional steps per side (nc may be 1: configs[0])
+                const int t1 = (idx * mag_x) >> 16;                 // idx / nx_c
+                const int t2 = (t1 * mag_y) >> 16;                  // idx / (nx_c ny_c)
+                const int ox = idx - t1 * nx_c - g.R[0], oy = t1 - t2 * ny_c - g.R[1], oz = t2 - g.R[2];
                 const int xx = c0 + ox, yy = c1 + oy, zz = c2 + oz;
-                const int nx = (xx >= 0) ? xx / g.nc[0] : -((-xx + g.nc[0] - 1) / g.nc[0]);
-                const int ny = (yy >= 0) ? yy / g.nc[1] : -((-yy + g.nc[1] - 1) / g.nc[1]);
-                const int nz = (zz >= 0) ? zz / g.nc[2] : -((-zz + g.nc[2] - 1) / g.nc[2]);
-                const int cc = ((zz - nz * g.nc[2]) * g.nc[1] + (yy - ny * g.nc[1])) * g.nc[0] + (xx - nx * g.nc[0]);
+                int wx = xx, wy = yy, wz = zz, nx = 0, ny = 0, nz = 0;
+#pragma unroll
+                for (int it = 0; it < 3; ++it) {
+                    if (wx < 0) { wx += g.nc[0]; --nx; } else if (wx >= g.nc[0]) { wx -= g.nc[0]; ++nx; }
+                    if (wy < 0) { wy += g.nc[1]; --ny; } else if (wy >= g.nc[1]) { wy -= g.nc[1]; ++ny; }
+                    if (wz < 0) { wz += g.nc[2]; --nz; } else if (wz >= g.nc[2]) { wz -= g.nc[2]; ++nz; }
+                }
+                const int cc = (wz * g.nc[1] + wy) * g.nc[0] + wx;
                 my_s0 = cs[cc]; my_s1 = cs[cc + 1];
                 // prune cells that lie entirely outside the cutoff sphere (about a third of the 27): distance from
                 // the centre to the cell's box in the unwrapped cell frame, with a 1e-6 relative margin on r^2 that
@@ -175,7 +193,7 @@ neighbor_env_kernel(int P, int N, GridGeom g, EnvConsts ec, const double* __rest
                 double dm2 = 0.0;
 #pragma unroll
                 for (int ax = 0; ax < 3; ++ax) {
-                    const double wc = 1.0 / ginv_w[ax];
+                    const double wc = gcw[ax];
                     const double lo = un[ax] * wc - wi[ax], hi = wi[ax] - (un[ax] + 1) * wc;
                     const double dd = fmax(fmax(lo, hi), 0.0);
                     dm2 += dd * dd;
@@ -330,6 +348,8 @@ int neighbor_build(Model& m, const ForceArgs& a, cudaStream_t s) {
         g.nc[c] = m.ncell[c];
         g.R[c] = m.R[c];
         g.inv_w[c] = (double)m.ncell[c] / a.box[c];
+        g.cw[c] = a.box[c] / (double)m.ncell[c];
+        g.inv_nc[c] = 1.0 / (double)m.ncell[c];
     }
     g.ncells = m.ncells;
     g.boxp = a.box_dev; g.rc = m.d.rcut; g.overflow = m.overflow;
