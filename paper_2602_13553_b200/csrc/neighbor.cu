@@ -204,33 +204,41 @@ neighbor_env_kernel(int P, int N, GridGeom g, EnvConsts ec, const double* __rest
         }
         // The candidates of the non-pruned cells form one flat list in the same (oz, oy, ox) / in-cell order; it is
         // walked 32 at a time with every lane busy (cells hold ~24 atoms, so a batch per cell left a quarter of the
-        // lanes idle and paid a per-cell header).  Lane l finds the cell of candidate g by a binary search over the
-        // inclusive prefix sums of the cell lengths, which live one per lane.
-        const int my_len = max(my_s1 - my_s0, 0);
-        int pre = my_len;
+        // lanes idle and paid a per-cell header).
+        // non-empty cells compacted to the low lanes (their order kept), prefix sums of their lengths
+        const unsigned ne = __ballot_sync(0xffffffffu, my_s1 > my_s0);
+        const int nne = __popc(ne);
+        const int srcl = (int)(__fns(ne, 0, lane + 1) & 31u);          // lane of the (lane+1)-th non-empty cell
+        const int c_s0 = __shfl_sync(0xffffffffu, my_s0, srcl);
+        const int c_code = __shfl_sync(0xffffffffu, my_code, srcl);
+        int c_len = __shfl_sync(0xffffffffu, my_s1, srcl) - c_s0;
+        if (lane >= nne) c_len = 0;
+        int pre = c_len;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
             const int t = __shfl_up_sync(0xffffffffu, pre, o);
             if (lane >= o) pre += t;
         }
         const int total = __shfl_sync(0xffffffffu, pre, 31);
-        const int my_beg = pre - my_len;
-        auto locate = [&](int gi, int& q, int& code) {
-            int c = 0;
-#pragma unroll
-            for (int step = 16; step > 0; step >>= 1) {
-                const int probe = __shfl_sync(0xffffffffu, pre, c + step - 1);
-                if (probe <= gi) c += step;
-            }
-            c = min(c, 31);
-            const int cbeg = __shfl_sync(0xffffffffu, my_beg, c), cs0 = __shfl_sync(0xffffffffu, my_s0, c);
-            code = __shfl_sync(0xffffffffu, my_code, c);
-            q = cs0 + (gi - cbeg);
+        const int c_beg = pre - c_len;
+        // Batches are located in order.  The cells that START inside the batch [g0, g0 + 32) are marked in a 32-bit
+        // mask (one warp OR-reduction); candidate g0 + l then belongs to cell cprev + popc(mask bits 0..l), cprev
+        // being the last cell started before the batch.
+        int cprev = -1;
+        auto locate = [&](int g0, int& q, int& code) {
+            const int rel = c_beg - g0;
+            const unsigned bit = (lane < nne && rel >= 0 && rel < 32) ? (1u << rel) : 0u;
+            const unsigned heads = __reduce_or_sync(0xffffffffu, bit);
+            const int c = min(cprev + __popc(heads & (0xffffffffu >> (31 - lane))), 31);
+            cprev += __popc(heads);
+            const int cbeg = __shfl_sync(0xffffffffu, c_beg, c), cs0 = __shfl_sync(0xffffffffu, c_s0, c);
+            code = __shfl_sync(0xffffffffu, c_code, c);
+            q = cs0 + (g0 + lane - cbeg);
         };
         int qn = 0, coden = 0;
         double4 wn = make_double4(0, 0, 0, 0);
         if (total > 0) {
-            locate(lane, qn, coden);
+            locate(0, qn, coden);
             if (lane < total) wn = ws[qn];
         }
         for (int g0 = 0; g0 < total; g0 += 32) {
@@ -238,7 +246,7 @@ neighbor_env_kernel(int P, int N, GridGeom g, EnvConsts ec, const double* __rest
             const double4 wj = wn;
             const bool act = g0 + lane < total;
             if (g0 + 32 < total) {                              // next batch in flight while this one is tested
-                locate(g0 + 32 + lane, qn, coden);
+                locate(g0 + 32, qn, coden);
                 if (g0 + 32 + lane < total) wn = ws[qn];
             }
             const int nx = (code & 7) - 3, ny = ((code >> 3) & 7) - 3, nz = ((code >> 6) & 7) - 3;
