@@ -297,11 +297,8 @@ neighbor_env_kernel(int P, int N, GridGeom g, EnvConsts ec, const double* __rest
                     // queue the accepted candidate in its final slot: {j | image code, index into the cell-sorted
                     // positions}.  The FP64 environment arithmetic runs afterwards over the compact slots with all
                     // lanes busy (inside this loop only ~20 % of the lanes would be active).
-                    NeighSlotB B;
-                    B.ds = 0.f; B.rinv = 0.f;
-                    B.jcode = (uint32_t)j | ((uint32_t)code << 23);
-                    B.pad = __int_as_float(q);
-                    slotB[slot0 + seloff_t + slot] = B;
+                    *reinterpret_cast<uint4*>(slotB + slot0 + seloff_t + slot) =
+                        make_uint4(0u, 0u, (uint32_t)j | ((uint32_t)code << 23), (uint32_t)q);     // {ds, rinv, jcode, pad}
                 }
             }
         }
