@@ -228,6 +228,10 @@ typedef struct pimd_barostat_state {
     double P_CV3[3];  /* diagonal of the centroid-virial stress tensor, Eq. E3 (P_CV is its mean) */
 } pimd_barostat_state;
 int pimd_get_barostat(pimd_ctx* ctx, pimd_barostat_state* b);
+/* The same outputs for each of the last `n` completed steps of the most recent pimd_step call, oldest first (the
+ * barostat companion of pimd_get_estimator_history; at most 4096 steps per call are recorded).  Returns the number
+ * written (<= cap) or < 0. */
+int pimd_get_barostat_history(pimd_ctx* ctx, pimd_barostat_state* b, int cap);
 
 /* Fitting-net GEMM path: 1 (default) = tcgen05 tensor cores, 3xTF32 split (fitting_tc.cu); 0 = the FP32
  * CUDA-core GEMMs kept as the in-tree reference for bisecting.  Both meet the parity tolerances. */

@@ -86,6 +86,7 @@ _SIGNATURES = {
     "pimd_set_barostat": (C.c_int, [C.c_void_p, C.c_double, C.c_double]),
     "pimd_set_barostat_aniso": (C.c_int, [C.c_void_p, C.c_double, C.c_double]),
     "pimd_get_barostat": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "pimd_get_barostat_history": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int]),
     "pimd_restore_cell": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "pimd_set_embedding_path": (C.c_int, [C.c_void_p, C.c_int]),
     "pimd_debug_gemm": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]),
@@ -307,6 +308,12 @@ def pimd_set_barostat_aniso(ctx, p_ext_bar, tau_p):
     return _check(ctx, lib().pimd_set_barostat_aniso(ctx, float(p_ext_bar), float(tau_p)))
 
 
+def pimd_get_barostat_history(ctx, cap):
+    arr = (BarostatState * cap)()
+    n = _check(ctx, lib().pimd_get_barostat_history(ctx, arr, cap))
+    return [arr[q].as_dict() for q in range(n)]
+
+
 def pimd_restore_cell(ctx, box, v_W, xi):
     box = np.ascontiguousarray(box, dtype=np.float64)
     v_W = np.ascontiguousarray(np.broadcast_to(np.asarray(v_W, dtype=np.float64), (3,)))
@@ -429,6 +436,7 @@ class PIMD:
         return (pimd_set_barostat_aniso if aniso else pimd_set_barostat)(self.ctx, p_ext_bar, tau_p)
 
     def barostat_state(self): return pimd_get_barostat(self.ctx)
+    def barostat_history(self, cap=4096): return pimd_get_barostat_history(self.ctx, cap)
     def restore_cell(self, box, v_W, xi): return pimd_restore_cell(self.ctx, box, v_W, xi)
     def estimator_history(self, cap=4096): return pimd_get_estimator_history(self.ctx, cap)
 

@@ -253,7 +253,7 @@ void fill_integrator_args(pimd_ctx* ctx, IntegratorArgs& a, int flags, int64_t s
 constexpr double kBarPerEvA3 = 1.602176634e6;    // DESIGN R-25
 
 // the barostat's share of launch s (barostat.cu): closing E1 of the step that ends, opening E1 / E4-E7 of the next
-int run_barostat(pimd_ctx* ctx, bool close, bool start, int64_t step) {
+int run_barostat(pimd_ctx* ctx, bool close, bool start, int64_t step, double* est_slot = nullptr) {
     BaroArgs b;
     b.P = ctx->P; b.N = ctx->N; b.n_dof = 3 * ctx->N;
     b.close = close; b.start = start; b.thermostat = (ctx->gamma0 != 0.0) ? 1 : 0;
@@ -269,7 +269,7 @@ int run_barostat(pimd_ctx* ctx, bool close, bool start, int64_t step) {
     b.step_lo = (uint32_t)(uint64_t)step; b.step_hi = (uint32_t)((uint64_t)step >> 32);
     { const uint64_t cs = (uint64_t)(step - 1); b.cstep_lo = (uint32_t)cs; b.cstep_hi = (uint32_t)(cs >> 32) | 0x80000000u; }
     b.x = ctx->x; b.vt = ctx->vt; b.f = ctx->f; b.mass = ctx->mass_atom; b.Xi = ctx->Xi;
-    b.state = ctx->baro_state; b.partial = ctx->baro_state + BS_WIDTH;
+    b.state = ctx->baro_state; b.partial = ctx->baro_state + BS_WIDTH; b.est_slot = est_slot;
     return launch_barostat(b, ctx->stream);
 }
 
@@ -520,6 +520,27 @@ int pimd_restore_cell(pimd_ctx* ctx, const double box[3], const double v_W[3], c
     return PIMD_OK;
 }
 
+// Appendix A outputs 8-15 from the raw device record {v_W[3], L[3], diag P_CV[3], sum Tr Xi} and the estimator sums
+static void finalize_baro(const pimd_ctx* ctx, const double* rec, const double* raw, pimd_barostat_state* b) {
+    const double n = ctx->P, N = ctx->N;
+    b->K_W = 0.0;
+    for (int c = 0; c < 3; ++c) {
+        b->v_W3[c] = rec[c];
+        b->box[c] = rec[3 + c];
+        b->P_CV3[c] = rec[6 + c] * kBarPerEvA3;                                            // E3 diagonal
+        if (ctx->baro_aniso) b->K_W += 0.5 * ctx->baro_W * rec[c] * rec[c];                // A14
+    }
+    b->v_W = (rec[0] + rec[1] + rec[2]) / 3.0;
+    if (!ctx->baro_aniso) b->K_W = 0.5 * ctx->baro_W * rec[0] * rec[0];                    // A13
+    b->V = rec[3] * rec[4] * rec[5];
+    b->P_CV = (rec[6] + rec[7] + rec[8]) / 3.0 * kBarPerEvA3;                              // A12 = the mean of E3's diagonal
+    b->P_PR = (3.0 * n * N * kKB * ctx->T - 2.0 * raw[1]) / (3.0 * b->V) * kBarPerEvA3;    // A10
+    b->P_MD = (2.0 * raw[0] + rec[9]) / (3.0 * b->V) * kBarPerEvA3;                        // A11
+    b->U_W = n * ctx->p_ext * b->V;                                                        // A15
+    b->J_W = -n * kKB * ctx->T * std::log(b->V);                                           // A16
+    b->enthalpy = raw[0] + raw[1] + raw[3] + b->K_W + b->U_W + b->J_W;                     // A17
+}
+
 int pimd_get_barostat(pimd_ctx* ctx, pimd_barostat_state* b) {
     if (!ctx || !b) return fail(ctx, PIMD_EINVAL, "null argument");
     if (!ctx->baro) return fail(ctx, PIMD_EINVAL, "no barostat set");
@@ -527,24 +548,26 @@ int pimd_get_barostat(pimd_ctx* ctx, pimd_barostat_state* b) {
     CK(cudaMemcpyAsync(st, ctx->baro_state, sizeof(st), cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaMemcpyAsync(raw, ctx->est + (size_t)kEstCap * kEstWidth, sizeof(raw), cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
-    const double n = ctx->P, N = ctx->N;
-    b->K_W = 0.0;
-    for (int c = 0; c < 3; ++c) {
-        b->box[c] = st[BS_LX + c];
-        b->v_W3[c] = st[BS_VW + c];
-        b->P_CV3[c] = st[BS_PCV + c] * kBarPerEvA3;                                        // E3 diagonal
-        if (ctx->baro_aniso) b->K_W += 0.5 * ctx->baro_W * st[BS_VW + c] * st[BS_VW + c];  // A14
-    }
-    b->v_W = (st[BS_VW] + st[BS_VW + 1] + st[BS_VW + 2]) / 3.0;
-    if (!ctx->baro_aniso) b->K_W = 0.5 * ctx->baro_W * st[BS_VW] * st[BS_VW];              // A13
-    b->V = st[BS_LX] * st[BS_LY] * st[BS_LZ];
-    b->P_CV = (st[BS_PCV] + st[BS_PCV + 1] + st[BS_PCV + 2]) / 3.0 * kBarPerEvA3;          // A12 = the mean of E3's diagonal
-    b->P_PR = (3.0 * n * N * kKB * ctx->T - 2.0 * raw[1]) / (3.0 * b->V) * kBarPerEvA3;    // A10
-    b->P_MD = (2.0 * raw[0] + st[BS_TRXI]) / (3.0 * b->V) * kBarPerEvA3;                   // A11
-    b->U_W = n * ctx->p_ext * b->V;                                                        // A15
-    b->J_W = -n * kKB * ctx->T * std::log(b->V);                                           // A16
-    b->enthalpy = raw[0] + raw[1] + raw[3] + b->K_W + b->U_W + b->J_W;                     // A17
+    const double rec[10] = {st[BS_VW], st[BS_VW + 1], st[BS_VW + 2], st[BS_LX], st[BS_LY], st[BS_LZ],
+                            st[BS_PCV], st[BS_PCV + 1], st[BS_PCV + 2], st[BS_TRXI]};
+    finalize_baro(ctx, rec, raw, b);
     return PIMD_OK;
+}
+
+int pimd_get_barostat_history(pimd_ctx* ctx, pimd_barostat_state* b, int cap) {
+    if (!ctx || !b || cap < 0) return fail(ctx, PIMD_EINVAL, "bad argument");
+    if (!ctx->baro) return fail(ctx, PIMD_EINVAL, "no barostat set");
+    const int n = std::min(cap, ctx->est_hist_n);
+    if (n == 0) return 0;
+    std::vector<double> raw((size_t)ctx->est_hist_n * kEstWidth);
+    CK(cudaMemcpyAsync(raw.data(), ctx->est, raw.size() * 8, cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    const int skip = ctx->est_hist_n - n;
+    for (int q = 0; q < n; ++q) {
+        const double* r = raw.data() + (size_t)(skip + q) * kEstWidth;
+        finalize_baro(ctx, r + kEstBaro, r, b + q);
+    }
+    return n;
 }
 
 int pimd_set_method(pimd_ctx* ctx, int method) {
@@ -775,7 +798,7 @@ int pimd_step(pimd_ctx* ctx, int64_t n_steps) {
         if (s < n_steps) flags |= I_START;
         IntegratorArgs a;
         rec(ctx, 0);
-        if (ctx->baro) ctx->launches += run_barostat(ctx, s > 0, s < n_steps, ctx->step + s);
+        if (ctx->baro) ctx->launches += run_barostat(ctx, s > 0, s < n_steps, ctx->step + s, s > 0 ? slot : nullptr);
         if (ctx->fixcom && s > 0) {
             // fixcom (R-19): the removal needs sum_i m_i v~_0,i over ALL atoms after the closing half,
             // so the launch splits: close + accumulate, then subtract + estimators (+ open)

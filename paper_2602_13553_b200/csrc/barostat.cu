@@ -139,6 +139,10 @@ __global__ void baro_update_kernel(const __grid_constant__ BaroArgs a) {
         for (int q = 0; q < kBaroSums; ++q) S[0][q] = S[0][q] + S[1][q] + S[2][q];
         tr[0] = tr[0] + tr[1] + tr[2];
     }
+    if (a.est_slot != nullptr) {                // per-step record: the cell and the stress the estimators of this step see
+        for (int c = 0; c < 3; ++c) { a.est_slot[kEstBaro + 3 + c] = L[c]; a.est_slot[kEstBaro + 6 + c] = st[BS_PCV + c]; }
+        a.est_slot[kEstBaro + 9] = st[BS_TRXI];
+    }
     const double dim = a.aniso ? 1.0 : 3.0;     // E1: 3 dt/W [..] with P_CV = trace/3;  E2: dt/W [..] with P_CV^aa
     for (int d = 0; d < nd; ++d) {
         double vW = st[BS_VW + d];
@@ -156,12 +160,14 @@ __global__ void baro_update_kernel(const __grid_constant__ BaroArgs a) {
             vW = a.c1 * vW + a.c2sig * ee;
         };
         double* fac = st + BS_FAC + 6 * d;
+        double vW_end = vW;
         if (a.obabo) {
             // [E1, B](h) [O, E7](h) | [O, E7](h) [E1, B](h) [E4-E6 + A](dt)      (R-24)
             if (a.close) {
                 press_v();
                 if (a.thermostat) press_o(a.cstep_lo, a.cstep_hi);
             }
+            vW_end = vW;
             if (a.start) {
                 if (a.thermostat) press_o(a.step_lo, a.step_hi);
                 Skin = S[d][5]; Sfv = S[d][6];
@@ -176,6 +182,7 @@ __global__ void baro_update_kernel(const __grid_constant__ BaroArgs a) {
                 Skin = Skin + 2.0 * h * Sfv + h * h * Sff;     // what B(h), v~0 += h F~0/m, does to the two velocity sums
                 Sfv = Sfv + h * Sff;
             }
+            vW_end = vW;
             if (a.start) {
                 press_v();
                 fac[0] = exp(h * vW); fac[1] = sinh_over(vW, h); fac[2] = exp(-h * vW);
@@ -184,6 +191,8 @@ __global__ void baro_update_kernel(const __grid_constant__ BaroArgs a) {
             }
         }
         st[BS_VW + d] = vW;
+        if (a.est_slot != nullptr)
+            for (int c = d; c < (a.aniso ? d + 1 : 3); ++c) a.est_slot[kEstBaro + c] = vW_end;
     }
     if (!a.aniso) {
         // the integrator reads one factor set per component

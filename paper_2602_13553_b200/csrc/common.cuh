@@ -19,7 +19,8 @@ constexpr double kKB      = 8.617333262e-5;                       // eV / K
 
 constexpr int kMaxBeads = 64;
 constexpr int kEstCap   = 4096;     // estimator history slots per pimd_step call
-constexpr int kEstWidth = 4;        // K_ring, S_ring, sum x.f - x~0.f~0, U_sum
+constexpr int kEstWidth = 16;       // K_ring, S_ring, sum x.f - x~0.f~0, U_sum; barostat record at kEstBaro
+constexpr int kEstBaro  = 4;        // v_W[3], L[3], diag P_CV[3] (eV/A^3), sum_k Tr Xi: the cell at the END of the step
 
 // integrator launch flags
 enum : int { I_BCLOSE = 1, I_EST = 2, I_START = 4, I_OBABO = 8, I_COMACC = 16, I_COMSUB = 32, I_CART = 64 };
@@ -74,6 +75,7 @@ struct BaroArgs {
     uint32_t cstep_lo, cstep_hi; // OBABO: the step this launch closes, bit 31 of word 1 set
     const double* x; const double* vt; const double* f; const double* mass; const double* Xi;
     double* state;               // [BS_WIDTH]
+    double* est_slot;            // estimator slot of the step this launch closes (barostat record at kEstBaro), or null
     double* partial;             // [blocks][3][kBaroSums] block partials of the sums, per Cartesian component
 };
 constexpr int kBaroSums = 7;     // S_kin, S_cv, S_fv, S_ff, and (OBABO) S_kin after kick + closing O, S_kin and S_fv after the opening O

@@ -337,6 +337,33 @@ def test_checkpoint_resume_under_the_barostat(pk, aniso):
     ref.close(); sim.close()
 
 
+@pytest.mark.parametrize("integ,aniso", [("baoab", False), ("obabo", True)])
+def test_barostat_history_every_step(pk, integ, aniso):
+    """Appendix A outputs 8-15 of EVERY step of one pimd_step call against the oracle stepped one by one."""
+    N, P = 30, 4
+    types, masses, x, p = _trap_system(N, P, seed=12)
+    args = (types, masses, [10.0, 10.5, 11.0], P, 300.0, 1e-3, 20.0)
+    sim = pk.PIMD(*args, seed=6, integrator=integ)
+    sim.set_state(x, p)
+    sim.set_model_harmonic(0.5)
+    sim.set_barostat(40.0, 0.05, aniso=aniso)
+    orc = OraclePIMD(*args, seed=6, integrator=integ)
+    orc.set_barostat(40.0, 0.05, aniso=aniso)
+    orc.set_state(x, p)
+    orc.set_model_harmonic(0.5)
+    sim.step(7)
+    hist = sim.barostat_history()
+    assert len(hist) == 7
+    for q in range(7):
+        orc.step(1)
+        _compare_state(hist[q], orc.barostat_state(), 1e-9)
+    last = sim.barostat_state()
+    for key in ("v_W", "V", "P_CV", "P_PR", "P_MD", "K_W", "U_W", "J_W", "enthalpy"):
+        assert hist[-1][key] == last[key], key
+    assert len(sim.barostat_history(cap=3)) == 3
+    sim.close()
+
+
 def test_barostat_argument_errors(pk):
     types, masses, x, p = _trap_system(5, 4, seed=1)
     sim = pk.PIMD(types, masses, [10.0] * 3, 4, 300.0, 1e-3, 0.0, seed=1)
