@@ -181,7 +181,6 @@ row_scan_fill_kernel(int PN, int ntypes, int nsel, SelOff so, const int* __restr
     const int* seloff = so.v;
     const int tj = blockIdx.y, b = blockIdx.x, nblk = gridDim.x;
     __shared__ int red[8];
-    __shared__ int s_start[etc::kScanBlock], s_cnt[etc::kScanBlock], s_ba[etc::kScanBlock];
     __shared__ int s_off;
     // offset of this block = sum of the block sums before it
     int s = 0;
@@ -221,22 +220,26 @@ row_scan_fill_kernel(int PN, int ntypes, int nsel, SelOff so, const int* __restr
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
         const int r = r0 + q;
-        s_start[threadIdx.x * 4 + q] = run;
-        s_cnt[threadIdx.x * 4 + q] = c[q];
-        s_ba[threadIdx.x * 4 + q] = ba[q];
         if (r < PN) rowstart[(size_t)tj * (PN + 1) + r] = run;
         run += c[q];
         if (r == PN - 1) rowstart[(size_t)tj * (PN + 1) + PN] = run;
     }
-    __syncthreads();
-    // slot index of every compact row: one warp per centre, coalesced
-    int* out = rowaddr + (size_t)PN * seloff[tj];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    for (int q = warp; q < etc::kScanBlock; q += 8) {
-        const int n = s_cnt[q];
-        const int base = s_ba[q] * nsel + seloff[tj];
-        for (int e = lane; e < n; e += 32) out[s_start[q] + e] = base + e;
-    }
+}
+
+// slot index of every compact row: one warp per (neighbour type, centre), coalesced.  Its own launch: inside the scan
+// kernel (96 CTAs, each warp 128 centres in sequence) the fill was latency-bound (27 of the kernel's 30 us).
+__global__ void __launch_bounds__(256)
+row_fill_kernel(int PN, int ntypes, int nsel, SelOff so, const int* __restrict__ cen_idx,
+                const int* __restrict__ rowstart, int* __restrict__ rowaddr) {
+    const long long w = ((long long)blockIdx.x * 256 + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (w >= (long long)PN * ntypes) return;
+    const int tj = (int)(w / PN), r = (int)(w - (long long)tj * PN);
+    const int* rs = rowstart + (size_t)tj * (PN + 1);
+    const int s0 = rs[r], n = rs[r + 1] - s0;
+    const int base = cen_idx[r] * nsel + so.v[tj];
+    int* out = rowaddr + (size_t)PN * so.v[tj];
+    for (int e = lane; e < n; e += 32) out[s0 + e] = base + e;
 }
 
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
@@ -945,7 +948,10 @@ int emb_tc_row_index(Model& m, const ForceArgs& fa, cudaStream_t s) {
     row_block_sums_kernel<<<grid, 256, 0, s>>>(PN, fa.ntypes, m.cen_idx, m.ncount, m.row_bsum);
     row_scan_fill_kernel<<<grid, 256, 0, s>>>(PN, fa.ntypes, m.nsel, so, m.cen_idx, m.ncount, m.row_bsum, m.rowstart,
                                               m.rowaddr);
-    return 2;
+    const long long nw = (long long)PN * fa.ntypes;
+    row_fill_kernel<<<(unsigned)((nw * 32 + 255) / 256), 256, 0, s>>>(PN, fa.ntypes, m.nsel, so, m.cen_idx, m.rowstart,
+                                                                      m.rowaddr);
+    return 3;
 }
 
 int embedding_forward_tc(Model& m, const ForceArgs& fa, int n_sms, cudaStream_t s) {
