@@ -76,15 +76,39 @@ class Model:
 # neighbours
 # ----------------------------------------------------------------------------------------------
 
-def neighbours_bruteforce(x, box, rcut, i_block=128):
+def neighbours_bruteforce(x, box, rcut, i_block=128, centres=None):
     """All rows (i, j, n) with |(w_j - w_i) + n*L| < rcut, (j, n) != (i, 0), by brute force over
     every pair and every periodic image n in {-s..s}^3, s = ceil(rcut/L) (DESIGN R-11; PAPER.md:
     L200-202 for the wrap).  w = x - L*floor(x/L).  The squared distance is evaluated as
     (dx*dx + dy*dy) + dz*dz in FP64 with no fused multiply-add, compared strictly (< rcut*rcut).
-    Returns i[M], j[M], n[M,3] (int) and d[M,3] sorted by (i, j, n_x, n_y, n_z)."""
+    Returns i[M], j[M], n[M,3] (int) and d[M,3] sorted by (i, j, n_x, n_y, n_z).
+    `centres` (sorted atom indices) restricts the rows to those centres i -- the sampled parity checks at sizes
+    where all N^2 x images distance tests would take minutes; the arithmetic per row is unchanged."""
     x = np.asarray(x, dtype=np.float64)
     L = np.asarray(box, dtype=np.float64)
     N = x.shape[0]
+    if centres is not None:
+        centres = np.asarray(centres, dtype=np.int64)
+        w = x - L * np.floor(x / L)
+        s = [int(math.ceil(rcut / L[a])) for a in range(3)]
+        shifts = np.array([(a, b, c) for a in range(-s[0], s[0] + 1)
+                           for b in range(-s[1], s[1] + 1)
+                           for c in range(-s[2], s[2] + 1)], dtype=np.int64)
+        shift_vec = shifts.astype(np.float64) * L
+        self_img = np.flatnonzero((shifts == 0).all(axis=1))[0]
+        oi, oj, on, od = [], [], [], []
+        for i in centres:
+            d = (w[:, None, :] - w[i][None, None, :]) + shift_vec[None, :, :]
+            r2 = (d[..., 0] * d[..., 0] + d[..., 1] * d[..., 1]) + d[..., 2] * d[..., 2]
+            mask = r2 < rcut * rcut
+            mask[i, self_img] = False
+            bj, bs = np.nonzero(mask)
+            oi.append(np.full(bj.size, i, dtype=np.int64))
+            oj.append(bj)
+            on.append(shifts[bs])
+            od.append(d[bj, bs])
+        return (np.concatenate(oi), np.concatenate(oj), np.concatenate(on).reshape(-1, 3),
+                np.concatenate(od).reshape(-1, 3))
     w = x - L * np.floor(x / L)
     s = [int(math.ceil(rcut / L[a])) for a in range(3)]
     shifts = np.array([(a, b, c) for a in range(-s[0], s[0] + 1)

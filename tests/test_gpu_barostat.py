@@ -297,12 +297,19 @@ def test_npt_config4_full_size_sampled(pk):
     # forces and virial of a sampled bead at the cell the barostat produced
     model = se_e2_a.Model(desc, w)
     k = 37
-    Eo, Fo, Xio = se_e2_a.energy_forces(x[k], wb["types"], bs["box"], model)
+    Eo, Fo, Xio, parts = se_e2_a.energy_forces(x[k], wb["types"], bs["box"], model, return_parts=True)
     frms = np.sqrt((Fo ** 2).mean())
     err = np.abs(f[k] - Fo) / np.maximum(np.abs(Fo), frms)
     assert err.max() <= 1e-4, "force error %.3e" % err.max()
     assert np.abs(Xi[k] - Xio).max() <= 1e-4 * np.abs(Xio).max()
     assert abs(sim.energies()[k] - Eo.sum()) / sim.N <= 1e-6
+    # the neighbour rows of that bead in the moved cell (6 cells per side, the cell read from the device), row for
+    # row against the brute-force rows the oracle has just used (all 6144 centres)
+    count, j, shift = sim.neighbors(k)
+    ri, rj, rn = parts["ri"], parts["rj"], parts["rn"]
+    order = np.lexsort((rn[:, 2], rn[:, 1], rn[:, 0], rj, np.asarray(wb["types"])[rj], ri))
+    assert np.array_equal(count, np.bincount(ri, minlength=sim.N))
+    assert np.array_equal(j, rj[order]) and np.array_equal(shift.astype(np.int64), rn[order])
     sim.close()
 
 

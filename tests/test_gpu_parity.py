@@ -244,6 +244,94 @@ def test_neighbour_lists_bit_exact(pk, cfg_idx, beads):
     sim.close()
 
 
+def test_neighbour_lists_bit_exact_config2_full_cell_grid(pk):
+    """BASELINE.json configs[2] (the headline size): 4 cells per side, so the pruning of cells outside the cut-off
+    sphere, the compacted non-empty-cell list and the flat candidate walk of neighbor_env_kernel all discriminate
+    between cells.  Beads 0 and 31, every row (1536^2 x 27 FP64 distance tests per bead in the oracle)."""
+    cfg, wb, desc, w = workloads.make_config(2)
+    sim = pk.PIMD(wb["types"], wb["masses"], wb["box"], cfg["P"], cfg["T"], cfg["dt"], cfg["gamma"], seed=0,
+                  model_desc=desc)
+    sim.set_state(wb["x"], wb["p"])
+    sim.set_model(w)
+    for k in (0, 31):
+        count, j, shift = sim.neighbors(k)
+        ri, rj, rn = _oracle_rows(wb["x"][k], wb["types"], wb["box"], desc["rcut"])
+        assert np.array_equal(count, np.bincount(ri, minlength=sim.N))
+        assert np.array_equal(j, rj)
+        assert np.array_equal(shift.astype(np.int64), rn)
+        assert np.abs(shift).max() == 1 and count.sum() > 120000
+    sim.close()
+
+
+def _rows_of_centres(count, j, shift, centres):
+    """Slices of the library's concatenated canonical rows that belong to the given centres."""
+    start = np.concatenate([[0], np.cumsum(count)])
+    idx = np.concatenate([np.arange(start[i], start[i + 1]) for i in centres])
+    return np.concatenate([np.full(count[i], i) for i in centres]), j[idx], shift[idx].astype(np.int64)
+
+
+def test_neighbour_lists_bit_exact_config3_sampled_centres(pk):
+    """configs[3] (12288 atoms, 8 cells per side): 96 sampled centres of beads 0 and 17 -- among them the atoms
+    closest to the cell faces and box corners -- each compared with the brute-force rows of that centre."""
+    cfg, wb, desc, w = workloads.make_config(3)
+    sim = pk.PIMD(wb["types"], wb["masses"], wb["box"], cfg["P"], cfg["T"], cfg["dt"], cfg["gamma"], seed=0,
+                  model_desc=desc)
+    sim.set_state(wb["x"], wb["p"])
+    sim.set_model(w)
+    rng = np.random.default_rng(33)
+    L = wb["box"][0]
+    for k in (0, 17):
+        wk = wb["x"][k] - L * np.floor(wb["x"][k] / L)
+        cw = L / 8.0
+        face_dist = np.abs(((wk / cw) + 0.5) % 1.0 - 0.5).min(axis=1)           # distance to the nearest cell face
+        near = np.argsort(face_dist)[:16]
+        corner = np.argsort(np.abs(wk - L / 2).min(axis=1) * -1.0)[:16]            # closest to a box face
+        centres = np.unique(np.concatenate([near, corner, rng.choice(sim.N, size=64, replace=False)]))
+        count, j, shift = sim.neighbors(k)
+        ri, rj, rn, _ = se_e2_a.neighbours_bruteforce(wb["x"][k], wb["box"], desc["rcut"], centres=centres)
+        tj = np.asarray(wb["types"])[rj]
+        order = np.lexsort((rn[:, 2], rn[:, 1], rn[:, 0], rj, tj, ri))
+        gi, gj, gs = _rows_of_centres(count, j, shift, centres)
+        assert np.array_equal(gi, ri[order]) and np.array_equal(gj, rj[order]) and np.array_equal(gs, rn[order])
+    sim.close()
+
+
+def test_neighbour_lists_bit_exact_orthorhombic_3x4x5_cells(pk):
+    """A non-cubic box with a different number of cells per side (3, 4, 5) and different cell widths: the index
+    arithmetic of the cell walk (strides, per-axis wrap and image code) is exercised per axis.  Jittered lattice of
+    O/H sites at liquid-water number density; every row of both beads."""
+    desc = workloads.model_desc()
+    w = workloads.model_weights(desc, 4)
+    box = np.array([3 * 6.2, 4 * 6.4, 5 * 6.05])
+    g = np.array([9, 12, 14])                                # ~0.105 atoms / A^3
+    rng = np.random.default_rng(12)
+    idx = np.array([(a, b, c) for a in range(g[0]) for b in range(g[1]) for c in range(g[2])], dtype=np.float64)
+    x1 = (idx + 0.5) * (box / g) + rng.uniform(-0.35, 0.35, size=idx.shape)
+    N = x1.shape[0]
+    types = (np.arange(N) % 3 != 0).astype(np.int32)
+    rng.shuffle(types)
+    P = 2
+    x = x1[None] + 0.02 * rng.standard_normal((P, N, 3))
+    x[1] += np.array([2 * box[0], -3 * box[1], box[2]])      # bead 1 sits several boxes away (unwrapped state)
+    p = rng.standard_normal((P, N, 3))
+    sim = pk.PIMD(types, [15.9994, 1.008], box, P, 300.0, 0.25e-3, 1.0, seed=1, model_desc=desc)
+    sim.set_state(x, p)
+    sim.set_model(w)
+    for k in range(P):
+        count, j, shift = sim.neighbors(k)
+        ri, rj, rn = _oracle_rows(x[k], types, box, desc["rcut"])
+        assert np.array_equal(count, np.bincount(ri, minlength=N))
+        assert np.array_equal(j, rj) and np.array_equal(shift.astype(np.int64), rn)
+        assert set(np.unique(shift[:, 0])) == {-1, 0, 1} and set(np.unique(shift[:, 2])) == {-1, 0, 1}
+    # and the force path runs on that grid: forces of bead 0 against the oracle
+    model = se_e2_a.Model(desc, w)
+    Eo, Fo, Xio = se_e2_a.energy_forces(x[0], types, box, model)
+    f = sim.forces()
+    frms = np.sqrt((Fo ** 2).mean())
+    assert (np.abs(f[0] - Fo) / np.maximum(np.abs(Fo), frms)).max() <= 1e-4
+    sim.close()
+
+
 def test_neighbours_atoms_far_outside_the_box_and_on_faces(pk):
     """Unwrapped coordinates several boxes away, and atoms exactly on the faces x = 0, x = L."""
     cfg, wb, desc, w = workloads.make_config(0)
@@ -414,6 +502,81 @@ def test_force_parity_config2_headline_size_sampled_beads(pk):
     X3 = Xi.reshape(-1, 3, 3)
     assert np.abs(X3 - np.swapaxes(X3, 1, 2)).max() <= 1e-5 * np.abs(X3).max()
     sim.close()
+
+
+def test_force_parity_config2_strong_model_one_bead(pk):
+    """configs[2] with the last fitting layer scaled by 10^3 (forces ~0.2 eV/A: every term of the backward pass
+    matters; the x1 random-init model gives 2e-4 eV/A).  Energies scale with the layer, so their bound is the
+    relative one of DESIGN R-17: 1e-6 eV/atom per unit of last-layer scale."""
+    cfg, wb, desc, _ = workloads.make_config(2)
+    w = workloads.model_weights(desc, cfg["weight_seed"], last_layer_scale=1.0e3)
+    sim = pk.PIMD(wb["types"], wb["masses"], wb["box"], cfg["P"], cfg["T"], cfg["dt"], cfg["gamma"], seed=0,
+                  model_desc=desc)
+    sim.set_state(wb["x"], wb["p"])
+    sim.set_model(w)
+    model = se_e2_a.Model(desc, w)
+    f, U, Xi, E = sim.forces(), sim.energies(), sim.virial().reshape(-1, 3, 3), sim.atom_energies()
+    k = 19
+    Eo, Fo, Xio = se_e2_a.energy_forces(wb["x"][k], wb["types"], wb["box"], model)
+    frms = np.sqrt((Fo ** 2).mean())
+    assert frms > 0.05                                    # the force matters
+    err = np.abs(f[k] - Fo) / np.maximum(np.abs(Fo), frms)
+    assert err.max() <= 1e-4, "force error %.3e" % err.max()
+    assert abs(U[k] - Eo.sum()) / sim.N <= 1e-6 * 1.0e3
+    assert np.abs(E[k] - Eo).max() <= 1e-6 * 1.0e3
+    assert np.abs(Xi[k] - Xio).max() <= 1e-4 * np.abs(Xio).max()
+    sim.close()
+
+
+@pytest.mark.slow
+def test_config1_as_specified_100_steps_estimators_every_step(pk):
+    """BASELINE.json configs[1] as north_star states it: 64 H2O x 32 beads, the se_e2_a model, 100 steps in ONE
+    pimd_step(100) call, and the primitive (Eq. A7) and centroid-virial (Eq. A9) kinetic-energy
+    estimators of EVERY step (L86-88) against the oracle's (3200 bead evaluations of 192 atoms on the CPU).
+    x, p <= 1e-6 at step 10 (north_star) and at step 100."""
+    cfg, wb, desc, w = workloads.make_config(1)
+    assert cfg["P"] == 32 and cfg["steps"] == 100
+    args = (wb["types"], wb["masses"], wb["box"], cfg["P"], cfg["T"], cfg["dt"], cfg["gamma"])
+    sim = pk.PIMD(*args, seed=5, model_desc=desc)
+    sim.set_state(wb["x"], wb["p"])
+    sim.set_model(w)
+    from _parallel_oracle import ParallelOraclePIMD     # the oracle, one bead per worker process
+    orc = ParallelOraclePIMD(*args, seed=5)
+    orc.set_state(wb["x"], wb["p"])
+    orc.set_model(desc, w)
+    # the first ten steps in a call of their own: positions and momenta at step 10
+    sim10 = pk.PIMD(*args, seed=5, model_desc=desc)
+    sim10.set_state(wb["x"], wb["p"])
+    sim10.set_model(w)
+    sim10.step(10)
+    sim.step(100)
+    hist = sim.estimator_history()
+    assert [h["step"] for h in hist] == list(range(1, 101))
+    worst = {"K_PR": 0.0, "K_CV": 0.0, "H": 0.0}
+    for n, h in enumerate(hist, start=1):
+        orc.step(1)
+        o = orc.estimators()
+        for key in ("K_PR", "K_CV"):
+            rel = abs(h[key] - o[key]) / abs(o[key])
+            worst[key] = max(worst[key], rel)
+            assert rel <= 1e-6, (n, key, h[key], o[key])
+        dH = abs(h["H"] - o["H"]) / (sim.N * sim.P)
+        worst["H"] = max(worst["H"], dH)
+        assert dH <= 1e-6, (n, h["H"], o["H"])                              # eV per bead-atom
+        assert abs(h["T_ring"] - o["T_ring"]) <= 1e-6 * o["T_ring"]
+        if n == 10:
+            ex, ep = _rel(sim10.positions(), orc.positions()), _rel(sim10.momenta(), orc.momenta())
+            assert ex <= 1e-6 and ep <= 1e-6, (ex, ep)
+            print("configs[1] step 10: rel err x %.2e p %.2e" % (ex, ep))
+    ex, ep = _rel(sim.positions(), orc.positions()), _rel(sim.momenta(), orc.momenta())
+    print("configs[1] step 100: rel err x %.2e p %.2e; worst per-step K_PR %.2e K_CV %.2e H/bead-atom %.2e eV"
+          % (ex, ep, worst["K_PR"], worst["K_CV"], worst["H"]))
+    assert ex <= 1e-6 and ep <= 1e-6, (ex, ep)
+    e, o = sim.estimators(), orc.estimators()
+    assert e["step"] == 100 and abs(e["K_CV"] - o["K_CV"]) <= 1e-6 * abs(o["K_CV"])
+    orc.close()
+    sim.close()
+    sim10.close()
 
 
 # ---------------------------------------------------------------------------------------------

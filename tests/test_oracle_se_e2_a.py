@@ -323,3 +323,15 @@ def test_padded_slots_contribute_nothing_descriptor_scales_with_nsel(c0):
             h = np.concatenate([h, h], axis=1) + t if W.shape[1] == 2 * W.shape[0] else t
         acc += np.outer(h[0], p["R"][r_])
     assert np.abs(acc / 138.0 - p["T"][i]).max() < 1e-15
+
+
+def test_bruteforce_neighbours_restricted_to_centres_are_the_same_rows():
+    """`centres=` (used by the sampled GPU parity checks at configs[3]) returns exactly the rows of those centres."""
+    cfg, wb, desc, w = wl.make_config(0)
+    full = se_e2_a.neighbours_bruteforce(wb["x"][1], wb["box"], desc["rcut"])
+    centres = np.array([0, 5, 17, 95])
+    part = se_e2_a.neighbours_bruteforce(wb["x"][1], wb["box"], desc["rcut"], centres=centres)
+    keep = np.isin(full[0], centres)
+    assert keep.sum() > 300
+    for a, b in zip(full, part):
+        assert np.array_equal(a[keep], b)
