@@ -34,7 +34,11 @@ extern "C" {
 #define PIMD_EINVAL         -1   /* bad argument (null pointer, non-positive size, unsupported P, ...) */
 #define PIMD_ENOSTATE       -2   /* pimd_set_state has not been called */
 #define PIMD_ENOMODEL       -3   /* no force model has been set */
-#define PIMD_ESEL_OVERFLOW  -4   /* an atom has more neighbours of one type than sel allows (R-11) */
+#define PIMD_ESEL_OVERFLOW  -4   /* an atom has more neighbours of one type than sel allows (R-11), or the cell outran
+                                  * its cell grid inside one call.  From pimd_step: the call is undone as a whole (x, p, f,
+                                  * U, Xi, cell and step counter are those at entry; the message names the failing step).
+                                  * From pimd_set_state / pimd_set_model / pimd_set_barostat: the context is left WITHOUT
+                                  * a state (the forces of a truncated neighbour list are not kept); set a new one. */
 #define PIMD_ECUDA          -5   /* CUDA runtime error; see pimd_last_error */
 #define PIMD_ENOMEM         -6   /* the caller-supplied workspace is too small */
 
@@ -99,8 +103,11 @@ int pimd_set_state(pimd_ctx* ctx, const double* x, const double* p);
 /* Resume from a checkpoint {x, p, f, U, step} (host arrays; SURVEY section 5 "checkpoint / resume"):
  * like pimd_set_state, but the forces f[P][N][3] and bead energies U[P] that belong to x are supplied,
  * so no force evaluation is run, and the step counter (which keys the Philox noise, R-10) is set to
- * `step`.  Because the noise is counter-based, restore + pimd_step(n) continues a trajectory exactly
- * as the uninterrupted run would have.  A model must already be set. */
+ * `step`.  Because the noise is counter-based, restore + pimd_step(n) draws exactly the random numbers the
+ * uninterrupted run would have drawn.  With the harmonic model the continued trajectory is bit-identical; with the
+ * se_e2_a model the forces, U and the estimator sums are accumulated with floating-point atomics whose order is not
+ * fixed, so two runs (restored or not) agree to rounding (~1e-16 relative per evaluation), not bit for bit.
+ * A model must already be set. */
 int pimd_restore(pimd_ctx* ctx, const double* x, const double* p, const double* f, const double* U, int64_t step);
 
 /* The se_e2_a Deep-Potential model (PAPER.md:L47, L76 cite it; definition DESIGN.md R-11..R-16).
@@ -118,7 +125,9 @@ int pimd_set_model_harmonic(pimd_ctx* ctx, double k_spring /* eV/A^2 */);
 
 /* n_steps BAOAB steps: B(dt/2) A(dt/2) O(dt) A(dt/2) [force] B(dt/2), with the three
  * normal-mode transforms of L192 and one force evaluation per step (R-7).  All work runs on the
- * GPU; there is no host round trip inside the loop. */
+ * GPU; there is no host round trip inside the loop.  Errors are detected when the call ends: on
+ * PIMD_ESEL_OVERFLOW the whole call is rolled back (see the code's comment above), so the caller can retry with
+ * a larger sel, fewer steps per call (barostat) or stop; the state is never left half-advanced. */
 int pimd_step(pimd_ctx* ctx, int64_t n_steps);
 
 /* ---- outputs -------------------------------------------------------------------------------- */

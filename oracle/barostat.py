@@ -162,9 +162,11 @@ def press_o_step_aniso(vW, P, N, T, W, gamma0, h, seed, step, half=0):
 
 
 def p_pr(S_ring, P, N, T, V):
-    """Eq. A10: (1/3V)(3 n N k_B T - sum m omega_n^2 |r^(k)-r^(k+1)|^2) with the square on
-    omega_n as in A7 (DESIGN R-6): the sum is twice the spring energy S_ring."""
-    return (3.0 * P * N * KB * T - 2.0 * S_ring) / (3.0 * V)
+    """Eq. A10: (1/3V)(3 n N k_B T - (1/n) sum m omega_n^2 |r^(k)-r^(k+1)|^2).  The printed spring sum
+    is A7's (L354), garbled the same way: the square on omega_n AND the 1/n of DESIGN R-6 -- with them A10 is
+    (2/3V) K_PR and the free ring polymer gives the ideal-gas pressure N k_B T / V (pinned in
+    tests/test_oracle_barostat.py); as printed it gives -n(n-2) N k_B T / V.  The sum is twice S_ring."""
+    return (3.0 * P * N * KB * T - 2.0 * S_ring / P) / (3.0 * V)
 
 
 def p_md(K_ring, Xi, V):

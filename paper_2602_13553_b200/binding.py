@@ -182,7 +182,21 @@ def pimd_set_state(ctx, x, p):
     return _check(ctx, lib().pimd_set_state(ctx, x.ctypes.data, p.ctypes.data))
 
 
-def pimd_set_state_dev(ctx, x_dev, p_dev):
+def _dev_f64(t, numel, what):
+    """A torch CUDA tensor handed to a `_dev` call crosses the C ABI as a raw pointer: check here that it is what the
+    library will read (float64, contiguous, on the GPU, `numel` elements).  Plain ints (raw device pointers) pass."""
+    if hasattr(t, "data_ptr"):
+        import torch
+        if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and t.numel() == numel):
+            raise ValueError("%s must be a contiguous float64 CUDA tensor of %d elements (got %s, %s, %d elements%s)"
+                             % (what, numel, t.device, t.dtype, t.numel(), "" if t.is_contiguous() else ", non-contiguous"))
+    return _ptr(t)
+
+
+def pimd_set_state_dev(ctx, x_dev, p_dev, numel=None):
+    """numel = P*N*3 enables the tensor checks of _dev_f64 (PIMD.set_state passes it)."""
+    if numel is not None:
+        return _check(ctx, lib().pimd_set_state_dev(ctx, _dev_f64(x_dev, numel, "x_dev"), _dev_f64(p_dev, numel, "p_dev")))
     return _check(ctx, lib().pimd_set_state_dev(ctx, _ptr(x_dev), _ptr(p_dev)))
 
 
@@ -333,12 +347,12 @@ def pimd_get_estimator_history(ctx, cap):
     return [arr[q].as_dict() for q in range(n)]
 
 
-def pimd_get_positions_dev(ctx, x_dev):
-    return _check(ctx, lib().pimd_get_positions_dev(ctx, _ptr(x_dev)))
+def pimd_get_positions_dev(ctx, x_dev, numel=None):
+    return _check(ctx, lib().pimd_get_positions_dev(ctx, _ptr(x_dev) if numel is None else _dev_f64(x_dev, numel, "x_dev")))
 
 
-def pimd_get_forces_dev(ctx, f_dev):
-    return _check(ctx, lib().pimd_get_forces_dev(ctx, _ptr(f_dev)))
+def pimd_get_forces_dev(ctx, f_dev, numel=None):
+    return _check(ctx, lib().pimd_get_forces_dev(ctx, _ptr(f_dev) if numel is None else _dev_f64(f_dev, numel, "f_dev")))
 
 
 def pimd_get_neighbors(ctx, bead, N, cap):
@@ -411,7 +425,10 @@ class PIMD:
 
     def set_state(self, x, p):
         if hasattr(x, "data_ptr"):
-            return pimd_set_state_dev(self.ctx, x, p)
+            return pimd_set_state_dev(self.ctx, x, p, numel=self.P * self.N * 3)
+        x, p = np.asarray(x), np.asarray(p)
+        if x.size != self.P * self.N * 3 or p.size != x.size:
+            raise ValueError("x and p must hold P*N*3 = %d values" % (self.P * self.N * 3))
         return pimd_set_state(self.ctx, x, p)
 
     def set_model(self, weights, desc=None):

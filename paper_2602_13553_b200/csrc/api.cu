@@ -8,7 +8,24 @@
 #include <new>
 #include "common.cuh"
 
+#include <mutex>
+#include <unordered_map>
+
 using namespace pimd;
+
+namespace pimd {
+void ensure_dyn_smem_impl(const void* kernel, int bytes) {
+    static std::mutex mu;
+    static std::unordered_map<const void*, unsigned long long> done;      // kernel -> bit per device ordinal
+    int dev = 0;
+    cudaGetDevice(&dev);
+    std::lock_guard<std::mutex> lock(mu);
+    unsigned long long& mask = done[kernel];
+    if (dev < 64 && ((mask >> dev) & 1ull)) return;
+    cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (dev < 64) mask |= 1ull << dev;
+}
+}  // namespace pimd
 
 struct pimd_ctx {
     int N = 0, P = 0, ntypes = 0;
@@ -40,7 +57,10 @@ struct pimd_ctx {
     int model_kind = 0;           // 0 none, 1 harmonic, 2 se_e2_a
     double k_spring = 0;
     double *x = nullptr, *vt = nullptr, *f = nullptr, *mass_atom = nullptr;
-    double *scratch_a = nullptr, *scratch_b = nullptr;     // [P][N][3] each: momenta staging / timing outputs
+    double *scratch_a = nullptr, *scratch_b = nullptr;     // [P][N][3] each: momenta staging / timing outputs; inside
+                                                           // pimd_step: the entry snapshot of x and v~ (rollback)
+    double *snap_f = nullptr, *snap_small = nullptr;       // entry snapshot of f [P][N][3]; of U, Xi, barostat state
+    int64_t evals_launched = 0;                            // force evaluations issued so far (mirrors model.overflow[2])
     int* types_d = nullptr;
     double *U = nullptr, *Xi = nullptr, *Eatom = nullptr;
     double* est = nullptr;        // [kEstCap + 2][kEstWidth]; slot kEstCap = "current", kEstCap+1 = scratch
@@ -91,7 +111,8 @@ int arena_alloc(pimd_ctx* ctx, T** out, size_t count) {
 size_t base_bytes(const pimd_ctx* c) {
     const size_t PN3 = (size_t)c->P * c->N * 3;
     size_t b = 0;
-    b += 5 * align_up(PN3 * 8, 256);                          // x, vt, f, scratch_a, scratch_b
+    b += 6 * align_up(PN3 * 8, 256);                          // x, vt, f, scratch_a, scratch_b, snap_f
+    b += align_up(((size_t)c->P * 10 + BS_WIDTH) * 8, 256);   // snap_small
     b += align_up((size_t)c->N * 8, 256) + align_up((size_t)c->N * 4, 256);
     b += align_up((size_t)c->P * 8, 256) + align_up((size_t)c->P * 72, 256) + align_up((size_t)c->P * c->N * 8, 256);
     b += align_up((size_t)(kEstCap + 2) * kEstWidth * 8, 256);
@@ -176,6 +197,8 @@ int alloc_base(pimd_ctx* ctx) {
     if ((rc = arena_alloc(ctx, &ctx->f, PN3))) return rc;
     if ((rc = arena_alloc(ctx, &ctx->scratch_a, PN3))) return rc;
     if ((rc = arena_alloc(ctx, &ctx->scratch_b, PN3))) return rc;
+    if ((rc = arena_alloc(ctx, &ctx->snap_f, PN3))) return rc;
+    if ((rc = arena_alloc(ctx, &ctx->snap_small, (size_t)ctx->P * 10 + BS_WIDTH))) return rc;
     if ((rc = arena_alloc(ctx, &ctx->mass_atom, (size_t)ctx->N))) return rc;
     if ((rc = arena_alloc(ctx, &ctx->types_d, (size_t)ctx->N))) return rc;
     if ((rc = arena_alloc(ctx, &ctx->U, (size_t)ctx->P))) return rc;
@@ -218,6 +241,7 @@ int eval_forces(pimd_ctx* ctx) {
     cudaMemsetAsync(ctx->U, 0, sizeof(double) * ctx->P, ctx->stream);
     cudaMemsetAsync(ctx->Xi, 0, sizeof(double) * 9 * ctx->P, ctx->stream);
     rec(ctx, 1);
+    ctx->evals_launched += 1;
     ctx->launches += neighbor_build(ctx->model, a, ctx->stream);
     const bool tc_emb = ctx->model.use_tc_emb && ctx->model.tc_emb_ready;
     if (tc_emb) ctx->launches += emb_tc_row_index(ctx->model, a, ctx->stream);
@@ -290,14 +314,19 @@ int sync_box(pimd_ctx* ctx) {
     return PIMD_OK;
 }
 
-int check_overflow(pimd_ctx* ctx) {
+// model.overflow = {flag, first failing force evaluation (1-based count since pimd_set_model), evaluation counter, -}.
+// Returns 0, or the error with *failed_eval = the 0-based index of the first evaluation that overflowed.
+int check_overflow(pimd_ctx* ctx, int64_t* failed_eval = nullptr) {
     if (ctx->model_kind != 2) return PIMD_OK;
-    int flag = 0;
-    CK(cudaMemcpyAsync(&flag, ctx->model.overflow, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+    unsigned flag[2] = {0u, 0u};
+    CK(cudaMemcpyAsync(flag, ctx->model.overflow, sizeof(flag), cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
-    if (flag) {
-        cudaMemsetAsync(ctx->model.overflow, 0, sizeof(int), ctx->stream);
-        if (flag & 2)
+    if (flag[0]) {
+        const unsigned reset[2] = {0u, 0xFFFFFFFFu};
+        cudaMemcpyAsync(ctx->model.overflow, reset, sizeof(reset), cudaMemcpyHostToDevice, ctx->stream);
+        cudaStreamSynchronize(ctx->stream);
+        if (failed_eval) *failed_eval = (int64_t)flag[1] - 1;
+        if (flag[0] & 2u)
             return fail(ctx, PIMD_ESEL_OVERFLOW, "the cell shrank past the cell-grid margin inside one pimd_step call; use fewer steps per call");
         return fail(ctx, PIMD_ESEL_OVERFLOW, "an atom has more neighbours of one type than sel allows");
     }
@@ -320,7 +349,9 @@ int refresh(pimd_ctx* ctx) {
     CK(cudaGetLastError());
     CK(cudaStreamSynchronize(ctx->stream));
     ctx->est_hist_n = 0;
-    return check_overflow(ctx);
+    rc = check_overflow(ctx);
+    if (rc) ctx->have_state = false;      // forces of a truncated neighbour list: nothing to integrate from (pimd.h)
+    return rc;
 }
 
 void finalize_est(const pimd_ctx* c, const double raw[kEstWidth], int64_t step, pimd_estimators* e) {
@@ -534,7 +565,7 @@ static void finalize_baro(const pimd_ctx* ctx, const double* rec, const double* 
     if (!ctx->baro_aniso) b->K_W = 0.5 * ctx->baro_W * rec[0] * rec[0];                    // A13
     b->V = rec[3] * rec[4] * rec[5];
     b->P_CV = (rec[6] + rec[7] + rec[8]) / 3.0 * kBarPerEvA3;                              // A12 = the mean of E3's diagonal
-    b->P_PR = (3.0 * n * N * kKB * ctx->T - 2.0 * raw[1]) / (3.0 * b->V) * kBarPerEvA3;    // A10
+    b->P_PR = (3.0 * n * N * kKB * ctx->T - 2.0 * raw[1] / n) / (3.0 * b->V) * kBarPerEvA3;  // A10 with R-6's 1/n: = 2 K_PR / (3V)
     b->P_MD = (2.0 * raw[0] + rec[9]) / (3.0 * b->V) * kBarPerEvA3;                        // A11
     b->U_W = n * ctx->p_ext * b->V;                                                        // A15
     b->J_W = -n * kKB * ctx->T * std::log(b->V);                                           // A16
@@ -753,7 +784,7 @@ int pimd_set_model(pimd_ctx* ctx, const pimd_model_desc* d, const double* w, siz
     if ((rc = arena_alloc(ctx, &m.ncount, PN * nt))) return rc;
     if ((rc = arena_alloc(ctx, &m.slotA, PN * m.nsel))) return rc;
     if ((rc = arena_alloc(ctx, &m.slotB, PN * m.nsel))) return rc;
-    if ((rc = arena_alloc(ctx, &m.overflow, (size_t)1))) return rc;
+    if ((rc = arena_alloc(ctx, &m.overflow, (size_t)4))) return rc;
     if ((rc = arena_alloc(ctx, &m.Tm, PN * m.M1 * 4))) return rc;
     if ((rc = arena_alloc(ctx, &m.dTm, PN * m.M1 * 4))) return rc;
     if ((rc = arena_alloc(ctx, &m.D, PN * m.ND))) return rc;
@@ -766,7 +797,10 @@ int pimd_set_model(pimd_ctx* ctx, const pimd_model_desc* d, const double* w, siz
     if ((rc = arena_alloc(ctx, &m.row_bsum, (size_t)nt * ((PN + 1023) / 1024)))) return rc;
     if ((rc = arena_alloc(ctx, &m.cpart, PN * 9))) return rc;
     m.tc_emb_ready = true;
-    CK(cudaMemsetAsync(m.overflow, 0, sizeof(int), ctx->stream));
+    {
+        const unsigned ov0[4] = {0u, 0xFFFFFFFFu, (unsigned)ctx->evals_launched, 0u};
+        CK(cudaMemcpyAsync(m.overflow, ov0, sizeof(ov0), cudaMemcpyHostToDevice, ctx->stream));
+    }
     CK(cudaStreamSynchronize(ctx->stream));     // host staging vectors go out of scope below
     tc_setup_maps(m, nt);        // tensor-core fitting path (falls back to the CUDA-core GEMMs only if unsupported widths)
     m.set = true;
@@ -781,6 +815,23 @@ int pimd_step(pimd_ctx* ctx, int64_t n_steps) {
     if (ctx->model_kind == 0) return fail(ctx, PIMD_ENOMODEL, "no force model set");
     if (n_steps == 0) return PIMD_OK;
     { int rc = sync_box(ctx); if (rc) return rc; }
+    // Entry snapshot (se_e2_a model only: the harmonic model cannot fail): a sel overflow or a cell that outruns its
+    // grid at step k leaves every later step of the call integrating truncated neighbour rows, so the call is then
+    // undone as a whole -- x, v~, f, U, Xi, the barostat state and the step counter return to their entry values.
+    const size_t PN3 = (size_t)ctx->P * ctx->N * 3;
+    const bool snap = ctx->model_kind == 2;
+    const int64_t evals0 = ctx->evals_launched;
+    double box0[3] = {ctx->box[0], ctx->box[1], ctx->box[2]};
+    if (snap) {
+        CK(cudaMemcpyAsync(ctx->scratch_a, ctx->x, PN3 * 8, cudaMemcpyDeviceToDevice, ctx->stream));
+        CK(cudaMemcpyAsync(ctx->scratch_b, ctx->vt, PN3 * 8, cudaMemcpyDeviceToDevice, ctx->stream));
+        CK(cudaMemcpyAsync(ctx->snap_f, ctx->f, PN3 * 8, cudaMemcpyDeviceToDevice, ctx->stream));
+        CK(cudaMemcpyAsync(ctx->snap_small, ctx->U, sizeof(double) * ctx->P, cudaMemcpyDeviceToDevice, ctx->stream));
+        CK(cudaMemcpyAsync(ctx->snap_small + ctx->P, ctx->Xi, sizeof(double) * 9 * ctx->P, cudaMemcpyDeviceToDevice, ctx->stream));
+        if (ctx->baro)
+            CK(cudaMemcpyAsync(ctx->snap_small + 10 * (size_t)ctx->P, ctx->baro_state, sizeof(double) * BS_WIDTH,
+                               cudaMemcpyDeviceToDevice, ctx->stream));
+    }
     const int hist = (int)std::min<int64_t>(n_steps, kEstCap);
     const int64_t first_hist = n_steps - hist;            // steps before this index are not recorded
     CK(cudaMemsetAsync(ctx->est, 0, sizeof(double) * (size_t)hist * kEstWidth, ctx->stream));
@@ -828,6 +879,30 @@ int pimd_step(pimd_ctx* ctx, int64_t n_steps) {
     CK(cudaMemcpyAsync(cur, ctx->est + (size_t)(hist - 1) * kEstWidth, sizeof(double) * kEstWidth,
                        cudaMemcpyDeviceToDevice, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
+    {
+        int64_t failed_eval = -1;
+        const int rc = check_overflow(ctx, &failed_eval);
+        if (rc) {
+            const std::string why = ctx->err;
+            CK(cudaMemcpyAsync(ctx->x, ctx->scratch_a, PN3 * 8, cudaMemcpyDeviceToDevice, ctx->stream));
+            CK(cudaMemcpyAsync(ctx->vt, ctx->scratch_b, PN3 * 8, cudaMemcpyDeviceToDevice, ctx->stream));
+            CK(cudaMemcpyAsync(ctx->f, ctx->snap_f, PN3 * 8, cudaMemcpyDeviceToDevice, ctx->stream));
+            CK(cudaMemcpyAsync(ctx->U, ctx->snap_small, sizeof(double) * ctx->P, cudaMemcpyDeviceToDevice, ctx->stream));
+            CK(cudaMemcpyAsync(ctx->Xi, ctx->snap_small + ctx->P, sizeof(double) * 9 * ctx->P, cudaMemcpyDeviceToDevice, ctx->stream));
+            if (ctx->baro) {
+                CK(cudaMemcpyAsync(ctx->baro_state, ctx->snap_small + 10 * (size_t)ctx->P, sizeof(double) * BS_WIDTH,
+                                   cudaMemcpyDeviceToDevice, ctx->stream));
+                for (int c = 0; c < 3; ++c) ctx->box[c] = box0[c];
+            }
+            CK(cudaStreamSynchronize(ctx->stream));
+            ctx->est_hist_n = 0;
+            char where[160];
+            snprintf(where, sizeof(where), " (first at step %lld of this call of %lld = absolute step %lld); the state has been "
+                     "rolled back to the start of the call",
+                     (long long)(failed_eval - evals0 + 1), (long long)n_steps, (long long)(ctx->step + failed_eval - evals0 + 1));
+            return fail(ctx, rc, why + where);
+        }
+    }
     ctx->step += n_steps;
     ctx->est_hist_n = hist;
     ctx->est_hist_first_step = ctx->step - hist + 1;
@@ -835,7 +910,7 @@ int pimd_step(pimd_ctx* ctx, int64_t n_steps) {
         for (int q = 0; q < 6; ++q) ctx->phase_ms[q] = ms_acc[q] / (double)n_steps;
         ctx->phase_steps = n_steps;
     }
-    return check_overflow(ctx);
+    return PIMD_OK;
 }
 
 static int copy_out(pimd_ctx* ctx, const void* dev, void* host, size_t bytes) {
@@ -968,10 +1043,10 @@ int pimd_debug_noise(pimd_ctx* ctx, int64_t step, int n, const int32_t* idx, uin
 int pimd_time_kernel(pimd_ctx* ctx, int kind, int reps, double* ms) {
     if (!ctx || !ms || reps <= 0) return fail(ctx, PIMD_EINVAL, "bad argument");
     if (!ctx->have_state || ctx->model_kind == 0) return fail(ctx, PIMD_ENOSTATE, "needs a state and a model");
-    if (kind != 0) return fail(ctx, PIMD_EINVAL, "unknown kernel kind");
+    if (kind != 0 && kind != 1) return fail(ctx, PIMD_EINVAL, "unknown kernel kind");
     IntegratorArgs a;
     double* scratch = ctx->est + (size_t)(kEstCap + 1) * kEstWidth;
-    fill_integrator_args(ctx, a, I_BCLOSE | I_EST | I_START, ctx->step, scratch);
+    fill_integrator_args(ctx, a, I_BCLOSE | I_EST | I_START | (kind == 1 ? I_NOISE_PER_MODE : 0), ctx->step, scratch);
     a.x_out = ctx->scratch_a; a.vt_out = ctx->scratch_b;          // state is not advanced
     for (int w = 0; w < 3; ++w) ctx->launches += launch_integrator(ctx->P, a, ctx->mc, ctx->stream);
     CK(cudaEventRecord(ctx->ev[6], ctx->stream));

@@ -23,7 +23,8 @@ constexpr int kEstWidth = 16;       // K_ring, S_ring, sum x.f - x~0.f~0, U_sum;
 constexpr int kEstBaro  = 4;        // v_W[3], L[3], diag P_CV[3] (eV/A^3), sum_k Tr Xi: the cell at the END of the step
 
 // integrator launch flags
-enum : int { I_BCLOSE = 1, I_EST = 2, I_START = 4, I_OBABO = 8, I_COMACC = 16, I_COMSUB = 32, I_CART = 64 };
+enum : int { I_BCLOSE = 1, I_EST = 2, I_START = 4, I_OBABO = 8, I_COMACC = 16, I_COMSUB = 32, I_CART = 64,
+              I_NOISE_PER_MODE = 128 /* timing only: one Philox draw per mode (DESIGN R-10 A/B) */ };
 
 // Per-mode constants of the A and O steps (DESIGN R-3, R-5), kernel parameter.
 struct ModeConsts {
@@ -80,6 +81,12 @@ struct BaroArgs {
 };
 constexpr int kBaroSums = 7;     // S_kin, S_cv, S_fv, S_ff, and (OBABO) S_kin after kick + closing O, S_kin and S_fv after the opening O
 int launch_barostat(const BaroArgs& a, cudaStream_t s);
+
+// Opt-in to more than 48 KB of dynamic shared memory, once per (kernel, device): the attribute belongs to the
+// kernel's image on ONE device, so a process-wide "done" flag would leave a second device without it.
+void ensure_dyn_smem_impl(const void* kernel, int bytes);
+template <typename K>
+inline void ensure_dyn_smem(K kernel, int bytes) { ensure_dyn_smem_impl(reinterpret_cast<const void*>(kernel), bytes); }
 size_t barostat_state_doubles(int n_dof);    // BS_WIDTH + the partials
 
 int launch_integrator(int P, const IntegratorArgs& a, const ModeConsts& mc, cudaStream_t s);

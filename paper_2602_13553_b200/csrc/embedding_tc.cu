@@ -956,11 +956,7 @@ int emb_tc_row_index(Model& m, const ForceArgs& fa, cudaStream_t s) {
 
 int embedding_forward_tc(Model& m, const ForceArgs& fa, int n_sms, cudaStream_t s) {
     EmbTcArgs a = make_tc_args(m, fa);
-    static bool attr = false;
-    if (!attr) {
-        cudaFuncSetAttribute(embed_fwd_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, f3::kSmemBytes);
-        attr = true;
-    }
+    ensure_dyn_smem(embed_fwd_tc_kernel, f3::kSmemBytes);
     cudaMemsetAsync(m.Tm, 0, sizeof(float) * (size_t)a.PN * etc::M1 * 4, s);
     embed_fwd_tc_kernel<<<n_sms, f3::kThreads, f3::kSmemBytes, s>>>(a);
     return 1;
@@ -968,11 +964,7 @@ int embedding_forward_tc(Model& m, const ForceArgs& fa, int n_sms, cudaStream_t 
 
 int embedding_backward_tc(Model& m, const ForceArgs& fa, int n_sms, cudaStream_t s) {
     EmbTcArgs a = make_tc_args(m, fa);
-    static bool attr = false;
-    if (!attr) {
-        cudaFuncSetAttribute(embed_bwd_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, etc::kSmemBytesBwd);
-        attr = true;
-    }
+    ensure_dyn_smem(embed_bwd_tc_kernel, etc::kSmemBytesBwd);
     cudaMemsetAsync(m.cpart, 0, sizeof(double) * (size_t)a.PN * 9, s);
     embed_bwd_tc_kernel<<<n_sms, etc::kThreads, etc::kSmemBytesBwd, s>>>(a);
     virial_reduce_kernel<<<fa.P, 256, 0, s>>>(fa.ntypes, a, fa.Xi);

@@ -750,12 +750,7 @@ constexpr int kNH = 1, kST = 4, kOCC = 1;     // 128-row tiles, 2 stages, 2 CTAs
 template <int BN, int EPI>
 static cudaError_t launch_tc(const TcMaps& maps, const TcGemmArgs& g, int mtiles, cudaStream_t s) {
     using SM = TcSmem<BN, kNH, kST>;
-    static bool attr = false;
-    if (!attr) {
-        cudaError_t e = cudaFuncSetAttribute(gemm3xtf32_kernel<BN, EPI, kNH, kST, kOCC>, cudaFuncAttributeMaxDynamicSharedMemorySize, SM::kTotal);
-        if (e != cudaSuccess) return e;
-        attr = true;
-    }
+    ensure_dyn_smem(gemm3xtf32_kernel<BN, EPI, kNH, kST, kOCC>, SM::kTotal);
     dim3 grid((g.N + BN - 1) / BN, mtiles);
     gemm3xtf32_kernel<BN, EPI, kNH, kST, kOCC><<<grid, kTcThreads, SM::kTotal, s>>>(maps, g);
     return cudaGetLastError();
@@ -897,12 +892,8 @@ static void chain_range(Model& m, const ForceArgs& fa, int t0, int ntl, cudaStre
 int fitting_chain_tc(Model& m, const ForceArgs& fa, cudaStream_t s) {
     TcGemmArgs g{};
     const int tiles = fill_types(m, fa.ntypes, g);
-    static bool attr = false;
-    if (!attr) {
-        cudaFuncSetAttribute(l1_desc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, L1Smem::kTotal);
-        cudaFuncSetAttribute(dd_dt_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, DdSmem::kTotal);
-        attr = true;
-    }
+    ensure_dyn_smem(l1_desc_kernel, L1Smem::kTotal);
+    ensure_dyn_smem(dd_dt_kernel, DdSmem::kTotal);
     constexpr int NR = Model::kChainStreams;
     if (!m.aux_stream[0]) {
         for (int q = 0; q < NR - 1; ++q) {

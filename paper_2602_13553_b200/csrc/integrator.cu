@@ -142,6 +142,18 @@ integrator_kernel(const __grid_constant__ IntegratorArgs a, const __grid_constan
     //      the step this launch opens; OBABO: first the closing O(dt/2) of the previous step (its second half-step
     //      stream), the opening O's normals are generated between the two mode loops below ----
     auto gen_normals = [&](uint32_t s_lo, uint32_t s_hi) {
+        if (a.flags & I_NOISE_PER_MODE) {
+            // TIMING ONLY (pimd_time_kernel kind 1; DESIGN R-10's A/B number): the keying SURVEY C-7 first proposed,
+            // one draw per mode, counter word 3 = 4k + alpha, sine branch discarded -- twice the Philox / log / sqrt /
+            // sincospi work of the pair scheme the library (and the oracle) use.  Never reached by pimd_step.
+#pragma unroll 4
+            for (int k = 0; k < P; ++k) {
+                double ee, eo;
+                philox_normal_pair(a.seed_lo, a.seed_hi, s_lo, s_hi, (uint32_t)i, (uint32_t)(4 * k + alpha), &ee, &eo);
+                eta_s[k * kIntThreads] = ee;
+            }
+            return;
+        }
 #pragma unroll 4
         for (int q = 0; q < (P + 1) / 2; ++q) {
             double ee, eo;
@@ -296,12 +308,8 @@ template <int P>
 static void launch_int_t(const IntegratorArgs& a, const ModeConsts& mc, cudaStream_t s) {
     const int blocks = (a.n_dof + kIntThreads - 1) / kIntThreads;
     const size_t smem = (size_t)3 * P * kIntThreads * sizeof(double);
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaFuncSetAttribute(integrator_kernel<P, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        cudaFuncSetAttribute(integrator_kernel<P, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        attr_done = true;
-    }
+    ensure_dyn_smem(integrator_kernel<P, false>, (int)smem);
+    ensure_dyn_smem(integrator_kernel<P, true>, (int)smem);
     if (a.flags & I_OBABO) integrator_kernel<P, true><<<blocks, kIntThreads, smem, s>>>(a, mc);
     else integrator_kernel<P, false><<<blocks, kIntThreads, smem, s>>>(a, mc);
 }
@@ -428,12 +436,8 @@ template <int P>
 static void launch_cart_t(const IntegratorArgs& a, const ModeConsts& mc, cudaStream_t s) {
     const int blocks = (a.n_dof + kIntThreads - 1) / kIntThreads;
     const size_t smem = (size_t)P * kIntThreads * sizeof(double);
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaFuncSetAttribute(integrator_cart_kernel<P, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        cudaFuncSetAttribute(integrator_cart_kernel<P, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        attr_done = true;
-    }
+    ensure_dyn_smem(integrator_cart_kernel<P, false>, (int)smem);
+    ensure_dyn_smem(integrator_cart_kernel<P, true>, (int)smem);
     if (a.flags & I_OBABO) integrator_cart_kernel<P, true><<<blocks, kIntThreads, smem, s>>>(a, mc);
     else integrator_cart_kernel<P, false><<<blocks, kIntThreads, smem, s>>>(a, mc);
 }

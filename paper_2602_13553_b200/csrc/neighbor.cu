@@ -44,10 +44,17 @@ __global__ void wrap_bin_kernel(int P, int N, GridGeom g, const double* __restri
     const int k = ba / N;
     double gL[3], ginv_w[3];
     load_geom(g, gL, ginv_w);
-    if (g.boxp && ba == 0) {
-        // the cell shrank so far inside one pimd_step call that rc spans more than R cells: neighbours would be missed
-        for (int a = 0; a < 3; ++a)
-            if (g.rc * ginv_w[a] > (double)g.R[a]) atomicOr(g.overflow, 2);
+    if (ba == 0) {
+        const int ev = g.overflow[2] + 1;            // force evaluations since pimd_set_model, this one included
+        g.overflow[2] = ev;
+        if (g.boxp) {
+            // the cell shrank so far inside one pimd_step call that rc spans more than R cells: neighbours would be missed
+            for (int a = 0; a < 3; ++a)
+                if (g.rc * ginv_w[a] > (double)g.R[a]) {
+                    atomicOr(g.overflow, 2);
+                    atomicMin(reinterpret_cast<unsigned*>(g.overflow) + 1, (unsigned)ev);
+                }
+        }
     }
     int c[3];
 #pragma unroll
@@ -292,7 +299,8 @@ neighbor_env_kernel(int P, int N, GridGeom g, EnvConsts ec, const double* __rest
             }
             if (keep) {
                 if (slot >= sel_t) {
-                    atomicMax(overflow, 1);
+                    atomicOr(overflow, 1);
+                    atomicMin(reinterpret_cast<unsigned*>(overflow) + 1, (unsigned)overflow[2]);    // which evaluation
                 } else {
                     // queue the accepted candidate in its final slot: {j | image code, index into the cell-sorted
                     // positions}.  The FP64 environment arithmetic runs afterwards over the compact slots with all

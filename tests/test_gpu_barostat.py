@@ -264,9 +264,18 @@ def test_cell_grid_follows_a_shrinking_cell_across_calls(pk):
 
 
 def test_cell_shrinking_past_the_grid_margin_inside_one_call_is_an_error(pk):
+    """... and the failed call is undone as a whole (positions, momenta, cell, step counter), so the caller can go on
+    with fewer steps per call."""
     sim, wb, desc = _squeezed_config1(pk, 3)
-    with pytest.raises(pk.PimdError, match="cell shrank|more neighbours"):
+    x0, p0, b0 = sim.positions(), sim.momenta(), sim.barostat_state()
+    with pytest.raises(pk.PimdError, match="cell shrank|more neighbours") as ei:
         sim.step(400)
+    assert "rolled back" in str(ei.value)
+    b1 = sim.barostat_state()
+    assert np.array_equal(sim.positions(), x0) and np.array_equal(sim.momenta(), p0)
+    assert np.array_equal(b1["box"], b0["box"]) and b1["v_W"] == b0["v_W"] and sim.estimators()["step"] == 0
+    sim.step(2)
+    assert sim.estimators()["step"] == 2
     sim.close()
 
 

@@ -431,6 +431,58 @@ def test_sel_overflow_is_an_error(pk):
     sim.close()
 
 
+def test_sel_overflow_inside_a_call_rolls_the_call_back(pk):
+    """sel set to the largest neighbour counts of the initial configuration (32 O / 67 H): the oracle's trajectory
+    overflows at step 2 (atom 17 gains a 33rd O neighbour).  pimd_step(5) must report that step and undo the WHOLE
+    call -- not leave steps 3..5 integrated on truncated rows: x, p, f and the step counter are those at entry."""
+    cfg, wb, desc, w = workloads.make_config(0)
+    tight = dict(desc, sel=[32, 67])
+    args = (wb["types"], wb["masses"], wb["box"], cfg["P"], cfg["T"], cfg["dt"], cfg["gamma"])
+    orc = OraclePIMD(*args, seed=11)
+    orc.set_state(wb["x"], wb["p"])
+    orc.set_model(tight, w)
+    orc.step(1)
+    with pytest.raises(OverflowError):
+        orc.step(1)
+    sim = pk.PIMD(*args, seed=11, model_desc=tight)
+    sim.set_state(wb["x"], wb["p"])
+    sim.set_model(w, tight)
+    x0, p0, f0, U0 = sim.positions(), sim.momenta(), sim.forces(), sim.energies()
+    with pytest.raises(pk.PimdError, match="step 2 of this call of 5 = absolute step 2") as ei:
+        sim.step(5)
+    assert ei.value.code == pk.PIMD_ESEL_OVERFLOW
+    assert np.array_equal(sim.positions(), x0) and np.array_equal(sim.momenta(), p0)
+    assert np.array_equal(sim.forces(), f0) and np.array_equal(sim.energies(), U0)
+    assert sim.estimators()["step"] == 0
+    sim.step(1)                                           # step 1 is fine and follows the oracle
+    assert sim.estimators()["step"] == 1
+    assert _rel(sim.positions(), orc.positions()) <= 1e-10
+    x1 = sim.positions()
+    with pytest.raises(pk.PimdError, match="step 1 of this call of 1 = absolute step 2"):
+        sim.step(1)
+    assert np.array_equal(sim.positions(), x1) and sim.estimators()["step"] == 1
+    sim.close()
+
+
+def test_binding_refuses_device_tensors_of_the_wrong_kind(pk):
+    import torch
+    types, masses, x, p = _random_system(10, 4, seed=2)
+    sim = pk.PIMD(types, masses, [30.0] * 3, 4, 300.0, 1e-3, 1.0, seed=1)
+    xd, pd = torch.from_numpy(x).cuda(), torch.from_numpy(p).cuda()
+    with pytest.raises(ValueError, match="float64"):
+        sim.set_state(xd.float(), pd)
+    with pytest.raises(ValueError, match="contiguous"):
+        sim.set_state(xd.transpose(0, 1), pd)
+    with pytest.raises(ValueError, match="elements"):
+        sim.set_state(xd[:2], pd)
+    with pytest.raises(ValueError):
+        sim.set_state(x[:2], p)
+    sim.set_state(xd, pd)
+    sim.set_model_harmonic(1.0)
+    sim.step(1)
+    sim.close()
+
+
 # ---------------------------------------------------------------------------------------------
 # force model
 # ---------------------------------------------------------------------------------------------

@@ -174,8 +174,29 @@ def test_p_pr_from_cartesian_springs():
     e = integrator.estimators(x, np.zeros_like(x), np.zeros_like(x), np.zeros(P), masses, M, om, T)
     wP = nm.omega_P(P, T)
     dr = x - np.roll(x, -1, axis=0)
-    direct = (3 * P * N * KB * T - np.sum(masses[None, :, None] * wP * wP * dr * dr) * MVV2E) / (3 * V)
+    direct = (3 * P * N * KB * T - np.sum(masses[None, :, None] * wP * wP * dr * dr) * MVV2E / P) / (3 * V)
     assert barostat.p_pr(e["S_ring"], P, N, T, V) == pytest.approx(direct, rel=1e-12)
+    assert barostat.p_pr(e["S_ring"], P, N, T, V) == pytest.approx(2.0 * e["K_PR"] / (3 * V), rel=1e-12)   # A10 = (2/3V) A7
+
+
+def test_p_pr_of_the_free_ring_polymer_is_the_ideal_gas_pressure():
+    """Pin of the 1/n in A10 (DESIGN R-6 / R-25): normal-mode coordinates of a FREE ring polymer drawn from their exact
+    Gaussians at the ring temperature nT, <x~_k^2> = n k_B T / (m omega_k^2 mvv2e), give <S_ring> = 3N(n-1) n k_B T / 2,
+    hence <P_PR> = N k_B T / V.  Without the 1/n the mean would be -n(n-2) N k_B T / V."""
+    P, N, T, V = 16, 40, 300.0, 5000.0
+    rng = np.random.default_rng(2)
+    masses = rng.uniform(1.0, 16.0, N)
+    om = nm.omegas(P, T)
+    sig = np.zeros((P, N))
+    sig[1:] = np.sqrt(P * KB * T / (masses[None, :] * om[1:, None] ** 2 * MVV2E))
+    acc = []
+    for _ in range(400):
+        xt = sig[:, :, None] * rng.standard_normal((P, N, 3))
+        S = 0.5 * np.sum(masses[None, :, None] * om[:, None, None] ** 2 * xt * xt) * MVV2E
+        acc.append(barostat.p_pr(S, P, N, T, V))
+    ideal = N * KB * T / V
+    err = np.std(acc) / np.sqrt(len(acc))
+    assert abs(np.mean(acc) - ideal) < 4 * err and err < 0.1 * ideal
 
 
 def test_E7_keeps_the_barostat_temperature_and_uses_the_documented_normal():
