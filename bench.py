@@ -26,9 +26,21 @@ if ROOT not in sys.path:
 import workloads  # noqa: E402
 
 METRIC = "bead-atom-steps/s"
-# dram__bytes_read.sum + dram__bytes_write.sum per launch at configs[2], from the committed ncu --set full capture
-# (profiles/r1f_README.md); None where the phase is several kernels
-NCU_DRAM_BYTES = {"embed_fwd": 284.17e6 + 75.11e6, "embed_bwd": 309.36e6 + 11.71e6, "fitting": None}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch come from the committed `ncu --set full` capture of THIS build
+# (profiles/r2_dram_bytes.csv, written from the .ncu-rep as profiles/r2_README.md says); bench.py only reads the file.
+DRAM_CSV = os.path.join(ROOT, "profiles", "r2_dram_bytes.csv")
+PHASE_KERNEL = {"embed_fwd": "embed_fwd_tc_kernel", "embed_bwd": "embed_bwd_tc_kernel"}
+
+
+def ncu_dram_bytes(kernel, workload):
+    """(read + write bytes per launch, source) of `kernel` at `workload` from the committed capture, or (None, why)."""
+    if not os.path.exists(DRAM_CSV):
+        return None, "no capture committed"
+    import csv
+    for row in csv.DictReader(l for l in open(DRAM_CSV) if not l.startswith("#")):
+        if row["kernel"] == kernel and row["workload"] == workload:
+            return float(row["dram_read_bytes"]) + float(row["dram_write_bytes"]), os.path.relpath(DRAM_CSV, ROOT)
+    return None, "kernel not in " + os.path.relpath(DRAM_CSV, ROOT)
 
 
 def _peaks():
@@ -83,6 +95,39 @@ class ClockSampler:
                     reasons.add(n)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": smax, "reasons": sorted(reasons),
                 "samples": len(sm)}
+
+
+def measure_tf32_peak(seconds=2.0, n=8192):
+    """Dense TF32 tensor peak of this GPU, measured the way MEASURED_PEAKS.json measured BF16: torch.matmul (cuBLAS,
+    TF32 enabled) on n^3, best of 10 (burst) and back to back for `seconds` (sustained, under the power cap).  Used
+    only as the roofline denominator of the kind::tf32 kernels; runs outside every timed region."""
+    import torch
+    old = torch.backends.cuda.matmul.allow_tf32
+    torch.backends.cuda.matmul.allow_tf32 = True
+    try:
+        a = torch.randn(n, n, device="cuda", dtype=torch.float32)
+        b = torch.randn(n, n, device="cuda", dtype=torch.float32)
+        c = torch.empty_like(a)
+        for _ in range(3):
+            torch.matmul(a, b, out=c)
+        torch.cuda.synchronize()
+        best = 1e30
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for _ in range(10):
+            e0.record(); torch.matmul(a, b, out=c); e1.record(); torch.cuda.synchronize()
+            best = min(best, e0.elapsed_time(e1))
+        reps = max(10, int(seconds * 1e3 / best))
+        e0.record()
+        for _ in range(reps):
+            torch.matmul(a, b, out=c)
+        e1.record(); torch.cuda.synchronize()
+        sus = e0.elapsed_time(e1) / reps
+        fl = 2.0 * n ** 3 / 1e12
+        return {"tf32": fl / (best * 1e-3), "tf32_sustained": fl / (sus * 1e-3)}
+    finally:
+        torch.backends.cuda.matmul.allow_tf32 = old
+        del a, b, c
+        torch.cuda.empty_cache()
 
 
 def max_over_ranks(value, world, device):
@@ -169,13 +214,20 @@ def algorithmic_work(counts, N, P):
     """SURVEY 8(d) per-unit figures: useful flops of each force kernel per step."""
     rows = int(counts.sum())
     PN = N * P
-    emb_mac = 25 + 1250 + 5000                      # layers 1..3 per row
+    # tensor-eligible work exactly as SURVEY 8(d) counts it: 1250 + 5000 MAC per row and direction for the embedding
+    # net, 384,000 + 2 x 57,600 MAC per bead-atom and direction for the fitting net (203 Gflop per step at configs[2])
     flops = {
-        "embed_fwd": 2.0 * rows * (emb_mac + 400),                    # + G (x) R
-        "embed_bwd": 2.0 * rows * (emb_mac + 400 + 400 + 100),        # backward of the same + dG, dR, ds
-        "fitting": 2.0 * PN * 2 * (1600 * 240 + 2 * 240 * 240) + 2.0 * PN * (1600 * 4 + 2 * 1600 * 4),
+        "embed_fwd": 2.0 * rows * 6250,
+        "embed_bwd": 2.0 * rows * 6250,
+        "fitting": 2.0 * PN * 2 * (1600 * 240 + 2 * 240 * 240),
     }
-    return rows, flops
+    # "other arithmetic" of 8(d), NOT in any roofline fraction: layer 1, G (x) R and its two backward products, D, dT
+    other = {
+        "embed_fwd": 2.0 * rows * (25 + 400),
+        "embed_bwd": 2.0 * rows * (25 + 400 + 400 + 100),
+        "fitting": 2.0 * PN * (1600 * 4 + 2 * 1600 * 4),
+    }
+    return rows, flops, other
 
 
 def run_ours(args):
@@ -190,6 +242,8 @@ def run_ours(args):
     else:
         torch.cuda.set_device(0)
     peaks = _peaks()
+    if rank == 0 and not args.no_tf32_peak:
+        peaks.update(measure_tf32_peak())
 
     cfg, wb, desc, w = workloads.make_config(args.config)
     P, N = cfg["P"], wb["types"].size
@@ -221,8 +275,7 @@ def run_ours(args):
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     t_wall0 = time.time()
     ev0.record()
-    for _ in range(args.steps):
-        sim.step(1)
+    sim.step(args.steps)                            # ONE pimd_step(K) call: K whole steps, no host round trip inside
     ev1.record()
     barrier()
     t_wall1 = time.time()
@@ -238,7 +291,7 @@ def run_ours(args):
     phase = pk.pimd_get_phase_ms(sim.ctx)
     pk.pimd_set_profiling(sim.ctx, 0)
     counts = pk.pimd_get_neighbor_counts(sim.ctx, P, N, 2)
-    rows, flops = algorithmic_work(counts, N, P)
+    rows, flops, other = algorithmic_work(counts, N, P)
     names = ["integrator", "neighbour_env", "embed_fwd", "fitting", "embed_bwd"]
     phases = {n: float(phase[q]) for q, n in enumerate(names)}
     dom = max(("embed_fwd", "fitting", "embed_bwd"), key=lambda n: phases[n])
@@ -248,7 +301,7 @@ def run_ours(args):
     # dense = 1/2 of it (the guide's nominal ratio).
     PN = P * N
     f16_peak = peaks["bf16_sustained"] or peaks["bf16"]
-    tf32_peak = 0.5 * f16_peak
+    tf32_peak = peaks.get("tf32_sustained") or 0.5 * f16_peak      # measured in this run; else the guide's nominal 1/2
     mufu_peak = 148 * 16 * peaks["sm_max_mhz"] * 1e6 / 1e12                         # T MUFU op/s
     emb_issue = 2.0 * rows * 3 * (32 * 64 + 64 * 112)                               # K2 x N2 + K3 x N3 of embedding_tc.cu, 3 passes
     issued = {   # (flops issued on padded tiles incl. the 3 passes, peak of that dtype)
@@ -261,10 +314,12 @@ def run_ours(args):
     dom_peak = f16_peak
     achieved = flops[dom] / (phases[dom] * 1e-3) / 1e12
     dom_issued = sum(f for f, _ in issued[dom]) / (phases[dom] * 1e-3) / 1e12
+    traffic, traffic_src = ncu_dram_bytes(PHASE_KERNEL.get(dom, dom), cfg["name"])
     roofline = {"kernel": dom, "bound": "tensor", "achieved": achieved, "peak": dom_peak, "unit": "TFLOP/s",
-                "frac": achieved / dom_peak, "traffic": NCU_DRAM_BYTES.get(dom) if args.config == 2 else None,
-                "issued_tflops": dom_issued,
-                "note": "achieved = USEFUL flops (SURVEY 8(d): no recompute, no extra hi/lo passes, no padding) / live "
+                "frac": achieved / dom_peak, "traffic": traffic, "traffic_src": traffic_src,
+                "issued_tflops": dom_issued, "other_arithmetic_gflop": other[dom] / 1e9,
+                "note": "achieved = USEFUL tensor-eligible flops exactly as SURVEY 8(d) counts them (6250 MAC per row and "
+                        "direction: no recompute, no extra hi/lo passes, no padding, no 'other arithmetic') / live "
                         "CUDA-event time of the phase; peak = FP16 dense = %s BF16 %.0f TFLOP/s (kind::f16 runs at the "
                         "BF16 rate); issued_tflops counts the 3 passes on padded tiles" % (
                             "measured sustained" if peaks["bf16_sustained"] else "measured burst", f16_peak)}
@@ -281,6 +336,29 @@ def run_ours(args):
     kernels["integrator"] = {"ms": phases["integrator"], "algorithmic_GBs": 120.0 * P * N / (phases["integrator"] * 1e-3) / 1e9,
                              "note": "L2-resident at this size (5.9 MB/step); includes 3 memsets"}
     kernels["neighbour_env"] = {"ms": phases["neighbour_env"]}
+
+    # ---- sustained leg: back-to-back steps for seconds, with the clock record (the K-step region above is a burst) ----
+    sustained = None
+    if args.sustain_s > 0:
+        per = max(1, int(0.25 / (ms / args.steps * 1e-3)))                  # steps per call: ~0.25 s of device time
+        sampler2 = ClockSampler(local)
+        if rank == 0:
+            sampler2.start()
+            time.sleep(0.25)
+        barrier()
+        tw0 = time.time()
+        ev0.record()
+        n_sus = 0
+        while time.time() - tw0 < args.sustain_s:
+            sim.step(per)
+            n_sus += per
+        ev1.record()
+        barrier()
+        tw1 = time.time()
+        ms_sus = max_over_ranks(ev0.elapsed_time(ev1), world, "cuda")
+        sustained = {"value": job_throughput(P * N * n_sus, world, ms_sus), "unit": METRIC, "steps": n_sus,
+                     "seconds": ms_sus * 1e-3, "ms_per_step": ms_sus / n_sus,
+                     "clocks": sampler2.stop(tw0, tw1) if rank == 0 else None}
 
     # ---- integrator alone at HBM-bound size (stand-alone leg, harmonic model) ----
     integ = None
@@ -331,7 +409,7 @@ def run_ours(args):
                        "l2": "no flush: per-step working set (neighbour rows %.0f MB, T and dT %.0f MB, fitting activations ~%.0f MB)%s" % (
                            rows * 32 / 1e6, 2 * P * N * 1600 / 1e6, P * N * 7740 / 1e6,
                            " exceeds the 126 MB L2" if rows * 32 + P * N * 3200 > 126e6 else " -- fits the 126 MB L2: small-case config, not a bench line")},
-            "roofline": roofline, "kernels": kernels, "integrator_hbm": integ, "cpu_baseline": cpu,
+            "roofline": roofline, "kernels": kernels, "sustained": sustained, "integrator_hbm": integ, "cpu_baseline": cpu,
             "e2e": {"value": world * P * N / e2e_s, "unit": METRIC, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": e2e_s * 1e3, "call": "pimd_restore(host x,p,f,U) + pimd_step(1) + pimd_get_{positions,momenta,forces,energies,estimators}"},
             "gpu_launches": int(launches), "clocks": clocks, "peaks": peaks,
@@ -361,6 +439,8 @@ def integrator_leg(pk, peaks, n_atoms=1 << 20, P=32):
         sim.set_model_harmonic(1.0)
         sim.set_state(x, p)
         ms[name] = pk.pimd_time_kernel(sim.ctx, 0, 10)
+        if name == "pile_l":
+            ms["per_mode_keying"] = pk.pimd_time_kernel(sim.ctx, 1, 10)      # DESIGN R-10's A/B partner (timing only)
         sim.close()
     del x, p
     torch.cuda.empty_cache()
@@ -369,6 +449,10 @@ def integrator_leg(pk, peaks, n_atoms=1 << 20, P=32):
     return {"kernel": "integrator_kernel<32>", "bound": "hbm", "achieved": gbs, "peak": peaks["hbm"], "unit": "GB/s",
             "frac": gbs / peaks["hbm"], "ms": ms["pile_l"], "atoms": n_atoms, "beads": P, "bytes": nbytes,
             "nve": {"achieved": gbs_nve, "frac": gbs_nve / peaks["hbm"], "ms": ms["nve"]},
+            "r10_ab": {"pair_keying_ms": ms["pile_l"], "per_mode_keying_ms": ms["per_mode_keying"],
+                       "per_mode_frac": nbytes / (ms["per_mode_keying"] * 1e-3) / 1e9 / peaks["hbm"],
+                       "note": "same launch with one Philox draw per mode (counter word 3 = 4k+alpha, sine branch "
+                               "discarded: SURVEY C-7's first proposal) instead of one per mode pair (DESIGN R-10)"},
             "note": "stand-alone: closing B + estimators + B A O A + transforms; 'nve' = same launch at gamma = 0 "
                     "(no O-step normals): the gap is Philox + Box-Muller FP64 arithmetic, not memory"}
 
@@ -382,6 +466,9 @@ def main():
     ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json configs (default: the headline)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-integrator-leg", action="store_true")
+    ap.add_argument("--no-tf32-peak", action="store_true", help="skip the cuBLAS TF32 peak measurement (roofline denominator)")
+    ap.add_argument("--sustain-s", type=float, default=3.0,
+                    help="seconds of back-to-back steps for the sustained-rate leg (0 = skip)")
     ap.add_argument("--integrator-only", action="store_true",
                     help="only the stand-alone integrator leg (2^20 atoms x 32 beads, HBM-bound size); prints its JSON")
     args = ap.parse_args()

@@ -147,7 +147,7 @@ int pimd_set_state_dev(pimd_ctx* ctx, const double* x_dev, const double* p_dev);
 int pimd_get_positions_dev(pimd_ctx* ctx, double* x_dev);
 int pimd_get_forces_dev(pimd_ctx* ctx, double* f_dev);
 
-/* ---- parity hooks --------------------------------------------------------------------------- */
+/* ---- parity hooks (more of them, and the bench / bisecting switches, in pimd_debug.h) -------- */
 
 /* Neighbour rows of one bead from the most recent force evaluation, in canonical order: for atom i
  * the rows sorted by (type_j, j, n_x, n_y, n_z).  count[N] receives the rows per atom; j[cap] and
@@ -161,11 +161,6 @@ int pimd_get_neighbor_counts(pimd_ctx* ctx, int32_t* counts);
 
 /* Number of kernels of this library launched on the context so far (the bench's gpu_launches). */
 int64_t pimd_get_launch_count(const pimd_ctx* ctx);
-
-/* The four Philox4x32-10 words and the normal eta the O step uses for (step, mode k, atom i,
- * component alpha) (R-10), evaluated ON THE DEVICE for n entries: idx[n][3] = (k, i, alpha);
- * words[n][4], eta[n].  */
-int pimd_debug_noise(pimd_ctx* ctx, int64_t step, int n, const int32_t* idx, uint32_t* words, double* eta);
 
 /* Trotter splitting of the step ("integrator"): PIMD_BAOAB (default here; north_star's path) or
  * PIMD_OBABO (the fix's own default): O(dt/2) B(dt/2) A(dt) B(dt/2) O(dt/2), each O with c1 = exp(-gamma_k dt/2)
@@ -241,24 +236,6 @@ int pimd_get_barostat(pimd_ctx* ctx, pimd_barostat_state* b);
  * barostat companion of pimd_get_estimator_history; at most 4096 steps per call are recorded).  Returns the number
  * written (<= cap) or < 0. */
 int pimd_get_barostat_history(pimd_ctx* ctx, pimd_barostat_state* b, int cap);
-
-/* Fitting-net GEMM path: 1 (default) = tcgen05 tensor cores, 3xTF32 split (fitting_tc.cu); 0 = the FP32
- * CUDA-core GEMMs kept as the in-tree reference for bisecting.  Both meet the parity tolerances. */
-int pimd_set_fitting_path(pimd_ctx* ctx, int use_tensor_cores);
-
-/* Embedding-net path: 1 (default) = tcgen05 tensor cores, 3xTF32, row tiles of one type pair
- * (embedding_tc.cu); 0 = the FP32 CUDA-core kernels kept as the in-tree reference.  Takes effect at the
- * next force evaluation (pimd_set_state / pimd_step). */
-int pimd_set_embedding_path(pimd_ctx* ctx, int use_tensor_cores);
-
-/* Parity hook for the tensor-core GEMM kernel alone: C[M][N] = A[M][K] Bt[N][K]^T, host FP32 arrays,
- * N == 240 or N % 160 == 0, K % 16 == 0 (the shapes the fitting net uses). */
-int pimd_debug_gemm(pimd_ctx* ctx, int M, int N, int K, const float* A, const float* Bt, float* C);
-
-/* Stand-alone timing of kernels (bench.py roofline legs): runs `reps` launches of the fused
- * integrator kernel (kind 0) on the current state WITHOUT advancing it (output to scratch), and
- * returns the mean device time per launch in milliseconds through *ms. */
-int pimd_time_kernel(pimd_ctx* ctx, int kind, int reps, double* ms);
 
 /* Mean device milliseconds per step of each phase of the last pimd_step call, when profiling was
  * enabled with pimd_set_profiling(ctx, 1) (CUDA events on the context's stream):

@@ -8,6 +8,7 @@
 #include <string>
 #include <vector>
 #include "../../include/pimd.h"
+#include "../../include/pimd_debug.h"
 
 namespace pimd {
 

@@ -1,4 +1,5 @@
-// embedding_tc.cu -- F3 and F5/F6 of SURVEY 8(a) on the 5th-generation tensor cores (tcgen05 + TMEM).
+// embedding_tc.cu -- F3 and F5/F6 of SURVEY 8(a) on the 5th-generation tensor cores (tcgen05 kind::f16 + TMEM,
+// three-pass FP16-split products with FP32 accumulation).
 //
 // Neighbour rows are processed in tiles of 128 rows of ONE ordered type pair (t_i, t_j) -- one weight set,
 // resident in shared memory as ready-made UMMA B operands (FP16 hi / lo split, swizzled K-major, bias folded
