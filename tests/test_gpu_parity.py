@@ -442,6 +442,7 @@ def test_sel_overflow_inside_a_call_rolls_the_call_back(pk):
     orc.set_state(wb["x"], wb["p"])
     orc.set_model(tight, w)
     orc.step(1)
+    x1_oracle = orc.positions()
     with pytest.raises(OverflowError):
         orc.step(1)
     sim = pk.PIMD(*args, seed=11, model_desc=tight)
@@ -456,7 +457,7 @@ def test_sel_overflow_inside_a_call_rolls_the_call_back(pk):
     assert sim.estimators()["step"] == 0
     sim.step(1)                                           # step 1 is fine and follows the oracle
     assert sim.estimators()["step"] == 1
-    assert _rel(sim.positions(), orc.positions()) <= 1e-10
+    assert _rel(sim.positions(), x1_oracle) <= 1e-10
     x1 = sim.positions()
     with pytest.raises(pk.PimdError, match="step 1 of this call of 1 = absolute step 2"):
         sim.step(1)
