@@ -255,6 +255,9 @@ def run_ours(args):
     x_dev, p_dev = x_host.cuda(non_blocking=True), p_host.cuda(non_blocking=True)
     sim.set_model(w)
     sim.set_state(x_dev, p_dev)                     # inputs resident in HBM before the timed region
+    if args.compressed:
+        sim.set_compressed(True)
+        args.no_compressed_leg = True
     if "p_ext_bar" in cfg:                          # configs[4]: NpT, isotropic BZP barostat
         sim.set_barostat(cfg["p_ext_bar"], cfg["tau_p"])
 
@@ -360,6 +363,42 @@ def run_ours(args):
                      "seconds": ms_sus * 1e-3, "ms_per_step": ms_sus / n_sus,
                      "clocks": sampler2.stop(tw0, tw1) if rank == 0 else None}
 
+    # ---- the paper's own model variant: compressed (tabulated) embedding, SURVEY 8(f) NEXT-3 ----
+    compressed = None
+    if not args.no_compressed_leg:
+        sim.set_compressed(True)
+        for _ in range(3):
+            sim.step(1)
+        barrier()
+        ev0.record()
+        sim.step(args.steps)
+        ev1.record()
+        barrier()
+        ms_c = max_over_ranks(ev0.elapsed_time(ev1), world, "cuda")
+        pk.pimd_set_profiling(sim.ctx, 1)
+        sim.step(max(3, min(10, args.steps)))
+        ph_c = pk.pimd_get_phase_ms(sim.ctx)
+        pk.pimd_set_profiling(sim.ctx, 0)
+        sim.set_compressed(False)
+        # moments x table products as dense GEMMs: 480 x 100 x 4 MAC per bead-atom and direction
+        cmp_flops = 2.0 * PN * 480 * 100 * 4
+        compressed = {
+            "value": job_throughput(P * N * args.steps, world, ms_c), "unit": METRIC, "ms_per_step": ms_c / args.steps,
+            "speedup_vs_mlp_embedding": (ms / args.steps) / (ms_c / args.steps),
+            "phases_ms": {"integrator": float(ph_c[0]), "neighbour_env": float(ph_c[1]), "cmp_fwd": float(ph_c[2]),
+                          "fitting": float(ph_c[3]), "cmp_bwd": float(ph_c[4])},
+            "cmp_fwd": {"ms": float(ph_c[2]), "bound": "alu (FP32 moment accumulation: shared-memory read-modify-write chain); "
+                        "the 480x100x4 products per centre run on tcgen05 from tensor-memory-resident tables",
+                        "dense_tflops": cmp_flops / (float(ph_c[2]) * 1e-3) / 1e12,
+                        "row_rate_G_per_s": rows / (float(ph_c[2]) * 1e-3) / 1e9},
+            "cmp_bwd": {"ms": float(ph_c[4]), "bound": "latency (per tile: dT operand -> 4 M tiles of MMAs -> Q to shared memory -> rows)",
+                        "dense_tflops": cmp_flops / (float(ph_c[4]) * 1e-3) / 1e12,
+                        "row_rate_G_per_s": rows / (float(ph_c[4]) * 1e-3) / 1e9},
+            "note": "same workload with pimd_set_embedding_compressed(1): the model variant the paper's timings use "
+                    "(PAPER.md:L76); an approximation of the MLP model (DESIGN R-28), parity against the oracle's compressed "
+                    "model in tests/test_gpu_compress.py; the headline `value` above is the MLP path north_star names",
+        }
+
     # ---- integrator alone at HBM-bound size (stand-alone leg, harmonic model) ----
     integ = None
     if rank == 0 and not args.no_integrator_leg:
@@ -403,13 +442,14 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": METRIC, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f16-split (3-pass hi/lo, f32 accumulate) network ~ f32 / f64 geometry+integrator", "data": "synthetic",
-            "config": {"workload": cfg["name"], "atoms": N, "beads": P, "bead_atoms": P * N, "neighbour_rows": rows,
+            "config": {"workload": cfg["name"] + ("+compressed_embedding" if args.compressed else ""), "atoms": N, "beads": P, "bead_atoms": P * N, "neighbour_rows": rows,
                        "parallelism": "replicas only" if world > 1 else "1 GPU",
                        "ensemble": ("NpT %g bar, BZP barostat tau_p %g ps" % (cfg["p_ext_bar"], cfg["tau_p"])) if "p_ext_bar" in cfg else "NVT",
                        "l2": "no flush: per-step working set (neighbour rows %.0f MB, T and dT %.0f MB, fitting activations ~%.0f MB)%s" % (
                            rows * 32 / 1e6, 2 * P * N * 1600 / 1e6, P * N * 7740 / 1e6,
                            " exceeds the 126 MB L2" if rows * 32 + P * N * 3200 > 126e6 else " -- fits the 126 MB L2: small-case config, not a bench line")},
-            "roofline": roofline, "kernels": kernels, "sustained": sustained, "integrator_hbm": integ, "cpu_baseline": cpu,
+            "roofline": roofline, "kernels": kernels, "sustained": sustained, "compressed": compressed,
+            "integrator_hbm": integ, "cpu_baseline": cpu,
             "e2e": {"value": world * P * N / e2e_s, "unit": METRIC, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": e2e_s * 1e3, "call": "pimd_restore(host x,p,f,U) + pimd_step(1) + pimd_get_{positions,momenta,forces,energies,estimators}"},
             "gpu_launches": int(launches), "clocks": clocks, "peaks": peaks,
@@ -466,6 +506,9 @@ def main():
     ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json configs (default: the headline)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-integrator-leg", action="store_true")
+    ap.add_argument("--no-compressed-leg", action="store_true", help="skip the compressed-embedding leg (SURVEY 8(f) NEXT-3)")
+    ap.add_argument("--compressed", action="store_true",
+                    help="time the compressed-embedding model as the main line (config.workload says so)")
     ap.add_argument("--no-tf32-peak", action="store_true", help="skip the cuBLAS TF32 peak measurement (roofline denominator)")
     ap.add_argument("--sustain-s", type=float, default=3.0,
                     help="seconds of back-to-back steps for the sustained-rate leg (0 = skip)")

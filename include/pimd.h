@@ -41,6 +41,8 @@ extern "C" {
                                   * a state (the forces of a truncated neighbour list are not kept); set a new one. */
 #define PIMD_ECUDA          -5   /* CUDA runtime error; see pimd_last_error */
 #define PIMD_ENOMEM         -6   /* the caller-supplied workspace is too small */
+#define PIMD_ETABLE_RANGE   -7   /* compressed embedding: a neighbour row lies outside the table (s > 2, r < 0.5 A; R-28).
+                                  * Reported like PIMD_ESEL_OVERFLOW (pimd_step rolls the call back). */
 
 typedef struct pimd_ctx pimd_ctx;   /* opaque; owned by the library */
 
@@ -116,6 +118,17 @@ int pimd_restore(pimd_ctx* ctx, const double* x, const double* p, const double* 
  * n_weights must equal pimd_model_n_weights(d).  The library converts to FP32 on the device. */
 size_t pimd_model_n_weights(const pimd_model_desc* d);
 int pimd_set_model(pimd_ctx* ctx, const pimd_model_desc* d, const double* weights, size_t n_weights);
+
+/* Compressed ("tabulated") embedding net -- the model variant the paper's own runs use ("We use a
+ * compressed DP model", L262; ref. 41 is only cited, so DESIGN R-28 fixes the table: per ordered type pair, G(s) on the
+ * uniform grid s in [0, 2] with stride 0.05 is replaced by the quintic Hermite polynomial matching G, G', G'' at both
+ * nodes of each interval; the backward pass differentiates the same polynomial, so forces remain the exact gradient of
+ * the compressed energy).  on = 1 builds the tables from the weights given to pimd_set_model (FP64 on the host) and
+ * switches the embedding steps F3 / F5 to them; on = 0 returns to the MLP.  The forces of the current state are
+ * re-evaluated.  It is an APPROXIMATION of the MLP model (|G~ - G| <= 3e-8 at this stride) and is compared with the
+ * oracle's compressed model.  PIMD_ENOMODEL before pimd_set_model; PIMD_EINVAL for more than two atom types.
+ * A row with s > 2 (an atom pair closer than 0.5 A) is an error: PIMD_ETABLE_RANGE. */
+int pimd_set_embedding_compressed(pimd_ctx* ctx, int on);
 
 /* Test model: U = sum_i 1/2 k |r_i|^2 about the origin on the unwrapped coordinates (FP64), used to
  * check the integrator alone against closed forms (north_star's harmonic-oscillator check). */

@@ -59,8 +59,12 @@ class OraclePIMD:
         if self.model is not None or self.k_spring is not None:
             self._forces()
 
-    def set_model(self, desc, weights):
+    def set_model(self, desc, weights, compressed=False):
+        """compressed=True: the tabulated embedding net of oracle/compress.py (DESIGN R-28)."""
         self.model = se_e2_a.Model(desc, weights)
+        if compressed:
+            from . import compress
+            compress.compress(self.model)
         self.k_spring = None
         if self.x is not None:
             self._forces()

@@ -10,7 +10,7 @@ import os
 import numpy as np
 
 PIMD_OK, PIMD_EINVAL, PIMD_ENOSTATE, PIMD_ENOMODEL = 0, -1, -2, -3
-PIMD_ESEL_OVERFLOW, PIMD_ECUDA, PIMD_ENOMEM = -4, -5, -6
+PIMD_ESEL_OVERFLOW, PIMD_ECUDA, PIMD_ENOMEM, PIMD_ETABLE_RANGE = -4, -5, -6, -7
 PIMD_MAX_TYPES = 4
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -89,6 +89,7 @@ _SIGNATURES = {
     "pimd_get_barostat_history": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int]),
     "pimd_restore_cell": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "pimd_set_embedding_path": (C.c_int, [C.c_void_p, C.c_int]),
+    "pimd_set_embedding_compressed": (C.c_int, [C.c_void_p, C.c_int]),
     "pimd_debug_gemm": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]),
     "pimd_model_n_weights": (C.c_size_t, [C.c_void_p]),
     "pimd_set_model": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t]),
@@ -244,6 +245,10 @@ def pimd_set_fitting_path(ctx, use_tensor_cores):
 
 def pimd_set_embedding_path(ctx, use_tensor_cores):
     return _check(ctx, lib().pimd_set_embedding_path(ctx, int(bool(use_tensor_cores))))
+
+
+def pimd_set_embedding_compressed(ctx, on=True):
+    return _check(ctx, lib().pimd_set_embedding_compressed(ctx, int(bool(on))))
 
 
 def pimd_debug_gemm(ctx, A, Bt):
@@ -435,6 +440,9 @@ class PIMD:
         if desc is not None:
             self.desc = ModelDesc.from_dict(desc) if isinstance(desc, dict) else desc
         return pimd_set_model(self.ctx, self.desc, weights)
+
+    def set_compressed(self, on=True):
+        return pimd_set_embedding_compressed(self.ctx, on)
 
     def set_model_harmonic(self, k):
         return pimd_set_model_harmonic(self.ctx, k)

@@ -68,6 +68,7 @@ struct pimd_ctx {
     int64_t est_hist_first_step = 0;
     ModeConsts mc;
     Model model;
+    std::vector<double> emb_w_host;   // embedding weights as passed to pimd_set_model (the tables are built from them)
 
     // profiling
     bool profiling = false;
@@ -158,6 +159,7 @@ size_t model_bytes(const pimd_ctx* c, const pimd_model_desc* d) {
     b += align_up((size_t)d->n_types * d->n_types * emb_tc_image_h_bytes(), 256);
     b += align_up((size_t)d->n_types * (PN + 1) * 4, 256) + align_up(PN * nsel * 4, 256);
     b += align_up((size_t)d->n_types * ((PN + 1023) / 1024) * 4, 256) + align_up(PN * 72, 256);
+    b += align_up(cmp_image_words_fw(d->n_types) * 4, 256) + align_up(cmp_image_words_bw(d->n_types) * 4, 256);
     return b + 65536;
 }
 
@@ -243,6 +245,17 @@ int eval_forces(pimd_ctx* ctx) {
     rec(ctx, 1);
     ctx->evals_launched += 1;
     ctx->launches += neighbor_build(ctx->model, a, ctx->stream);
+    if (ctx->model.compressed) {
+        // tabulated embedding (NEXT-3): moments x table in tensor memory; no compact row index needed
+        rec(ctx, 2);
+        ctx->launches += compressed_forward(ctx->model, a, ctx->n_sms, ctx->stream);
+        rec(ctx, 3);
+        ctx->launches += fitting_forward_backward(ctx->model, a, ctx->stream);
+        rec(ctx, 4);
+        ctx->launches += compressed_backward(ctx->model, a, ctx->n_sms, ctx->stream);
+        rec(ctx, 5);
+        return PIMD_OK;
+    }
     const bool tc_emb = ctx->model.use_tc_emb && ctx->model.tc_emb_ready;
     if (tc_emb) ctx->launches += emb_tc_row_index(ctx->model, a, ctx->stream);
     rec(ctx, 2);
@@ -326,6 +339,8 @@ int check_overflow(pimd_ctx* ctx, int64_t* failed_eval = nullptr) {
         cudaMemcpyAsync(ctx->model.overflow, reset, sizeof(reset), cudaMemcpyHostToDevice, ctx->stream);
         cudaStreamSynchronize(ctx->stream);
         if (failed_eval) *failed_eval = (int64_t)flag[1] - 1;
+        if (flag[0] & 4u)
+            return fail(ctx, PIMD_ETABLE_RANGE, "a neighbour row lies outside the compression table (s > 2, i.e. r < 0.5 A; DESIGN R-28)");
         if (flag[0] & 2u)
             return fail(ctx, PIMD_ESEL_OVERFLOW, "the cell shrank past the cell-grid margin inside one pimd_step call; use fewer steps per call");
         return fail(ctx, PIMD_ESEL_OVERFLOW, "an atom has more neighbours of one type than sel allows");
@@ -688,6 +703,7 @@ int pimd_set_model(pimd_ctx* ctx, const pimd_model_desc* d, const double* w, siz
             for (int n = 0; n < M1; ++n) o[ob3 + n] = (float)w[pos + n];
             pos += M1;
         }
+    ctx->emb_w_host.assign(w, w + pos);          // the embedding part of the weight vector (all ordered pairs)
     if ((rc = arena_alloc(ctx, &m.emb_w, ew.size()))) return rc;
     CK(cudaMemcpyAsync(m.emb_w, ew.data(), ew.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
     std::vector<uint8_t> img_h((size_t)nt * nt * emb_tc_image_h_bytes());
@@ -808,6 +824,26 @@ int pimd_set_model(pimd_ctx* ctx, const pimd_model_desc* d, const double* w, siz
     return refresh(ctx);
 }
 
+int pimd_set_embedding_compressed(pimd_ctx* ctx, int on) {
+    if (!ctx) return PIMD_EINVAL;
+    if (!ctx->model.set) return fail(ctx, PIMD_ENOMODEL, "set the se_e2_a model first: the tables are built from its weights");
+    Model& m = ctx->model;
+    if (on && ctx->ntypes > 2)
+        return fail(ctx, PIMD_EINVAL, "the tensor-memory resident tables hold two neighbour types (2 x 40 intervals x 6 coefficients)");
+    if (on && !m.cmp_img_fw) {
+        int rc;
+        std::vector<uint32_t> fw(cmp_image_words_fw(ctx->ntypes)), bw(cmp_image_words_bw(ctx->ntypes));
+        cmp_build_images(ctx->emb_w_host.data(), ctx->ntypes, fw.data(), bw.data());     // FP64 on the host -> FP16 hi / lo
+        if ((rc = arena_alloc(ctx, &m.cmp_img_fw, fw.size()))) return rc;
+        if ((rc = arena_alloc(ctx, &m.cmp_img_bw, bw.size()))) return rc;
+        CK(cudaMemcpyAsync(m.cmp_img_fw, fw.data(), fw.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
+        CK(cudaMemcpyAsync(m.cmp_img_bw, bw.data(), bw.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
+        CK(cudaStreamSynchronize(ctx->stream));
+    }
+    m.compressed = on != 0;
+    return refresh(ctx);
+}
+
 int pimd_step(pimd_ctx* ctx, int64_t n_steps) {
     if (!ctx) return PIMD_EINVAL;
     if (n_steps < 0) return fail(ctx, PIMD_EINVAL, "n_steps < 0");
@@ -896,7 +932,7 @@ int pimd_step(pimd_ctx* ctx, int64_t n_steps) {
             }
             CK(cudaStreamSynchronize(ctx->stream));
             ctx->est_hist_n = 0;
-            char where[160];
+            char where[256];
             snprintf(where, sizeof(where), " (first at step %lld of this call of %lld = absolute step %lld); the state has been "
                      "rolled back to the start of the call",
                      (long long)(failed_eval - evals0 + 1), (long long)n_steps, (long long)(ctx->step + failed_eval - evals0 + 1));

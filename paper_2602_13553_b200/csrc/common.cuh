@@ -168,6 +168,10 @@ struct Model {
     int*     rowaddr = nullptr;        // [PN*nsel] compact row -> slot index
     int*     row_bsum = nullptr;       // [ntypes][ceil(PN/1024)] scan block sums
     double*  cpart = nullptr;          // [PN][9] per-centre virial share
+    // compressed (tabulated) embedding, SURVEY 8(f) NEXT-3 (compress_tc.cu)
+    bool     compressed = false;
+    uint32_t* cmp_img_fw = nullptr;    // tensor-memory images of the tables: forward A operand per centre type
+    uint32_t* cmp_img_bw = nullptr;    // backward A operand (four M tiles) per centre type
 };
 
 struct ForceArgs {
@@ -197,5 +201,10 @@ int emb_tc_row_index(Model& m, const ForceArgs& a, cudaStream_t s);
 int embedding_forward_tc(Model& m, const ForceArgs& a, int n_sms, cudaStream_t s);
 int embedding_backward_tc(Model& m, const ForceArgs& a, int n_sms, cudaStream_t s);
 int debug_tc_gemm(int M, int N, int K, const float* A_dev, const float* Bt_dev, float* C_dev, cudaStream_t s);
+size_t cmp_image_words_fw(int ntypes);
+size_t cmp_image_words_bw(int ntypes);
+void cmp_build_images(const double* w_emb, int ntypes, uint32_t* img_fw, uint32_t* img_bw);
+int compressed_forward(Model& m, const ForceArgs& a, int n_sms, cudaStream_t s);
+int compressed_backward(Model& m, const ForceArgs& a, int n_sms, cudaStream_t s);
 
 }  // namespace pimd

@@ -46,7 +46,7 @@ class ParallelOraclePIMD(OraclePIMD):
         self.close()
         self._pool = mp.get_context("spawn").Pool(self._workers, initializer=_init,
                                                   initargs=(desc, np.asarray(weights), self.types, compressed))
-        super().set_model(desc, weights)
+        super().set_model(desc, weights, compressed=compressed)
 
     def _forces(self):
         if self._pool is None or self.k_spring is not None:
