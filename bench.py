@@ -366,17 +366,42 @@ def run_ours(args):
     # ---- the paper's own model variant: compressed (tabulated) embedding, SURVEY 8(f) NEXT-3 ----
     compressed = None
     if not args.no_compressed_leg:
+        # Fresh state: the synthetic workload has no binding potential (random-init weights), so after the ~10^3 steps of
+        # the legs above atoms have drifted through each other and some pair sits closer than 0.5 A -- outside the
+        # table, which R-28 makes an error (PIMD_ETABLE_RANGE; pimd_step rolls the call back).  The leg therefore starts
+        # from the initial configuration again and halves its step count if a ring polymer still reaches r < 0.5 A.
+        sim.set_state(x_dev, p_dev)
         sim.set_compressed(True)
-        for _ in range(3):
-            sim.step(1)
+
+        def guarded(n):
+            while n >= 1:
+                try:
+                    sim.step(n)
+                    return n
+                except pk.PimdError as e:
+                    if e.code != pk.PIMD_ETABLE_RANGE:
+                        raise
+                    n //= 2
+            return 0
+
+        guarded(3)
         barrier()
         ev0.record()
-        sim.step(args.steps)
+        k_c = guarded(args.steps)
         ev1.record()
         barrier()
-        ms_c = max_over_ranks(ev0.elapsed_time(ev1), world, "cuda")
+        # a retry leaves the failed (rolled-back) attempt inside the event pair: time the successful count again, cleanly
+        if k_c != args.steps and k_c > 0:
+            sim.set_state(x_dev, p_dev)
+            barrier()
+            ev0.record()
+            k_c = guarded(k_c)
+            ev1.record()
+            barrier()
+        ms_c = max_over_ranks(ev0.elapsed_time(ev1), world, "cuda") * (args.steps / max(k_c, 1))
+        sim.set_state(x_dev, p_dev)
         pk.pimd_set_profiling(sim.ctx, 1)
-        sim.step(max(3, min(10, args.steps)))
+        guarded(3)
         ph_c = pk.pimd_get_phase_ms(sim.ctx)
         pk.pimd_set_profiling(sim.ctx, 0)
         sim.set_compressed(False)
@@ -384,6 +409,7 @@ def run_ours(args):
         cmp_flops = 2.0 * PN * 480 * 100 * 4
         compressed = {
             "value": job_throughput(P * N * args.steps, world, ms_c), "unit": METRIC, "ms_per_step": ms_c / args.steps,
+            "steps_timed": k_c,
             "speedup_vs_mlp_embedding": (ms / args.steps) / (ms_c / args.steps),
             "phases_ms": {"integrator": float(ph_c[0]), "neighbour_env": float(ph_c[1]), "cmp_fwd": float(ph_c[2]),
                           "fitting": float(ph_c[3]), "cmp_bwd": float(ph_c[4])},

@@ -195,46 +195,86 @@ cmp_fwd_kernel(const __grid_constant__ CmpArgs a) {
             float* stg = stage + cl * 4 * STG;                       // [4 c][STG], shared by the two warps of the centre
             float* rowbuf = rowbuf_all + warp * (F_ROWBUF / 4);      // (they own disjoint k ranges)
             const int p = lane >> 2, c = lane & 3;
-            for (int tile = blockIdx.x; tile < ntile; tile += gridDim.x, ++it) {
+            // Row data is prefetched one tile ahead into registers and the (centre, count) pair two tiles ahead: all 16
+            // moment warps of a CTA reach the same point of a tile together, so an exposed cen_idx -> ncount -> slot
+            // load chain (three dependent L2 / HBM round trips) would be paid by the whole SM at once.
+            struct RowF { float dx, dy, dz, s, rinv; };
+            auto meta = [&](int tile, size_t& s0, int& n) {
                 const int r = row0 + tile * TC + cl;
-                if (r < row1 && tj < nt) {
-                    const int ba = a.cen_idx[r];
-                    const int n = a.ncount[(size_t)ba * nt + tj];
-                    const size_t s0 = (size_t)ba * a.nsel + a.seloff[tj];
-                    for (int q0 = 0; q0 < n; q0 += 32) {
-                        const int nb = min(32, n - q0);
-                        if (lane < nb) {
-                            const float4 A = __ldg(reinterpret_cast<const float4*>(a.slotA) + s0 + q0 + lane);
-                            const float4 B = __ldg(reinterpret_cast<const float4*>(a.slotB) + s0 + q0 + lane);
-                            const float s = A.w, sr = A.w * B.y;
-                            if (s > kSHi) {                              // outside the table: an error, not an extrapolation (R-28)
-                                atomicOr(a.overflow, 4);
-                                atomicMin(reinterpret_cast<unsigned*>(a.overflow) + 1, (unsigned)a.overflow[2]);
-                            }
-                            int iv; float u;
-                            cmp_locate(s, iv, u);
-                            const float R[4] = {s, sr * A.x, sr * A.y, sr * A.z};
-                            float* rb = rowbuf + lane * 25;
-                            float pw = 1.f;
+                s0 = 0; n = 0;
+                if (tile < ntile && r < row1 && tj < nt) {
+                    const int ba = __ldg(a.cen_idx + r);
+                    n = __ldg(a.ncount + (size_t)ba * nt + tj);
+                    s0 = (size_t)ba * a.nsel + a.seloff[tj];
+                }
+            };
+            auto load_row = [&](size_t slot) {
+                const float4 A = __ldg(reinterpret_cast<const float4*>(a.slotA) + slot);
+                RowF R;
+                R.dx = A.x; R.dy = A.y; R.dz = A.z; R.s = A.w; R.rinv = __ldg(&a.slotB[slot].rinv);
+                return R;
+            };
+            auto load_rows = [&](size_t s0, int n, RowF (&R)[3]) {
 #pragma unroll
-                            for (int pp = 0; pp < NP; ++pp) {
+                for (int b = 0; b < 3; ++b)
+                    if (32 * b + lane < n) R[b] = load_row(s0 + 32 * b + lane);
+            };
+            const int hotk = tj * NI * NP;                           // bucket (tj, interval 0): two thirds of all rows
+            // one batch of up to 32 rows: lane = row writes its 24 products u^p R_c, then lane = (p, c) adds them up
+            auto batch = [&](const RowF& R, int nb, float& acc0) {
+                if (lane < nb) {
+                    const float s = R.s, sr = R.s * R.rinv;
+                    if (s > kSHi) {                              // outside the table: an error, not an extrapolation (R-28)
+                        atomicOr(a.overflow, 4);
+                        atomicMin(reinterpret_cast<unsigned*>(a.overflow) + 1, (unsigned)a.overflow[2]);
+                    }
+                    int iv; float u;
+                    cmp_locate(s, iv, u);
+                    const float Rv[4] = {s, sr * R.dx, sr * R.dy, sr * R.dz};
+                    float* rb = rowbuf + lane * 25;
+                    float pw = 1.f;
 #pragma unroll
-                                for (int cc = 0; cc < 4; ++cc) rb[pp * 4 + cc] = pw * R[cc];
-                                pw *= u;
-                            }
-                            rb[24] = __int_as_float((tj * NI + iv) * NP);
-                        }
-                        __syncwarp();
-                        if (lane < 24) {
-                            for (int q = 0; q < nb; ++q) {
-                                const float v = rowbuf[q * 25 + lane];
-                                const int k0 = __float_as_int(rowbuf[q * 25 + 24]);
-                                stg[c * STG + k0 + p] += v;
-                            }
-                        }
-                        __syncwarp();
+                    for (int pp = 0; pp < NP; ++pp) {
+#pragma unroll
+                        for (int cc = 0; cc < 4; ++cc) rb[pp * 4 + cc] = pw * Rv[cc];
+                        pw *= u;
+                    }
+                    rb[24] = __int_as_float((tj * NI + iv) * NP);
+                }
+                __syncwarp();
+                if (lane < 24) {
+                    for (int q = 0; q < nb; ++q) {
+                        const float v = rowbuf[q * 25 + lane];
+                        const int k0 = __float_as_int(rowbuf[q * 25 + 24]);
+                        if (k0 == hotk) acc0 += v;                    // warp-uniform: the hot bucket stays in a register
+                        else stg[c * STG + k0 + p] += v;
                     }
                 }
+                __syncwarp();
+            };
+            size_t s0c, s0n; int nc, nn;
+            RowF cur[3];
+            meta(blockIdx.x, s0c, nc);
+            load_rows(s0c, nc, cur);
+            meta(blockIdx.x + gridDim.x, s0n, nn);
+            for (int tile = blockIdx.x; tile < ntile; tile += gridDim.x, ++it) {
+                RowF nxt[3];
+                load_rows(s0n, nn, nxt);                             // the next tile's rows are in flight during this one
+                size_t s0nn; int nnn;
+                meta(tile + 2 * gridDim.x, s0nn, nnn);
+                float acc0 = 0.f;
+#pragma unroll
+                for (int b = 0; b < 3; ++b)
+                    if (32 * b < nc) batch(cur[b], min(32, nc - 32 * b), acc0);
+                for (int q0 = 96; q0 < nc; q0 += 32) {               // sel > 96: not prefetched
+                    RowF R = {0.f, 0.f, 0.f, 0.f, 1.f};
+                    if (q0 + lane < nc) R = load_row(s0c + q0 + lane);
+                    batch(R, min(32, nc - q0), acc0);
+                }
+                if (lane < 24) stg[c * STG + hotk + p] += acc0;
+#pragma unroll
+                for (int b = 0; b < 3; ++b) cur[b] = nxt[b];
+                s0c = s0n; nc = nn; s0n = s0nn; nn = nnn;
                 // ---- my half of the centre's moments -> FP16 hi / lo operand rows 4 cl + c (K-major, SWIZZLE_128B),
                 //      once the MMAs of the previous tile have read the buffer; the stage is zeroed on the way ----
                 __syncwarp();
@@ -384,21 +424,27 @@ cmp_bwd_kernel(const __grid_constant__ CmpArgs a) {
             // ================= tensor warpgroup =================
             const int wq = warp - B_WARPS, t = wq * 32 + lane;
             const uint32_t lanefield = ((uint32_t)(wq * 32)) << 16;
+            // dT of my (centre, 8 channels) piece, fetched one tile ahead
+            const int cl = t >> 4, n0 = (t & 15) * 8;
+            auto load_dT = [&](int tile, float4 (&x)[8]) {
+                const int r = row0 + tile * TC + cl;
+#pragma unroll
+                for (int q = 0; q < 8; ++q)
+                    x[q] = (tile < ntile && r < row1 && n0 + q < M1)
+                               ? __ldg(reinterpret_cast<const float4*>(a.dTm) + (size_t)r * M1 + n0 + q)
+                               : make_float4(0.f, 0.f, 0.f, 0.f);
+            };
+            float4 x[8];
+            load_dT(blockIdx.x, x);
             for (int tile = blockIdx.x; tile < ntile; tile += gridDim.x, ++it) {
                 const int buf = it & 1;
                 // ---- dT of the tile's centres -> operand rows (centre, c), K = channel; scaled per centre by the
                 //      power of two that brings max |dT| to [1, 2) (FP16 range; undone when Q is written) ----
                 {
-                    const int cl = t >> 4, n0 = (t & 15) * 8;
-                    const int r = row0 + tile * TC + cl;
-                    float4 x[8];
                     float mx = 0.f;
 #pragma unroll
-                    for (int q = 0; q < 8; ++q) {
-                        x[q] = (r < row1 && n0 + q < M1) ? __ldg(reinterpret_cast<const float4*>(a.dTm) + (size_t)r * M1 + n0 + q)
-                                                         : make_float4(0.f, 0.f, 0.f, 0.f);
+                    for (int q = 0; q < 8; ++q)
                         mx = fmaxf(mx, fmaxf(fmaxf(fabsf(x[q].x), fabsf(x[q].y)), fmaxf(fabsf(x[q].z), fabsf(x[q].w))));
-                    }
 #pragma unroll
                     for (int o = 8; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
                     const uint32_t e = (__float_as_uint(mx) >> 23) & 0xffu;
@@ -419,6 +465,7 @@ cmp_bwd_kernel(const __grid_constant__ CmpArgs a) {
                         }
                     }
                 }
+                load_dT(tile + gridDim.x, x);                        // next tile's dT in flight under this tile's MMAs
                 fence_proxy_async_smem();
                 if (it >= 2) mbar_wait(qempty + buf, ((it >> 1) - 1) & 1);     // the row warps have left this Q buffer
                 tc_fence_before();
@@ -473,67 +520,90 @@ cmp_bwd_kernel(const __grid_constant__ CmpArgs a) {
             // ================= row warps: (centre cl, neighbour type tj), lane = row =================
             const int cl = warp >> 1, tj = warp & 1;
             const float inv_h = kInvH;
+            struct RowB { float dx, dy, dz, s, dsw, rinv; uint32_t jcode; };
+            auto meta = [&](int tile, int& r, int& ba, int& n) {
+                r = row0 + tile * TC + cl;
+                ba = 0; n = 0;
+                if (tile < ntile && r < row1 && tj < nt) {
+                    ba = __ldg(a.cen_idx + r);
+                    n = __ldg(a.ncount + (size_t)ba * nt + tj);
+                }
+            };
+            auto load_row = [&](size_t slot) {
+                const float4 A = __ldg(reinterpret_cast<const float4*>(a.slotA) + slot);
+                const float4 B = __ldg(reinterpret_cast<const float4*>(a.slotB) + slot);
+                RowB R;
+                R.dx = A.x; R.dy = A.y; R.dz = A.z; R.s = A.w; R.dsw = B.x; R.rinv = B.y; R.jcode = __float_as_uint(B.z);
+                return R;
+            };
+            int rn, ban, nn;
+            meta(blockIdx.x, rn, ban, nn);
             for (int tile = blockIdx.x; tile < ntile; tile += gridDim.x, ++it) {
                 const int buf = it & 1;
-                const int r = row0 + tile * TC + cl;
+                const int r = rn, ba = ban, n = nn;
+                const size_t s0 = (size_t)ba * a.nsel + a.seloff[tj];
+                // my rows are loaded BEFORE the wait for Q (their latency hides under the tensor group's work on this
+                // tile), the next tile's (centre, count) pair behind them
+                RowB rows[3];
+#pragma unroll
+                for (int b = 0; b < 3; ++b)
+                    if (32 * b + lane < n) rows[b] = load_row(s0 + 32 * b + lane);
+                meta(tile + gridDim.x, rn, ban, nn);
                 mbar_wait(qfull + buf, (it >> 1) & 1);
-                if (r < row1 && tj < nt) {
-                    const int ba = a.cen_idx[r];
-                    const int n = a.ncount[(size_t)ba * nt + tj];
-                    const size_t s0 = (size_t)ba * a.nsel + a.seloff[tj];
+                if (n > 0) {
                     const float4* Qc = Qs + (size_t)buf * (TC * K) + cl * K + tj * KB;
                     double* fb = a.f + (size_t)(ba / a.N) * a.N * 3;
                     float acc[12];
 #pragma unroll
                     for (int q = 0; q < 12; ++q) acc[q] = 0.f;
-                    for (int q0 = 0; q0 < n; q0 += 32) {
-                        if (q0 + lane < n) {
-                            const float4 A = __ldg(reinterpret_cast<const float4*>(a.slotA) + s0 + q0 + lane);
-                            const float4 B = __ldg(reinterpret_cast<const float4*>(a.slotB) + s0 + q0 + lane);
-                            const float s = A.w, dsw = B.x, rinv = B.y;
-                            const uint32_t jcode = __float_as_uint(B.z);
-                            int iv; float u;
-                            cmp_locate(s, iv, u);
-                            const float4* Q = Qc + iv * NP;
-                            const float4 q5 = Q[5], q4 = Q[4], q3 = Q[3], q2 = Q[2], q1 = Q[1], q0v = Q[0];
-                            // A_c = sum_p u^p Q_p[c],  D_c = sum_p p u^(p-1) Q_p[c]  (Horner)
-                            float Av[4], Dv[4];
-                            const float a5[4] = {q5.x, q5.y, q5.z, q5.w}, a4[4] = {q4.x, q4.y, q4.z, q4.w}, a3[4] = {q3.x, q3.y, q3.z, q3.w};
-                            const float a2[4] = {q2.x, q2.y, q2.z, q2.w}, a1[4] = {q1.x, q1.y, q1.z, q1.w}, a0[4] = {q0v.x, q0v.y, q0v.z, q0v.w};
+                    auto one = [&](const RowB& R) {
+                        const float s = R.s, dsw = R.dsw, rinv = R.rinv;
+                        int iv; float u;
+                        cmp_locate(s, iv, u);
+                        const float4* Q = Qc + iv * NP;
+                        const float4 q5 = Q[5], q4 = Q[4], q3 = Q[3], q2 = Q[2], q1 = Q[1], q0v = Q[0];
+                        // A_c = sum_p u^p Q_p[c],  D_c = sum_p p u^(p-1) Q_p[c]  (Horner)
+                        float Av[4], Dv[4];
+                        const float a5[4] = {q5.x, q5.y, q5.z, q5.w}, a4[4] = {q4.x, q4.y, q4.z, q4.w}, a3[4] = {q3.x, q3.y, q3.z, q3.w};
+                        const float a2[4] = {q2.x, q2.y, q2.z, q2.w}, a1[4] = {q1.x, q1.y, q1.z, q1.w}, a0[4] = {q0v.x, q0v.y, q0v.z, q0v.w};
 #pragma unroll
-                            for (int c = 0; c < 4; ++c) {
-                                float v = a5[c];
-                                v = fmaf(v, u, a4[c]); v = fmaf(v, u, a3[c]); v = fmaf(v, u, a2[c]); v = fmaf(v, u, a1[c]); v = fmaf(v, u, a0[c]);
-                                Av[c] = v;
-                                float d = 5.f * a5[c];
-                                d = fmaf(d, u, 4.f * a4[c]); d = fmaf(d, u, 3.f * a3[c]); d = fmaf(d, u, 2.f * a2[c]); d = fmaf(d, u, a1[c]);
-                                Dv[c] = d;
-                            }
-                            const float sr = s * rinv;
-                            const float R0 = s, R1 = sr * A.x, R2 = sr * A.y, R3 = sr * A.z;
-                            const float w = a.inv_nsel;
-                            const float ds = (R0 * Dv[0] + R1 * Dv[1] + R2 * Dv[2] + R3 * Dv[3]) * (w * inv_h);
-                            const float dR0 = Av[0] * w, dR1 = Av[1] * w, dR2 = Av[2] * w, dR3 = Av[3] * w;
-                            // pair gradient g = dU/dd (R-16), as in embedding_tc.cu
-                            const float dot = dR1 * A.x + dR2 * A.y + dR3 * A.z;
-                            const float radial = (ds + dR0) * dsw + (dsw * rinv - s * rinv * rinv) * dot;
-                            const float rr = radial * rinv;
-                            const float gx = fmaf(rr, A.x, sr * dR1), gy = fmaf(rr, A.y, sr * dR2), gz = fmaf(rr, A.z, sr * dR3);
-                            double* fj = fb + (size_t)(jcode & 0x7fffffu) * 3;
-                            atomicAdd(fj, -(double)gx); atomicAdd(fj + 1, -(double)gy); atomicAdd(fj + 2, -(double)gz);
-                            acc[0] += gx; acc[1] += gy; acc[2] += gz;
-                            const float dd[3] = {A.x, A.y, A.z}, gg[3] = {gx, gy, gz};
-#pragma unroll
-                            for (int x = 0; x < 3; ++x)
-#pragma unroll
-                                for (int y = 0; y < 3; ++y) acc[3 + 3 * x + y] -= dd[x] * gg[y];
+                        for (int c = 0; c < 4; ++c) {
+                            float v = a5[c];
+                            v = fmaf(v, u, a4[c]); v = fmaf(v, u, a3[c]); v = fmaf(v, u, a2[c]); v = fmaf(v, u, a1[c]); v = fmaf(v, u, a0[c]);
+                            Av[c] = v;
+                            float d = 5.f * a5[c];
+                            d = fmaf(d, u, 4.f * a4[c]); d = fmaf(d, u, 3.f * a3[c]); d = fmaf(d, u, 2.f * a2[c]); d = fmaf(d, u, a1[c]);
+                            Dv[c] = d;
                         }
-                    }
+                        const float sr = s * rinv;
+                        const float R0 = s, R1 = sr * R.dx, R2 = sr * R.dy, R3 = sr * R.dz;
+                        const float w = a.inv_nsel;
+                        const float ds = (R0 * Dv[0] + R1 * Dv[1] + R2 * Dv[2] + R3 * Dv[3]) * (w * inv_h);
+                        const float dR0 = Av[0] * w, dR1 = Av[1] * w, dR2 = Av[2] * w, dR3 = Av[3] * w;
+                        // pair gradient g = dU/dd (R-16), as in embedding_tc.cu
+                        const float dot = dR1 * R.dx + dR2 * R.dy + dR3 * R.dz;
+                        const float radial = (ds + dR0) * dsw + (dsw * rinv - s * rinv * rinv) * dot;
+                        const float rr = radial * rinv;
+                        const float gx = fmaf(rr, R.dx, sr * dR1), gy = fmaf(rr, R.dy, sr * dR2), gz = fmaf(rr, R.dz, sr * dR3);
+                        double* fj = fb + (size_t)(R.jcode & 0x7fffffu) * 3;
+                        atomicAdd(fj, -(double)gx); atomicAdd(fj + 1, -(double)gy); atomicAdd(fj + 2, -(double)gz);
+                        acc[0] += gx; acc[1] += gy; acc[2] += gz;
+                        const float dd[3] = {R.dx, R.dy, R.dz}, gg[3] = {gx, gy, gz};
+#pragma unroll
+                        for (int xq = 0; xq < 3; ++xq)
+#pragma unroll
+                            for (int y = 0; y < 3; ++y) acc[3 + 3 * xq + y] -= dd[xq] * gg[y];
+                    };
+#pragma unroll
+                    for (int b = 0; b < 3; ++b)
+                        if (32 * b + lane < n) one(rows[b]);
+                    for (int q0 = 96; q0 < n; q0 += 32)              // sel > 96: not prefetched
+                        if (q0 + lane < n) one(load_row(s0 + q0 + lane));
 #pragma unroll
                     for (int q = 0; q < 12; ++q)
 #pragma unroll
                         for (int o = 16; o > 0; o >>= 1) acc[q] += __shfl_xor_sync(0xffffffffu, acc[q], o);
-                    if (lane == 0 && n > 0) {
+                    if (lane == 0) {
                         double* fi = a.f + (size_t)ba * 3;
                         atomicAdd(fi, (double)acc[0]); atomicAdd(fi + 1, (double)acc[1]); atomicAdd(fi + 2, (double)acc[2]);
                         double* cp = a.cpart + (size_t)r * 9;
