@@ -160,6 +160,7 @@ size_t model_bytes(const pimd_ctx* c, const pimd_model_desc* d) {
     b += align_up((size_t)d->n_types * (PN + 1) * 4, 256) + align_up(PN * nsel * 4, 256);
     b += align_up((size_t)d->n_types * ((PN + 1023) / 1024) * 4, 256) + align_up(PN * 72, 256);
     b += align_up(cmp_image_words_fw(d->n_types) * 4, 256) + align_up(cmp_image_words_bw(d->n_types) * 4, 256);
+    b += align_up((PN / 8 + d->n_types + 1) * 4, 256);
     return b + 65536;
 }
 
@@ -836,6 +837,7 @@ int pimd_set_embedding_compressed(pimd_ctx* ctx, int on) {
         cmp_build_images(ctx->emb_w_host.data(), ctx->ntypes, fw.data(), bw.data());     // FP64 on the host -> FP16 hi / lo
         if ((rc = arena_alloc(ctx, &m.cmp_img_fw, fw.size()))) return rc;
         if ((rc = arena_alloc(ctx, &m.cmp_img_bw, bw.size()))) return rc;
+        if ((rc = arena_alloc(ctx, &m.cmp_need, (size_t)ctx->P * ctx->N / 8 + ctx->ntypes + 1))) return rc;
         CK(cudaMemcpyAsync(m.cmp_img_fw, fw.data(), fw.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
         CK(cudaMemcpyAsync(m.cmp_img_bw, bw.data(), bw.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
         CK(cudaStreamSynchronize(ctx->stream));

@@ -172,6 +172,7 @@ struct Model {
     bool     compressed = false;
     uint32_t* cmp_img_fw = nullptr;    // tensor-memory images of the tables: forward A operand per centre type
     uint32_t* cmp_img_bw = nullptr;    // backward A operand (four M tiles) per centre type
+    uint32_t* cmp_need = nullptr;      // [PN / 8 + ntypes + 1] per tile: which upper M tiles the backward kernel needs
 };
 
 struct ForceArgs {

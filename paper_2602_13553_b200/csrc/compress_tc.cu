@@ -107,15 +107,48 @@ struct CmpArgs {
     const int* ncount;         // [PN][ntypes]
     const NeighSlotA* slotA;
     const NeighSlotB* slotB;
-    const uint32_t* img_fw;    // [ntypes][2 hi/lo][128 lanes][FW_COLS]
-    const uint32_t* img_bw;    // [ntypes][2 hi/lo][BW_MT][128 lanes][BW_COLS]
+    const uint32_t* img_fw;    // [ntypes][128 lanes][2 hi/lo][FW_COLS]           (the column order of tensor memory)
+    const uint32_t* img_bw;    // [ntypes][128 lanes][BW_MT][2 hi/lo][BW_COLS]
     float* Tm;                 // [PN rows][100][4]
     const float* dTm;
     double* f;                 // [P][N][3]
     double* cpart;             // [PN][9]
     int* overflow;             // bit 2 (value 4): a row outside the table (s > 2)
+    uint32_t* need;            // [PN / TC + ntypes + 1] per tile of 8 centres, written by the forward kernel: bit tj = some row
+                               // of neighbour type tj sits in the upper 20 positions (backward: which M tiles to compute)
     float inv_nsel;
 };
+
+// The table image of one centre type, [128 lanes][ncols] words in global memory with the column order of tensor memory,
+// is written to TMEM columns [0, ncols) by ALL warps of the CTA: warp w serves lane quarter w % 4 (the quarter it may
+// address) and every (nwarps / 4)-th chunk of 8 columns; two chunks of loads are in flight before their stores.
+__device__ __forceinline__ void cmp_load_image(uint32_t tmem, const uint32_t* __restrict__ img, int ncols, int warp, int lane, int nwarps) {
+    const int quarter = warp & 3, slice = warp >> 2, nslice = nwarps >> 2;
+    const uint32_t lanefield = ((uint32_t)(quarter * 32)) << 16;
+    const uint4* src = reinterpret_cast<const uint4*>(img + (size_t)(quarter * 32 + lane) * ncols);
+    const int nch = ncols >> 3;
+    for (int ch0 = slice; ch0 < nch; ch0 += 2 * nslice) {
+        const int ch1 = ch0 + nslice;
+        const uint4 x0 = __ldg(src + 2 * ch0), x1 = __ldg(src + 2 * ch0 + 1);
+        uint4 y0 = x0, y1 = x1;
+        if (ch1 < nch) { y0 = __ldg(src + 2 * ch1); y1 = __ldg(src + 2 * ch1 + 1); }
+        {
+            const uint32_t v[8] = {x0.x, x0.y, x0.z, x0.w, x1.x, x1.y, x1.z, x1.w};
+            tmem_st8(tmem + lanefield + ch0 * 8, v);
+        }
+        if (ch1 < nch) {                                                // warp-uniform
+            const uint32_t v[8] = {y0.x, y0.y, y0.z, y0.w, y1.x, y1.y, y1.z, y1.w};
+            tmem_st8(tmem + lanefield + ch1 * 8, v);
+        }
+    }
+    tmem_st_wait();
+}
+
+// Position of interval iv inside the K order of the images.  Liquid water populates intervals 0..13 (r > 1.45 A) and
+// 20, 21 (the O-H bond, s ~ 1.05); the order 0..13, 20, 21, 14..19, 22..39 puts all of them into the first 20
+// positions = the first M tile of a neighbour type in the backward kernel and the first 8 k-steps in the forward one,
+// so that the remaining MMAs are issued only for tiles that hold a row elsewhere (close contacts).
+__host__ __device__ __forceinline__ int cmp_pos(int iv) { return iv < 14 ? iv : (iv < 20 ? iv + 2 : (iv < 22 ? iv - 6 : iv)); }
 
 // interval and normalised offset of a row (R-28): iv = min(floor(s / h), 39), u = s / h - iv
 __device__ __forceinline__ void cmp_locate(float s, int& iv, float& u) {
@@ -141,7 +174,8 @@ cmp_fwd_kernel(const __grid_constant__ CmpArgs a) {
     uint64_t* mma_done = bars + 2;     // accumulator complete                                               (commit)
     uint64_t* d_free = bars + 3;       // epilogue has read the accumulator                                  (count 128)
     uint32_t* kmask = reinterpret_cast<uint32_t*>(bars + 4);      // [F_WARPS] k-steps with non-zero moments
-    uint32_t* tmem_ptr = kmask + F_WARPS;
+    uint32_t* upm = kmask + F_WARPS;                               // [F_WARPS] the warp saw a row in the upper 20 positions
+    uint32_t* tmem_ptr = upm + F_WARPS;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) {
@@ -170,21 +204,7 @@ cmp_fwd_kernel(const __grid_constant__ CmpArgs a) {
         // ---- the table of centre type t_i goes into tensor memory (all MMAs of the previous type have retired:
         //      every role has passed its last tile, whose epilogue waited for mma_done) ----
         __syncthreads();
-        if (warp >= F_WARPS) {
-            const int L = (warp - F_WARPS) * 32 + lane;
-            const uint32_t lanefield = ((uint32_t)((warp - F_WARPS) * 32)) << 16;
-#pragma unroll 1
-            for (int copy = 0; copy < 2; ++copy) {
-                const uint4* src = reinterpret_cast<const uint4*>(a.img_fw + (((size_t)ti * 2 + copy) * 128 + L) * FW_COLS);
-#pragma unroll 1
-                for (int c8 = 0; c8 < FW_COLS / 8; ++c8) {
-                    const uint4 x0 = __ldg(src + 2 * c8), x1 = __ldg(src + 2 * c8 + 1);
-                    const uint32_t v[8] = {x0.x, x0.y, x0.z, x0.w, x1.x, x1.y, x1.z, x1.w};
-                    tmem_st8(tmem + lanefield + copy * FW_COLS + c8 * 8, v);
-                }
-            }
-            tmem_st_wait();
-        }
+        cmp_load_image(tmem, a.img_fw + (size_t)ti * 128 * (2 * FW_COLS), 2 * FW_COLS, warp, lane, F_THREADS / 32);
         tc_fence_before();
         __syncthreads();
         tc_fence_after();
@@ -221,6 +241,7 @@ cmp_fwd_kernel(const __grid_constant__ CmpArgs a) {
             };
             const int hotk = tj * NI * NP;                           // bucket (tj, interval 0): two thirds of all rows
             // one batch of up to 32 rows: lane = row writes its 24 products u^p R_c, then lane = (p, c) adds them up
+            bool up = false;
             auto batch = [&](const RowF& R, int nb, float& acc0) {
                 if (lane < nb) {
                     const float s = R.s, sr = R.s * R.rinv;
@@ -239,7 +260,9 @@ cmp_fwd_kernel(const __grid_constant__ CmpArgs a) {
                         for (int cc = 0; cc < 4; ++cc) rb[pp * 4 + cc] = pw * Rv[cc];
                         pw *= u;
                     }
-                    rb[24] = __int_as_float((tj * NI + iv) * NP);
+                    const int pos = cmp_pos(iv);
+                    up |= pos >= NI / 2;
+                    rb[24] = __int_as_float((tj * NI + pos) * NP);
                 }
                 __syncwarp();
                 if (lane < 24) {
@@ -300,8 +323,11 @@ cmp_fwd_kernel(const __grid_constant__ CmpArgs a) {
                 km = __reduce_or_sync(0xffffffffu, km);
                 fence_proxy_async_smem();
                 __syncwarp();
+                const bool upw = __any_sync(0xffffffffu, up);
+                up = false;
                 if (lane == 0) {
                     kmask[warp] = km;
+                    upm[warp] = upw ? 1u : 0u;
                     mbar_arrive(ready);
                 }
             }
@@ -316,8 +342,9 @@ cmp_fwd_kernel(const __grid_constant__ CmpArgs a) {
                     if (it > 0) mbar_wait(d_free, (it - 1) & 1);
                     tc_fence_after();
                     if (lane == 0) {
-                        uint32_t km = 1u;                          // k-step 0 always: the accumulator is always written
-                        for (int w = 0; w < F_WARPS; ++w) km |= kmask[w];
+                        uint32_t km = 1u, nd = 0u;                 // k-step 0 always: the accumulator is always written
+                        for (int w = 0; w < F_WARPS; ++w) { km |= kmask[w]; nd |= upm[w] << (w & 1); }
+                        a.need[row0 / TC + ti + tile] = nd;
                         const uint32_t bh = smem_u32(opB_hi), bl = smem_u32(opB_lo);
                         uint32_t acc = 0;
                         for (int ks = 0; ks < K / 16; ++ks) {
@@ -398,24 +425,7 @@ cmp_bwd_kernel(const __grid_constant__ CmpArgs a) {
         const int row0 = a.type_row0[ti], row1 = a.type_row0[ti + 1];
         const int ntile = (row1 - row0 + TC - 1) / TC;
         __syncthreads();
-        if (warp >= B_WARPS) {
-            const int L = (warp - B_WARPS) * 32 + lane;
-            const uint32_t lanefield = ((uint32_t)((warp - B_WARPS) * 32)) << 16;
-#pragma unroll 1
-            for (int copy = 0; copy < 2; ++copy)
-#pragma unroll 1
-                for (int j = 0; j < BW_MT; ++j) {
-                    const uint4* src = reinterpret_cast<const uint4*>(
-                        a.img_bw + ((((size_t)ti * 2 + copy) * BW_MT + j) * 128 + L) * BW_COLS);
-#pragma unroll 1
-                    for (int c8 = 0; c8 < BW_COLS / 8; ++c8) {
-                        const uint4 x0 = __ldg(src + 2 * c8), x1 = __ldg(src + 2 * c8 + 1);
-                        const uint32_t v[8] = {x0.x, x0.y, x0.z, x0.w, x1.x, x1.y, x1.z, x1.w};
-                        tmem_st8(tmem + lanefield + j * 2 * BW_COLS + copy * BW_COLS + c8 * 8, v);
-                    }
-                }
-            tmem_st_wait();
-        }
+        cmp_load_image(tmem, a.img_bw + (size_t)ti * 128 * BW_D, BW_D, warp, lane, B_THREADS / 32);
         tc_fence_before();
         __syncthreads();
         tc_fence_after();
@@ -436,6 +446,7 @@ cmp_bwd_kernel(const __grid_constant__ CmpArgs a) {
             };
             float4 x[8];
             load_dT(blockIdx.x, x);
+            uint32_t nd_next = ((int)blockIdx.x < ntile) ? __ldg(a.need + row0 / TC + ti + blockIdx.x) : 0u;
             for (int tile = blockIdx.x; tile < ntile; tile += gridDim.x, ++it) {
                 const int buf = it & 1;
                 // ---- dT of the tile's centres -> operand rows (centre, c), K = channel; scaled per centre by the
@@ -470,11 +481,11 @@ cmp_bwd_kernel(const __grid_constant__ CmpArgs a) {
                 if (it >= 2) mbar_wait(qempty + buf, ((it >> 1) - 1) & 1);     // the row warps have left this Q buffer
                 tc_fence_before();
                 cmp_bar_sync(1, 128);
-                auto issue = [&](int j) {
+                auto issue = [&](int j, int db) {
                     if (t == 0) {
                         tc_fence_after();
                         const uint32_t bh = smem_u32(opB_hi), bl = smem_u32(opB_lo);
-                        const uint32_t d = tmem + BW_D + (j & 1) * NROW;
+                        const uint32_t d = tmem + BW_D + db * NROW;
                         for (int ks = 0; ks < BW_KP / 16; ++ks) {
                             const uint32_t boff = (uint32_t)((ks >> 2) * (NROW * 128) + (ks & 3) * 32);
                             const uint64_t dbh = make_smem_desc_kmajor(bh + boff, 128), dbl = make_smem_desc_kmajor(bl + boff, 128);
@@ -483,15 +494,21 @@ cmp_bwd_kernel(const __grid_constant__ CmpArgs a) {
                             umma_f16_ts(d, alo, dbh, idesc, 1u);
                             umma_f16_ts(d, ahi, dbl, idesc, 1u);
                         }
-                        umma_commit(dfull + (j & 1));
+                        umma_commit(dfull + db);
                     }
                 };
-                issue(0);
-                issue(1);
+                // M tiles of this tile of centres: the lower 20 positions of both neighbour types always (j = 0, 2), the
+                // upper ones (j = 1, 3) only when a row sits there.  Two accumulator buffers, used in turn.
+                const uint32_t nd = nd_next;
+                nd_next = (tile + (int)gridDim.x < ntile) ? __ldg(a.need + row0 / TC + ti + tile + gridDim.x) : 0u;
+                const int nj = 2 + (int)(nd & 1u) + (int)((nd >> 1) & 1u);
+                auto jof = [&](int idx) { return idx == 0 ? 0 : idx == 1 ? 2 : (idx == 2 ? ((nd & 1u) ? 1 : 3) : 3); };
+                issue(0, 0);
+                issue(2, 1);
                 float4* Qb = Qs + (size_t)buf * (TC * K);
 #pragma unroll 1
-                for (int j = 0; j < BW_MT; ++j) {
-                    const int db = j & 1;
+                for (int idx = 0; idx < nj; ++idx) {
+                    const int db = idx & 1, j = jof(idx);
                     mbar_wait(dfull + db, (db ? ndf1 : ndf0) & 1);
                     if (db) ++ndf1; else ++ndf0;
                     tc_fence_after();
@@ -500,16 +517,16 @@ cmp_bwd_kernel(const __grid_constant__ CmpArgs a) {
                     tmem_ld_wait();
                     if (t < BW_ROWS) {
 #pragma unroll
-                        for (int cl = 0; cl < TC; ++cl) {
-                            const float is = inv_scale[cl];
-                            Qb[cl * K + j * BW_ROWS + t] = make_float4(__uint_as_float(v[4 * cl]) * is, __uint_as_float(v[4 * cl + 1]) * is,
-                                                                       __uint_as_float(v[4 * cl + 2]) * is, __uint_as_float(v[4 * cl + 3]) * is);
+                        for (int cl2 = 0; cl2 < TC; ++cl2) {
+                            const float is = inv_scale[cl2];
+                            Qb[cl2 * K + j * BW_ROWS + t] = make_float4(__uint_as_float(v[4 * cl2]) * is, __uint_as_float(v[4 * cl2 + 1]) * is,
+                                                                        __uint_as_float(v[4 * cl2 + 2]) * is, __uint_as_float(v[4 * cl2 + 3]) * is);
                         }
                     }
-                    if (j + 2 < BW_MT) {
+                    if (idx + 2 < nj) {
                         tc_fence_before();
                         cmp_bar_sync(1, 128);                       // every thread has read this accumulator buffer
-                        issue(j + 2);
+                        issue(jof(idx + 2), db);
                     }
                 }
                 tc_fence_before();
@@ -560,7 +577,7 @@ cmp_bwd_kernel(const __grid_constant__ CmpArgs a) {
                         const float s = R.s, dsw = R.dsw, rinv = R.rinv;
                         int iv; float u;
                         cmp_locate(s, iv, u);
-                        const float4* Q = Qc + iv * NP;
+                        const float4* Q = Qc + cmp_pos(iv) * NP;
                         const float4 q5 = Q[5], q4 = Q[4], q3 = Q[3], q2 = Q[2], q1 = Q[1], q0v = Q[0];
                         // A_c = sum_p u^p Q_p[c],  D_c = sum_p p u^(p-1) Q_p[c]  (Horner)
                         float Av[4], Dv[4];
@@ -727,11 +744,11 @@ void cmp_build_images(const double* w_emb, int ntypes, uint32_t* img_fw, uint32_
                 for (int p = 0; p < NP; ++p)
                     for (int m = 0; m < M1; ++m) {
                         const float v = (float)C[((size_t)iv * NP + p) * M1 + m];
-                        const int k = tj * KB + iv * NP + p;
+                        const int k = tj * KB + cmp_pos(iv) * NP + p;
                         for (int copy = 0; copy < 2; ++copy) {
-                            put(img_fw + (((size_t)ti * 2 + copy) * 128 + m) * FW_COLS + (k >> 1), k & 1, v, copy == 1);
+                            put(img_fw + (((size_t)ti * 128 + m) * 2 + copy) * FW_COLS + (k >> 1), k & 1, v, copy == 1);
                             const int j = k / BW_ROWS, lanek = k - j * BW_ROWS;
-                            put(img_bw + ((((size_t)ti * 2 + copy) * BW_MT + j) * 128 + lanek) * BW_COLS + (m >> 1), m & 1, v, copy == 1);
+                            put(img_bw + ((((size_t)ti * 128 + lanek) * BW_MT + j) * 2 + copy) * BW_COLS + (m >> 1), m & 1, v, copy == 1);
                         }
                     }
         }
@@ -744,7 +761,7 @@ static CmpArgs make_cmp_args(Model& m, const ForceArgs& fa) {
     for (int t = 0; t < PIMD_MAX_TYPES; ++t) a.n_of_type[t] = (t < fa.ntypes) ? m.n_of_type[t] : 0;
     a.cen_idx = m.cen_idx; a.ncount = m.ncount; a.slotA = m.slotA; a.slotB = m.slotB;
     a.img_fw = m.cmp_img_fw; a.img_bw = m.cmp_img_bw;
-    a.Tm = m.Tm; a.dTm = m.dTm; a.f = fa.f; a.cpart = m.cpart; a.overflow = m.overflow;
+    a.Tm = m.Tm; a.dTm = m.dTm; a.f = fa.f; a.cpart = m.cpart; a.overflow = m.overflow; a.need = m.cmp_need;
     a.inv_nsel = 1.0f / (float)m.nsel;
     return a;
 }
