@@ -41,6 +41,8 @@ extern "C" {
                                   * a state (the forces of a truncated neighbour list are not kept); set a new one. */
 #define PIMD_ECUDA          -5   /* CUDA runtime error; see pimd_last_error */
 #define PIMD_ENOMEM         -6   /* the caller-supplied workspace is too small */
+#define PIMD_ECONTACT       -8   /* two atoms closer than 0.01 A (s = 1/r > 100): outside the range the fixed FP16 operand
+                                  * scales of the descriptor / fitting kernels assume.  Reported like PIMD_ESEL_OVERFLOW. */
 #define PIMD_ETABLE_RANGE   -7   /* compressed embedding: a neighbour row lies outside the table (s > 2, r < 0.5 A; R-28).
                                   * Reported like PIMD_ESEL_OVERFLOW (pimd_step rolls the call back). */
 
@@ -115,7 +117,9 @@ int pimd_restore(pimd_ctx* ctx, const double* x, const double* p, const double* 
 /* The se_e2_a Deep-Potential model (PAPER.md:L47, L76 cite it; definition DESIGN.md R-11..R-16).
  * weights: n_weights doubles, row-major W[in][out] then bias[out] per layer, in the order
  *   for t_i: for t_j: embedding layers 1..3;  then for t_i: fitting layers 1..4 (last out = 1).
- * n_weights must equal pimd_model_n_weights(d).  The library converts to FP32 on the device. */
+ * n_weights must equal pimd_model_n_weights(d).  The library converts to FP32 on the device.  Every weight must be
+ * finite and at most 1000 in magnitude (the tensor-core kernels use FP16 hi / lo operand pairs with fixed scales):
+ * PIMD_EINVAL otherwise. */
 size_t pimd_model_n_weights(const pimd_model_desc* d);
 int pimd_set_model(pimd_ctx* ctx, const pimd_model_desc* d, const double* weights, size_t n_weights);
 

@@ -8,7 +8,7 @@ checked), but every compute call needs the compiled library and a CUDA device.
 """
 from .binding import (  # noqa: F401
     PIMD_OK, PIMD_EINVAL, PIMD_ENOSTATE, PIMD_ENOMODEL, PIMD_ESEL_OVERFLOW, PIMD_ECUDA, PIMD_ENOMEM,
-    PIMD_ETABLE_RANGE, pimd_set_embedding_compressed,
+    PIMD_ETABLE_RANGE, PIMD_ECONTACT, pimd_set_embedding_compressed,
     PimdError, ModelDesc, Estimators, lib, library_path,
     pimd_create, pimd_destroy, pimd_last_error, pimd_workspace_bytes, pimd_set_workspace,
     pimd_set_state, pimd_set_state_dev, pimd_model_n_weights, pimd_set_model, pimd_set_model_harmonic,

@@ -10,7 +10,7 @@ import os
 import numpy as np
 
 PIMD_OK, PIMD_EINVAL, PIMD_ENOSTATE, PIMD_ENOMODEL = 0, -1, -2, -3
-PIMD_ESEL_OVERFLOW, PIMD_ECUDA, PIMD_ENOMEM, PIMD_ETABLE_RANGE = -4, -5, -6, -7
+PIMD_ESEL_OVERFLOW, PIMD_ECUDA, PIMD_ENOMEM, PIMD_ETABLE_RANGE, PIMD_ECONTACT = -4, -5, -6, -7, -8
 PIMD_MAX_TYPES = 4
 
 _HERE = os.path.dirname(os.path.abspath(__file__))

@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include "common.cuh"
@@ -61,6 +62,13 @@ struct pimd_ctx {
                                                            // pimd_step: the entry snapshot of x and v~ (rollback)
     double *snap_f = nullptr, *snap_small = nullptr;       // entry snapshot of f [P][N][3]; of U, Xi, barostat state
     int64_t evals_launched = 0;                            // force evaluations issued so far (mirrors model.overflow[2])
+    // one captured launch sequence per step: {integrator, force evaluation} as a CUDA graph that is
+    // replayed for the inner steps of a pimd_step call; step counter and estimator slot live on the device (ctl_dev)
+    long long* ctl_dev = nullptr;                          // {step the next integrator launch opens, step of history slot 0}
+    cudaGraphExec_t step_graph = nullptr;
+    uint64_t graph_key = 0;
+    int64_t graph_launches = 0;                            // kernels inside one replay
+    bool graph_failed = false;
     int* types_d = nullptr;
     double *U = nullptr, *Xi = nullptr, *Eatom = nullptr;
     double* est = nullptr;        // [kEstCap + 2][kEstWidth]; slot kEstCap = "current", kEstCap+1 = scratch
@@ -114,6 +122,7 @@ size_t base_bytes(const pimd_ctx* c) {
     size_t b = 0;
     b += 6 * align_up(PN3 * 8, 256);                          // x, vt, f, scratch_a, scratch_b, snap_f
     b += align_up(((size_t)c->P * 10 + BS_WIDTH) * 8, 256);   // snap_small
+    b += 256;                                                 // ctl_dev
     b += align_up((size_t)c->N * 8, 256) + align_up((size_t)c->N * 4, 256);
     b += align_up((size_t)c->P * 8, 256) + align_up((size_t)c->P * 72, 256) + align_up((size_t)c->P * c->N * 8, 256);
     b += align_up((size_t)(kEstCap + 2) * kEstWidth * 8, 256);
@@ -202,6 +211,8 @@ int alloc_base(pimd_ctx* ctx) {
     if ((rc = arena_alloc(ctx, &ctx->scratch_b, PN3))) return rc;
     if ((rc = arena_alloc(ctx, &ctx->snap_f, PN3))) return rc;
     if ((rc = arena_alloc(ctx, &ctx->snap_small, (size_t)ctx->P * 10 + BS_WIDTH))) return rc;
+    if ((rc = arena_alloc(ctx, &ctx->ctl_dev, (size_t)2))) return rc;
+    CK(cudaMemsetAsync(ctx->ctl_dev, 0, 2 * sizeof(long long), ctx->stream));
     if ((rc = arena_alloc(ctx, &ctx->mass_atom, (size_t)ctx->N))) return rc;
     if ((rc = arena_alloc(ctx, &ctx->types_d, (size_t)ctx->N))) return rc;
     if ((rc = arena_alloc(ctx, &ctx->U, (size_t)ctx->P))) return rc;
@@ -239,6 +250,7 @@ int eval_forces(pimd_ctx* ctx) {
     for (int c = 0; c < 3; ++c) a.box[c] = ctx->box[c];
     a.box_dev = ctx->baro ? ctx->baro_state + BS_LX : nullptr;
     a.x = ctx->x; a.types = ctx->types_d; a.f = ctx->f; a.U = ctx->U; a.Xi = ctx->Xi; a.Eatom = ctx->Eatom;
+    a.ctl = ctx->ctl_dev;
     const size_t PN3 = (size_t)ctx->P * ctx->N * 3;
     cudaMemsetAsync(ctx->f, 0, PN3 * 8, ctx->stream);
     cudaMemsetAsync(ctx->U, 0, sizeof(double) * ctx->P, ctx->stream);
@@ -286,6 +298,9 @@ void fill_integrator_args(pimd_ctx* ctx, IntegratorArgs& a, int flags, int64_t s
     a.baro = ctx->baro ? ctx->baro_state : nullptr;
     { const double wP = ctx->P * kKB * ctx->T / kHbar; a.wP2 = wP * wP; }
     if (ctx->method == PIMD_CART) a.flags |= I_CART;
+    a.ctl = nullptr;
+    a.est_base = ctx->est;
+    a.est_scratch = ctx->est + (size_t)(kEstCap + 1) * kEstWidth;
 }
 
 constexpr double kBarPerEvA3 = 1.602176634e6;    // DESIGN R-25
@@ -340,6 +355,8 @@ int check_overflow(pimd_ctx* ctx, int64_t* failed_eval = nullptr) {
         cudaMemcpyAsync(ctx->model.overflow, reset, sizeof(reset), cudaMemcpyHostToDevice, ctx->stream);
         cudaStreamSynchronize(ctx->stream);
         if (failed_eval) *failed_eval = (int64_t)flag[1] - 1;
+        if (flag[0] & 8u)
+            return fail(ctx, PIMD_ECONTACT, "two atoms are closer than 0.01 A: s = 1/r leaves the range the FP16-split descriptor operands assume");
         if (flag[0] & 4u)
             return fail(ctx, PIMD_ETABLE_RANGE, "a neighbour row lies outside the compression table (s > 2, i.e. r < 0.5 A; DESIGN R-28)");
         if (flag[0] & 2u)
@@ -417,6 +434,7 @@ int pimd_create(pimd_ctx** out, int n_atoms, const int32_t* types, int n_types, 
 void pimd_destroy(pimd_ctx* ctx) {
     if (!ctx) return;
     cudaStreamSynchronize(ctx->stream);
+    if (ctx->step_graph) cudaGraphExecDestroy(ctx->step_graph);
     if (ctx->model.aux_stream[0]) {
         for (int q = 0; q < Model::kChainStreams - 1; ++q) {
             cudaStreamSynchronize(ctx->model.aux_stream[q]);
@@ -663,6 +681,14 @@ int pimd_set_model(pimd_ctx* ctx, const pimd_model_desc* d, const double* w, siz
         return fail(ctx, PIMD_EINVAL, "fitting widths must be equal and a multiple of 16");
     if (!(d->rcut > d->rcut_smth && d->rcut_smth >= 0)) return fail(ctx, PIMD_EINVAL, "need rcut > rcut_smth >= 0");
     if (ctx->model.set) return fail(ctx, PIMD_EINVAL, "the model of a context can be set once");
+    // The tensor-core kernels split every operand into FP16 hi / lo pairs with FIXED power-of-two scales (D x 256,
+    // W1 x 64, unscaled embedding operands; DESIGN section 6 "Precision").  Those scales assume weights of order one;
+    // a weight outside +-1000 (64 x 1000 is FP16's largest finite value) or a non-finite one is refused here rather
+    // than turning into inf / NaN inside a kernel.
+    for (size_t q = 0; q < n_weights; ++q)
+        if (!(std::fabs(w[q]) <= 1000.0))
+            return fail(ctx, PIMD_EINVAL, "weight " + std::to_string(q) + " is non-finite or exceeds 1000 in magnitude: outside the "
+                                          "range of the FP16-split tensor-core operands");
     int rc;
     if ((rc = alloc_base(ctx))) return rc;
     Model& m = ctx->model;
@@ -876,8 +902,9 @@ int pimd_step(pimd_ctx* ctx, int64_t n_steps) {
     double* cur = ctx->est + (size_t)kEstCap * kEstWidth;
     double* scratch = ctx->est + (size_t)(kEstCap + 1) * kEstWidth;
     float ms_acc[6] = {0, 0, 0, 0, 0, 0};
-    for (int64_t s = 0; s <= n_steps; ++s) {
-        // launch s: closes step s-1 (B, estimators) and opens step s (B A O A)
+    // launch s: closes step s-1 (B, estimators) and opens step s (B A O A).  ctl_mode: step counter and estimator slot
+    // come from the device (graph replay), the host values are then ignored by the kernels.
+    auto integ = [&](int64_t s, bool ctl_mode) {
         int flags = 0;
         double* slot = scratch;
         if (s > 0) {
@@ -893,24 +920,73 @@ int pimd_step(pimd_ctx* ctx, int64_t n_steps) {
             // so the launch splits: close + accumulate, then subtract + estimators (+ open)
             cudaMemsetAsync(ctx->com, 0, sizeof(double) * 3, ctx->stream);
             fill_integrator_args(ctx, a, I_BCLOSE | I_COMACC, ctx->step + s, scratch);
+            if (ctl_mode) a.ctl = ctx->ctl_dev;
             ctx->launches += launch_integrator(ctx->P, a, ctx->mc, ctx->stream);
             flags = (flags & ~I_BCLOSE) | I_COMSUB;
         }
         fill_integrator_args(ctx, a, flags, ctx->step + s, slot);
+        if (ctl_mode) a.ctl = ctx->ctl_dev;
         ctx->launches += launch_integrator(ctx->P, a, ctx->mc, ctx->stream);
-        if (s < n_steps) {
-            int rc = eval_forces(ctx);
-            if (rc) return rc;
-            if (ctx->profiling) {
-                rec(ctx, 6);
-                cudaEventSynchronize(ctx->ev[6]);
-                float t;
-                if (ctx->model_kind == 2) {
-                    cudaEventElapsedTime(&t, ctx->ev[0], ctx->ev[1]); ms_acc[0] += t;
-                    for (int q = 1; q < 5; ++q) { cudaEventElapsedTime(&t, ctx->ev[q], ctx->ev[q + 1]); ms_acc[q] += t; }
+    };
+    const bool use_graph = ctx->model_kind == 2 && !ctx->baro && !ctx->profiling && n_steps >= 3 && !ctx->graph_failed &&
+                           getenv("PIMD_NO_GRAPH") == nullptr;
+    if (!use_graph) {
+        for (int64_t s = 0; s <= n_steps; ++s) {
+            integ(s, false);
+            if (s < n_steps) {
+                int rc = eval_forces(ctx);
+                if (rc) return rc;
+                if (ctx->profiling) {
+                    rec(ctx, 6);
+                    cudaEventSynchronize(ctx->ev[6]);
+                    float t;
+                    if (ctx->model_kind == 2) {
+                        cudaEventElapsedTime(&t, ctx->ev[0], ctx->ev[1]); ms_acc[0] += t;
+                        for (int q = 1; q < 5; ++q) { cudaEventElapsedTime(&t, ctx->ev[q], ctx->ev[q + 1]); ms_acc[q] += t; }
+                    }
                 }
             }
         }
+    } else {
+        // One captured launch sequence per step: {integrator launch of an inner step, force evaluation} becomes a CUDA
+        // graph (the three streams of the fitting chain included) and is replayed n_steps - 1 times.
+        const long long ctl_h[2] = {(long long)ctx->step, (long long)(ctx->step + first_hist)};
+        CK(cudaMemcpyAsync(ctx->ctl_dev, ctl_h, sizeof(ctl_h), cudaMemcpyHostToDevice, ctx->stream));
+        integ(0, true);
+        { int rc = eval_forces(ctx); if (rc) return rc; }
+        const Model& mm = ctx->model;
+        const uint64_t key = 1ull | ((uint64_t)ctx->integrator << 1) | ((uint64_t)ctx->fixcom << 2) | ((uint64_t)ctx->method << 3) |
+                             ((uint64_t)mm.compressed << 4) | ((uint64_t)mm.use_tc << 5) | ((uint64_t)mm.use_tc_emb << 6) |
+                             ((uint64_t)(ctx->gamma0 != 0.0) << 7);
+        if (ctx->step_graph && ctx->graph_key != key) { cudaGraphExecDestroy(ctx->step_graph); ctx->step_graph = nullptr; }
+        if (!ctx->step_graph) {
+            const int64_t l0 = ctx->launches, e0 = ctx->evals_launched;
+            cudaGraph_t g = nullptr;
+            bool ok = cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeRelaxed) == cudaSuccess;
+            if (ok) {
+                integ(1, true);                         // an inner step: n_steps >= 3, so 0 < 1 < n_steps
+                eval_forces(ctx);
+                ok = cudaStreamEndCapture(ctx->stream, &g) == cudaSuccess && g != nullptr;
+            }
+            ctx->graph_launches = ctx->launches - l0;
+            ctx->launches = l0; ctx->evals_launched = e0;     // a capture launches nothing
+            if (ok) ok = cudaGraphInstantiate(&ctx->step_graph, g, 0) == cudaSuccess;
+            if (g) cudaGraphDestroy(g);
+            if (!ok) { ctx->step_graph = nullptr; ctx->graph_failed = true; cudaGetLastError(); }
+            ctx->graph_key = key;
+        }
+        for (int64_t s = 1; s < n_steps; ++s) {
+            if (ctx->step_graph) {
+                CK(cudaGraphLaunch(ctx->step_graph, ctx->stream));
+                ctx->launches += ctx->graph_launches;
+                ctx->evals_launched += 1;
+            } else {
+                integ(s, true);
+                int rc = eval_forces(ctx);
+                if (rc) return rc;
+            }
+        }
+        integ(n_steps, true);
     }
     CK(cudaGetLastError());
     // the last slot is also "current"

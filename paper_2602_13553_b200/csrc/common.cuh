@@ -55,6 +55,13 @@ struct IntegratorArgs {
     double   inv_mtot;           // 1 / sum_i m_i
     double   wP2;                // omega_n^2 (Cartesian method: ring-spring force)
     const double* baro;          // barostat state (BaroSlot layout) or null: centroid drift by Eq. E4/E5
+    // Graph replay (api.cu): when ctl != null the step counter and the estimator slot are NOT launch arguments but are
+    // read from the device -- ctl[0] = the step this launch opens (advanced once per force evaluation by
+    // wrap_bin_kernel), ctl[1] = the absolute step whose estimators go to history slot 0 -- so that one captured
+    // launch sequence serves every step of a pimd_step call.
+    const long long* ctl;
+    double*  est_base;           // estimator history [kEstCap][kEstWidth]
+    double*  est_scratch;        // slot for steps outside the recorded window
 };
 
 // Barostat state on the device (Appendix E; DESIGN R-20..R-25), doubles:
@@ -185,6 +192,7 @@ struct ForceArgs {
     double* U;            // [P]
     double* Xi;           // [P][9]
     double* Eatom;        // [P][N]
+    long long* ctl;       // device step counter (graph replay) or null
 };
 
 int neighbor_build(Model& m, const ForceArgs& a, cudaStream_t s);

@@ -102,6 +102,21 @@ __device__ __forceinline__ void nm_inverse(double* a) {
 
 constexpr int kIntThreads = 128;
 
+// step counters (Philox counter words 0, 1; R-10) and estimator slot of a launch: launch arguments, or -- under graph
+// replay -- derived from the device-resident step counter
+struct StepView { uint32_t step_lo, step_hi, cstep_lo, cstep_hi; double* est; };
+__device__ __forceinline__ StepView resolve_step(const IntegratorArgs& a) {
+    StepView v = {a.step_lo, a.step_hi, a.cstep_lo, a.cstep_hi, a.est};
+    if (a.ctl != nullptr) {
+        const unsigned long long st = (unsigned long long)a.ctl[0], cs = st - 1ull;
+        v.step_lo = (uint32_t)st; v.step_hi = (uint32_t)(st >> 32);
+        v.cstep_lo = (uint32_t)cs; v.cstep_hi = (uint32_t)(cs >> 32) | 0x80000000u;
+        const long long idx = a.ctl[0] - 1 - a.ctl[1];
+        v.est = (idx >= 0 && idx < kEstCap) ? a.est_base + (size_t)idx * kEstWidth : a.est_scratch;
+    }
+    return v;
+}
+
 template <int P, bool kObabo>
 __global__ void __launch_bounds__(kIntThreads)
 integrator_kernel(const __grid_constant__ IntegratorArgs a, const __grid_constant__ ModeConsts mc) {
@@ -121,6 +136,7 @@ integrator_kernel(const __grid_constant__ IntegratorArgs a, const __grid_constan
     const bool start = (a.flags & I_START) != 0;
     const bool thermo = start && a.thermostat;
     const size_t stride = (size_t)a.n_dof;
+    const StepView sv = resolve_step(a);
 
 #pragma unroll
     for (int k = 0; k < P; ++k) __pipeline_memcpy_async(fs + k * kIntThreads, a.f + k * stride + ec, sizeof(double));
@@ -164,9 +180,9 @@ integrator_kernel(const __grid_constant__ IntegratorArgs a, const __grid_constan
     };
     const bool thermo_close = kObabo && a.thermostat && (a.flags & I_BCLOSE);
     if (kObabo) {
-        if (thermo_close) gen_normals(a.cstep_lo, a.cstep_hi);
+        if (thermo_close) gen_normals(sv.cstep_lo, sv.cstep_hi);
     } else if (thermo) {
-        gen_normals(a.step_lo, a.step_hi);
+        gen_normals(sv.step_lo, sv.step_hi);
     }
 
     __pipeline_wait_prior(1);
@@ -234,7 +250,7 @@ integrator_kernel(const __grid_constant__ IntegratorArgs a, const __grid_constan
             vs[k * kIntThreads] = v;
         }
         // ... and open the next one with O(dt/2) B(dt/2) A(dt) (mc holds cos/sin for dt and c1, c2 for dt/2)
-        if (thermo) gen_normals(a.step_lo, a.step_hi);
+        if (thermo) gen_normals(sv.step_lo, sv.step_hi);
 #pragma unroll
         for (int k = 0; k < P; ++k) {
             double v = vs[k * kIntThreads];
@@ -286,12 +302,12 @@ integrator_kernel(const __grid_constant__ IntegratorArgs a, const __grid_constan
             double t = 0.0;
 #pragma unroll
             for (int q = 0; q < kIntThreads / 32; ++q) t += red[threadIdx.x][q];
-            atomicAdd(a.est + threadIdx.x, t);
+            atomicAdd(sv.est + threadIdx.x, t);
         }
         if (blockIdx.x == 0 && threadIdx.x == 3 && a.U != nullptr) {
             double u = 0.0;
             for (int k = 0; k < P; ++k) u += a.U[k];
-            atomicAdd(a.est + 3, u);
+            atomicAdd(sv.est + 3, u);
         }
     }
 
@@ -334,6 +350,7 @@ integrator_cart_kernel(const __grid_constant__ IntegratorArgs a, const __grid_co
     const bool close = (a.flags & I_BCLOSE) != 0;
     const bool thermo = start && a.thermostat;
     const size_t stride = (size_t)a.n_dof;
+    const StepView sv = resolve_step(a);
     const double m = a.mass[i];
     double x[P], v[P], g[P];             // g: total acceleration-kick h (f + f_spring)/(m mvv2e)
 #pragma unroll
@@ -368,7 +385,7 @@ integrator_cart_kernel(const __grid_constant__ IntegratorArgs a, const __grid_co
 #pragma unroll
         for (int k = 0; k < P; ++k) v[k] += g[k];        // closing B(dt/2)
         if (kObabo && a.thermostat) {                    // closing O(dt/2), second half-step stream
-            gen_normals(a.cstep_lo, a.cstep_hi);
+            gen_normals(sv.cstep_lo, sv.cstep_hi);
 #pragma unroll
             for (int k = 0; k < P; ++k) v[k] = mc.c1[0] * v[k] + mc.c2[0] * sigma * eta_s[k * kIntThreads];
         }
@@ -378,7 +395,7 @@ integrator_cart_kernel(const __grid_constant__ IntegratorArgs a, const __grid_co
     for (int k = 0; k < P; ++k) accK += v[k] * v[k];
     if (start) {
         const double hd = mc.sinA_w[0];                  // drift length: dt/2 (BAOAB), dt (OBABO)
-        if (thermo) gen_normals(a.step_lo, a.step_hi);
+        if (thermo) gen_normals(sv.step_lo, sv.step_hi);
         if (kObabo) {
 #pragma unroll
             for (int k = 0; k < P; ++k) {
@@ -422,12 +439,12 @@ integrator_cart_kernel(const __grid_constant__ IntegratorArgs a, const __grid_co
             double t = 0.0;
 #pragma unroll
             for (int q = 0; q < kIntThreads / 32; ++q) t += red[threadIdx.x][q];
-            atomicAdd(a.est + threadIdx.x, t);
+            atomicAdd(sv.est + threadIdx.x, t);
         }
         if (blockIdx.x == 0 && threadIdx.x == 3 && a.U != nullptr) {
             double u = 0.0;
             for (int k = 0; k < P; ++k) u += a.U[k];
-            atomicAdd(a.est + 3, u);
+            atomicAdd(sv.est + 3, u);
         }
     }
 }

@@ -21,6 +21,7 @@ struct GridGeom {
     const double* boxp;  // barostat (PAPER.md Eq. E6): the cell is rescaled on the device every step; null = use L
     double rc;
     int* overflow;
+    long long* ctl;      // device step counter of the graph-replayed step loop (api.cu): advanced once per evaluation
 };
 
 // cell lengths and inverse cell widths of this launch: kernel arguments, or the device-resident cell under a barostat
@@ -47,6 +48,7 @@ __global__ void wrap_bin_kernel(int P, int N, GridGeom g, const double* __restri
     if (ba == 0) {
         const int ev = g.overflow[2] + 1;            // force evaluations since pimd_set_model, this one included
         g.overflow[2] = ev;
+        if (g.ctl) g.ctl[0] += 1;                    // the next integrator launch opens the next step
         if (g.boxp) {
             // the cell shrank so far inside one pimd_step call that rc spans more than R cells: neighbours would be missed
             for (int a = 0; a < 3; ++a)
@@ -330,6 +332,10 @@ neighbor_env_kernel(int P, int N, GridGeom g, EnvConsts ec, const double* __rest
             d[2] = __dadd_rn(__dsub_rn(wj.z, wi[2]), __dmul_rn((double)nz, gL[2]));
             const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2]));
             const double r = sqrt(r2);
+            if (r < 0.01) {          // |R| = 1/r > 100: beyond what the fixed FP16 scales of the descriptor kernels hold
+                atomicOr(overflow, 8);
+                atomicMin(reinterpret_cast<unsigned*>(overflow) + 1, (unsigned)overflow[2]);
+            }
             double sw = 1.0, dsw = 0.0;
             if (r >= ec.rs) {
                 const double u = (r - ec.rs) * ec.inv_range;
@@ -365,7 +371,7 @@ int neighbor_build(Model& m, const ForceArgs& a, cudaStream_t s) {
         g.inv_nc[c] = 1.0 / (double)m.ncell[c];
     }
     g.ncells = m.ncells;
-    g.boxp = a.box_dev; g.rc = m.d.rcut; g.overflow = m.overflow;
+    g.boxp = a.box_dev; g.rc = m.d.rcut; g.overflow = m.overflow; g.ctl = a.ctl;
     EnvConsts ec;
     ec.rc = m.d.rcut; ec.rs = m.d.rcut_smth; ec.rc2 = m.d.rcut * m.d.rcut;
     ec.inv_range = 1.0 / (m.d.rcut - m.d.rcut_smth);

@@ -465,6 +465,35 @@ def test_sel_overflow_inside_a_call_rolls_the_call_back(pk):
     sim.close()
 
 
+def test_operands_outside_the_fp16_split_range_are_errors_not_nans(pk):
+    """The tensor-core kernels split operands into FP16 hi / lo pairs with fixed scales: a weight beyond +-1000 (or a
+    non-finite one) is refused by pimd_set_model, and a pair of atoms closer than 0.01 A (s = 1/r > 100) is reported
+    as PIMD_ECONTACT instead of producing inf / NaN forces."""
+    desc = workloads.model_desc()
+    w = workloads.model_weights(desc, 3)
+    types = np.array([0, 1, 1], dtype=np.int32)
+    x = np.array([[[5.0, 5.0, 5.0], [5.9, 5.2, 5.0], [4.8, 5.9, 5.1]]])
+    for bad in (2.0e3, np.inf, np.nan):
+        wb = w.copy()
+        wb[30000] = bad
+        sim = pk.PIMD(types, [15.9994, 1.008], [40.0] * 3, 1, 300.0, 0.5e-3, 1.0, seed=1, model_desc=desc)
+        sim.set_state(x, np.zeros_like(x))
+        with pytest.raises(pk.PimdError) as ei:
+            sim.set_model(wb)
+        assert ei.value.code == pk.PIMD_EINVAL and "weight 30000" in str(ei.value)
+        sim.close()
+    xc = x.copy()
+    xc[0, 1] = xc[0, 0] + np.array([0.004, 0.0, 0.0])
+    sim = pk.PIMD(types, [15.9994, 1.008], [40.0] * 3, 1, 300.0, 0.5e-3, 1.0, seed=1, model_desc=desc)
+    sim.set_model(w)
+    with pytest.raises(pk.PimdError) as ei:
+        sim.set_state(xc, np.zeros_like(xc))
+    assert ei.value.code == pk.PIMD_ECONTACT
+    sim.set_state(x, np.zeros_like(x))                    # a sane configuration afterwards is accepted
+    assert np.all(np.isfinite(sim.forces()))
+    sim.close()
+
+
 def test_binding_refuses_device_tensors_of_the_wrong_kind(pk):
     import torch
     types, masses, x, p = _random_system(10, 4, seed=2)
