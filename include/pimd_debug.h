@@ -38,6 +38,11 @@ int pimd_debug_gemm(pimd_ctx* ctx, int M, int N, int K, const float* A, const fl
  * number behind DESIGN R-10. */
 int pimd_time_kernel(pimd_ctx* ctx, int kind, int reps, double* ms);
 
+/* 1 when the step loop of pimd_step has been captured as a CUDA graph and is replayed (se_e2_a model, no barostat, no
+ * profiling, calls of at least 3 steps; environment variable PIMD_NO_GRAPH disables it), 0 when no graph exists yet,
+ * -100 when a capture failed and the loop fell back to plain launches. */
+int pimd_debug_graph_state(const pimd_ctx* ctx);
+
 #ifdef __cplusplus
 }
 #endif

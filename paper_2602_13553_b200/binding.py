@@ -109,6 +109,7 @@ _SIGNATURES = {
     "pimd_debug_noise": (C.c_int, [C.c_void_p, C.c_int64, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]),
     "pimd_time_kernel": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.POINTER(C.c_double)]),
     "pimd_set_profiling": (C.c_int, [C.c_void_p, C.c_int]),
+    "pimd_debug_graph_state": (C.c_int, [C.c_void_p]),
     "pimd_get_phase_ms": (C.c_int, [C.c_void_p, C.c_void_p]),
 }
 
@@ -382,6 +383,10 @@ def pimd_time_kernel(ctx, kind, reps):
     ms = C.c_double()
     _check(ctx, lib().pimd_time_kernel(ctx, int(kind), int(reps), C.byref(ms)))
     return ms.value
+
+
+def pimd_debug_graph_state(ctx):
+    return int(lib().pimd_debug_graph_state(ctx))
 
 
 def pimd_set_profiling(ctx, on):

@@ -66,6 +66,8 @@ struct pimd_ctx {
     // replayed for the inner steps of a pimd_step call; step counter and estimator slot live on the device (ctl_dev)
     long long* ctl_dev = nullptr;                          // {step the next integrator launch opens, step of history slot 0}
     cudaGraphExec_t step_graph = nullptr;
+    cudaStream_t graph_stream = nullptr;                   // the replayed loop runs here: the caller's stream may be the
+    cudaEvent_t graph_ev = nullptr;                        // legacy default stream, which cannot be captured
     uint64_t graph_key = 0;
     int64_t graph_launches = 0;                            // kernels inside one replay
     bool graph_failed = false;
@@ -435,6 +437,7 @@ void pimd_destroy(pimd_ctx* ctx) {
     if (!ctx) return;
     cudaStreamSynchronize(ctx->stream);
     if (ctx->step_graph) cudaGraphExecDestroy(ctx->step_graph);
+    if (ctx->graph_stream) { cudaStreamDestroy(ctx->graph_stream); cudaEventDestroy(ctx->graph_ev); }
     if (ctx->model.aux_stream[0]) {
         for (int q = 0; q < Model::kChainStreams - 1; ++q) {
             cudaStreamSynchronize(ctx->model.aux_stream[q]);
@@ -950,6 +953,18 @@ int pimd_step(pimd_ctx* ctx, int64_t n_steps) {
     } else {
         // One captured launch sequence per step: {integrator launch of an inner step, force evaluation} becomes a CUDA
         // graph (the three streams of the fitting chain included) and is replayed n_steps - 1 times.
+        if (!ctx->graph_stream) {
+            CK(cudaStreamCreateWithFlags(&ctx->graph_stream, cudaStreamNonBlocking));
+            CK(cudaEventCreateWithFlags(&ctx->graph_ev, cudaEventDisableTiming));
+        }
+        // hand over from the caller's stream: everything issued so far (snapshot copies, memsets) precedes the loop
+        CK(cudaEventRecord(ctx->graph_ev, ctx->stream));
+        CK(cudaStreamWaitEvent(ctx->graph_stream, ctx->graph_ev, 0));
+        struct StreamSwap {
+            pimd_ctx* c; cudaStream_t user;
+            StreamSwap(pimd_ctx* c_) : c(c_), user(c_->stream) { c->stream = c->graph_stream; }
+            ~StreamSwap() { cudaStreamSynchronize(c->graph_stream); c->stream = user; }
+        } swap(ctx);
         const long long ctl_h[2] = {(long long)ctx->step, (long long)(ctx->step + first_hist)};
         CK(cudaMemcpyAsync(ctx->ctl_dev, ctl_h, sizeof(ctl_h), cudaMemcpyHostToDevice, ctx->stream));
         integ(0, true);
@@ -972,7 +987,10 @@ int pimd_step(pimd_ctx* ctx, int64_t n_steps) {
             ctx->launches = l0; ctx->evals_launched = e0;     // a capture launches nothing
             if (ok) ok = cudaGraphInstantiate(&ctx->step_graph, g, 0) == cudaSuccess;
             if (g) cudaGraphDestroy(g);
-            if (!ok) { ctx->step_graph = nullptr; ctx->graph_failed = true; cudaGetLastError(); }
+            if (!ok) {
+                ctx->step_graph = nullptr; ctx->graph_failed = true;
+                ctx->err = std::string("graph capture failed, plain launches used: ") + cudaGetErrorString(cudaGetLastError());
+            }
             ctx->graph_key = key;
         }
         for (int64_t s = 1; s < n_steps; ++s) {
@@ -1205,6 +1223,11 @@ int pimd_debug_gemm(pimd_ctx* ctx, int M, int N, int K, const float* A, const fl
     if (rc != 0) return fail(ctx, PIMD_EINVAL, "debug gemm: unsupported shape or tensor-map failure");
     if (e != cudaSuccess) return fail(ctx, PIMD_ECUDA, std::string("debug gemm: ") + cudaGetErrorString(e));
     return PIMD_OK;
+}
+
+int pimd_debug_graph_state(const pimd_ctx* ctx) {
+    if (!ctx) return PIMD_EINVAL;
+    return ctx->step_graph ? 1 : (ctx->graph_failed ? -100 : 0);
 }
 
 int pimd_set_profiling(pimd_ctx* ctx, int on) {

@@ -200,6 +200,37 @@ def test_estimator_history_every_step(pk):
     sim.close()
 
 
+def test_step_loop_is_replayed_as_a_cuda_graph_and_matches_plain_launches(pk):
+    """pimd_step(n >= 3) with the se_e2_a model replays one captured {integrator, force evaluation} sequence; the
+    trajectory and the per-step estimator history equal those of step(1) calls (plain launches) to rounding."""
+    cfg, wb, desc, w = workloads.make_config(0)
+    args = (wb["types"], wb["masses"], wb["box"], cfg["P"], cfg["T"], cfg["dt"], cfg["gamma"])
+    a = pk.PIMD(*args, seed=3, model_desc=desc)
+    a.set_state(wb["x"], wb["p"])
+    a.set_model(w)
+    assert pk.pimd_debug_graph_state(a.ctx) == 0
+    a.step(6)
+    assert pk.pimd_debug_graph_state(a.ctx) == 1
+    b = pk.PIMD(*args, seed=3, model_desc=desc)
+    b.set_state(wb["x"], wb["p"])
+    b.set_model(w)
+    hb = []
+    for _ in range(6):
+        b.step(1)
+        hb.append(b.estimators())
+    assert pk.pimd_debug_graph_state(b.ctx) == 0
+    assert _rel(a.positions(), b.positions()) < 1e-12 and _rel(a.momenta(), b.momenta()) < 1e-11
+    ha = a.estimator_history()
+    assert [h["step"] for h in ha] == [1, 2, 3, 4, 5, 6]
+    for x, y in zip(ha, hb):
+        assert abs(x["K_CV"] - y["K_CV"]) <= 1e-9 * abs(y["K_CV"])
+        assert abs(x["H"] - y["H"]) <= 1e-7 * abs(y["H"])          # U is an FP32-network sum accumulated by atomics
+    a.step(4)                                             # the graph is reused by the next call
+    assert a.estimators()["step"] == 10
+    a.close()
+    b.close()
+
+
 def test_split_calls_equal_one_call_bitwise(pk):
     """step(3)+step(4) == step(7): the noise is keyed by the absolute step counter (R-10)."""
     N, P = 20, 4
