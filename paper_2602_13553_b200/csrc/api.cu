@@ -301,6 +301,10 @@ void fill_integrator_args(pimd_ctx* ctx, IntegratorArgs& a, int flags, int64_t s
     { const double wP = ctx->P * kKB * ctx->T / kHbar; a.wP2 = wP * wP; }
     if (ctx->method == PIMD_CART) a.flags |= I_CART;
     a.ctl = nullptr;
+    {
+        static const char* pf = getenv("PIMD_INT_PREFETCH");          // blocks per SM ahead (measured best: 1)
+        a.prefetch_ahead = (pf ? atoi(pf) : 1) * ctx->n_sms;
+    }
     a.est_base = ctx->est;
     a.est_scratch = ctx->est + (size_t)(kEstCap + 1) * kEstWidth;
 }

@@ -59,6 +59,7 @@ struct IntegratorArgs {
     // read from the device -- ctl[0] = the step this launch opens (advanced once per force evaluation by
     // wrap_bin_kernel), ctl[1] = the absolute step whose estimators go to history slot 0 -- so that one captured
     // launch sequence serves every step of a pimd_step call.
+    int      prefetch_ahead;     // blocks ahead whose inputs this block prefetches into L2 (0 = none)
     const long long* ctl;
     double*  est_base;           // estimator history [kEstCap][kEstWidth]
     double*  est_scratch;        // slot for steps outside the recorded window
@@ -98,6 +99,7 @@ inline void ensure_dyn_smem(K kernel, int bytes) { ensure_dyn_smem_impl(reinterp
 size_t barostat_state_doubles(int n_dof);    // BS_WIDTH + the partials
 
 int launch_integrator(int P, const IntegratorArgs& a, const ModeConsts& mc, cudaStream_t s);
+int launch_integrator4(int P, const IntegratorArgs& a, const ModeConsts& mc, cudaStream_t s);   // 0: not taken
 int launch_cart_convert(int P, int N, const double* in, const double* mass, double* out, int forward, cudaStream_t s);
 int launch_to_nm_velocity(int P, int N, const double* p_cart, const double* mass, double* vt, cudaStream_t s);
 int launch_from_nm_momenta(int P, int N, const double* vt, const double* mass, double* p_cart, cudaStream_t s);
@@ -114,7 +116,8 @@ struct NeighSlotB { float ds, rinv; uint32_t jcode; float pad; };   // jcode = j
 
 struct Model {
     bool     set = false;
-    static constexpr int kChainStreams = 3; // tile ranges of the fitting chain run on this many streams (fitting_tc.cu)
+    static constexpr int kChainStreams = 8; // at most; tile ranges of the fitting chain run on chain_streams streams (fitting_tc.cu)
+    int      chain_streams = 4;             // measured at configs[2]: 1: 0.613, 2: 0.542, 3: 0.543, 4: 0.532, 6: 0.550, 8: 0.549 ms
     cudaStream_t aux_stream[kChainStreams - 1] = {};
     cudaEvent_t  ev_fork = nullptr, ev_join[kChainStreams - 1] = {};
     pimd_model_desc d;

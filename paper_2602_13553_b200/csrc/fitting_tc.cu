@@ -13,6 +13,8 @@
 //   warps 2-5 split A into hi/lo in shared memory (elementwise, so the swizzled layout is preserved), then
 //            the epilogue: tcgen05.ld accumulators -> bias / tanh / skip / derivative / energy -> global
 // Two CTAs share an SM (2 x 256 TMEM columns, 2 x 2 stages), so one CTA's epilogue runs under the other's MMAs.
+#include <algorithm>
+#include <cstdlib>
 #include <cuda_fp16.h>
 #include "common.cuh"
 #include "tc_gemm.cuh"
@@ -894,14 +896,15 @@ int fitting_chain_tc(Model& m, const ForceArgs& fa, cudaStream_t s) {
     const int tiles = fill_types(m, fa.ntypes, g);
     ensure_dyn_smem(l1_desc_kernel, L1Smem::kTotal);
     ensure_dyn_smem(dd_dt_kernel, DdSmem::kTotal);
-    constexpr int NR = Model::kChainStreams;
     if (!m.aux_stream[0]) {
-        for (int q = 0; q < NR - 1; ++q) {
+        if (const char* e = getenv("PIMD_CHAIN_STREAMS")) m.chain_streams = std::min(std::max(atoi(e), 1), (int)Model::kChainStreams);
+        for (int q = 0; q < Model::kChainStreams - 1; ++q) {
             cudaStreamCreateWithFlags(&m.aux_stream[q], cudaStreamNonBlocking);
             cudaEventCreateWithFlags(&m.ev_join[q], cudaEventDisableTiming);
         }
         cudaEventCreateWithFlags(&m.ev_fork, cudaEventDisableTiming);
     }
+    const int NR = m.chain_streams;
     if (tiles < 2 * NR) {
         chain_range(m, fa, 0, tiles, s);
         return 6;

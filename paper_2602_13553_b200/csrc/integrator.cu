@@ -9,6 +9,7 @@
 //   x = M^T x~                                       Eq. B3
 // reads x, v~, f once and writes x, v~ once: 40 B per bead-atom-dim.
 #include "common.cuh"
+#include <cstdlib>
 #include <cuda_pipeline.h>
 #include "philox.cuh"
 
@@ -147,6 +148,21 @@ integrator_kernel(const __grid_constant__ IntegratorArgs a, const __grid_constan
 #pragma unroll
     for (int k = 0; k < P; ++k) __pipeline_memcpy_async(vs + k * kIntThreads, a.vt_in + k * stride + ec, sizeof(double));
     __pipeline_commit();
+
+    // The block that will take this block's place on the SM (blockIdx.x + one wave) finds its inputs in L2: the ALU
+    // phases of this kernel (O-step normals, transforms) and its memory phases do not overlap inside a block, and the
+    // two blocks an SM holds drift into lockstep, so HBM would idle while both compute.  One prefetch per 128 B line.
+    if ((threadIdx.x & 15) == 0) {
+        const long long e2 = (long long)e + (long long)a.prefetch_ahead * kIntThreads;
+        if (a.prefetch_ahead > 0 && e2 < (long long)a.n_dof) {
+#pragma unroll 8
+            for (int k = 0; k < P; ++k) {
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(a.f + k * stride + e2));
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(a.x_in + k * stride + e2));
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(a.vt_in + k * stride + e2));
+            }
+        }
+    }
 
     const double m = a.mass[i];
     double xt[P], ft[P];
@@ -474,6 +490,9 @@ int launch_cart_convert(int P, int N, const double* in, const double* mass, doub
 }
 
 int launch_integrator(int P, const IntegratorArgs& a, const ModeConsts& mc, cudaStream_t s) {
+    // north_star's layout -- four lanes per atom-dimension, shuffles for the transforms (integrator4.cu) -- is parity-correct
+    // but FP64-bound at twice this kernel's time; it runs only on request: PIMD_INT4=1
+    if (P >= 16 && getenv("PIMD_INT4") != nullptr && launch_integrator4(P, a, mc, s)) return 1;
     if (a.flags & I_CART) {
         switch (P) {
             case 1: launch_cart_t<1>(a, mc, s); break;

@@ -180,6 +180,32 @@ def test_full_step_parity_config0_obabo(pk):
     sim.close()
 
 
+@pytest.mark.parametrize("P", [16, 32, 64])
+def test_four_lane_integrator_variant_parity(pk, P, monkeypatch):
+    """north_star's layout (a group of four lanes owns the beads of an atom-dimension, shuffles for the transforms;
+    integrator4.cu) is the measured A/B partner of the default kernel: same parity bar."""
+    monkeypatch.setenv("PIMD_INT4", "1")
+    N = 37
+    types, masses, x, p = _random_system(N, P, seed=70 + P)
+    args = (types, masses, [30.0] * 3, P, 300.0, 0.25e-3, 5.0)
+    sim = pk.PIMD(*args, seed=99)
+    sim.set_state(x, p)
+    sim.set_model_harmonic(2.5)
+    orc = OraclePIMD(*args, seed=99)
+    orc.set_state(x, p)
+    orc.set_model_harmonic(2.5)
+    sim.step(1)
+    orc.step(1)
+    assert _rel(sim.positions(), orc.positions()) < 1e-10 and _rel(sim.momenta(), orc.momenta()) < 1e-10
+    sim.step(9)
+    orc.step(9)
+    assert _rel(sim.positions(), orc.positions()) < 1e-11 and _rel(sim.momenta(), orc.momenta()) < 1e-10
+    e, o = sim.estimators(), orc.estimators()
+    for key in ("K_PR", "K_CV", "H", "K_ring", "S_ring"):
+        assert abs(e[key] - o[key]) <= 1e-9 * max(1.0, abs(o[key])), key
+    sim.close()
+
+
 def test_estimator_history_every_step(pk):
     N, P = 50, 8
     types, masses, x, p = _random_system(N, P, seed=5)
