@@ -102,6 +102,10 @@ __device__ __forceinline__ void nm_inverse(double* a) {
 }
 
 constexpr int kIntThreads = 128;
+#ifndef PIMD_NOISE_WIDE
+#define PIMD_NOISE_WIDE 4
+#endif
+constexpr int kNoiseWide = PIMD_NOISE_WIDE;     // draws generated side by side (4: 0.927 ms at 2^20 x 32)
 
 // step counters (Philox counter words 0, 1; R-10) and estimator slot of a launch: launch arguments, or -- under graph
 // replay -- derived from the device-resident step counter
@@ -186,12 +190,27 @@ integrator_kernel(const __grid_constant__ IntegratorArgs a, const __grid_constan
             }
             return;
         }
+        if constexpr (P >= 8) {
+            // W draws side by side (philox.cuh): the dependent chains of a draw interleave
+            constexpr int W = kNoiseWide < P / 2 ? kNoiseWide : P / 2;
+#pragma unroll 1
+            for (int q = 0; q < P / 2; q += W) {
+                double ee[W], eo[W];
+                philox_normal_pairs<W>(a.seed_lo, a.seed_hi, s_lo, s_hi, (uint32_t)i, (uint32_t)(4 * q + alpha), ee, eo);
+#pragma unroll
+                for (int j = 0; j < W; ++j) {
+                    eta_s[(2 * (q + j)) * kIntThreads] = ee[j];
+                    eta_s[(2 * (q + j) + 1) * kIntThreads] = eo[j];
+                }
+            }
+        } else {
 #pragma unroll 4
-        for (int q = 0; q < (P + 1) / 2; ++q) {
-            double ee, eo;
-            philox_normal_pair(a.seed_lo, a.seed_hi, s_lo, s_hi, (uint32_t)i, (uint32_t)(4 * q + alpha), &ee, &eo);
-            eta_s[(2 * q) * kIntThreads] = ee;
-            if (2 * q + 1 < P) eta_s[(2 * q + 1) * kIntThreads] = eo;
+            for (int q = 0; q < (P + 1) / 2; ++q) {
+                double ee, eo;
+                philox_normal_pair(a.seed_lo, a.seed_hi, s_lo, s_hi, (uint32_t)i, (uint32_t)(4 * q + alpha), &ee, &eo);
+                eta_s[(2 * q) * kIntThreads] = ee;
+                if (2 * q + 1 < P) eta_s[(2 * q + 1) * kIntThreads] = eo;
+            }
         }
     };
     const bool thermo_close = kObabo && a.thermostat && (a.flags & I_BCLOSE);
@@ -615,8 +634,16 @@ __global__ void debug_noise_kernel(uint32_t seed_lo, uint32_t seed_hi, uint32_t 
     uint32_t w[4];
     philox4x32_10(step_lo, step_hi, i, 4u * (k >> 1) + al, seed_lo, seed_hi, w);
     for (int q = 0; q < 4; ++q) words[4 * t + q] = w[q];
+    // both generators of the library: the four-wide branch-free one (integrator kernels, P >= 8) for even entries of the
+    // request, the libm-based one (P < 8, barostat) for odd entries
     double ee, eo;
-    philox_normal_pair(seed_lo, seed_hi, step_lo, step_hi, i, 4u * (k >> 1) + al, &ee, &eo);
+    if (t & 1) {
+        philox_normal_pair(seed_lo, seed_hi, step_lo, step_hi, i, 4u * (k >> 1) + al, &ee, &eo);
+    } else {
+        double e4[4], o4[4];
+        philox_normal_pairs4(seed_lo, seed_hi, step_lo, step_hi, i, 4u * (k >> 1) + al, e4, o4);
+        ee = e4[0]; eo = o4[0];
+    }
     eta[t] = (k & 1u) ? eo : ee;
 }
 
