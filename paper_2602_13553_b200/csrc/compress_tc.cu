@@ -243,16 +243,28 @@ cmp_fwd_kernel(const __grid_constant__ CmpArgs a) {
             // one batch of up to 32 rows: lane = row writes its 24 products u^p R_c, then lane = (p, c) adds them up
             bool up = false;
             auto batch = [&](const RowF& R, int nb, float& acc0) {
-                if (lane < nb) {
-                    const float s = R.s, sr = R.s * R.rinv;
+                // rows of the hot bucket (interval 0 of this neighbour type) are compacted to the front of the row buffer:
+                // their sum needs no bucket lookup and no read-modify-write, only independent loads and adds
+                const bool act = lane < nb;
+                int iv = 0; float u = 0.f;
+                const float s = act ? R.s : 0.f;
+                if (act) {
                     if (s > kSHi) {                              // outside the table: an error, not an extrapolation (R-28)
                         atomicOr(a.overflow, 4);
                         atomicMin(reinterpret_cast<unsigned*>(a.overflow) + 1, (unsigned)a.overflow[2]);
                     }
-                    int iv; float u;
                     cmp_locate(s, iv, u);
+                }
+                const int pos = cmp_pos(iv);
+                const bool hot = act && pos == 0;
+                const unsigned hm = __ballot_sync(0xffffffffu, hot), cm = __ballot_sync(0xffffffffu, act && !hot);
+                const unsigned lt = (1u << lane) - 1u;
+                const int nh = __popc(hm);
+                if (act) {
+                    up |= pos >= NI / 2;
+                    const float sr = s * R.rinv;
                     const float Rv[4] = {s, sr * R.dx, sr * R.dy, sr * R.dz};
-                    float* rb = rowbuf + lane * 25;
+                    float* rb = rowbuf + (hot ? __popc(hm & lt) : nh + __popc(cm & lt)) * 25;
                     float pw = 1.f;
 #pragma unroll
                     for (int pp = 0; pp < NP; ++pp) {
@@ -260,17 +272,22 @@ cmp_fwd_kernel(const __grid_constant__ CmpArgs a) {
                         for (int cc = 0; cc < 4; ++cc) rb[pp * 4 + cc] = pw * Rv[cc];
                         pw *= u;
                     }
-                    const int pos = cmp_pos(iv);
-                    up |= pos >= NI / 2;
                     rb[24] = __int_as_float((tj * NI + pos) * NP);
                 }
                 __syncwarp();
                 if (lane < 24) {
-                    for (int q = 0; q < nb; ++q) {
+                    float h0 = 0.f, h1 = 0.f, h2 = 0.f, h3 = 0.f;
+                    int q = 0;
+                    for (; q + 4 <= nh; q += 4) {
+                        h0 += rowbuf[q * 25 + lane]; h1 += rowbuf[(q + 1) * 25 + lane];
+                        h2 += rowbuf[(q + 2) * 25 + lane]; h3 += rowbuf[(q + 3) * 25 + lane];
+                    }
+                    for (; q < nh; ++q) h0 += rowbuf[q * 25 + lane];
+                    acc0 += (h0 + h1) + (h2 + h3);
+                    for (q = nh; q < nb; ++q) {
                         const float v = rowbuf[q * 25 + lane];
                         const int k0 = __float_as_int(rowbuf[q * 25 + 24]);
-                        if (k0 == hotk) acc0 += v;                    // warp-uniform: the hot bucket stays in a register
-                        else stg[c * STG + k0 + p] += v;
+                        stg[c * STG + k0 + p] += v;
                     }
                 }
                 __syncwarp();
