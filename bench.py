@@ -276,19 +276,36 @@ def run_ours(args):
         time.sleep(0.25)
     barrier()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    # The synthetic workload has no binding potential (random-init weights, forces ~1e-4 eV/A): its atoms drift freely
+    # and after ~200 steps two of them overlap (r < 0.01 A), which the library reports as PIMD_ECONTACT.  Long runs are
+    # therefore cut into chunks of at most CHUNK steps, each restarted (untimed) from the initial configuration.
+    CHUNK = 100
+
+    def timed_steps(n_total):
+        ms_sum, done = 0.0, 0
+        while done < n_total:
+            n = min(CHUNK, n_total - done)
+            if done > 0:
+                sim.set_state(x_dev, p_dev)
+                barrier()
+            ev0.record()
+            sim.step(n)                             # ONE pimd_step(n) call: n whole steps, no host round trip inside
+            ev1.record()
+            barrier()
+            ms_sum += ev0.elapsed_time(ev1)
+            done += n
+        return ms_sum
+
     t_wall0 = time.time()
-    ev0.record()
-    sim.step(args.steps)                            # ONE pimd_step(K) call: K whole steps, no host round trip inside
-    ev1.record()
-    barrier()
+    ms = timed_steps(args.steps)
     t_wall1 = time.time()
-    ms = ev0.elapsed_time(ev1)
     launches = pk.pimd_get_launch_count(sim.ctx) - launches0
     clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
     ms = max_over_ranks(ms, world, "cuda")
     value = job_throughput(P * N * args.steps, world, ms)
 
     # ---- per-phase device times (CUDA events on the library's stream) ----
+    sim.set_state(x_dev, p_dev)
     pk.pimd_set_profiling(sim.ctx, 1)
     sim.step(max(3, min(10, args.steps)))
     phase = pk.pimd_get_phase_ms(sim.ctx)
@@ -350,15 +367,19 @@ def run_ours(args):
             time.sleep(0.25)
         barrier()
         tw0 = time.time()
-        ev0.record()
-        n_sus = 0
+        n_sus, ms_sus, per = 0, 0.0, min(per, CHUNK)
         while time.time() - tw0 < args.sustain_s:
+            sim.set_state(x_dev, p_dev)             # restart (see CHUNK above); its one force evaluation is not timed
+            torch.cuda.synchronize()
+            ev0.record()
             sim.step(per)
+            ev1.record()
+            torch.cuda.synchronize()
+            ms_sus += ev0.elapsed_time(ev1)
             n_sus += per
-        ev1.record()
         barrier()
         tw1 = time.time()
-        ms_sus = max_over_ranks(ev0.elapsed_time(ev1), world, "cuda")
+        ms_sus = max_over_ranks(ms_sus, world, "cuda")
         sustained = {"value": job_throughput(P * N * n_sus, world, ms_sus), "unit": METRIC, "steps": n_sus,
                      "seconds": ms_sus * 1e-3, "ms_per_step": ms_sus / n_sus,
                      "clocks": sampler2.stop(tw0, tw1) if rank == 0 else None}
@@ -432,6 +453,7 @@ def run_ours(args):
 
     # ---- end to end through the C ABI with host buffers ----
     f_host = torch.empty_like(x_host).pin_memory()
+    sim.set_state(x_dev, p_dev)                     # fresh configuration (see CHUNK above)
     xo, po, fo = sim.positions(), sim.momenta(), sim.forces()
     Uo = sim.energies()
     x_host.copy_(torch.from_numpy(xo)); p_host.copy_(torch.from_numpy(po)); f_host.copy_(torch.from_numpy(fo))
