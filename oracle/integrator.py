@@ -170,6 +170,14 @@ def remove_centroid_com(vt, masses):
     return out
 
 
+def remove_bead_com(v, masses):
+    """`fixcom yes` under `method pimd`: the center-of-mass velocity is removed "for each bead
+    individually".  v_k,i <- v_k,i - sum_j m_j v_k,j / sum_j m_j for every bead k, per Cartesian component; applied once
+    per step after its last velocity update, like the centroid variant (DESIGN R-19).  v[P,N,3] Cartesian."""
+    vcom = np.sum(masses[None, :, None] * v, axis=1) / np.sum(masses)          # [P, 3]
+    return v - vcom[:, None, :]
+
+
 def estimators(x, vt, f, U, masses, M, om, T):
     """Appendix A outputs that the hot path reports, on unwrapped coordinates
     (L202).  x, f Cartesian [P,N,3]; vt normal-mode velocities; U[P] bead potential energies.

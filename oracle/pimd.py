@@ -29,7 +29,6 @@ class OraclePIMD:
         self.fixcom = bool(fixcom)
         assert method in ("nmpimd", "pimd")
         self.method = method                             # PAPER.md:L164; "pimd" = Cartesian (DESIGN R-27)
-        assert not (self.method == "pimd" and self.fixcom)
         self.M = nm.nm_matrix(self.P)
         self.om = nm.omegas(self.P, self.T)
         self.step_count = 0
@@ -170,6 +169,8 @@ class OraclePIMD:
         self._forces()
         self.vt = integrator.cart_finish(self.x, self.vt, self.f, self.masses, self.T, wP, self.gamma0, self.dt,
                                          self.seed, self.step_count, ob)
+        if self.fixcom:
+            self.vt = integrator.remove_bead_com(self.vt, self.masses)      # L180: "for each bead individually"
         self.step_count += 1
 
     def step(self, n_steps=1):

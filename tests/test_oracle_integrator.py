@@ -221,6 +221,37 @@ def test_fixcom_removes_exactly_the_centroid_momentum(integ):
     assert np.abs(np.sum(m[:, None] * o.vt[0], axis=0)).max() < 1e-12 * np.abs(m[:, None] * o.vt[0]).max()
 
 
+@pytest.mark.parametrize("integ", ["baoab", "obabo"])
+def test_fixcom_under_the_cartesian_method_removes_every_beads_momentum(integ):
+    """fixcom under `method pimd` ("for each bead individually"): after every step the total momentum of
+    EVERY bead vanishes; within a step the run differs from the fixcom-free one by one uniform velocity shift per bead
+    (= that bead's centre-of-mass velocity), positions are untouched, and a second removal is a no-op."""
+    P, T, dt, N = 4, 300.0, 0.2e-3, 7
+    rng = np.random.default_rng(19)
+    masses_t = [15.9994, 1.008]
+    types = rng.integers(0, 2, N)
+    o = OraclePIMD(types, masses_t, [50.0] * 3, P, T, dt, 5.0, 3, integrator=integ, fixcom=True, method="pimd")
+    ref = OraclePIMD(types, masses_t, [50.0] * 3, P, T, dt, 5.0, 3, integrator=integ, fixcom=False, method="pimd")
+    x0, p0 = 0.1 * rng.standard_normal((P, N, 3)), 20 * rng.standard_normal((P, N, 3))
+    for sim in (o, ref):
+        sim.set_model_harmonic(1.5)
+        sim.set_state(x0, p0)
+        sim.step(1)
+    m = o.masses
+    pk = np.sum(m[None, :, None] * o.vt, axis=1)                     # [P, 3]
+    assert np.abs(pk).max() < 1e-12 * np.abs(m[None, :, None] * o.vt).max()
+    shift = ref.vt - o.vt                                            # uniform over the atoms of a bead
+    assert np.abs(shift - shift[:, :1]).max() < 1e-12 * np.abs(ref.vt).max()
+    vcom = np.sum(m[None, :, None] * ref.vt, axis=1) / m.sum()
+    assert np.abs(shift[:, 0] - vcom).max() < 1e-12 * np.abs(ref.vt).max()
+    assert np.ptp(vcom, axis=0).max() > 0                            # the beads' shifts differ: not the centroid variant
+    assert np.array_equal(o.x, ref.x)
+    again = integrator.remove_bead_com(o.vt, m)
+    assert np.abs(again - o.vt).max() < 1e-13 * np.abs(o.vt).max()
+    o.step(5)
+    assert np.abs(np.sum(m[None, :, None] * o.vt, axis=1)).max() < 1e-12 * np.abs(m[None, :, None] * o.vt).max()
+
+
 def test_nve_energy_is_conserved_with_dt2_scaling():
     T, P, N = 300.0, 16, 20
     drift = []
