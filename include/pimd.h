@@ -193,12 +193,14 @@ int pimd_set_integrator(pimd_ctx* ctx, int kind);
  * force of Eq. 1, A is the drift x += h v, and the thermostat is Eq. D3 (L478-484): the same tau = 1/(2 omega_n) on
  * every bead, normals keyed by the bead index (DESIGN R-27); both splittings; estimators as in Appendix A.  Call it
  * BEFORE pimd_set_state: a change of method drops the state (the stored velocities change representation).
- * PIMD_EINVAL for an unknown method, or for PIMD_CART with fixcom or a barostat on (and those refuse under PIMD_CART). */
+ * PIMD_EINVAL for an unknown method, or for PIMD_CART with a barostat on (and the barostat refuses under PIMD_CART).
+ * fixcom under PIMD_CART removes the centre-of-mass velocity of EACH BEAD. */
 #define PIMD_NMPIMD 0
 #define PIMD_CART 1
 int pimd_set_method(pimd_ctx* ctx, int method);
 
-/* `fixcom`: when on, the centre-of-mass velocity of the centroid mode is removed once per step,
+/* `fixcom`: when on, the centre-of-mass velocity of the centroid mode (PIMD_NMPIMD) or of every bead
+ * individually (PIMD_CART) is removed once per step,
  * after the step's last velocity update and before its estimators (DESIGN R-19).  Off by default (north_star's
  * create() list has no such argument).  The removal needs a reduction over all atoms between the closing and the
  * opening half of the fused integrator launch, so a step then costs two integrator launches instead of one. */

@@ -124,7 +124,7 @@ size_t base_bytes(const pimd_ctx* c) {
     size_t b = 0;
     b += 6 * align_up(PN3 * 8, 256);                          // x, vt, f, scratch_a, scratch_b, snap_f
     b += align_up(((size_t)c->P * 10 + BS_WIDTH) * 8, 256);   // snap_small
-    b += 256;                                                 // ctl_dev
+    b += 256 + align_up((size_t)3 * kMaxBeads * 8, 256);      // ctl_dev, com
     b += align_up((size_t)c->N * 8, 256) + align_up((size_t)c->N * 4, 256);
     b += align_up((size_t)c->P * 8, 256) + align_up((size_t)c->P * 72, 256) + align_up((size_t)c->P * c->N * 8, 256);
     b += align_up((size_t)(kEstCap + 2) * kEstWidth * 8, 256);
@@ -221,7 +221,7 @@ int alloc_base(pimd_ctx* ctx) {
     if ((rc = arena_alloc(ctx, &ctx->Xi, (size_t)ctx->P * 9))) return rc;
     if ((rc = arena_alloc(ctx, &ctx->Eatom, (size_t)ctx->P * ctx->N))) return rc;
     if ((rc = arena_alloc(ctx, &ctx->est, (size_t)(kEstCap + 2) * kEstWidth))) return rc;
-    if ((rc = arena_alloc(ctx, &ctx->com, (size_t)4))) return rc;
+    if ((rc = arena_alloc(ctx, &ctx->com, (size_t)3 * kMaxBeads))) return rc;      // nmpimd: [3]; Cartesian method: [P][3]
     std::vector<double> ma(ctx->N);
     double mtot = 0;
     for (int i = 0; i < ctx->N; ++i) { ma[i] = ctx->masses[ctx->types[i]]; mtot += ma[i]; }
@@ -645,8 +645,8 @@ int pimd_get_barostat_history(pimd_ctx* ctx, pimd_barostat_state* b, int cap) {
 int pimd_set_method(pimd_ctx* ctx, int method) {
     if (!ctx) return PIMD_EINVAL;
     if (method != PIMD_NMPIMD && method != PIMD_CART) return fail(ctx, PIMD_EINVAL, "unknown method");
-    if (method == PIMD_CART && (ctx->baro || ctx->fixcom))
-        return fail(ctx, PIMD_EINVAL, "the Cartesian method is implemented without barostat and fixcom (DESIGN R-27)");
+    if (method == PIMD_CART && ctx->baro)
+        return fail(ctx, PIMD_EINVAL, "the Cartesian method is implemented without a barostat (DESIGN R-27)");
     if (method != ctx->method) ctx->have_state = false;      // the stored velocities change representation
     ctx->method = method;
     mode_constants(ctx);
@@ -655,7 +655,6 @@ int pimd_set_method(pimd_ctx* ctx, int method) {
 
 int pimd_set_fixcom(pimd_ctx* ctx, int on) {
     if (!ctx) return PIMD_EINVAL;
-    if (on && ctx->method == PIMD_CART) return fail(ctx, PIMD_EINVAL, "fixcom is not available with the Cartesian method (DESIGN R-27)");
     if (on && ctx->baro) return fail(ctx, PIMD_EINVAL, "fixcom is not available with the barostat (DESIGN R-24)");
     ctx->fixcom = on != 0;
     return PIMD_OK;
@@ -925,7 +924,7 @@ int pimd_step(pimd_ctx* ctx, int64_t n_steps) {
         if (ctx->fixcom && s > 0) {
             // fixcom (R-19): the removal needs sum_i m_i v~_0,i over ALL atoms after the closing half,
             // so the launch splits: close + accumulate, then subtract + estimators (+ open)
-            cudaMemsetAsync(ctx->com, 0, sizeof(double) * 3, ctx->stream);
+            cudaMemsetAsync(ctx->com, 0, sizeof(double) * 3 * (ctx->method == PIMD_CART ? ctx->P : 1), ctx->stream);
             fill_integrator_args(ctx, a, I_BCLOSE | I_COMACC, ctx->step + s, scratch);
             if (ctl_mode) a.ctl = ctx->ctl_dev;
             ctx->launches += launch_integrator(ctx->P, a, ctx->mc, ctx->stream);

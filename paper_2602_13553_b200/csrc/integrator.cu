@@ -416,6 +416,10 @@ integrator_cart_kernel(const __grid_constant__ IntegratorArgs a, const __grid_co
         g[k] = kick * g[k] - hh * a.wP2 * lap;
     }
     const double cv_term = xf - (sx / (double)P) * sf;   // A9: sum_k (r_k - r_c).F_k
+    if (a.flags & I_COMSUB) {                            // fixcom, "for each bead individually"
+#pragma unroll
+        for (int k = 0; k < P; ++k) v[k] -= a.com[3 * k + alpha] * a.inv_mtot;
+    }
     if (close) {
 #pragma unroll
         for (int k = 0; k < P; ++k) v[k] += g[k];        // closing B(dt/2)
@@ -424,6 +428,17 @@ integrator_cart_kernel(const __grid_constant__ IntegratorArgs a, const __grid_co
 #pragma unroll
             for (int k = 0; k < P; ++k) v[k] = mc.c1[0] * v[k] + mc.c2[0] * sigma * eta_s[k * kIntThreads];
         }
+    }
+    if (a.flags & I_COMACC) {                            // sum_i m_i v_k,i per bead and component -> com[3k + alpha]
+        __shared__ double s_com[3 * P];
+        for (int q = threadIdx.x; q < 3 * P; q += kIntThreads) s_com[q] = 0.0;
+        __syncthreads();
+        if (live) {
+#pragma unroll
+            for (int k = 0; k < P; ++k) atomicAdd(&s_com[3 * k + alpha], m * v[k]);
+        }
+        __syncthreads();
+        for (int q = threadIdx.x; q < 3 * P; q += kIntThreads) atomicAdd(a.com + q, s_com[q]);
     }
     double accK = 0.0;
 #pragma unroll
@@ -448,7 +463,7 @@ integrator_cart_kernel(const __grid_constant__ IntegratorArgs a, const __grid_co
             }
         }
     }
-    if (live && (close || start)) {
+    if (live && (close || start || (a.flags & I_COMSUB))) {
 #pragma unroll
         for (int k = 0; k < P; ++k) a.vt_out[k * stride + ec] = v[k];
     }

@@ -858,6 +858,37 @@ def test_cartesian_method_full_step_parity_config0(pk):
     sim.close()
 
 
+@pytest.mark.parametrize("integ", ["baoab", "obabo"])
+@pytest.mark.parametrize("P", [1, 8, 32])
+def test_cartesian_method_fixcom_removes_every_beads_momentum(pk, integ, P):
+    """fixcom under `method pimd` ("for each bead individually"): trajectories follow the oracle and the
+    total momentum of every bead vanishes after every step."""
+    N = 301
+    types, masses, x, p = _random_system(N, P, seed=60 + P)
+    args = (types, masses, [30.0] * 3, P, 300.0, 0.1e-3, 5.0)
+    sim = pk.PIMD(*args, seed=7, integrator=integ, fixcom=True, method="pimd")
+    sim.set_state(x, p)
+    sim.set_model_harmonic(2.5)
+    orc = OraclePIMD(*args, seed=7, integrator=integ, fixcom=True, method="pimd")
+    orc.set_state(x, p)
+    orc.set_model_harmonic(2.5)
+    sim.step(1)
+    orc.step(1)
+    assert _rel(sim.positions(), orc.positions()) < 1e-10 and _rel(sim.momenta(), orc.momenta()) < 1e-10
+    pb = sim.momenta().sum(axis=1)
+    assert np.abs(pb).max() < 1e-10 * np.abs(sim.momenta()).max() * N ** 0.5
+    sim.step(3)
+    sim.step(2)
+    orc.step(5)
+    assert _rel(sim.positions(), orc.positions()) < 1e-10 and _rel(sim.momenta(), orc.momenta()) < 1e-9
+    pb = sim.momenta().sum(axis=1)
+    assert np.abs(pb).max() < 1e-10 * np.abs(sim.momenta()).max() * N ** 0.5
+    e, o = sim.estimators(), orc.estimators()
+    for key in ("K_PR", "K_CV", "H", "K_ring", "S_ring"):
+        assert abs(e[key] - o[key]) <= 1e-9 * max(1.0, abs(o[key])), key
+    sim.close()
+
+
 def test_cartesian_method_argument_rules(pk):
     types, masses, x, p = _random_system(5, 4, seed=1)
     sim = pk.PIMD(types, masses, [30.0] * 3, 4, 300.0, 1e-4, 1.0, seed=1)
@@ -866,8 +897,6 @@ def test_cartesian_method_argument_rules(pk):
     pk.pimd_set_method(sim.ctx, "pimd")
     with pytest.raises(pk.PimdError):
         sim.step(1)                                  # the change of representation dropped the state
-    with pytest.raises(pk.PimdError):
-        pk.pimd_set_fixcom(sim.ctx, True)
     with pytest.raises(pk.PimdError):
         sim.set_barostat(1.0, 0.1)
     with pytest.raises(pk.PimdError):
