@@ -12,7 +12,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpimd_b200.so")
-SOURCES = ["api.cu", "integrator.cu", "integrator4.cu", "barostat.cu", "neighbor.cu", "embedding.cu", "embedding_tc.cu", "compress_tc.cu", "fitting.cu", "fitting_tc.cu"]
+SOURCES = ["api.cu", "integrator.cu", "integrator4.cu", "barostat.cu", "neighbor.cu", "embedding.cu", "embedding_tc.cu", "compress_tc.cu", "fitting.cu", "fitting_tc.cu", "fitting_mid.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 

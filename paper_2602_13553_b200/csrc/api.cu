@@ -158,6 +158,7 @@ size_t model_bytes(const pimd_ctx* c, const pimd_model_desc* d) {
     b += (size_t)d->n_types * 4 * align_up((size_t)ND * NF * 2, 256);                  // FP16-split layer-1 images
     b += (size_t)d->n_types * 6 * (align_up((size_t)ND * NF * 4, 256) + 2 * align_up((size_t)NF * NF * 4, 256) + align_up(NF * 4, 256));
     b += (size_t)d->n_types * 4 * align_up((size_t)NF * 4, 256);
+    b += (size_t)d->n_types * 8 * align_up((size_t)NF * NF * 2, 256);                  // FP16-split operands of the fused middle
     b += 4 * align_up(PN * 4, 256);                                                    // cen_idx,row_of,cell_id,cell_tmp
     b += 3 * align_up((size_t)c->P * (ncells + 1) * 4, 256);
     b += align_up(PN * 24, 256) + align_up(PN * 32, 256);
@@ -783,6 +784,14 @@ int pimd_set_model(pimd_ctx* ctx, const pimd_model_desc* d, const double* w, siz
                     if ((rc = arena_alloc(ctx, &m.w1T_h_lo[t], W.size()))) return rc;
                     tc_split_weights_h(W.size(), m.fit_w[t][l], 64.f, m.w1_h_hi[t], m.w1_h_lo[t], ctx->stream);
                     tc_split_weights_h(W.size(), m.fit_wT[t][l], 64.f, m.w1T_h_hi[t], m.w1T_h_lo[t], ctx->stream);
+                } else {          // FP16-split operands of the fused middle (fitting_mid.cu): phases W2^T, W3^T, W3, W2
+                    const int pf = l - 1, pb = 4 - l;
+                    for (int h = 0; h < 2; ++h) {
+                        if ((rc = arena_alloc(ctx, &m.wmid_h[t][pf][h], W.size()))) return rc;
+                        if ((rc = arena_alloc(ctx, &m.wmid_h[t][pb][h], W.size()))) return rc;
+                    }
+                    tc_split_weights_h(W.size(), m.fit_wT[t][l], 64.f, m.wmid_h[t][pf][0], m.wmid_h[t][pf][1], ctx->stream);
+                    tc_split_weights_h(W.size(), m.fit_w[t][l], 64.f, m.wmid_h[t][pb][0], m.wmid_h[t][pb][1], ctx->stream);
                 }
             }
             keep.push_back(std::move(W)); keep.push_back(std::move(WT)); keep.push_back(std::move(b));
@@ -851,7 +860,8 @@ int pimd_set_model(pimd_ctx* ctx, const pimd_model_desc* d, const double* w, siz
         CK(cudaMemcpyAsync(m.overflow, ov0, sizeof(ov0), cudaMemcpyHostToDevice, ctx->stream));
     }
     CK(cudaStreamSynchronize(ctx->stream));     // host staging vectors go out of scope below
-    tc_setup_maps(m, nt);        // tensor-core fitting path (falls back to the CUDA-core GEMMs only if unsupported widths)
+    if (tc_setup_maps(m, nt))    // tensor-core fitting path (falls back to the CUDA-core GEMMs only if unsupported widths)
+        fitting_mid_setup(m, nt);
     m.set = true;
     ctx->model_kind = 2;
     return refresh(ctx);

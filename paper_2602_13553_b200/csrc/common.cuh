@@ -170,6 +170,12 @@ struct Model {
     CUtensorMap mapAh_G1[PIMD_MAX_TYPES], mapAh_G2[PIMD_MAX_TYPES];           // da1 as FP16 hi / lo (x bwd_scale)
     uint16_t* da1_h_hi = nullptr, *da1_h_lo = nullptr;   // [rows][240] halfs, carved out of D
     float    bwd_scale = 1.f;          // power of two that brings the backward activations to O(1..16)
+    // fused middle of the fitting chain (fitting_mid.cu): y1 as FP16 hi / lo (carved out of Y1), the four 240 x 240
+    // weight operands (W2^T, W3^T, W3, W2) x 64 as FP16 hi / lo, and their TMA maps
+    bool     mid_ready = false;
+    uint16_t* y1_h_hi = nullptr, *y1_h_lo = nullptr;
+    uint16_t* wmid_h[PIMD_MAX_TYPES][4][2];
+    CUtensorMap mapMidA_hi[PIMD_MAX_TYPES], mapMidA_lo[PIMD_MAX_TYPES], mapMidB[PIMD_MAX_TYPES][4][2];
     // tensor-core embedding path (embedding_tc.cu)
     bool     use_tc_emb = true;
     bool     tc_emb_ready = false;
@@ -207,6 +213,10 @@ bool tc_setup_maps(Model& m, int ntypes);
 void tc_split_weights(size_t n, const float* w, float* hi, float* lo, cudaStream_t s);
 void tc_split_weights_h(size_t n, const float* w, float scale, uint16_t* hi, uint16_t* lo, cudaStream_t s);
 int fitting_chain_tc(Model& m, const ForceArgs& a, cudaStream_t s);
+bool tc_make_map_h(CUtensorMap* map, const uint16_t* base, uint64_t rows, uint64_t cols, uint64_t ld, uint32_t box_rows);
+bool tc_make_map_h16(CUtensorMap* map, const uint16_t* base, uint64_t rows, uint64_t cols, uint64_t ld, uint32_t box_rows);
+bool fitting_mid_setup(Model& m, int ntypes);
+void fitting_mid_launch(Model& m, const ForceArgs& a, int tile_off, int ntiles, cudaStream_t s);
 size_t emb_tc_image_h_bytes();
 void emb_tc_build_image_h(const double* w_pair, uint8_t* img);
 int emb_tc_row_index(Model& m, const ForceArgs& a, cudaStream_t s);

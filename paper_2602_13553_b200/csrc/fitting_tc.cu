@@ -329,7 +329,8 @@ struct L1Args {
     int row0[kMaxT + 1];
     const float* bias[kMaxT];
     const float* Tm;      // [rows][100][4]
-    float* out; int ldo;  // Y1
+    float* out; int ldo;  // Y1 (FP32), or
+    __half* out_hi; __half* out_lo;   // Y1 as an FP16 hi / lo pair for fit_mid_kernel (when out_hi is set)
     int M1;
 };
 
@@ -338,6 +339,7 @@ struct L1Args {
 // construction (|G| <= 3, |R| <= ~1.2, at most N_sel rows), so 256 |D| < 65504 -- and the epilogue multiplies the
 // accumulator by 2^-14.  A stage holds K = 32 (two m1 values): 50 stages of 6 MMAs instead of 100.
 constexpr int kL1BN = 240, kL1ST = 4;
+constexpr int kL1Threads = 320;         // warp 0: TMA, warp 1: MMA issue, warps 2-9: operand producers + epilogue
 constexpr float kL1DScale = 256.f, kW1Scale = 64.f;
 struct L1Smem {
     static constexpr int kABytes = 128 * 64, kBBytes = kL1BN * 64;        // 64 B rows = 32 halfs, SWIZZLE_64B
@@ -347,7 +349,7 @@ struct L1Smem {
     static constexpr int kTotal = oBars + 256 + 1024;
 };
 
-__global__ void __launch_bounds__(kTcThreads, 1)
+__global__ void __launch_bounds__(kL1Threads, 1)
 l1_desc_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ L1Args g) {
     using SM = L1Smem;
     constexpr int ST = kL1ST, BN = kL1BN;
@@ -375,7 +377,7 @@ l1_desc_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ L1Ar
     if (warp == 0 && lane == 0) {
         tma_prefetch_desc(mapBhi);
         tma_prefetch_desc(mapBlo);
-        for (int s = 0; s < ST; ++s) { mbar_init(full + s, 1); mbar_init(ready + s, 128); mbar_init(empty + s, 1); }
+        for (int s = 0; s < ST; ++s) { mbar_init(full + s, 1); mbar_init(ready + s, 256); mbar_init(empty + s, 1); }
         mbar_init(tmem_full, 1);
         fence_barrier_init();
     }
@@ -420,7 +422,10 @@ l1_desc_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ L1Ar
             umma_commit(tmem_full);
         }
     } else {
-        const int quarter = warp & 3;
+        // two warps per TMEM lane quarter (a warp alone on its scheduler cannot hide the latency of its own loads and
+        // conversions; the round-2 profile had the tensor pipe 46 % active behind four producer warps): warp `half`
+        // of a quarter produces m1 = 2 kb + half of every stage and takes the epilogue chunks c = half, half + 2, ...
+        const int quarter = warp & 3, half = (warp - 2) >> 2;
         const int row = quarter * 32 + lane;                   // tile row = TMEM lane
         const int ml = m0 + row;
         const bool row_ok = ml < rows_t;
@@ -435,18 +440,17 @@ l1_desc_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ L1Ar
         }
         // SWIZZLE_64B K-major block: 64 B rows (32 halfs), 16 B chunk index XOR ((row >> 1) & 3)
         const int rbase = row * 64, sw = (row >> 1) & 3;
-        float4 T1a = row_ok ? __ldg(Trow) : zero4, T1b = row_ok ? __ldg(Trow + 1) : zero4;
+        auto load_T1 = [&](int kb) { return (row_ok && kb < nk) ? __ldg(Trow + 2 * kb + half) : zero4; };
+        float4 Ta = load_T1(0), Tb = load_T1(1), Tc = load_T1(2);          // T[i][m1] three stages ahead of its use
         for (int kb = 0; kb < nk; ++kb) {
             const int s = kb % ST, ph = (kb / ST) & 1;
-            const bool more = row_ok && kb + 1 < nk;
-            const float4 T1an = more ? __ldg(Trow + 2 * kb + 2) : zero4, T1bn = more ? __ldg(Trow + 2 * kb + 3) : zero4;
-            uint32_t hi[16], lo[16];                            // 32 halfs each, packed in pairs
+            const float4 Tn = load_T1(kb + 3);
+            uint32_t hi[8], lo[8];                              // K indices 16 half .. 16 half + 15 of the stage, packed in pairs
 #pragma unroll
-            for (int q = 0; q < 16; ++q) {                      // K index 2q, 2q+1: m1 = 2 kb + (q >> 3), m2 = 2 (q & 7) ..
-                const float4 T1 = (q < 8) ? T1a : T1b;
-                const int m2 = 2 * (q & 7);
-                const float d0 = T1.x * T2[m2].x + T1.y * T2[m2].y + T1.z * T2[m2].z + T1.w * T2[m2].w;
-                const float d1 = T1.x * T2[m2 + 1].x + T1.y * T2[m2 + 1].y + T1.z * T2[m2 + 1].z + T1.w * T2[m2 + 1].w;
+            for (int q = 0; q < 8; ++q) {
+                const int m2 = 2 * q;
+                const float d0 = Ta.x * T2[m2].x + Ta.y * T2[m2].y + Ta.z * T2[m2].z + Ta.w * T2[m2].w;
+                const float d1 = Ta.x * T2[m2 + 1].x + Ta.y * T2[m2 + 1].y + Ta.z * T2[m2 + 1].z + Ta.w * T2[m2 + 1].w;
                 const __half2 h = __floats2half2_rn(d0, d1);
                 const float2 hf = __half22float2(h);
                 const __half2 l = __floats2half2_rn(d0 - hf.x, d1 - hf.y);
@@ -456,14 +460,14 @@ l1_desc_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ L1Ar
             mbar_wait(empty + s, ph ^ 1);                       // the MMAs that read this stage have retired
             uint8_t* st = smem + s * SM::kStage;
 #pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                const int off = rbase + ((c ^ sw) << 4);
-                *reinterpret_cast<uint4*>(st + SM::oAhi + off) = make_uint4(hi[4 * c], hi[4 * c + 1], hi[4 * c + 2], hi[4 * c + 3]);
-                *reinterpret_cast<uint4*>(st + SM::oAlo + off) = make_uint4(lo[4 * c], lo[4 * c + 1], lo[4 * c + 2], lo[4 * c + 3]);
+            for (int c2 = 0; c2 < 2; ++c2) {
+                const int off = rbase + (((2 * half + c2) ^ sw) << 4);
+                *reinterpret_cast<uint4*>(st + SM::oAhi + off) = make_uint4(hi[4 * c2], hi[4 * c2 + 1], hi[4 * c2 + 2], hi[4 * c2 + 3]);
+                *reinterpret_cast<uint4*>(st + SM::oAlo + off) = make_uint4(lo[4 * c2], lo[4 * c2 + 1], lo[4 * c2 + 2], lo[4 * c2 + 3]);
             }
             fence_proxy_async_smem();
             mbar_arrive(ready + s);
-            T1a = T1an; T1b = T1bn;
+            Ta = Tb; Tb = Tc; Tc = Tn;
         }
         // ---- epilogue: Y1 = tanh(acc 2^-14 + b1) ----
         mbar_wait(tmem_full, 0);
@@ -471,15 +475,36 @@ l1_desc_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ L1Ar
         float* orow = g.out + m * g.ldo;
         constexpr float kInv = 1.f / (kL1DScale * kW1Scale);
 #pragma unroll 1
-        for (int c = 0; c < BN / 16; ++c) {
+        for (int c = half; c < BN / 16; c += 2) {
             uint32_t v[16];
             tmem_ld16(tmem_base + ((uint32_t)(quarter * 32) << 16) + c * 16, v);
+            float bv[16];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const float4 b4 = __ldg(reinterpret_cast<const float4*>(g.bias[ty] + c * 16) + q);
+                bv[4 * q] = b4.x; bv[4 * q + 1] = b4.y; bv[4 * q + 2] = b4.z; bv[4 * q + 3] = b4.w;
+            }
             tmem_ld_wait();
             if (!row_ok) continue;
-            const float* bias = g.bias[ty] + c * 16;
             float r[16];
 #pragma unroll
-            for (int q = 0; q < 16; ++q) r[q] = tanh_fast(fmaf(__uint_as_float(v[q]), kInv, __ldg(bias + q)));
+            for (int q = 0; q < 16; ++q) r[q] = tanh_fast(fmaf(__uint_as_float(v[q]), kInv, bv[q]));
+            if (g.out_hi) {
+                uint32_t hi[8], lo[8];
+#pragma unroll
+                for (int q = 0; q < 8; ++q) {
+                    const __half2 h = __floats2half2_rn(r[2 * q], r[2 * q + 1]);
+                    const float2 hf = __half22float2(h);
+                    const __half2 l = __floats2half2_rn(r[2 * q] - hf.x, r[2 * q + 1] - hf.y);
+                    hi[q] = *reinterpret_cast<const uint32_t*>(&h);
+                    lo[q] = *reinterpret_cast<const uint32_t*>(&l);
+                }
+                uint4* oh = reinterpret_cast<uint4*>(g.out_hi + m * g.ldo + c * 16);
+                uint4* ol = reinterpret_cast<uint4*>(g.out_lo + m * g.ldo + c * 16);
+                oh[0] = make_uint4(hi[0], hi[1], hi[2], hi[3]); oh[1] = make_uint4(hi[4], hi[5], hi[6], hi[7]);
+                ol[0] = make_uint4(lo[0], lo[1], lo[2], lo[3]); ol[1] = make_uint4(lo[4], lo[5], lo[6], lo[7]);
+                continue;
+            }
 #pragma unroll
             for (int q = 0; q < 4; ++q)
                 reinterpret_cast<float4*>(orow + c * 16)[q] = make_float4(r[4 * q], r[4 * q + 1], r[4 * q + 2], r[4 * q + 3]);
@@ -526,7 +551,7 @@ struct DdSmem {
     static constexpr int kTotal = oBars + 256 + 1024;
 };
 
-__global__ void __launch_bounds__(kTcThreads, 1)
+__global__ void __launch_bounds__(kL1Threads, 1)
 dd_dt_kernel(const __grid_constant__ DdMaps maps, const __grid_constant__ DdDtArgs g) {
     using SM = DdSmem;
     constexpr int ST = kDdST, BN = kDdBN;
@@ -555,7 +580,7 @@ dd_dt_kernel(const __grid_constant__ DdMaps maps, const __grid_constant__ DdDtAr
         tma_prefetch_desc(&maps.Bhi[ty]);
         tma_prefetch_desc(&maps.Blo[ty]);
         for (int s = 0; s < ST; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, 1); }
-        for (int b = 0; b < 2; ++b) { mbar_init(tmem_full + b, 1); mbar_init(tmem_empty + b, 128); }
+        for (int b = 0; b < 2; ++b) { mbar_init(tmem_full + b, 1); mbar_init(tmem_empty + b, 256); }
         fence_barrier_init();
     }
     if (warp == 1) tmem_alloc(tmem_ptr, 512);
@@ -610,60 +635,79 @@ dd_dt_kernel(const __grid_constant__ DdMaps maps, const __grid_constant__ DdDtAr
             }
         }
     } else {
-        const int quarter = warp & 3;
+        // two warps per TMEM lane quarter: warp `half` contracts the m1 values j = 5 half .. 5 half + 4 of every chunk
+        // (round-2 profile: four epilogue warps, each alone on its scheduler, ran this loop at 0.16 IPC behind the
+        // shared-memory reads and left the tensor pipe 39 % active)
+        constexpr int JH = BN / 32;                            // 5 m1 values per warp and chunk
+        const int quarter = warp & 3, half = (warp - 2) >> 2;
         const int ml = m0 + quarter * 32 + lane;               // my row inside the type (TMEM lane)
         const bool row_ok = ml < rows_t;
         const size_t m = (size_t)(g.row0[ty] + (row_ok ? ml : 0));
         const float4* Trow = reinterpret_cast<const float4*>(g.Tm) + m * g.M1;
         float4* dTrow = reinterpret_cast<float4*>(g.dTm) + m * g.M1;
         const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
-        // T[i][0:16] of my row -> shared memory, [m2][thread] (conflict-free 16 B accesses)
+        // T[i][0:16] of my row -> shared memory, [m2][thread] (conflict-free 16 B accesses); both warps of the
+        // quarter write the same values
         float4* T2s = reinterpret_cast<float4*>(smem + SM::oT2) + (quarter * 32 + lane);
 #pragma unroll
         for (int m2 = 0; m2 < 16; ++m2) T2s[m2 * 128] = row_ok ? __ldg(Trow + m2) : zero4;
         float4 accB[16];
 #pragma unroll
         for (int m2 = 0; m2 < 16; ++m2) accB[m2] = zero4;
-        float4 T1[BN / 16];                                     // T[i][m1] of the chunk, fetched one chunk ahead
+        float4 T1[JH];                                          // T[i][m1] of the chunk, fetched one chunk ahead
 #pragma unroll
-        for (int j = 0; j < BN / 16; ++j) T1[j] = row_ok ? __ldg(Trow + j) : zero4;
+        for (int j = 0; j < JH; ++j) T1[j] = row_ok ? __ldg(Trow + JH * half + j) : zero4;
+        const float inv_scale = g.inv_scale;
 
         for (int nc = 0; nc < nch; ++nc) {
             const int buf = nc & 1;
-            float4 T1n[BN / 16];
+            float4 T1n[JH];
 #pragma unroll
-            for (int j = 0; j < BN / 16; ++j)
-                T1n[j] = (row_ok && nc + 1 < nch) ? __ldg(Trow + (nc + 1) * (BN / 16) + j) : zero4;
+            for (int j = 0; j < JH; ++j)
+                T1n[j] = (row_ok && nc + 1 < nch) ? __ldg(Trow + (nc + 1) * (BN / 16) + JH * half + j) : zero4;
             mbar_wait(tmem_full + buf, (nc >> 1) & 1);
             tc_fence_after();
-            const uint32_t dcol = tmem_base + ((uint32_t)(quarter * 32) << 16) + buf * 256;
+            const uint32_t dcol = tmem_base + ((uint32_t)(quarter * 32) << 16) + buf * 256 + half * (JH * 16);
 #pragma unroll
-            for (int j = 0; j < BN / 16; ++j) {
+            for (int j = 0; j < JH; ++j) {
                 uint32_t v[16];
                 tmem_ld16(dcol + j * 16, v);
                 tmem_ld_wait();
                 float4 accA = zero4;
 #pragma unroll
                 for (int m2 = 0; m2 < 16; ++m2) {
-                    const float d = __uint_as_float(v[m2]) * g.inv_scale;
+                    const float d = __uint_as_float(v[m2]);     // the common factor 1 / scale is applied at the stores
                     const float4 T2 = T2s[m2 * 128];
                     accA.x = fmaf(d, T2.x, accA.x); accA.y = fmaf(d, T2.y, accA.y);
                     accA.z = fmaf(d, T2.z, accA.z); accA.w = fmaf(d, T2.w, accA.w);
                     accB[m2].x = fmaf(d, T1[j].x, accB[m2].x); accB[m2].y = fmaf(d, T1[j].y, accB[m2].y);
                     accB[m2].z = fmaf(d, T1[j].z, accB[m2].z); accB[m2].w = fmaf(d, T1[j].w, accB[m2].w);
                 }
-                if (row_ok) dTrow[nc * (BN / 16) + j] = accA;
+                accA.x *= inv_scale; accA.y *= inv_scale; accA.z *= inv_scale; accA.w *= inv_scale;
+                if (row_ok) dTrow[nc * (BN / 16) + JH * half + j] = accA;
             }
             tc_fence_before();
             mbar_arrive(tmem_empty + buf);
 #pragma unroll
-            for (int j = 0; j < BN / 16; ++j) T1[j] = T1n[j];
+            for (int j = 0; j < JH; ++j) T1[j] = T1n[j];
         }
-        if (row_ok) {
+        // second term: the two warps of a quarter hold shares over disjoint m1; the second warp hands its share over
+        // through the (now idle: the last tmem_full says every MMA has retired) stage memory, the first adds both to
+        // the rows m < 16, which either warp may have stored above (bar.sync orders those stores)
+        float4* xch = reinterpret_cast<float4*>(smem) + (quarter * 32 + lane);
+        if (half == 1) {
+#pragma unroll
+            for (int m2 = 0; m2 < 16; ++m2) xch[m2 * 128] = accB[m2];
+        }
+        __threadfence_block();
+        asm volatile("bar.sync %0, 64;" ::"r"(1 + quarter) : "memory");
+        if (half == 0 && row_ok) {
 #pragma unroll
             for (int m2 = 0; m2 < 16; ++m2) {
                 float4 o = dTrow[m2];
-                o.x += accB[m2].x; o.y += accB[m2].y; o.z += accB[m2].z; o.w += accB[m2].w;
+                const float4 x = xch[m2 * 128];
+                o.x = fmaf(accB[m2].x + x.x, inv_scale, o.x); o.y = fmaf(accB[m2].y + x.y, inv_scale, o.y);
+                o.z = fmaf(accB[m2].z + x.z, inv_scale, o.z); o.w = fmaf(accB[m2].w + x.w, inv_scale, o.w);
                 dTrow[m2] = o;
             }
         }
@@ -716,6 +760,19 @@ bool tc_make_map_h(CUtensorMap* map, const uint16_t* base, uint64_t rows, uint64
     cuuint32_t estr[2] = {1, 1};
     return enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, const_cast<uint16_t*>(base), dims, strides, box, estr,
                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// the same matrix walked one k-step at a time: box = 16 halfs x box_rows, SWIZZLE_32B (fitting_mid.cu)
+bool tc_make_map_h16(CUtensorMap* map, const uint16_t* base, uint64_t rows, uint64_t cols, uint64_t ld, uint32_t box_rows) {
+    EncodeTiledFn enc = get_encode();
+    if (!enc) return false;
+    cuuint64_t dims[2] = {cols, rows};
+    cuuint64_t strides[1] = {ld * 2};
+    cuuint32_t box[2] = {16, box_rows};
+    cuuint32_t estr[2] = {1, 1};
+    return enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, const_cast<uint16_t*>(base), dims, strides, box, estr,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_32B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
@@ -836,22 +893,29 @@ static void gather_maps(TcMaps& mp, const CUtensorMap* A, const CUtensorMap (*Bh
 // the whole fitting chain of all centre types on the tensor cores: 3 forward GEMMs (the third also yields
 // E_i, U and the seed of the backward pass), 3 backward GEMMs.  Returns the number of launches.
 // tiles [t0, t0 + nt_) of the chain on stream s
-static void chain_range(Model& m, const ForceArgs& fa, int t0, int ntl, cudaStream_t s) {
+static int chain_range(Model& m, const ForceArgs& fa, int t0, int ntl, cudaStream_t s) {
     const int NF = m.NF, ND = m.ND, nt = fa.ntypes;
     TcGemmArgs g{};
     TcMaps mp;
     fill_types(m, nt, g);
     auto base = [&]() { TcGemmArgs q{}; fill_types(m, nt, q); q.tile_off = t0; return q; };
+    static const bool old_chain = getenv("PIMD_FIT_OLD") != nullptr;      // A/B partner: the round-1 chain of four GEMM launches
+    const bool fused = m.mid_ready && !old_chain;
     // layer 1: Y1 = tanh(D W1 + b1), D produced on the fly from T
     {
         L1Args a1{};
         a1.tile_off = t0;
         a1.ntypes = nt; a1.K = ND; a1.Tm = m.Tm; a1.out = m.Y1; a1.ldo = NF; a1.M1 = m.M1;
+        if (fused) { a1.out_hi = reinterpret_cast<__half*>(m.y1_h_hi); a1.out_lo = reinterpret_cast<__half*>(m.y1_h_lo); }
         for (int t = 0; t <= kMaxT; ++t) { a1.tile0[t] = g.tile0[t]; a1.row0[t] = g.row0[t]; }
         for (int t = 0; t < nt; ++t) a1.bias[t] = m.fit_b[t][0];
         for (int t = 0; t < kMaxT; ++t) { const int q = t < nt ? t : 0; mp.A[t] = m.mapA_D[q]; mp.Bhi[t] = m.mapBh_l1_hi[q]; mp.Blo[t] = m.mapBh_l1_lo[q]; }
-        l1_desc_kernel<<<ntl, kTcThreads, L1Smem::kTotal, s>>>(mp, a1);
+        l1_desc_kernel<<<ntl, kL1Threads, L1Smem::kTotal, s>>>(mp, a1);
     }
+    if (fused) {
+        // layers 2 and 3, the energy and their backward products in one kernel (fitting_mid.cu)
+        fitting_mid_launch(m, fa, t0, ntl, s);
+    } else {
     // layer 2: T2 = tanh(Y1 W2 + b2); Y2 = Y1 + T2
     g = base(); g.N = NF; g.K = NF; g.add = m.Y1; g.ldadd = NF; g.out0 = m.T2; g.out1 = m.Y2; g.ldo = NF;
     for (int t = 0; t < nt; ++t) g.bias[t] = m.fit_b[t][1];
@@ -872,6 +936,7 @@ static void chain_range(Model& m, const ForceArgs& fa, int t0, int ntl, cudaStre
     g = base(); g.N = NF; g.K = NF; g.add = m.Y3; g.ldadd = NF; g.tt = m.Y1; g.ldtt = NF; g.out1 = reinterpret_cast<float*>(m.da1_h_hi); g.out0 = reinterpret_cast<float*>(m.da1_h_lo); g.ldo = NF; g.scale = m.bwd_scale;
     gather_maps(mp, m.mapA_T3, m.mapB_bwd_hi, m.mapB_bwd_lo, 1, nt);
     tc_gemm(TEPI_BWD_FIRST, 240, mp, g, ntl, s);
+    }
     // dD = da1 W1^T contracted with T on the fly -> dT                   (A = G1 = da1)
     {
         DdDtArgs d{};
@@ -884,11 +949,12 @@ static void chain_range(Model& m, const ForceArgs& fa, int t0, int ntl, cudaStre
             dm.Ahi[t] = m.mapAh_G1[q]; dm.Alo[t] = m.mapAh_G2[q];
             dm.Bhi[t] = m.mapBh_dd_hi[q]; dm.Blo[t] = m.mapBh_dd_lo[q];
         }
-        dd_dt_kernel<<<ntl, kTcThreads, DdSmem::kTotal, s>>>(dm, d);
+        dd_dt_kernel<<<ntl, kL1Threads, DdSmem::kTotal, s>>>(dm, d);
     }
+    return fused ? 3 : 6;
 }
 
-// The whole fitting chain of all centre types on the tensor cores: 6 kernels per tile range.  Every kernel of
+// The whole fitting chain of all centre types on the tensor cores: 3 kernels per tile range (6 with PIMD_FIT_OLD).  Every kernel of
 // the chain is row-local, so the tiles are cut into ranges that run on separate streams: the tail wave of one
 // range's kernel (384 tiles on 148 SMs are 2.6 waves) is filled by the other range's kernels.
 int fitting_chain_tc(Model& m, const ForceArgs& fa, cudaStream_t s) {
@@ -906,19 +972,19 @@ int fitting_chain_tc(Model& m, const ForceArgs& fa, cudaStream_t s) {
     }
     const int NR = m.chain_streams;
     if (tiles < 2 * NR) {
-        chain_range(m, fa, 0, tiles, s);
-        return 6;
+        return chain_range(m, fa, 0, tiles, s);
     }
     cudaEventRecord(m.ev_fork, s);
+    int launches = 0;
     for (int q = 0; q < NR; ++q) {
         const int t0 = (int)((long long)tiles * q / NR), t1 = (int)((long long)tiles * (q + 1) / NR);
         cudaStream_t sq = (q == 0) ? s : m.aux_stream[q - 1];
         if (q > 0) cudaStreamWaitEvent(sq, m.ev_fork, 0);
-        chain_range(m, fa, t0, t1 - t0, sq);
+        launches += chain_range(m, fa, t0, t1 - t0, sq);
         if (q > 0) cudaEventRecord(m.ev_join[q - 1], sq);
     }
     for (int q = 1; q < NR; ++q) cudaStreamWaitEvent(s, m.ev_join[q - 1], 0);
-    return 6 * NR;
+    return launches;
 }
 
 // parity hook: C[M][N] = A[M][K] Bt[N][K]^T through the tensor-core kernel (N == 240 or N % 160 == 0, K % 16 == 0)
