@@ -155,10 +155,10 @@ size_t model_bytes(const pimd_ctx* c, const pimd_model_desc* d) {
     cell_grid(c->box, d->rcut, ncell, R, &ncells);
     size_t b = 0;
     b += align_up((size_t)d->n_types * d->n_types * 8192 * 4, 256);                     // embedding weights (padded)
-    b += (size_t)d->n_types * 4 * align_up((size_t)ND * NF * 2, 256);                  // FP16-split layer-1 images
+    b += (size_t)d->n_types * (align_up(l1_wimg_bytes(ND), 256) + align_up(dd_wimg_bytes(ND) + 65536, 256));   // operand images of layer 1
     b += (size_t)d->n_types * 6 * (align_up((size_t)ND * NF * 4, 256) + 2 * align_up((size_t)NF * NF * 4, 256) + align_up(NF * 4, 256));
     b += (size_t)d->n_types * 4 * align_up((size_t)NF * 4, 256);
-    b += (size_t)d->n_types * 8 * align_up((size_t)NF * NF * 2, 256);                  // FP16-split operands of the fused middle
+    b += (size_t)d->n_types * align_up(mid_wimg_bytes(), 256);
     b += 4 * align_up(PN * 4, 256);                                                    // cen_idx,row_of,cell_id,cell_tmp
     b += 3 * align_up((size_t)c->P * (ncells + 1) * 4, 256);
     b += align_up(PN * 24, 256) + align_up(PN * 32, 256);
@@ -168,6 +168,7 @@ size_t model_bytes(const pimd_ctx* c, const pimd_model_desc* d) {
     b += 2 * align_up(PN * M1 * 16, 256);
     b += 2 * align_up(PN * ND * 4, 256);
     b += 7 * align_up(PN * NF * 4, 256);
+    b += 2 * align_up((PN / 128 + d->n_types + 1) * mid_image_bytes(), 256) + 2 * align_up((PN / 128 + d->n_types + 1) * mid_scratch_bytes(), 256);
     b += align_up((size_t)d->n_types * d->n_types * emb_tc_image_h_bytes(), 256);
     b += align_up((size_t)d->n_types * (PN + 1) * 4, 256) + align_up(PN * nsel * 4, 256);
     b += align_up((size_t)d->n_types * ((PN + 1023) / 1024) * 4, 256) + align_up(PN * 72, 256);
@@ -750,6 +751,7 @@ int pimd_set_model(pimd_ctx* ctx, const pimd_model_desc* d, const double* w, siz
 
     // ---- fitting weights: W, W^T, b per layer ----
     std::vector<std::vector<float>> keep;
+    std::vector<std::vector<uint8_t>> imgs;
     for (int t = 0; t < nt; ++t) {
         int nin = m.ND;
         for (int l = 0; l < 4; ++l) {
@@ -777,25 +779,29 @@ int pimd_set_model(pimd_ctx* ctx, const pimd_model_desc* d, const double* w, siz
                 if ((rc = arena_alloc(ctx, &m.fit_wT_lo[t][l], W.size()))) return rc;
                 tc_split_weights(W.size(), m.fit_w[t][l], m.fit_w_hi[t][l], m.fit_w_lo[t][l], ctx->stream);
                 tc_split_weights(W.size(), m.fit_wT[t][l], m.fit_wT_hi[t][l], m.fit_wT_lo[t][l], ctx->stream);
-                if (l == 0) {     // FP16-split images of layer 1 (fitting_tc.cu: l1_desc_kernel, dd_dt_kernel)
-                    if ((rc = arena_alloc(ctx, &m.w1_h_hi[t], W.size()))) return rc;
-                    if ((rc = arena_alloc(ctx, &m.w1_h_lo[t], W.size()))) return rc;
-                    if ((rc = arena_alloc(ctx, &m.w1T_h_hi[t], W.size()))) return rc;
-                    if ((rc = arena_alloc(ctx, &m.w1T_h_lo[t], W.size()))) return rc;
-                    tc_split_weights_h(W.size(), m.fit_w[t][l], 64.f, m.w1_h_hi[t], m.w1_h_lo[t], ctx->stream);
-                    tc_split_weights_h(W.size(), m.fit_wT[t][l], 64.f, m.w1T_h_hi[t], m.w1T_h_lo[t], ctx->stream);
-                } else {          // FP16-split operands of the fused middle (fitting_mid.cu): phases W2^T, W3^T, W3, W2
-                    const int pf = l - 1, pb = 4 - l;
-                    for (int h = 0; h < 2; ++h) {
-                        if ((rc = arena_alloc(ctx, &m.wmid_h[t][pf][h], W.size()))) return rc;
-                        if ((rc = arena_alloc(ctx, &m.wmid_h[t][pb][h], W.size()))) return rc;
+                if (l == 0) {     // operand images of layer 1 (fitting_tc.cu: l1_desc_kernel, dd_dt_kernel)
+                    if (m.NF == 240 && nin % 160 == 0) {
+                        std::vector<uint8_t> i1(l1_wimg_bytes(nin)), i2(dd_wimg_bytes(nin));
+                        l1_build_wimg(WT.data(), nin, i1.data());
+                        dd_build_wimg(W.data(), nin, i2.data());
+                        if ((rc = arena_alloc(ctx, &m.l1_wimg[t], i1.size()))) return rc;
+                        if ((rc = arena_alloc(ctx, &m.dd_wimg[t], i2.size()))) return rc;
+                        CK(cudaMemcpyAsync(m.l1_wimg[t], i1.data(), i1.size(), cudaMemcpyHostToDevice, ctx->stream));
+                        CK(cudaMemcpyAsync(m.dd_wimg[t], i2.data(), i2.size(), cudaMemcpyHostToDevice, ctx->stream));
+                        imgs.push_back(std::move(i1)); imgs.push_back(std::move(i2));
                     }
-                    tc_split_weights_h(W.size(), m.fit_wT[t][l], 64.f, m.wmid_h[t][pf][0], m.wmid_h[t][pf][1], ctx->stream);
-                    tc_split_weights_h(W.size(), m.fit_w[t][l], 64.f, m.wmid_h[t][pb][0], m.wmid_h[t][pb][1], ctx->stream);
                 }
             }
             keep.push_back(std::move(W)); keep.push_back(std::move(WT)); keep.push_back(std::move(b));
             nin = nout;
+        }
+        if (m.NF == 240) {   // operand images of the fused middle of the chain (fitting_mid.cu)
+            const size_t k0 = keep.size() - 12;              // W, WT, b of the four layers of this type
+            std::vector<uint8_t> img(mid_wimg_bytes());
+            mid_build_wimg(keep[k0 + 3].data(), keep[k0 + 4].data(), keep[k0 + 6].data(), keep[k0 + 7].data(), img.data());
+            if ((rc = arena_alloc(ctx, &m.mid_wimg[t], img.size()))) return rc;
+            CK(cudaMemcpyAsync(m.mid_wimg[t], img.data(), img.size(), cudaMemcpyHostToDevice, ctx->stream));
+            imgs.push_back(std::move(img));
         }
     }
 
@@ -850,6 +856,13 @@ int pimd_set_model(pimd_ctx* ctx, const pimd_model_desc* d, const double* w, siz
     float** fb[7] = {&m.Y1, &m.T2, &m.Y2, &m.T3, &m.Y3, &m.G1, &m.G2};
     for (int q = 0; q < 7; ++q)
         if ((rc = arena_alloc(ctx, fb[q], PN * m.NF))) return rc;
+    if (m.NF == 240) {   // hand-over images and scratch of the fused fitting chain, per 128-row tile
+        const size_t tiles = PN / 128 + nt + 1;
+        if ((rc = arena_alloc(ctx, &m.y1_img, tiles * mid_image_bytes()))) return rc;
+        if ((rc = arena_alloc(ctx, &m.da1_img, tiles * mid_image_bytes()))) return rc;
+        if ((rc = arena_alloc(ctx, &m.mid_t2, tiles * mid_scratch_bytes() / 16))) return rc;
+        if ((rc = arena_alloc(ctx, &m.mid_g1, tiles * mid_scratch_bytes() / 16))) return rc;
+    }
     if ((rc = arena_alloc(ctx, &m.rowstart, (size_t)nt * (PN + 1)))) return rc;
     if ((rc = arena_alloc(ctx, &m.rowaddr, PN * m.nsel))) return rc;
     if ((rc = arena_alloc(ctx, &m.row_bsum, (size_t)nt * ((PN + 1023) / 1024)))) return rc;

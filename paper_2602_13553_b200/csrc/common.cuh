@@ -163,19 +163,17 @@ struct Model {
     float*   fit_w_hi[PIMD_MAX_TYPES][3], *fit_w_lo[PIMD_MAX_TYPES][3];           // pre-split weights (layers 1..3)
     float*   fit_wT_hi[PIMD_MAX_TYPES][3], *fit_wT_lo[PIMD_MAX_TYPES][3];
     // FP16-split images of the first fitting layer (x kW1Scale) for the two K = 1600 / N = 1600 kernels
-    uint16_t* w1T_h_hi[PIMD_MAX_TYPES], *w1T_h_lo[PIMD_MAX_TYPES];   // W1^T [240][1600]
-    uint16_t* w1_h_hi[PIMD_MAX_TYPES], *w1_h_lo[PIMD_MAX_TYPES];     // W1   [1600][240]
-    CUtensorMap mapBh_l1_hi[PIMD_MAX_TYPES], mapBh_l1_lo[PIMD_MAX_TYPES];     // layer-1 forward B
-    CUtensorMap mapBh_dd_hi[PIMD_MAX_TYPES], mapBh_dd_lo[PIMD_MAX_TYPES];     // dD GEMM B
+    uint8_t* l1_wimg[PIMD_MAX_TYPES];    // W1^T: one image per K block of 32 (l1_desc_kernel's B operand, one bulk copy per stage)
+    uint8_t* dd_wimg[PIMD_MAX_TYPES];    // W1: one image per (chunk of 160 rows, K block of 32) (dd_dt_kernel's B operand)
     CUtensorMap mapAh_G1[PIMD_MAX_TYPES], mapAh_G2[PIMD_MAX_TYPES];           // da1 as FP16 hi / lo (x bwd_scale)
     uint16_t* da1_h_hi = nullptr, *da1_h_lo = nullptr;   // [rows][240] halfs, carved out of D
     float    bwd_scale = 1.f;          // power of two that brings the backward activations to O(1..16)
-    // fused middle of the fitting chain (fitting_mid.cu): y1 as FP16 hi / lo (carved out of Y1), the four 240 x 240
-    // weight operands (W2^T, W3^T, W3, W2) x 64 as FP16 hi / lo, and their TMA maps
+    // fused middle of the fitting chain (fitting_mid.cu): operand images handed from kernel to kernel (per 128-row
+    // tile: y1 from l1_desc_kernel, bwd_scale * da1 to dd_dt_kernel), tile-private scratch, weight images
     bool     mid_ready = false;
-    uint16_t* y1_h_hi = nullptr, *y1_h_lo = nullptr;
-    uint16_t* wmid_h[PIMD_MAX_TYPES][4][2];
-    CUtensorMap mapMidA_hi[PIMD_MAX_TYPES], mapMidA_lo[PIMD_MAX_TYPES], mapMidB[PIMD_MAX_TYPES][4][2];
+    uint8_t* y1_img = nullptr, *da1_img = nullptr;      // [tiles] x mid_image_bytes()
+    float4*  mid_t2 = nullptr, *mid_g1 = nullptr;       // [tiles] x mid_scratch_bytes()
+    uint8_t* mid_wimg[PIMD_MAX_TYPES];   // [phase 4][k-step 15][hi | lo][240 rows x 32 B, SWIZZLE_32B order]: one bulk copy per k-step
     // tensor-core embedding path (embedding_tc.cu)
     bool     use_tc_emb = true;
     bool     tc_emb_ready = false;
@@ -214,8 +212,17 @@ void tc_split_weights(size_t n, const float* w, float* hi, float* lo, cudaStream
 void tc_split_weights_h(size_t n, const float* w, float scale, uint16_t* hi, uint16_t* lo, cudaStream_t s);
 int fitting_chain_tc(Model& m, const ForceArgs& a, cudaStream_t s);
 bool tc_make_map_h(CUtensorMap* map, const uint16_t* base, uint64_t rows, uint64_t cols, uint64_t ld, uint32_t box_rows);
-bool tc_make_map_h16(CUtensorMap* map, const uint16_t* base, uint64_t rows, uint64_t cols, uint64_t ld, uint32_t box_rows);
 bool fitting_mid_setup(Model& m, int ntypes);
+size_t kmajor_image_bytes(int nrows, int kc);
+void kmajor_image(const float* Bt, int N, int K, int n0, int nr, int k0, int kc, float scale, uint8_t* img);
+size_t mid_wimg_bytes();
+size_t mid_image_bytes();
+size_t mid_scratch_bytes();
+size_t l1_wimg_bytes(int ND);
+void l1_build_wimg(const float* WT, int ND, uint8_t* img);
+size_t dd_wimg_bytes(int ND);
+void dd_build_wimg(const float* W, int ND, uint8_t* img);
+void mid_build_wimg(const float* W2, const float* W2T, const float* W3, const float* W3T, uint8_t* img);
 void fitting_mid_launch(Model& m, const ForceArgs& a, int tile_off, int ntiles, cudaStream_t s);
 size_t emb_tc_image_h_bytes();
 void emb_tc_build_image_h(const double* w_pair, uint8_t* img);

@@ -14,6 +14,7 @@
 //            the epilogue: tcgen05.ld accumulators -> bias / tanh / skip / derivative / energy -> global
 // Two CTAs share an SM (2 x 256 TMEM columns, 2 x 2 stages), so one CTA's epilogue runs under the other's MMAs.
 #include <algorithm>
+#include <type_traits>
 #include <cstdlib>
 #include <cuda_fp16.h>
 #include "common.cuh"
@@ -330,7 +331,8 @@ struct L1Args {
     const float* bias[kMaxT];
     const float* Tm;      // [rows][100][4]
     float* out; int ldo;  // Y1 (FP32), or
-    __half* out_hi; __half* out_lo;   // Y1 as an FP16 hi / lo pair for fit_mid_kernel (when out_hi is set)
+    uint8_t* out_img;     // when set: Y1 as the operand image of fit_mid_kernel, [tile] x 128 KB: [hi | lo][K block 8][128 rows x 64 B, SWIZZLE_64B order]
+    const uint8_t* wimg[kMaxT];       // W1^T x 64 as shared-memory images, [K block of 32][hi | lo][240 rows x 64 B]
     int M1;
 };
 
@@ -345,7 +347,8 @@ struct L1Smem {
     static constexpr int kABytes = 128 * 64, kBBytes = kL1BN * 64;        // 64 B rows = 32 halfs, SWIZZLE_64B
     static constexpr int oAhi = 0, oAlo = kABytes, oBhi = 2 * kABytes, oBlo = 2 * kABytes + kBBytes;
     static constexpr int kStage = 2 * kABytes + 2 * kBBytes;               // 47104
-    static constexpr int oBars = kL1ST * kStage;
+    static constexpr int oBias = kL1ST * kStage;                           // float [240]
+    static constexpr int oBars = oBias + kL1BN * 4;
     static constexpr int kTotal = oBars + 256 + 1024;
 };
 
@@ -371,17 +374,14 @@ l1_desc_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ L1Ar
     const int m0 = (tile - g.tile0[ty]) * 128;
     const int rows_t = g.row0[ty + 1] - g.row0[ty];
     const int nk = g.K / 32;                   // K = 16 m1: two m1 per stage
-    const CUtensorMap* mapBhi = &maps.Bhi[ty];
-    const CUtensorMap* mapBlo = &maps.Blo[ty];
 
     if (warp == 0 && lane == 0) {
-        tma_prefetch_desc(mapBhi);
-        tma_prefetch_desc(mapBlo);
         for (int s = 0; s < ST; ++s) { mbar_init(full + s, 1); mbar_init(ready + s, 256); mbar_init(empty + s, 1); }
         mbar_init(tmem_full, 1);
         fence_barrier_init();
     }
     if (warp == 1) tmem_alloc(tmem_ptr, 256);
+    if (threadIdx.x < BN) reinterpret_cast<float*>(smem + SM::oBias)[threadIdx.x] = __ldg(g.bias[ty] + threadIdx.x);
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
@@ -394,8 +394,7 @@ l1_desc_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ L1Ar
                 mbar_wait(empty + s, ph ^ 1);
                 uint8_t* st = smem + s * SM::kStage;
                 mbar_arrive_expect_tx(full + s, 2 * SM::kBBytes);
-                tma_load_2d(st + SM::oBhi, mapBhi, full + s, kb * 32, 0);
-                tma_load_2d(st + SM::oBlo, mapBlo, full + s, kb * 32, 0);
+                bulk_load(st + SM::oBhi, g.wimg[ty] + (size_t)kb * (2 * SM::kBBytes), 2 * SM::kBBytes, full + s);
             }
         }
     } else if (warp == 1) {
@@ -441,10 +440,12 @@ l1_desc_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ L1Ar
         // SWIZZLE_64B K-major block: 64 B rows (32 halfs), 16 B chunk index XOR ((row >> 1) & 3)
         const int rbase = row * 64, sw = (row >> 1) & 3;
         auto load_T1 = [&](int kb) { return (row_ok && kb < nk) ? __ldg(Trow + 2 * kb + half) : zero4; };
-        float4 Ta = load_T1(0), Tb = load_T1(1), Tc = load_T1(2);          // T[i][m1] three stages ahead of its use
-        for (int kb = 0; kb < nk; ++kb) {
+        // T[i][m1] is fetched three stages ahead of its use into three named registers; the loop is unrolled by hand
+        // so that no register that is the target of a load in flight gets moved (a rotation Ta = Tb; Tb = Tc; ... makes
+        // every move wait for the load behind it, which cut the prefetch distance to one stage in the first version)
+        float4 Ta = load_T1(0), Tb = load_T1(1), Tc = load_T1(2);
+        auto stage = [&](int kb, const float4 Ta) {
             const int s = kb % ST, ph = (kb / ST) & 1;
-            const float4 Tn = load_T1(kb + 3);
             uint32_t hi[8], lo[8];                              // K indices 16 half .. 16 half + 15 of the stage, packed in pairs
 #pragma unroll
             for (int q = 0; q < 8; ++q) {
@@ -467,7 +468,14 @@ l1_desc_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ L1Ar
             }
             fence_proxy_async_smem();
             mbar_arrive(ready + s);
-            Ta = Tb; Tb = Tc; Tc = Tn;
+        };
+        for (int kb = 0; kb < nk; kb += 3) {
+            stage(kb, Ta);
+            Ta = load_T1(kb + 3);
+            if (kb + 1 < nk) stage(kb + 1, Tb);
+            Tb = load_T1(kb + 4);
+            if (kb + 2 < nk) stage(kb + 2, Tc);
+            Tc = load_T1(kb + 5);
         }
         // ---- epilogue: Y1 = tanh(acc 2^-14 + b1) ----
         mbar_wait(tmem_full, 0);
@@ -481,7 +489,7 @@ l1_desc_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ L1Ar
             float bv[16];
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
-                const float4 b4 = __ldg(reinterpret_cast<const float4*>(g.bias[ty] + c * 16) + q);
+                const float4 b4 = reinterpret_cast<const float4*>(smem + SM::oBias + c * 64)[q];
                 bv[4 * q] = b4.x; bv[4 * q + 1] = b4.y; bv[4 * q + 2] = b4.z; bv[4 * q + 3] = b4.w;
             }
             tmem_ld_wait();
@@ -489,7 +497,8 @@ l1_desc_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ L1Ar
             float r[16];
 #pragma unroll
             for (int q = 0; q < 16; ++q) r[q] = tanh_fast(fmaf(__uint_as_float(v[q]), kInv, bv[q]));
-            if (g.out_hi) {
+            if (g.out_img) {
+                // the stage memory is idle (tmem_full: every MMA has retired): the image of this tile is put together there
                 uint32_t hi[8], lo[8];
 #pragma unroll
                 for (int q = 0; q < 8; ++q) {
@@ -499,15 +508,28 @@ l1_desc_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ L1Ar
                     hi[q] = *reinterpret_cast<const uint32_t*>(&h);
                     lo[q] = *reinterpret_cast<const uint32_t*>(&l);
                 }
-                uint4* oh = reinterpret_cast<uint4*>(g.out_hi + m * g.ldo + c * 16);
-                uint4* ol = reinterpret_cast<uint4*>(g.out_lo + m * g.ldo + c * 16);
-                oh[0] = make_uint4(hi[0], hi[1], hi[2], hi[3]); oh[1] = make_uint4(hi[4], hi[5], hi[6], hi[7]);
-                ol[0] = make_uint4(lo[0], lo[1], lo[2], lo[3]); ol[1] = make_uint4(lo[4], lo[5], lo[6], lo[7]);
+                const int base = (c >> 1) * (128 * 64) + rbase, ci = 2 * (c & 1);
+                const int o0 = base + ((ci ^ sw) << 4), o1 = base + (((ci + 1) ^ sw) << 4);
+                *reinterpret_cast<uint4*>(smem + o0) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+                *reinterpret_cast<uint4*>(smem + o1) = make_uint4(hi[4], hi[5], hi[6], hi[7]);
+                *reinterpret_cast<uint4*>(smem + 65536 + o0) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+                *reinterpret_cast<uint4*>(smem + 65536 + o1) = make_uint4(lo[4], lo[5], lo[6], lo[7]);
                 continue;
             }
 #pragma unroll
             for (int q = 0; q < 4; ++q)
                 reinterpret_cast<float4*>(orow + c * 16)[q] = make_float4(r[4 * q], r[4 * q + 1], r[4 * q + 2], r[4 * q + 3]);
+        }
+        if (g.out_img) {
+            fence_proxy_async_smem();
+            asm volatile("bar.sync 5, 256;" ::: "memory");
+            if (warp == 2 && lane == 0) {
+                uint8_t* img = g.out_img + (size_t)tile * 131072;
+                bulk_store(img, smem, 65536);
+                bulk_store(img + 65536, smem + 65536, 65536);
+                bulk_commit();
+                bulk_wait0();
+            }
         }
     }
     tc_fence_before();
@@ -532,6 +554,8 @@ struct DdDtArgs {
     float* dTm;           // [rows][100][4]
     int M1;               // 100
     float inv_scale;      // 1 / (bwd_scale x W1 scale): the operands are FP16-split images of scaled values
+    const uint8_t* wimg[kMaxT];   // W1 x 64 as shared-memory images, [chunk of 160 rows][K block of 32][hi | lo][160 rows x 64 B]
+    const uint8_t* a_img;         // when set: da1 as fit_mid_kernel's image, [tile] x 128 KB: [K block 8][hi | lo][128 rows x 64 B]; else the TMA maps
 };
 
 // A (= da1) arrives pre-split as well (the producing epilogue writes hi and lo), so nothing stands between TMA
@@ -577,8 +601,6 @@ dd_dt_kernel(const __grid_constant__ DdMaps maps, const __grid_constant__ DdDtAr
     if (warp == 0 && lane == 0) {
         tma_prefetch_desc(&maps.Ahi[ty]);
         tma_prefetch_desc(&maps.Alo[ty]);
-        tma_prefetch_desc(&maps.Bhi[ty]);
-        tma_prefetch_desc(&maps.Blo[ty]);
         for (int s = 0; s < ST; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, 1); }
         for (int b = 0; b < 2; ++b) { mbar_init(tmem_full + b, 1); mbar_init(tmem_empty + b, 256); }
         fence_barrier_init();
@@ -597,10 +619,13 @@ dd_dt_kernel(const __grid_constant__ DdMaps maps, const __grid_constant__ DdDtAr
                 mbar_wait(empty + s, ph ^ 1);
                 uint8_t* st = smem + s * SM::kStage;
                 mbar_arrive_expect_tx(full + s, 2 * SM::kABytes + 2 * SM::kBBytes);
-                tma_load_2d(st + SM::oAhi, &maps.Ahi[ty], full + s, kb * 32, m0);
-                tma_load_2d(st + SM::oAlo, &maps.Alo[ty], full + s, kb * 32, m0);
-                tma_load_2d(st + SM::oBhi, &maps.Bhi[ty], full + s, kb * 32, nc * BN);
-                tma_load_2d(st + SM::oBlo, &maps.Blo[ty], full + s, kb * 32, nc * BN);
+                if (g.a_img) {
+                    bulk_load(st + SM::oAhi, g.a_img + (size_t)tile * 131072 + kb * (2 * SM::kABytes), 2 * SM::kABytes, full + s);
+                } else {
+                    tma_load_2d(st + SM::oAhi, &maps.Ahi[ty], full + s, kb * 32, m0);
+                    tma_load_2d(st + SM::oAlo, &maps.Alo[ty], full + s, kb * 32, m0);
+                }
+                bulk_load(st + SM::oBhi, g.wimg[ty] + (size_t)it * (2 * SM::kBBytes), 2 * SM::kBBytes, full + s);
             }
         }
     } else if (warp == 1) {
@@ -619,8 +644,8 @@ dd_dt_kernel(const __grid_constant__ DdMaps maps, const __grid_constant__ DdDtAr
                     mbar_wait(full + s, ph);
                     tc_fence_after();
                     const uint32_t st = smem_u32(smem + s * SM::kStage);
-#pragma unroll
-                    for (int ks = 0; ks < 2; ++ks) {
+                    const int nks = (kb == nk - 1 && (g.K & 31)) ? 1 : 2;   // K = 240: the last block holds one k-step (the image has no zero padding behind it)
+                    for (int ks = 0; ks < nks; ++ks) {
                         const uint64_t a_hi = make_smem_desc_kmajor(st + SM::oAhi + ks * 32, 64);
                         const uint64_t a_lo = make_smem_desc_kmajor(st + SM::oAlo + ks * 32, 64);
                         const uint64_t b_hi = make_smem_desc_kmajor(st + SM::oBhi + ks * 32, 64);
@@ -635,82 +660,88 @@ dd_dt_kernel(const __grid_constant__ DdMaps maps, const __grid_constant__ DdDtAr
             }
         }
     } else {
-        // two warps per TMEM lane quarter: warp `half` contracts the m1 values j = 5 half .. 5 half + 4 of every chunk
-        // (round-2 profile: four epilogue warps, each alone on its scheduler, ran this loop at 0.16 IPC behind the
-        // shared-memory reads and left the tensor pipe 39 % active)
-        constexpr int JH = BN / 32;                            // 5 m1 values per warp and chunk
-        const int quarter = warp & 3, half = (warp - 2) >> 2;
+        // Two warps per TMEM lane quarter (a warp alone on its scheduler ran this loop at 0.16 IPC); warp `half` owns the
+        // m2 values 8 half .. 8 half + 7 of every m1 group: its eight T[i][m2] and second-term sums stay in registers
+        // (no shared-memory read per product, the stall that dominated the first two versions), and it reads only its
+        // eight accumulator columns of each group.  The first term is a sum over all sixteen m2: the two warps swap
+        // the halves they do not finalise through shared memory (warp `half` finalises j = 5 half .. 5 half + 4).
+        constexpr int NJ = BN / 16, JH = NJ / 2;               // 10 m1 values per chunk, 5 finalised per warp
+        const int quarter = warp & 3;
+        auto epilogue = [&](auto half_c) {
+        constexpr int half = decltype(half_c)::value;          // compile-time: it selects registers below
         const int ml = m0 + quarter * 32 + lane;               // my row inside the type (TMEM lane)
         const bool row_ok = ml < rows_t;
         const size_t m = (size_t)(g.row0[ty] + (row_ok ? ml : 0));
         const float4* Trow = reinterpret_cast<const float4*>(g.Tm) + m * g.M1;
         float4* dTrow = reinterpret_cast<float4*>(g.dTm) + m * g.M1;
         const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
-        // T[i][0:16] of my row -> shared memory, [m2][thread] (conflict-free 16 B accesses); both warps of the
-        // quarter write the same values
-        float4* T2s = reinterpret_cast<float4*>(smem + SM::oT2) + (quarter * 32 + lane);
+        float4 T2[8], accB[8];
 #pragma unroll
-        for (int m2 = 0; m2 < 16; ++m2) T2s[m2 * 128] = row_ok ? __ldg(Trow + m2) : zero4;
-        float4 accB[16];
+        for (int k = 0; k < 8; ++k) { T2[k] = row_ok ? __ldg(Trow + 8 * half + k) : zero4; accB[k] = zero4; }
+        float4 T1[NJ];                                          // T[i][m1] of the chunk; refilled for the next chunk as it is used up
 #pragma unroll
-        for (int m2 = 0; m2 < 16; ++m2) accB[m2] = zero4;
-        float4 T1[JH];                                          // T[i][m1] of the chunk, fetched one chunk ahead
-#pragma unroll
-        for (int j = 0; j < JH; ++j) T1[j] = row_ok ? __ldg(Trow + JH * half + j) : zero4;
+        for (int j = 0; j < NJ; ++j) T1[j] = row_ok ? __ldg(Trow + j) : zero4;
         const float inv_scale = g.inv_scale;
+        // exchange buffer [writer half][jj][row] (float4), in the place of the former T[i][0:16] copy
+        float4* xw = reinterpret_cast<float4*>(smem + SM::oT2) + half * (JH * 128) + (quarter * 32 + lane);
+        const float4* xr = reinterpret_cast<const float4*>(smem + SM::oT2) + (1 - half) * (JH * 128) + (quarter * 32 + lane);
+        const int bar_id = 1 + quarter;
 
         for (int nc = 0; nc < nch; ++nc) {
             const int buf = nc & 1;
-            float4 T1n[JH];
-#pragma unroll
-            for (int j = 0; j < JH; ++j)
-                T1n[j] = (row_ok && nc + 1 < nch) ? __ldg(Trow + (nc + 1) * (BN / 16) + JH * half + j) : zero4;
+            const bool more = row_ok && nc + 1 < nch;
             mbar_wait(tmem_full + buf, (nc >> 1) & 1);
             tc_fence_after();
-            const uint32_t dcol = tmem_base + ((uint32_t)(quarter * 32) << 16) + buf * 256 + half * (JH * 16);
+            const uint32_t dcol = tmem_base + ((uint32_t)(quarter * 32) << 16) + buf * 256 + 8 * half;
+            float4 keep[JH];
+            uint32_t vq[2][8];                                  // the next group's columns are in flight while this one is contracted
+            tmem_ld8(dcol, vq[0]);
 #pragma unroll
-            for (int j = 0; j < JH; ++j) {
-                uint32_t v[16];
-                tmem_ld16(dcol + j * 16, v);
+            for (int j = 0; j < NJ; ++j) {
                 tmem_ld_wait();
+                if (j + 1 < NJ) tmem_ld8(dcol + (j + 1) * 16, vq[(j + 1) & 1]);
+                const uint32_t* v = vq[j & 1];
                 float4 accA = zero4;
+                const float4 t1 = T1[j];
 #pragma unroll
-                for (int m2 = 0; m2 < 16; ++m2) {
-                    const float d = __uint_as_float(v[m2]);     // the common factor 1 / scale is applied at the stores
-                    const float4 T2 = T2s[m2 * 128];
-                    accA.x = fmaf(d, T2.x, accA.x); accA.y = fmaf(d, T2.y, accA.y);
-                    accA.z = fmaf(d, T2.z, accA.z); accA.w = fmaf(d, T2.w, accA.w);
-                    accB[m2].x = fmaf(d, T1[j].x, accB[m2].x); accB[m2].y = fmaf(d, T1[j].y, accB[m2].y);
-                    accB[m2].z = fmaf(d, T1[j].z, accB[m2].z); accB[m2].w = fmaf(d, T1[j].w, accB[m2].w);
+                for (int k = 0; k < 8; ++k) {
+                    const float d = __uint_as_float(v[k]);      // the common factor 1 / scale is applied at the stores
+                    accA.x = fmaf(d, T2[k].x, accA.x); accA.y = fmaf(d, T2[k].y, accA.y);
+                    accA.z = fmaf(d, T2[k].z, accA.z); accA.w = fmaf(d, T2[k].w, accA.w);
+                    accB[k].x = fmaf(d, t1.x, accB[k].x); accB[k].y = fmaf(d, t1.y, accB[k].y);
+                    accB[k].z = fmaf(d, t1.z, accB[k].z); accB[k].w = fmaf(d, t1.w, accB[k].w);
                 }
-                accA.x *= inv_scale; accA.y *= inv_scale; accA.z *= inv_scale; accA.w *= inv_scale;
-                if (row_ok) dTrow[nc * (BN / 16) + JH * half + j] = accA;
+                T1[j] = more ? __ldg(Trow + (nc + 1) * NJ + j) : zero4;
+                if (j >= JH * half && j < JH * half + JH) keep[j - JH * half] = accA;      // mine to finalise
+                else xw[(j - JH * (1 - half)) * 128] = accA;                                // my partner's
             }
             tc_fence_before();
             mbar_arrive(tmem_empty + buf);
+            asm volatile("bar.sync %0, 64;" ::"r"(bar_id) : "memory");
+            if (row_ok) {
 #pragma unroll
-            for (int j = 0; j < JH; ++j) T1[j] = T1n[j];
+                for (int jj = 0; jj < JH; ++jj) {
+                    const float4 x = xr[jj * 128];
+                    dTrow[nc * NJ + JH * half + jj] = make_float4((keep[jj].x + x.x) * inv_scale, (keep[jj].y + x.y) * inv_scale,
+                                                                   (keep[jj].z + x.z) * inv_scale, (keep[jj].w + x.w) * inv_scale);
+                }
+            }
+            asm volatile("bar.sync %0, 64;" ::"r"(bar_id) : "memory");     // the buffer is free again; orders the stores too
         }
-        // second term: the two warps of a quarter hold shares over disjoint m1; the second warp hands its share over
-        // through the (now idle: the last tmem_full says every MMA has retired) stage memory, the first adds both to
-        // the rows m < 16, which either warp may have stored above (bar.sync orders those stores)
-        float4* xch = reinterpret_cast<float4*>(smem) + (quarter * 32 + lane);
-        if (half == 1) {
+        // second term: complete in this warp for its eight m2 (it saw every m1); the rows m < 16 it is added to were
+        // stored above by either warp of the quarter, ordered by the barrier that closed the last chunk
+        if (row_ok) {
 #pragma unroll
-            for (int m2 = 0; m2 < 16; ++m2) xch[m2 * 128] = accB[m2];
-        }
-        __threadfence_block();
-        asm volatile("bar.sync %0, 64;" ::"r"(1 + quarter) : "memory");
-        if (half == 0 && row_ok) {
-#pragma unroll
-            for (int m2 = 0; m2 < 16; ++m2) {
-                float4 o = dTrow[m2];
-                const float4 x = xch[m2 * 128];
-                o.x = fmaf(accB[m2].x + x.x, inv_scale, o.x); o.y = fmaf(accB[m2].y + x.y, inv_scale, o.y);
-                o.z = fmaf(accB[m2].z + x.z, inv_scale, o.z); o.w = fmaf(accB[m2].w + x.w, inv_scale, o.w);
-                dTrow[m2] = o;
+            for (int k = 0; k < 8; ++k) {
+                float4 o = dTrow[8 * half + k];
+                o.x = fmaf(accB[k].x, inv_scale, o.x); o.y = fmaf(accB[k].y, inv_scale, o.y);
+                o.z = fmaf(accB[k].z, inv_scale, o.z); o.w = fmaf(accB[k].w, inv_scale, o.w);
+                dTrow[8 * half + k] = o;
             }
         }
+        };
+        if (warp < 6) epilogue(std::integral_constant<int, 0>{});
+        else epilogue(std::integral_constant<int, 1>{});
     }
     tc_fence_before();
     __syncthreads();
@@ -763,17 +794,16 @@ bool tc_make_map_h(CUtensorMap* map, const uint16_t* base, uint64_t rows, uint64
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-// the same matrix walked one k-step at a time: box = 16 halfs x box_rows, SWIZZLE_32B (fitting_mid.cu)
-bool tc_make_map_h16(CUtensorMap* map, const uint16_t* base, uint64_t rows, uint64_t cols, uint64_t ld, uint32_t box_rows) {
-    EncodeTiledFn enc = get_encode();
-    if (!enc) return false;
-    cuuint64_t dims[2] = {cols, rows};
-    cuuint64_t strides[1] = {ld * 2};
-    cuuint32_t box[2] = {16, box_rows};
-    cuuint32_t estr[2] = {1, 1};
-    return enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, const_cast<uint16_t*>(base), dims, strides, box, estr,
-               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_32B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+// operand images of the first fitting layer (see kmajor_image in fitting_mid.cu): W is [ND][NF] row-major, WT [NF][ND]
+size_t l1_wimg_bytes(int ND) { return (size_t)(ND / 32) * 2 * L1Smem::kBBytes; }
+void l1_build_wimg(const float* WT, int ND, uint8_t* img) {
+    for (int kb = 0; kb < ND / 32; ++kb) kmajor_image(WT, kL1BN, ND, 0, kL1BN, 32 * kb, 32, kW1Scale, img + (size_t)kb * 2 * L1Smem::kBBytes);
+}
+size_t dd_wimg_bytes(int ND) { return (size_t)(ND / kDdBN) * 8 * 2 * DdSmem::kBBytes; }
+void dd_build_wimg(const float* W, int ND, uint8_t* img) {
+    for (int nc = 0; nc < ND / kDdBN; ++nc)
+        for (int kb = 0; kb < 8; ++kb)
+            kmajor_image(W, ND, kL1BN, nc * kDdBN, kDdBN, 32 * kb, 32, kW1Scale, img + (size_t)(nc * 8 + kb) * 2 * DdSmem::kBBytes);
 }
 
 // FP16 split of scale * w: hi = fp16(v), lo = fp16(v - hi)
@@ -866,10 +896,6 @@ bool tc_setup_maps(Model& m, int ntypes) {
         ok &= tc_make_map(&m.mapA_G2[t], m.G2 + row0 * NF, rows, NF, NF, 128);
         ok &= tc_make_map_h(&m.mapAh_G1[t], m.da1_h_hi + row0 * NF, rows, NF, NF, 128);
         ok &= tc_make_map_h(&m.mapAh_G2[t], m.da1_h_lo + row0 * NF, rows, NF, NF, 128);
-        ok &= tc_make_map_h(&m.mapBh_l1_hi[t], m.w1T_h_hi[t], NF, ND, ND, 240);
-        ok &= tc_make_map_h(&m.mapBh_l1_lo[t], m.w1T_h_lo[t], NF, ND, ND, 240);
-        ok &= tc_make_map_h(&m.mapBh_dd_hi[t], m.w1_h_hi[t], ND, NF, NF, 160);
-        ok &= tc_make_map_h(&m.mapBh_dd_lo[t], m.w1_h_lo[t], ND, NF, NF, 160);
         ok &= tc_make_map(&m.mapA_T3[t], m.T3 + row0 * NF, rows, NF, NF, 128);
         for (int l = 0; l < 3; ++l) {
             const uint64_t nin = (l == 0) ? ND : NF;
@@ -906,10 +932,10 @@ static int chain_range(Model& m, const ForceArgs& fa, int t0, int ntl, cudaStrea
         L1Args a1{};
         a1.tile_off = t0;
         a1.ntypes = nt; a1.K = ND; a1.Tm = m.Tm; a1.out = m.Y1; a1.ldo = NF; a1.M1 = m.M1;
-        if (fused) { a1.out_hi = reinterpret_cast<__half*>(m.y1_h_hi); a1.out_lo = reinterpret_cast<__half*>(m.y1_h_lo); }
+        if (fused) a1.out_img = m.y1_img;
         for (int t = 0; t <= kMaxT; ++t) { a1.tile0[t] = g.tile0[t]; a1.row0[t] = g.row0[t]; }
         for (int t = 0; t < nt; ++t) a1.bias[t] = m.fit_b[t][0];
-        for (int t = 0; t < kMaxT; ++t) { const int q = t < nt ? t : 0; mp.A[t] = m.mapA_D[q]; mp.Bhi[t] = m.mapBh_l1_hi[q]; mp.Blo[t] = m.mapBh_l1_lo[q]; }
+        for (int t = 0; t < kMaxT; ++t) { const int q = t < nt ? t : 0; mp.A[t] = m.mapA_D[q]; mp.Bhi[t] = m.mapA_D[q]; mp.Blo[t] = m.mapA_D[q]; a1.wimg[t] = m.l1_wimg[q]; }
         l1_desc_kernel<<<ntl, kL1Threads, L1Smem::kTotal, s>>>(mp, a1);
     }
     if (fused) {
@@ -947,7 +973,9 @@ static int chain_range(Model& m, const ForceArgs& fa, int t0, int ntl, cudaStrea
         for (int t = 0; t < kMaxT; ++t) {
             const int q = t < nt ? t : 0;
             dm.Ahi[t] = m.mapAh_G1[q]; dm.Alo[t] = m.mapAh_G2[q];
-            dm.Bhi[t] = m.mapBh_dd_hi[q]; dm.Blo[t] = m.mapBh_dd_lo[q];
+            dm.Bhi[t] = dm.Ahi[t]; dm.Blo[t] = dm.Alo[t];
+            d.wimg[t] = m.dd_wimg[q];
+            d.a_img = fused ? m.da1_img : nullptr;
         }
         dd_dt_kernel<<<ntl, kL1Threads, DdSmem::kTotal, s>>>(dm, d);
     }
