@@ -140,45 +140,39 @@ fit_mid_kernel(const __grid_constant__ MidArgs g) {
     tc_fence_after();
     const uint32_t tmem = *tmem_ptr;
 
+    // control warps: all 32 lanes run the loop converged, one elected lane issues (tc_gemm.cuh)
     if (warp == 0) {
-        if (lane == 0) {
-            // the resident A operand: the y1 image of this tile, FP16 hi then lo (columns 240..255 of the last K block are never read)
-            const uint8_t* img = g.y1_img + (size_t)tile * kImage;
-            mbar_arrive_expect_tx(a_full, kImage);
-            bulk_load(smem + oAhi, img, kAcopy, a_full);
-            bulk_load(smem + oAlo, img + kAcopy, kAcopy, a_full);
-            // the weights of the four phases, one k-step per stage; the ring runs ahead across the phase boundaries
-            for (int it = 0; it < 4 * kKS; ++it) {
-                const int s = it % kST, ph = (it / kST) & 1;
-                mbar_wait(empty + s, ph ^ 1);
-                mbar_arrive_expect_tx(full + s, kStage);
-                bulk_load(smem + oB + s * kStage, g.wimg[ty] + (size_t)it * kStage, kStage, full + s);
-            }
+        // the resident A operand: the y1 image of this tile, FP16 hi then lo (columns 240..255 of the last K block are never read)
+        bulk_load_expect_elect(smem + oAhi, g.y1_img + (size_t)tile * kImage, kImage, a_full);
+        // the weights of the four phases, one k-step per stage; the ring runs ahead across the phase boundaries
+        const uint8_t* wimg = g.wimg[ty];
+        int s = 0, ph = 1;
+        for (int it = 0; it < 4 * kKS; ++it) {
+            mbar_wait(empty + s, ph);
+            bulk_load_expect_elect(smem + oB + s * kStage, wimg + (size_t)it * kStage, kStage, full + s);
+            if (++s == kST) { s = 0; ph ^= 1; }
         }
     } else if (warp == 1) {
-        if (lane == 0) {
-            constexpr uint32_t idesc = make_idesc_f16(128, kN);
-            const uint32_t a_hi = smem_u32(smem + oAhi), a_lo = smem_u32(smem + oAlo);
-            mbar_wait(a_full, 0);
-            for (int p = 0; p < 4; ++p) {
-                const uint32_t acc = tmem + (uint32_t)(p & 1) * 256;
-                for (int ks = 0; ks < kKS; ++ks) {
-                    const int it = p * kKS + ks;
-                    const int s = it % kST, ph = (it / kST) & 1;
-                    if (p > 0) mbar_wait(chunk_ready + ks, (p - 1) & 1);     // k-step ks of this operand = chunk ks of the last epilogue
-                    mbar_wait(full + s, ph);
-                    tc_fence_after();
-                    const uint32_t aoff = (uint32_t)((ks >> 1) * (128 * 64) + (ks & 1) * 32);
-                    const uint32_t st = smem_u32(smem + oB + s * kStage);
-                    const uint64_t dah = make_smem_desc_kmajor(a_hi + aoff, 64), dal = make_smem_desc_kmajor(a_lo + aoff, 64);
-                    const uint64_t dbh = make_smem_desc_kmajor(st, 32), dbl = make_smem_desc_kmajor(st + kBcopy, 32);
-                    umma_f16(acc, dah, dbh, idesc, ks ? 1u : 0u);
-                    umma_f16(acc, dal, dbh, idesc, 1u);
-                    umma_f16(acc, dah, dbl, idesc, 1u);
-                    umma_commit(empty + s);
-                }
-                umma_commit(acc_full + (p & 1));
+        constexpr uint32_t idesc = make_idesc_f16(128, kN);
+        const uint32_t sb = smem_u32(smem);
+        const uint64_t dAh = make_smem_desc_kmajor(sb + oAhi, 64), dAl = make_smem_desc_kmajor(sb + oAlo, 64);
+        const uint64_t dBh = make_smem_desc_kmajor(sb + oB, 32), dBl = make_smem_desc_kmajor(sb + oB + kBcopy, 32);
+        mbar_wait(a_full, 0);
+        int s = 0, ph = 0;
+        for (int p = 0; p < 4; ++p) {
+            const uint32_t acc = tmem + (uint32_t)(p & 1) * 256;
+            for (int ks = 0; ks < kKS; ++ks) {
+                if (p > 0) mbar_wait(chunk_ready + ks, (p - 1) & 1);     // k-step ks of this operand = chunk ks of the last epilogue
+                mbar_wait(full + s, ph);
+                tc_fence_after();
+                const uint64_t ao = (uint64_t)(((ks >> 1) * (128 * 64) + (ks & 1) * 32) >> 4), bo = (uint64_t)((s * kStage) >> 4);
+                umma_f16_elect(acc, dAh + ao, dBh + bo, idesc, ks ? 1u : 0u);
+                umma_f16_elect(acc, dAl + ao, dBh + bo, idesc, 1u);
+                umma_f16_elect(acc, dAh + ao, dBl + bo, idesc, 1u);
+                umma_commit_elect(empty + s);
+                if (++s == kST) { s = 0; ph ^= 1; }
             }
+            umma_commit_elect(acc_full + (p & 1));
         }
     } else {
         // ---- epilogues: thread <-> tile row (= TMEM lane); two warps per lane quarter, warp `half` of a quarter takes the

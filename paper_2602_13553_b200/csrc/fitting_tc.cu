@@ -387,39 +387,36 @@ l1_desc_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ L1Ar
     tc_fence_after();
     const uint32_t tmem_base = *tmem_ptr;
 
+    // control warps: all 32 lanes run the loop converged, one elected lane issues (tc_gemm.cuh)
     if (warp == 0) {
-        if (lane == 0) {
-            for (int kb = 0; kb < nk; ++kb) {
-                const int s = kb % ST, ph = (kb / ST) & 1;
-                mbar_wait(empty + s, ph ^ 1);
-                uint8_t* st = smem + s * SM::kStage;
-                mbar_arrive_expect_tx(full + s, 2 * SM::kBBytes);
-                bulk_load(st + SM::oBhi, g.wimg[ty] + (size_t)kb * (2 * SM::kBBytes), 2 * SM::kBBytes, full + s);
-            }
+        const uint8_t* wimg = g.wimg[ty];
+        int s = 0, ph = 1;
+        for (int kb = 0; kb < nk; ++kb) {
+            mbar_wait(empty + s, ph);
+            bulk_load_expect_elect(smem + s * SM::kStage + SM::oBhi, wimg + (size_t)kb * (2 * SM::kBBytes), 2 * SM::kBBytes, full + s);
+            if (++s == ST) { s = 0; ph ^= 1; }
         }
     } else if (warp == 1) {
-        if (lane == 0) {
-            constexpr uint32_t idesc = make_idesc_f16(128, BN);
-            for (int kb = 0; kb < nk; ++kb) {
-                const int s = kb % ST, ph = (kb / ST) & 1;
-                mbar_wait(full + s, ph);
-                mbar_wait(ready + s, ph);
-                tc_fence_after();
-                const uint32_t st = smem_u32(smem + s * SM::kStage);
-#pragma unroll
-                for (int ks = 0; ks < 2; ++ks) {
-                    const uint64_t a_hi = make_smem_desc_kmajor(st + SM::oAhi + ks * 32, 64);
-                    const uint64_t a_lo = make_smem_desc_kmajor(st + SM::oAlo + ks * 32, 64);
-                    const uint64_t b_hi = make_smem_desc_kmajor(st + SM::oBhi + ks * 32, 64);
-                    const uint64_t b_lo = make_smem_desc_kmajor(st + SM::oBlo + ks * 32, 64);
-                    umma_f16(tmem_base, a_hi, b_hi, idesc, (kb | ks) ? 1u : 0u);
-                    umma_f16(tmem_base, a_lo, b_hi, idesc, 1u);
-                    umma_f16(tmem_base, a_hi, b_lo, idesc, 1u);
-                }
-                umma_commit(empty + s);
-            }
-            umma_commit(tmem_full);
+        constexpr uint32_t idesc = make_idesc_f16(128, BN);
+        const uint32_t sb = smem_u32(smem);
+        const uint64_t dAh = make_smem_desc_kmajor(sb + SM::oAhi, 64), dAl = make_smem_desc_kmajor(sb + SM::oAlo, 64);
+        const uint64_t dBh = make_smem_desc_kmajor(sb + SM::oBhi, 64), dBl = make_smem_desc_kmajor(sb + SM::oBlo, 64);
+        int s = 0, ph = 0;
+        for (int kb = 0; kb < nk; ++kb) {
+            mbar_wait(full + s, ph);
+            mbar_wait(ready + s, ph);
+            tc_fence_after();
+            const uint64_t so = (uint64_t)((s * SM::kStage) >> 4);
+            umma_f16_elect(tmem_base, dAh + so, dBh + so, idesc, kb ? 1u : 0u);
+            umma_f16_elect(tmem_base, dAl + so, dBh + so, idesc, 1u);
+            umma_f16_elect(tmem_base, dAh + so, dBl + so, idesc, 1u);
+            umma_f16_elect(tmem_base, dAh + so + 2, dBh + so + 2, idesc, 1u);
+            umma_f16_elect(tmem_base, dAl + so + 2, dBh + so + 2, idesc, 1u);
+            umma_f16_elect(tmem_base, dAh + so + 2, dBl + so + 2, idesc, 1u);
+            umma_commit_elect(empty + s);
+            if (++s == ST) { s = 0; ph ^= 1; }
         }
+        umma_commit_elect(tmem_full);
     } else {
         // two warps per TMEM lane quarter (a warp alone on its scheduler cannot hide the latency of its own loads and
         // conversions; the round-2 profile had the tensor pipe 46 % active behind four producer warps): warp `half`
@@ -611,53 +608,76 @@ dd_dt_kernel(const __grid_constant__ DdMaps maps, const __grid_constant__ DdDtAr
     tc_fence_after();
     const uint32_t tmem_base = *tmem_ptr;
 
+    // The two control warps run their loops with all 32 lanes converged and let one elected lane issue (tc_gemm.cuh):
+    // with N = 160 an MMA lasts 80 clk, which the single-lane form of the issue loop did not keep up with.
     if (warp == 0) {
-        if (lane == 0) {
+        if (g.a_img) {
+            const uint8_t* aimg = g.a_img + (size_t)tile * 131072;
+            const uint8_t* wimg = g.wimg[ty];
+            int s = 0, ph = 1;
+            for (int nc = 0; nc < nch; ++nc)
+                for (int kb = 0; kb < nk; ++kb) {
+                    mbar_wait(empty + s, ph);
+                    uint8_t* st = smem + s * SM::kStage;
+                    // one barrier, two copies: the expect_tx of the first covers both
+                    asm volatile(
+                        "{\n\t"
+                        ".reg .pred q;\n\t"
+                        "elect.sync _|q, 0xffffffff;\n\t"
+                        "@q mbarrier.arrive.expect_tx.shared::cta.b64 _, [%6], %5;\n\t"
+                        "@q cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%6];\n\t"
+                        "@q cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%3], [%4], %7, [%6];\n\t"
+                        "}" ::"r"(smem_u32(st + SM::oAhi)),
+                        "l"(aimg + kb * (2 * SM::kABytes)), "r"(2 * SM::kABytes), "r"(smem_u32(st + SM::oBhi)),
+                        "l"(wimg + (size_t)(nc * nk + kb) * (2 * SM::kBBytes)), "r"(2 * SM::kABytes + 2 * SM::kBBytes), "r"(smem_u32(full + s)),
+                        "r"(2 * SM::kBBytes)
+                        : "memory");
+                    if (++s == ST) { s = 0; ph ^= 1; }
+                }
+        } else if (lane == 0) {
             for (int it = 0; it < nch * nk; ++it) {
                 const int nc = it / nk, kb = it - nc * nk;
                 const int s = it % ST, ph = (it / ST) & 1;
                 mbar_wait(empty + s, ph ^ 1);
                 uint8_t* st = smem + s * SM::kStage;
                 mbar_arrive_expect_tx(full + s, 2 * SM::kABytes + 2 * SM::kBBytes);
-                if (g.a_img) {
-                    bulk_load(st + SM::oAhi, g.a_img + (size_t)tile * 131072 + kb * (2 * SM::kABytes), 2 * SM::kABytes, full + s);
-                } else {
-                    tma_load_2d(st + SM::oAhi, &maps.Ahi[ty], full + s, kb * 32, m0);
-                    tma_load_2d(st + SM::oAlo, &maps.Alo[ty], full + s, kb * 32, m0);
-                }
+                tma_load_2d(st + SM::oAhi, &maps.Ahi[ty], full + s, kb * 32, m0);
+                tma_load_2d(st + SM::oAlo, &maps.Alo[ty], full + s, kb * 32, m0);
                 bulk_load(st + SM::oBhi, g.wimg[ty] + (size_t)it * (2 * SM::kBBytes), 2 * SM::kBBytes, full + s);
+                (void)nc;
             }
         }
     } else if (warp == 1) {
-        if (lane == 0) {
-            constexpr uint32_t idesc = make_idesc_f16(128, BN);
-            for (int nc = 0; nc < nch; ++nc) {
-                const int buf = nc & 1;
-                if (nc >= 2) {                     // the epilogue has drained this buffer (chunk nc - 2)
-                    mbar_wait(tmem_empty + buf, ((nc >> 1) - 1) & 1);
-                    tc_fence_after();
-                }
-                const uint32_t dcol = tmem_base + buf * 256;
-                for (int kb = 0; kb < nk; ++kb) {
-                    const int it = nc * nk + kb;
-                    const int s = it % ST, ph = (it / ST) & 1;
-                    mbar_wait(full + s, ph);
-                    tc_fence_after();
-                    const uint32_t st = smem_u32(smem + s * SM::kStage);
-                    const int nks = (kb == nk - 1 && (g.K & 31)) ? 1 : 2;   // K = 240: the last block holds one k-step (the image has no zero padding behind it)
-                    for (int ks = 0; ks < nks; ++ks) {
-                        const uint64_t a_hi = make_smem_desc_kmajor(st + SM::oAhi + ks * 32, 64);
-                        const uint64_t a_lo = make_smem_desc_kmajor(st + SM::oAlo + ks * 32, 64);
-                        const uint64_t b_hi = make_smem_desc_kmajor(st + SM::oBhi + ks * 32, 64);
-                        const uint64_t b_lo = make_smem_desc_kmajor(st + SM::oBlo + ks * 32, 64);
-                        umma_f16(dcol, a_hi, b_hi, idesc, (kb | ks) ? 1u : 0u);
-                        umma_f16(dcol, a_lo, b_hi, idesc, 1u);
-                        umma_f16(dcol, a_hi, b_lo, idesc, 1u);
-                    }
-                    umma_commit(empty + s);
-                }
-                umma_commit(tmem_full + buf);
+        constexpr uint32_t idesc = make_idesc_f16(128, BN);
+        // descriptors of stage 0; stage s and k-step ks add (s kStage + 32 ks) >> 4 to the address field
+        const uint32_t sb = smem_u32(smem);
+        const uint64_t dAh = make_smem_desc_kmajor(sb + SM::oAhi, 64), dAl = make_smem_desc_kmajor(sb + SM::oAlo, 64);
+        const uint64_t dBh = make_smem_desc_kmajor(sb + SM::oBhi, 64), dBl = make_smem_desc_kmajor(sb + SM::oBlo, 64);
+        const bool short_last = (g.K & 31) != 0;      // K = 240: the last block holds one k-step (the image has no zero padding behind it)
+        int s = 0, ph = 0;
+        for (int nc = 0; nc < nch; ++nc) {
+            const int buf = nc & 1;
+            if (nc >= 2) {                     // the epilogue has drained this buffer (chunk nc - 2)
+                mbar_wait(tmem_empty + buf, ((nc >> 1) - 1) & 1);
+                tc_fence_after();
             }
+            const uint32_t dcol = tmem_base + buf * 256;
+            for (int kb = 0; kb < nk; ++kb) {
+                mbar_wait(full + s, ph);
+                tc_fence_after();
+                const uint64_t so = (uint64_t)((s * SM::kStage) >> 4);
+                umma_f16_elect(dcol, dAh + so, dBh + so, idesc, kb ? 1u : 0u);
+                umma_f16_elect(dcol, dAl + so, dBh + so, idesc, 1u);
+                umma_f16_elect(dcol, dAh + so, dBl + so, idesc, 1u);
+                if (!(short_last && kb == nk - 1)) {
+                    umma_f16_elect(dcol, dAh + so + 2, dBh + so + 2, idesc, 1u);
+                    umma_f16_elect(dcol, dAl + so + 2, dBh + so + 2, idesc, 1u);
+                    umma_f16_elect(dcol, dAh + so + 2, dBl + so + 2, idesc, 1u);
+                }
+                umma_commit_elect(empty + s);
+                if (++s == ST) { s = 0; ph ^= 1; }
+            }
+            umma_commit_elect(tmem_full + buf);
         }
     } else {
         // Two warps per TMEM lane quarter (a warp alone on its scheduler ran this loop at 0.16 IPC); warp `half` owns the
