@@ -130,6 +130,23 @@ __device__ __forceinline__ void mma_3x_f16(uint32_t d_tmem, uint32_t a_hi, uint3
     }
 }
 
+// the same by a converged warp (one elected lane issues, tc_gemm.cuh), descriptors built once per product: with
+// N = 64 / 112 an MMA lasts 32 / 56 clk and the issue loop, not the tensor pipe, sets the length of the round trip
+template <int ROWB>
+__device__ __forceinline__ void mma_3x_f16_elect(uint32_t d_tmem, uint32_t a_hi, uint32_t a_lo, uint32_t b_hi, uint32_t b_lo,
+                                                 uint32_t idesc, int nks) {
+    const uint64_t dah = make_smem_desc_kmajor(a_hi, ROWB), dal = make_smem_desc_kmajor(a_lo, ROWB);
+    const uint64_t dbh = make_smem_desc_kmajor(b_hi, ROWB), dbl = make_smem_desc_kmajor(b_lo, ROWB);
+#pragma unroll
+    for (int ks = 0; ks < 4; ++ks) {
+        if (ks >= nks) break;
+        const uint64_t o = (uint64_t)(2 * ks);             // 32 bytes of K per step, address field in units of 16 B
+        umma_f16_elect(d_tmem, dah + o, dbh + o, idesc, ks == 0 ? 0u : 1u);
+        umma_f16_elect(d_tmem, dal + o, dbh + o, idesc, 1u);
+        umma_f16_elect(d_tmem, dah + o, dbl + o, idesc, 1u);
+    }
+}
+
 struct EmbTcArgs {
     int PN, N, ntypes, nsel;
     int seloff[PIMD_MAX_TYPES + 1];
@@ -282,7 +299,7 @@ struct CtxSetup {
 };
 
 // common prologue: barriers, TMEM allocation of `ncols` columns; returns after a CTA-wide sync
-__device__ __forceinline__ CtxSetup ctx_setup_at(uint8_t* smem_raw, uint32_t ncols, int img_pad, int ctx_bytes) {
+__device__ __forceinline__ CtxSetup ctx_setup_at(uint8_t* smem_raw, uint32_t ncols, int img_pad, int ctx_bytes, int commits = 1) {
     CtxSetup c;
     // pad to 1024 B by pointer arithmetic on the __shared__ array (a uintptr_t round trip loses the address
     // space and turns every access into a generic LD/ST)
@@ -293,8 +310,8 @@ __device__ __forceinline__ CtxSetup ctx_setup_at(uint8_t* smem_raw, uint32_t nco
     c.mma_bar = bars + wg;
     uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(bars + 2);
     if (threadIdx.x == 0) {
-        mbar_init(bars, 1);
-        mbar_init(bars + 1, 1);
+        mbar_init(bars, commits);          // tcgen05.commit arrivals per MMA round trip
+        mbar_init(bars + 1, commits);
         fence_barrier_init();
     }
     if ((threadIdx.x >> 5) == 0) tmem_alloc(tmem_ptr, ncols);
@@ -436,10 +453,10 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
             fence_proxy_async_smem();
             tc_fence_before();
             named_bar_sync(bar_ctx, 128);
-            if (t == 0) {
+            if (t < 32) {
                 tc_fence_after();
-                mma_3x_f16<64>(tmem_d, actx + eh::oA1hi, actx + eh::oA1lo, wbase + eh::oW2hi, wbase + eh::oW2lo, idesc2, 2);
-                umma_commit(mma_bar);
+                mma_3x_f16_elect<64>(tmem_d, actx + eh::oA1hi, actx + eh::oA1lo, wbase + eh::oW2hi, wbase + eh::oW2lo, idesc2, 2);
+                umma_commit_elect(mma_bar);
             }
             mbar_wait(mma_bar, phase);
             phase ^= 1;
@@ -467,10 +484,10 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
             fence_proxy_async_smem();
             tc_fence_before();
             named_bar_sync(bar_ctx, 128);
-            if (t == 0) {
+            if (t < 32) {
                 tc_fence_after();
-                mma_3x_f16<128>(tmem_d, actx + eh::oA2hi, actx + eh::oA2lo, wbase + eh::oW3hi, wbase + eh::oW3lo, idesc3, 4);
-                umma_commit(mma_bar);
+                mma_3x_f16_elect<128>(tmem_d, actx + eh::oA2hi, actx + eh::oA2lo, wbase + eh::oW3hi, wbase + eh::oW3lo, idesc3, 4);
+                umma_commit_elect(mma_bar);
             }
             mbar_wait(mma_bar, phase);
             phase ^= 1;
@@ -576,7 +593,7 @@ __global__ void __launch_bounds__(etc::kThreads, 1)
 embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
     using namespace etc;
     extern __shared__ uint8_t smem_raw[];
-    const CtxSetup cs = ctx_setup_at(smem_raw, 512, kImgPadBwd, kCtxBytes);
+    const CtxSetup cs = ctx_setup_at(smem_raw, 512, kImgPadBwd, kCtxBytes, 2);
     const int cx = threadIdx.x >> 8, half = (threadIdx.x >> 7) & 1, t = threadIdx.x & 127, lane = threadIdx.x & 31;
     const int bar_ctx = 1 + cx, bar_pair = 3 + cx * 4 + (t >> 5);
     uint8_t* ctx = cs.ctx;
@@ -668,11 +685,12 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
             fence_proxy_async_smem();
             tc_fence_before();
             named_bar_sync(bar_ctx, 256);
-            if ((threadIdx.x & 255) == 0) {
+            // the value and the derivative products are independent: two warps issue them side by side (the barrier counts both commits)
+            if ((threadIdx.x & 255) < 64) {
                 tc_fence_after();
-                mma_3x_f16<64>(tmem_v, actx, actx + 8192, wbase + eh::oW2hi, wbase + eh::oW2lo, idesc2, 2);
-                mma_3x_f16<64>(tmem_g, actx + 16384, actx + 24576, wbase + eh::oW2hi, wbase + eh::oW2lo, idesc2, 2);
-                umma_commit(cs.mma_bar);
+                if ((threadIdx.x & 255) < 32) mma_3x_f16_elect<64>(tmem_v, actx, actx + 8192, wbase + eh::oW2hi, wbase + eh::oW2lo, idesc2, 2);
+                else mma_3x_f16_elect<64>(tmem_g, actx + 16384, actx + 24576, wbase + eh::oW2hi, wbase + eh::oW2lo, idesc2, 2);
+                umma_commit_elect(cs.mma_bar);
             }
             mbar_wait(cs.mma_bar, phase);
             phase ^= 1;
@@ -708,11 +726,11 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
             fence_proxy_async_smem();
             tc_fence_before();
             named_bar_sync(bar_ctx, 256);
-            if ((threadIdx.x & 255) == 0) {
+            if ((threadIdx.x & 255) < 64) {
                 tc_fence_after();
-                mma_3x_f16<128>(tmem_v, actx, actx + 16384, wbase + eh::oW3hi, wbase + eh::oW3lo, idesc3, 4);
-                mma_3x_f16<128>(tmem_g, actx + oY, actx + oY + 16384, wbase + eh::oW3hi, wbase + eh::oW3lo, idesc3, 4);
-                umma_commit(cs.mma_bar);
+                if ((threadIdx.x & 255) < 32) mma_3x_f16_elect<128>(tmem_v, actx, actx + 16384, wbase + eh::oW3hi, wbase + eh::oW3lo, idesc3, 4);
+                else mma_3x_f16_elect<128>(tmem_g, actx + oY, actx + oY + 16384, wbase + eh::oW3hi, wbase + eh::oW3lo, idesc3, 4);
+                umma_commit_elect(cs.mma_bar);
             }
             // ---- while the MMAs run: dT of this tile's centres goes global -> shared by cp.async (no registers in
             // between), and the rest of my row arrives ----
