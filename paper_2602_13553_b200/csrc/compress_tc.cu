@@ -71,6 +71,19 @@ __device__ __forceinline__ void umma_f16_ts(uint32_t tmem_d, uint32_t tmem_a, ui
         "r"(tmem_a), "l"(bdesc), "r"(idesc), "r"(accumulate)
         : "memory");
 }
+// the same issued by one elected lane of a converged warp (tc_gemm.cuh: the single-lane form costs ~77 clk per MMA,
+// and with N = 32 an MMA lasts 16 clk, so the issue loop is the length of the round trip)
+__device__ __forceinline__ void umma_f16_ts_elect(uint32_t tmem_d, uint32_t tmem_a, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p, q;\n\t"
+        "elect.sync _|q, 0xffffffff;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "@q tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t"
+        "}" ::"r"(tmem_d),
+        "r"(tmem_a), "l"(bdesc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
 // 32 lanes x 8 columns: register i of lane t -> TMEM[lane_base + t][col + i]
 __device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t* v) {
     asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"r"(taddr), "r"(v[0]),
@@ -358,24 +371,23 @@ cmp_fwd_kernel(const __grid_constant__ CmpArgs a) {
                     mbar_wait(ready, it & 1);
                     if (it > 0) mbar_wait(d_free, (it - 1) & 1);
                     tc_fence_after();
-                    if (lane == 0) {
+                    {   // all 32 lanes run the (uniform) loop, one elected lane issues
                         uint32_t km = 1u, nd = 0u;                 // k-step 0 always: the accumulator is always written
                         for (int w = 0; w < F_WARPS; ++w) { km |= kmask[w]; nd |= upm[w] << (w & 1); }
-                        a.need[row0 / TC + ti + tile] = nd;
-                        const uint32_t bh = smem_u32(opB_hi), bl = smem_u32(opB_lo);
+                        if (lane == 0) a.need[row0 / TC + ti + tile] = nd;
+                        const uint64_t dbh0 = make_smem_desc_kmajor(smem_u32(opB_hi), 128), dbl0 = make_smem_desc_kmajor(smem_u32(opB_lo), 128);
                         uint32_t acc = 0;
                         for (int ks = 0; ks < K / 16; ++ks) {
                             if (!((km >> ks) & 1u)) continue;
-                            const uint32_t boff = (uint32_t)((ks >> 2) * (NROW * 128) + (ks & 3) * 32);
-                            const uint64_t dbh = make_smem_desc_kmajor(bh + boff, 128), dbl = make_smem_desc_kmajor(bl + boff, 128);
+                            const uint64_t bo = (uint64_t)(((ks >> 2) * (NROW * 128) + (ks & 3) * 32) >> 4);
                             const uint32_t ahi = tmem + ks * 8, alo = tmem + FW_COLS + ks * 8;
-                            umma_f16_ts(tmem + FW_D, ahi, dbh, idesc, acc);
-                            umma_f16_ts(tmem + FW_D, alo, dbh, idesc, 1u);
-                            umma_f16_ts(tmem + FW_D, ahi, dbl, idesc, 1u);
+                            umma_f16_ts_elect(tmem + FW_D, ahi, dbh0 + bo, idesc, acc);
+                            umma_f16_ts_elect(tmem + FW_D, alo, dbh0 + bo, idesc, 1u);
+                            umma_f16_ts_elect(tmem + FW_D, ahi, dbl0 + bo, idesc, 1u);
                             acc = 1u;
                         }
-                        umma_commit(opfree);
-                        umma_commit(mma_done);
+                        umma_commit_elect(opfree);
+                        umma_commit_elect(mma_done);
                     }
                     __syncwarp();
                 }
@@ -499,19 +511,19 @@ cmp_bwd_kernel(const __grid_constant__ CmpArgs a) {
                 tc_fence_before();
                 cmp_bar_sync(1, 128);
                 auto issue = [&](int j, int db) {
-                    if (t == 0) {
+                    if (t < 32) {                          // converged warp, one elected lane issues
                         tc_fence_after();
-                        const uint32_t bh = smem_u32(opB_hi), bl = smem_u32(opB_lo);
+                        const uint64_t dbh0 = make_smem_desc_kmajor(smem_u32(opB_hi), 128), dbl0 = make_smem_desc_kmajor(smem_u32(opB_lo), 128);
                         const uint32_t d = tmem + BW_D + db * NROW;
+#pragma unroll
                         for (int ks = 0; ks < BW_KP / 16; ++ks) {
-                            const uint32_t boff = (uint32_t)((ks >> 2) * (NROW * 128) + (ks & 3) * 32);
-                            const uint64_t dbh = make_smem_desc_kmajor(bh + boff, 128), dbl = make_smem_desc_kmajor(bl + boff, 128);
+                            const uint64_t bo = (uint64_t)(((ks >> 2) * (NROW * 128) + (ks & 3) * 32) >> 4);
                             const uint32_t ahi = tmem + j * 2 * BW_COLS + ks * 8, alo = ahi + BW_COLS;
-                            umma_f16_ts(d, ahi, dbh, idesc, ks ? 1u : 0u);
-                            umma_f16_ts(d, alo, dbh, idesc, 1u);
-                            umma_f16_ts(d, ahi, dbl, idesc, 1u);
+                            umma_f16_ts_elect(d, ahi, dbh0 + bo, idesc, ks ? 1u : 0u);
+                            umma_f16_ts_elect(d, alo, dbh0 + bo, idesc, 1u);
+                            umma_f16_ts_elect(d, ahi, dbl0 + bo, idesc, 1u);
                         }
-                        umma_commit(dfull + db);
+                        umma_commit_elect(dfull + db);
                     }
                 };
                 // M tiles of this tile of centres: the lower 20 positions of both neighbour types always (j = 0, 2), the
