@@ -35,7 +35,7 @@ constexpr int oAhi = 0, oAlo = kAcopy, oB = 2 * kAcopy;
 constexpr int oVec = oB + kST * kStage;          // float [3][240]: b2, b3, w4 of this tile's centre type
 constexpr int oEx = oVec + 3 * kN * 4;           // float [128]: energy shares of the second warp of a quarter
 constexpr int oBars = oEx + 128 * 4;
-constexpr int kSmem = oBars + 256 + 1024;
+constexpr int kSmem = oBars + 320 + 1024;          // 35 barriers + the TMEM address
 static_assert(kSmem <= 232448, "shared memory budget");
 constexpr float kWScale = 64.f;        // the weights are split as FP16 pairs of 64 w
 constexpr int kScratch = kKS * 4 * 128 * 16;     // bytes per tile of one scratch array: [chunk 15][float4 4][row 128]
@@ -104,10 +104,10 @@ fit_mid_kernel(const __grid_constant__ MidArgs g) {
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + oBars);
     uint64_t* full = bars;                    // [kST] weights landed -> MMA
     uint64_t* empty = bars + kST;             // [kST] MMA -> TMA
-    uint64_t* a_full = bars + 2 * kST;        // y1 image landed -> MMA, epilogue
-    uint64_t* acc_full = bars + 2 * kST + 1;  // [2] MMA -> epilogue, one per accumulator buffer
-    uint64_t* chunk_ready = bars + 2 * kST + 3;   // [kKS] epilogue -> MMA: columns 16 c .. 16 c + 15 of the next operand are in place (count 128)
-    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(bars + 2 * kST + 3 + kKS);
+    uint64_t* a_full = bars + 2 * kST;        // [8] K block kb of the y1 image landed -> MMA, epilogue
+    uint64_t* acc_full = bars + 2 * kST + 8;  // [2] MMA -> epilogue, one per accumulator buffer
+    uint64_t* chunk_ready = bars + 2 * kST + 10;  // [kKS] epilogue -> MMA: columns 16 c .. 16 c + 15 of the next operand are in place (count 128)
+    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(bars + 2 * kST + 10 + kKS);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int tile = (int)blockIdx.x + g.tile_off;
@@ -120,7 +120,7 @@ fit_mid_kernel(const __grid_constant__ MidArgs g) {
 
     if (warp == 0 && lane == 0) {
         for (int s = 0; s < kST; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, 1); }
-        mbar_init(a_full, 1);
+        for (int kb = 0; kb < 8; ++kb) mbar_init(a_full + kb, 1);
         mbar_init(acc_full, 1);
         mbar_init(acc_full + 1, 1);
         for (int c = 0; c < kKS; ++c) mbar_init(chunk_ready + c, 128);
@@ -143,7 +143,20 @@ fit_mid_kernel(const __grid_constant__ MidArgs g) {
     // control warps: all 32 lanes run the loop converged, one elected lane issues (tc_gemm.cuh)
     if (warp == 0) {
         // the resident A operand: the y1 image of this tile, FP16 hi then lo (columns 240..255 of the last K block are never read)
-        bulk_load_expect_elect(smem + oAhi, g.y1_img + (size_t)tile * kImage, kImage, a_full);
+        // one barrier per K block, so that the first product starts when 16 of the 128 KB are there
+        for (int kb = 0; kb < 8; ++kb) {
+            const uint8_t* img = g.y1_img + (size_t)tile * kImage + kb * 8192;
+            asm volatile(
+                "{\n\t"
+                ".reg .pred q;\n\t"
+                "elect.sync _|q, 0xffffffff;\n\t"
+                "@q mbarrier.arrive.expect_tx.shared::cta.b64 _, [%4], %5;\n\t"
+                "@q cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %6, [%4];\n\t"
+                "@q cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%2], [%3], %6, [%4];\n\t"
+                "}" ::"r"(smem_u32(smem + oAhi + kb * 8192)),
+                "l"(img), "r"(smem_u32(smem + oAlo + kb * 8192)), "l"(img + kAcopy), "r"(smem_u32(a_full + kb)), "r"(16384), "r"(8192)
+                : "memory");
+        }
         // the weights of the four phases, one k-step per stage; the ring runs ahead across the phase boundaries
         const uint8_t* wimg = g.wimg[ty];
         int s = 0, ph = 1;
@@ -157,12 +170,12 @@ fit_mid_kernel(const __grid_constant__ MidArgs g) {
         const uint32_t sb = smem_u32(smem);
         const uint64_t dAh = make_smem_desc_kmajor(sb + oAhi, 64), dAl = make_smem_desc_kmajor(sb + oAlo, 64);
         const uint64_t dBh = make_smem_desc_kmajor(sb + oB, 32), dBl = make_smem_desc_kmajor(sb + oB + kBcopy, 32);
-        mbar_wait(a_full, 0);
         int s = 0, ph = 0;
         for (int p = 0; p < 4; ++p) {
             const uint32_t acc = tmem + (uint32_t)(p & 1) * 256;
             for (int ks = 0; ks < kKS; ++ks) {
                 if (p > 0) mbar_wait(chunk_ready + ks, (p - 1) & 1);     // k-step ks of this operand = chunk ks of the last epilogue
+                else if (!(ks & 1)) mbar_wait(a_full + (ks >> 1), 0);
                 mbar_wait(full + s, ph);
                 tc_fence_after();
                 const uint64_t ao = (uint64_t)(((ks >> 1) * (128 * 64) + (ks & 1) * 32) >> 4), bo = (uint64_t)((s * kStage) >> 4);
@@ -186,7 +199,7 @@ fit_mid_kernel(const __grid_constant__ MidArgs g) {
         float4* t2s = g.sc_t2 + (size_t)tile * (kScratch / 16) + row;      // + (4 c + q) * 128
         float4* g1s = g.sc_g1 + (size_t)tile * (kScratch / 16) + row;
         float e_acc = 0.f;
-        mbar_wait(a_full, 0);                                  // phase 0 reads y1 from the operand
+        for (int kb = 0; kb < 8; ++kb) mbar_wait(a_full + kb, 0);   // phase 0 reads y1 from the operand
 #pragma unroll 1
         for (int p = 0; p < 4; ++p) {
             mbar_wait(acc_full + (p & 1), (p >> 1) & 1);
@@ -296,7 +309,7 @@ fit_mid_kernel(const __grid_constant__ MidArgs g) {
                 bulk_store(img + kb * 16384 + 8192, smem + oAlo + kb * 8192, 8192);
             }
             bulk_commit();
-            bulk_wait0();
+            bulk_wait_read0();                 // shared memory may go once it has been read; the writes complete with the grid
         }
     }
     tc_fence_before();

@@ -525,7 +525,7 @@ l1_desc_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ L1Ar
                 bulk_store(img, smem, 65536);
                 bulk_store(img + 65536, smem + 65536, 65536);
                 bulk_commit();
-                bulk_wait0();
+                bulk_wait_read0();             // shared memory may go once it has been read; the writes complete with the grid
             }
         }
     }
