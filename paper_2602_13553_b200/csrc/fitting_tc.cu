@@ -535,6 +535,203 @@ l1_desc_kernel(const __grid_constant__ TcMaps maps, const __grid_constant__ L1Ar
 }
 
 // ---------------------------------------------------------------------------------------------
+// The same layer with the A operand in TENSOR MEMORY (tcgen05.mma TS mode; the path of the fused chain).  The D block
+// of a stage is produced by the thread that owns the row = TMEM lane, so it goes where it was made: tcgen05.st into
+// a 4-stage ring of 32 columns (16 hi + 16 lo, two FP16 per column) behind the accumulator -- no swizzle, no proxy
+// fence, no shared-memory traffic for A -- and the 128 KB of shared memory this frees hold SEVEN weight stages
+// instead of four: the weight stream through a 4-deep ring was what this kernel waited for (24.9 us with MMAs and
+// producers switched off, profiles/r2_README.md).
+// ---------------------------------------------------------------------------------------------
+struct L1TsSmem {
+    static constexpr int kST = 7;                                          // weight stages
+    static constexpr int kBBytes = kL1BN * 64;                             // one copy (hi or lo) of a K block of 32: 64 B rows, SWIZZLE_64B
+    static constexpr int kStage = 2 * kBBytes;                             // 30720
+    static constexpr int oBias = kST * kStage;                             // float [240]
+    static constexpr int oBars = oBias + kL1BN * 4;
+    static constexpr int kTotal = oBars + 256 + 1024;
+};
+static_assert(L1TsSmem::kTotal <= 232448 && L1TsSmem::oBias >= 131072, "shared memory budget / room for the y1 image");
+constexpr int kL1AST = 4, kL1ACol = 256;      // A ring: stage s at TMEM columns 256 + 32 s (hi: +0..15, lo: +16..31)
+
+__global__ void __launch_bounds__(kL1Threads, 1)
+l1_desc_ts_kernel(const __grid_constant__ L1Args g) {
+    using SM = L1TsSmem;
+    constexpr int ST = SM::kST, AST = kL1AST, BN = kL1BN;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + SM::oBars);
+    uint64_t* b_full = bars;                   // [ST]  weights landed -> MMA
+    uint64_t* b_empty = bars + ST;             // [ST]  MMA -> TMA
+    uint64_t* a_ready = bars + 2 * ST;         // [AST] producers -> MMA (count 256)
+    uint64_t* a_empty = bars + 2 * ST + AST;   // [AST] MMA -> producers
+    uint64_t* tmem_full = bars + 2 * ST + 2 * AST;
+    uint64_t* blk_done = bars + 2 * ST + 2 * AST + 1;   // [8] epilogue -> store: K block kb of the y1 image is complete (count 256)
+    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(bars + 2 * ST + 2 * AST + 9);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int tile = (int)blockIdx.x + g.tile_off;
+    int ty = 0;
+#pragma unroll
+    for (int t = 1; t < kMaxT; ++t)
+        if (t < g.ntypes && tile >= g.tile0[t]) ty = t;
+    const int m0 = (tile - g.tile0[ty]) * 128;
+    const int rows_t = g.row0[ty + 1] - g.row0[ty];
+    const int nk = g.K / 32;                   // K = 16 m1: two m1 per stage
+
+    if (warp == 0 && lane == 0) {
+        for (int s = 0; s < ST; ++s) { mbar_init(b_full + s, 1); mbar_init(b_empty + s, 1); }
+        for (int s = 0; s < AST; ++s) { mbar_init(a_ready + s, 256); mbar_init(a_empty + s, 1); }
+        mbar_init(tmem_full, 1);
+        for (int kb = 0; kb < 8; ++kb) mbar_init(blk_done + kb, 256);
+        fence_barrier_init();
+    }
+    if (warp == 1) tmem_alloc(tmem_ptr, 512);
+    if (threadIdx.x < BN) reinterpret_cast<float*>(smem + SM::oBias)[threadIdx.x] = __ldg(g.bias[ty] + threadIdx.x);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_ptr;
+
+    // control warps: all 32 lanes run the loop converged, one elected lane issues (tc_gemm.cuh)
+    if (warp == 0) {
+        const uint8_t* wimg = g.wimg[ty];
+        int s = 0, ph = 1;
+        for (int kb = 0; kb < nk; ++kb) {
+            mbar_wait(b_empty + s, ph);
+            bulk_load_expect_elect(smem + s * SM::kStage, wimg + (size_t)kb * SM::kStage, SM::kStage, b_full + s);
+            if (++s == ST) { s = 0; ph ^= 1; }
+        }
+        // the y1 image leaves K block by K block, behind the epilogue (a single 128 KB store at the end took 2.4 us)
+        uint8_t* img = g.out_img + (size_t)tile * 131072;
+        for (int kb = 0; kb < 8; ++kb) {
+            mbar_wait(blk_done + kb, 0);
+            if (lane == 0) {
+                bulk_store(img + kb * 8192, smem + kb * 8192, 8192);
+                bulk_store(img + 65536 + kb * 8192, smem + 65536 + kb * 8192, 8192);
+                bulk_commit();
+            }
+        }
+        if (lane == 0) bulk_wait_read0();      // shared memory may go once it has been read; the writes complete with the grid
+    } else if (warp == 1) {
+        constexpr uint32_t idesc = make_idesc_f16(128, BN);
+        const uint32_t sb = smem_u32(smem);
+        const uint64_t dBh = make_smem_desc_kmajor(sb, 64), dBl = make_smem_desc_kmajor(sb + SM::kBBytes, 64);
+        int s = 0, ph = 0;
+        for (int kb = 0; kb < nk; ++kb) {
+            const int sa = kb & (AST - 1), pa = (kb / AST) & 1;
+            mbar_wait(b_full + s, ph);
+            mbar_wait(a_ready + sa, pa);
+            tc_fence_after();
+            const uint64_t bo = (uint64_t)((s * SM::kStage) >> 4);
+            const uint32_t acol = tmem_base + kL1ACol + 32 * sa;
+            umma_f16_ts_elect(tmem_base, acol, dBh + bo, idesc, kb ? 1u : 0u);
+            umma_f16_ts_elect(tmem_base, acol + 16, dBh + bo, idesc, 1u);
+            umma_f16_ts_elect(tmem_base, acol, dBl + bo, idesc, 1u);
+            umma_f16_ts_elect(tmem_base, acol + 8, dBh + bo + 2, idesc, 1u);
+            umma_f16_ts_elect(tmem_base, acol + 24, dBh + bo + 2, idesc, 1u);
+            umma_f16_ts_elect(tmem_base, acol + 8, dBl + bo + 2, idesc, 1u);
+            umma_commit_elect(a_empty + sa);
+            umma_commit_elect(b_empty + s);
+            if (++s == ST) { s = 0; ph ^= 1; }
+        }
+        umma_commit_elect(tmem_full);
+    } else {
+        // two warps per TMEM lane quarter: warp `half` of a quarter produces m1 = 2 kb + half of every stage (= k-step
+        // `half` of the stage: 8 columns of hi, 8 of lo) and takes the epilogue chunks c = half, half + 2, ...
+        const int quarter = warp & 3, half = (warp - 2) >> 2;
+        const int row = quarter * 32 + lane;                   // tile row = TMEM lane
+        const int ml = m0 + row;
+        const bool row_ok = ml < rows_t;
+        const size_t m = (size_t)(g.row0[ty] + (row_ok ? ml : 0));
+        const float4* Trow = reinterpret_cast<const float4*>(g.Tm) + m * g.M1;
+        const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
+        const uint32_t lanefield = ((uint32_t)(quarter * 32)) << 16;
+        float4 T2[16];
+#pragma unroll
+        for (int m2 = 0; m2 < 16; ++m2) {
+            T2[m2] = row_ok ? __ldg(Trow + m2) : zero4;
+            T2[m2].x *= kL1DScale; T2[m2].y *= kL1DScale; T2[m2].z *= kL1DScale; T2[m2].w *= kL1DScale;   // D x 256
+        }
+        auto load_T1 = [&](int kb) { return (row_ok && kb < nk) ? __ldg(Trow + 2 * kb + half) : zero4; };
+        // T[i][m1] three stages ahead in three named registers, loop unrolled by hand (no moves of registers with a load in flight)
+        float4 Ta = load_T1(0), Tb = load_T1(1), Tc = load_T1(2);
+        auto stage = [&](int kb, const float4 Ta) {
+            const int sa = kb & (AST - 1), pa = (kb / AST) & 1;
+            uint32_t hi[8], lo[8];                              // K indices 16 half .. 16 half + 15 of the stage, two per word
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+                const int m2 = 2 * q;
+                const float d0 = Ta.x * T2[m2].x + Ta.y * T2[m2].y + Ta.z * T2[m2].z + Ta.w * T2[m2].w;
+                const float d1 = Ta.x * T2[m2 + 1].x + Ta.y * T2[m2 + 1].y + Ta.z * T2[m2 + 1].z + Ta.w * T2[m2 + 1].w;
+                const __half2 h = __floats2half2_rn(d0, d1);
+                const float2 hf = __half22float2(h);
+                const __half2 l = __floats2half2_rn(d0 - hf.x, d1 - hf.y);
+                hi[q] = *reinterpret_cast<const uint32_t*>(&h);
+                lo[q] = *reinterpret_cast<const uint32_t*>(&l);
+            }
+            mbar_wait(a_empty + sa, pa ^ 1);                    // the MMAs that read this A stage have retired
+            tc_fence_after();
+            const uint32_t col = tmem_base + lanefield + kL1ACol + 32 * sa + 8 * half;
+            tmem_st8(col, hi);
+            tmem_st8(col + 16, lo);
+            tmem_st_wait();
+            tc_fence_before();
+            mbar_arrive(a_ready + sa);
+        };
+        for (int kb = 0; kb < nk; kb += 3) {
+            stage(kb, Ta);
+            Ta = load_T1(kb + 3);
+            if (kb + 1 < nk) stage(kb + 1, Tb);
+            Tb = load_T1(kb + 4);
+            if (kb + 2 < nk) stage(kb + 2, Tc);
+            Tc = load_T1(kb + 5);
+        }
+        // ---- epilogue: Y1 = tanh(acc 2^-14 + b1), assembled as the operand image of fit_mid_kernel in the (now idle:
+        // tmem_full says every MMA has retired) weight stages and handed over with one bulk store ----
+        mbar_wait(tmem_full, 0);
+        tc_fence_after();
+        constexpr float kInv = 1.f / (kL1DScale * kW1Scale);
+        const int rbase = row * 64, sw = (row >> 1) & 3;
+#pragma unroll 1
+        for (int c = half; c < BN / 16; c += 2) {
+            uint32_t v[16];
+            tmem_ld16(tmem_base + lanefield + c * 16, v);
+            float bv[16];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const float4 b4 = reinterpret_cast<const float4*>(smem + SM::oBias + c * 64)[q];
+                bv[4 * q] = b4.x; bv[4 * q + 1] = b4.y; bv[4 * q + 2] = b4.z; bv[4 * q + 3] = b4.w;
+            }
+            tmem_ld_wait();
+            if (!row_ok) { mbar_arrive(blk_done + (c >> 1)); continue; }
+            uint32_t hi[8], lo[8];
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+                const float r0 = tanh_fast(fmaf(__uint_as_float(v[2 * q]), kInv, bv[2 * q]));
+                const float r1 = tanh_fast(fmaf(__uint_as_float(v[2 * q + 1]), kInv, bv[2 * q + 1]));
+                const __half2 h = __floats2half2_rn(r0, r1);
+                const float2 hf = __half22float2(h);
+                const __half2 l = __floats2half2_rn(r0 - hf.x, r1 - hf.y);
+                hi[q] = *reinterpret_cast<const uint32_t*>(&h);
+                lo[q] = *reinterpret_cast<const uint32_t*>(&l);
+            }
+            const int base = (c >> 1) * (128 * 64) + rbase, ci = 2 * (c & 1);
+            const int o0 = base + ((ci ^ sw) << 4), o1 = base + (((ci + 1) ^ sw) << 4);
+            *reinterpret_cast<uint4*>(smem + o0) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+            *reinterpret_cast<uint4*>(smem + o1) = make_uint4(hi[4], hi[5], hi[6], hi[7]);
+            *reinterpret_cast<uint4*>(smem + 65536 + o0) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+            *reinterpret_cast<uint4*>(smem + 65536 + o1) = make_uint4(lo[4], lo[5], lo[6], lo[7]);
+            fence_proxy_async_smem();
+            mbar_arrive(blk_done + (c >> 1));
+        }
+        if (half == 1) mbar_arrive(blk_done + 7);      // 15 chunks: the last K block holds only chunk 14 (a half-0 chunk)
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) tmem_dealloc(tmem_base, 512);
+}
+
+// ---------------------------------------------------------------------------------------------
 // dD = da1 W1^T fused with the descriptor backward (F4 -> F5 hand-over): dD (rows x 1600, 315 MB at
 // configs[2]) never reaches HBM.  One CTA owns 128 rows and walks the 10 column chunks of 160 = 10 m1 x 16 m2;
 // the epilogue thread of row i contracts each accumulator chunk with T_i on the fly (R-14):
@@ -956,7 +1153,9 @@ static int chain_range(Model& m, const ForceArgs& fa, int t0, int ntl, cudaStrea
         for (int t = 0; t <= kMaxT; ++t) { a1.tile0[t] = g.tile0[t]; a1.row0[t] = g.row0[t]; }
         for (int t = 0; t < nt; ++t) a1.bias[t] = m.fit_b[t][0];
         for (int t = 0; t < kMaxT; ++t) { const int q = t < nt ? t : 0; mp.A[t] = m.mapA_D[q]; mp.Bhi[t] = m.mapA_D[q]; mp.Blo[t] = m.mapA_D[q]; a1.wimg[t] = m.l1_wimg[q]; }
-        l1_desc_kernel<<<ntl, kL1Threads, L1Smem::kTotal, s>>>(mp, a1);
+        static const bool l1_ss = getenv("PIMD_L1_SS") != nullptr;            // A/B partner: the A operand through shared memory
+        if (fused && !l1_ss) l1_desc_ts_kernel<<<ntl, kL1Threads, L1TsSmem::kTotal, s>>>(a1);
+        else l1_desc_kernel<<<ntl, kL1Threads, L1Smem::kTotal, s>>>(mp, a1);
     }
     if (fused) {
         // layers 2 and 3, the energy and their backward products in one kernel (fitting_mid.cu)
@@ -1009,6 +1208,7 @@ int fitting_chain_tc(Model& m, const ForceArgs& fa, cudaStream_t s) {
     TcGemmArgs g{};
     const int tiles = fill_types(m, fa.ntypes, g);
     ensure_dyn_smem(l1_desc_kernel, L1Smem::kTotal);
+    ensure_dyn_smem(l1_desc_ts_kernel, L1TsSmem::kTotal);
     ensure_dyn_smem(dd_dt_kernel, DdSmem::kTotal);
     if (!m.aux_stream[0]) {
         if (const char* e = getenv("PIMD_CHAIN_STREAMS")) m.chain_streams = std::min(std::max(atoi(e), 1), (int)Model::kChainStreams);
