@@ -35,7 +35,7 @@ constexpr int oAhi = 0, oAlo = kAcopy, oB = 2 * kAcopy;
 constexpr int oVec = oB + kST * kStage;          // float [3][240]: b2, b3, w4 of this tile's centre type
 constexpr int oEx = oVec + 3 * kN * 4;           // float [128]: energy shares of the second warp of a quarter
 constexpr int oBars = oEx + 128 * 4;
-constexpr int kSmem = oBars + 320 + 1024;          // 35 barriers + the TMEM address
+constexpr int kSmem = oBars + 384 + 1024;          // 43 barriers + the TMEM address
 static_assert(kSmem <= 232448, "shared memory budget");
 constexpr float kWScale = 64.f;        // the weights are split as FP16 pairs of 64 w
 constexpr int kScratch = kKS * 4 * 128 * 16;     // bytes per tile of one scratch array: [chunk 15][float4 4][row 128]
@@ -107,7 +107,8 @@ fit_mid_kernel(const __grid_constant__ MidArgs g) {
     uint64_t* a_full = bars + 2 * kST;        // [8] K block kb of the y1 image landed -> MMA, epilogue
     uint64_t* acc_full = bars + 2 * kST + 8;  // [2] MMA -> epilogue, one per accumulator buffer
     uint64_t* chunk_ready = bars + 2 * kST + 10;  // [kKS] epilogue -> MMA: columns 16 c .. 16 c + 15 of the next operand are in place (count 128)
-    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(bars + 2 * kST + 10 + kKS);
+    uint64_t* blk_done = bars + 2 * kST + 10 + kKS;   // [8] last epilogue -> store: K block kb of the da1 image is complete (count 256)
+    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(bars + 2 * kST + 18 + kKS);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int tile = (int)blockIdx.x + g.tile_off;
@@ -124,6 +125,7 @@ fit_mid_kernel(const __grid_constant__ MidArgs g) {
         mbar_init(acc_full, 1);
         mbar_init(acc_full + 1, 1);
         for (int c = 0; c < kKS; ++c) mbar_init(chunk_ready + c, 128);
+        for (int kb = 0; kb < 8; ++kb) mbar_init(blk_done + kb, 256);
         fence_barrier_init();
     }
     if (warp == 1) tmem_alloc(tmem_ptr, 512);
@@ -165,6 +167,18 @@ fit_mid_kernel(const __grid_constant__ MidArgs g) {
             bulk_load_expect_elect(smem + oB + s * kStage, wimg + (size_t)it * kStage, kStage, full + s);
             if (++s == kST) { s = 0; ph ^= 1; }
         }
+        // after the last product the operand holds bwd_scale * da1: out as the image dd_dt_kernel loads, K block by K
+        // block behind the last epilogue, hi next to lo
+        uint8_t* img = g.da1_img + (size_t)tile * kImage;
+        for (int kb = 0; kb < 8; ++kb) {
+            mbar_wait(blk_done + kb, 0);
+            if (lane == 0) {
+                bulk_store(img + kb * 16384, smem + oAhi + kb * 8192, 8192);
+                bulk_store(img + kb * 16384 + 8192, smem + oAlo + kb * 8192, 8192);
+                bulk_commit();
+            }
+        }
+        if (lane == 0) bulk_wait_read0();      // shared memory may go once it has been read; the writes complete with the grid
     } else if (warp == 1) {
         constexpr uint32_t idesc = make_idesc_f16(128, kN);
         const uint32_t sb = smem_u32(smem);
@@ -274,8 +288,11 @@ fit_mid_kernel(const __grid_constant__ MidArgs g) {
                 if (p < 3) {
                     tc_fence_before();
                     mbar_arrive(chunk_ready + c);
+                } else {
+                    mbar_arrive(blk_done + (c >> 1));
                 }
             }
+            if (p == 3 && half == 1) mbar_arrive(blk_done + 7);     // 15 chunks: the last K block holds only chunk 14 (a half-0 chunk)
             if (p == 1) {
                 // E_i = y3 . w4 + b4: the two warps of a quarter hold shares over their chunks; U^(bead) += E_i with one
                 // atomic per warp when all its rows share the bead
@@ -299,17 +316,6 @@ fit_mid_kernel(const __grid_constant__ MidArgs g) {
                     }
                 }
             }
-        }
-        // the operand now holds bwd_scale * da1: out as the image dd_dt_kernel loads, K block by K block, hi next to lo
-        asm volatile("bar.sync 5, 256;" ::: "memory");
-        if (warp == 2 && lane == 0) {
-            uint8_t* img = g.da1_img + (size_t)tile * kImage;
-            for (int kb = 0; kb < 8; ++kb) {
-                bulk_store(img + kb * 16384, smem + oAhi + kb * 8192, 8192);
-                bulk_store(img + kb * 16384 + 8192, smem + oAlo + kb * 8192, 8192);
-            }
-            bulk_commit();
-            bulk_wait_read0();                 // shared memory may go once it has been read; the writes complete with the grid
         }
     }
     tc_fence_before();
