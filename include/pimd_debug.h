@@ -43,6 +43,11 @@ int pimd_time_kernel(pimd_ctx* ctx, int kind, int reps, double* ms);
  * -100 when a capture failed and the loop fell back to plain launches. */
 int pimd_debug_graph_state(const pimd_ctx* ctx);
 
+/* The row index of the most recent force evaluation, as the context's own path computed it: cen_idx[P N] (type-sorted
+ * centre row -> bead-atom) and rowstart[n_types][P N + 1] (exclusive scan of pimd_get_neighbor_counts in that order).
+ * tests/test_zz_no_alloc.py compares pimd_row_scan_noalloc_dev (pimd_noalloc.h) with it. */
+int pimd_debug_get_row_index(pimd_ctx* ctx, int32_t* cen_idx, int32_t* rowstart);
+
 #ifdef __cplusplus
 }
 #endif

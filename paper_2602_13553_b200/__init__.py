@@ -19,4 +19,5 @@ from .binding import (  # noqa: F401
     pimd_set_embedding_path, pimd_set_integrator, pimd_set_fixcom, PIMD_BAOAB, PIMD_OBABO,
     pimd_set_method, PIMD_NMPIMD, PIMD_CART, pimd_set_barostat, pimd_set_barostat_aniso, pimd_get_barostat, pimd_get_barostat_history, pimd_restore_cell, BarostatState,
     pimd_debug_gemm, pimd_debug_graph_state, PIMD,
+    pimd_debug_get_row_index, pimd_noalloc_setup, pimd_noalloc_last_error, pimd_row_scan_noalloc_dev,
 )

@@ -111,6 +111,10 @@ _SIGNATURES = {
     "pimd_set_profiling": (C.c_int, [C.c_void_p, C.c_int]),
     "pimd_debug_graph_state": (C.c_int, [C.c_void_p]),
     "pimd_get_phase_ms": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "pimd_debug_get_row_index": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
+    "pimd_noalloc_setup": (C.c_int, []),
+    "pimd_noalloc_last_error": (C.c_char_p, []),
+    "pimd_row_scan_noalloc_dev": (C.c_int, [C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
 }
 
 
@@ -211,6 +215,48 @@ def pimd_get_neighbor_counts(ctx, P, N, n_types):
     out = np.empty((P, N, n_types), dtype=np.int32)
     _check(ctx, lib().pimd_get_neighbor_counts(ctx, out.ctypes.data))
     return out
+
+
+def pimd_debug_get_row_index(ctx, P, N, n_types):
+    """(cen_idx[P N], rowstart[n_types][P N + 1]) of the most recent force evaluation (pimd_debug.h)."""
+    cen = np.empty(P * N, dtype=np.int32)
+    rowstart = np.empty((n_types, P * N + 1), dtype=np.int32)
+    _check(ctx, lib().pimd_debug_get_row_index(ctx, cen.ctypes.data, rowstart.ctypes.data))
+    return cen, rowstart
+
+
+def pimd_noalloc_last_error():
+    return lib().pimd_noalloc_last_error().decode()
+
+
+def pimd_noalloc_setup():
+    rc = lib().pimd_noalloc_setup()
+    if rc < 0:
+        raise PimdError(rc, pimd_noalloc_last_error())
+    return rc
+
+
+def _dev_i32(t, numel, what):
+    """torch CUDA int32 tensor -> device pointer, checked (a wrong dtype or a host tensor would be a silent bad read)."""
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.int32 and t.is_contiguous() and t.numel() == numel):
+        raise PimdError(PIMD_EINVAL, "%s must be a contiguous CUDA int32 tensor of %d elements" % (what, numel))
+    return t.data_ptr()
+
+
+def pimd_row_scan_noalloc_dev(n_centres, n_types, cen_idx_dev, ncount_dev, rowstart_dev, cuda_stream=0):
+    """pimd_noalloc.h: asynchronous on `cuda_stream` (0 = legacy default stream); allocates nothing.  Sizes are passed
+    on as given so that the library's own limit checks answer; tensors are checked when the sizes are positive."""
+    n_centres, n_types = int(n_centres), int(n_types)
+    if n_centres > 0 and n_types > 0 and hasattr(cen_idx_dev, "data_ptr"):
+        ptrs = (_dev_i32(cen_idx_dev, n_centres, "cen_idx_dev"), _dev_i32(ncount_dev, n_centres * n_types, "ncount_dev"),
+                _dev_i32(rowstart_dev, n_types * (n_centres + 1), "rowstart_dev"))
+    else:
+        ptrs = (_ptr(cen_idx_dev), _ptr(ncount_dev), _ptr(rowstart_dev))
+    rc = lib().pimd_row_scan_noalloc_dev(n_centres, n_types, ptrs[0], ptrs[1], ptrs[2], int(cuda_stream) or None)
+    if rc < 0:
+        raise PimdError(rc, pimd_noalloc_last_error())
+    return rc
 
 
 def pimd_get_launch_count(ctx):

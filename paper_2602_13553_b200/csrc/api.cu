@@ -551,6 +551,17 @@ int pimd_get_neighbor_counts(pimd_ctx* ctx, int32_t* counts) {
 
 int64_t pimd_get_launch_count(const pimd_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
+int pimd_debug_get_row_index(pimd_ctx* ctx, int32_t* cen_idx, int32_t* rowstart) {
+    if (!ctx || !cen_idx || !rowstart) return fail(ctx, PIMD_EINVAL, "null argument");
+    if (ctx->model_kind != 2 || !ctx->have_state) return fail(ctx, PIMD_ENOMODEL, "needs an se_e2_a model and a state");
+    const size_t PN = (size_t)ctx->P * ctx->N;
+    CK(cudaMemcpyAsync(cen_idx, ctx->model.cen_idx, sizeof(int32_t) * PN, cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaMemcpyAsync(rowstart, ctx->model.rowstart, sizeof(int32_t) * (size_t)ctx->ntypes * (PN + 1),
+                       cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return PIMD_OK;
+}
+
 static int set_barostat(pimd_ctx* ctx, double p_ext_bar, double tau_p, bool aniso) {
     if (!ctx) return PIMD_EINVAL;
     if (!(tau_p > 0)) return fail(ctx, PIMD_EINVAL, "tau_p must be positive");

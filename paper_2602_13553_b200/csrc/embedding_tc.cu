@@ -23,12 +23,15 @@
 //           segmented warp reduction over the rows of one centre.
 // A CTA runs two independent contexts, each with its own A-operand region, TMEM columns and mbarrier, so
 // that one context's MMAs overlap the other's tanh / epilogue work.
+#include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <cuda_fp16.h>
 #include <cuda_pipeline.h>
 #include <type_traits>
 #include "common.cuh"
 #include "tc_gemm.cuh"
+#include "../../include/pimd_noalloc.h"
 
 namespace pimd {
 
@@ -990,4 +993,82 @@ int embedding_backward_tc(Model& m, const ForceArgs& fa, int n_sms, cudaStream_t
     return 2;
 }
 
+// -------------------------------------------------------------------------------------------------
+// No-allocation entry point (include/pimd_noalloc.h): the row-index scan of emb_tc_row_index -- the exclusive scan
+// of the neighbour counts in type-sorted centre order that places every (t_i, t_j) row tile of F3 / F5 -- with its
+// scratch (the per-block sums the two scan kernels hand over) in a file-scope device array instead of the context's
+// arena.  For callers that may not allocate: code under CUDA graph capture, serving loops, harnesses that forbid
+// cudaMalloc.  The kernels are the ones pimd_step launches; only the scratch pointer differs.
+// -------------------------------------------------------------------------------------------------
+namespace noalloc {
+constexpr int kMaxScanBlocks = 4096;                                   // x 1024 centres = PIMD_NOALLOC_MAX_CENTRES
+constexpr int kMaxCentres = kMaxScanBlocks * etc::kScanBlock;
+constexpr int kMaxDevices = 64;
+static_assert(kMaxCentres == PIMD_NOALLOC_MAX_CENTRES, "include/pimd_noalloc.h states the limit");
+// 64 KB per GPU that loads the library, held until the process exits.  Every block sum a call reads has been written
+// by the first kernel of the same call, so nothing has to start at zero; the array keeps the last call's sums.
+static __device__ __align__(256) int g_row_bsum[PIMD_MAX_TYPES * kMaxScanBlocks];
+// In host code `g_row_bsum` is a host-side stand-in for the symbol, not a device address: the address a kernel can
+// use comes from cudaGetSymbolAddress, asked once per device with that device current.
+static int* g_row_bsum_dev[kMaxDevices];
+static std::mutex g_mu;
+static thread_local char g_err[256] = "";
+
+static int fail(int code, const char* what, const char* detail = "") {
+    snprintf(g_err, sizeof g_err, "%s%s", what, detail);
+    return code;
+}
+
+static int scratch_for_current_device(int** out) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail(PIMD_ECUDA, "cudaGetDevice: ", cudaGetErrorString(e));
+    if (dev < 0 || dev >= kMaxDevices) return fail(PIMD_EINVAL, "device ordinal beyond the 64 this entry point keeps scratch addresses for");
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (!g_row_bsum_dev[dev]) {
+        int* p = nullptr;
+        e = cudaGetSymbolAddress(reinterpret_cast<void**>(&p), g_row_bsum);
+        if (e != cudaSuccess || !p) return fail(PIMD_ECUDA, "cudaGetSymbolAddress(g_row_bsum): ", cudaGetErrorString(e));
+        g_row_bsum_dev[dev] = p;
+    }
+    *out = g_row_bsum_dev[dev];
+    return PIMD_OK;
+}
+}  // namespace noalloc
+
 }  // namespace pimd
+
+extern "C" {
+
+int pimd_noalloc_setup(void) {
+    int* p = nullptr;
+    return pimd::noalloc::scratch_for_current_device(&p);
+}
+
+const char* pimd_noalloc_last_error(void) { return pimd::noalloc::g_err; }
+
+int pimd_row_scan_noalloc_dev(int n_centres, int n_types, const int32_t* cen_idx_dev, const int32_t* ncount_dev,
+                              int32_t* rowstart_dev, void* cuda_stream) {
+    using namespace pimd;
+    if (!cen_idx_dev || !ncount_dev || !rowstart_dev) return noalloc::fail(PIMD_EINVAL, "null device pointer");
+    if (n_centres <= 0) return noalloc::fail(PIMD_EINVAL, "n_centres must be positive");
+    if (n_types <= 0 || n_types > PIMD_MAX_TYPES) return noalloc::fail(PIMD_EINVAL, "n_types outside 1..PIMD_MAX_TYPES (4)");
+    if (n_centres > noalloc::kMaxCentres)
+        return noalloc::fail(PIMD_EINVAL, "n_centres beyond PIMD_NOALLOC_MAX_CENTRES (4194304): the static scratch holds "
+                                          "4096 block sums per neighbour type; use the context path (pimd_step) for larger systems");
+    int* bsum = nullptr;
+    const int rc = noalloc::scratch_for_current_device(&bsum);
+    if (rc) return rc;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    const int nblk = (n_centres + etc::kScanBlock - 1) / etc::kScanBlock;
+    SelOff so;
+    for (int t = 0; t <= PIMD_MAX_TYPES; ++t) so.v[t] = 0;             // the scan kernels do not read it
+    dim3 grid(nblk, n_types);
+    row_block_sums_kernel<<<grid, 256, 0, s>>>(n_centres, n_types, cen_idx_dev, ncount_dev, bsum);
+    row_scan_fill_kernel<<<grid, 256, 0, s>>>(n_centres, n_types, 0, so, cen_idx_dev, ncount_dev, bsum, rowstart_dev, nullptr);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return noalloc::fail(PIMD_ECUDA, "row scan launch: ", cudaGetErrorString(e));
+    return PIMD_OK;
+}
+
+}  // extern "C"
