@@ -448,7 +448,10 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
             for (int h = 0; h < 2; ++h) {
                 float v16[16];
 #pragma unroll
-                for (int i = 0; i < H1; ++i) { h1[h][i] = tanh_fast(fmaf(s, W1s[H1 * h + i], b1s[H1 * h + i])); v16[i] = h1[h][i]; }
+                for (int i = 0; i < H1; ++i) h1[h][i] = fmaf(s, W1s[H1 * h + i], b1s[H1 * h + i]);
+                tanh_fast_n<H1>(h1[h]);
+#pragma unroll
+                for (int i = 0; i < H1; ++i) v16[i] = h1[h][i];
                 v16[13] = h ? 0.f : 1.f; v16[14] = 0.f; v16[15] = 0.f;
                 store_chunk_h<64>(ctx + eh::oA1hi, ctx + eh::oA1lo, t, 2 * h, v16);
                 store_chunk_h<64>(ctx + eh::oA1hi, ctx + eh::oA1lo, t, 2 * h + 1, v16 + 8);
@@ -476,7 +479,10 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
                 tmem_ld_wait();
                 float v32[32];
 #pragma unroll
-                for (int j = 0; j < H2; ++j) { h2[h][j] = h1[h][j % H1] + tanh_fast(__uint_as_float(v[j])); v32[j] = h2[h][j]; }
+                for (int j = 0; j < H2; ++j) v32[j] = __uint_as_float(v[j]);
+                tanh_fast_n<H2>(v32);
+#pragma unroll
+                for (int j = 0; j < H2; ++j) { h2[h][j] = h1[h][j % H1] + v32[j]; v32[j] = h2[h][j]; }
                 v32[26] = h ? 0.f : 1.f;
 #pragma unroll
                 for (int j = 27; j < 32; ++j) v32[j] = 0.f;
@@ -509,10 +515,9 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
                     for (int q = 0; q < 4; ++q) {
                         const int g = 16 * pc + 4 * q;
                         float4 gq;
-                        gq.x = h2[h][g % H2] + tanh_fast(__uint_as_float(v[4 * q]));
-                        gq.y = h2[h][(g + 1) % H2] + tanh_fast(__uint_as_float(v[4 * q + 1]));
-                        gq.z = h2[h][(g + 2) % H2] + tanh_fast(__uint_as_float(v[4 * q + 2]));
-                        gq.w = h2[h][(g + 3) % H2] + tanh_fast(__uint_as_float(v[4 * q + 3]));
+                        tanh_fast4(__uint_as_float(v[4 * q]), __uint_as_float(v[4 * q + 1]), __uint_as_float(v[4 * q + 2]),
+                                   __uint_as_float(v[4 * q + 3]), gq.x, gq.y, gq.z, gq.w);
+                        gq.x += h2[h][g % H2]; gq.y += h2[h][(g + 1) % H2]; gq.z += h2[h][(g + 2) % H2]; gq.w += h2[h][(g + 3) % H2];
                         *reinterpret_cast<float4*>(grow + g) = gq;
                     }
                 }
@@ -520,10 +525,8 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
                 tmem_ld4(col + 48, v);
                 tmem_ld_wait();
                 float4 gq;
-                gq.x = h2[h][48 % H2] + tanh_fast(__uint_as_float(v[0]));
-                gq.y = h2[h][49 % H2] + tanh_fast(__uint_as_float(v[1]));
-                gq.z = h2[h][50 % H2] + tanh_fast(__uint_as_float(v[2]));
-                gq.w = h2[h][51 % H2] + tanh_fast(__uint_as_float(v[3]));
+                tanh_fast4(__uint_as_float(v[0]), __uint_as_float(v[1]), __uint_as_float(v[2]), __uint_as_float(v[3]), gq.x, gq.y, gq.z, gq.w);
+                gq.x += h2[h][48 % H2]; gq.y += h2[h][49 % H2]; gq.z += h2[h][50 % H2]; gq.w += h2[h][51 % H2];
                 *reinterpret_cast<float4*>(grow + 48) = gq;
             }
             tc_fence_before();
@@ -781,13 +784,15 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
                     }
                 };
                 const uint32_t cv = tmem_v + lanefield + 56 * half, cd = tmem_g + lanefield + 56 * half;
-                uint32_t v[16], d[16];
+                // eight columns of each accumulator at a time: sixteen cost 16 more registers, which at the 128 this block
+                // size allows spilled the row prefetch (a store of a value still in flight: a stall per tile)
+                uint32_t v[8], d[8];
 #pragma unroll
-                for (int cc = 0; cc < 3; ++cc) {
-                    tmem_ld16(cv + 16 * cc, v);
-                    tmem_ld16(cd + 16 * cc, d);
+                for (int cc = 0; cc < 6; ++cc) {
+                    tmem_ld8(cv + 8 * cc, v);
+                    tmem_ld8(cd + 8 * cc, d);
                     tmem_ld_wait();
-                    piece(std::integral_constant<int, 16>{}, 16 * cc, v, d);
+                    piece(std::integral_constant<int, 8>{}, 8 * cc, v, d);
                 }
                 tmem_ld4(cv + 48, v);
                 tmem_ld4(cd + 48, d);

@@ -105,7 +105,7 @@ constexpr int kIntThreads = 128;
 #ifndef PIMD_NOISE_WIDE
 #define PIMD_NOISE_WIDE 4
 #endif
-constexpr int kNoiseWide = PIMD_NOISE_WIDE;     // draws generated side by side (4: 0.927 ms at 2^20 x 32)
+constexpr int kNoiseWide = PIMD_NOISE_WIDE;     // draws generated side by side (4: 0.874 ms at 2^20 x 32; 8: 0.927)
 
 // step counters (Philox counter words 0, 1; R-10) and estimator slot of a launch: launch arguments, or -- under graph
 // replay -- derived from the device-resident step counter
