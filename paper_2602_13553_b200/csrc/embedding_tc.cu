@@ -50,10 +50,9 @@ constexpr int kImgBytes = 2 * 64 * 64 + 2 * 112 * 128 + 256;     // 37120
 constexpr int kImgPad = (kImgBytes + 1023) / 1024 * 1024;
 // per-context shared memory
 constexpr int kABlk = 128 * 128;                                 // one K-block of 32 for 128 rows: 16 KB
-constexpr int oRs = 4 * kABlk;                                   // float4 R[128]
-constexpr int oCen = oRs + 128 * 16;                             // int centre[128]
-constexpr int oPart = oCen + 128 * 4;                            // float part[128][8]: half B -> half A (bwd)
-constexpr int kCtxBytes = (oPart + 128 * 32 + 1023) / 1024 * 1024;   // 72704
+constexpr int oPark = 4 * kABlk;                                 // float4 park[128][3]: a finished row waiting for its tail (bwd)
+constexpr int oCen = oPark + 128 * 48;                           // int centre[128]
+constexpr int kCtxBytes = (oCen + 128 * 4 + 1023) / 1024 * 1024;     // 72704
 constexpr int kSmemBytes = kImgPad + 2 * kCtxBytes + 64 + 1024;  // + barriers + alignment slack = 184320
 // The backward kernel keeps its contexts where they were before the weight image shrank (73 KB into the block) and
 // the largest carve-out: measured 6 % faster than the compact layout (the forward kernel is 5 % faster compact).
@@ -601,11 +600,11 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
     extern __shared__ uint8_t smem_raw[];
     const CtxSetup cs = ctx_setup_at(smem_raw, 512, kImgPadBwd, kCtxBytes, 2);
     const int cx = threadIdx.x >> 8, half = (threadIdx.x >> 7) & 1, t = threadIdx.x & 127, lane = threadIdx.x & 31;
-    const int bar_ctx = 1 + cx, bar_pair = 3 + cx * 4 + (t >> 5);
+    const int bar_ctx = 1 + cx;
     uint8_t* ctx = cs.ctx;
     int* cen_s = reinterpret_cast<int*>(ctx + oCen);
     float4* dTs = reinterpret_cast<float4*>(cs.smem + kImgPad + cx * kDtBufBytes);   // dedicated dT buffer (cp.async target)
-    float* part = reinterpret_cast<float*>(ctx + oPart) + t * 8;
+    float4* park = reinterpret_cast<float4*>(ctx + oPark) + t * 3;       // {A's dR}, {A's ds, slot index, centre, B's ds}, {B's dR}
     const float* W1s = reinterpret_cast<const float*>(cs.smem + eh::oW1) + H1 * half;
     const float* b1s = W1s + 32;
     const uint32_t tmem_v = cs.tmem_base + cx * 256, tmem_g = tmem_v + 128;     // value / derivative accumulators
@@ -617,6 +616,71 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
     constexpr int oY = 2 * kABlk;
     uint32_t phase = 0;
     const int nt = a.ntypes;
+
+    // The tail of a finished tile -- pair gradient g = dU/dd (R-16), F_j -= g, and the sums over the rows of a centre
+    // (F_i, virial share) -- does not run at the end of its tile but one tile later, UNDER THE LAYER-3 MMAs of the next
+    // tile, where the context would otherwise only wait.  The contraction parks a row as {partial sums of both halves,
+    // slot index, centre}; the geometry is read again from the slot (L2).  Both threads of a row rebuild g; half A sends
+    // F_j and reduces the three force components, half B reduces the nine virial components.
+    auto tail = [&]() {
+        const float4 pa = park[0], pm = park[1], pb = park[2];
+        const int addr = __float_as_int(pm.y), cen = __float_as_int(pm.z);
+        float4 A = make_float4(0.f, 0.f, 0.f, 0.f), B = make_float4(0.f, 1.f, 0.f, 0.f);
+        if (addr >= 0) {
+            A = __ldg(reinterpret_cast<const float4*>(a.slotA) + addr);
+            B = __ldg(reinterpret_cast<const float4*>(a.slotB) + addr);
+        }
+        const float w = (cen >= 0) ? a.inv_nsel : 0.f;
+        const float ds = (pm.x + pm.w) * w, dR0 = (pa.x + pb.x) * w, dR1 = (pa.y + pb.y) * w, dR2 = (pa.z + pb.z) * w,
+                    dR3 = (pa.w + pb.w) * w;
+        const float s = A.w, dsw = B.x, rinv = B.y, sr = s * rinv;
+        const float dot = dR1 * A.x + dR2 * A.y + dR3 * A.z;
+        const float radial = (ds + dR0) * dsw + (dsw * rinv - s * rinv * rinv) * dot;
+        const float rr = radial * rinv;
+        const float gx = fmaf(rr, A.x, sr * dR1), gy = fmaf(rr, A.y, sr * dR2), gz = fmaf(rr, A.z, sr * dR3);
+        const int ba = addr >= 0 ? addr / a.nsel : 0;
+        // segmented warp reduction over the rows of one centre (rows of a centre are contiguous)
+        auto seg_reduce = [&](auto NQ, float* red) {
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int ko = __shfl_down_sync(0xffffffffu, cen, o);
+                const bool take = (lane + o < 32) && (ko == cen);
+#pragma unroll
+                for (int q = 0; q < decltype(NQ)::value; ++q) {
+                    const float vo = __shfl_down_sync(0xffffffffu, red[q], o);
+                    if (take) red[q] += vo;
+                }
+            }
+        };
+        const int cprev = __shfl_up_sync(0xffffffffu, cen, 1);
+        const bool head = cen >= 0 && (lane == 0 || cprev != cen);
+        if (half == 0) {
+            if (cen >= 0) {
+                const int j = (int)(__float_as_uint(B.z) & 0x7fffffu);
+                double* fj = a.f + ((size_t)(ba / a.N) * a.N + j) * 3;
+                atomicAdd(fj, -(double)gx); atomicAdd(fj + 1, -(double)gy); atomicAdd(fj + 2, -(double)gz);
+            }
+            float red[3] = {gx, gy, gz};
+            seg_reduce(std::integral_constant<int, 3>{}, red);
+            if (head) {
+                double* fi = a.f + (size_t)ba * 3;
+                atomicAdd(fi, (double)red[0]); atomicAdd(fi + 1, (double)red[1]); atomicAdd(fi + 2, (double)red[2]);
+            }
+        } else {
+            float red[9];
+            const float dd[3] = {A.x, A.y, A.z}, gg[3] = {gx, gy, gz};
+#pragma unroll
+            for (int u = 0; u < 3; ++u)
+#pragma unroll
+                for (int w2 = 0; w2 < 3; ++w2) red[3 * u + w2] = -dd[u] * gg[w2];
+            seg_reduce(std::integral_constant<int, 9>{}, red);
+            if (head) {
+                double* cp = a.cpart + (size_t)cen * 9;
+#pragma unroll
+                for (int q = 0; q < 9; ++q) atomicAdd(cp + q, (double)red[q]);
+            }
+        }
+    };
 
     // Work split (unlike the forward kernel's contiguous shares): every context takes its 1/(2G) slice of EVERY
     // pair, which keeps the two contexts of a CTA on far-apart centres -- measured 3 % faster here, presumably
@@ -756,6 +820,7 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
             }
             const float sr = cur.s * cur.rinv;
             const float R0 = s, R1 = sr * cur.dx, R2 = sr * cur.dy, R3 = sr * cur.dz;
+            if (tile > tl0) tail();                        // the previous tile's rows (parked before two context barriers)
             mbar_wait(cs.mma_bar, phase);
             phase ^= 1;
             tc_fence_after();
@@ -805,63 +870,20 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
                 contract(reinterpret_cast<const float4*>(a.dTm) + (size_t)max(cur.cen, 0) * M1 + H1 * half);
             }
             tc_fence_before();
-            // half B hands its partial sums to half A, which finishes the row
-            if (half) {
-                *reinterpret_cast<float4*>(part) = make_float4(dR0, dR1, dR2, dR3);
-                part[4] = ds;
-            }
-            named_bar_sync(bar_pair, 64);
+            // park the row for its tail (above); the context barriers of the next tile order these stores before the
+            // reads, and the reads before the next tile's stores
             if (half == 0) {
-                {
-                    const float4 o = *reinterpret_cast<const float4*>(part);
-                    dR0 += o.x; dR1 += o.y; dR2 += o.z; dR3 += o.w;
-                    ds += part[4];
-                }
-                // ---- pair gradient g = dU/dd (R-16) ----
-                float red[12];
-                {
-                    const float w = (cur.cen >= 0) ? a.inv_nsel : 0.f;
-                    ds *= w; dR0 *= w; dR1 *= w; dR2 *= w; dR3 *= w;
-                    const float rinv = cur.rinv;
-                    const float dot = dR1 * cur.dx + dR2 * cur.dy + dR3 * cur.dz;
-                    const float radial = (ds + dR0) * cur.ds + (cur.ds * rinv - s * rinv * rinv) * dot;
-                    const float rr = radial * rinv;
-                    const float gx = fmaf(rr, cur.dx, sr * dR1), gy = fmaf(rr, cur.dy, sr * dR2), gz = fmaf(rr, cur.dz, sr * dR3);
-                    if (cur.cen >= 0) {
-                        const int j = (int)(cur.jcode & 0x7fffffu);
-                        double* fj = a.f + ((size_t)(cur.ba / a.N) * a.N + j) * 3;
-                        atomicAdd(fj, -(double)gx); atomicAdd(fj + 1, -(double)gy); atomicAdd(fj + 2, -(double)gz);
-                    }
-                    red[0] = gx; red[1] = gy; red[2] = gz;
-                    const float dd[3] = {cur.dx, cur.dy, cur.dz}, gg[3] = {gx, gy, gz};
-#pragma unroll
-                    for (int u = 0; u < 3; ++u)
-#pragma unroll
-                        for (int w2 = 0; w2 < 3; ++w2) red[3 + 3 * u + w2] = -dd[u] * gg[w2];
-                }
-                // segmented warp reduction over the rows of one centre (rows of a centre are contiguous)
-                const int key = cur.cen;
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const int ko = __shfl_down_sync(0xffffffffu, key, o);
-                    const bool take = (lane + o < 32) && (ko == key);
-#pragma unroll
-                    for (int q = 0; q < 12; ++q) {
-                        const float vo = __shfl_down_sync(0xffffffffu, red[q], o);
-                        if (take) red[q] += vo;
-                    }
-                }
-                const int kprev = __shfl_up_sync(0xffffffffu, key, 1);
-                if (key >= 0 && (lane == 0 || kprev != key)) {
-                    double* fi = a.f + (size_t)cur.ba * 3;
-                    atomicAdd(fi, (double)red[0]); atomicAdd(fi + 1, (double)red[1]); atomicAdd(fi + 2, (double)red[2]);
-                    double* cp = a.cpart + (size_t)key * 9;
-#pragma unroll
-                    for (int q = 0; q < 9; ++q) atomicAdd(cp + q, (double)red[3 + q]);
-                }
+                park[0] = make_float4(dR0, dR1, dR2, dR3);
+                float* pm = reinterpret_cast<float*>(park + 1);
+                pm[0] = ds; pm[1] = __int_as_float(addr_c); pm[2] = __int_as_float(cur.cen);
+            } else {
+                park[2] = make_float4(dR0, dR1, dR2, dR3);
+                reinterpret_cast<float*>(park + 1)[3] = ds;
             }
-            named_bar_sync(bar_ctx, 256);                  // dT stage / centre / partial buffers are free again
         }
+        // the last tile's tail
+        named_bar_sync(bar_ctx, 256);
+        tail();
     }
     tc_fence_before();
     __syncthreads();
