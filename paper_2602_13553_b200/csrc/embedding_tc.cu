@@ -621,7 +621,7 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
     // (F_i, virial share) -- does not run at the end of its tile but one tile later, UNDER THE LAYER-3 MMAs of the next
     // tile, where the context would otherwise only wait.  The contraction parks a row as {partial sums of both halves,
     // slot index, centre}; the geometry is read again from the slot (L2).  Both threads of a row rebuild g; half A sends
-    // F_j and reduces the three force components, half B reduces the nine virial components.
+    // F_j, half B reduces the twelve sums of a centre (force, virial share).
     auto tail = [&]() {
         const float4 pa = park[0], pm = park[1], pb = park[2];
         const int addr = __float_as_int(pm.y), cen = __float_as_int(pm.z);
@@ -658,26 +658,25 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
             if (cen >= 0) {
                 const int j = (int)(__float_as_uint(B.z) & 0x7fffffu);
                 double* fj = a.f + ((size_t)(ba / a.N) * a.N + j) * 3;
-                atomicAdd(fj, -(double)gx); atomicAdd(fj + 1, -(double)gy); atomicAdd(fj + 2, -(double)gz);
-            }
-            float red[3] = {gx, gy, gz};
-            seg_reduce(std::integral_constant<int, 3>{}, red);
-            if (head) {
-                double* fi = a.f + (size_t)ba * 3;
-                atomicAdd(fi, (double)red[0]); atomicAdd(fi + 1, (double)red[1]); atomicAdd(fi + 2, (double)red[2]);
+                atomicAdd(fj, (double)(-gx)); atomicAdd(fj + 1, (double)(-gy)); atomicAdd(fj + 2, (double)(-gz));
             }
         } else {
-            float red[9];
+            // half B: every sum over the rows of a centre (half A's warps also issue the MMAs and send F_j: measured,
+            // 3 + 9 or 6 + 6 sums split between the halves are slower)
+            float red[12];
+            red[0] = gx; red[1] = gy; red[2] = gz;
             const float dd[3] = {A.x, A.y, A.z}, gg[3] = {gx, gy, gz};
 #pragma unroll
             for (int u = 0; u < 3; ++u)
 #pragma unroll
-                for (int w2 = 0; w2 < 3; ++w2) red[3 * u + w2] = -dd[u] * gg[w2];
-            seg_reduce(std::integral_constant<int, 9>{}, red);
+                for (int w2 = 0; w2 < 3; ++w2) red[3 + 3 * u + w2] = -dd[u] * gg[w2];
+            seg_reduce(std::integral_constant<int, 12>{}, red);
             if (head) {
+                double* fi = a.f + (size_t)ba * 3;
+                atomicAdd(fi, (double)red[0]); atomicAdd(fi + 1, (double)red[1]); atomicAdd(fi + 2, (double)red[2]);
                 double* cp = a.cpart + (size_t)cen * 9;
 #pragma unroll
-                for (int q = 0; q < 9; ++q) atomicAdd(cp + q, (double)red[q]);
+                for (int q = 0; q < 9; ++q) atomicAdd(cp + q, (double)red[3 + q]);
             }
         }
     };
