@@ -165,8 +165,22 @@ struct EmbTcArgs {
     double* f;                 // [P][N][3]
     double* cpart;             // [PN][9] per-centre virial share (zeroed before the backward kernel)
     float inv_nsel;
+    uint32_t nsel_mul, nsel_sh, n_mul, n_sh;   // x / nsel and x / N as a multiply and a shift (FastDiv below)
     int skew_fwd, skew_bwd;    // head start (cycles) of context 0 over context 1 after every weight load
 };
+
+// x / d for 0 <= x < 2^31 as one wide multiply and a shift: m = ceil(2^sh / d), sh = 31 + ceil(log2 d) (m <= 2^31 for a
+// power of two, < 2^32 otherwise; exact because x (m d - 2^sh) < 2^31 d <= 2^sh).  The kernels divide a slot index by nsel
+// and a bead-atom index by N per row and tile.
+__host__ __device__ inline void fastdiv_make(uint32_t d, uint32_t* mul, uint32_t* sh) {
+    uint32_t l = 0;
+    while ((1ull << l) < d) ++l;                        // ceil(log2 d)
+    *sh = 31 + l;
+    *mul = (uint32_t)((((unsigned long long)1 << (31 + l)) + d - 1) / d);
+}
+__device__ __forceinline__ int fastdiv(int x, uint32_t mul, uint32_t sh) {
+    return (int)(((unsigned long long)(uint32_t)x * mul) >> sh);
+}
 
 // -------------------------------------------------------------------------------------------------
 // row bookkeeping: exclusive scan of the neighbour counts in type-sorted centre order, slot index per row
@@ -288,7 +302,7 @@ __device__ __forceinline__ RowIn load_row(const EmbTcArgs& a, int addr) {
     const float4 B = __ldg(reinterpret_cast<const float4*>(a.slotB) + addr);
     r.dx = A.x; r.dy = A.y; r.dz = A.z; r.s = A.w;
     r.ds = B.x; r.rinv = B.y; r.jcode = __float_as_uint(B.z);
-    r.ba = addr / a.nsel;
+    r.ba = fastdiv(addr, a.nsel_mul, a.nsel_sh);
     r.cen = __ldg(a.row_of + r.ba);
     return r;
 }
@@ -638,7 +652,7 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
         const float radial = (ds + dR0) * dsw + (dsw * rinv - s * rinv * rinv) * dot;
         const float rr = radial * rinv;
         const float gx = fmaf(rr, A.x, sr * dR1), gy = fmaf(rr, A.y, sr * dR2), gz = fmaf(rr, A.z, sr * dR3);
-        const int ba = addr >= 0 ? addr / a.nsel : 0;
+        const int ba = addr >= 0 ? fastdiv(addr, a.nsel_mul, a.nsel_sh) : 0;
         // segmented warp reduction over the rows of one centre (rows of a centre are contiguous)
         auto seg_reduce = [&](auto NQ, float* red) {
 #pragma unroll
@@ -657,7 +671,7 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
         if (half == 0) {
             if (cen >= 0) {
                 const int j = (int)(__float_as_uint(B.z) & 0x7fffffu);
-                double* fj = a.f + ((size_t)(ba / a.N) * a.N + j) * 3;
+                double* fj = a.f + ((size_t)fastdiv(ba, a.n_mul, a.n_sh) * a.N + j) * 3;
                 atomicAdd(fj, (double)(-gx)); atomicAdd(fj + 1, (double)(-gy)); atomicAdd(fj + 2, (double)(-gz));
             }
         } else {
@@ -712,7 +726,7 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
         auto load_A = [&](int addr) -> float4 {
             return addr >= 0 ? __ldg(reinterpret_cast<const float4*>(a.slotA) + addr) : make_float4(0.f, 0.f, 0.f, 0.f);
         };
-        auto load_cen = [&](int addr) -> int { return addr >= 0 ? __ldg(a.row_of + addr / a.nsel) : -1; };
+        auto load_cen = [&](int addr) -> int { return addr >= 0 ? __ldg(a.row_of + fastdiv(addr, a.nsel_mul, a.nsel_sh)) : -1; };
         int addr_nx = addr_of(tl0), addr_n2 = addr_of(tl0 + 1);
         float4 nxtA = load_A(addr_nx);
         int nxtCen = load_cen(addr_nx);
@@ -722,7 +736,7 @@ embed_bwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
             RowIn cur;
             const int addr_c = addr_nx;
             cur.dx = nxtA.x; cur.dy = nxtA.y; cur.dz = nxtA.z; cur.s = nxtA.w;
-            cur.cen = nxtCen; cur.ba = addr_c >= 0 ? addr_c / a.nsel : 0;
+            cur.cen = nxtCen;
             addr_nx = addr_n2;
             nxtA = load_A(addr_nx);
             nxtCen = load_cen(addr_nx);
@@ -982,6 +996,8 @@ static EmbTcArgs make_tc_args(Model& m, const ForceArgs& fa) {
     a.slotA = m.slotA; a.slotB = m.slotB; a.wimg_h = m.emb_img_h;
     a.Tm = m.Tm; a.dTm = m.dTm; a.f = fa.f; a.cpart = m.cpart;
     a.inv_nsel = 1.0f / (float)m.nsel;
+    fastdiv_make((uint32_t)m.nsel, &a.nsel_mul, &a.nsel_sh);
+    fastdiv_make((uint32_t)fa.N, &a.n_mul, &a.n_sh);
     // measured on B200: plateaus at 4-6 k cycles (forward, -20 %) and 5-13 k cycles (backward, -8 %)
     a.skew_fwd = 5000;
     a.skew_bwd = 9000;
