@@ -137,6 +137,36 @@ __device__ __forceinline__ void cmp_locate(float s, int& iv, float& u) {
     u = fmaf(s, cmp::kInvH, -(float)iv);
 }
 
+// The CTAs are dealt out to the centre types in proportion to their tile counts, so that a CTA loads ONE table image into
+// tensor memory instead of one per type (the image load is ~8 us of a ~220 us kernel, per type).  Returns the CTA's index
+// and the number of CTAs inside the share of type ti (bid < 0: none of this type's tiles are mine).  With fewer than two
+// CTAs per type every CTA walks every type, as before.
+__device__ __forceinline__ void cmp_cta_share(const CmpArgs& a, int ti, int& bid, int& gsz) {
+    const int G = (int)gridDim.x, nt = a.ntypes;
+    int ntile[PIMD_MAX_TYPES], tot = 0, live = 0;
+#pragma unroll
+    for (int t = 0; t < PIMD_MAX_TYPES; ++t) {
+        ntile[t] = t < nt ? (a.type_row0[t + 1] - a.type_row0[t] + cmp::TC - 1) / cmp::TC : 0;
+        tot += ntile[t];
+        live += ntile[t] > 0 ? 1 : 0;
+    }
+    if (G < 2 * live || live < 2) { bid = (int)blockIdx.x; gsz = G; return; }
+    int c0 = 0, pre = 0, left = live;
+    bid = -1; gsz = 1;
+#pragma unroll
+    for (int t = 0; t < PIMD_MAX_TYPES; ++t) {
+        if (ntile[t] == 0) continue;
+        pre += ntile[t];
+        --left;
+        int c1 = (int)(((long long)G * pre + tot / 2) / tot);
+        c1 = max(c1, c0 + 1);                              // at least one CTA for a type that has tiles ..
+        c1 = min(c1, G - left);                            // .. and for every type still to come
+        if (left == 0) c1 = G;
+        if (t == ti && (int)blockIdx.x >= c0 && (int)blockIdx.x < c1) { bid = (int)blockIdx.x - c0; gsz = c1 - c0; }
+        c0 = c1;
+    }
+}
+
 // -------------------------------------------------------------------------------------------------
 // forward: T_i = 1/N_sel  C^T Mom_i
 // -------------------------------------------------------------------------------------------------
@@ -182,6 +212,9 @@ cmp_fwd_kernel(const __grid_constant__ CmpArgs a) {
     for (int ti = 0; ti < nt; ++ti) {
         const int row0 = a.type_row0[ti], row1 = a.type_row0[ti + 1];
         const int ntile = (row1 - row0 + TC - 1) / TC;
+        int bid, gsz;
+        cmp_cta_share(a, ti, bid, gsz);
+        if (bid < 0 || ntile == 0) continue;               // CTA-uniform
         // ---- the table of centre type t_i goes into tensor memory (all MMAs of the previous type have retired:
         //      every role has passed its last tile, whose epilogue waited for mma_done) ----
         __syncthreads();
@@ -275,14 +308,14 @@ cmp_fwd_kernel(const __grid_constant__ CmpArgs a) {
             };
             size_t s0c, s0n; int nc, nn;
             RowF cur[3];
-            meta(blockIdx.x, s0c, nc);
+            meta(bid, s0c, nc);
             load_rows(s0c, nc, cur);
-            meta(blockIdx.x + gridDim.x, s0n, nn);
-            for (int tile = blockIdx.x; tile < ntile; tile += gridDim.x, ++it) {
+            meta(bid + gsz, s0n, nn);
+            for (int tile = bid; tile < ntile; tile += gsz, ++it) {
                 RowF nxt[3];
                 load_rows(s0n, nn, nxt);                             // the next tile's rows are in flight during this one
                 size_t s0nn; int nnn;
-                meta(tile + 2 * gridDim.x, s0nn, nnn);
+                meta(tile + 2 * gsz, s0nn, nnn);
                 float acc0 = 0.f;
 #pragma unroll
                 for (int b = 0; b < 3; ++b)
@@ -334,7 +367,7 @@ cmp_fwd_kernel(const __grid_constant__ CmpArgs a) {
             const int wq = warp - F_WARPS;
             const int m = wq * 32 + lane;
             const uint32_t lanefield = ((uint32_t)(wq * 32)) << 16;
-            for (int tile = blockIdx.x; tile < ntile; tile += gridDim.x, ++it) {
+            for (int tile = bid; tile < ntile; tile += gsz, ++it) {
                 if (wq == 0) {
                     mbar_wait(ready, it & 1);
                     if (it > 0) mbar_wait(d_free, (it - 1) & 1);
@@ -421,6 +454,9 @@ cmp_bwd_kernel(const __grid_constant__ CmpArgs a) {
     for (int ti = 0; ti < nt; ++ti) {
         const int row0 = a.type_row0[ti], row1 = a.type_row0[ti + 1];
         const int ntile = (row1 - row0 + TC - 1) / TC;
+        int bid, gsz;
+        cmp_cta_share(a, ti, bid, gsz);
+        if (bid < 0 || ntile == 0) continue;               // CTA-uniform
         __syncthreads();
         cmp_load_image(tmem, a.img_bw + (size_t)ti * 128 * BW_D, BW_D, warp, lane, B_THREADS / 32);
         tc_fence_before();
@@ -442,9 +478,9 @@ cmp_bwd_kernel(const __grid_constant__ CmpArgs a) {
                                : make_float4(0.f, 0.f, 0.f, 0.f);
             };
             float4 x[8];
-            load_dT(blockIdx.x, x);
-            uint32_t nd_next = ((int)blockIdx.x < ntile) ? __ldg(a.need + row0 / TC + ti + blockIdx.x) : 0u;
-            for (int tile = blockIdx.x; tile < ntile; tile += gridDim.x, ++it) {
+            load_dT(bid, x);
+            uint32_t nd_next = (bid < ntile) ? __ldg(a.need + row0 / TC + ti + bid) : 0u;
+            for (int tile = bid; tile < ntile; tile += gsz, ++it) {
                 const int buf = it & 1;
                 // ---- dT of the tile's centres -> operand rows (centre, c), K = channel; scaled per centre by the
                 //      power of two that brings max |dT| to [1, 2) (FP16 range; undone when Q is written) ----
@@ -473,7 +509,7 @@ cmp_bwd_kernel(const __grid_constant__ CmpArgs a) {
                         }
                     }
                 }
-                load_dT(tile + gridDim.x, x);                        // next tile's dT in flight under this tile's MMAs
+                load_dT(tile + gsz, x);                        // next tile's dT in flight under this tile's MMAs
                 fence_proxy_async_smem();
                 if (it >= 2) mbar_wait(qempty + buf, ((it >> 1) - 1) & 1);     // the row warps have left this Q buffer
                 tc_fence_before();
@@ -497,7 +533,7 @@ cmp_bwd_kernel(const __grid_constant__ CmpArgs a) {
                 // M tiles of this tile of centres: the lower 20 positions of both neighbour types always (j = 0, 2), the
                 // upper ones (j = 1, 3) only when a row sits there.  Two accumulator buffers, used in turn.
                 const uint32_t nd = nd_next;
-                nd_next = (tile + (int)gridDim.x < ntile) ? __ldg(a.need + row0 / TC + ti + tile + gridDim.x) : 0u;
+                nd_next = (tile + gsz < ntile) ? __ldg(a.need + row0 / TC + ti + tile + gsz) : 0u;
                 const int nj = 2 + (int)(nd & 1u) + (int)((nd >> 1) & 1u);
                 auto jof = [&](int idx) { return idx == 0 ? 0 : idx == 1 ? 2 : (idx == 2 ? ((nd & 1u) ? 1 : 3) : 3); };
                 issue(0, 0);
@@ -551,8 +587,8 @@ cmp_bwd_kernel(const __grid_constant__ CmpArgs a) {
                 return R;
             };
             int rn, ban, nn;
-            meta(blockIdx.x, rn, ban, nn);
-            for (int tile = blockIdx.x; tile < ntile; tile += gridDim.x, ++it) {
+            meta(bid, rn, ban, nn);
+            for (int tile = bid; tile < ntile; tile += gsz, ++it) {
                 const int buf = it & 1;
                 const int r = rn, ba = ban, n = nn;
                 const size_t s0 = (size_t)ba * a.nsel + a.seloff[tj];
@@ -562,7 +598,7 @@ cmp_bwd_kernel(const __grid_constant__ CmpArgs a) {
 #pragma unroll
                 for (int b = 0; b < 3; ++b)
                     if (32 * b + lane < n) rows[b] = load_row(s0 + 32 * b + lane);
-                meta(tile + gridDim.x, rn, ban, nn);
+                meta(tile + gsz, rn, ban, nn);
                 mbar_wait(qfull + buf, (it >> 1) & 1);
                 if (n > 0) {
                     const float4* Qc = Qs + (size_t)buf * (TC * K) + cl * K + tj * KB;
