@@ -18,9 +18,10 @@
 // Forward:  T_i += (1/N_sel) sum_rows G (x) R  (R-14): G tile through smem; the two warps of a lane quarter
 //           split its 32 rows, lane <-> 4 G positions, red.global.add.v4.f32 on (warp-uniform) centre change.
 // Backward: forward-mode -- the derivative rows h' = dh/ds go through the same weights (bias slot 0):
-//           G' = [h2',h2'] + (1 - tanh^2 z3) z3';  ds = sum_n (dT_n . R) G'_n;  dR_c = sum_n dT_nc G_n;
-//           pair gradient g = dU/dd (R-16), F_j -= g (f64 atomics), F_i and the virial share by a
-//           segmented warp reduction over the rows of one centre.
+//           G' = [h2',h2'] + (1 - tanh^2 z3) z3';  ds = sum_n (dT_n . R) G'_n = R . E, E_c = sum_n dT_nc G'_n;
+//           dR_c = sum_n dT_nc G_n;  pair gradient g = dU/dd (R-16), F_j -= g (f64 atomics), F_i and the virial
+//           share by a segmented warp reduction over the rows of one centre.  This tail of tile n runs under the
+//           layer-3 MMAs of tile n + 1, from rows parked in shared memory (see `tail` in the kernel).
 // A CTA runs two independent contexts, each with its own A-operand region, TMEM columns and mbarrier, so
 // that one context's MMAs overlap the other's tanh / epilogue work.
 #include <cstdio>
