@@ -479,6 +479,41 @@ def test_dilute_gas_many_centres_per_row_tile(pk):
     sim.close()
 
 
+@pytest.mark.parametrize("N,sel,L", [(256, [46, 92], 15.0), (128, [32, 64], 14.0), (250, [40, 85], 15.5)])
+def test_force_parity_power_of_two_atom_counts_and_other_sel(pk, N, sel, L):
+    """The embedding kernels divide a slot index by N_sel and a bead-atom index by N with a host-made multiply-shift pair
+    (embedding_tc.cu `fastdiv`); every BASELINE config has N = 3 x molecules and N_sel = 138.  Powers of two take the other
+    branch of the constant's construction (m = 2^31), other N_sel other constants: forces and energies against the oracle."""
+    desc = dict(workloads.model_desc(), sel=sel)
+    w = workloads.model_weights(desc, 11)
+    model = se_e2_a.Model(desc, w)
+    rng = np.random.default_rng(N)
+    pts = []                                             # box sizes keep the largest neighbour count under sel (asserted below)
+    while len(pts) < N:                                  # random positions at least 1.3 A apart
+        c = rng.uniform(0, L, 3)
+        if all(np.linalg.norm((c - q + L / 2) % L - L / 2) > 1.3 for q in pts):
+            pts.append(c)
+    x1 = np.array(pts)
+    types = (np.arange(N) % 3 != 0).astype(np.int32)
+    P = 4
+    x = x1[None] + 0.02 * rng.standard_normal((P, N, 3))
+    p = rng.standard_normal((P, N, 3))
+    box = np.array([L, L, L])
+    sim = pk.PIMD(types, [15.9994, 1.008], box, P, 300.0, 0.5e-3, 1.0, seed=1, model_desc=desc)
+    sim.set_state(x, p)
+    sim.set_model(w, desc)
+    f, U, E = sim.forces(), sim.energies(), sim.atom_energies()
+    counts = pk.pimd_get_neighbor_counts(sim.ctx, P, N, 2)
+    assert counts[..., 0].max() <= sel[0] and counts[..., 1].max() <= sel[1] and counts.sum() / (P * N) > 20
+    for k in (0, P - 1):
+        Eo, Fo, Xio = se_e2_a.energy_forces(x[k], types, box, model)
+        frms = np.sqrt((Fo ** 2).mean())
+        assert (np.abs(f[k] - Fo) / np.maximum(np.abs(Fo), frms)).max() <= 1e-4
+        assert np.abs(E[k] - Eo).max() <= 1e-6
+        assert abs(U[k] - Eo.sum()) / N <= 1e-6
+    sim.close()
+
+
 def test_sel_overflow_is_an_error(pk):
     cfg, wb, desc, w = workloads.make_config(0)
     small = dict(desc, sel=[8, 16])
