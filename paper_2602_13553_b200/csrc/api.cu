@@ -169,7 +169,7 @@ size_t model_bytes(const pimd_ctx* c, const pimd_model_desc* d) {
     b += 2 * align_up(PN * ND * 4, 256);
     b += 7 * align_up(PN * NF * 4, 256);
     b += 2 * align_up((PN / 128 + d->n_types + 1) * mid_image_bytes(), 256) + 2 * align_up((PN / 128 + d->n_types + 1) * mid_scratch_bytes(), 256);
-    b += align_up((size_t)d->n_types * d->n_types * emb_tc_image_h_bytes(), 256);
+    b += 2 * align_up((size_t)d->n_types * d->n_types * emb_tc_image_h_bytes(), 256);
     b += align_up((size_t)d->n_types * (PN + 1) * 4, 256) + align_up(PN * nsel * 4, 256);
     b += align_up((size_t)d->n_types * ((PN + 1023) / 1024) * 4, 256) + align_up(PN * 72, 256);
     b += align_up(cmp_image_words_fw(d->n_types) * 4, 256) + align_up(cmp_image_words_bw(d->n_types) * 4, 256);
@@ -759,6 +759,15 @@ int pimd_set_model(pimd_ctx* ctx, const pimd_model_desc* d, const double* w, siz
     }
     if ((rc = arena_alloc(ctx, &m.emb_img_h, img_h.size()))) return rc;
     CK(cudaMemcpyAsync(m.emb_img_h, img_h.data(), img_h.size(), cudaMemcpyHostToDevice, ctx->stream));
+    std::vector<uint8_t> img_f(img_h.size());        // the forward kernel's copy: weights and biases x 2 log2(e) (tanh's exponent)
+    {
+        const size_t per_pair = (size_t)2 * E1 + (size_t)E1 * E2 + E2 + (size_t)E2 * M1 + M1;
+        for (int q = 0; q < nt * nt; ++q)
+            emb_tc_build_image_h(w + q * per_pair, img_f.data() + (size_t)q * emb_tc_image_h_bytes(), 2.8853900817779268);
+    }
+    if ((rc = arena_alloc(ctx, &m.emb_img_h_fwd, img_f.size()))) return rc;
+    CK(cudaMemcpyAsync(m.emb_img_h_fwd, img_f.data(), img_f.size(), cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));          // img_f leaves scope below
 
     // ---- fitting weights: W, W^T, b per layer ----
     std::vector<std::vector<float>> keep;

@@ -178,6 +178,7 @@ struct Model {
     bool     use_tc_emb = true;
     bool     tc_emb_ready = false;
     uint8_t* emb_img_h = nullptr;      // [ntypes*ntypes][emb_tc_image_h_bytes()] FP16-split shared-memory images of the nets
+    uint8_t* emb_img_h_fwd = nullptr;  // the same, weights x 2 log2(e) (forward kernel)
     int*     rowstart = nullptr;       // [ntypes][PN+1] exclusive scan of ncount[.][tj] over type-sorted centres
     int*     rowaddr = nullptr;        // [PN*nsel] compact row -> slot index
     int*     row_bsum = nullptr;       // [ntypes][ceil(PN/1024)] scan block sums
@@ -225,7 +226,7 @@ void dd_build_wimg(const float* W, int ND, uint8_t* img);
 void mid_build_wimg(const float* W2, const float* W2T, const float* W3, const float* W3T, uint8_t* img);
 void fitting_mid_launch(Model& m, const ForceArgs& a, int tile_off, int ntiles, cudaStream_t s);
 size_t emb_tc_image_h_bytes();
-void emb_tc_build_image_h(const double* w_pair, uint8_t* img);
+void emb_tc_build_image_h(const double* w_pair, uint8_t* img, double scale = 1.0);
 int emb_tc_row_index(Model& m, const ForceArgs& a, cudaStream_t s);
 int embedding_forward_tc(Model& m, const ForceArgs& a, int n_sms, cudaStream_t s);
 int embedding_backward_tc(Model& m, const ForceArgs& a, int n_sms, cudaStream_t s);

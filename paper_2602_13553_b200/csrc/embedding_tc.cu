@@ -161,6 +161,8 @@ struct EmbTcArgs {
     const NeighSlotA* slotA;
     const NeighSlotB* slotB;
     const uint8_t* wimg_h;     // [ntypes*ntypes][eh::kImgBytes]  FP16-split weight images
+    const uint8_t* wimg_fwd;   // the same with every weight and bias times 2 log2(e): the forward kernel's tanh takes the
+                               // accumulator as the exponent's argument (one multiply per tanh less)
     float* Tm;                 // [PN][100][4]  (zeroed before the forward kernel)
     const float* dTm;
     double* f;                 // [P][N][3]
@@ -424,7 +426,7 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
         }
         __syncthreads();                                   // all contexts are done with the previous weights
         {
-            const float4* s4 = reinterpret_cast<const float4*>(a.wimg_h + (size_t)p * eh::kImgBytes);
+            const float4* s4 = reinterpret_cast<const float4*>(a.wimg_fwd + (size_t)p * eh::kImgBytes);    // weights x 2 log2(e)
             float4* d4 = reinterpret_cast<float4*>(smem);
             for (int q = threadIdx.x; q < eh::kImgBytes / 16; q += f3::kThreads) d4[q] = __ldg(s4 + q);
             fence_proxy_async_smem();
@@ -463,7 +465,7 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
                 float v16[16];
 #pragma unroll
                 for (int i = 0; i < H1; ++i) h1[h][i] = fmaf(s, W1s[H1 * h + i], b1s[H1 * h + i]);
-                tanh_fast_n<H1>(h1[h]);
+                tanh_fast_n<H1, true>(h1[h]);
 #pragma unroll
                 for (int i = 0; i < H1; ++i) v16[i] = h1[h][i];
                 v16[13] = h ? 0.f : 1.f; v16[14] = 0.f; v16[15] = 0.f;
@@ -494,7 +496,7 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
                 float v32[32];
 #pragma unroll
                 for (int j = 0; j < H2; ++j) v32[j] = __uint_as_float(v[j]);
-                tanh_fast_n<H2>(v32);
+                tanh_fast_n<H2, true>(v32);
 #pragma unroll
                 for (int j = 0; j < H2; ++j) { h2[h][j] = h1[h][j % H1] + v32[j]; v32[j] = h2[h][j]; }
                 v32[26] = h ? 0.f : 1.f;
@@ -529,7 +531,7 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
                     for (int q = 0; q < 4; ++q) {
                         const int g = 16 * pc + 4 * q;
                         float4 gq;
-                        tanh_fast4(__uint_as_float(v[4 * q]), __uint_as_float(v[4 * q + 1]), __uint_as_float(v[4 * q + 2]),
+                        tanh_fast4<true>(__uint_as_float(v[4 * q]), __uint_as_float(v[4 * q + 1]), __uint_as_float(v[4 * q + 2]),
                                    __uint_as_float(v[4 * q + 3]), gq.x, gq.y, gq.z, gq.w);
                         gq.x += h2[h][g % H2]; gq.y += h2[h][(g + 1) % H2]; gq.z += h2[h][(g + 2) % H2]; gq.w += h2[h][(g + 3) % H2];
                         *reinterpret_cast<float4*>(grow + g) = gq;
@@ -539,7 +541,7 @@ embed_fwd_tc_kernel(const __grid_constant__ EmbTcArgs a) {
                 tmem_ld4(col + 48, v);
                 tmem_ld_wait();
                 float4 gq;
-                tanh_fast4(__uint_as_float(v[0]), __uint_as_float(v[1]), __uint_as_float(v[2]), __uint_as_float(v[3]), gq.x, gq.y, gq.z, gq.w);
+                tanh_fast4<true>(__uint_as_float(v[0]), __uint_as_float(v[1]), __uint_as_float(v[2]), __uint_as_float(v[3]), gq.x, gq.y, gq.z, gq.w);
                 gq.x += h2[h][48 % H2]; gq.y += h2[h][49 % H2]; gq.z += h2[h][50 % H2]; gq.w += h2[h][51 % H2];
                 *reinterpret_cast<float4*>(grow + 48) = gq;
             }
@@ -943,7 +945,7 @@ size_t emb_tc_image_h_bytes() { return eh::kImgBytes; }
 // Builds the shared-memory image of one (t_i, t_j) embedding net from its packed FP64 weights
 // (W1[1][25], b1[25], W2[25][50], b2[50], W3[50][100], b3[100], row-major in x out) as FP16-split
 // UMMA B operands, with the channel permutation / padding of `etc` applied (dummy channels: zero weights, biases).
-void emb_tc_build_image_h(const double* w, uint8_t* img) {
+void emb_tc_build_image_h(const double* w, uint8_t* img, double scale) {
     using namespace etc;
     memset(img, 0, eh::kImgBytes);
     const double* W1 = w;
@@ -968,9 +970,9 @@ void emb_tc_build_image_h(const double* w, uint8_t* img) {
             for (int hh = 0; hh < 2; ++hh)
                 for (int i = 0; i < H1; ++i) {
                     const int c1 = H1 * hh + i;
-                    if (c1 < E1) put(eh::oW2hi, eh::oW2lo, 64, n, eh::k2_of(hh, i), (float)W2[c1 * E2 + n_orig]);
+                    if (c1 < E1) put(eh::oW2hi, eh::oW2lo, 64, n, eh::k2_of(hh, i), (float)(scale * W2[c1 * E2 + n_orig]));
                 }
-            put(eh::oW2hi, eh::oW2lo, 64, n, eh::kBias2, (float)b2[n_orig]);
+            put(eh::oW2hi, eh::oW2lo, 64, n, eh::kBias2, (float)(scale * b2[n_orig]));
         }
     for (int h = 0; h < 2; ++h)
         for (int g = 0; g < H3; ++g) {
@@ -980,12 +982,12 @@ void emb_tc_build_image_h(const double* w, uint8_t* img) {
             for (int hh = 0; hh < 2; ++hh)
                 for (int j = 0; j < H2; ++j) {
                     const int k_orig = h2_orig(hh, j);
-                    if (k_orig >= 0) put(eh::oW3hi, eh::oW3lo, 128, n, eh::k3_of(hh, j), (float)W3[k_orig * M1 + n_orig]);
+                    if (k_orig >= 0) put(eh::oW3hi, eh::oW3lo, 128, n, eh::k3_of(hh, j), (float)(scale * W3[k_orig * M1 + n_orig]));
                 }
-            put(eh::oW3hi, eh::oW3lo, 128, n, eh::kBias3, (float)b3[n_orig]);
+            put(eh::oW3hi, eh::oW3lo, 128, n, eh::kBias3, (float)(scale * b3[n_orig]));
         }
     float* l1 = reinterpret_cast<float*>(img + eh::oW1);
-    for (int k = 0; k < E1; ++k) { l1[k] = (float)W1[k]; l1[32 + k] = (float)b1[k]; }
+    for (int k = 0; k < E1; ++k) { l1[k] = (float)(scale * W1[k]); l1[32 + k] = (float)(scale * b1[k]); }
 }
 
 static EmbTcArgs make_tc_args(Model& m, const ForceArgs& fa) {
@@ -994,7 +996,7 @@ static EmbTcArgs make_tc_args(Model& m, const ForceArgs& fa) {
     for (int t = 0; t <= PIMD_MAX_TYPES; ++t) { a.seloff[t] = m.seloff[t]; a.type_row0[t] = m.type_row0[t]; }
     for (int t = 0; t < PIMD_MAX_TYPES; ++t) a.n_of_type[t] = (t < fa.ntypes) ? m.n_of_type[t] : 0;
     a.rowstart = m.rowstart; a.rowaddr = m.rowaddr; a.row_of = m.row_of;
-    a.slotA = m.slotA; a.slotB = m.slotB; a.wimg_h = m.emb_img_h;
+    a.slotA = m.slotA; a.slotB = m.slotB; a.wimg_h = m.emb_img_h; a.wimg_fwd = m.emb_img_h_fwd;
     a.Tm = m.Tm; a.dTm = m.dTm; a.f = fa.f; a.cpart = m.cpart;
     a.inv_nsel = 1.0f / (float)m.nsel;
     fastdiv_make((uint32_t)m.nsel, &a.nsel_mul, &a.nsel_sh);

@@ -254,13 +254,16 @@ __device__ __forceinline__ float tanh_fast(float x) {
 // kernels are bound by the MUFU pipe (16 lanes per clock and SM; ex2 + rcp per tanh): this takes 5 MUFU operations per
 // four tanh instead of 8, for 9 extra multiplies on the FMA pipe.  The exponent is clamped at 2^29 (tanh(10) rounds to 1
 // in FP32) so that the product of four stays finite.  Absolute error ~3e-7 (three more roundings than tanh_fast).
+// PRE: the arguments are 2 log2(e) x already (the forward embedding kernel folds the factor into its weight image)
+constexpr float kTanhScale = 2.8853900817779268f;      // 2 log2(e)
+template <bool PRE = false>
 __device__ __forceinline__ void tanh_fast4(const float x0, const float x1, const float x2, const float x3,
                                            float& t0, float& t1, float& t2, float& t3) {
     float d0, d1, d2, d3, r;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(d0) : "f"(fminf(x0 * 2.8853900817779268f, 29.0f)));
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(d1) : "f"(fminf(x1 * 2.8853900817779268f, 29.0f)));
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(d2) : "f"(fminf(x2 * 2.8853900817779268f, 29.0f)));
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(d3) : "f"(fminf(x3 * 2.8853900817779268f, 29.0f)));
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(d0) : "f"(fminf(PRE ? x0 : x0 * kTanhScale, 29.0f)));
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(d1) : "f"(fminf(PRE ? x1 : x1 * kTanhScale, 29.0f)));
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(d2) : "f"(fminf(PRE ? x2 : x2 * kTanhScale, 29.0f)));
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(d3) : "f"(fminf(PRE ? x3 : x3 * kTanhScale, 29.0f)));
     d0 += 1.0f; d1 += 1.0f; d2 += 1.0f; d3 += 1.0f;
     const float p01 = d0 * d1, p23 = d2 * d3;
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(p01 * p23));
@@ -271,22 +274,23 @@ __device__ __forceinline__ void tanh_fast4(const float x0, const float x1, const
     t3 = fmaf(-2.0f, r23 * d2, 1.0f);
 }
 // the same for two
+template <bool PRE = false>
 __device__ __forceinline__ void tanh_fast2(const float x0, const float x1, float& t0, float& t1) {
     float d0, d1, r;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(d0) : "f"(fminf(x0 * 2.8853900817779268f, 29.0f)));
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(d1) : "f"(fminf(x1 * 2.8853900817779268f, 29.0f)));
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(d0) : "f"(fminf(PRE ? x0 : x0 * kTanhScale, 29.0f)));
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(d1) : "f"(fminf(PRE ? x1 : x1 * kTanhScale, 29.0f)));
     d0 += 1.0f; d1 += 1.0f;
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(d0 * d1));
     t0 = fmaf(-2.0f, r * d1, 1.0f);
     t1 = fmaf(-2.0f, r * d0, 1.0f);
 }
 // n tanh in place (compile-time n): groups of four, then two, then one
-template <int N>
+template <int N, bool PRE = false>
 __device__ __forceinline__ void tanh_fast_n(float* v) {
 #pragma unroll
-    for (int q = 0; q + 4 <= N; q += 4) tanh_fast4(v[q], v[q + 1], v[q + 2], v[q + 3], v[q], v[q + 1], v[q + 2], v[q + 3]);
-    if constexpr (N % 4 >= 2) tanh_fast2(v[N - N % 4], v[N - N % 4 + 1], v[N - N % 4], v[N - N % 4 + 1]);
-    if constexpr (N % 2 == 1) v[N - 1] = tanh_fast(v[N - 1]);
+    for (int q = 0; q + 4 <= N; q += 4) tanh_fast4<PRE>(v[q], v[q + 1], v[q + 2], v[q + 3], v[q], v[q + 1], v[q + 2], v[q + 3]);
+    if constexpr (N % 4 >= 2) tanh_fast2<PRE>(v[N - N % 4], v[N - N % 4 + 1], v[N - N % 4], v[N - N % 4 + 1]);
+    if constexpr (N % 2 == 1) v[N - 1] = tanh_fast(PRE ? v[N - 1] * (1.0f / kTanhScale) : v[N - 1]);
 }
 
 }  // namespace pimd
